@@ -1,0 +1,200 @@
+/*
+ * soap_b200.h - C ABI of the B200-native SOAP disk-integration hot path.
+ *
+ * What the library computes (Zhao & Dumusque 2023, "SOAP-GPU", arXiv:2301.04259; "P:n" = line n of
+ * PAPER.md, "S#" = a reading listed in DESIGN.md section 3):
+ *
+ *   A star is an N x N grid of cells over [-1,1]^2.  Every visible cell carries a rotational
+ *   velocity and a limb-darkening intensity (Fig. 1).  The cell's local spectrum - the row of a
+ *   mu-binned spectrum table whose mu is closest to the cell's - is Doppler-shifted by the
+ *   cell's velocity and linearly interpolated back onto the uniform wavelength grid (Eq. 5-9,
+ *   P:160-186), weighted, and summed over cells: once for the quiet star (Alg. 1) and, for
+ *   every rotational phase, over the cells covered by active regions only (InfoMap, Alg. 5)
+ *   to give the active-minus-quiet delta spectrum (Eq. 3-4).
+ *
+ * Conventions common to every entry point
+ *   - Every function returns an int status: SOAP_OK (0) or a negative soap_status.  Nothing throws or
+ *     aborts across the ABI.  Argument errors are detected before any device write (no partial output).
+ *   - "DEVICE" pointers are CUDA device pointers on the device the handle was created for; "HOST"
+ *     pointers are ordinary host memory.  The caller owns every input and output buffer.  The library
+ *     owns only what lives inside soap_star (geometry, binned weights, scratch, active-entry lists) and
+ *     frees it in soap_destroy.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All device work
+ *     is enqueued on it; a call is asynchronous unless it has a non-NULL HOST output pointer
+ *     (`info`, `n_active`, export, stats), in which case it synchronises that stream before returning.
+ *     Scratch is (re)allocated with cudaMalloc when a call needs more than any earlier call did; once
+ *     sizes have been seen, calls allocate nothing and can be captured in a CUDA graph.
+ *   - There is no CPU fallback and no other backend: without a CUDA device every compute entry point
+ *     returns SOAP_ERR_CUDA.
+ *   - Cell indexing: c = j * N + i with j the column (x) index and i the row (y) index;
+ *     x_j = -1 + (2j+1)/N, y_i = -1 + (2i+1)/N (S1).
+ *   - Results are run-to-run bit-identical (no unordered floating-point atomics).
+ */
+#ifndef SOAP_B200_H
+#define SOAP_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SOAP_B200_VERSION 100 /* major*100 + minor */
+
+typedef struct soap_star soap_star; /* opaque; one star's device-resident state */
+
+enum soap_status {
+    SOAP_OK = 0,
+    SOAP_ERR_INVALID_ARG = -1, /* bad pointer / size / flag; nothing was written */
+    SOAP_ERR_NOT_READY = -2,   /* soap_disk_geometry has not been called on this handle */
+    SOAP_ERR_CUDA = -3,        /* a CUDA runtime call failed (see soap_last_error) */
+    SOAP_ERR_OOM = -4,         /* device or host allocation failed */
+    SOAP_ERR_UNSUPPORTED = -5  /* valid request this build does not implement */
+};
+
+enum soap_dtype { SOAP_F32 = 0, SOAP_F64 = 1 };
+enum soap_region_type { SOAP_SPOT = 1, SOAP_FACULA = 2 };
+
+/* How the shift-interpolate-accumulate sum is evaluated.  All forms compute the same sums (Alg. 1,
+ * Eq. 3) and differ only in rounding order. */
+enum soap_form {
+    SOAP_FORM_AUTO = 0,   /* library picks (currently SOAP_FORM_BINNED for solid-body rotation) */
+    SOAP_FORM_BINNED = 1, /* cells pre-binned by (column, mu-bin): all cells of a column share one
+                             velocity under solid-body rotation (BASELINE.json north_star) */
+    SOAP_FORM_CELLS = 2,  /* one entry per visible cell - the literal double loop of Alg. 1 */
+    SOAP_FORM_FIR = 3     /* per-tile collapse of all entries with equal integer shift into FIR taps
+                             linear in the pixel index (exact in exact arithmetic) */
+};
+
+enum soap_option {
+    SOAP_OPT_FORM = 1,         /* value: enum soap_form; default SOAP_FORM_AUTO */
+    SOAP_OPT_QUIET_SPLITS = 2, /* value: >0 forces the number of entry-chunks the quiet sum is split
+                                  into across CTAs; 0 (default) = sized from the SM count */
+    SOAP_OPT_KERNEL_TIMING = 3 /* value: 1 brackets the shift-interpolate-accumulate kernel of each call with
+                                  CUDA events on the caller's stream; soap_get_stats reports the durations */
+};
+
+/* Star / disk description.  HOST, read only during the call. */
+typedef struct {
+    int32_t grid_n;           /* N >= 1 */
+    double vsini_kms;         /* v_cell = x * vsini_kms * sin(incl)  (S5; +x is the receding limb) */
+    double incl_deg;          /* angle between spin axis and line of sight (S13) */
+    double ld_u1, ld_u2;      /* quadratic limb darkening: w = 1 - u1 (1-mu) - u2 (1-mu)^2  (S3, S4) */
+    int32_t n_mu;             /* number of mu bins, 1..SOAP_MAX_MU */
+    const double *mu_centres; /* HOST [n_mu], strictly ascending (S9: nearest centre, tie -> larger mu) */
+    int32_t doppler_mode;     /* 0: relativistic, Eq. 6 (source wavelength lambda * sqrt((1-b)/(1+b)));
+                                 1: first order, lambda * (1 - v/c)  (S6) */
+} soap_star_params;
+
+#define SOAP_MAX_MU 64
+
+/* One table of mu-binned spectra on the uniform grid lambda_m = lambda0 + m * dlambda (Eq. 5). */
+typedef struct {
+    const void *data;         /* DEVICE [n_mu][pitch] row-major, n_pix valid values per row,
+                                 base address 16-byte aligned */
+    int64_t n_pix;            /* P >= 2 */
+    int64_t pitch;            /* row pitch in elements, >= n_pix, multiple of 4 */
+    int32_t dtype;            /* enum soap_dtype; outputs use the same dtype */
+    double lambda0, dlambda;  /* dlambda > 0, lambda0 > 0 */
+    const void *contrast;     /* DEVICE [n_pix] of `dtype`, or NULL (== 1).  I_ratio of Eq. 3, applied
+                                 at the output pixel after the shift (S17).  Ignored for quiet. */
+    double lb_c0, lb_c1, lb_c2; /* LB(mu) = c0 + c1 mu + c2 mu^2, per cell with its exact mu (Eq. 11-12,
+                                   P:372-379).  Ignored for quiet; (1,0,0) for spots. */
+} soap_spectra;
+
+typedef struct {
+    double lat_deg, lon_deg;  /* region centre; effective longitude = lon + 360 * phase, 0 = sub-observer
+                                 meridian, increasing toward +x (S12) */
+    double radius;            /* in stellar radii, 0 < radius < 1: radius of the circle the region projects
+                                 to at disk centre; angular radius asin(radius) (S11) */
+    int32_t type;             /* enum soap_region_type */
+} soap_region;
+
+typedef struct {
+    int64_t n_visible;        /* cells whose centre lies on the disk (S2) */
+    int64_t n_entries;        /* (column, mu-bin) pairs with non-zero weight (n_visible for FORM_CELLS) */
+    double sum_weights;       /* sum of w over visible cells: the integrated continuum of a unit spectrum (S4) */
+    double max_abs_dshift;    /* max |D - 1| over cells; |shift in pixels| <= this * (lambda0/dlambda + P) */
+} soap_geom_info;
+
+typedef struct {
+    int64_t quiet_entries;        /* entries summed per pixel by the last soap_integrate_quiet */
+    int64_t active_entries;       /* sum over phases of (row, column) entries of the last time series,
+                                     counting the quiet-row and the active-row entry of a pair separately */
+    int64_t active_cells;         /* sum over phases of covered cells */
+    int32_t quiet_splits, tile_px;
+    int32_t form;                 /* enum soap_form actually used */
+    int32_t launches;             /* kernels launched by this handle since soap_create */
+    float quiet_kernel_ms;        /* SOAP_OPT_KERNEL_TIMING: device time of the last quiet / active */
+    float active_kernel_ms;       /*   shift-interpolate-accumulate kernel launch; else 0 */
+} soap_stats;
+
+/* ---- lifetime ---------------------------------------------------------------------------------- */
+int soap_version(void);
+/* Create an empty handle bound to CUDA device `device`.  *out is set to NULL on failure. */
+int soap_create(soap_star **out, int device);
+/* Frees all device and host memory of the handle.  NULL is allowed. */
+int soap_destroy(soap_star *star);
+/* Library-owned, NUL-terminated description of the last error on this handle (valid until the next
+ * call on it).  star == NULL returns the message of the last failed soap_create. */
+const char *soap_last_error(const soap_star *star);
+int soap_set_option(soap_star *star, int32_t option, int64_t value);
+/* Copies counters of the last calls to HOST *stats; synchronises `stream`. */
+int soap_get_stats(soap_star *star, soap_stats *stats, void *stream);
+
+/* ---- a1 + a2: geometry and (column, mu-bin) weight binning (S1-S5, S9, S10) ----------------
+ * Computes, on the device, every cell's (x, y, mu, v, w, bin), the per-column Doppler shift factor
+ * D_j - 1 in fp64, and the binned weights W[j,b] = sum of w over the cells of column j in bin b.
+ * `info` (HOST, nullable) receives the summary; non-NULL makes the call synchronous. */
+int soap_disk_geometry(soap_star *star, const soap_star_params *params, void *stream, soap_geom_info *info);
+
+/* ---- a3: quiet integrated spectrum (Alg. 1) ---------------------------------------------
+ * out[m] = sum over visible cells of w_c * lerp(S_quiet[bin_c]; source coordinate of pixel m under D_c),
+ * clamped to the end values outside the grid (S8).  `out`: DEVICE [n_pix] of quiet->dtype. */
+int soap_integrate_quiet(soap_star *star, const soap_spectra *quiet, void *out, void *stream);
+
+/* ---- a4 + a5 + a6: active-region delta spectra for every phase (Alg. 5, Eq. 3; S11-S19) ----------
+ * For phase p: type[c] = type of the LAST region in list order covering visible cell c, and
+ *   out_delta[p][m] = sum over covered cells of
+ *        w_c * ( C_t[m] * LB_t(mu_c) * lerp(S_t[bin_c]; c, m)  -  lerp(S_quiet[bin_c]; c, m) )
+ * i.e. active minus quiet (the negative of Eq. 3), so that S_final = S_quiet,integrated + delta (Eq. 4).
+ * Phases without covered cells give exact zeros.
+ *   spot / facula: nullable if no region of that type is listed; must match quiet in n_pix, pitch
+ *                  rules, dtype, lambda0, dlambda.
+ *   regions: HOST [n_regions] (n_regions may be 0);  phases: HOST [n_phases], in rotations, any real.
+ *   out_delta: DEVICE [n_phases][out_pitch] of quiet->dtype, out_pitch >= n_pix.
+ *   n_active: HOST [n_phases] or NULL; number of covered cells per phase (non-NULL => synchronous). */
+int soap_active_timeseries(soap_star *star, const soap_spectra *quiet, const soap_spectra *spot,
+                           const soap_spectra *facula, const soap_region *regions, int32_t n_regions,
+                           const double *phases, int32_t n_phases, void *out_delta, int64_t out_pitch,
+                           int32_t *n_active, void *stream);
+
+/* ---- debug export of the geometry (HOST outputs, N*N each, any may be NULL; synchronous) --------
+ * Hidden cells: mu = 0, vel = 0, w = 0, bin = -1. */
+int soap_export_geometry(soap_star *star, double *mu, double *vel, double *w, int32_t *bin);
+
+/* ---- end-to-end convenience with HOST buffers ---------------------------------------------------
+ * Same computation as soap_disk_geometry + soap_integrate_quiet + soap_active_timeseries, but every
+ * spectra / contrast pointer in quiet / spot / facula, `out_quiet` ([n_pix]) and `out_delta`
+ * ([n_phases][n_pix], densely packed) are HOST pointers; the library stages them through device
+ * buffers it owns (host->device and device->host copies are part of the call).  Synchronous. */
+int soap_synthesize_host(soap_star *star, const soap_star_params *params, const soap_spectra *quiet,
+                         const soap_spectra *spot, const soap_spectra *facula, const soap_region *regions,
+                         int32_t n_regions, const double *phases, int32_t n_phases, void *out_quiet,
+                         void *out_delta, int32_t *n_active, void *stream);
+
+/* ---- config 5: many independent stars in one call ----------------------------------------------
+ * Arrays of length n_stars of the arguments above; star k uses stars[k], quiet[k], ...  All device
+ * work of all stars is enqueued on `stream`. */
+int soap_batch_integrate_quiet(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet,
+                               void *const *out, void *stream);
+int soap_batch_active_timeseries(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet,
+                                 const soap_spectra *const *spot, const soap_spectra *const *facula,
+                                 const soap_region *const *regions, const int32_t *n_regions,
+                                 const double *const *phases, const int32_t *n_phases,
+                                 void *const *out_delta, const int64_t *out_pitch, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SOAP_B200_H */

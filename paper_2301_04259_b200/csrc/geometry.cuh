@@ -1,0 +1,219 @@
+// a1 + a2 of SURVEY section 8: disk geometry (Fig. 1) and (column, mu-bin) weight binning.
+//
+// All geometry is fp64 with explicitly rounded operations (no FMA contraction), so that the integer
+// decisions taken here (visible / hidden, mu bin) are taken in the same precision as the fp64 definition.
+// N^2 <= a few 10^5 cells: these kernels are launch-latency sized, not a cost centre.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace soap {
+
+constexpr double kSpeedOfLightKms = 299792.458;
+
+struct DevInfo {            // device-resident summary, mirrored to soap_geom_info on request
+    long long n_visible;
+    long long n_entries;
+    double sum_weights;
+    double max_abs_dshift;
+};
+
+__device__ __forceinline__ double cell_coord(int idx, int N) {
+    // -1 + (2 idx + 1)/N, each operation rounded once (reading S1)
+    return __dadd_rn(-1.0, __ddiv_rn(__dadd_rn(__dmul_rn(2.0, (double)idx), 1.0), (double)N));
+}
+
+// One thread per cell c = j*N + i: mu, limb-darkening weight, velocity and nearest mu bin.
+__global__ void geometry_cells_kernel(int N, double vsini_sini, double u1, double u2, int n_mu,
+                                      const double *__restrict__ mu_centres, double *__restrict__ mu_out,
+                                      double *__restrict__ w_out, double *__restrict__ vel_out,
+                                      int *__restrict__ bin_out) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= N * N) return;
+    const int j = c / N, i = c - j * N;
+    const double x = cell_coord(j, N), y = cell_coord(i, N);
+    const double r2 = __dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y));
+    double mu = 0.0, w = 0.0, v = 0.0;
+    int bin = -1;
+    if (r2 <= 1.0) {  // cell counts iff its centre is on the disk (reading S2)
+        const double a = __dadd_rn(1.0, -r2);
+        mu = __dsqrt_rn(a > 0.0 ? a : 0.0);
+        v = __dmul_rn(x, vsini_sini);
+        const double om = __dadd_rn(1.0, -mu);
+        // w = 1 - u1 (1-mu) - u2 (1-mu)^2, evaluated left to right
+        w = __dadd_rn(__dadd_rn(1.0, -__dmul_rn(u1, om)), -__dmul_rn(__dmul_rn(u2, om), om));
+        // closest mu centre; on an exact tie the larger mu wins (reading S9)
+        double best = fabs(__dadd_rn(mu, -mu_centres[0]));
+        bin = 0;
+        for (int b = 1; b < n_mu; ++b) {
+            const double d = fabs(__dadd_rn(mu, -mu_centres[b]));
+            if (d <= best) {
+                best = d;
+                bin = b;
+            }
+        }
+    }
+    mu_out[c] = mu;
+    w_out[c] = w;
+    vel_out[c] = v;
+    bin_out[c] = bin;
+}
+
+// D - 1 without cancellation.  mode 0: D = sqrt((1-b)/(1+b))  =>  D - 1 = -2b / ((1+b) + sqrt(1-b^2));
+// mode 1: D = 1 - b.
+__device__ __forceinline__ double doppler_minus_one(double v_kms, int mode) {
+    const double b = v_kms / kSpeedOfLightKms;
+    if (mode == 1) return -b;
+    return -2.0 * b / ((1.0 + b) + sqrt(1.0 - b * b));
+}
+
+// One thread per column j: the column's shift factor a_j = D_j - 1 (all cells of a column share one
+// velocity under solid-body rotation), its binned weights W[j][b] (serial fp64 sum in i order:
+// deterministic), and its visible-cell count / weight sum.
+__global__ void geometry_columns_kernel(int N, double vsini_sini, int mode, int n_mu,
+                                        const double *__restrict__ w, const int *__restrict__ bin,
+                                        double *__restrict__ col_a, double *__restrict__ Wbin /*[N][n_mu]*/,
+                                        double *__restrict__ col_sumw, int *__restrict__ col_nvis) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    const double x = cell_coord(j, N);
+    col_a[j] = doppler_minus_one(__dmul_rn(x, vsini_sini), mode);
+    double *Wj = Wbin + (size_t)j * n_mu;
+    for (int b = 0; b < n_mu; ++b) Wj[b] = 0.0;
+    double sum = 0.0, run = 0.0;
+    int nvis = 0, cur = -1;
+    for (int i = 0; i < N; ++i) {
+        const int b = bin[(size_t)j * N + i];
+        if (b < 0) continue;
+        const double wc = w[(size_t)j * N + i];
+        if (b != cur) {
+            if (cur >= 0) Wj[cur] += run;
+            cur = b;
+            run = 0.0;
+        }
+        run += wc;
+        sum += wc;
+        ++nvis;
+    }
+    if (cur >= 0) Wj[cur] += run;
+    col_sumw[j] = sum;
+    col_nvis[j] = nvis;
+}
+
+// Single CTA: compacts the non-zero W[j][b] into the entry list of the pre-binned form, sorted by
+// (row b, column j), each row padded with a zero-weight entry to an even length so that every row
+// starts 16-byte aligned for the TMA bulk copy; writes row_start[n_mu+1] and the summary.
+// Entries are (a_j, W) in fp32 (float2) and fp64 (double2).
+__global__ void build_binned_entries_kernel(int N, int n_mu, const double *__restrict__ col_a,
+                                            const double *__restrict__ Wbin,
+                                            const double *__restrict__ col_sumw,
+                                            const int *__restrict__ col_nvis, float2 *__restrict__ ent32,
+                                            double2 *__restrict__ ent64, int *__restrict__ row_start,
+                                            DevInfo *__restrict__ info) {
+    __shared__ int s_cnt[64];
+    __shared__ int s_start[65];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+    for (int b = warp; b < n_mu; b += n_warps) {
+        int cnt = 0;
+        for (int j0 = 0; j0 < N; j0 += 32) {
+            const int j = j0 + lane;
+            const bool nz = (j < N) && (Wbin[(size_t)j * n_mu + b] != 0.0);
+            cnt += __popc(__ballot_sync(0xffffffffu, nz));
+        }
+        if (lane == 0) s_cnt[b] = cnt;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int off = 0, total = 0;
+        for (int b = 0; b < n_mu; ++b) {
+            s_start[b] = off;
+            total += s_cnt[b];
+            off += (s_cnt[b] + 1) & ~1;
+        }
+        s_start[n_mu] = off;
+        long long nvis = 0;
+        double sw = 0.0, amax = 0.0;
+        for (int j = 0; j < N; ++j) {
+            nvis += col_nvis[j];
+            sw += col_sumw[j];
+            if (col_nvis[j] > 0) amax = fmax(amax, fabs(col_a[j]));
+        }
+        info->n_visible = nvis;
+        info->n_entries = total;
+        info->sum_weights = sw;
+        info->max_abs_dshift = amax;
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b <= n_mu; b += blockDim.x) row_start[b] = s_start[b];
+    for (int b = warp; b < n_mu; b += n_warps) {
+        int pos = s_start[b];
+        for (int j0 = 0; j0 < N; j0 += 32) {
+            const int j = j0 + lane;
+            const double W = (j < N) ? Wbin[(size_t)j * n_mu + b] : 0.0;
+            const unsigned m = __ballot_sync(0xffffffffu, W != 0.0);
+            if (W != 0.0) {
+                const int k = pos + __popc(m & ((1u << lane) - 1u));
+                const double a = col_a[j];
+                ent32[k] = make_float2((float)a, (float)W);
+                ent64[k] = make_double2(a, W);
+            }
+            pos += __popc(m);
+        }
+        if (lane == 0 && (s_cnt[b] & 1)) {
+            ent32[pos] = make_float2(0.f, 0.f);
+            ent64[pos] = make_double2(0.0, 0.0);
+        }
+    }
+}
+
+// SOAP_FORM_CELLS: one entry per visible cell (the literal double loop of Alg. 1), same layout.
+// Two passes over the cells by one CTA; within a row the entries keep (j, i) order.
+__global__ void build_cell_entries_kernel(int N, int n_mu, const double *__restrict__ col_a,
+                                          const double *__restrict__ w, const int *__restrict__ bin,
+                                          float2 *__restrict__ ent32, double2 *__restrict__ ent64,
+                                          int *__restrict__ row_start) {
+    __shared__ int s_cnt[64];
+    __shared__ int s_start[65];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+    const int ncell = N * N;
+    for (int b = warp; b < n_mu; b += n_warps) {
+        int cnt = 0;
+        for (int c0 = 0; c0 < ncell; c0 += 32) {
+            const int c = c0 + lane;
+            cnt += __popc(__ballot_sync(0xffffffffu, (c < ncell) && bin[c] == b));
+        }
+        if (lane == 0) s_cnt[b] = cnt;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int off = 0;
+        for (int b = 0; b < n_mu; ++b) {
+            s_start[b] = off;
+            off += (s_cnt[b] + 1) & ~1;
+        }
+        s_start[n_mu] = off;
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b <= n_mu; b += blockDim.x) row_start[b] = s_start[b];
+    for (int b = warp; b < n_mu; b += n_warps) {
+        int pos = s_start[b];
+        for (int c0 = 0; c0 < ncell; c0 += 32) {
+            const int c = c0 + lane;
+            const bool in = (c < ncell) && bin[c] == b;
+            const unsigned m = __ballot_sync(0xffffffffu, in);
+            if (in) {
+                const int k = pos + __popc(m & ((1u << lane) - 1u));
+                const double a = col_a[c / N];
+                ent32[k] = make_float2((float)a, (float)w[c]);
+                ent64[k] = make_double2(a, w[c]);
+            }
+            pos += __popc(m);
+        }
+        if (lane == 0 && (s_cnt[b] & 1)) {
+            ent32[pos] = make_float2(0.f, 0.f);
+            ent64[pos] = make_double2(0.0, 0.0);
+        }
+    }
+}
+
+}  // namespace soap

@@ -1,0 +1,666 @@
+// Host side of the C ABI declared in include/soap_b200.h: argument checks, scratch management and
+// kernel launches.  Every step of the path runs in the kernels of geometry.cuh / active.cuh / sia.cuh;
+// nothing here computes spectra on the CPU.  The only host arithmetic is O(n_regions * n_phases) region
+// centres (Localize of PAPER.md:69-71) and halo / grid sizing from the star parameters.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/soap_b200.h"
+#include "active.cuh"
+#include "geometry.cuh"
+#include "sia.cuh"
+
+namespace {
+
+using namespace soap;
+
+std::string g_create_error;
+
+template <typename T>
+struct DevBuf {
+    T *ptr = nullptr;
+    size_t cap = 0;  // elements
+    cudaError_t reserve(size_t n) {
+        if (n <= cap) return cudaSuccess;
+        if (ptr) cudaFree(ptr);
+        ptr = nullptr;
+        cap = 0;
+        cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&ptr), n * sizeof(T));
+        if (e == cudaSuccess) cap = n;
+        return e;
+    }
+    void release() {
+        if (ptr) cudaFree(ptr);
+        ptr = nullptr;
+        cap = 0;
+    }
+};
+
+struct Counters {  // device-resident, read back by soap_get_stats
+    unsigned long long active_entries;
+    unsigned long long pad;
+};
+
+}  // namespace
+
+struct soap_star {
+    int device = 0;
+    int n_sm = 148;
+    std::string err;
+    bool ready = false;
+
+    // star
+    soap_star_params prm{};
+    std::vector<double> mu_centres;
+    double sini = 1.0, cosi = 0.0;
+    double amax = 0.0;  // host bound on max |D - 1|
+    int form = SOAP_FORM_AUTO, form_used = SOAP_FORM_BINNED;
+    int opt_quiet_splits = 0;
+    bool opt_timing = false;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};  // quiet start/stop, active start/stop
+    bool ev_valid[2] = {false, false};
+
+    // geometry (device)
+    DevBuf<double> d_mu_centres, d_mu, d_w, d_vel, d_col_a, d_Wbin, d_col_sumw;
+    DevBuf<int> d_bin, d_col_nvis, d_row_start;
+    DevBuf<float2> d_ent32;
+    DevBuf<double2> d_ent64;
+    DevBuf<DevInfo> d_info;
+    size_t ent_cap = 0;
+
+    // quiet scratch
+    DevBuf<double> d_partial;
+
+    // active scratch
+    DevBuf<RegionAtPhase> d_rp;
+    struct PinnedSlot {  // ring of pinned staging buffers: a slot is reused only after its copy completed
+        RegionAtPhase *ptr = nullptr;
+        size_t cap = 0;
+        cudaEvent_t done = nullptr;
+        bool in_flight = false;
+    } h_rp[4];
+    int h_rp_next = 0;
+    DevBuf<double> d_WD;
+    DevBuf<unsigned char> d_aent;
+    DevBuf<int> d_segcnt, d_nactive;
+    DevBuf<Counters> d_counters;
+
+    // host-buffer staging (soap_synthesize_host)
+    DevBuf<unsigned char> d_stage[3], d_stage_c[3], d_out_q, d_out_d;
+
+    // stats
+    int last_quiet_splits = 0, last_tile_px = 0, launches = 0;
+    long long last_active_cells = 0;
+
+    int fail(int code, const char *fmt, ...) {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof(buf), fmt, ap);
+        va_end(ap);
+        err = buf;
+        return code;
+    }
+};
+
+namespace {
+
+#define SOAP_CUDA(star, call)                                                                            \
+    do {                                                                                                 \
+        cudaError_t e__ = (call);                                                                        \
+        if (e__ != cudaSuccess)                                                                          \
+            return (star)->fail(e__ == cudaErrorMemoryAllocation ? SOAP_ERR_OOM : SOAP_ERR_CUDA,         \
+                                "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__, __LINE__); \
+    } while (0)
+
+#define SOAP_LAUNCH_CHECK(star, name)                                                                    \
+    do {                                                                                                 \
+        cudaError_t e__ = cudaGetLastError();                                                            \
+        if (e__ != cudaSuccess)                                                                          \
+            return (star)->fail(SOAP_ERR_CUDA, "launch of %s failed: %s", name, cudaGetErrorString(e__)); \
+        (star)->launches++;                                                                              \
+    } while (0)
+
+inline double host_dshift(double v_kms, int mode) {
+    const double b = v_kms / kSpeedOfLightKms;
+    if (mode == 1) return -b;
+    return -2.0 * b / ((1.0 + b) + std::sqrt(1.0 - b * b));
+}
+
+inline int round_up4(long long v) { return (int)((v + 3) & ~3LL); }
+
+int check_spectra(soap_star *s, const soap_spectra *sp, const char *name) {
+    if (!sp) return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: NULL", name);
+    if (!sp->data) return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: data is NULL", name);
+    if (sp->n_pix < 2) return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: n_pix must be >= 2", name);
+    if (sp->n_pix > (1LL << 30)) return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: n_pix too large", name);
+    if (sp->pitch < sp->n_pix || (sp->pitch & 3))
+        return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: pitch must be >= n_pix and a multiple of 4", name);
+    if (sp->dtype != SOAP_F32 && sp->dtype != SOAP_F64)
+        return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: unknown dtype %d", name, sp->dtype);
+    if (reinterpret_cast<uintptr_t>(sp->data) & 15)
+        return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: data must be 16-byte aligned", name);
+    if (!(sp->dlambda > 0.0) || !(sp->lambda0 > 0.0) || !std::isfinite(sp->dlambda) || !std::isfinite(sp->lambda0))
+        return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: lambda0 and dlambda must be positive and finite", name);
+    if (!std::isfinite(sp->lb_c0) || !std::isfinite(sp->lb_c1) || !std::isfinite(sp->lb_c2))
+        return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: limb-brightening coefficients must be finite", name);
+    return SOAP_OK;
+}
+
+int check_same_grid(soap_star *s, const soap_spectra *a, const soap_spectra *b, const char *name) {
+    if (a->n_pix != b->n_pix || a->dtype != b->dtype || a->lambda0 != b->lambda0 || a->dlambda != b->dlambda)
+        return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: n_pix / dtype / lambda0 / dlambda differ from quiet", name);
+    if (a->pitch != b->pitch) return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: pitch differs from quiet", name);
+    return SOAP_OK;
+}
+
+int halo_for(const soap_star *s, const soap_spectra *sp) {
+    const double c0 = sp->lambda0 / sp->dlambda;
+    const double maxd = s->amax * (c0 + (double)sp->n_pix) * (1.0 + 1e-6);
+    return round_up4((long long)std::ceil(maxd) + 2);
+}
+
+template <typename T, bool ACTIVE>
+int launch_sia(soap_star *s, const SiaParams<T> &p, dim3 grid, cudaStream_t st) {
+    const size_t smem = sia_smem_bytes<T>(p.halo);
+    if (smem > 227 * 1024) return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", p.halo, smem);
+    if (smem > 48 * 1024)
+        SOAP_CUDA(s, cudaFuncSetAttribute(sia_kernel<T, ACTIVE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int e0 = ACTIVE ? 2 : 0;
+    if (s->opt_timing) {
+        for (int k = e0; k < e0 + 2; ++k)
+            if (!s->ev[k]) SOAP_CUDA(s, cudaEventCreate(&s->ev[k]));
+        SOAP_CUDA(s, cudaEventRecord(s->ev[e0], st));
+    }
+    sia_kernel<T, ACTIVE><<<grid, kThreads, smem, st>>>(p);
+    SOAP_LAUNCH_CHECK(s, ACTIVE ? "sia_kernel<active>" : "sia_kernel<quiet>");
+    if (s->opt_timing) {
+        SOAP_CUDA(s, cudaEventRecord(s->ev[e0 + 1], st));
+        s->ev_valid[ACTIVE ? 1 : 0] = true;
+    }
+    return SOAP_OK;
+}
+
+template <typename T>
+int quiet_impl(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
+    constexpr int TP = sia_tile_px<T>();
+    const long long P = q->n_pix;
+    const int n_tiles = (int)((P + TP - 1) / TP);
+    int splits = s->opt_quiet_splits;
+    if (splits <= 0) {
+        // ~8 CTAs of 128 threads per SM; the entry list is cut into `splits` chunks per wavelength tile
+        splits = (int)std::lround((double)(s->n_sm * 8) / n_tiles);
+        const long long max_entries = (long long)s->prm.grid_n * (s->form_used == SOAP_FORM_CELLS ? s->prm.grid_n : s->prm.n_mu);
+        const int cap = (int)std::max(1LL, max_entries / 16);
+        splits = std::max(1, std::min(std::min(splits, 256), cap));
+    }
+    const long long part_pitch = (P + 3) & ~3LL;
+    SOAP_CUDA(s, s->d_partial.reserve((size_t)splits * part_pitch));
+    SiaParams<T> p{};
+    p.base[0] = static_cast<const T *>(q->data);
+    p.pitch = q->pitch;
+    p.n_pix = P;
+    p.c0 = q->lambda0 / q->dlambda;
+    p.n_mu = s->prm.n_mu;
+    p.halo = halo_for(s, q);
+    if (sizeof(T) == 4) p.ent = reinterpret_cast<const typename SiaTraits<T>::Ent *>(s->d_ent32.ptr);
+    else p.ent = reinterpret_cast<const typename SiaTraits<T>::Ent *>(s->d_ent64.ptr);
+    p.row_start = s->d_row_start.ptr;
+    p.n_splits = splits;
+    p.partial = s->d_partial.ptr;
+    p.part_pitch = part_pitch;
+    int rc = launch_sia<T, false>(s, p, dim3(n_tiles, splits), st);
+    if (rc) return rc;
+    const int threads = 256;
+    const long long quads = (P + 3) / 4;
+    reduce_partials_kernel<T><<<(unsigned)((quads + threads - 1) / threads), threads, 0, st>>>(
+        s->d_partial.ptr, part_pitch, splits, P, static_cast<T *>(out));
+    SOAP_LAUNCH_CHECK(s, "reduce_partials_kernel");
+    s->last_quiet_splits = splits;
+    s->last_tile_px = TP;
+    return SOAP_OK;
+}
+
+template <typename T>
+int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, const soap_spectra *fac,
+                int n_regions, int n_phases, void *out, long long out_pitch, cudaStream_t st) {
+    using Ent = typename SiaTraits<T>::Ent;
+    constexpr int TP = sia_tile_px<T>();
+    const int N = s->prm.grid_n, n_mu = s->prm.n_mu;
+    const int ncap = ((N + 1) & ~1) + 2;
+    const long long n_seg = (long long)n_phases * 3 * n_mu;
+    if (n_seg * ncap >= (1LL << 31)) return s->fail(SOAP_ERR_UNSUPPORTED, "n_phases * 3 * n_mu * N too large for one call");
+    SOAP_CUDA(s, s->d_WD.reserve((size_t)n_seg * ncap));
+    SOAP_CUDA(s, s->d_aent.reserve((size_t)n_seg * ncap * sizeof(Ent) + 64));
+    SOAP_CUDA(s, s->d_segcnt.reserve((size_t)n_seg));
+    SOAP_CUDA(s, s->d_nactive.reserve((size_t)n_phases));
+    SOAP_CUDA(s, s->d_counters.reserve(1));
+    SOAP_CUDA(s, cudaMemsetAsync(s->d_WD.ptr, 0, (size_t)n_seg * ncap * sizeof(double), st));
+    SOAP_CUDA(s, cudaMemsetAsync(s->d_nactive.ptr, 0, (size_t)n_phases * sizeof(int), st));
+    SOAP_CUDA(s, cudaMemsetAsync(s->d_counters.ptr, 0, sizeof(Counters), st));
+    if (n_regions > 0) {
+        LbCoef lb{};
+        lb.c[1][0] = spot ? spot->lb_c0 : 1.0; lb.c[1][1] = spot ? spot->lb_c1 : 0.0; lb.c[1][2] = spot ? spot->lb_c2 : 0.0;
+        lb.c[2][0] = fac ? fac->lb_c0 : 1.0;  lb.c[2][1] = fac ? fac->lb_c1 : 0.0;  lb.c[2][2] = fac ? fac->lb_c2 : 0.0;
+        active_bin_kernel<<<dim3((N + 127) / 128, n_phases), 128, 0, st>>>(
+            N, n_regions, n_mu, ncap, s->d_rp.ptr, s->d_mu.ptr, s->d_w.ptr, s->d_bin.ptr, lb, s->d_WD.ptr,
+            s->d_nactive.ptr);
+        SOAP_LAUNCH_CHECK(s, "active_bin_kernel");
+    }
+    {
+        const int warps_per_block = 8;
+        const unsigned blocks = (unsigned)((n_seg + warps_per_block - 1) / warps_per_block);
+        active_compact_kernel<Ent><<<blocks, warps_per_block * 32, 0, st>>>(
+            N, n_mu, ncap, (int)n_seg, s->d_col_a.ptr, s->d_WD.ptr, reinterpret_cast<Ent *>(s->d_aent.ptr),
+            s->d_segcnt.ptr, &s->d_counters.ptr->active_entries);
+        SOAP_LAUNCH_CHECK(s, "active_compact_kernel");
+    }
+    SiaParams<T> p{};
+    p.base[0] = static_cast<const T *>(q->data);
+    p.base[1] = spot ? static_cast<const T *>(spot->data) : p.base[0];
+    p.base[2] = fac ? static_cast<const T *>(fac->data) : p.base[0];
+    p.contrast[1] = spot ? static_cast<const T *>(spot->contrast) : nullptr;
+    p.contrast[2] = fac ? static_cast<const T *>(fac->contrast) : nullptr;
+    p.pitch = q->pitch;
+    p.n_pix = q->n_pix;
+    p.c0 = q->lambda0 / q->dlambda;
+    p.n_mu = n_mu;
+    p.halo = halo_for(s, q);
+    p.ent = reinterpret_cast<const Ent *>(s->d_aent.ptr);
+    p.seg_count = s->d_segcnt.ptr;
+    p.seg_cap = ncap;
+    p.out = static_cast<T *>(out);
+    p.out_pitch = out_pitch;
+    const int n_tiles = (int)((q->n_pix + TP - 1) / TP);
+    s->last_tile_px = TP;
+    return launch_sia<T, true>(s, p, dim3(n_tiles, n_phases), st);
+}
+
+int check_regions(soap_star *s, const soap_region *regions, int n_regions, const double *phases, int n_phases,
+                  const soap_spectra *spot, const soap_spectra *fac) {
+    if (n_regions < 0 || n_phases < 0) return s->fail(SOAP_ERR_INVALID_ARG, "negative n_regions / n_phases");
+    if (n_regions > 0 && !regions) return s->fail(SOAP_ERR_INVALID_ARG, "regions is NULL");
+    if (n_phases > 0 && !phases) return s->fail(SOAP_ERR_INVALID_ARG, "phases is NULL");
+    for (int r = 0; r < n_regions; ++r) {
+        const soap_region &g = regions[r];
+        if (g.type != SOAP_SPOT && g.type != SOAP_FACULA) return s->fail(SOAP_ERR_INVALID_ARG, "region %d: unknown type %d", r, g.type);
+        if (!(g.radius > 0.0 && g.radius < 1.0)) return s->fail(SOAP_ERR_INVALID_ARG, "region %d: radius must be in (0,1)", r);
+        if (!std::isfinite(g.lat_deg) || !std::isfinite(g.lon_deg)) return s->fail(SOAP_ERR_INVALID_ARG, "region %d: lat/lon not finite", r);
+        if (g.type == SOAP_SPOT && !spot) return s->fail(SOAP_ERR_INVALID_ARG, "region %d is a spot but spot spectra are NULL", r);
+        if (g.type == SOAP_FACULA && !fac) return s->fail(SOAP_ERR_INVALID_ARG, "region %d is a facula but facula spectra are NULL", r);
+    }
+    for (int p = 0; p < n_phases; ++p)
+        if (!std::isfinite(phases[p])) return s->fail(SOAP_ERR_INVALID_ARG, "phase %d not finite", p);
+    return SOAP_OK;
+}
+
+// Localize (readings S11-S13): region centres in the observer frame for every phase.
+int upload_region_centres(soap_star *s, const soap_region *regions, int n_regions, const double *phases,
+                          int n_phases, cudaStream_t st) {
+    const size_t n = (size_t)n_regions * n_phases;
+    if (n == 0) return SOAP_OK;
+    soap_star::PinnedSlot &slot = s->h_rp[s->h_rp_next];
+    s->h_rp_next = (s->h_rp_next + 1) & 3;
+    if (slot.in_flight) {
+        SOAP_CUDA(s, cudaEventSynchronize(slot.done));
+        slot.in_flight = false;
+    }
+    if (!slot.done) SOAP_CUDA(s, cudaEventCreateWithFlags(&slot.done, cudaEventDisableTiming));
+    if (n > slot.cap) {
+        if (slot.ptr) cudaFreeHost(slot.ptr);
+        slot.ptr = nullptr;
+        slot.cap = 0;
+        SOAP_CUDA(s, cudaMallocHost(reinterpret_cast<void **>(&slot.ptr), n * sizeof(RegionAtPhase)));
+        slot.cap = n;
+    }
+    if (n > s->d_rp.cap) {
+        // growing d_rp frees the old buffer, which an earlier call's kernel may still be reading
+        SOAP_CUDA(s, cudaDeviceSynchronize());
+        SOAP_CUDA(s, s->d_rp.reserve(n));
+    }
+    const double pi = 3.14159265358979323846;
+    for (int p = 0; p < n_phases; ++p) {
+        for (int r = 0; r < n_regions; ++r) {
+            const soap_region &g = regions[r];
+            const double lat = g.lat_deg * pi / 180.0;
+            const double L = g.lon_deg * pi / 180.0 + 2.0 * pi * phases[p];
+            const double sx = std::cos(lat) * std::sin(L), sy = std::sin(lat), sz = std::cos(lat) * std::cos(L);
+            RegionAtPhase &o = slot.ptr[(size_t)p * n_regions + r];
+            o.xr = sx;
+            o.yr = sy * s->sini - sz * s->cosi;
+            o.zr = sy * s->cosi + sz * s->sini;
+            o.cos_alpha = std::sqrt(1.0 - g.radius * g.radius);
+            o.chord = 2.0 * std::sin(0.5 * std::asin(g.radius));
+            o.type = (o.zr < -g.radius - 1e-9) ? 0 : g.type;  // cap entirely on the far side
+            o.pad = 0;
+        }
+    }
+    SOAP_CUDA(s, cudaMemcpyAsync(s->d_rp.ptr, slot.ptr, n * sizeof(RegionAtPhase), cudaMemcpyHostToDevice, st));
+    SOAP_CUDA(s, cudaEventRecord(slot.done, st));
+    slot.in_flight = true;
+    return SOAP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int soap_version(void) { return SOAP_B200_VERSION; }
+
+const char *soap_last_error(const soap_star *star) { return star ? star->err.c_str() : g_create_error.c_str(); }
+
+int soap_create(soap_star **out, int device) {
+    if (!out) {
+        g_create_error = "soap_create: out is NULL";
+        return SOAP_ERR_INVALID_ARG;
+    }
+    *out = nullptr;
+    int n_dev = 0;
+    cudaError_t e = cudaGetDeviceCount(&n_dev);
+    if (e != cudaSuccess || n_dev == 0) {
+        g_create_error = std::string("soap_create: no CUDA device (") + cudaGetErrorString(e) + "); this library has no CPU fallback";
+        return SOAP_ERR_CUDA;
+    }
+    if (device < 0 || device >= n_dev) {
+        g_create_error = "soap_create: device index out of range";
+        return SOAP_ERR_INVALID_ARG;
+    }
+    soap_star *s = new (std::nothrow) soap_star();
+    if (!s) {
+        g_create_error = "soap_create: out of host memory";
+        return SOAP_ERR_OOM;
+    }
+    s->device = device;
+    cudaSetDevice(device);
+    int n_sm = 0;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) == cudaSuccess && n_sm > 0) s->n_sm = n_sm;
+    *out = s;
+    return SOAP_OK;
+}
+
+int soap_destroy(soap_star *s) {
+    if (!s) return SOAP_OK;
+    cudaSetDevice(s->device);
+    s->d_mu_centres.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
+    s->d_Wbin.release(); s->d_col_sumw.release(); s->d_bin.release(); s->d_col_nvis.release(); s->d_row_start.release();
+    s->d_ent32.release(); s->d_ent64.release(); s->d_info.release(); s->d_partial.release(); s->d_rp.release();
+    s->d_WD.release(); s->d_aent.release(); s->d_segcnt.release(); s->d_nactive.release(); s->d_counters.release();
+    for (int k = 0; k < 3; ++k) { s->d_stage[k].release(); s->d_stage_c[k].release(); }
+    s->d_out_q.release(); s->d_out_d.release();
+    for (auto &e : s->ev)
+        if (e) cudaEventDestroy(e);
+    for (auto &slot : s->h_rp) {
+        if (slot.ptr) cudaFreeHost(slot.ptr);
+        if (slot.done) cudaEventDestroy(slot.done);
+    }
+    delete s;
+    return SOAP_OK;
+}
+
+int soap_set_option(soap_star *s, int32_t option, int64_t value) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    switch (option) {
+        case SOAP_OPT_FORM:
+            if (value < SOAP_FORM_AUTO || value > SOAP_FORM_FIR) return s->fail(SOAP_ERR_INVALID_ARG, "unknown form %lld", (long long)value);
+            if (value == SOAP_FORM_FIR) return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_FIR is not implemented in this build");
+            if ((int)value != s->form) s->ready = false;  // entry list must be rebuilt
+            s->form = (int)value;
+            return SOAP_OK;
+        case SOAP_OPT_QUIET_SPLITS:
+            if (value < 0 || value > 1024) return s->fail(SOAP_ERR_INVALID_ARG, "quiet splits out of range");
+            s->opt_quiet_splits = (int)value;
+            return SOAP_OK;
+        case SOAP_OPT_KERNEL_TIMING:
+            s->opt_timing = value != 0;
+            s->ev_valid[0] = s->ev_valid[1] = false;
+            return SOAP_OK;
+        default:
+            return s->fail(SOAP_ERR_INVALID_ARG, "unknown option %d", option);
+    }
+}
+
+int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, soap_geom_info *info) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!prm) return s->fail(SOAP_ERR_INVALID_ARG, "params is NULL");
+    if (prm->grid_n < 1 || prm->grid_n > 8192) return s->fail(SOAP_ERR_INVALID_ARG, "grid_n must be in 1..8192");
+    if (prm->n_mu < 1 || prm->n_mu > SOAP_MAX_MU) return s->fail(SOAP_ERR_INVALID_ARG, "n_mu must be in 1..%d", SOAP_MAX_MU);
+    if (!prm->mu_centres) return s->fail(SOAP_ERR_INVALID_ARG, "mu_centres is NULL");
+    for (int b = 0; b < prm->n_mu; ++b) {
+        if (!std::isfinite(prm->mu_centres[b])) return s->fail(SOAP_ERR_INVALID_ARG, "mu_centres[%d] not finite", b);
+        if (b && !(prm->mu_centres[b] > prm->mu_centres[b - 1])) return s->fail(SOAP_ERR_INVALID_ARG, "mu_centres must be strictly ascending");
+    }
+    if (!std::isfinite(prm->vsini_kms) || !std::isfinite(prm->incl_deg) || !std::isfinite(prm->ld_u1) || !std::isfinite(prm->ld_u2))
+        return s->fail(SOAP_ERR_INVALID_ARG, "vsini / incl / limb-darkening coefficients must be finite");
+    if (prm->doppler_mode != 0 && prm->doppler_mode != 1) return s->fail(SOAP_ERR_INVALID_ARG, "doppler_mode must be 0 or 1");
+    const double pi = 3.14159265358979323846;
+    const double sini = std::sin(prm->incl_deg * pi / 180.0), cosi = std::cos(prm->incl_deg * pi / 180.0);
+    if (std::fabs(prm->vsini_kms * sini) >= 0.1 * kSpeedOfLightKms) return s->fail(SOAP_ERR_INVALID_ARG, "|v| must be below 0.1 c");
+
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    s->ready = false;
+    s->prm = *prm;
+    s->mu_centres.assign(prm->mu_centres, prm->mu_centres + prm->n_mu);
+    s->prm.mu_centres = s->mu_centres.data();
+    s->sini = sini;
+    s->cosi = cosi;
+    const int N = prm->grid_n, n_mu = prm->n_mu;
+    const size_t ncell = (size_t)N * N;
+    s->form_used = (s->form == SOAP_FORM_CELLS) ? SOAP_FORM_CELLS : SOAP_FORM_BINNED;
+    const double vmax = std::fabs(prm->vsini_kms * sini) * (double)(N - 1) / (double)N;
+    s->amax = std::max(std::fabs(host_dshift(vmax, prm->doppler_mode)), std::fabs(host_dshift(-vmax, prm->doppler_mode)));
+
+    SOAP_CUDA(s, s->d_mu_centres.reserve(n_mu));
+    SOAP_CUDA(s, s->d_mu.reserve(ncell));
+    SOAP_CUDA(s, s->d_w.reserve(ncell));
+    SOAP_CUDA(s, s->d_vel.reserve(ncell));
+    SOAP_CUDA(s, s->d_bin.reserve(ncell));
+    SOAP_CUDA(s, s->d_col_a.reserve(N));
+    SOAP_CUDA(s, s->d_Wbin.reserve((size_t)N * n_mu));
+    SOAP_CUDA(s, s->d_col_sumw.reserve(N));
+    SOAP_CUDA(s, s->d_col_nvis.reserve(N));
+    SOAP_CUDA(s, s->d_row_start.reserve(n_mu + 1));
+    SOAP_CUDA(s, s->d_info.reserve(1));
+    const size_t ent_cap = std::max(s->form_used == SOAP_FORM_CELLS ? ncell : (size_t)0, (size_t)N * n_mu) + 2 * (size_t)n_mu + 8;
+    SOAP_CUDA(s, s->d_ent32.reserve(ent_cap));
+    SOAP_CUDA(s, s->d_ent64.reserve(ent_cap));
+
+    // mu_centres: tiny pageable copy; the source is the handle's own vector, which outlives the copy
+    SOAP_CUDA(s, cudaMemcpyAsync(s->d_mu_centres.ptr, s->mu_centres.data(), n_mu * sizeof(double), cudaMemcpyHostToDevice, st));
+    const double vs = prm->vsini_kms * sini;
+    geometry_cells_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, st>>>(N, vs, prm->ld_u1, prm->ld_u2, n_mu, s->d_mu_centres.ptr,
+                                                                           s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr, s->d_bin.ptr);
+    SOAP_LAUNCH_CHECK(s, "geometry_cells_kernel");
+    geometry_columns_kernel<<<(N + 127) / 128, 128, 0, st>>>(N, vs, prm->doppler_mode, n_mu, s->d_w.ptr, s->d_bin.ptr, s->d_col_a.ptr,
+                                                             s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr);
+    SOAP_LAUNCH_CHECK(s, "geometry_columns_kernel");
+    build_binned_entries_kernel<<<1, 1024, 0, st>>>(N, n_mu, s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr,
+                                                    s->d_ent32.ptr, s->d_ent64.ptr, s->d_row_start.ptr, s->d_info.ptr);
+    SOAP_LAUNCH_CHECK(s, "build_binned_entries_kernel");
+    if (s->form_used == SOAP_FORM_CELLS) {
+        build_cell_entries_kernel<<<1, 1024, 0, st>>>(N, n_mu, s->d_col_a.ptr, s->d_w.ptr, s->d_bin.ptr, s->d_ent32.ptr,
+                                                      s->d_ent64.ptr, s->d_row_start.ptr);
+        SOAP_LAUNCH_CHECK(s, "build_cell_entries_kernel");
+    }
+    s->ready = true;
+    if (info) {
+        DevInfo di;
+        SOAP_CUDA(s, cudaMemcpyAsync(&di, s->d_info.ptr, sizeof(di), cudaMemcpyDeviceToHost, st));
+        SOAP_CUDA(s, cudaStreamSynchronize(st));
+        info->n_visible = di.n_visible;
+        info->n_entries = (s->form_used == SOAP_FORM_CELLS) ? di.n_visible : di.n_entries;
+        info->sum_weights = di.sum_weights;
+        info->max_abs_dshift = di.max_abs_dshift;
+    }
+    return SOAP_OK;
+}
+
+int soap_integrate_quiet(soap_star *s, const soap_spectra *quiet, void *out, void *stream) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!s->ready) return s->fail(SOAP_ERR_NOT_READY, "soap_disk_geometry has not been called");
+    int rc = check_spectra(s, quiet, "quiet");
+    if (rc) return rc;
+    if (!out) return s->fail(SOAP_ERR_INVALID_ARG, "out is NULL");
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    return quiet->dtype == SOAP_F32 ? quiet_impl<float>(s, quiet, out, st) : quiet_impl<double>(s, quiet, out, st);
+}
+
+int soap_active_timeseries(soap_star *s, const soap_spectra *quiet, const soap_spectra *spot, const soap_spectra *facula,
+                           const soap_region *regions, int32_t n_regions, const double *phases, int32_t n_phases,
+                           void *out_delta, int64_t out_pitch, int32_t *n_active, void *stream) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!s->ready) return s->fail(SOAP_ERR_NOT_READY, "soap_disk_geometry has not been called");
+    int rc = check_spectra(s, quiet, "quiet");
+    if (rc) return rc;
+    if (spot && ((rc = check_spectra(s, spot, "spot")) || (rc = check_same_grid(s, quiet, spot, "spot")))) return rc;
+    if (facula && ((rc = check_spectra(s, facula, "facula")) || (rc = check_same_grid(s, quiet, facula, "facula")))) return rc;
+    if ((rc = check_regions(s, regions, n_regions, phases, n_phases, spot, facula))) return rc;
+    if (n_phases == 0) return SOAP_OK;
+    if (!out_delta) return s->fail(SOAP_ERR_INVALID_ARG, "out_delta is NULL");
+    if (out_pitch < quiet->n_pix) return s->fail(SOAP_ERR_INVALID_ARG, "out_pitch must be >= n_pix");
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((rc = upload_region_centres(s, regions, n_regions, phases, n_phases, st))) return rc;
+    rc = quiet->dtype == SOAP_F32 ? active_impl<float>(s, quiet, spot, facula, n_regions, n_phases, out_delta, out_pitch, st)
+                                  : active_impl<double>(s, quiet, spot, facula, n_regions, n_phases, out_delta, out_pitch, st);
+    if (rc) return rc;
+    if (n_active) {
+        SOAP_CUDA(s, cudaMemcpyAsync(n_active, s->d_nactive.ptr, (size_t)n_phases * sizeof(int), cudaMemcpyDeviceToHost, st));
+        SOAP_CUDA(s, cudaStreamSynchronize(st));
+        long long tot = 0;
+        for (int p = 0; p < n_phases; ++p) tot += n_active[p];
+        s->last_active_cells = tot;
+    }
+    return SOAP_OK;
+}
+
+int soap_get_stats(soap_star *s, soap_stats *stats, void *stream) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!stats) return s->fail(SOAP_ERR_INVALID_ARG, "stats is NULL");
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::memset(stats, 0, sizeof(*stats));
+    if (s->ready) {
+        DevInfo di;
+        SOAP_CUDA(s, cudaMemcpyAsync(&di, s->d_info.ptr, sizeof(di), cudaMemcpyDeviceToHost, st));
+        SOAP_CUDA(s, cudaStreamSynchronize(st));
+        stats->quiet_entries = (s->form_used == SOAP_FORM_CELLS) ? di.n_visible : di.n_entries;
+    }
+    if (s->d_counters.ptr) {
+        Counters c;
+        SOAP_CUDA(s, cudaMemcpyAsync(&c, s->d_counters.ptr, sizeof(c), cudaMemcpyDeviceToHost, st));
+        SOAP_CUDA(s, cudaStreamSynchronize(st));
+        stats->active_entries = (long long)c.active_entries;
+    }
+    stats->active_cells = s->last_active_cells;
+    stats->quiet_splits = s->last_quiet_splits;
+    stats->tile_px = s->last_tile_px;
+    stats->form = s->form_used;
+    stats->launches = s->launches;
+    if (s->opt_timing) {
+        SOAP_CUDA(s, cudaStreamSynchronize(st));
+        if (s->ev_valid[0]) SOAP_CUDA(s, cudaEventElapsedTime(&stats->quiet_kernel_ms, s->ev[0], s->ev[1]));
+        if (s->ev_valid[1]) SOAP_CUDA(s, cudaEventElapsedTime(&stats->active_kernel_ms, s->ev[2], s->ev[3]));
+    }
+    return SOAP_OK;
+}
+
+int soap_export_geometry(soap_star *s, double *mu, double *vel, double *w, int32_t *bin) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!s->ready) return s->fail(SOAP_ERR_NOT_READY, "soap_disk_geometry has not been called");
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    SOAP_CUDA(s, cudaDeviceSynchronize());
+    const size_t ncell = (size_t)s->prm.grid_n * s->prm.grid_n;
+    if (mu) SOAP_CUDA(s, cudaMemcpy(mu, s->d_mu.ptr, ncell * sizeof(double), cudaMemcpyDeviceToHost));
+    if (vel) SOAP_CUDA(s, cudaMemcpy(vel, s->d_vel.ptr, ncell * sizeof(double), cudaMemcpyDeviceToHost));
+    if (w) SOAP_CUDA(s, cudaMemcpy(w, s->d_w.ptr, ncell * sizeof(double), cudaMemcpyDeviceToHost));
+    if (bin) SOAP_CUDA(s, cudaMemcpy(bin, s->d_bin.ptr, ncell * sizeof(int), cudaMemcpyDeviceToHost));
+    return SOAP_OK;
+}
+
+int soap_synthesize_host(soap_star *s, const soap_star_params *prm, const soap_spectra *quiet, const soap_spectra *spot,
+                         const soap_spectra *facula, const soap_region *regions, int32_t n_regions, const double *phases,
+                         int32_t n_phases, void *out_quiet, void *out_delta, int32_t *n_active, void *stream) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!quiet || !quiet->data) return s->fail(SOAP_ERR_INVALID_ARG, "quiet spectra missing");
+    if (!out_quiet) return s->fail(SOAP_ERR_INVALID_ARG, "out_quiet is NULL");
+    if (n_phases > 0 && !out_delta) return s->fail(SOAP_ERR_INVALID_ARG, "out_delta is NULL");
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const soap_spectra *in[3] = {quiet, spot, facula};
+    soap_spectra dev[3];
+    const size_t esz = quiet->dtype == SOAP_F64 ? 8 : 4;
+    if (!prm) return s->fail(SOAP_ERR_INVALID_ARG, "params is NULL");
+    if (prm->n_mu < 1 || prm->n_mu > SOAP_MAX_MU) return s->fail(SOAP_ERR_INVALID_ARG, "n_mu must be in 1..%d", SOAP_MAX_MU);
+    for (int k = 0; k < 3; ++k) {
+        if (!in[k]) continue;
+        if (!in[k]->data) return s->fail(SOAP_ERR_INVALID_ARG, "spectra %d: data is NULL", k);
+        if (in[k]->n_pix < 2 || in[k]->pitch < in[k]->n_pix || (in[k]->pitch & 3) || in[k]->dtype != quiet->dtype)
+            return s->fail(SOAP_ERR_INVALID_ARG, "spectra %d: bad n_pix / pitch / dtype", k);
+        const size_t bytes = (size_t)prm->n_mu * in[k]->pitch * esz;
+        SOAP_CUDA(s, s->d_stage[k].reserve(bytes));
+        SOAP_CUDA(s, cudaMemcpyAsync(s->d_stage[k].ptr, in[k]->data, bytes, cudaMemcpyHostToDevice, st));
+        dev[k] = *in[k];
+        dev[k].data = s->d_stage[k].ptr;
+        if (k > 0 && in[k]->contrast) {
+            SOAP_CUDA(s, s->d_stage_c[k].reserve((size_t)in[k]->n_pix * esz));
+            SOAP_CUDA(s, cudaMemcpyAsync(s->d_stage_c[k].ptr, in[k]->contrast, (size_t)in[k]->n_pix * esz, cudaMemcpyHostToDevice, st));
+            dev[k].contrast = s->d_stage_c[k].ptr;
+        } else {
+            dev[k].contrast = nullptr;
+        }
+    }
+    const long long P = quiet->n_pix;
+    SOAP_CUDA(s, s->d_out_q.reserve((size_t)P * esz));
+    if (n_phases > 0) SOAP_CUDA(s, s->d_out_d.reserve((size_t)n_phases * P * esz));
+    int rc = soap_disk_geometry(s, prm, stream, nullptr);
+    if (rc) return rc;
+    if ((rc = soap_integrate_quiet(s, &dev[0], s->d_out_q.ptr, stream))) return rc;
+    if (n_phases > 0) {
+        rc = soap_active_timeseries(s, &dev[0], spot ? &dev[1] : nullptr, facula ? &dev[2] : nullptr, regions, n_regions, phases,
+                                    n_phases, s->d_out_d.ptr, P, nullptr, stream);
+        if (rc) return rc;
+        SOAP_CUDA(s, cudaMemcpyAsync(out_delta, s->d_out_d.ptr, (size_t)n_phases * P * esz, cudaMemcpyDeviceToHost, st));
+        if (n_active)
+            SOAP_CUDA(s, cudaMemcpyAsync(n_active, s->d_nactive.ptr, (size_t)n_phases * sizeof(int), cudaMemcpyDeviceToHost, st));
+    }
+    SOAP_CUDA(s, cudaMemcpyAsync(out_quiet, s->d_out_q.ptr, (size_t)P * esz, cudaMemcpyDeviceToHost, st));
+    SOAP_CUDA(s, cudaStreamSynchronize(st));
+    return SOAP_OK;
+}
+
+int soap_batch_integrate_quiet(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet, void *const *out,
+                               void *stream) {
+    if (!stars || !quiet || !out || n_stars < 0) return SOAP_ERR_INVALID_ARG;
+    for (int k = 0; k < n_stars; ++k) {
+        if (!stars[k]) return SOAP_ERR_INVALID_ARG;
+        int rc = soap_integrate_quiet(stars[k], quiet[k], out[k], stream);
+        if (rc) return rc;
+    }
+    return SOAP_OK;
+}
+
+int soap_batch_active_timeseries(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet,
+                                 const soap_spectra *const *spot, const soap_spectra *const *facula,
+                                 const soap_region *const *regions, const int32_t *n_regions, const double *const *phases,
+                                 const int32_t *n_phases, void *const *out_delta, const int64_t *out_pitch, void *stream) {
+    if (!stars || !quiet || !regions || !n_regions || !phases || !n_phases || !out_delta || !out_pitch || n_stars < 0)
+        return SOAP_ERR_INVALID_ARG;
+    for (int k = 0; k < n_stars; ++k) {
+        if (!stars[k]) return SOAP_ERR_INVALID_ARG;
+        int rc = soap_active_timeseries(stars[k], quiet[k], spot ? spot[k] : nullptr, facula ? facula[k] : nullptr, regions[k],
+                                        n_regions[k], phases[k], n_phases[k], out_delta[k], out_pitch[k], nullptr, stream);
+        if (rc) return rc;
+    }
+    return SOAP_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,314 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 CPU oracle.  Needs a B200: -m gpu.
+
+Tolerances are BASELINE.json north_star's: quiet <= 1e-5 of the integrated continuum, deltas <= 1e-4 of
+max|delta|, per-line first-moment RV within 1 cm/s; integer outputs (bins, visible cells, active-cell
+counts) bit-exact.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from helpers import DELTA_TOL, QUIET_TOL, RV_TOL_CMS, check_delta, check_quiet, max_rv_diff
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def soap():
+    import paper_2301_04259_b200 as soap_mod
+    soap_mod.binding.load_library()
+    return soap_mod
+
+
+def run_gpu(soap, wl, form=None, splits=None, want_n_active=True):
+    dev = torch.device("cuda:0")
+    star = soap.soap_create(0)
+    if form is not None:
+        soap.soap_set_option(star, soap.binding.SOAP_OPT_FORM, form)
+    if splits is not None:
+        soap.soap_set_option(star, soap.binding.SOAP_OPT_QUIET_SPLITS, splits)
+    info = soap.soap_disk_geometry(star, wl)
+    q = soap.to_device_spectra(wl.quiet, wl.lambda0, wl.dlambda, dev)
+    s = None if wl.spot is None else soap.to_device_spectra(wl.spot, wl.lambda0, wl.dlambda, dev, wl.spot_contrast, wl.spot_lb)
+    f = None if wl.facula is None else soap.to_device_spectra(wl.facula, wl.lambda0, wl.dlambda, dev, wl.facula_contrast, wl.facula_lb)
+    tdt = torch.float32 if wl.dtype == np.float32 else torch.float64
+    Q = torch.full((wl.n_pix,), float("nan"), dtype=tdt, device=dev)
+    soap.soap_integrate_quiet(star, q, Q)
+    n_ph = len(wl.phases)
+    D = torch.full((n_ph, wl.n_pix), float("nan"), dtype=tdt, device=dev)
+    na = soap.soap_active_timeseries(star, q, s, f, wl.regions, wl.phases, D, want_n_active=want_n_active)
+    torch.cuda.synchronize()
+    stats = soap.soap_get_stats(star)
+    geo = soap.soap_export_geometry(star, wl.grid_n)
+    soap.soap_destroy(star)
+    return dict(Q=Q.cpu().numpy(), D=D.cpu().numpy(), n_active=na, info=info, stats=stats, geo=geo)
+
+
+def assert_parity(wl, g, m_lo=0, m_hi=None, check_rv=True):
+    Qo, Do, nao = oracle.run_workload(wl, m_lo, m_hi)
+    sw = oracle.geometry(wl)["sum_w"]
+    sl = slice(m_lo, m_hi)
+    eq = check_quiet(g["Q"][sl], Qo, sw)
+    assert eq <= QUIET_TOL, f"quiet: {eq:.3e} of continuum"
+    ed = check_delta(g["D"][:, sl], Do)
+    assert ed <= DELTA_TOL, f"delta: {ed:.3e} of max|delta|"
+    assert np.array_equal(g["n_active"], nao)
+    for p in range(len(wl.phases)):
+        if nao[p] == 0:
+            assert np.all(g["D"][p] == 0.0), "empty phase must be exact zeros"
+    if check_rv and len(wl.line_centres):
+        rvq, n_lines = max_rv_diff(g["Q"][sl].astype(np.float64), Qo, sw, wl, m_lo)
+        assert rvq <= RV_TOL_CMS, f"quiet line RV differs by {rvq:.3f} cm/s over {n_lines} lines"
+        F_gpu = g["Q"][sl].astype(np.float64)[None, :] + g["D"][:, sl].astype(np.float64)
+        rvd, _ = max_rv_diff(F_gpu, Qo[None, :] + Do, sw, wl, m_lo)
+        assert rvd <= RV_TOL_CMS, f"Q+delta line RV differs by {rvd:.3f} cm/s"
+    return eq, ed
+
+
+def test_geometry_matches_oracle_exactly(soap):
+    wl = workloads.make_config2(n_pix=2000, n_phases=2)
+    g = run_gpu(soap, wl)
+    og = oracle.geometry(wl)
+    assert g["info"]["n_visible"] == og["n_visible"] == 70688
+    assert np.array_equal(g["geo"]["bin"], og["bin"])
+    np.testing.assert_array_equal(g["geo"]["mu"], og["mu"])
+    np.testing.assert_array_equal(g["geo"]["w"], og["w"])
+    np.testing.assert_array_equal(g["geo"]["vel"], og["vel"])
+    assert abs(g["info"]["sum_weights"] / og["sum_w"] - 1) < 1e-13
+    assert g["info"]["n_entries"] == len({(c // 300, b) for c, b in enumerate(og["bin"]) if b >= 0}) == 4554
+
+
+def test_config1_fp64(soap):
+    wl = workloads.make_config1()
+    g = run_gpu(soap, wl)
+    Qo, Do, nao = oracle.run_workload(wl)
+    sw = oracle.geometry(wl)["sum_w"]
+    # fp64 end to end: only the ~5e-12 px difference between the oracle's direct source coordinate and the
+    # kernel's shift form (pin P10) is left
+    assert check_quiet(g["Q"], Qo, sw) <= 1e-10
+    assert check_delta(g["D"], Do) <= 1e-9
+    assert np.array_equal(g["n_active"], nao) and nao.max() > 0
+    assert_parity(wl, g)
+
+
+def test_config1_paper_phases(soap):
+    """BASELINE.json's literal '4 phases evenly over one rotation' {0, 1/4, 1/2, 3/4}: only 1/2 is active."""
+    wl = workloads.make_config1(phases=np.array([0.0, 0.25, 0.5, 0.75]))
+    g = run_gpu(soap, wl)
+    assert list(g["n_active"]) == [0, 0, 16, 0]
+    assert_parity(wl, g)
+
+
+def test_config2_full(soap):
+    wl = workloads.make_config2()
+    g = run_gpu(soap, wl)
+    assert g["n_active"].max() == 668 and int(g["n_active"].sum()) == 21178
+    assert_parity(wl, g)
+
+
+@pytest.mark.parametrize("form", [1, 2])
+def test_forms_agree_with_oracle(soap, form):
+    """Pre-binned (column, mu-bin) entries and the literal one-entry-per-cell form."""
+    wl = workloads.make_config2(n_pix=3000, n_phases=8, grid_n=120)
+    wl.phases = np.linspace(0.3, 0.7, 8)
+    g = run_gpu(soap, wl, form=form)
+    assert g["stats"]["form"] == form
+    assert_parity(wl, g)
+
+
+@pytest.mark.parametrize("n_pix", [2, 3, 5, 127, 1023, 1024, 1025, 4099])
+def test_ragged_sizes(soap, n_pix):
+    wl = workloads.make_config2(n_pix=max(n_pix, 400), n_phases=3, grid_n=40)
+    # cut the arrays down to n_pix (keeps line structure near the start)
+    wl.n_pix = n_pix
+    wl.quiet = np.ascontiguousarray(wl.quiet[:, :n_pix])
+    wl.spot = np.ascontiguousarray(wl.spot[:, :n_pix])
+    wl.spot_contrast = np.ascontiguousarray(wl.spot_contrast[:n_pix])
+    wl.phases = np.array([0.45, 0.5, 0.0])
+    wl.vsini_kms = 25.0
+    g = run_gpu(soap, wl)
+    assert_parity(wl, g, check_rv=False)
+
+
+def test_fast_rotator_large_halo_and_inclination(soap):
+    wl = workloads.make_config5_star(3, n_pix=6000, n_phases=6, grid_n=90)
+    wl.vsini_kms = 20.0
+    wl.incl_deg = 35.0
+    wl.regions = [(20.0, 170.0, 0.25, 2), (25.0, 175.0, 0.1, 1), (-30.0, 30.0, 0.15, 1)]
+    wl.phases = np.linspace(0.0, 1.0, 6, endpoint=False)
+    g = run_gpu(soap, wl)
+    assert_parity(wl, g)
+
+
+def test_first_order_doppler_mode(soap):
+    wl = workloads.make_config2(n_pix=3000, n_phases=2, grid_n=60)
+    wl.vsini_kms = 20.0
+    wl.doppler_mode = 1
+    wl.phases = np.array([0.5, 0.55])
+    g = run_gpu(soap, wl)
+    assert_parity(wl, g)
+
+
+def test_nonuniform_mu_centres_and_facula_contrast(soap):
+    wl = workloads.make_config3(n_pix=2500, n_phases=4, grid_n=80, nested=True)
+    wl.mu_centres = np.array([0.1, 0.3, 0.35, 0.6, 0.9, 1.0])
+    wl.quiet, wl.spot, wl.facula = (np.ascontiguousarray(a[:6]) for a in (wl.quiet, wl.spot, wl.facula))
+    wl.facula_contrast = (1.0 + 0.05 * np.sin(np.arange(wl.n_pix) / 50.0)).astype(np.float32)
+    wl.phases = np.array([0.4, 0.5, 0.6, 0.9])
+    g = run_gpu(soap, wl)
+    assert_parity(wl, g)
+
+
+def test_splits_do_not_change_parity_and_runs_are_deterministic(soap):
+    wl = workloads.make_config2(n_pix=5000, n_phases=4, grid_n=100)
+    wl.phases = np.array([0.4, 0.5, 0.6, 0.0])
+    a = run_gpu(soap, wl, splits=1)
+    b = run_gpu(soap, wl, splits=7)
+    c = run_gpu(soap, wl, splits=7)
+    assert_parity(wl, a)
+    assert_parity(wl, b)
+    assert np.array_equal(b["Q"], c["Q"]) and np.array_equal(b["D"], c["D"])
+
+
+def test_overlap_override_and_duplicates(soap):
+    wl = workloads.make_config3(n_pix=2000, n_phases=3, grid_n=100, nested=True)
+    wl.phases = np.array([0.45, 0.5, 0.55])
+    g1 = run_gpu(soap, wl)
+    assert_parity(wl, g1)
+    wl2 = workloads.make_config3(n_pix=2000, n_phases=3, grid_n=100, nested=True)
+    wl2.phases = wl.phases
+    wl2.regions = [wl.regions[0], wl.regions[0], wl.regions[1], wl.regions[1]]
+    g2 = run_gpu(soap, wl2)
+    assert np.array_equal(g1["D"], g2["D"]) and np.array_equal(g1["n_active"], g2["n_active"])
+
+
+def test_no_regions_and_zero_rotation(soap):
+    wl = workloads.make_config2(n_pix=1500, n_phases=2, grid_n=50)
+    wl.regions = []
+    wl.vsini_kms = 0.0
+    g = run_gpu(soap, wl)
+    assert np.all(g["D"] == 0.0) and np.all(g["n_active"] == 0)
+    assert_parity(wl, g)
+
+
+# ---- BASELINE.json full sizes, in the launch configuration bench.py times: sampled pixel ranges ----
+def _sample_ranges(n_pix, width=768, n=6):
+    rng = np.random.default_rng(123)
+    starts = [0, n_pix - width] + [int(v) for v in rng.integers(2048, n_pix - width - 2048, n)]
+    # make two of them straddle a tile boundary (tiles are 1024 px wide in fp32)
+    starts[2] = 1024 * (starts[2] // 1024) - width // 2
+    starts[3] = 1024 * (starts[3] // 1024) - 3
+    return [(s, s + width) for s in starts]
+
+
+def test_config3_full_size_sampled(soap):
+    wl = workloads.make_config3()
+    g = run_gpu(soap, wl)
+    assert g["info"]["n_visible"] == 70688
+    assert g["n_active"].max() == 1920 and int(g["n_active"].sum()) == 20650
+    for lo, hi in _sample_ranges(wl.n_pix):
+        assert_parity(wl, g, lo, hi)
+
+
+def test_config3_nested_variant_sampled(soap):
+    wl = workloads.make_config3(nested=True)
+    g = run_gpu(soap, wl)
+    assert g["n_active"].max() == 1825 and int(g["n_active"].sum()) == 14694
+    for lo, hi in _sample_ranges(wl.n_pix, n=3):
+        assert_parity(wl, g, lo, hi)
+
+
+def test_config4_full_size_sampled(soap):
+    wl = workloads.make_config4()
+    g = run_gpu(soap, wl)
+    assert g["info"]["n_visible"] == 125676
+    for lo, hi in _sample_ranges(wl.n_pix, width=512, n=2):
+        assert_parity(wl, g, lo, hi)
+
+
+def test_config5_batch_sampled(soap):
+    """64 stars through the batch entry points; 3 stars x 2 ranges are checked against the oracle."""
+    dev = torch.device("cuda:0")
+    n_stars, n_pix, n_ph = 64, 200_000, 50
+    shared = workloads.make_config5_star(0, n_pix=n_pix, n_phases=n_ph)
+    wls = [shared] + [workloads.make_config5_star(k, n_pix=n_pix, n_phases=n_ph, shared=shared) for k in range(1, n_stars)]
+    q = soap.to_device_spectra(shared.quiet, shared.lambda0, shared.dlambda, dev)
+    s = soap.to_device_spectra(shared.spot, shared.lambda0, shared.dlambda, dev, shared.spot_contrast, shared.spot_lb)
+    f = soap.to_device_spectra(shared.facula, shared.lambda0, shared.dlambda, dev, shared.facula_contrast, shared.facula_lb)
+    stars = [soap.soap_create(0) for _ in range(n_stars)]
+    for st, wl in zip(stars, wls):
+        soap.soap_disk_geometry(st, wl, want_info=False)
+    Q = torch.empty((n_stars, n_pix), dtype=torch.float32, device=dev)
+    D = torch.empty((n_stars, n_ph, n_pix), dtype=torch.float32, device=dev)
+    soap.soap_batch_integrate_quiet(stars, [q] * n_stars, [Q[k] for k in range(n_stars)])
+    soap.soap_batch_active_timeseries(stars, [q] * n_stars, [s] * n_stars, [f] * n_stars, [w.regions for w in wls],
+                                      [w.phases for w in wls], [D[k] for k in range(n_stars)])
+    torch.cuda.synchronize()
+    fastest = int(np.argmax([w.vsini_kms for w in wls]))
+    for k in sorted({0, fastest, 63}):
+        g = dict(Q=Q[k].cpu().numpy(), D=D[k].cpu().numpy(), n_active=None)
+        wl = wls[k]
+        for lo, hi in [(0, 512), (123_456, 123_456 + 512)]:
+            Qo, Do, nao = oracle.run_workload(wl, lo, hi)
+            sw = oracle.geometry(wl)["sum_w"]
+            assert check_quiet(g["Q"][lo:hi], Qo, sw) <= QUIET_TOL
+            if np.abs(Do).max() > 0:
+                assert check_delta(g["D"][:, lo:hi], Do) <= DELTA_TOL
+            else:
+                assert np.all(g["D"][:, lo:hi] == 0.0)
+            rv, _ = max_rv_diff(g["Q"][lo:hi].astype(np.float64), Qo, sw, wl, lo)
+            assert rv <= RV_TOL_CMS
+    for st in stars:
+        soap.soap_destroy(st)
+
+
+def test_host_buffer_entry_point(soap):
+    wl = workloads.make_config2(n_pix=4000, n_phases=5, grid_n=80)
+    wl.phases = np.linspace(0.35, 0.65, 5)
+    star = soap.soap_create(0)
+    pitch = (wl.n_pix + 3) & ~3
+
+    def host(rows):
+        t = torch.zeros((rows.shape[0], pitch), dtype=torch.float32).pin_memory()
+        t[:, :wl.n_pix] = torch.from_numpy(rows)
+        return t
+
+    q = soap.Spectra(host(wl.quiet), wl.n_pix, wl.lambda0, wl.dlambda)
+    s = soap.Spectra(host(wl.spot), wl.n_pix, wl.lambda0, wl.dlambda,
+                     contrast=torch.from_numpy(wl.spot_contrast).pin_memory(), lb=wl.spot_lb)
+    Q = torch.empty(wl.n_pix, dtype=torch.float32).pin_memory()
+    D = torch.empty((len(wl.phases), wl.n_pix), dtype=torch.float32).pin_memory()
+    na = soap.soap_synthesize_host(star, wl, q, s, None, wl.regions, wl.phases, Q, D, want_n_active=True)
+    soap.soap_destroy(star)
+    assert_parity(wl, dict(Q=Q.numpy(), D=D.numpy(), n_active=na))
+
+
+def test_argument_errors_leave_outputs_untouched(soap):
+    b = soap.binding
+    wl = workloads.make_config2(n_pix=1000, n_phases=2, grid_n=30)
+    dev = torch.device("cuda:0")
+    star = soap.soap_create(0)
+    q = soap.to_device_spectra(wl.quiet, wl.lambda0, wl.dlambda, dev)
+    out = torch.full((wl.n_pix,), -7.0, dtype=torch.float32, device=dev)
+    with pytest.raises(soap.SoapError) as e:
+        soap.soap_integrate_quiet(star, q, out)
+    assert e.value.code == b.SOAP_ERR_NOT_READY
+    soap.soap_disk_geometry(star, wl)
+    bad = soap.Spectra(q.data, q.n_pix, -1.0, q.dlambda)
+    with pytest.raises(soap.SoapError) as e:
+        soap.soap_integrate_quiet(star, bad, out)
+    assert e.value.code == b.SOAP_ERR_INVALID_ARG
+    D = torch.full((2, wl.n_pix), -7.0, dtype=torch.float32, device=dev)
+    with pytest.raises(soap.SoapError) as e:  # a spot region without spot spectra
+        soap.soap_active_timeseries(star, q, None, None, [(0.0, 180.0, 0.1, 1)], wl.phases, D)
+    assert e.value.code == b.SOAP_ERR_INVALID_ARG
+    with pytest.raises(soap.SoapError):
+        soap.soap_active_timeseries(star, q, q, None, [(0.0, 180.0, 1.5, 1)], wl.phases, D)
+    torch.cuda.synchronize()
+    assert torch.all(out == -7.0) and torch.all(D == -7.0)
+    soap.soap_destroy(star)
