@@ -16,6 +16,7 @@
 #include "active.cuh"
 #include "geometry.cuh"
 #include "sia.cuh"
+#include "sia_f32.cuh"
 
 namespace {
 
@@ -188,8 +189,67 @@ int launch_sia(soap_star *s, const SiaParams<T> &p, dim3 grid, cudaStream_t st) 
     return SOAP_OK;
 }
 
+// fp32 spectra: warp-specialised kernel of sia_f32.cuh.  `which`: 0 = quiet, 1 = active (event slots).
+template <bool ACTIVE>
+int launch_sia_f32(soap_star *s, const f32::Params &p, dim3 grid, cudaStream_t st) {
+    const size_t smem = f32::smem_bytes(p.halo, ACTIVE);
+    if (smem > 227 * 1024) return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", p.halo, smem);
+    SOAP_CUDA(s, cudaFuncSetAttribute(f32::sia_f32_kernel<ACTIVE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int e0 = ACTIVE ? 2 : 0;
+    if (s->opt_timing) {
+        for (int k = e0; k < e0 + 2; ++k)
+            if (!s->ev[k]) SOAP_CUDA(s, cudaEventCreate(&s->ev[k]));
+        SOAP_CUDA(s, cudaEventRecord(s->ev[e0], st));
+    }
+    f32::sia_f32_kernel<ACTIVE><<<grid, f32::kThreads, smem, st>>>(p);
+    SOAP_LAUNCH_CHECK(s, ACTIVE ? "sia_f32_kernel<active>" : "sia_f32_kernel<quiet>");
+    if (s->opt_timing) {
+        SOAP_CUDA(s, cudaEventRecord(s->ev[e0 + 1], st));
+        s->ev_valid[ACTIVE ? 1 : 0] = true;
+    }
+    return SOAP_OK;
+}
+
+int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
+    const long long P = q->n_pix;
+    const int n_tiles = (int)((P + f32::kTile - 1) / f32::kTile);
+    f32::Params p{};
+    p.base[0] = static_cast<const float *>(q->data);
+    p.pitch = q->pitch;
+    p.n_pix = P;
+    p.c0 = q->lambda0 / q->dlambda;
+    p.n_mu = s->prm.n_mu;
+    p.halo = halo_for(s, q);
+    p.ent = s->d_ent32.ptr;
+    p.row_start = s->d_row_start.ptr;
+    p.n_tiles = n_tiles;
+    // one CTA per resident slot (a single wave); fewer when there is too little work to share out
+    const size_t smem = f32::smem_bytes(p.halo, false);
+    if (smem > 227 * 1024) return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", p.halo, smem);
+    SOAP_CUDA(s, cudaFuncSetAttribute(f32::sia_f32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    SOAP_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f32::sia_f32_kernel<false>, f32::kThreads, smem));
+    if (occ < 1) return s->fail(SOAP_ERR_UNSUPPORTED, "quiet kernel does not fit on an SM (halo %d)", p.halo);
+    long long G = s->opt_quiet_splits > 0 ? (long long)s->opt_quiet_splits : (long long)s->n_sm * occ;
+    const long long max_entries = (long long)s->prm.grid_n * (s->form_used == SOAP_FORM_CELLS ? s->prm.grid_n : s->prm.n_mu);
+    G = std::max(1LL, std::min(G, (long long)n_tiles * max_entries / 64));
+    p.max_seg = (int)(n_tiles / G) + 3;
+    SOAP_CUDA(s, s->d_partial.reserve((size_t)G * p.max_seg * f32::kTile));
+    p.partial = s->d_partial.ptr;
+    int rc = launch_sia_f32<false>(s, p, dim3((unsigned)G), st);
+    if (rc) return rc;
+    const int threads = 256;
+    f32::reduce_ranges_kernel<<<(unsigned)((P + threads - 1) / threads), threads, 0, st>>>(
+        s->d_partial.ptr, p.max_seg, s->d_row_start.ptr, p.n_mu, (int)G, n_tiles, P, static_cast<float *>(out));
+    SOAP_LAUNCH_CHECK(s, "reduce_ranges_kernel");
+    s->last_quiet_splits = (int)G;
+    s->last_tile_px = f32::kTile;
+    return SOAP_OK;
+}
+
 template <typename T>
 int quiet_impl(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
+    if (sizeof(T) == 4) return quiet_f32(s, q, out, st);
     constexpr int TP = sia_tile_px<T>();
     const long long P = q->n_pix;
     const int n_tiles = (int)((P + TP - 1) / TP);
@@ -261,6 +321,27 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
             N, n_mu, ncap, (int)n_seg, s->d_col_a.ptr, s->d_WD.ptr, reinterpret_cast<Ent *>(s->d_aent.ptr),
             s->d_segcnt.ptr, &s->d_counters.ptr->active_entries);
         SOAP_LAUNCH_CHECK(s, "active_compact_kernel");
+    }
+    if (sizeof(T) == 4) {
+        f32::Params p{};
+        p.base[0] = static_cast<const float *>(q->data);
+        p.base[1] = spot ? static_cast<const float *>(spot->data) : p.base[0];
+        p.base[2] = fac ? static_cast<const float *>(fac->data) : p.base[0];
+        p.contrast[1] = spot ? static_cast<const float *>(spot->contrast) : nullptr;
+        p.contrast[2] = fac ? static_cast<const float *>(fac->contrast) : nullptr;
+        p.pitch = q->pitch;
+        p.n_pix = q->n_pix;
+        p.c0 = q->lambda0 / q->dlambda;
+        p.n_mu = n_mu;
+        p.halo = halo_for(s, q);
+        p.ent = reinterpret_cast<const float2 *>(s->d_aent.ptr);
+        p.seg_count = s->d_segcnt.ptr;
+        p.seg_cap = ncap;
+        p.out = static_cast<float *>(out);
+        p.out_pitch = out_pitch;
+        const int n_tiles = (int)((q->n_pix + f32::kTile - 1) / f32::kTile);
+        s->last_tile_px = f32::kTile;
+        return launch_sia_f32<true>(s, p, dim3(n_tiles, n_phases), st);
     }
     SiaParams<T> p{};
     p.base[0] = static_cast<const T *>(q->data);
