@@ -26,7 +26,7 @@ if ROOT not in sys.path:
 
 METRIC = "integrated spectra/s and cell*pixel interps/s (full visible, 300^2 grid), % roofline"
 N_SM, FP32_LANES_PER_SM = 148, 128
-FLOPS_PER_UNIT = 6  # one lerp-accumulate = 3 FP32 FMAs (t_r, W*s_r, (W t_r)*d_r) = 6 FLOP
+FLOPS_PER_UNIT = 4  # one lerp-accumulate = 2 FP32 FMAs per (entry, pixel): acc += W u_r; acc += (W a) v_r
 # dram bytes per launch of the dominant kernel from the committed ncu --set full capture
 # (profiles/r01_sia_full_summary.md); None until a capture exists for the current kernel.
 NCU_DRAM_TRAFFIC_BYTES = {"sia_kernel<quiet>": None, "sia_kernel<active>": None}

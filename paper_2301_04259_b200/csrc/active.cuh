@@ -26,13 +26,17 @@ struct LbCoef {
     double c[3][3];  // [kind][power]; kind 0 unused
 };
 
-// grid: (ceil(N/128), n_phases).  WD: [n_phases][3][n_mu][ncap] fp64, pre-zeroed.
-__global__ void active_bin_kernel(int N, int n_regions, int n_mu, int ncap,
-                                  const RegionAtPhase *__restrict__ rp /*[n_phases][n_regions]*/,
-                                  const double *__restrict__ mu, const double *__restrict__ w,
-                                  const int *__restrict__ bin, LbCoef lb, double *__restrict__ WD,
-                                  int *__restrict__ n_active /*[n_phases]*/) {
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+constexpr int kBinWarps = 8;  // warps (columns) per CTA of active_bin_kernel
+
+// grid: (ceil(N/kBinWarps), n_phases); one warp per (phase, column), lanes over the rows (coalesced).
+// WD: [n_phases][3][n_mu][ncap] fp64, pre-zeroed.  Cells of equal (mu-bin, type) are contiguous in a
+// column: segmented warp scans, added to WD in row order by one lane at a time (deterministic).
+__global__ void __launch_bounds__(32 * kBinWarps)
+active_bin_kernel(int N, int n_regions, int n_mu, int ncap, const RegionAtPhase *__restrict__ rp /*[n_phases][n_regions]*/,
+                  const double *__restrict__ mu, const double *__restrict__ w, const int *__restrict__ bin, LbCoef lb,
+                  double *__restrict__ WD, int *__restrict__ n_active /*[n_phases]*/) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int j = blockIdx.x * kBinWarps + warp;
     const int p = blockIdx.y;
     if (j >= N) return;
     const RegionAtPhase *reg = rp + (size_t)p * n_regions;
@@ -52,44 +56,46 @@ __global__ void active_bin_kernel(int N, int n_regions, int n_mu, int ncap,
     i_lo = max(i_lo, 0);
     i_hi = min(i_hi, N - 1);
     double *WDp = WD + (size_t)p * 3 * n_mu * ncap;
-    int cur_b = -1, cur_t = 0, count = 0;
-    double run_w = 0.0, run_wlb = 0.0;
-    for (int i = i_lo; i <= i_hi; ++i) {
-        const size_t c = (size_t)j * N + i;
-        const int b = bin[c];
-        int t = 0;
-        if (b >= 0) {
-            const double y = cell_coord(i, N), m = mu[c];
-            for (int r = 0; r < n_regions; ++r) {  // list order: the last covering region wins
-                if (reg[r].type == 0) continue;
-                const double dot =
-                    __dadd_rn(__dadd_rn(__dmul_rn(x, reg[r].xr), __dmul_rn(y, reg[r].yr)), __dmul_rn(m, reg[r].zr));
-                if (dot >= reg[r].cos_alpha) t = reg[r].type;
+    int count = 0;
+    for (int i0 = i_lo; i0 <= i_hi; i0 += 32) {
+        const int i = i0 + lane;
+        int b = -1, t = 0;
+        double wc = 0.0, wl = 0.0;
+        if (i <= i_hi) {
+            const size_t c = (size_t)j * N + i;
+            b = bin[c];
+            if (b >= 0) {
+                const double y = cell_coord(i, N), m = mu[c];
+                for (int r = 0; r < n_regions; ++r) {  // list order: the last covering region wins
+                    if (reg[r].type == 0) continue;
+                    const double dot =
+                        __dadd_rn(__dadd_rn(__dmul_rn(x, reg[r].xr), __dmul_rn(y, reg[r].yr)), __dmul_rn(m, reg[r].zr));
+                    if (dot >= reg[r].cos_alpha) t = reg[r].type;
+                }
+                if (t != 0) {
+                    wc = w[c];
+                    wl = wc * (lb.c[t][0] + lb.c[t][1] * m + lb.c[t][2] * m * m);
+                }
             }
         }
-        if (t != cur_t || b != cur_b) {
-            if (cur_t != 0) {
-                WDp[((size_t)0 * n_mu + cur_b) * ncap + j] += run_w;
-                WDp[((size_t)cur_t * n_mu + cur_b) * ncap + j] += run_wlb;
+        const int key = (t != 0) ? (b * 4 + t) : -1;
+        int start;
+        bool tail;
+        const double seg_w = warp_segmented_scan(wc, key, lane, start, tail);
+        const double seg_wl = warp_segmented_scan(wl, key, lane, start, tail);
+        unsigned tails = __ballot_sync(0xffffffffu, tail && t != 0);
+        while (tails) {
+            const int l = __ffs(tails) - 1;
+            if (lane == l) {
+                WDp[((size_t)0 * n_mu + b) * ncap + j] += seg_w;
+                WDp[((size_t)t * n_mu + b) * ncap + j] += seg_wl;
             }
-            cur_t = t;
-            cur_b = b;
-            run_w = 0.0;
-            run_wlb = 0.0;
+            __syncwarp();
+            tails &= tails - 1;
         }
-        if (t != 0) {
-            const double m = mu[c], wc = w[c];
-            const double l = lb.c[t][0] + lb.c[t][1] * m + lb.c[t][2] * m * m;
-            run_w += wc;
-            run_wlb += wc * l;
-            ++count;
-        }
+        count += __popc(__ballot_sync(0xffffffffu, t != 0));
     }
-    if (cur_t != 0) {
-        WDp[((size_t)0 * n_mu + cur_b) * ncap + j] += run_w;
-        WDp[((size_t)cur_t * n_mu + cur_b) * ncap + j] += run_wlb;
-    }
-    if (count) atomicAdd(&n_active[p], count);  // integer: order-independent
+    if (lane == 0 && count) atomicAdd(&n_active[p], count);  // integer: order-independent
 }
 
 // One warp per (phase, kind, mu-bin) segment: ordered compaction of the non-zero columns into

@@ -23,18 +23,16 @@ __device__ __forceinline__ double cell_coord(int idx, int N) {
     return __dadd_rn(-1.0, __ddiv_rn(__dadd_rn(__dmul_rn(2.0, (double)idx), 1.0), (double)N));
 }
 
-// One thread per cell c = j*N + i: mu, limb-darkening weight, velocity and nearest mu bin.
-__global__ void geometry_cells_kernel(int N, double vsini_sini, double u1, double u2, int n_mu,
-                                      const double *__restrict__ mu_centres, double *__restrict__ mu_out,
-                                      double *__restrict__ w_out, double *__restrict__ vel_out,
-                                      int *__restrict__ bin_out) {
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= N * N) return;
-    const int j = c / N, i = c - j * N;
+// One cell c = j*N + i: mu, limb-darkening weight, velocity and nearest mu bin (hidden: 0, 0, 0, -1).
+__device__ __forceinline__ void cell_geometry(int j, int i, int N, double vsini_sini, double u1, double u2, int n_mu,
+                                              const double *__restrict__ mu_centres, double &mu, double &w, double &v,
+                                              int &bin) {
     const double x = cell_coord(j, N), y = cell_coord(i, N);
     const double r2 = __dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y));
-    double mu = 0.0, w = 0.0, v = 0.0;
-    int bin = -1;
+    mu = 0.0;
+    w = 0.0;
+    v = 0.0;
+    bin = -1;
     if (r2 <= 1.0) {  // cell counts iff its centre is on the disk (reading S2)
         const double a = __dadd_rn(1.0, -r2);
         mu = __dsqrt_rn(a > 0.0 ? a : 0.0);
@@ -53,10 +51,6 @@ __global__ void geometry_cells_kernel(int N, double vsini_sini, double u1, doubl
             }
         }
     }
-    mu_out[c] = mu;
-    w_out[c] = w;
-    vel_out[c] = v;
-    bin_out[c] = bin;
 }
 
 // D - 1 without cancellation.  mode 0: D = sqrt((1-b)/(1+b))  =>  D - 1 = -2b / ((1+b) + sqrt(1-b^2));
@@ -67,37 +61,78 @@ __device__ __forceinline__ double doppler_minus_one(double v_kms, int mode) {
     return -2.0 * b / ((1.0 + b) + sqrt(1.0 - b * b));
 }
 
-// One thread per column j: the column's shift factor a_j = D_j - 1 (all cells of a column share one
-// velocity under solid-body rotation), its binned weights W[j][b] (serial fp64 sum in i order:
-// deterministic), and its visible-cell count / weight sum.
-__global__ void geometry_columns_kernel(int N, double vsini_sini, int mode, int n_mu,
-                                        const double *__restrict__ w, const int *__restrict__ bin,
-                                        double *__restrict__ col_a, double *__restrict__ Wbin /*[N][n_mu]*/,
-                                        double *__restrict__ col_sumw, int *__restrict__ col_nvis) {
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= N) return;
-    const double x = cell_coord(j, N);
-    col_a[j] = doppler_minus_one(__dmul_rn(x, vsini_sini), mode);
-    double *Wj = Wbin + (size_t)j * n_mu;
-    for (int b = 0; b < n_mu; ++b) Wj[b] = 0.0;
-    double sum = 0.0, run = 0.0;
-    int nvis = 0, cur = -1;
-    for (int i = 0; i < N; ++i) {
-        const int b = bin[(size_t)j * N + i];
-        if (b < 0) continue;
-        const double wc = w[(size_t)j * N + i];
-        if (b != cur) {
-            if (cur >= 0) Wj[cur] += run;
-            cur = b;
-            run = 0.0;
-        }
-        run += wc;
-        sum += wc;
-        ++nvis;
+// Inclusive segmented scan over the lanes of a warp: lanes with equal consecutive `key` form a segment;
+// returns the sum of v over the lanes of the caller's segment up to and including the caller.  Fixed
+// shuffle tree: deterministic.  `start` receives the first lane of the caller's segment.
+__device__ __forceinline__ double warp_segmented_scan(double v, int key, int lane, int &start, bool &is_tail) {
+    const int prev = __shfl_up_sync(0xffffffffu, key, 1);
+    const bool head = (lane == 0) || (key != prev);
+    const unsigned heads = __ballot_sync(0xffffffffu, head);
+    start = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
+    is_tail = (lane == 31) || ((heads >> (lane + 1)) & 1u);
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const double t = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane - d >= start) v += t;
     }
-    if (cur >= 0) Wj[cur] += run;
-    col_sumw[j] = sum;
-    col_nvis[j] = nvis;
+    return v;
+}
+
+constexpr int kGeomWarps = 8;  // warps (columns) per CTA of geometry_kernel
+
+// a1 + a2.  One warp per column j, lanes over the rows i (coalesced): every cell's (mu, w, v, bin), the
+// column's shift factor a_j = D_j - 1 (all cells of a column share one velocity under solid-body
+// rotation), its binned weights W[j][b] (segmented warp scans added in row order: deterministic), and
+// its visible-cell count / weight sum.
+__global__ void __launch_bounds__(32 * kGeomWarps)
+geometry_kernel(int N, double vsini_sini, double u1, double u2, int mode, int n_mu,
+                const double *__restrict__ mu_centres, double *__restrict__ mu_out, double *__restrict__ w_out,
+                double *__restrict__ vel_out, int *__restrict__ bin_out, double *__restrict__ col_a,
+                double *__restrict__ Wbin /*[N][n_mu]*/, double *__restrict__ col_sumw, int *__restrict__ col_nvis) {
+    __shared__ double s_W[kGeomWarps][64];
+    __shared__ double s_mu[64];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int b = threadIdx.x; b < n_mu; b += blockDim.x) s_mu[b] = mu_centres[b];
+    for (int b = lane; b < 64; b += 32) s_W[warp][b] = 0.0;
+    __syncthreads();
+    const int j = blockIdx.x * kGeomWarps + warp;
+    if (j >= N) return;
+    double sum = 0.0;
+    int nvis = 0;
+    for (int i0 = 0; i0 < N; i0 += 32) {
+        const int i = i0 + lane;
+        double mu = 0.0, w = 0.0, v = 0.0;
+        int bin = -1;
+        if (i < N) {
+            cell_geometry(j, i, N, vsini_sini, u1, u2, n_mu, s_mu, mu, w, v, bin);
+            const size_t c = (size_t)j * N + i;
+            mu_out[c] = mu;
+            w_out[c] = w;
+            vel_out[c] = v;
+            bin_out[c] = bin;
+        }
+        int start;
+        bool tail;
+        const double seg = warp_segmented_scan(w, bin, lane, start, tail);
+        unsigned tails = __ballot_sync(0xffffffffu, tail && bin >= 0);
+        while (tails) {  // segments of one bin may repeat inside a chunk (apex of the column): add in lane order
+            const int l = __ffs(tails) - 1;
+            if (lane == l) s_W[warp][bin] += seg;
+            __syncwarp();
+            tails &= tails - 1;
+        }
+        double cs = w;  // chunk total, fixed xor tree
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) cs += __shfl_xor_sync(0xffffffffu, cs, d);
+        sum += cs;
+        nvis += __popc(__ballot_sync(0xffffffffu, bin >= 0));
+    }
+    for (int b = lane; b < n_mu; b += 32) Wbin[(size_t)j * n_mu + b] = s_W[warp][b];
+    if (lane == 0) {
+        col_a[j] = doppler_minus_one(__dmul_rn(cell_coord(j, N), vsini_sini), mode);
+        col_sumw[j] = sum;
+        col_nvis[j] = nvis;
+    }
 }
 
 // Single CTA: compacts the non-zero W[j][b] into the entry list of the pre-binned form, sorted by
@@ -112,6 +147,8 @@ __global__ void build_binned_entries_kernel(int N, int n_mu, const double *__res
                                             DevInfo *__restrict__ info) {
     __shared__ int s_cnt[64];
     __shared__ int s_start[65];
+    __shared__ int s_nv[1024];  // blockDim.x == 1024 (a power of two); N <= 8192 so N^2 fits an int
+    __shared__ double s_sw[1024], s_am[1024];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
     for (int b = warp; b < n_mu; b += n_warps) {
         int cnt = 0;
@@ -123,6 +160,29 @@ __global__ void build_binned_entries_kernel(int N, int n_mu, const double *__res
         if (lane == 0) s_cnt[b] = cnt;
     }
     __syncthreads();
+    // summary: per-thread strided partials, then a fixed shared-memory tree (deterministic)
+    {
+        long long nv = 0;
+        double sw = 0.0, am = 0.0;
+        for (int j = threadIdx.x; j < N; j += blockDim.x) {
+            const int c = col_nvis[j];
+            nv += c;
+            sw += col_sumw[j];
+            if (c > 0) am = fmax(am, fabs(col_a[j]));
+        }
+        s_nv[threadIdx.x] = (int)nv;
+        s_sw[threadIdx.x] = sw;
+        s_am[threadIdx.x] = am;
+    }
+    __syncthreads();
+    for (int d = blockDim.x >> 1; d > 0; d >>= 1) {
+        if (threadIdx.x < d) {
+            s_nv[threadIdx.x] += s_nv[threadIdx.x + d];
+            s_sw[threadIdx.x] += s_sw[threadIdx.x + d];
+            s_am[threadIdx.x] = fmax(s_am[threadIdx.x], s_am[threadIdx.x + d]);
+        }
+        __syncthreads();
+    }
     if (threadIdx.x == 0) {
         int off = 0, total = 0;
         for (int b = 0; b < n_mu; ++b) {
@@ -131,17 +191,10 @@ __global__ void build_binned_entries_kernel(int N, int n_mu, const double *__res
             off += (s_cnt[b] + 1) & ~1;
         }
         s_start[n_mu] = off;
-        long long nvis = 0;
-        double sw = 0.0, amax = 0.0;
-        for (int j = 0; j < N; ++j) {
-            nvis += col_nvis[j];
-            sw += col_sumw[j];
-            if (col_nvis[j] > 0) amax = fmax(amax, fabs(col_a[j]));
-        }
-        info->n_visible = nvis;
+        info->n_visible = s_nv[0];
         info->n_entries = total;
-        info->sum_weights = sw;
-        info->max_abs_dshift = amax;
+        info->sum_weights = s_sw[0];
+        info->max_abs_dshift = s_am[0];
     }
     __syncthreads();
     for (int b = threadIdx.x; b <= n_mu; b += blockDim.x) row_start[b] = s_start[b];

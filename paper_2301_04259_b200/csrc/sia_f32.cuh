@@ -16,14 +16,18 @@
 //   * "jobs" = (spectrum row, <= 128 entries).  The producer warp keeps a ring of kStages jobs in flight:
 //     lane 0 issues two 1-D TMA bulk copies per job (the span of the row the tile's shifts can reach, and
 //     the job's raw entries), then the whole warp turns the raw entries into what the consumers need:
-//       - record {W a, W q, W, 128 W a} per entry, so that a consumer forms W t for its first pixel with ONE
+//       - record {W a, -W q, W, 128 W a} per entry, so that a consumer forms W t for its first pixel with ONE
 //         FMA (W a (lambda0/k + m) - W q) and for pixel r with one more (+ 128 W a r): no floor, no test;
 //       - a run table: maximal groups of consecutive entries whose integer shift q is the same for every
 //         pixel of the tile.  Consumers load their 16 samples and 16 sample differences once per run.
 //       - entries whose q changes inside the tile ("flips", ~1 %) become runs of their own and take a
 //         per-pixel path.  The producer also writes the clamp-to-edge halo (reading S8) of end tiles.
 //     Full/empty mbarriers per stage; consumers never meet a CTA-wide barrier.
-//   * per (entry, thread): 1 LDS.128 (broadcast) + 1 FFMA + 48 FFMA for 16 pixels.
+//   * per (entry, thread): 1 LDS.128 (broadcast) + 1 FFMA + 24 packed FFMA2 (fma.rn.f32x2: two pixels per
+//     issue slot, so the FP32 pipe and not instruction issue is the limit) for 16 pixels.  Measured on
+//     B200: FFMA2 runs at the full lane rate (126 of 128 lane-FMA/clk/SM) only with one scalar-broadcast
+//     operand; with three register-pair operands it drops to ~70.  Hence W t_r d_r is split as
+//     (W t_0) d_r + (128 W a) (r d_r) with r d_r kept in registers per run.
 //   * precision: only the shift delta (|delta| < ~50) is formed in fp32, never the absolute source
 //     coordinate; fp32 partial sums are folded into fp64 every kFold entries.
 //   * quiet launch: the flattened (tile, entry) work list is cut into equal contiguous ranges, one per
@@ -87,7 +91,7 @@ __host__ __device__ inline StageLayout stage_layout(int halo) {
     l.row_bytes = ((size_t)span_px(halo) * sizeof(float) + 127) & ~(size_t)127;
     l.raw_off = l.row_bytes;
     l.rec_off = l.raw_off + kJobCap * sizeof(float2);
-    l.run_off = l.rec_off + kJobCap * sizeof(float4);
+    l.run_off = l.rec_off + kJobCap * sizeof(float2);
     l.stage_bytes = (l.run_off + (kJobCap + 2) * sizeof(int2) + 127) & ~(size_t)127;
     return l;
 }
@@ -247,7 +251,7 @@ __global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
                 unsigned char *sb = stage0 + (size_t)st * L.stage_bytes;
                 float *rs = reinterpret_cast<float *>(sb);
                 const float2 *raw = reinterpret_cast<const float2 *>(sb + L.raw_off);
-                float4 *rec = reinterpret_cast<float4 *>(sb + L.rec_off);
+                float2 *rec = reinterpret_cast<float2 *>(sb + L.rec_off);
                 int2 *runs = reinterpret_cast<int2 *>(sb + L.run_off);
                 const long long m_t0 = jp.tile * kTile;
                 const float c_first = (float)(p.c0 + (double)m_t0);
@@ -262,8 +266,7 @@ __global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
                         const float qf = floorf(en.x * c_first), ql = floorf(en.x * c_last);
                         int qi = (int)qf;
                         qi = max(-H, min(H + 2, qi));
-                        const float Wa = en.y * en.x;
-                        rec[i] = make_float4(Wa, en.y * (float)qi, en.y, Wa * (float)kConsumers);
+                        rec[i] = make_float2(en.y, en.y * en.x);  // {W, W a}
                         if (qf == ql) code = qi;
                     }
                     int prev = __shfl_up_sync(0xffffffffu, code, 1);
@@ -312,20 +315,22 @@ __global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
     for (long long tile = t_first; tile <= t_last; ++tile) {
         const long long m_t0 = tile * kTile;
         const float cmf = (float)(p.c0 + (double)(m_t0 + tid));  // lambda0/k + m of this thread's first pixel
-        float acc[kR];
+        float2 acc[kR / 2];  // pair k = pixels r = 2k, 2k + 1: the operands of one packed FMA
         double tot[kR];
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
-            acc[r] = 0.f;
+            if (r & 1) acc[r / 2].y = 0.f;
+            else acc[r / 2].x = 0.f;
             tot[r] = 0.0;
             if (ACTIVE) fin[r * kConsumers + tid] = 0.0;  // only this thread ever touches its 16 slots
         }
         int cnt = 0, cur_kind = 0;
         auto fold = [&]() {
 #pragma unroll
-            for (int r = 0; r < kR; ++r) {
-                tot[r] += (double)acc[r];
-                acc[r] = 0.f;
+            for (int k = 0; k < kR / 2; ++k) {
+                tot[2 * k] += (double)acc[k].x;
+                tot[2 * k + 1] += (double)acc[k].y;
+                acc[k] = make_float2(0.f, 0.f);
             }
             cnt = 0;
         };
@@ -346,7 +351,7 @@ __global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
             const unsigned char *sb = stage0 + (size_t)st * L.stage_bytes;
             const float *rs = reinterpret_cast<const float *>(sb);
             const float2 *raw = reinterpret_cast<const float2 *>(sb + L.raw_off);
-            const float4 *rec = reinterpret_cast<const float4 *>(sb + L.rec_off);
+            const float2 *rec = reinterpret_cast<const float2 *>(sb + L.rec_off);
             const int2 *runs = reinterpret_cast<const int2 *>(sb + L.run_off);
             if (ACTIVE) {
                 const int kind = job.seg / p.n_mu;
@@ -371,19 +376,27 @@ __global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
                         int qi = (int)q;
                         qi = max(-H, min(H + 2, qi));
                         const float s0 = rs[base0 + kConsumers * r + qi], s1 = rs[base0 + kConsumers * r + qi + 1];
-                        acc[r] = fmaf(en.y, fmaf(t, s1 - s0, s0), acc[r]);
+                        float &ar = (r & 1) ? acc[r / 2].y : acc[r / 2].x;
+                        ar = fmaf(en.y, fmaf(t, s1 - s0, s0), ar);
                     }
                     if (++cnt >= kFold) fold();
                     continue;
                 }
-                float s[kR], d[kR];
+                // With t = a c - q (c = lambda0/k + m, q the run's integer shift), W lerp = W (s + t d) regroups
+                // to W u + (W a) v with u = s - q d and v = c d: u_r, v_r are per-pixel registers of the run and
+                // every entry costs two FMAs per pixel, each with one scalar (broadcast) operand.
+                float2 u[kR / 2], v[kR / 2];
                 {
                     const float *wv = rs + base0 + run.y;
+                    const float2 nq = bcast2(-(float)run.y);
 #pragma unroll
-                    for (int r = 0; r < kR; ++r) {
-                        const float s0 = wv[kConsumers * r], s1 = wv[kConsumers * r + 1];
-                        s[r] = s0;
-                        d[r] = s1 - s0;
+                    for (int k = 0; k < kR / 2; ++k) {
+                        const float2 s0 = make_float2(wv[kConsumers * 2 * k], wv[kConsumers * (2 * k + 1)]);
+                        const float2 s1 = make_float2(wv[kConsumers * 2 * k + 1], wv[kConsumers * (2 * k + 1) + 1]);
+                        const float2 d = fma2(bcast2(-1.f), s0, s1);
+                        const float2 c = make_float2(cmf + (float)(kConsumers * 2 * k), cmf + (float)(kConsumers * (2 * k + 1)));
+                        u[k] = fma2(nq, d, s0);
+                        v[k] = fma2(c, d, bcast2(0.f));
                     }
                 }
                 int e = run.x;
@@ -391,14 +404,11 @@ __global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
                     const int n = min(nxt - e, kFold - cnt);
 #pragma unroll 2
                     for (int i = 0; i < n; ++i) {
-                        const float4 rc = rec[e + i];                // {W a, W q, W, 128 W a}
-                        const float wa = fmaf(rc.x, cmf, -rc.y);     // W t of pixel r = 0
+                        const float2 rc = rec[e + i];  // {W, W a}
 #pragma unroll
-                        for (int r = 0; r < kR; ++r) {
-                            const float wt = fmaf(rc.w, (float)r, wa);  // (1) W t_r
-                            acc[r] = fmaf(rc.z, s[r], acc[r]);          // (2) + W s_r
-                            acc[r] = fmaf(wt, d[r], acc[r]);            // (3) + W t_r d_r
-                        }
+                        for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.x), u[k], acc[k]);  // (1) + W u_r
+#pragma unroll
+                        for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.y), v[k], acc[k]);  // (2) + W a v_r
                     }
                     e += n;
                     cnt += n;
@@ -430,25 +440,52 @@ __global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
 }
 
 // a6 for the quiet spectrum: adds, in CTA order, the partials of every CTA whose range touched the
-// pixel's tile, and rounds once to fp32.
-__global__ void reduce_ranges_kernel(const double *__restrict__ partial, int max_seg, const int *__restrict__ row_start,
-                                     int n_mu, int n_cta, int n_tiles, long long n_pix, float *__restrict__ out) {
-    const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (m >= n_pix) return;
-    const long long t = m / kTile, off = m - t * kTile;
+// pixel's tile, and rounds once to fp32.  blockDim.x divides kTile, so a block lies inside one tile and
+// thread 0 finds the contributing CTAs once for the block.
+constexpr int kReduceThreads = 256;
+constexpr int kReduceMaxSrc = 64;
+__global__ void __launch_bounds__(kReduceThreads)
+reduce_ranges_kernel(const double *__restrict__ partial, int max_seg, const int *__restrict__ row_start, int n_mu,
+                     int n_cta, int n_tiles, long long n_pix, float *__restrict__ out) {
+    __shared__ long long s_src[kReduceMaxSrc];  // element offset of each contributing partial tile
+    __shared__ int s_n, s_c0, s_c1;
+    const long long m0 = (long long)blockIdx.x * kReduceThreads;
+    const long long t = m0 / kTile;
     const long long E = row_start[n_mu], U = E * n_tiles, G = n_cta;
+    if (threadIdx.x == 0) {
+        int n = 0;
+        s_c0 = 0;
+        s_c1 = 0;
+        if (U > 0) {
+            const long long ub = t * E, ue = ub + E;
+            long long c = (ub * G) / U;
+            while (c > 0 && range_begin(c, U, G) > ub) --c;
+            while (c + 1 < G && range_begin(c + 1, U, G) <= ub) ++c;
+            s_c0 = (int)c;
+            for (; c < G; ++c) {
+                const long long b = range_begin(c, U, G), e = range_begin(c + 1, U, G);
+                if (b >= ue) break;
+                if (e <= b || e <= ub) continue;
+                if (n < kReduceMaxSrc) s_src[n] = (c * max_seg + (t - b / E)) * kTile;
+                ++n;
+            }
+            s_c1 = (int)c;
+        }
+        s_n = n;
+    }
+    __syncthreads();
+    const long long m = m0 + threadIdx.x;
+    if (m >= n_pix) return;
+    const long long off = m - t * kTile;
     double v = 0.0;
-    if (U > 0) {
-        const long long ub = t * E, ue = ub + E;
-        long long c = (ub * G) / U;
-        while (c > 0 && range_begin(c, U, G) > ub) --c;
-        while (c + 1 < G && range_begin(c + 1, U, G) <= ub) ++c;
-        for (; c < G; ++c) {
+    if (s_n <= kReduceMaxSrc) {
+        for (int k = 0; k < s_n; ++k) v += partial[s_src[k] + off];
+    } else {  // more contributing CTAs than the table holds (tiny entry lists): walk the ranges directly
+        const long long ub = t * E;
+        for (long long c = s_c0; c < s_c1; ++c) {
             const long long b = range_begin(c, U, G), e = range_begin(c + 1, U, G);
-            if (b >= ue) break;
             if (e <= b || e <= ub) continue;
-            const long long k = t - b / E;
-            v += partial[((c * max_seg + k) * kTile) + off];
+            v += partial[(c * max_seg + (t - b / E)) * kTile + off];
         }
     }
     out[m] = (float)v;

@@ -238,8 +238,8 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     p.partial = s->d_partial.ptr;
     int rc = launch_sia_f32<false>(s, p, dim3((unsigned)G), st);
     if (rc) return rc;
-    const int threads = 256;
-    f32::reduce_ranges_kernel<<<(unsigned)((P + threads - 1) / threads), threads, 0, st>>>(
+    static_assert(f32::kTile % f32::kReduceThreads == 0, "a reduce block must lie inside one tile");
+    f32::reduce_ranges_kernel<<<(unsigned)((P + f32::kReduceThreads - 1) / f32::kReduceThreads), f32::kReduceThreads, 0, st>>>(
         s->d_partial.ptr, p.max_seg, s->d_row_start.ptr, p.n_mu, (int)G, n_tiles, P, static_cast<float *>(out));
     SOAP_LAUNCH_CHECK(s, "reduce_ranges_kernel");
     s->last_quiet_splits = (int)G;
@@ -309,7 +309,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         LbCoef lb{};
         lb.c[1][0] = spot ? spot->lb_c0 : 1.0; lb.c[1][1] = spot ? spot->lb_c1 : 0.0; lb.c[1][2] = spot ? spot->lb_c2 : 0.0;
         lb.c[2][0] = fac ? fac->lb_c0 : 1.0;  lb.c[2][1] = fac ? fac->lb_c1 : 0.0;  lb.c[2][2] = fac ? fac->lb_c2 : 0.0;
-        active_bin_kernel<<<dim3((N + 127) / 128, n_phases), 128, 0, st>>>(
+        active_bin_kernel<<<dim3((N + kBinWarps - 1) / kBinWarps, n_phases), 32 * kBinWarps, 0, st>>>(
             N, n_regions, n_mu, ncap, s->d_rp.ptr, s->d_mu.ptr, s->d_w.ptr, s->d_bin.ptr, lb, s->d_WD.ptr,
             s->d_nactive.ptr);
         SOAP_LAUNCH_CHECK(s, "active_bin_kernel");
@@ -556,12 +556,10 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     // mu_centres: tiny pageable copy; the source is the handle's own vector, which outlives the copy
     SOAP_CUDA(s, cudaMemcpyAsync(s->d_mu_centres.ptr, s->mu_centres.data(), n_mu * sizeof(double), cudaMemcpyHostToDevice, st));
     const double vs = prm->vsini_kms * sini;
-    geometry_cells_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, st>>>(N, vs, prm->ld_u1, prm->ld_u2, n_mu, s->d_mu_centres.ptr,
-                                                                           s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr, s->d_bin.ptr);
-    SOAP_LAUNCH_CHECK(s, "geometry_cells_kernel");
-    geometry_columns_kernel<<<(N + 127) / 128, 128, 0, st>>>(N, vs, prm->doppler_mode, n_mu, s->d_w.ptr, s->d_bin.ptr, s->d_col_a.ptr,
-                                                             s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr);
-    SOAP_LAUNCH_CHECK(s, "geometry_columns_kernel");
+    geometry_kernel<<<(N + kGeomWarps - 1) / kGeomWarps, 32 * kGeomWarps, 0, st>>>(
+        N, vs, prm->ld_u1, prm->ld_u2, prm->doppler_mode, n_mu, s->d_mu_centres.ptr, s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr,
+        s->d_bin.ptr, s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr);
+    SOAP_LAUNCH_CHECK(s, "geometry_kernel");
     build_binned_entries_kernel<<<1, 1024, 0, st>>>(N, n_mu, s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr,
                                                     s->d_ent32.ptr, s->d_ent64.ptr, s->d_row_start.ptr, s->d_info.ptr);
     SOAP_LAUNCH_CHECK(s, "build_binned_entries_kernel");
