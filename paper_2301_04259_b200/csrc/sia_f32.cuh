@@ -7,37 +7,43 @@
 // generic-precision kernel that serves fp64 I/O.)  An entry is a (column, mu-bin) pair with its binned
 // weight, or a single cell; entries of a spectrum row are ordered by shift factor a_e.
 //
-// The path is bound by FP32 instruction issue: one issue slot per SM sub-partition
-// per clock, and the 3 FMAs of a lerp-accumulate are the only instructions the method needs per
-// (entry, pixel).  Everything here exists to keep every other instruction out of the consumers' loop:
+// The path is bound by the FP32 pipe: the 2 FMAs of a lerp-accumulate are the only
+// instructions the method needs per (entry, pixel).  Everything here exists to keep every other
+// instruction out of the consumers' loop and to keep the four SM sub-partitions equally loaded:
 //
-//   * CTA = 4 consumer warps + 1 producer warp.  A consumer thread owns R = 16 pixels of a 2048-pixel
-//     wavelength tile (pixel m_t0 + tid + 128 r: conflict-free shared-memory reads, coalesced stores).
-//   * "jobs" = (spectrum row, <= 128 entries).  The producer warp keeps a ring of kStages jobs in flight:
-//     lane 0 issues two 1-D TMA bulk copies per job (the span of the row the tile's shifts can reach, and
-//     the job's raw entries), then the whole warp turns the raw entries into what the consumers need:
-//       - record {W a, -W q, W, 128 W a} per entry, so that a consumer forms W t for its first pixel with ONE
-//         FMA (W a (lambda0/k + m) - W q) and for pixel r with one more (+ 128 W a r): no floor, no test;
+//   * CTA = 2 warpgroups: warps 0-3 consume, warps 4-7 produce.  Warp w runs on sub-partition w % 4, so
+//     every sub-partition holds one consumer and one producer warp of each resident CTA; `setmaxnreg`
+//     moves the producers' registers to the consumers (40 / 120 per thread, 3 CTAs per SM).
+//   * A consumer thread owns R = 16 pixels of a 2048-pixel wavelength tile (pixel m_t0 + tid + 128 r:
+//     conflict-free shared-memory reads, coalesced stores).
+//   * "jobs" = (spectrum row, <= 128 entries) of one tile.  Stage k of the 4-deep ring belongs to producer
+//     warp k, which handles jobs k, k+4, ... of the CTA: lane 0 issues two 1-D TMA bulk copies (the span of
+//     the row the tile's shifts can reach, and the job's raw entries), then the warp turns the raw entries
+//     into what the consumers need:
+//       - a record {W, W a} per entry;
 //       - a run table: maximal groups of consecutive entries whose integer shift q is the same for every
-//         pixel of the tile.  Consumers load their 16 samples and 16 sample differences once per run.
+//         pixel of the tile.  Consumers load their 16 samples and 16 sample differences once per run;
 //       - entries whose q changes inside the tile ("flips", ~1 %) become runs of their own and take a
-//         per-pixel path.  The producer also writes the clamp-to-edge halo (reading S8) of end tiles.
+//         per-pixel path.  The producer also writes the clamp-to-edge halo (reading S8) of end tiles;
+//       - a descriptor {tile origin, kind, first / last job of the tile, where the result goes}: the
+//         consumers are driven by descriptors alone and walk no work list.
 //     Full/empty mbarriers per stage; consumers never meet a CTA-wide barrier.
-//   * per (entry, thread): 1 LDS.128 (broadcast) + 1 FFMA + 24 packed FFMA2 (fma.rn.f32x2: two pixels per
-//     issue slot, so the FP32 pipe and not instruction issue is the limit) for 16 pixels.  Measured on
-//     B200: FFMA2 runs at the full lane rate (126 of 128 lane-FMA/clk/SM) only with one scalar-broadcast
-//     operand; with three register-pair operands it drops to ~70.  Hence W t_r d_r is split as
-//     (W t_0) d_r + (128 W a) (r d_r) with r d_r kept in registers per run.
+//   * per (entry, thread): 1 LDS.64 (broadcast) + 16 packed FFMA2 (fma.rn.f32x2: two pixels per issue
+//     slot) for 16 pixels.  With t = a c - q (c = lambda0/k + m, q the run's integer shift), W lerp =
+//     W (s + t d) regroups to W u + (W a) v with u = s - q d and v = c d per pixel of the run: every FMA
+//     has one scalar (broadcast) operand, the form that runs at the full lane rate on B200.
 //   * precision: only the shift delta (|delta| < ~50) is formed in fp32, never the absolute source
 //     coordinate; fp32 partial sums are folded into fp64 every kFold entries.
 //   * quiet launch: the flattened (tile, entry) work list is cut into equal contiguous ranges, one per
 //     CTA, grid = resident CTA slots (one wave, no tail); a CTA writes one fp64 partial per tile it
 //     touches and reduce_ranges_kernel adds the partials of a tile in CTA order (deterministic).
-//   * active launch: CTA = (tile, phase); the post-shift contrast (I_ratio of Eq. 3) multiplies each
-//     kind's fp64 sum once per pixel (a6).
+//   * active launch: persistent CTAs; the (phase, tile) items, heaviest phase first, are dealt to the
+//     CTAs in snake order (schedule_active_kernel builds the per-phase job lists and the order); the
+//     post-shift contrast (I_ratio of Eq. 3) multiplies each kind's fp64 sum once per pixel (a6).
 #pragma once
 #include <climits>
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
 
 #include "ptx_helpers.cuh"
@@ -46,15 +52,26 @@ namespace soap {
 namespace f32 {
 
 constexpr int kConsumerWarps = 4;
-constexpr int kConsumers = 32 * kConsumerWarps;  // consumer threads
-constexpr int kThreads = kConsumers + 32;         // + producer warp
-constexpr int kR = 16;                            // pixels per consumer thread
-constexpr int kTile = kConsumers * kR;            // pixels per tile
-constexpr int kStages = 4;                        // jobs in flight
-constexpr int kJobCap = 128;                      // entries per job (even)
-constexpr int kFold = 64;                         // fp32 -> fp64 fold interval (entries)
-constexpr int kMaxSeg = 3 * 64;                   // 3 kinds x SOAP_MAX_MU
-constexpr int kFlip = INT_MIN;                    // run marker: per-pixel path
+constexpr int kProducerWarps = 4;
+constexpr int kConsumers = 32 * kConsumerWarps;             // consumer threads
+constexpr int kThreads = kConsumers + 32 * kProducerWarps;  // two warpgroups
+constexpr int kR = 16;                                      // pixels per consumer thread
+constexpr int kTile = kConsumers * kR;                      // pixels per tile
+constexpr int kStages = kProducerWarps;                     // jobs in flight: stage k belongs to producer warp k
+constexpr int kJobCap = 128;                                // entries per job (even)
+constexpr int kFold = 64;                                   // fp32 -> fp64 fold interval (entries)
+constexpr int kFlip = INT_MIN;                              // run marker: per-pixel path
+constexpr int kCtasPerSm = 3;
+constexpr int kRegsConsumer = 120, kRegsProducer = 40;      // (120 + 40) * 128 = 80 * 256: the launch allocation
+static_assert(kConsumerWarps == 4 && kProducerWarps == 4, "setmaxnreg acts on aligned groups of 4 warps");
+
+enum : int { kJobFirst = 1, kJobLast = 2, kJobExit = 4 };
+
+struct ActiveJob {  // one job of a phase's list (schedule_active_kernel)
+    int begin;      // first entry (global index, even)
+    int count;      // entries, 1..kJobCap
+    int kind, row;
+};
 
 struct Params {
     const float *base[3];      // spectrum tables per kind (quiet launch: base[0] only)
@@ -64,14 +81,16 @@ struct Params {
     int n_mu;
     int halo;                  // H: multiple of 4, >= max |delta| + 2
     const float2 *ent;         // raw entries (a_e, W_e)
+    int n_tiles;
     // quiet launch
     const int *row_start;      // [n_mu + 1] entry offsets (even)
-    int n_tiles;
     double *partial;           // [gridDim.x][max_seg][kTile]
     int max_seg;
     // active launch
-    const int *seg_count;      // [n_phases][3][n_mu]
-    int seg_cap;               // entries reserved per segment (even)
+    const ActiveJob *jobs;     // [n_phases][job_cap]
+    const int *n_jobs;         // [n_phases]
+    const int *phase_order;    // [n_phases] heaviest first
+    int job_cap, n_phases;
     float *out;                // [n_phases][out_pitch]
     long long out_pitch;
 };
@@ -83,79 +102,168 @@ __host__ __device__ inline long long range_begin(long long c, long long U, long 
 
 __host__ __device__ constexpr int span_px(int halo) { return kTile + 2 * halo + 4; }
 
+struct Desc {  // written by the producer with the rest of the stage
+    long long m_t0;  // first pixel of the tile
+    int flags, kind, out_idx, n_runs;
+    int pad[2];
+};
+
 struct StageLayout {
-    size_t row_bytes, raw_off, rec_off, run_off, stage_bytes;
+    size_t row_bytes, raw_off, rec_off, run_off, desc_off, stage_bytes;
 };
 __host__ __device__ inline StageLayout stage_layout(int halo) {
     StageLayout l;
     l.row_bytes = ((size_t)span_px(halo) * sizeof(float) + 127) & ~(size_t)127;
     l.raw_off = l.row_bytes;
     l.rec_off = l.raw_off + kJobCap * sizeof(float2);
-    l.run_off = l.rec_off + kJobCap * sizeof(float2);
-    l.stage_bytes = (l.run_off + (kJobCap + 2) * sizeof(int2) + 127) & ~(size_t)127;
+    l.run_off = l.rec_off + (kJobCap + 2) * sizeof(float2);
+    l.desc_off = (l.run_off + (kJobCap + 2) * sizeof(int2) + 15) & ~(size_t)15;
+    l.stage_bytes = (l.desc_off + sizeof(Desc) + 127) & ~(size_t)127;
     return l;
 }
-constexpr size_t kHeaderBytes = 128 + 2 * kMaxSeg * sizeof(int);  // mbarriers + segment table (multiple of 128)
-constexpr size_t kFinBytes = (size_t)kTile * sizeof(double);      // active launch: per-pixel fp64 delta accumulators
+constexpr size_t kHeaderBytes = 128;                          // mbarriers
+constexpr size_t kFinBytes = (size_t)kTile * sizeof(double);  // active launch: per-pixel fp64 delta accumulators
 __host__ inline size_t smem_bytes(int halo, bool active) {
     return kHeaderBytes + (active ? kFinBytes : 0) + kStages * stage_layout(halo).stage_bytes;
 }
 
 struct Job {
     long long tile;
-    int seg;    // segment index (kind * n_mu + row)
+    int kind, row;
     int begin;  // first entry (global index, even)
-    int count;  // entries, <= kJobCap
+    int count;  // entries, <= kJobCap (0: an item without entries)
+    int flags, out_idx;
 };
 
-// Enumerates the jobs of a CTA: for each tile of its range, for each segment, chunks of <= kJobCap
-// entries.  The producer (twice: issue and post-process) and every consumer walk the same sequence.
-struct WorkIter {
-    long long t, t_end, u0, u1, E;
-    int s, pos, e_lo, e_hi;
-    bool ranged;
-    __device__ void open_tile() {
-        if (ranged) {
-            const long long lo = u0 - t * E, hi = u1 - t * E;
-            e_lo = (int)(lo > 0 ? lo : 0);
-            e_hi = (int)(hi < E ? hi : E);
-        } else {
-            e_lo = 0;
-            e_hi = INT_MAX;
-        }
-        s = 0;
-        pos = 0;
+// ---- job sources: the n-th job of this CTA (every lane of a producer warp computes the same answer) ----------
+enum : int { kSrcJob = 0, kSrcExit = 1, kSrcBeyond = 2 };
+
+// Quiet launch: CTA c owns units [range_begin(c), range_begin(c+1)) of the flattened (tile, entry) list; the
+// entries of a tile are contiguous (rows back to back), so a job is a chunk of one row inside that range.
+struct QuietSource {
+    const int *row_start;
+    long long E, u0, u1, t, t_first;
+    int e, e_lo, e_hi, s, cur;
+    bool done;
+    __device__ void init(const Params &p, long long cta, long long G) {
+        row_start = p.row_start;
+        E = __ldg(&row_start[p.n_mu]);
+        const long long U = E * p.n_tiles;
+        u0 = range_begin(cta, U, G);
+        u1 = range_begin(cta + 1, U, G);
+        done = u1 <= u0;
+        t = t_first = done ? 0 : u0 / E;
+        cur = 0;
+        open_tile();
     }
-    __device__ bool next(const int *seg_lo, const int *seg_hi, int n_seg, Job &j) {
-        for (;;) {
-            while (s < n_seg) {
-                const int lo = max(seg_lo[s], e_lo), hi = min(seg_hi[s], e_hi);
-                const int p = max(pos, lo);
-                if (p < hi) {
-                    j.tile = t;
-                    j.seg = s;
-                    j.begin = p;
-                    j.count = min(hi - p, kJobCap);
-                    pos = p + j.count;
-                    return true;
-                }
-                ++s;
-            }
-            if (t >= t_end) return false;
+    __device__ void open_tile() {
+        const long long lo = u0 - t * E, hi = u1 - t * E;
+        e_lo = (int)(lo > 0 ? lo : 0);
+        e_hi = (int)(hi < E ? hi : E);
+        e = e_lo;
+        s = 0;
+    }
+    __device__ bool next(Job &j) {
+        if (done) return false;
+        while (e >= e_hi) {
             ++t;
+            if (t * E >= u1) {
+                done = true;
+                return false;
+            }
             open_tile();
         }
+        while (__ldg(&row_start[s + 1]) <= e) ++s;  // rows without entries are skipped
+        const int end = min(min(e + kJobCap, __ldg(&row_start[s + 1])), e_hi);
+        j.tile = t;
+        j.kind = 0;
+        j.row = s;
+        j.begin = e;
+        j.count = end - e;
+        j.flags = (e == e_lo ? kJobFirst : 0) | (end == e_hi ? kJobLast : 0);
+        j.out_idx = (int)(t - t_first);
+        e = end;
+        return true;
+    }
+    __device__ int get(int n, Job &j) {
+        while (cur <= n) {
+            if (!next(j)) return n == cur ? kSrcExit : kSrcBeyond;
+            ++cur;
+        }
+        return kSrcJob;
     }
 };
 
+// Active launch: items = (phase, tile), ordered heaviest phase first; round i deals items i G .. i G + G - 1 to
+// the G CTAs, forwards in even rounds and backwards in odd ones (snake order: static, hence deterministic,
+// and within one item's work of balanced).  An item's jobs are its phase's job list applied to its tile; a
+// phase without covered cells yields one empty job so that its zeros are written (reading S19).
+struct ActiveSource {
+    const ActiveJob *jobs;
+    const int *n_jobs, *phase_order;
+    long long n_items, G, c;
+    int n_tiles, job_cap;
+    long long i;
+    int n0, nj, cnt, phase, tile;
+    bool done;
+    __device__ void load_item() {
+        const long long idx = i * G + ((i & 1) ? (G - 1 - c) : c);
+        done = idx >= n_items;
+        if (done) return;
+        phase = __ldg(&phase_order[idx / n_tiles]);
+        tile = (int)(idx % n_tiles);
+        cnt = __ldg(&n_jobs[phase]);
+        nj = cnt > 0 ? cnt : 1;
+    }
+    __device__ void init(const Params &p, long long cta, long long G_) {
+        jobs = p.jobs;
+        n_jobs = p.n_jobs;
+        phase_order = p.phase_order;
+        n_tiles = p.n_tiles;
+        job_cap = p.job_cap;
+        n_items = (long long)p.n_phases * p.n_tiles;
+        G = G_;
+        c = cta;
+        i = 0;
+        n0 = 0;
+        nj = 0;
+        load_item();
+    }
+    __device__ int get(int n, Job &j) {
+        while (!done && n >= n0 + nj) {
+            n0 += nj;
+            ++i;
+            load_item();
+        }
+        if (done) return n == n0 ? kSrcExit : kSrcBeyond;
+        const int k = n - n0;
+        j.tile = tile;
+        j.out_idx = phase;
+        if (cnt == 0) {
+            j.kind = j.row = j.begin = j.count = 0;
+            j.flags = kJobFirst | kJobLast;
+        } else {
+            const int4 a = __ldg(reinterpret_cast<const int4 *>(jobs + (size_t)phase * job_cap + k));
+            j.begin = a.x;
+            j.count = a.y;
+            j.kind = a.z;
+            j.row = a.w;
+            j.flags = (k == 0 ? kJobFirst : 0) | (k == cnt - 1 ? kJobLast : 0);
+        }
+        return kSrcJob;
+    }
+};
+
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t *bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) __nanosleep(40);
+}
+
 template <bool ACTIVE>
-__global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Params p) {
     extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t *bar_tma = reinterpret_cast<uint64_t *>(smem);  // [kStages] TMA landed      (count 1 + tx)
-    uint64_t *bar_ready = bar_tma + kStages;                 // [kStages] records written (count 1)
-    uint64_t *bar_empty = bar_ready + kStages;               // [kStages] consumers done  (count kConsumerWarps)
-    int *seg_lo = reinterpret_cast<int *>(smem + 128);
-    int *seg_hi = seg_lo + kMaxSeg;
+    uint64_t *bar_tma = reinterpret_cast<uint64_t *>(smem);  // [kStages] TMA landed          (count 1 + tx)
+    uint64_t *bar_ready = bar_tma + kStages;                 // [kStages] stage post-processed (count 1)
+    uint64_t *bar_empty = bar_ready + kStages;               // [kStages] consumers done       (count kConsumerWarps)
     const int H = p.halo;
     const int span = span_px(H);
     const StageLayout L = stage_layout(H);
@@ -164,37 +272,6 @@ __global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
 
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
-    const int n_seg = ACTIVE ? 3 * p.n_mu : p.n_mu;
-
-    // ---- this CTA's work ---------------------------------------------------------------------------
-    WorkIter w0;
-    if (ACTIVE) {
-        const int phase = blockIdx.y;
-        for (int s = tid; s < n_seg; s += kThreads) {
-            const int gs = phase * n_seg + s;
-            seg_lo[s] = gs * p.seg_cap;  // fits: host checks n_phases*3*n_mu*seg_cap < 2^31
-            seg_hi[s] = gs * p.seg_cap + p.seg_count[gs];
-        }
-        w0.ranged = false;
-        w0.t = w0.t_end = blockIdx.x;
-        w0.u0 = w0.u1 = w0.E = 0;
-    } else {
-        for (int s = tid; s < n_seg; s += kThreads) {
-            seg_lo[s] = p.row_start[s];
-            seg_hi[s] = p.row_start[s + 1];
-        }
-        const long long E = p.row_start[p.n_mu];
-        const long long U = E * p.n_tiles;
-        w0.ranged = true;
-        w0.E = E;
-        w0.u0 = range_begin(blockIdx.x, U, gridDim.x);
-        w0.u1 = range_begin(blockIdx.x + 1, U, gridDim.x);
-        if (w0.u1 <= w0.u0) return;  // more CTAs than work (whole CTA leaves before any barrier)
-        w0.t = w0.u0 / E;
-        w0.t_end = (w0.u1 - 1) / E;
-    }
-    w0.open_tile();
-    const long long t_first = w0.t, t_last = w0.t_end;
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) {
             mbar_init(&bar_tma[s], 1);
@@ -205,237 +282,274 @@ __global__ void __launch_bounds__(kThreads, 3) sia_f32_kernel(const Params p) {
     }
     __syncthreads();
 
-    if (warp == kConsumerWarps) {
-        // =============================== producer warp ===============================================
-        WorkIter it_issue = w0, it_proc = w0;
-        Job ji, jp;
-        bool have_ji = false, more = true;
-        int n_issued = 0, n_proc = 0;
-        for (;;) {
-            // -- keep the TMA ring full -----------------------------------------------------------------
-            for (;;) {
-                if (!have_ji && more) {
-                    more = it_issue.next(seg_lo, seg_hi, n_seg, ji);
-                    have_ji = more;
-                }
-                if (!have_ji || n_issued >= n_proc + kStages) break;
-                const int st = n_issued % kStages;
-                const uint32_t par = (uint32_t)(((n_issued / kStages) & 1) ^ 1);
-                int free_ = 0;
-                if (lane == 0) free_ = mbar_try_wait(&bar_empty[st], par) ? 1 : 0;
-                free_ = __shfl_sync(0xffffffffu, free_, 0);
-                if (!free_) break;
+    if (warp >= kConsumerWarps) {
+        // =============================== producer warps ==============================================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsProducer));
+        const int st = warp - kConsumerWarps;  // this warp's stage
+        unsigned char *sb = stage0 + (size_t)st * L.stage_bytes;
+        float *rs = reinterpret_cast<float *>(sb);
+        const float2 *raw = reinterpret_cast<const float2 *>(sb + L.raw_off);
+        float2 *rec = reinterpret_cast<float2 *>(sb + L.rec_off);
+        int2 *runs = reinterpret_cast<int2 *>(sb + L.run_off);
+        Desc *desc = reinterpret_cast<Desc *>(sb + L.desc_off);
+        typename std::conditional<ACTIVE, ActiveSource, QuietSource>::type src;
+        src.init(p, blockIdx.x, gridDim.x);
+        Job jb;
+        for (int n = st, use = 0;; n += kStages, ++use) {
+            const int status = src.get(n, jb);
+            if (status == kSrcBeyond) break;
+            mbar_wait_backoff(&bar_empty[st], (uint32_t)((use & 1) ^ 1));
+            if (status == kSrcExit) {
                 if (lane == 0) {
-                    const long long s_start = ji.tile * kTile - H;  // global pixel of smem position 0 (multiple of 4)
+                    desc->flags = kJobExit;
+                    mbar_arrive(&bar_ready[st]);
+                }
+                break;
+            }
+            const long long m_t0 = jb.tile * kTile;
+            const long long s_start = m_t0 - H;  // global pixel of smem position 0 (multiple of 4)
+            if (lane == 0) {
+                if (jb.count > 0) {
                     const long long g_lo = s_start < 0 ? 0 : s_start;
                     const long long g_hi = (s_start + span) < p.pitch ? (s_start + span) : p.pitch;
                     const uint32_t row_bytes = (uint32_t)((g_hi - g_lo) * (long long)sizeof(float));
-                    const int kind = ACTIVE ? ji.seg / p.n_mu : 0;
-                    const int row = ACTIVE ? ji.seg - kind * p.n_mu : ji.seg;
-                    const float *src = p.base[kind] + (long long)row * p.pitch + g_lo;
-                    const uint32_t ent_bytes = (uint32_t)(((ji.count + 1) & ~1) * (int)sizeof(float2));
-                    unsigned char *sb = stage0 + (size_t)st * L.stage_bytes;
+                    const float *src_row = p.base[jb.kind] + (long long)jb.row * p.pitch + g_lo;
+                    const uint32_t ent_bytes = (uint32_t)(((jb.count + 1) & ~1) * (int)sizeof(float2));
                     fence_proxy_async_smem();
                     mbar_arrive_expect_tx(&bar_tma[st], row_bytes + ent_bytes);
-                    tma_load_1d(sb + (size_t)(g_lo - s_start) * sizeof(float), src, row_bytes, &bar_tma[st]);
-                    tma_load_1d(sb + L.raw_off, p.ent + ji.begin, ent_bytes, &bar_tma[st]);
+                    tma_load_1d(sb + (size_t)(g_lo - s_start) * sizeof(float), src_row, row_bytes, &bar_tma[st]);
+                    tma_load_1d(sb + L.raw_off, p.ent + jb.begin, ent_bytes, &bar_tma[st]);
+                } else {
+                    mbar_arrive(&bar_tma[st]);  // nothing to load: keeps the barrier's phase in step
                 }
-                ++n_issued;
-                have_ji = false;
             }
-            if (n_proc < n_issued) {
-                // -- post-process one landed job: records, run table, edge halo ---------------------------
-                it_proc.next(seg_lo, seg_hi, n_seg, jp);
-                const int st = n_proc % kStages;
-                mbar_wait(&bar_tma[st], (uint32_t)((n_proc / kStages) & 1));
-                unsigned char *sb = stage0 + (size_t)st * L.stage_bytes;
-                float *rs = reinterpret_cast<float *>(sb);
-                const float2 *raw = reinterpret_cast<const float2 *>(sb + L.raw_off);
-                float2 *rec = reinterpret_cast<float2 *>(sb + L.rec_off);
-                int2 *runs = reinterpret_cast<int2 *>(sb + L.run_off);
-                const long long m_t0 = jp.tile * kTile;
-                const float c_first = (float)(p.c0 + (double)m_t0);
-                const float c_last = (float)(p.c0 + (double)(m_t0 + kTile - 1));
-                int n_runs = 0, carry = kFlip;  // kFlip never equals a q: the first entry opens a run
-                for (int i0 = 0; i0 < jp.count; i0 += 32) {
-                    const int i = i0 + lane;
-                    const bool valid = i < jp.count;
-                    int code = kFlip;
-                    if (valid) {
-                        const float2 en = raw[i];
-                        const float qf = floorf(en.x * c_first), ql = floorf(en.x * c_last);
-                        int qi = (int)qf;
-                        qi = max(-H, min(H + 2, qi));
-                        rec[i] = make_float2(en.y, en.y * en.x);  // {W, W a}
-                        if (qf == ql) code = qi;
-                    }
-                    int prev = __shfl_up_sync(0xffffffffu, code, 1);
-                    if (lane == 0) prev = carry;
-                    const bool start = valid && (code == kFlip || code != prev);
-                    const unsigned mask = __ballot_sync(0xffffffffu, start);
-                    if (start) runs[1 + n_runs + __popc(mask & ((1u << lane) - 1u))] = make_int2(i, code);
-                    n_runs += __popc(mask);
-                    carry = __shfl_sync(0xffffffffu, code, 31);
+            mbar_wait(&bar_tma[st], (uint32_t)(use & 1));
+            // -- records, run table, edge halo, descriptor ---------------------------------------------
+            const float c_first = (float)(p.c0 + (double)m_t0);
+            const float c_last = (float)(p.c0 + (double)(m_t0 + kTile - 1));
+            int n_runs = 0, carry = kFlip;  // kFlip never equals a q: the first entry opens a run
+            for (int i0 = 0; i0 < jb.count; i0 += 32) {
+                const int i = i0 + lane;
+                const bool valid = i < jb.count;
+                int code = kFlip;
+                if (valid) {
+                    const float2 en = raw[i];
+                    const float qf = floorf(en.x * c_first), ql = floorf(en.x * c_last);
+                    int qi = (int)qf;
+                    qi = max(-H, min(H + 2, qi));
+                    rec[i] = make_float2(en.y, en.y * en.x);  // {W, W a}
+                    if (qf == ql) code = qi;
                 }
-                if (lane == 0) {
-                    runs[0] = make_int2(n_runs, 0);
-                    runs[1 + n_runs] = make_int2(jp.count, 0);  // sentinel: end of the last run
-                }
-                const long long s_start = m_t0 - H;
+                int prev = __shfl_up_sync(0xffffffffu, code, 1);
+                if (lane == 0) prev = carry;
+                const bool start = valid && (code == kFlip || code != prev);
+                const unsigned mask = __ballot_sync(0xffffffffu, start);
+                if (start) runs[n_runs + __popc(mask & ((1u << lane) - 1u))] = make_int2(i, code);
+                n_runs += __popc(mask);
+                carry = __shfl_sync(0xffffffffu, code, 31);
+            }
+            if (lane == 0) {
+                runs[n_runs] = make_int2(jb.count, 0);  // sentinel: end of the last run
+                desc->m_t0 = m_t0;
+                desc->flags = jb.flags;
+                desc->kind = jb.kind;
+                desc->out_idx = jb.out_idx;
+                desc->n_runs = n_runs;
+            }
+            if (jb.count > 0) {
                 if (s_start < 0) {  // clamp-to-edge below the grid (reading S8)
-                    const int n = (int)(-s_start);
-                    const float v = rs[n];
-                    for (int q = lane; q < n; q += 32) rs[q] = v;
+                    const int nb = (int)(-s_start);
+                    const float v = rs[nb];
+                    for (int q = lane; q < nb; q += 32) rs[q] = v;
                 }
                 if (s_start + span > p.n_pix) {  // ... and above it
                     const int first = (int)(p.n_pix - s_start);
                     const float v = rs[first - 1];
                     for (int q = first + lane; q < span; q += 32) rs[q] = v;
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&bar_ready[st]);
-                ++n_proc;
-            } else if (!have_ji) {
-                break;  // everything issued and processed
-            } else {
-                // ring full of jobs the consumers still hold: wait for the oldest stage
-                const int st = n_issued % kStages;
-                mbar_wait(&bar_empty[st], (uint32_t)(((n_issued / kStages) & 1) ^ 1));
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bar_ready[st]);
         }
         return;
     }
 
     // =================================== consumer warps ===============================================
-    WorkIter it = w0;
-    Job job;
-    bool have = it.next(seg_lo, seg_hi, n_seg, job);
-    int n_done = 0;
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsConsumer));
     const int base0 = H + tid;  // smem position of pixel r = 0 at zero shift
-    for (long long tile = t_first; tile <= t_last; ++tile) {
-        const long long m_t0 = tile * kTile;
-        const float cmf = (float)(p.c0 + (double)(m_t0 + tid));  // lambda0/k + m of this thread's first pixel
-        float2 acc[kR / 2];  // pair k = pixels r = 2k, 2k + 1: the operands of one packed FMA
-        double tot[kR];
+    long long m_t0 = 0;
+    float cmf = 0.f;      // lambda0/k + m of this thread's first pixel
+    float2 acc[kR / 2];   // pair k = pixels r = 2k, 2k + 1: the operands of one packed FMA
+    double tot[kR];
+    int cnt = 0, cur_kind = 0;
+    auto fold = [&]() {
+#pragma unroll
+        for (int k = 0; k < kR / 2; ++k) {
+            tot[2 * k] += (double)acc[k].x;
+            tot[2 * k + 1] += (double)acc[k].y;
+            acc[k] = make_float2(0.f, 0.f);
+        }
+        cnt = 0;
+    };
+    auto fold_kind = [&](int kind) {  // a6: post-shift contrast (I_ratio of Eq. 3) per output pixel
+        const float *ck = kind > 0 ? p.contrast[kind] : nullptr;
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
-            if (r & 1) acc[r / 2].y = 0.f;
-            else acc[r / 2].x = 0.f;
+            const long long m = m_t0 + tid + kConsumers * r;
+            double c = 1.0;
+            if (ck != nullptr && m < p.n_pix) c = (double)__ldg(&ck[m]);
+            fin[r * kConsumers + tid] += c * tot[r];
             tot[r] = 0.0;
-            if (ACTIVE) fin[r * kConsumers + tid] = 0.0;  // only this thread ever touches its 16 slots
         }
-        int cnt = 0, cur_kind = 0;
-        auto fold = [&]() {
+    };
+
+    for (int n = 0;; ++n) {
+        const int st = n % kStages;
+        mbar_wait(&bar_ready[st], (uint32_t)((n / kStages) & 1));
+        const unsigned char *sb = stage0 + (size_t)st * L.stage_bytes;
+        const float *rs = reinterpret_cast<const float *>(sb);
+        const float2 *raw = reinterpret_cast<const float2 *>(sb + L.raw_off);
+        const float2 *rec = reinterpret_cast<const float2 *>(sb + L.rec_off);
+        const int2 *runs = reinterpret_cast<const int2 *>(sb + L.run_off);
+        const Desc *desc = reinterpret_cast<const Desc *>(sb + L.desc_off);
+        const int flags = desc->flags;
+        if (flags & kJobExit) break;
+        const int n_runs = desc->n_runs;
+        const int kind = desc->kind;
+        const int out_idx = desc->out_idx;
+        if (flags & kJobFirst) {
+            m_t0 = desc->m_t0;
+            cmf = (float)(p.c0 + (double)(m_t0 + tid));
 #pragma unroll
-            for (int k = 0; k < kR / 2; ++k) {
-                tot[2 * k] += (double)acc[k].x;
-                tot[2 * k + 1] += (double)acc[k].y;
-                acc[k] = make_float2(0.f, 0.f);
+            for (int r = 0; r < kR; ++r) {
+                if (r & 1) acc[r / 2].y = 0.f;
+                else acc[r / 2].x = 0.f;
+                tot[r] = 0.0;
+                if (ACTIVE) fin[r * kConsumers + tid] = 0.0;  // only this thread ever touches its 16 slots
             }
             cnt = 0;
-        };
-        auto fold_kind = [&](int kind) {  // a6: post-shift contrast (I_ratio of Eq. 3) per output pixel
-#pragma unroll
-            for (int r = 0; r < kR; ++r) {
-                const long long m = m_t0 + tid + kConsumers * r;
-                double c = 1.0;
-                if (kind > 0 && p.contrast[kind] != nullptr && m < p.n_pix) c = (double)p.contrast[kind][m];
-                if (ACTIVE) fin[r * kConsumers + tid] += c * tot[r];
-                tot[r] = 0.0;
-            }
-        };
-
-        while (have && job.tile == tile) {
-            const int st = n_done % kStages;
-            mbar_wait(&bar_ready[st], (uint32_t)((n_done / kStages) & 1));
-            const unsigned char *sb = stage0 + (size_t)st * L.stage_bytes;
-            const float *rs = reinterpret_cast<const float *>(sb);
-            const float2 *raw = reinterpret_cast<const float2 *>(sb + L.raw_off);
-            const float2 *rec = reinterpret_cast<const float2 *>(sb + L.rec_off);
-            const int2 *runs = reinterpret_cast<const int2 *>(sb + L.run_off);
-            if (ACTIVE) {
-                const int kind = job.seg / p.n_mu;
-                if (kind != cur_kind) {
-                    fold();
-                    fold_kind(cur_kind);
-                    cur_kind = kind;
-                }
-            }
-            const int n_runs = runs[0].x;
-            for (int ri = 1; ri <= n_runs; ++ri) {
-                const int2 run = runs[ri];
-                const int nxt = runs[ri + 1].x;
-                if (run.y == kFlip) {
-                    // integer shift changes inside the tile: per-pixel floor
-                    const float2 en = raw[run.x];
-#pragma unroll
-                    for (int r = 0; r < kR; ++r) {
-                        const float cm = cmf + (float)(kConsumers * r);
-                        const float q = floorf(en.x * cm);
-                        const float t = fmaf(en.x, cm, -q);
-                        int qi = (int)q;
-                        qi = max(-H, min(H + 2, qi));
-                        const float s0 = rs[base0 + kConsumers * r + qi], s1 = rs[base0 + kConsumers * r + qi + 1];
-                        float &ar = (r & 1) ? acc[r / 2].y : acc[r / 2].x;
-                        ar = fmaf(en.y, fmaf(t, s1 - s0, s0), ar);
-                    }
-                    if (++cnt >= kFold) fold();
-                    continue;
-                }
-                // With t = a c - q (c = lambda0/k + m, q the run's integer shift), W lerp = W (s + t d) regroups
-                // to W u + (W a) v with u = s - q d and v = c d: u_r, v_r are per-pixel registers of the run and
-                // every entry costs two FMAs per pixel, each with one scalar (broadcast) operand.
-                float2 u[kR / 2], v[kR / 2];
-                {
-                    const float *wv = rs + base0 + run.y;
-                    const float2 nq = bcast2(-(float)run.y);
-#pragma unroll
-                    for (int k = 0; k < kR / 2; ++k) {
-                        const float2 s0 = make_float2(wv[kConsumers * 2 * k], wv[kConsumers * (2 * k + 1)]);
-                        const float2 s1 = make_float2(wv[kConsumers * 2 * k + 1], wv[kConsumers * (2 * k + 1) + 1]);
-                        const float2 d = fma2(bcast2(-1.f), s0, s1);
-                        const float2 c = make_float2(cmf + (float)(kConsumers * 2 * k), cmf + (float)(kConsumers * (2 * k + 1)));
-                        u[k] = fma2(nq, d, s0);
-                        v[k] = fma2(c, d, bcast2(0.f));
-                    }
-                }
-                int e = run.x;
-                while (e < nxt) {
-                    const int n = min(nxt - e, kFold - cnt);
-#pragma unroll 2
-                    for (int i = 0; i < n; ++i) {
-                        const float2 rc = rec[e + i];  // {W, W a}
-#pragma unroll
-                        for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.x), u[k], acc[k]);  // (1) + W u_r
-#pragma unroll
-                        for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.y), v[k], acc[k]);  // (2) + W a v_r
-                    }
-                    e += n;
-                    cnt += n;
-                    if (cnt >= kFold) fold();
-                }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&bar_empty[st]);
-            ++n_done;
-            have = it.next(seg_lo, seg_hi, n_seg, job);
+            cur_kind = kind;
         }
-
-        // ---- store ---------------------------------------------------------------------------------
-        fold();
-        if (ACTIVE) {
+        if (ACTIVE && kind != cur_kind) {
+            fold();
             fold_kind(cur_kind);
-            float *o = p.out + (long long)blockIdx.y * p.out_pitch;
-#pragma unroll
-            for (int r = 0; r < kR; ++r) {
-                const long long m = m_t0 + tid + kConsumers * r;
-                if (m < p.n_pix) o[m] = (float)fin[r * kConsumers + tid];
-            }
-        } else {
-            double *o = p.partial + ((long long)blockIdx.x * p.max_seg + (tile - t_first)) * kTile;
-#pragma unroll
-            for (int r = 0; r < kR; ++r) o[tid + kConsumers * r] = tot[r];
+            cur_kind = kind;
         }
+        for (int ri = 0; ri < n_runs; ++ri) {
+            const int2 run = runs[ri];
+            const int nxt = runs[ri + 1].x;
+            if (run.y == kFlip) {
+                // integer shift changes inside the tile: per-pixel floor
+                const float2 en = raw[run.x];
+#pragma unroll
+                for (int r = 0; r < kR; ++r) {
+                    const float cm = cmf + (float)(kConsumers * r);
+                    const float q = floorf(en.x * cm);
+                    const float t = fmaf(en.x, cm, -q);
+                    int qi = (int)q;
+                    qi = max(-H, min(H + 2, qi));
+                    const float s0 = rs[base0 + kConsumers * r + qi], s1 = rs[base0 + kConsumers * r + qi + 1];
+                    float &ar = (r & 1) ? acc[r / 2].y : acc[r / 2].x;
+                    ar = fmaf(en.y, fmaf(t, s1 - s0, s0), ar);
+                }
+                if (++cnt >= kFold) fold();
+                continue;
+            }
+            // W lerp = W u + (W a) v with u = s - q d and v = c d: u_r, v_r are per-pixel registers of the run
+            float2 u[kR / 2], v[kR / 2];
+            {
+                const float *wv = rs + base0 + run.y;
+                const float2 nq = bcast2(-(float)run.y);
+#pragma unroll
+                for (int k = 0; k < kR / 2; ++k) {
+                    const float2 s0 = make_float2(wv[kConsumers * 2 * k], wv[kConsumers * (2 * k + 1)]);
+                    const float2 s1 = make_float2(wv[kConsumers * 2 * k + 1], wv[kConsumers * (2 * k + 1) + 1]);
+                    const float2 d = fma2(bcast2(-1.f), s0, s1);
+                    const float2 c = make_float2(cmf + (float)(kConsumers * 2 * k), cmf + (float)(kConsumers * (2 * k + 1)));
+                    u[k] = fma2(nq, d, s0);
+                    v[k] = fma2(c, d, bcast2(0.f));
+                }
+            }
+            int e = run.x;
+            float2 rc = rec[e];  // {W, W a}; the next record is fetched while this one is used
+            while (e < nxt) {
+                const int nn = min(nxt - e, kFold - cnt);
+#pragma unroll 2
+                for (int i = 0; i < nn; ++i) {
+                    const float2 nx = rec[e + i + 1];  // one past the run's end is still inside the stage
+#pragma unroll
+                    for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.x), u[k], acc[k]);  // (1) + W u_r
+#pragma unroll
+                    for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.y), v[k], acc[k]);  // (2) + W a v_r
+                    rc = nx;
+                }
+                e += nn;
+                cnt += nn;
+                if (cnt >= kFold) fold();
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bar_empty[st]);  // the stage may be refilled while the tile is stored
+
+        if (flags & kJobLast) {
+            fold();
+            if (ACTIVE) {
+                fold_kind(cur_kind);
+                float *o = p.out + (long long)out_idx * p.out_pitch;
+#pragma unroll
+                for (int r = 0; r < kR; ++r) {
+                    const long long m = m_t0 + tid + kConsumers * r;
+                    if (m < p.n_pix) o[m] = (float)fin[r * kConsumers + tid];
+                }
+            } else {
+                double *o = p.partial + ((long long)blockIdx.x * p.max_seg + out_idx) * kTile;
+#pragma unroll
+                for (int r = 0; r < kR; ++r) o[tid + kConsumers * r] = tot[r];
+            }
+        }
+    }
+}
+
+// a4 -> a5 hand-over: turns the per-(phase, kind, mu-bin) segment counts of active_compact_kernel into each
+// phase's job list (chunks of <= kJobCap entries of one segment) and orders the phases by work, heaviest
+// first (ties by phase index: deterministic).  One CTA; n_phases is at most a few thousand.
+constexpr int kScheduleThreads = 1024;
+constexpr int kScheduleSortMax = 4096;  // beyond this many phases the order is left as given
+__global__ void __launch_bounds__(kScheduleThreads)
+schedule_active_kernel(const int *__restrict__ seg_count /*[n_phases][3 n_mu]*/, int n_phases, int n_mu, int seg_cap,
+                       int job_cap, ActiveJob *__restrict__ jobs, int *__restrict__ n_jobs, int *__restrict__ phase_order,
+                       int *__restrict__ work) {
+    const int n_seg = 3 * n_mu;
+    for (int ph = threadIdx.x; ph < n_phases; ph += blockDim.x) {
+        int k = 0, w = 0;
+        for (int s = 0; s < n_seg; ++s) {
+            const int gs = ph * n_seg + s;
+            const int c = seg_count[gs];
+            for (int off = 0; off < c; off += kJobCap) {
+                ActiveJob j;
+                j.begin = gs * seg_cap + off;  // fits: host checks n_phases * 3 n_mu * seg_cap < 2^31
+                j.count = min(kJobCap, c - off);
+                j.kind = s / n_mu;
+                j.row = s - j.kind * n_mu;
+                jobs[(size_t)ph * job_cap + k++] = j;
+            }
+            w += c;
+        }
+        n_jobs[ph] = k;
+        work[ph] = w;
+    }
+    __syncthreads();
+    for (int ph = threadIdx.x; ph < n_phases; ph += blockDim.x) {
+        int rank = ph;
+        if (n_phases <= kScheduleSortMax) {
+            const int w = work[ph];
+            rank = 0;
+            for (int q = 0; q < n_phases; ++q) {
+                const int wq = work[q];
+                rank += (wq > w || (wq == w && q < ph)) ? 1 : 0;
+            }
+        }
+        phase_order[rank] = ph;
     }
 }
 

@@ -6,6 +6,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <type_traits>
 #include <new>
 #include <string>
 #include <vector>
@@ -90,7 +91,8 @@ struct soap_star {
     int h_rp_next = 0;
     DevBuf<double> d_WD;
     DevBuf<unsigned char> d_aent;
-    DevBuf<int> d_segcnt, d_nactive;
+    DevBuf<int> d_segcnt, d_nactive, d_sched;
+    DevBuf<f32::ActiveJob> d_jobs;
     DevBuf<Counters> d_counters;
 
     // host-buffer staging (soap_synthesize_host)
@@ -323,6 +325,14 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         SOAP_LAUNCH_CHECK(s, "active_compact_kernel");
     }
     if (sizeof(T) == 4) {
+        // per-phase job lists + heaviest-first phase order for the persistent active launch
+        const int job_cap = 3 * n_mu * ((ncap + f32::kJobCap - 1) / f32::kJobCap);
+        SOAP_CUDA(s, s->d_jobs.reserve((size_t)n_phases * job_cap));
+        SOAP_CUDA(s, s->d_sched.reserve((size_t)3 * n_phases));
+        int *d_njobs = s->d_sched.ptr, *d_order = d_njobs + n_phases, *d_work = d_order + n_phases;
+        f32::schedule_active_kernel<<<1, f32::kScheduleThreads, 0, st>>>(s->d_segcnt.ptr, n_phases, n_mu, ncap, job_cap,
+                                                                         s->d_jobs.ptr, d_njobs, d_order, d_work);
+        SOAP_LAUNCH_CHECK(s, "schedule_active_kernel");
         f32::Params p{};
         p.base[0] = static_cast<const float *>(q->data);
         p.base[1] = spot ? static_cast<const float *>(spot->data) : p.base[0];
@@ -335,13 +345,25 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         p.n_mu = n_mu;
         p.halo = halo_for(s, q);
         p.ent = reinterpret_cast<const float2 *>(s->d_aent.ptr);
-        p.seg_count = s->d_segcnt.ptr;
-        p.seg_cap = ncap;
+        p.n_tiles = (int)((q->n_pix + f32::kTile - 1) / f32::kTile);
+        p.jobs = s->d_jobs.ptr;
+        p.n_jobs = d_njobs;
+        p.phase_order = d_order;
+        p.job_cap = job_cap;
+        p.n_phases = n_phases;
         p.out = static_cast<float *>(out);
         p.out_pitch = out_pitch;
-        const int n_tiles = (int)((q->n_pix + f32::kTile - 1) / f32::kTile);
         s->last_tile_px = f32::kTile;
-        return launch_sia_f32<true>(s, p, dim3(n_tiles, n_phases), st);
+        // persistent CTAs: one per resident slot, fewer when there are fewer (phase, tile) items
+        const size_t smem = f32::smem_bytes(p.halo, true);
+        if (smem > 227 * 1024) return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", p.halo, smem);
+        SOAP_CUDA(s, cudaFuncSetAttribute(f32::sia_f32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int occ = 0;
+        SOAP_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f32::sia_f32_kernel<true>, f32::kThreads, smem));
+        if (occ < 1) return s->fail(SOAP_ERR_UNSUPPORTED, "active kernel does not fit on an SM (halo %d)", p.halo);
+        const long long items = (long long)n_phases * p.n_tiles;
+        const long long G = std::max(1LL, std::min((long long)s->n_sm * occ, items));
+        return launch_sia_f32<true>(s, p, dim3((unsigned)G), st);
     }
     SiaParams<T> p{};
     p.base[0] = static_cast<const T *>(q->data);
@@ -472,7 +494,7 @@ int soap_destroy(soap_star *s) {
     s->d_mu_centres.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
     s->d_Wbin.release(); s->d_col_sumw.release(); s->d_bin.release(); s->d_col_nvis.release(); s->d_row_start.release();
     s->d_ent32.release(); s->d_ent64.release(); s->d_info.release(); s->d_partial.release(); s->d_rp.release();
-    s->d_WD.release(); s->d_aent.release(); s->d_segcnt.release(); s->d_nactive.release(); s->d_counters.release();
+    s->d_WD.release(); s->d_aent.release(); s->d_segcnt.release(); s->d_nactive.release(); s->d_counters.release(); s->d_sched.release(); s->d_jobs.release();
     for (int k = 0; k < 3; ++k) { s->d_stage[k].release(); s->d_stage_c[k].release(); }
     s->d_out_q.release(); s->d_out_d.release();
     for (auto &e : s->ev)
