@@ -122,7 +122,8 @@ __host__ __device__ inline StageLayout stage_layout(int halo) {
     return l;
 }
 constexpr size_t kHeaderBytes = 128;                          // mbarriers
-constexpr size_t kFinBytes = (size_t)kTile * sizeof(double);  // active launch: per-pixel fp64 delta accumulators
+constexpr size_t kFinBytes = (size_t)kTile * (sizeof(double) + sizeof(float));  // active launch: per-pixel fp64
+                                                                              // contrast-weighted sums + staged contrast
 __host__ inline size_t smem_bytes(int halo, bool active) {
     return kHeaderBytes + (active ? kFinBytes : 0) + kStages * stage_layout(halo).stage_bytes;
 }
@@ -268,6 +269,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     const int span = span_px(H);
     const StageLayout L = stage_layout(H);
     double *fin = reinterpret_cast<double *>(smem + kHeaderBytes);  // active launch only: [kR][kConsumers]
+    float *cst = reinterpret_cast<float *>(fin + kTile);            // active launch only: contrast of the current kind
     unsigned char *stage0 = smem + kHeaderBytes + (ACTIVE ? kFinBytes : 0);
 
     const int tid = threadIdx.x;
@@ -391,16 +393,31 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         }
         cnt = 0;
     };
-    auto fold_kind = [&](int kind) {  // a6: post-shift contrast (I_ratio of Eq. 3) per output pixel
-        const float *ck = kind > 0 ? p.contrast[kind] : nullptr;
+    // a6: post-shift contrast (I_ratio of Eq. 3) per output pixel.  Kinds with a contrast array come first in
+    // a phase's job list (schedule_active_kernel); their fp64 sums are weighted into `fin` when the kind ends.
+    // The contrast values of the current kind are fetched with cp.async while its jobs run.
+    int rmax = 0;            // pixels r < rmax of this thread lie inside the spectrum
+    bool fin_valid = false;  // `fin` holds a weighted sum of this item
+    auto prefetch_contrast = [&](int kind) {
+        const float *ck = p.contrast[kind];
+        if (ck == nullptr) return;
+#pragma unroll
+        for (int r = 0; r < kR; ++r)
+            if (r < rmax) cp_async_4(&cst[r * kConsumers + tid], ck + m_t0 + tid + kConsumers * r);
+        cp_async_commit();
+    };
+    auto fold_kind = [&](int kind) {
+        if (p.contrast[kind] == nullptr) return;  // weight 1: keeps accumulating with the next kind
+        fold();
+        cp_async_wait_all();
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
-            const long long m = m_t0 + tid + kConsumers * r;
-            double c = 1.0;
-            if (ck != nullptr && m < p.n_pix) c = (double)__ldg(&ck[m]);
-            fin[r * kConsumers + tid] += c * tot[r];
+            const double c = r < rmax ? (double)cst[r * kConsumers + tid] : 1.0;
+            const double f = fin_valid ? fin[r * kConsumers + tid] : 0.0;
+            fin[r * kConsumers + tid] = f + c * tot[r];
             tot[r] = 0.0;
         }
+        fin_valid = true;
     };
 
     for (int n = 0;; ++n) {
@@ -425,15 +442,20 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                 if (r & 1) acc[r / 2].y = 0.f;
                 else acc[r / 2].x = 0.f;
                 tot[r] = 0.0;
-                if (ACTIVE) fin[r * kConsumers + tid] = 0.0;  // only this thread ever touches its 16 slots
             }
             cnt = 0;
-            cur_kind = kind;
+            if (ACTIVE) {
+                const long long rem = p.n_pix - (m_t0 + tid);
+                rmax = rem <= 0 ? 0 : (int)min((long long)kR, (rem + kConsumers - 1) / kConsumers);
+                fin_valid = false;  // only this thread ever touches its 16 slots of `fin` and `cst`
+                cur_kind = kind;
+                prefetch_contrast(kind);
+            }
         }
         if (ACTIVE && kind != cur_kind) {
-            fold();
             fold_kind(cur_kind);
             cur_kind = kind;
+            prefetch_contrast(kind);
         }
         for (int ri = 0; ri < n_runs; ++ri) {
             const int2 run = runs[ri];
@@ -460,33 +482,31 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             {
                 const float *wv = rs + base0 + run.y;
                 const float2 nq = bcast2(-(float)run.y);
+                float2 c = make_float2(cmf, cmf + (float)kConsumers);
 #pragma unroll
                 for (int k = 0; k < kR / 2; ++k) {
                     const float2 s0 = make_float2(wv[kConsumers * 2 * k], wv[kConsumers * (2 * k + 1)]);
                     const float2 s1 = make_float2(wv[kConsumers * 2 * k + 1], wv[kConsumers * (2 * k + 1) + 1]);
                     const float2 d = fma2(bcast2(-1.f), s0, s1);
-                    const float2 c = make_float2(cmf + (float)(kConsumers * 2 * k), cmf + (float)(kConsumers * (2 * k + 1)));
                     u[k] = fma2(nq, d, s0);
                     v[k] = fma2(c, d, bcast2(0.f));
+                    c = add2(c, bcast2((float)(2 * kConsumers)));  // rounding of c moves the shift by < 1e-6 px
                 }
             }
-            int e = run.x;
-            float2 rc = rec[e];  // {W, W a}; the next record is fetched while this one is used
-            while (e < nxt) {
-                const int nn = min(nxt - e, kFold - cnt);
+            const int len = nxt - run.x;
+            const float2 *re = rec + run.x;
+            float2 rc = re[0];  // {W, W a}; the next record is fetched while this one is used
 #pragma unroll 2
-                for (int i = 0; i < nn; ++i) {
-                    const float2 nx = rec[e + i + 1];  // one past the run's end is still inside the stage
+            for (int i = 0; i < len; ++i) {
+                const float2 nx = re[i + 1];  // one past the run's end is still inside the stage
 #pragma unroll
-                    for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.x), u[k], acc[k]);  // (1) + W u_r
+                for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.x), u[k], acc[k]);  // (1) + W u_r
 #pragma unroll
-                    for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.y), v[k], acc[k]);  // (2) + W a v_r
-                    rc = nx;
-                }
-                e += nn;
-                cnt += nn;
-                if (cnt >= kFold) fold();
+                for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.y), v[k], acc[k]);  // (2) + W a v_r
+                rc = nx;
             }
+            cnt += len;
+            if (cnt >= kFold) fold();  // at most kFold + one run's entries are ever summed in fp32
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&bar_empty[st]);  // the stage may be refilled while the tile is stored
@@ -495,11 +515,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             fold();
             if (ACTIVE) {
                 fold_kind(cur_kind);
-                float *o = p.out + (long long)out_idx * p.out_pitch;
+                float *o = p.out + (long long)out_idx * p.out_pitch + m_t0 + tid;
 #pragma unroll
                 for (int r = 0; r < kR; ++r) {
-                    const long long m = m_t0 + tid + kConsumers * r;
-                    if (m < p.n_pix) o[m] = (float)fin[r * kConsumers + tid];
+                    const double f = fin_valid ? fin[r * kConsumers + tid] : 0.0;
+                    if (r < rmax) o[kConsumers * r] = (float)(tot[r] + f);
                 }
             } else {
                 double *o = p.partial + ((long long)blockIdx.x * p.max_seg + out_idx) * kTile;
@@ -522,7 +542,8 @@ schedule_active_kernel(const int *__restrict__ seg_count /*[n_phases][3 n_mu]*/,
     const int n_seg = 3 * n_mu;
     for (int ph = threadIdx.x; ph < n_phases; ph += blockDim.x) {
         int k = 0, w = 0;
-        for (int s = 0; s < n_seg; ++s) {
+        for (int ss = 0; ss < n_seg; ++ss) {
+            const int s = (ss + n_mu) % n_seg;  // kinds 1, 2 (which may carry a contrast array), then 0
             const int gs = ph * n_seg + s;
             const int c = seg_count[gs];
             for (int off = 0; off < c; off += kJobCap) {
