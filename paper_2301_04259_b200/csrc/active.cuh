@@ -1,13 +1,18 @@
 // a4 of SURVEY section 8: per-phase active map and compaction (InfoMap of Alg. 5).
 //
 // The paper rewrites an N x N type map on the device at every timestamp.  Here the map is never
-// materialised: one thread per (phase, column) walks its column, decides each cell's type by spherical
-// angular distance with list-order override, and bins the covered cells by (mu-bin, kind) - all cells
-// of a column share one velocity - and a second kernel compacts the non-zero bins of every
-// (phase, kind, mu-bin) into the entry list the shift-interpolate-accumulate kernel consumes.
+// materialised.  One thread-block cluster of 8 CTAs per phase; CTA `rank` owns a contiguous eighth of the
+// columns the phase's regions can reach.  A warp walks a column, decides each cell's type by spherical
+// angular distance with list-order override, and bins the covered cells by (kind, mu-bin) - all cells of a
+// column share one velocity - into shared memory.  The CTAs exchange their per-segment entry counts through
+// distributed shared memory, so that each can compact its non-zero bins of every (kind, mu-bin) segment
+// behind those of the lower ranks: the entry list the shift-interpolate-accumulate kernel consumes is in
+// column order.  Rank 0 writes the phase's job list; the last phase to finish orders the phases by work.
+// One launch, no scratch to zero, no floating-point atomics (every sum has a fixed order).
 // Kinds: 0 = quiet row of a covered cell (weight -w), 1 = spot row, 2 = facula row (weight +w LB_t(mu)).
 #pragma once
 #include <cstdint>
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 
 #include "geometry.cuh"
@@ -26,114 +31,287 @@ struct LbCoef {
     double c[3][3];  // [kind][power]; kind 0 unused
 };
 
-constexpr int kBinWarps = 8;  // warps (columns) per CTA of active_bin_kernel
+struct ActiveJob {  // one job of a phase's list: <= kActiveJobCap consecutive entries of one segment
+    int begin;      // first entry (global index, even)
+    int count;      // entries, 1..kActiveJobCap
+    int kind, row;
+};
+constexpr int kActiveJobCap = 128;      // == f32::kJobCap
+constexpr int kPrepCluster = 8;         // CTAs per phase (portable cluster size)
+constexpr int kPrepThreads = 512;       // 16 warps per CTA
+constexpr int kPrepChunks = 4;          // 32-row chunks of a column whose cell data is loaded together
+constexpr int kScheduleSortMax = 4096;  // beyond this many phases the order is left as given
 
-// grid: (ceil(N/kBinWarps), n_phases); one warp per (phase, column), lanes over the rows (coalesced).
-// WD: [n_phases][3][n_mu][ncap] fp64, pre-zeroed.  Cells of equal (mu-bin, type) are contiguous in a
-// column: segmented warp scans, added to WD in row order by one lane at a time (deterministic).
-__global__ void __launch_bounds__(32 * kBinWarps)
-active_bin_kernel(int N, int n_regions, int n_mu, int ncap, const RegionAtPhase *__restrict__ rp /*[n_phases][n_regions]*/,
-                  const double *__restrict__ mu, const double *__restrict__ w, const int *__restrict__ bin, LbCoef lb,
-                  double *__restrict__ WD, int *__restrict__ n_active /*[n_phases]*/) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int j = blockIdx.x * kBinWarps + warp;
-    const int p = blockIdx.y;
-    if (j >= N) return;
-    const RegionAtPhase *reg = rp + (size_t)p * n_regions;
-    const double x = cell_coord(j, N);
-    // rows of this column that any region can reach (conservative: chord bound, slightly inflated)
-    double ylo = 2.0, yhi = -2.0;
-    for (int r = 0; r < n_regions; ++r) {
-        if (reg[r].type == 0) continue;
-        const double ch = reg[r].chord * (1.0 + 1e-9) + 1e-12;
-        if (fabs(x - reg[r].xr) > ch) continue;
-        ylo = fmin(ylo, reg[r].yr - ch);
-        yhi = fmax(yhi, reg[r].yr + ch);
-    }
-    if (ylo > yhi) return;
-    int i_lo = (int)floor((ylo + 1.0) * 0.5 * N - 0.5) - 1;
-    int i_hi = (int)ceil((yhi + 1.0) * 0.5 * N - 0.5) + 1;
-    i_lo = max(i_lo, 0);
-    i_hi = min(i_hi, N - 1);
-    double *WDp = WD + (size_t)p * 3 * n_mu * ncap;
-    int count = 0;
-    for (int i0 = i_lo; i0 <= i_hi; i0 += 32) {
-        const int i = i0 + lane;
-        int b = -1, t = 0;
-        double wc = 0.0, wl = 0.0;
-        if (i <= i_hi) {
-            const size_t c = (size_t)j * N + i;
-            b = bin[c];
-            if (b >= 0) {
-                const double y = cell_coord(i, N), m = mu[c];
-                for (int r = 0; r < n_regions; ++r) {  // list order: the last covering region wins
-                    if (reg[r].type == 0) continue;
-                    const double dot =
-                        __dadd_rn(__dadd_rn(__dmul_rn(x, reg[r].xr), __dmul_rn(y, reg[r].yr)), __dmul_rn(m, reg[r].zr));
-                    if (dot >= reg[r].cos_alpha) t = reg[r].type;
-                }
-                if (t != 0) {
-                    wc = w[c];
-                    wl = wc * (lb.c[t][0] + lb.c[t][1] * m + lb.c[t][2] * m * m);
-                }
-            }
-        }
-        const int key = (t != 0) ? (b * 4 + t) : -1;
-        int start;
-        bool tail;
-        const double seg_w = warp_segmented_scan(wc, key, lane, start, tail);
-        const double seg_wl = warp_segmented_scan(wl, key, lane, start, tail);
-        unsigned tails = __ballot_sync(0xffffffffu, tail && t != 0);
-        while (tails) {
-            const int l = __ffs(tails) - 1;
-            if (lane == l) {
-                WDp[((size_t)0 * n_mu + b) * ncap + j] += seg_w;
-                WDp[((size_t)t * n_mu + b) * ncap + j] += seg_wl;
-            }
-            __syncwarp();
-            tails &= tails - 1;
-        }
-        count += __popc(__ballot_sync(0xffffffffu, t != 0));
-    }
-    if (lane == 0 && count) atomicAdd(&n_active[p], count);  // integer: order-independent
+struct ActiveCounters {  // device-resident
+    unsigned long long active_entries;  // sum over phases of entries (pad entries not counted)
+    unsigned int done;                  // CTAs finished (reset by the last one)
+    unsigned int pad;
+};
+
+struct PrepArgs {
+    int N, n_regions, n_mu, seg_cap, chunk_cols, job_cap, n_phases;
+    const RegionAtPhase *rp;  // [n_phases][n_regions]
+    const double *mu, *w, *col_a;
+    const int *bin;
+    LbCoef lb;
+    void *ent;                // [n_phases * 3 n_mu][seg_cap] of EntT
+    int *seg_count;           // [n_phases * 3 n_mu]
+    int *n_active;            // [n_phases] covered cells
+    ActiveJob *jobs;          // [n_phases][job_cap]
+    int *n_jobs, *work, *phase_order;  // [n_phases] each
+    ActiveCounters *counters;
+};
+
+__host__ __device__ inline size_t prep_smem_bytes(int n_mu, int chunk_cols) {
+    return (size_t)3 * n_mu * chunk_cols * sizeof(double) + (size_t)3 * 3 * n_mu * sizeof(int) + 64;
 }
 
-// One warp per (phase, kind, mu-bin) segment: ordered compaction of the non-zero columns into
-// entries (a_j, +-W).  Segment s = (p*3 + kind)*n_mu + b owns ent[s*ncap .. s*ncap + ncap); counts are
-// padded to even with a zero-weight entry.  EntT = float2 or double2.
+
+// grid = n_phases * kPrepCluster, block = kPrepThreads, cluster = kPrepCluster CTAs;
+// dynamic shared memory = prep_smem_bytes(n_mu, chunk_cols) with chunk_cols >= ceil(N / kPrepCluster).
 template <typename EntT>
-__global__ void active_compact_kernel(int N, int n_mu, int ncap, int n_segments,
-                                      const double *__restrict__ col_a, const double *__restrict__ WD,
-                                      EntT *__restrict__ ent, int *__restrict__ seg_count,
-                                      unsigned long long *__restrict__ total_entries) {
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (warp >= n_segments) return;
-    const int kind = (warp / n_mu) % 3;
-    const double sign = (kind == 0) ? -1.0 : 1.0;
-    const double *src = WD + (size_t)warp * ncap;
-    EntT *dst = ent + (size_t)warp * ncap;
-    int pos = 0;
-    for (int j0 = 0; j0 < N; j0 += 32) {
-        const int j = j0 + lane;
-        const double W = (j < N) ? src[j] : 0.0;
-        const unsigned m = __ballot_sync(0xffffffffu, W != 0.0);
-        if (W != 0.0) {
-            EntT e;
-            e.x = (decltype(e.x))col_a[j];
-            e.y = (decltype(e.y))(sign * W);
-            dst[pos + __popc(m & ((1u << lane) - 1u))] = e;
-        }
-        pos += __popc(m);
+__global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThreads) active_prepare_kernel(const PrepArgs a) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    extern __shared__ __align__(16) unsigned char prep_smem[];
+    const int n_seg = 3 * a.n_mu, N = a.N, cc = a.chunk_cols;
+    double *WDs = reinterpret_cast<double *>(prep_smem);           // [n_seg][cc]: this CTA's columns
+    int *cnt = reinterpret_cast<int *>(WDs + (size_t)n_seg * cc);   // [n_seg] entries of this CTA (read by the others)
+    int *off = cnt + n_seg;                                         // [n_seg] entries of the lower ranks
+    int *tot = off + n_seg;                                         // [n_seg] entries of the whole phase
+    int *s_misc = tot + n_seg;  // j_lo, j_hi, covered cells of this CTA (read by rank 0), last-phase flag
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = kPrepThreads / 32;
+    const int p = blockIdx.x / kPrepCluster;
+    const int rank = (int)cluster.block_rank();
+    const RegionAtPhase *reg = a.rp + (size_t)p * a.n_regions;
+    EntT *ent = static_cast<EntT *>(a.ent) + (size_t)p * n_seg * a.seg_cap;
+
+    if (tid == 0) {
+        s_misc[0] = N;
+        s_misc[1] = -1;
+        s_misc[2] = 0;
+        s_misc[3] = 0;
     }
-    if (lane == 0) {
-        if (pos & 1) {
+    __syncthreads();
+    // columns any region of this phase can reach (conservative: chord bound, slightly inflated)
+    for (int r = tid; r < a.n_regions; r += kPrepThreads) {
+        if (reg[r].type == 0) continue;
+        const double ch = reg[r].chord * (1.0 + 1e-9) + 1e-12;
+        int jl = (int)floor((reg[r].xr - ch + 1.0) * 0.5 * N - 0.5) - 1;
+        int jh = (int)ceil((reg[r].xr + ch + 1.0) * 0.5 * N - 0.5) + 1;
+        atomicMin(&s_misc[0], max(jl, 0));
+        atomicMax(&s_misc[1], min(jh, N - 1));
+    }
+    __syncthreads();
+    const int j_lo = s_misc[0], j_hi = s_misc[1];
+    const int per = (j_hi >= j_lo) ? (j_hi - j_lo + kPrepCluster) / kPrepCluster : 0;  // columns per CTA, <= cc
+    const int c0 = j_lo + rank * per;
+    const int cols = max(0, min(per, j_hi + 1 - c0));
+
+    for (int s = warp; s < n_seg; s += n_warps)
+        for (int k = lane; k < cols; k += 32) WDs[(size_t)s * cc + k] = 0.0;
+    __syncthreads();
+    // ---- bin: one warp per column, lanes over the rows (coalesced) --------------------------------------
+    for (int j = c0 + warp; j < c0 + cols; j += n_warps) {
+        const double x = cell_coord(j, N);
+        double ylo = 2.0, yhi = -2.0;
+        for (int r = 0; r < a.n_regions; ++r) {
+            if (reg[r].type == 0) continue;
+            const double ch = reg[r].chord * (1.0 + 1e-9) + 1e-12;
+            if (fabs(x - reg[r].xr) > ch) continue;
+            ylo = fmin(ylo, reg[r].yr - ch);
+            yhi = fmax(yhi, reg[r].yr + ch);
+        }
+        if (ylo > yhi) continue;
+        int i_lo = (int)floor((ylo + 1.0) * 0.5 * N - 0.5) - 1;
+        int i_hi = (int)ceil((yhi + 1.0) * 0.5 * N - 0.5) + 1;
+        i_lo = max(i_lo, 0);
+        i_hi = min(i_hi, N - 1);
+        double *col = WDs + (j - c0);
+        int count = 0;
+        for (int i00 = i_lo; i00 <= i_hi; i00 += 32 * kPrepChunks) {
+            // all loads of up to kPrepChunks chunks are issued before any is used: one memory round trip
+            int bb[kPrepChunks];
+            double mm[kPrepChunks], ww[kPrepChunks];
+#pragma unroll
+            for (int k = 0; k < kPrepChunks; ++k) {
+                const int i = i00 + 32 * k + lane;
+                const bool in = i <= i_hi;
+                const size_t c = (size_t)j * N + (in ? i : i_hi);
+                bb[k] = in ? a.bin[c] : -1;  // hidden cells: bin -1, mu 0, w 0
+                mm[k] = a.mu[c];
+                ww[k] = a.w[c];
+            }
+#pragma unroll
+            for (int k = 0; k < kPrepChunks; ++k) {
+                if (i00 + 32 * k > i_hi) break;
+                const int i = i00 + 32 * k + lane;
+                const int b = bb[k];
+                const double m = mm[k];
+                int t = 0;
+                double wc = 0.0, wl = 0.0;
+                if (b >= 0) {
+                    const double y = cell_coord(i, N);
+                    for (int r = 0; r < a.n_regions; ++r) {  // list order: the last covering region wins
+                        if (reg[r].type == 0) continue;
+                        const double dot = __dadd_rn(__dadd_rn(__dmul_rn(x, reg[r].xr), __dmul_rn(y, reg[r].yr)),
+                                                     __dmul_rn(m, reg[r].zr));
+                        if (dot >= reg[r].cos_alpha) t = reg[r].type;
+                    }
+                    if (t != 0) {
+                        wc = ww[k];
+                        wl = wc * (a.lb.c[t][0] + a.lb.c[t][1] * m + a.lb.c[t][2] * m * m);
+                    }
+                }
+                // cells of equal (mu-bin, type) are contiguous in a column: segmented scans, added in row order
+                const int key = (t != 0) ? (b * 4 + t) : -1;
+                int start;
+                bool tail;
+                const double seg_w = warp_segmented_scan(wc, key, lane, start, tail);
+                const double seg_wl = warp_segmented_scan(wl, key, lane, start, tail);
+                unsigned tails = __ballot_sync(0xffffffffu, tail && t != 0);
+                while (tails) {
+                    const int l = __ffs(tails) - 1;
+                    if (lane == l) {
+                        col[(size_t)(0 * a.n_mu + b) * cc] += seg_w;
+                        col[(size_t)(t * a.n_mu + b) * cc] += seg_wl;
+                    }
+                    __syncwarp();
+                    tails &= tails - 1;
+                }
+                count += __popc(__ballot_sync(0xffffffffu, t != 0));
+            }
+        }
+        if (lane == 0 && count) atomicAdd(&s_misc[2], count);  // integer: order-independent
+    }
+    __syncthreads();
+    // ---- count this CTA's entries per segment, exchange through distributed shared memory ------------------
+    for (int s = warp; s < n_seg; s += n_warps) {
+        const double *src = WDs + (size_t)s * cc;
+        int c = 0;
+        for (int k0 = 0; k0 < cols; k0 += 32) {
+            const int k = k0 + lane;
+            c += __popc(__ballot_sync(0xffffffffu, k < cols && src[k] != 0.0));
+        }
+        if (lane == 0) cnt[s] = c;
+    }
+    cluster.sync();
+    for (int s = tid; s < n_seg; s += kPrepThreads) {
+        int before = 0, all = 0;
+        for (int r = 0; r < kPrepCluster; ++r) {
+            const int c = cluster.map_shared_rank(cnt, r)[s];
+            before += r < rank ? c : 0;
+            all += c;
+        }
+        off[s] = before;
+        tot[s] = all;
+    }
+    int covered = 0;
+    if (rank == 0 && tid == 0)
+        for (int r = 0; r < kPrepCluster; ++r) covered += cluster.map_shared_rank(s_misc, r)[2];
+    cluster.sync();  // no CTA leaves (or goes on to change cnt) while its shared memory is being read
+    // ---- compact: one warp per segment, this CTA's columns in order, behind the lower ranks' entries -------
+    for (int s = warp; s < n_seg; s += n_warps) {
+        const double sign = (s < a.n_mu) ? -1.0 : 1.0;
+        const double *src = WDs + (size_t)s * cc;
+        int ps = off[s];
+        EntT *dst = ent + (size_t)s * a.seg_cap;
+        for (int k0 = 0; k0 < cols; k0 += 32) {
+            const int k = k0 + lane;
+            const double W = (k < cols) ? src[k] : 0.0;
+            const unsigned m = __ballot_sync(0xffffffffu, W != 0.0);
+            if (W != 0.0) {
+                EntT e;
+                e.x = (decltype(e.x))a.col_a[c0 + k];
+                e.y = (decltype(e.y))(sign * W);
+                dst[ps + __popc(m & ((1u << lane) - 1u))] = e;
+            }
+            ps += __popc(m);
+        }
+    }
+    if (rank != 0) return;
+    // ---- rank 0 finalises the phase: pad odd segments, counts, job list (contrast-carrying kinds 1, 2 first)
+    for (int s = tid; s < n_seg; s += kPrepThreads) {
+        const int c = tot[s];
+        if (c & 1) {  // zero-weight pad entry: every job's entry block stays a multiple of 16 bytes
             EntT z;
             z.x = 0;
             z.y = 0;
-            dst[pos] = z;
+            ent[(size_t)s * a.seg_cap + c] = z;
         }
-        seg_count[warp] = pos;
-        if (pos) atomicAdd(total_entries, (unsigned long long)pos);
+        a.seg_count[p * n_seg + s] = c;
+    }
+    if (warp == 0) {
+        // lane l takes the segments ss in [l per_lane, (l+1) per_lane) of the job order; jobs are numbered by an
+        // exclusive warp scan of the lanes' job counts
+        const int per_lane = (n_seg + 31) / 32;
+        const int ss0 = lane * per_lane, ss1 = min(n_seg, ss0 + per_lane);
+        int nj = 0, wsum = 0;
+        for (int ss = ss0; ss < ss1; ++ss) {
+            const int c = tot[(ss + a.n_mu) % n_seg];
+            nj += (c + kActiveJobCap - 1) / kActiveJobCap;
+            wsum += c;
+        }
+        int incl = nj;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        int k = incl - nj;
+        for (int ss = ss0; ss < ss1; ++ss) {
+            const int s = (ss + a.n_mu) % n_seg;
+            const int c = tot[s];
+            for (int o = 0; o < c; o += kActiveJobCap) {
+                ActiveJob jb;
+                jb.begin = (p * n_seg + s) * a.seg_cap + o;  // fits: host checks n_phases * 3 n_mu * seg_cap < 2^31
+                jb.count = min(kActiveJobCap, c - o);
+                jb.kind = s / a.n_mu;
+                jb.row = s - jb.kind * a.n_mu;
+                a.jobs[(size_t)p * a.job_cap + k++] = jb;
+            }
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) wsum += __shfl_xor_sync(0xffffffffu, wsum, d);
+        const int n_jobs_total = __shfl_sync(0xffffffffu, incl, 31);
+        if (lane == 0) {
+            a.n_jobs[p] = n_jobs_total;
+            a.work[p] = wsum;
+            a.n_active[p] = covered;
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned ticket = atomicAdd(&a.counters->done, 1u);
+        s_misc[3] = (ticket == (unsigned)a.n_phases - 1u) ? 1 : 0;
+    }
+    __syncthreads();
+    if (!s_misc[3]) return;
+    // ---- last phase to finish: order the phases by work, heaviest first (ties by phase index: deterministic)
+    __threadfence();
+    const volatile int *work = a.work;
+    for (int ph = tid; ph < a.n_phases; ph += kPrepThreads) {
+        int rk = ph;
+        if (a.n_phases <= kScheduleSortMax) {
+            const int w = work[ph];
+            rk = 0;
+            for (int q = 0; q < a.n_phases; ++q) {
+                const int wq = work[q];
+                rk += (wq > w || (wq == w && q < ph)) ? 1 : 0;
+            }
+        }
+        a.phase_order[rk] = ph;
+    }
+    if (warp == 0) {
+        unsigned long long total = 0;
+        for (int ph = lane; ph < a.n_phases; ph += 32) total += (unsigned long long)work[ph];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) total += __shfl_xor_sync(0xffffffffu, total, d);
+        if (lane == 0) {
+            a.counters->active_entries = total;
+            a.counters->done = 0;  // ready for the next call on this handle
+        }
     }
 }
 

@@ -78,28 +78,25 @@ __device__ __forceinline__ double warp_segmented_scan(double v, int key, int lan
     return v;
 }
 
-constexpr int kGeomWarps = 8;  // warps (columns) per CTA of geometry_kernel
+constexpr int kGeomWarps = 32;  // warps (columns) per CTA of geometry_kernel
 
-// a1 + a2.  One warp per column j, lanes over the rows i (coalesced): every cell's (mu, w, v, bin), the
-// column's shift factor a_j = D_j - 1 (all cells of a column share one velocity under solid-body
-// rotation), its binned weights W[j][b] (segmented warp scans added in row order: deterministic), and
-// its visible-cell count / weight sum.
-__global__ void __launch_bounds__(32 * kGeomWarps)
-geometry_kernel(int N, double vsini_sini, double u1, double u2, int mode, int n_mu,
-                const double *__restrict__ mu_centres, double *__restrict__ mu_out, double *__restrict__ w_out,
-                double *__restrict__ vel_out, int *__restrict__ bin_out, double *__restrict__ col_a,
-                double *__restrict__ Wbin /*[N][n_mu]*/, double *__restrict__ col_sumw, int *__restrict__ col_nvis) {
-    __shared__ double s_W[kGeomWarps][64];
-    __shared__ double s_mu[64];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int b = threadIdx.x; b < n_mu; b += blockDim.x) s_mu[b] = mu_centres[b];
-    for (int b = lane; b < 64; b += 32) s_W[warp][b] = 0.0;
-    __syncthreads();
-    const int j = blockIdx.x * kGeomWarps + warp;
-    if (j >= N) return;
-    double sum = 0.0;
-    int nvis = 0;
-    for (int i0 = 0; i0 < N; i0 += 32) {
+struct MuCentres {  // passed by value as a kernel argument: no host -> device copy per call
+    double v[64];
+};
+
+
+
+// One warp, one column j, the 32-row chunks `chunk`, `chunk + stride`, ...: writes the cells' (mu, w, v, bin)
+// and adds the chunk's binned weights to s_W[64] (segmented warp scans, added in row order), returning
+// the warp's weight sum and visible-cell count.
+__device__ __forceinline__ void geometry_chunks(int j, int chunk, int stride, int N, double vsini_sini, double u1, double u2,
+                                                int n_mu, const double *s_mu, double *s_W, double *__restrict__ mu_out,
+                                                double *__restrict__ w_out, double *__restrict__ vel_out,
+                                                int *__restrict__ bin_out, double &sum, int &nvis) {
+    const int lane = threadIdx.x & 31;
+    sum = 0.0;
+    nvis = 0;
+    for (int i0 = 32 * chunk; i0 < N; i0 += 32 * stride) {
         const int i = i0 + lane;
         double mu = 0.0, w = 0.0, v = 0.0;
         int bin = -1;
@@ -117,7 +114,7 @@ geometry_kernel(int N, double vsini_sini, double u1, double u2, int mode, int n_
         unsigned tails = __ballot_sync(0xffffffffu, tail && bin >= 0);
         while (tails) {  // segments of one bin may repeat inside a chunk (apex of the column): add in lane order
             const int l = __ffs(tails) - 1;
-            if (lane == l) s_W[warp][bin] += seg;
+            if (lane == l) s_W[bin] += seg;
             __syncwarp();
             tails &= tails - 1;
         }
@@ -127,35 +124,31 @@ geometry_kernel(int N, double vsini_sini, double u1, double u2, int mode, int n_
         sum += cs;
         nvis += __popc(__ballot_sync(0xffffffffu, bin >= 0));
     }
-    for (int b = lane; b < n_mu; b += 32) Wbin[(size_t)j * n_mu + b] = s_W[warp][b];
-    if (lane == 0) {
-        col_a[j] = doppler_minus_one(__dmul_rn(cell_coord(j, N), vsini_sini), mode);
-        col_sumw[j] = sum;
-        col_nvis[j] = nvis;
-    }
 }
 
 // Single CTA: compacts the non-zero W[j][b] into the entry list of the pre-binned form, sorted by
 // (row b, column j), each row padded with a zero-weight entry to an even length so that every row
 // starts 16-byte aligned for the TMA bulk copy; writes row_start[n_mu+1] and the summary.
 // Entries are (a_j, W) in fp32 (float2) and fp64 (double2).
-__global__ void build_binned_entries_kernel(int N, int n_mu, const double *__restrict__ col_a,
-                                            const double *__restrict__ Wbin,
-                                            const double *__restrict__ col_sumw,
-                                            const int *__restrict__ col_nvis, float2 *__restrict__ ent32,
-                                            double2 *__restrict__ ent64, int *__restrict__ row_start,
-                                            DevInfo *__restrict__ info) {
+__device__ void build_binned_entries(int N, int n_mu, const double *col_a, const double *Wbin, const double *col_sumw,
+                                     const int *col_nvis, float2 *ent32, double2 *ent64, int *row_start, DevInfo *info) {
     __shared__ int s_cnt[64];
     __shared__ int s_start[65];
     __shared__ int s_nv[1024];  // blockDim.x == 1024 (a power of two); N <= 8192 so N^2 fits an int
     __shared__ double s_sw[1024], s_am[1024];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+    constexpr int kBatch = 8;  // loads of 8 x 32 columns are issued together: one memory round trip per batch
     for (int b = warp; b < n_mu; b += n_warps) {
         int cnt = 0;
-        for (int j0 = 0; j0 < N; j0 += 32) {
-            const int j = j0 + lane;
-            const bool nz = (j < N) && (Wbin[(size_t)j * n_mu + b] != 0.0);
-            cnt += __popc(__ballot_sync(0xffffffffu, nz));
+        for (int j0 = 0; j0 < N; j0 += 32 * kBatch) {
+            double W[kBatch];
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) {
+                const int j = j0 + 32 * k + lane;
+                W[k] = (j < N) ? Wbin[(size_t)j * n_mu + b] : 0.0;
+            }
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) cnt += __popc(__ballot_sync(0xffffffffu, W[k] != 0.0));
         }
         if (lane == 0) s_cnt[b] = cnt;
     }
@@ -200,23 +193,103 @@ __global__ void build_binned_entries_kernel(int N, int n_mu, const double *__res
     for (int b = threadIdx.x; b <= n_mu; b += blockDim.x) row_start[b] = s_start[b];
     for (int b = warp; b < n_mu; b += n_warps) {
         int pos = s_start[b];
-        for (int j0 = 0; j0 < N; j0 += 32) {
-            const int j = j0 + lane;
-            const double W = (j < N) ? Wbin[(size_t)j * n_mu + b] : 0.0;
-            const unsigned m = __ballot_sync(0xffffffffu, W != 0.0);
-            if (W != 0.0) {
-                const int k = pos + __popc(m & ((1u << lane) - 1u));
-                const double a = col_a[j];
-                ent32[k] = make_float2((float)a, (float)W);
-                ent64[k] = make_double2(a, W);
+        for (int j0 = 0; j0 < N; j0 += 32 * kBatch) {
+            double W[kBatch], A[kBatch];
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) {
+                const int j = j0 + 32 * k + lane;
+                W[k] = (j < N) ? Wbin[(size_t)j * n_mu + b] : 0.0;
+                A[k] = (j < N) ? col_a[j] : 0.0;
             }
-            pos += __popc(m);
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) {
+                const unsigned m = __ballot_sync(0xffffffffu, W[k] != 0.0);
+                if (W[k] != 0.0) {
+                    const int e = pos + __popc(m & ((1u << lane) - 1u));
+                    ent32[e] = make_float2((float)A[k], (float)W[k]);
+                    ent64[e] = make_double2(A[k], W[k]);
+                }
+                pos += __popc(m);
+            }
         }
         if (lane == 0 && (s_cnt[b] & 1)) {
             ent32[pos] = make_float2(0.f, 0.f);
             ent64[pos] = make_double2(0.0, 0.0);
         }
     }
+}
+
+// a1 + a2.  The fp64 geometry of a cell costs a few hundred instructions, so the cells are spread over the
+// whole GPU: a CTA of 32 warps takes `cols_per_cta` columns, a warp takes one 32-row chunk of one column
+// (or several, strided, when a column has more chunks than the CTA has warps per column).  Per column:
+// every cell's (mu, w, v, bin), the shift factor a_j = D_j - 1 (all cells of a column share one velocity
+// under solid-body rotation), the binned weights W[j][b] (per-warp partial sums added in warp order:
+// deterministic) and the visible-cell count / weight sum.  The last CTA to finish compacts the binned
+// weights into the entry list (build_binned_entries), so a1 + a2 are one launch.  `done` is zero on entry
+// and is left zero.
+__host__ __device__ inline int geom_warps_per_col(int N) {
+    const int nc = (N + 31) / 32;
+    return nc < kGeomWarps ? nc : kGeomWarps;
+}
+__host__ __device__ inline int geom_cols_per_cta(int N) { return kGeomWarps / geom_warps_per_col(N); }
+
+__global__ void __launch_bounds__(32 * kGeomWarps)
+geometry_kernel(int N, double vsini_sini, double u1, double u2, int mode, int n_mu, const MuCentres mu_centres,
+                double *__restrict__ mu_out, double *__restrict__ w_out, double *__restrict__ vel_out,
+                int *__restrict__ bin_out, double *__restrict__ col_a, double *__restrict__ Wbin /*[N][n_mu]*/,
+                double *__restrict__ col_sumw, int *__restrict__ col_nvis, float2 *__restrict__ ent32,
+                double2 *__restrict__ ent64, int *__restrict__ row_start, DevInfo *__restrict__ info,
+                unsigned int *__restrict__ done) {
+    __shared__ double s_W[kGeomWarps][64];
+    __shared__ double s_mu[64];
+    __shared__ double s_sum[kGeomWarps];
+    __shared__ int s_nvis[kGeomWarps];
+    __shared__ int s_last;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int b = threadIdx.x; b < n_mu; b += blockDim.x) s_mu[b] = mu_centres.v[b];
+    for (int b = lane; b < 64; b += 32) s_W[warp][b] = 0.0;
+    __syncthreads();
+    const int wpc = geom_warps_per_col(N), cpc = kGeomWarps / wpc;
+    const int cl = warp / wpc, chunk = warp - cl * wpc;  // local column, first chunk
+    const int j = blockIdx.x * cpc + cl;
+    double sum = 0.0;
+    int nvis = 0;
+    if (cl < cpc && j < N)
+        geometry_chunks(j, chunk, wpc, N, vsini_sini, u1, u2, n_mu, s_mu, s_W[warp], mu_out, w_out, vel_out, bin_out, sum, nvis);
+    if (lane == 0) {
+        s_sum[warp] = sum;
+        s_nvis[warp] = nvis;
+    }
+    __syncthreads();
+    if (warp < cpc) {  // warp `warp` finishes local column `warp`
+        const int jj = blockIdx.x * cpc + warp;
+        if (jj < N) {
+            for (int b = lane; b < n_mu; b += 32) {
+                double W = 0.0;
+                for (int k = 0; k < wpc; ++k) W += s_W[warp * wpc + k][b];
+                Wbin[(size_t)jj * n_mu + b] = W;
+            }
+            if (lane == 0) {
+                double sw = 0.0;
+                int nv = 0;
+                for (int k = 0; k < wpc; ++k) {
+                    sw += s_sum[warp * wpc + k];
+                    nv += s_nvis[warp * wpc + k];
+                }
+                col_a[jj] = doppler_minus_one(__dmul_rn(cell_coord(jj, N), vsini_sini), mode);
+                col_sumw[jj] = sw;
+                col_nvis[jj] = nv;
+            }
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(done, 1u) == gridDim.x - 1) ? 1 : 0;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (threadIdx.x == 0) *done = 0;
+    build_binned_entries(N, n_mu, col_a, Wbin, col_sumw, col_nvis, ent32, ent64, row_start, info);
 }
 
 // SOAP_FORM_CELLS: one entry per visible cell (the literal double loop of Alg. 1), same layout.

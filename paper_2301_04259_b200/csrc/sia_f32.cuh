@@ -38,7 +38,7 @@
 //     CTA, grid = resident CTA slots (one wave, no tail); a CTA writes one fp64 partial per tile it
 //     touches and reduce_ranges_kernel adds the partials of a tile in CTA order (deterministic).
 //   * active launch: persistent CTAs; the (phase, tile) items, heaviest phase first, are dealt to the
-//     CTAs in snake order (schedule_active_kernel builds the per-phase job lists and the order); the
+//     CTAs in snake order (active_prepare_kernel builds the per-phase job lists and the order); the
 //     post-shift contrast (I_ratio of Eq. 3) multiplies each kind's fp64 sum once per pixel (a6).
 #pragma once
 #include <climits>
@@ -46,6 +46,7 @@
 #include <type_traits>
 #include <cuda_runtime.h>
 
+#include "active.cuh"
 #include "ptx_helpers.cuh"
 
 namespace soap {
@@ -58,7 +59,7 @@ constexpr int kThreads = kConsumers + 32 * kProducerWarps;  // two warpgroups
 constexpr int kR = 16;                                      // pixels per consumer thread
 constexpr int kTile = kConsumers * kR;                      // pixels per tile
 constexpr int kStages = kProducerWarps;                     // jobs in flight: stage k belongs to producer warp k
-constexpr int kJobCap = 128;                                // entries per job (even)
+constexpr int kJobCap = kActiveJobCap;                      // entries per job (even)
 constexpr int kFold = 64;                                   // fp32 -> fp64 fold interval (entries)
 constexpr int kFlip = INT_MIN;                              // run marker: per-pixel path
 constexpr int kCtasPerSm = 3;
@@ -66,12 +67,6 @@ constexpr int kRegsConsumer = 120, kRegsProducer = 40;      // (120 + 40) * 128 
 static_assert(kConsumerWarps == 4 && kProducerWarps == 4, "setmaxnreg acts on aligned groups of 4 warps");
 
 enum : int { kJobFirst = 1, kJobLast = 2, kJobExit = 4 };
-
-struct ActiveJob {  // one job of a phase's list (schedule_active_kernel)
-    int begin;      // first entry (global index, even)
-    int count;      // entries, 1..kJobCap
-    int kind, row;
-};
 
 struct Params {
     const float *base[3];      // spectrum tables per kind (quiet launch: base[0] only)
@@ -394,7 +389,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         cnt = 0;
     };
     // a6: post-shift contrast (I_ratio of Eq. 3) per output pixel.  Kinds with a contrast array come first in
-    // a phase's job list (schedule_active_kernel); their fp64 sums are weighted into `fin` when the kind ends.
+    // a phase's job list (active_prepare_kernel); their fp64 sums are weighted into `fin` when the kind ends.
     // The contrast values of the current kind are fetched with cp.async while its jobs run.
     int rmax = 0;            // pixels r < rmax of this thread lie inside the spectrum
     bool fin_valid = false;  // `fin` holds a weighted sum of this item
@@ -527,50 +522,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                 for (int r = 0; r < kR; ++r) o[tid + kConsumers * r] = tot[r];
             }
         }
-    }
-}
-
-// a4 -> a5 hand-over: turns the per-(phase, kind, mu-bin) segment counts of active_compact_kernel into each
-// phase's job list (chunks of <= kJobCap entries of one segment) and orders the phases by work, heaviest
-// first (ties by phase index: deterministic).  One CTA; n_phases is at most a few thousand.
-constexpr int kScheduleThreads = 1024;
-constexpr int kScheduleSortMax = 4096;  // beyond this many phases the order is left as given
-__global__ void __launch_bounds__(kScheduleThreads)
-schedule_active_kernel(const int *__restrict__ seg_count /*[n_phases][3 n_mu]*/, int n_phases, int n_mu, int seg_cap,
-                       int job_cap, ActiveJob *__restrict__ jobs, int *__restrict__ n_jobs, int *__restrict__ phase_order,
-                       int *__restrict__ work) {
-    const int n_seg = 3 * n_mu;
-    for (int ph = threadIdx.x; ph < n_phases; ph += blockDim.x) {
-        int k = 0, w = 0;
-        for (int ss = 0; ss < n_seg; ++ss) {
-            const int s = (ss + n_mu) % n_seg;  // kinds 1, 2 (which may carry a contrast array), then 0
-            const int gs = ph * n_seg + s;
-            const int c = seg_count[gs];
-            for (int off = 0; off < c; off += kJobCap) {
-                ActiveJob j;
-                j.begin = gs * seg_cap + off;  // fits: host checks n_phases * 3 n_mu * seg_cap < 2^31
-                j.count = min(kJobCap, c - off);
-                j.kind = s / n_mu;
-                j.row = s - j.kind * n_mu;
-                jobs[(size_t)ph * job_cap + k++] = j;
-            }
-            w += c;
-        }
-        n_jobs[ph] = k;
-        work[ph] = w;
-    }
-    __syncthreads();
-    for (int ph = threadIdx.x; ph < n_phases; ph += blockDim.x) {
-        int rank = ph;
-        if (n_phases <= kScheduleSortMax) {
-            const int w = work[ph];
-            rank = 0;
-            for (int q = 0; q < n_phases; ++q) {
-                const int wq = work[q];
-                rank += (wq > w || (wq == w && q < ph)) ? 1 : 0;
-            }
-        }
-        phase_order[rank] = ph;
     }
 }
 

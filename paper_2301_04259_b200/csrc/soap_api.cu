@@ -45,11 +45,6 @@ struct DevBuf {
     }
 };
 
-struct Counters {  // device-resident, read back by soap_get_stats
-    unsigned long long active_entries;
-    unsigned long long pad;
-};
-
 }  // namespace
 
 struct soap_star {
@@ -70,11 +65,12 @@ struct soap_star {
     bool ev_valid[2] = {false, false};
 
     // geometry (device)
-    DevBuf<double> d_mu_centres, d_mu, d_w, d_vel, d_col_a, d_Wbin, d_col_sumw;
+    DevBuf<double> d_mu, d_w, d_vel, d_col_a, d_Wbin, d_col_sumw;
     DevBuf<int> d_bin, d_col_nvis, d_row_start;
     DevBuf<float2> d_ent32;
     DevBuf<double2> d_ent64;
     DevBuf<DevInfo> d_info;
+    DevBuf<unsigned int> d_geom_done;
     size_t ent_cap = 0;
 
     // quiet scratch
@@ -89,11 +85,10 @@ struct soap_star {
         bool in_flight = false;
     } h_rp[4];
     int h_rp_next = 0;
-    DevBuf<double> d_WD;
     DevBuf<unsigned char> d_aent;
     DevBuf<int> d_segcnt, d_nactive, d_sched;
-    DevBuf<f32::ActiveJob> d_jobs;
-    DevBuf<Counters> d_counters;
+    DevBuf<ActiveJob> d_jobs;
+    DevBuf<ActiveCounters> d_counters;
 
     // host-buffer staging (soap_synthesize_host)
     DevBuf<unsigned char> d_stage[3], d_stage_c[3], d_out_q, d_out_d;
@@ -299,40 +294,50 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
     const int ncap = ((N + 1) & ~1) + 2;
     const long long n_seg = (long long)n_phases * 3 * n_mu;
     if (n_seg * ncap >= (1LL << 31)) return s->fail(SOAP_ERR_UNSUPPORTED, "n_phases * 3 * n_mu * N too large for one call");
-    SOAP_CUDA(s, s->d_WD.reserve((size_t)n_seg * ncap));
     SOAP_CUDA(s, s->d_aent.reserve((size_t)n_seg * ncap * sizeof(Ent) + 64));
     SOAP_CUDA(s, s->d_segcnt.reserve((size_t)n_seg));
     SOAP_CUDA(s, s->d_nactive.reserve((size_t)n_phases));
-    SOAP_CUDA(s, s->d_counters.reserve(1));
-    SOAP_CUDA(s, cudaMemsetAsync(s->d_WD.ptr, 0, (size_t)n_seg * ncap * sizeof(double), st));
-    SOAP_CUDA(s, cudaMemsetAsync(s->d_nactive.ptr, 0, (size_t)n_phases * sizeof(int), st));
-    SOAP_CUDA(s, cudaMemsetAsync(s->d_counters.ptr, 0, sizeof(Counters), st));
-    if (n_regions > 0) {
-        LbCoef lb{};
-        lb.c[1][0] = spot ? spot->lb_c0 : 1.0; lb.c[1][1] = spot ? spot->lb_c1 : 0.0; lb.c[1][2] = spot ? spot->lb_c2 : 0.0;
-        lb.c[2][0] = fac ? fac->lb_c0 : 1.0;  lb.c[2][1] = fac ? fac->lb_c1 : 0.0;  lb.c[2][2] = fac ? fac->lb_c2 : 0.0;
-        active_bin_kernel<<<dim3((N + kBinWarps - 1) / kBinWarps, n_phases), 32 * kBinWarps, 0, st>>>(
-            N, n_regions, n_mu, ncap, s->d_rp.ptr, s->d_mu.ptr, s->d_w.ptr, s->d_bin.ptr, lb, s->d_WD.ptr,
-            s->d_nactive.ptr);
-        SOAP_LAUNCH_CHECK(s, "active_bin_kernel");
+    if (!s->d_counters.ptr) {
+        SOAP_CUDA(s, s->d_counters.reserve(1));
+        SOAP_CUDA(s, cudaMemsetAsync(s->d_counters.ptr, 0, sizeof(ActiveCounters), st));  // once per handle
     }
+    const int job_cap = 3 * n_mu * ((ncap + kActiveJobCap - 1) / kActiveJobCap);
+    SOAP_CUDA(s, s->d_jobs.reserve((size_t)n_phases * job_cap));
+    SOAP_CUDA(s, s->d_sched.reserve((size_t)3 * n_phases));
+    int *d_njobs = s->d_sched.ptr, *d_order = d_njobs + n_phases, *d_work = d_order + n_phases;
     {
-        const int warps_per_block = 8;
-        const unsigned blocks = (unsigned)((n_seg + warps_per_block - 1) / warps_per_block);
-        active_compact_kernel<Ent><<<blocks, warps_per_block * 32, 0, st>>>(
-            N, n_mu, ncap, (int)n_seg, s->d_col_a.ptr, s->d_WD.ptr, reinterpret_cast<Ent *>(s->d_aent.ptr),
-            s->d_segcnt.ptr, &s->d_counters.ptr->active_entries);
-        SOAP_LAUNCH_CHECK(s, "active_compact_kernel");
+        // a4 in one launch: one cluster of CTAs per phase bins, compacts and schedules (active.cuh)
+        PrepArgs a{};
+        a.N = N;
+        a.n_regions = n_regions;
+        a.n_mu = n_mu;
+        a.seg_cap = ncap;
+        a.job_cap = job_cap;
+        a.n_phases = n_phases;
+        a.chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);  // columns a CTA of the cluster may own
+        if (prep_smem_bytes(n_mu, a.chunk_cols) > 200 * 1024)
+            return s->fail(SOAP_ERR_UNSUPPORTED, "grid_n %d with %d mu bins exceeds the active-map kernel's shared memory", N, n_mu);
+        a.rp = s->d_rp.ptr;
+        a.mu = s->d_mu.ptr;
+        a.w = s->d_w.ptr;
+        a.col_a = s->d_col_a.ptr;
+        a.bin = s->d_bin.ptr;
+        a.lb.c[1][0] = spot ? spot->lb_c0 : 1.0; a.lb.c[1][1] = spot ? spot->lb_c1 : 0.0; a.lb.c[1][2] = spot ? spot->lb_c2 : 0.0;
+        a.lb.c[2][0] = fac ? fac->lb_c0 : 1.0;  a.lb.c[2][1] = fac ? fac->lb_c1 : 0.0;  a.lb.c[2][2] = fac ? fac->lb_c2 : 0.0;
+        a.ent = s->d_aent.ptr;
+        a.seg_count = s->d_segcnt.ptr;
+        a.n_active = s->d_nactive.ptr;
+        a.jobs = s->d_jobs.ptr;
+        a.n_jobs = d_njobs;
+        a.work = d_work;
+        a.phase_order = d_order;
+        a.counters = s->d_counters.ptr;
+        const size_t smem = prep_smem_bytes(n_mu, a.chunk_cols);
+        SOAP_CUDA(s, cudaFuncSetAttribute(active_prepare_kernel<Ent>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        active_prepare_kernel<Ent><<<n_phases * kPrepCluster, kPrepThreads, smem, st>>>(a);
+        SOAP_LAUNCH_CHECK(s, "active_prepare_kernel");
     }
     if (sizeof(T) == 4) {
-        // per-phase job lists + heaviest-first phase order for the persistent active launch
-        const int job_cap = 3 * n_mu * ((ncap + f32::kJobCap - 1) / f32::kJobCap);
-        SOAP_CUDA(s, s->d_jobs.reserve((size_t)n_phases * job_cap));
-        SOAP_CUDA(s, s->d_sched.reserve((size_t)3 * n_phases));
-        int *d_njobs = s->d_sched.ptr, *d_order = d_njobs + n_phases, *d_work = d_order + n_phases;
-        f32::schedule_active_kernel<<<1, f32::kScheduleThreads, 0, st>>>(s->d_segcnt.ptr, n_phases, n_mu, ncap, job_cap,
-                                                                         s->d_jobs.ptr, d_njobs, d_order, d_work);
-        SOAP_LAUNCH_CHECK(s, "schedule_active_kernel");
         f32::Params p{};
         p.base[0] = static_cast<const float *>(q->data);
         p.base[1] = spot ? static_cast<const float *>(spot->data) : p.base[0];
@@ -491,10 +496,10 @@ int soap_create(soap_star **out, int device) {
 int soap_destroy(soap_star *s) {
     if (!s) return SOAP_OK;
     cudaSetDevice(s->device);
-    s->d_mu_centres.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
+    s->d_geom_done.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
     s->d_Wbin.release(); s->d_col_sumw.release(); s->d_bin.release(); s->d_col_nvis.release(); s->d_row_start.release();
     s->d_ent32.release(); s->d_ent64.release(); s->d_info.release(); s->d_partial.release(); s->d_rp.release();
-    s->d_WD.release(); s->d_aent.release(); s->d_segcnt.release(); s->d_nactive.release(); s->d_counters.release(); s->d_sched.release(); s->d_jobs.release();
+    s->d_aent.release(); s->d_segcnt.release(); s->d_nactive.release(); s->d_counters.release(); s->d_sched.release(); s->d_jobs.release();
     for (int k = 0; k < 3; ++k) { s->d_stage[k].release(); s->d_stage_c[k].release(); }
     s->d_out_q.release(); s->d_out_d.release();
     for (auto &e : s->ev)
@@ -560,7 +565,6 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     const double vmax = std::fabs(prm->vsini_kms * sini) * (double)(N - 1) / (double)N;
     s->amax = std::max(std::fabs(host_dshift(vmax, prm->doppler_mode)), std::fabs(host_dshift(-vmax, prm->doppler_mode)));
 
-    SOAP_CUDA(s, s->d_mu_centres.reserve(n_mu));
     SOAP_CUDA(s, s->d_mu.reserve(ncell));
     SOAP_CUDA(s, s->d_w.reserve(ncell));
     SOAP_CUDA(s, s->d_vel.reserve(ncell));
@@ -575,16 +579,19 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     SOAP_CUDA(s, s->d_ent32.reserve(ent_cap));
     SOAP_CUDA(s, s->d_ent64.reserve(ent_cap));
 
-    // mu_centres: tiny pageable copy; the source is the handle's own vector, which outlives the copy
-    SOAP_CUDA(s, cudaMemcpyAsync(s->d_mu_centres.ptr, s->mu_centres.data(), n_mu * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (!s->d_geom_done.ptr) {
+        SOAP_CUDA(s, s->d_geom_done.reserve(1));
+        SOAP_CUDA(s, cudaMemsetAsync(s->d_geom_done.ptr, 0, sizeof(unsigned int), st));  // once per handle
+    }
+    MuCentres mc{};
+    for (int b = 0; b < n_mu; ++b) mc.v[b] = prm->mu_centres[b];
     const double vs = prm->vsini_kms * sini;
-    geometry_kernel<<<(N + kGeomWarps - 1) / kGeomWarps, 32 * kGeomWarps, 0, st>>>(
-        N, vs, prm->ld_u1, prm->ld_u2, prm->doppler_mode, n_mu, s->d_mu_centres.ptr, s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr,
-        s->d_bin.ptr, s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr);
+    // a1 + a2 in one launch: the last CTA compacts the binned weights into the entry list
+    geometry_kernel<<<(N + geom_cols_per_cta(N) - 1) / geom_cols_per_cta(N), 32 * kGeomWarps, 0, st>>>(
+        N, vs, prm->ld_u1, prm->ld_u2, prm->doppler_mode, n_mu, mc, s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr, s->d_bin.ptr,
+        s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr, s->d_ent32.ptr, s->d_ent64.ptr, s->d_row_start.ptr,
+        s->d_info.ptr, s->d_geom_done.ptr);
     SOAP_LAUNCH_CHECK(s, "geometry_kernel");
-    build_binned_entries_kernel<<<1, 1024, 0, st>>>(N, n_mu, s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr,
-                                                    s->d_ent32.ptr, s->d_ent64.ptr, s->d_row_start.ptr, s->d_info.ptr);
-    SOAP_LAUNCH_CHECK(s, "build_binned_entries_kernel");
     if (s->form_used == SOAP_FORM_CELLS) {
         build_cell_entries_kernel<<<1, 1024, 0, st>>>(N, n_mu, s->d_col_a.ptr, s->d_w.ptr, s->d_bin.ptr, s->d_ent32.ptr,
                                                       s->d_ent64.ptr, s->d_row_start.ptr);
@@ -656,7 +663,7 @@ int soap_get_stats(soap_star *s, soap_stats *stats, void *stream) {
         stats->quiet_entries = (s->form_used == SOAP_FORM_CELLS) ? di.n_visible : di.n_entries;
     }
     if (s->d_counters.ptr) {
-        Counters c;
+        ActiveCounters c;
         SOAP_CUDA(s, cudaMemcpyAsync(&c, s->d_counters.ptr, sizeof(c), cudaMemcpyDeviceToHost, st));
         SOAP_CUDA(s, cudaStreamSynchronize(st));
         stats->active_entries = (long long)c.active_entries;
