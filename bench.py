@@ -27,9 +27,9 @@ if ROOT not in sys.path:
 METRIC = "integrated spectra/s and cell*pixel interps/s (full visible, 300^2 grid), % roofline"
 N_SM, FP32_LANES_PER_SM = 148, 128
 FLOPS_PER_UNIT = 4  # one lerp-accumulate = 2 FP32 FMAs per (entry, pixel): acc += W u_r; acc += (W a) v_r
-# dram bytes per launch of the dominant kernel from the committed ncu --set full capture
-# (profiles/r01_sia_full_summary.md); None until a capture exists for the current kernel.
-NCU_DRAM_TRAFFIC_BYTES = {"sia_kernel<quiet>": None, "sia_kernel<active>": None}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this
+# workload (profiles/r01_v3_sia_full.md); algorithmic: active 74.4 MB in + 31 MB out, quiet 24.8 MB in.
+NCU_DRAM_TRAFFIC_BYTES = {"sia_f32_kernel<quiet>": 25.1e6, "sia_f32_kernel<active>": 109.5e6}
 
 
 def load_peaks():
@@ -156,6 +156,7 @@ def run_graft(args):
 
     import paper_2301_04259_b200 as soap
     import workloads
+    from paper_2301_04259_b200 import sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -219,10 +220,7 @@ def run_graft(args):
     total_ms = float(sum(step_ms))
     stats1 = soap.soap_get_stats(star)
     launches = stats1["launches"] - stats0["launches"]
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = sharding.max_over_ranks(total_ms, dev)
     ms_per_step = total_ms / args.steps
     value = world * n_spec / (ms_per_step * 1e-3)
 
@@ -240,8 +238,8 @@ def run_graft(args):
     units_q = stats["quiet_entries"] * P
     units_a = stats["active_entries"] * P
     kern = {
-        "sia_kernel<quiet>": dict(ms=float(np.mean(kq)), units=units_q),
-        "sia_kernel<active>": dict(ms=float(np.mean(ka)), units=units_a),
+        "sia_f32_kernel<quiet>": dict(ms=float(np.mean(kq)), units=units_q),
+        "sia_f32_kernel<active>": dict(ms=float(np.mean(ka)), units=units_a),
     }
     dom = max(kern, key=lambda k: kern[k]["ms"])
     peak_tflops = N_SM * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
@@ -285,10 +283,7 @@ def run_graft(args):
         b.record()
         b.synchronize()
         e2e_ms += a.elapsed_time(b)
-    if world > 1:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = sharding.max_over_ranks(e2e_ms, dev)
     e2e_value = world * n_spec / (e2e_ms / e2e_steps * 1e-3)
     h2d = 3 * wl.n_mu * pitch * 4 + P * 4
     d2h = n_spec * P * 4

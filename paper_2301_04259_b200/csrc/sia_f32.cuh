@@ -452,9 +452,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             cur_kind = kind;
             prefetch_contrast(kind);
         }
+        int2 run_next = runs[0];
         for (int ri = 0; ri < n_runs; ++ri) {
-            const int2 run = runs[ri];
-            const int nxt = runs[ri + 1].x;
+            const int2 run = run_next;
+            run_next = runs[ri + 1];  // the next run's header is fetched while this run is processed
+            const int nxt = run_next.x;
             if (run.y == kFlip) {
                 // integer shift changes inside the tile: per-pixel floor
                 const float2 en = raw[run.x];
