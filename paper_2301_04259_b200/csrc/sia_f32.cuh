@@ -36,7 +36,7 @@
 //     coordinate; fp32 partial sums are folded into fp64 every kFold entries.
 //   * quiet launch: the flattened (tile, entry) work list is cut into equal contiguous ranges, one per
 //     CTA, grid = resident CTA slots (one wave, no tail); a CTA writes one fp64 partial per tile it
-//     touches and reduce_ranges_kernel adds the partials of a tile in CTA order (deterministic).
+//     touches and the last CTA to deliver its share of a tile adds the shares in CTA order (deterministic).
 //   * active launch: persistent CTAs; the (phase, tile) items, heaviest phase first, are dealt to the
 //     CTAs in snake order (active_prepare_kernel builds the per-phase job lists and the order); the
 //     post-shift contrast (I_ratio of Eq. 3) multiplies each kind's fp64 sum once per pixel (a6).
@@ -81,6 +81,7 @@ struct Params {
     const int *row_start;      // [n_mu + 1] entry offsets (even)
     double *partial;           // [gridDim.x][max_seg][kTile]
     int max_seg;
+    int *tile_ticket;          // [n_tiles] shares delivered per tile; zero between launches
     // active launch
     const ActiveJob *jobs;     // [n_phases][job_cap]
     const int *n_jobs;         // [n_phases]
@@ -116,7 +117,7 @@ __host__ __device__ inline StageLayout stage_layout(int halo) {
     l.stage_bytes = (l.desc_off + sizeof(Desc) + 127) & ~(size_t)127;
     return l;
 }
-constexpr size_t kHeaderBytes = 128;                          // mbarriers
+constexpr size_t kHeaderBytes = 128;                          // mbarriers (96 B) + tile hand-over words
 constexpr size_t kFinBytes = (size_t)kTile * (sizeof(double) + sizeof(float));  // active launch: per-pixel fp64
                                                                               // contrast-weighted sums + staged contrast
 __host__ inline size_t smem_bytes(int halo, bool active) {
@@ -250,6 +251,9 @@ struct ActiveSource {
     }
 };
 
+// Barrier among the 128 consumer threads only (the producers never take part).
+__device__ __forceinline__ void consumer_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory"); }
+
 __device__ __forceinline__ void mbar_wait_backoff(uint64_t *bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) __nanosleep(40);
 }
@@ -260,6 +264,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     uint64_t *bar_tma = reinterpret_cast<uint64_t *>(smem);  // [kStages] TMA landed          (count 1 + tx)
     uint64_t *bar_ready = bar_tma + kStages;                 // [kStages] stage post-processed (count 1)
     uint64_t *bar_empty = bar_ready + kStages;               // [kStages] consumers done       (count kConsumerWarps)
+    int *tile_ctl = reinterpret_cast<int *>(smem + 96);      // quiet launch: last-CTA flag, first / last sharing CTA
     const int H = p.halo;
     const int span = span_px(H);
     const StageLayout L = stage_layout(H);
@@ -522,61 +527,55 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                 double *o = p.partial + ((long long)blockIdx.x * p.max_seg + out_idx) * kTile;
 #pragma unroll
                 for (int r = 0; r < kR; ++r) o[tid + kConsumers * r] = tot[r];
+                // a6: the last CTA to deliver its share of this tile adds all shares in CTA order (the same
+                // order whoever comes last: deterministic) and rounds once to fp32.
+                const long long tile = m_t0 / kTile;
+                const long long E = __ldg(&p.row_start[p.n_mu]), U = E * p.n_tiles, G = gridDim.x;
+                const long long ub = tile * E, ue = ub + E;
+                __threadfence();
+                consumer_bar_sync();
+                if (tid == 0) {
+                    long long c = (ub * G) / U;
+                    while (c > 0 && range_begin(c, U, G) > ub) --c;
+                    while (c + 1 < G && range_begin(c + 1, U, G) <= ub) ++c;
+                    int n = 0;
+                    long long c_lo = c, c_hi = c;
+                    for (; c < G; ++c) {
+                        const long long b = range_begin(c, U, G), e = range_begin(c + 1, U, G);
+                        if (b >= ue) break;
+                        if (e <= b || e <= ub) continue;
+                        c_hi = c;
+                        ++n;
+                    }
+                    const int ticket = atomicAdd(&p.tile_ticket[tile], 1);
+                    const bool last = ticket == n - 1;
+                    if (last) p.tile_ticket[tile] = 0;  // ready for the next launch
+                    tile_ctl[0] = last ? 1 : 0;
+                    tile_ctl[1] = (int)c_lo;
+                    tile_ctl[2] = (int)c_hi;
+                }
+                consumer_bar_sync();
+                if (tile_ctl[0]) {
+                    __threadfence();
+                    double sum[kR];
+#pragma unroll
+                    for (int r = 0; r < kR; ++r) sum[r] = 0.0;
+                    for (long long c = tile_ctl[1]; c <= tile_ctl[2]; ++c) {
+                        const long long b = range_begin(c, U, G), e = range_begin(c + 1, U, G);
+                        if (e <= b || e <= ub) continue;
+                        const double *src = p.partial + ((c * p.max_seg + (tile - b / E)) * kTile) + tid;
+#pragma unroll
+                        for (int r = 0; r < kR; ++r) sum[r] += __ldcg(&src[kConsumers * r]);
+                    }
+                    float *qo = p.out + m_t0 + tid;
+#pragma unroll
+                    for (int r = 0; r < kR; ++r)
+                        if (m_t0 + tid + kConsumers * r < p.n_pix) qo[kConsumers * r] = (float)sum[r];
+                }
+                consumer_bar_sync();  // tile_ctl may be rewritten by the next tile
             }
         }
     }
-}
-
-// a6 for the quiet spectrum: adds, in CTA order, the partials of every CTA whose range touched the
-// pixel's tile, and rounds once to fp32.  blockDim.x divides kTile, so a block lies inside one tile and
-// thread 0 finds the contributing CTAs once for the block.
-constexpr int kReduceThreads = 256;
-constexpr int kReduceMaxSrc = 64;
-__global__ void __launch_bounds__(kReduceThreads)
-reduce_ranges_kernel(const double *__restrict__ partial, int max_seg, const int *__restrict__ row_start, int n_mu,
-                     int n_cta, int n_tiles, long long n_pix, float *__restrict__ out) {
-    __shared__ long long s_src[kReduceMaxSrc];  // element offset of each contributing partial tile
-    __shared__ int s_n, s_c0, s_c1;
-    const long long m0 = (long long)blockIdx.x * kReduceThreads;
-    const long long t = m0 / kTile;
-    const long long E = row_start[n_mu], U = E * n_tiles, G = n_cta;
-    if (threadIdx.x == 0) {
-        int n = 0;
-        s_c0 = 0;
-        s_c1 = 0;
-        if (U > 0) {
-            const long long ub = t * E, ue = ub + E;
-            long long c = (ub * G) / U;
-            while (c > 0 && range_begin(c, U, G) > ub) --c;
-            while (c + 1 < G && range_begin(c + 1, U, G) <= ub) ++c;
-            s_c0 = (int)c;
-            for (; c < G; ++c) {
-                const long long b = range_begin(c, U, G), e = range_begin(c + 1, U, G);
-                if (b >= ue) break;
-                if (e <= b || e <= ub) continue;
-                if (n < kReduceMaxSrc) s_src[n] = (c * max_seg + (t - b / E)) * kTile;
-                ++n;
-            }
-            s_c1 = (int)c;
-        }
-        s_n = n;
-    }
-    __syncthreads();
-    const long long m = m0 + threadIdx.x;
-    if (m >= n_pix) return;
-    const long long off = m - t * kTile;
-    double v = 0.0;
-    if (s_n <= kReduceMaxSrc) {
-        for (int k = 0; k < s_n; ++k) v += partial[s_src[k] + off];
-    } else {  // more contributing CTAs than the table holds (tiny entry lists): walk the ranges directly
-        const long long ub = t * E;
-        for (long long c = s_c0; c < s_c1; ++c) {
-            const long long b = range_begin(c, U, G), e = range_begin(c + 1, U, G);
-            if (e <= b || e <= ub) continue;
-            v += partial[(c * max_seg + (t - b / E)) * kTile + off];
-        }
-    }
-    out[m] = (float)v;
 }
 
 }  // namespace f32

@@ -75,6 +75,7 @@ struct soap_star {
 
     // quiet scratch
     DevBuf<double> d_partial;
+    DevBuf<int> d_tile_ticket;
 
     // active scratch
     DevBuf<RegionAtPhase> d_rp;
@@ -233,12 +234,14 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     p.max_seg = (int)(n_tiles / G) + 3;
     SOAP_CUDA(s, s->d_partial.reserve((size_t)G * p.max_seg * f32::kTile));
     p.partial = s->d_partial.ptr;
+    if ((size_t)n_tiles > s->d_tile_ticket.cap) {
+        SOAP_CUDA(s, s->d_tile_ticket.reserve((size_t)n_tiles));
+        SOAP_CUDA(s, cudaMemsetAsync(s->d_tile_ticket.ptr, 0, s->d_tile_ticket.cap * sizeof(int), st));  // self-resetting after
+    }
+    p.tile_ticket = s->d_tile_ticket.ptr;
+    p.out = static_cast<float *>(out);
     int rc = launch_sia_f32<false>(s, p, dim3((unsigned)G), st);
     if (rc) return rc;
-    static_assert(f32::kTile % f32::kReduceThreads == 0, "a reduce block must lie inside one tile");
-    f32::reduce_ranges_kernel<<<(unsigned)((P + f32::kReduceThreads - 1) / f32::kReduceThreads), f32::kReduceThreads, 0, st>>>(
-        s->d_partial.ptr, p.max_seg, s->d_row_start.ptr, p.n_mu, (int)G, n_tiles, P, static_cast<float *>(out));
-    SOAP_LAUNCH_CHECK(s, "reduce_ranges_kernel");
     s->last_quiet_splits = (int)G;
     s->last_tile_px = f32::kTile;
     return SOAP_OK;
@@ -498,7 +501,7 @@ int soap_destroy(soap_star *s) {
     cudaSetDevice(s->device);
     s->d_geom_done.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
     s->d_Wbin.release(); s->d_col_sumw.release(); s->d_bin.release(); s->d_col_nvis.release(); s->d_row_start.release();
-    s->d_ent32.release(); s->d_ent64.release(); s->d_info.release(); s->d_partial.release(); s->d_rp.release();
+    s->d_ent32.release(); s->d_ent64.release(); s->d_info.release(); s->d_partial.release(); s->d_tile_ticket.release(); s->d_rp.release();
     s->d_aent.release(); s->d_segcnt.release(); s->d_nactive.release(); s->d_counters.release(); s->d_sched.release(); s->d_jobs.release();
     for (int k = 0; k < 3; ++k) { s->d_stage[k].release(); s->d_stage_c[k].release(); }
     s->d_out_q.release(); s->d_out_d.release();
