@@ -75,6 +75,7 @@ struct Params {
     double c0;                 // lambda0 / dlambda
     int n_mu;
     int halo;                  // H: multiple of 4, >= max |delta| + 2
+    int stage_bytes, raw_off, rec_off, run_off, desc_off;  // stage_layout(halo), filled by set_layout()
     const float2 *ent;         // raw entries (a_e, W_e)
     int n_tiles;
     // quiet launch
@@ -122,6 +123,15 @@ constexpr size_t kFinBytes = (size_t)kTile * (sizeof(double) + sizeof(float));  
                                                                               // contrast-weighted sums + staged contrast
 __host__ inline size_t smem_bytes(int halo, bool active) {
     return kHeaderBytes + (active ? kFinBytes : 0) + kStages * stage_layout(halo).stage_bytes;
+}
+
+inline void set_layout(Params &p) {  // host: the stage layout travels as kernel arguments (constant bank)
+    const StageLayout l = stage_layout(p.halo);
+    p.stage_bytes = (int)l.stage_bytes;
+    p.raw_off = (int)l.raw_off;
+    p.rec_off = (int)l.rec_off;
+    p.run_off = (int)l.run_off;
+    p.desc_off = (int)l.desc_off;
 }
 
 struct Job {
@@ -267,7 +277,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     int *tile_ctl = reinterpret_cast<int *>(smem + 96);      // quiet launch: last-CTA flag, first / last sharing CTA
     const int H = p.halo;
     const int span = span_px(H);
-    const StageLayout L = stage_layout(H);
     double *fin = reinterpret_cast<double *>(smem + kHeaderBytes);  // active launch only: [kR][kConsumers]
     float *cst = reinterpret_cast<float *>(fin + kTile);            // active launch only: contrast of the current kind
     unsigned char *stage0 = smem + kHeaderBytes + (ACTIVE ? kFinBytes : 0);
@@ -288,12 +297,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         // =============================== producer warps ==============================================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsProducer));
         const int st = warp - kConsumerWarps;  // this warp's stage
-        unsigned char *sb = stage0 + (size_t)st * L.stage_bytes;
+        unsigned char *sb = stage0 + (size_t)st * p.stage_bytes;
         float *rs = reinterpret_cast<float *>(sb);
-        const float2 *raw = reinterpret_cast<const float2 *>(sb + L.raw_off);
-        float2 *rec = reinterpret_cast<float2 *>(sb + L.rec_off);
-        int2 *runs = reinterpret_cast<int2 *>(sb + L.run_off);
-        Desc *desc = reinterpret_cast<Desc *>(sb + L.desc_off);
+        const float2 *raw = reinterpret_cast<const float2 *>(sb + p.raw_off);
+        float2 *rec = reinterpret_cast<float2 *>(sb + p.rec_off);
+        int2 *runs = reinterpret_cast<int2 *>(sb + p.run_off);
+        Desc *desc = reinterpret_cast<Desc *>(sb + p.desc_off);
         typename std::conditional<ACTIVE, ActiveSource, QuietSource>::type src;
         src.init(p, blockIdx.x, gridDim.x);
         Job jb;
@@ -320,7 +329,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                     fence_proxy_async_smem();
                     mbar_arrive_expect_tx(&bar_tma[st], row_bytes + ent_bytes);
                     tma_load_1d(sb + (size_t)(g_lo - s_start) * sizeof(float), src_row, row_bytes, &bar_tma[st]);
-                    tma_load_1d(sb + L.raw_off, p.ent + jb.begin, ent_bytes, &bar_tma[st]);
+                    tma_load_1d(sb + p.raw_off, p.ent + jb.begin, ent_bytes, &bar_tma[st]);
                 } else {
                     mbar_arrive(&bar_tma[st]);  // nothing to load: keeps the barrier's phase in step
                 }
@@ -423,12 +432,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     for (int n = 0;; ++n) {
         const int st = n % kStages;
         mbar_wait(&bar_ready[st], (uint32_t)((n / kStages) & 1));
-        const unsigned char *sb = stage0 + (size_t)st * L.stage_bytes;
+        const unsigned char *sb = stage0 + (size_t)st * p.stage_bytes;
         const float *rs = reinterpret_cast<const float *>(sb);
-        const float2 *raw = reinterpret_cast<const float2 *>(sb + L.raw_off);
-        const float2 *rec = reinterpret_cast<const float2 *>(sb + L.rec_off);
-        const int2 *runs = reinterpret_cast<const int2 *>(sb + L.run_off);
-        const Desc *desc = reinterpret_cast<const Desc *>(sb + L.desc_off);
+        const float2 *raw = reinterpret_cast<const float2 *>(sb + p.raw_off);
+        const float2 *rec = reinterpret_cast<const float2 *>(sb + p.rec_off);
+        const int2 *runs = reinterpret_cast<const int2 *>(sb + p.run_off);
+        const Desc *desc = reinterpret_cast<const Desc *>(sb + p.desc_off);
         const int flags = desc->flags;
         if (flags & kJobExit) break;
         const int n_runs = desc->n_runs;

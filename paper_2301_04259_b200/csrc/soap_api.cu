@@ -218,6 +218,7 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     p.c0 = q->lambda0 / q->dlambda;
     p.n_mu = s->prm.n_mu;
     p.halo = halo_for(s, q);
+    f32::set_layout(p);
     p.ent = s->d_ent32.ptr;
     p.row_start = s->d_row_start.ptr;
     p.n_tiles = n_tiles;
@@ -352,6 +353,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         p.c0 = q->lambda0 / q->dlambda;
         p.n_mu = n_mu;
         p.halo = halo_for(s, q);
+        f32::set_layout(p);
         p.ent = reinterpret_cast<const float2 *>(s->d_aent.ptr);
         p.n_tiles = (int)((q->n_pix + f32::kTile - 1) / f32::kTile);
         p.jobs = s->d_jobs.ptr;
