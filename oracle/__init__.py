@@ -65,6 +65,11 @@ def _load():
         lib.soap_oracle_active.argtypes = [ctypes.POINTER(_Star)] + [ctypes.c_void_p] * 7 + [
             ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.POINTER(_Region), ctypes.c_int32,
             ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
+        lib.soap_oracle_active_effect.restype = ctypes.c_int
+        lib.soap_oracle_active_effect.argtypes = [ctypes.POINTER(_Star)] + [ctypes.c_void_p] * 7 + [
+            ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.POINTER(_Region), ctypes.c_int32,
+            ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_void_p,
+            ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -155,8 +160,9 @@ def info_map(star, regions: Sequence, phase: float):
 
 def active(star, S_quiet, S_spot, S_facula, lambda0: float, k: float, regions: Sequence, phases,
            C_spot=None, C_facula=None, lb_spot=(1.0, 0.0, 0.0), lb_facula=(1.0, 0.0, 0.0),
-           m_lo: int = 0, m_hi: Optional[int] = None):
-    """Alg. 5 + Eq. 3 (north_star sign) over pixels [m_lo, m_hi).  Returns (delta [n_ph, n], n_active [n_ph])."""
+           m_lo: int = 0, m_hi: Optional[int] = None, effect: int = 0):
+    """Alg. 5 + Eq. 3 (north_star sign) over pixels [m_lo, m_hi).  Returns (delta [n_ph, n], n_active [n_ph]).
+    effect: 0 = total (Eq. 3), 1 = flux only (Eq. 1), 2 = convective blueshift only (Eq. 2)."""
     lib = _load()
     st, _keep = _star(star)
     Sq, Ss, Sf = _f64(S_quiet), _f64(S_spot), _f64(S_facula)
@@ -167,19 +173,19 @@ def active(star, S_quiet, S_spot, S_facula, lambda0: float, k: float, regions: S
     ph = _f64(phases)
     delta = np.zeros((ph.shape[0], m_hi - m_lo), dtype=np.float64)
     n_active = np.zeros(ph.shape[0], dtype=np.int32)
-    rc = lib.soap_oracle_active(ctypes.byref(st), _ptr(Sq), _ptr(Ss), _ptr(Sf), _ptr(Cs), _ptr(Cf),
-                                _ptr(lbs), _ptr(lbf), P, float(lambda0), float(k), _regions(regions),
-                                len(regions), ph.ctypes.data, ph.shape[0], int(m_lo), int(m_hi),
-                                delta.ctypes.data, n_active.ctypes.data)
+    rc = lib.soap_oracle_active_effect(ctypes.byref(st), _ptr(Sq), _ptr(Ss), _ptr(Sf), _ptr(Cs), _ptr(Cf),
+                                       _ptr(lbs), _ptr(lbf), P, float(lambda0), float(k), _regions(regions),
+                                       len(regions), ph.ctypes.data, ph.shape[0], int(m_lo), int(m_hi),
+                                       int(effect), delta.ctypes.data, n_active.ctypes.data)
     if rc != 0:
         raise RuntimeError(f"soap_oracle_active failed: {rc}")
     return delta, n_active
 
 
-def run_workload(wl, m_lo: int = 0, m_hi: Optional[int] = None):
+def run_workload(wl, m_lo: int = 0, m_hi: Optional[int] = None, effect: int = 0):
     """Convenience: (Q, delta, n_active, geometry-info) of a workloads.Workload-like object."""
     Q = quiet(wl, wl.quiet, wl.lambda0, wl.dlambda, m_lo, m_hi)
     delta, n_active = active(wl, wl.quiet, wl.spot, wl.facula, wl.lambda0, wl.dlambda, wl.regions,
                              wl.phases, wl.spot_contrast, wl.facula_contrast, wl.spot_lb, wl.facula_lb,
-                             m_lo, m_hi)
+                             m_lo, m_hi, effect)
     return Q, delta, n_active

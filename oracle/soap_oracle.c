@@ -249,11 +249,36 @@ int64_t soap_oracle_info_map(const oracle_star *st, const oracle_region *regions
  * delta: [n_phases][m_hi - m_lo];  n_active: [n_phases] or NULL.
  * Returns 0, or -2 if a region needs a spectrum that is NULL.
  */
+int soap_oracle_active_effect(const oracle_star *st, const double *S_quiet, const double *S_spot,
+                              const double *S_facula, const double *C_spot, const double *C_facula,
+                              const double *lb_spot, const double *lb_facula, int64_t P, double lambda0,
+                              double k, const oracle_region *regions, int32_t n_regions,
+                              const double *phases, int32_t n_phases, int64_t m_lo, int64_t m_hi,
+                              int32_t effect, double *delta, int32_t *n_active);
+
 int soap_oracle_active(const oracle_star *st, const double *S_quiet, const double *S_spot,
                        const double *S_facula, const double *C_spot, const double *C_facula,
                        const double *lb_spot, const double *lb_facula, int64_t P, double lambda0,
                        double k, const oracle_region *regions, int32_t n_regions, const double *phases,
                        int32_t n_phases, int64_t m_lo, int64_t m_hi, double *delta, int32_t *n_active) {
+    return soap_oracle_active_effect(st, S_quiet, S_spot, S_facula, C_spot, C_facula, lb_spot, lb_facula, P,
+                                     lambda0, k, regions, n_regions, phases, n_phases, m_lo, m_hi, 0, delta,
+                                     n_active);
+}
+
+/* The three effects of PAPER.md:73-79, per covered cell, with north_star's sign (active minus quiet: the
+ * negatives of Eq. 1-3), I_ratio = C_t[m] * LB_t(mu_c):
+ *   effect 0 (total, Eq. 3):      w * ( I_ratio * S'_active - S'_quiet )
+ *   effect 1 (flux only, Eq. 1):  w * ( I_ratio * S'_quiet  - S'_quiet )
+ *   effect 2 (CB only, Eq. 2):    w * (           S'_active - S'_quiet )
+ * Everything else as soap_oracle_active.  Returns -4 for an unknown effect. */
+int soap_oracle_active_effect(const oracle_star *st, const double *S_quiet, const double *S_spot,
+                              const double *S_facula, const double *C_spot, const double *C_facula,
+                              const double *lb_spot, const double *lb_facula, int64_t P, double lambda0,
+                              double k, const oracle_region *regions, int32_t n_regions,
+                              const double *phases, int32_t n_phases, int64_t m_lo, int64_t m_hi,
+                              int32_t effect, double *delta, int32_t *n_active) {
+    if (effect < 0 || effect > 2) return -4;
     const int32_t N = st->grid_n;
     const int64_t ncell = (int64_t)N * N;
     for (int32_t r = 0; r < n_regions; ++r) {
@@ -293,8 +318,13 @@ int soap_oracle_active(const oracle_star *st, const double *S_quiet, const doubl
                     const double wc = w[c], Dc = D[c];
                     for (int64_t m = a; m < b; ++m) {
                         const double cm = C ? C[m] : 1.0;
-                        dp[m - m_lo] += wc * (cm * lb * shifted_at(ra, P, lambda0, k, Dc, m) -
-                                              shifted_at(rq, P, lambda0, k, Dc, m));
+                        const double sq = shifted_at(rq, P, lambda0, k, Dc, m);
+                        if (effect == 0)
+                            dp[m - m_lo] += wc * (cm * lb * shifted_at(ra, P, lambda0, k, Dc, m) - sq);
+                        else if (effect == 1)
+                            dp[m - m_lo] += wc * (cm * lb * sq - sq);
+                        else
+                            dp[m - m_lo] += wc * (shifted_at(ra, P, lambda0, k, Dc, m) - sq);
                     }
                 }
             }

@@ -77,8 +77,10 @@ def info_map(cells, regions, incl_deg, phase):
 
 
 def active(cells, incl_deg, S_quiet, S_spot, S_facula, C_spot, C_facula, lb_spot, lb_facula,
-           lambda0, k, regions, phases):
-    """delta[p] = sum_active w (C_t LB_t(mu) shifted(S_t[bin]) - shifted(S_quiet[bin]))  (Eq. 3, north_star sign)."""
+           lambda0, k, regions, phases, effect=0):
+    """delta[p] = sum_active w (C_t LB_t(mu) shifted(S_t[bin]) - shifted(S_quiet[bin]))  (Eq. 3, north_star sign).
+    effect 1: flux only, w (I_ratio shifted(S_quiet) - shifted(S_quiet)) (Eq. 1); effect 2: convective blueshift
+    only, w (shifted(S_t) - shifted(S_quiet)) (Eq. 2); PAPER.md:73-79."""
     S_quiet = np.asarray(S_quiet, dtype=np.float64)
     P = S_quiet.shape[1]
     lam = lambda0 + k * np.arange(P, dtype=np.float64)
@@ -96,5 +98,14 @@ def active(cells, incl_deg, S_quiet, S_spot, S_facula, C_spot, C_facula, lb_spot
             lb = lbc[0] + lbc[1] * c["mu"] + lbc[2] * c["mu"] ** 2
             cm = 1.0 if C is None else np.asarray(C, dtype=np.float64)
             x = lam * c["D"]
-            out[p] += c["w"] * (cm * lb * np.interp(x, lam, Sa[c["bin"]]) - np.interp(x, lam, S_quiet[c["bin"]]))
+            sq = np.interp(x, lam, S_quiet[c["bin"]])
+            sa = np.interp(x, lam, Sa[c["bin"]])
+            if effect == 0:
+                out[p] += c["w"] * (cm * lb * sa - sq)
+            elif effect == 1:
+                out[p] += c["w"] * (cm * lb * sq - sq)
+            elif effect == 2:
+                out[p] += c["w"] * (sa - sq)
+            else:
+                raise ValueError("effect must be 0, 1 or 2")
     return out, n_active
