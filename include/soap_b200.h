@@ -54,6 +54,8 @@ enum soap_status {
 
 enum soap_dtype { SOAP_F32 = 0, SOAP_F64 = 1 };
 enum soap_region_type { SOAP_SPOT = 1, SOAP_FACULA = 2 };
+/* The three per-cell differences of PAPER.md:73-79, with this library's sign (active minus quiet). */
+enum soap_effect { SOAP_EFFECT_TOTAL = 0, SOAP_EFFECT_FLUX = 1, SOAP_EFFECT_CB = 2 };
 
 /* How the shift-interpolate-accumulate sum is evaluated.  All forms compute the same sums (Alg. 1,
  * Eq. 3) and differ only in rounding order. */
@@ -168,6 +170,19 @@ int soap_active_timeseries(soap_star *star, const soap_spectra *quiet, const soa
                            const soap_spectra *facula, const soap_region *regions, int32_t n_regions,
                            const double *phases, int32_t n_phases, void *out_delta, int64_t out_pitch,
                            int32_t *n_active, void *stream);
+
+/* ---- flux-only and convective-blueshift-only time series beside the total (Eq. 1-3) -----
+ * Same arguments, covered cells and conventions as soap_active_timeseries; I_ratio = C_t[m] LB_t(mu_c):
+ *   out_total[p][m] = sum w_c ( I_ratio lerp(S_t[bin_c]) - lerp(S_quiet[bin_c]) )     (negative of Eq. 3)
+ *   out_flux [p][m] = sum w_c ( I_ratio lerp(S_quiet[bin_c]) - lerp(S_quiet[bin_c]) ) (negative of Eq. 1)
+ *   out_cb   [p][m] = sum w_c (         lerp(S_t[bin_c]) - lerp(S_quiet[bin_c]) )     (negative of Eq. 2)
+ * Each output: DEVICE [n_phases][out_pitch] or NULL (that effect is skipped); at least one non-NULL.
+ * One shift-interpolate-accumulate launch per requested effect; the active map is built once for total and
+ * flux, and once more for CB only when a limb-brightening law differs from 1. */
+int soap_active_timeseries_effects(soap_star *star, const soap_spectra *quiet, const soap_spectra *spot,
+                                   const soap_spectra *facula, const soap_region *regions, int32_t n_regions,
+                                   const double *phases, int32_t n_phases, void *out_total, void *out_flux,
+                                   void *out_cb, int64_t out_pitch, int32_t *n_active, void *stream);
 
 /* ---- debug export of the geometry (HOST outputs, N*N each, any may be NULL; synchronous) --------
  * Hidden cells: mu = 0, vel = 0, w = 0, bin = -1. */

@@ -291,7 +291,12 @@ int quiet_impl(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) 
 
 template <typename T>
 int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, const soap_spectra *fac,
-                int n_regions, int n_phases, void *out, long long out_pitch, cudaStream_t st) {
+                int n_regions, int n_phases, int effect, bool prepare, void *out, long long out_pitch, cudaStream_t st) {
+    // The three effects of Eq. 1-3 differ only in which table, weight and contrast an active entry uses:
+    //   total: S_t, w LB_t(mu), C_t;   flux only: S_quiet, w LB_t(mu), C_t;   CB only: S_t, w, 1.
+    // `prepare` = false reuses the entry lists of the previous pass (same weights).
+    const bool use_lb = effect != SOAP_EFFECT_CB, use_contrast = effect != SOAP_EFFECT_CB;
+    const bool quiet_rows = effect == SOAP_EFFECT_FLUX;
     using Ent = typename SiaTraits<T>::Ent;
     constexpr int TP = sia_tile_px<T>();
     const int N = s->prm.grid_n, n_mu = s->prm.n_mu;
@@ -309,7 +314,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
     SOAP_CUDA(s, s->d_jobs.reserve((size_t)n_phases * job_cap));
     SOAP_CUDA(s, s->d_sched.reserve((size_t)3 * n_phases));
     int *d_njobs = s->d_sched.ptr, *d_order = d_njobs + n_phases, *d_work = d_order + n_phases;
-    {
+    if (prepare) {
         // a4 in one launch: one cluster of CTAs per phase bins, compacts and schedules (active.cuh)
         PrepArgs a{};
         a.N = N;
@@ -326,8 +331,10 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         a.w = s->d_w.ptr;
         a.col_a = s->d_col_a.ptr;
         a.bin = s->d_bin.ptr;
-        a.lb.c[1][0] = spot ? spot->lb_c0 : 1.0; a.lb.c[1][1] = spot ? spot->lb_c1 : 0.0; a.lb.c[1][2] = spot ? spot->lb_c2 : 0.0;
-        a.lb.c[2][0] = fac ? fac->lb_c0 : 1.0;  a.lb.c[2][1] = fac ? fac->lb_c1 : 0.0;  a.lb.c[2][2] = fac ? fac->lb_c2 : 0.0;
+        a.lb.c[1][0] = 1.0;
+        a.lb.c[2][0] = 1.0;
+        if (use_lb && spot) { a.lb.c[1][0] = spot->lb_c0; a.lb.c[1][1] = spot->lb_c1; a.lb.c[1][2] = spot->lb_c2; }
+        if (use_lb && fac) { a.lb.c[2][0] = fac->lb_c0; a.lb.c[2][1] = fac->lb_c1; a.lb.c[2][2] = fac->lb_c2; }
         a.ent = s->d_aent.ptr;
         a.seg_count = s->d_segcnt.ptr;
         a.n_active = s->d_nactive.ptr;
@@ -344,10 +351,10 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
     if (sizeof(T) == 4) {
         f32::Params p{};
         p.base[0] = static_cast<const float *>(q->data);
-        p.base[1] = spot ? static_cast<const float *>(spot->data) : p.base[0];
-        p.base[2] = fac ? static_cast<const float *>(fac->data) : p.base[0];
-        p.contrast[1] = spot ? static_cast<const float *>(spot->contrast) : nullptr;
-        p.contrast[2] = fac ? static_cast<const float *>(fac->contrast) : nullptr;
+        p.base[1] = (spot && !quiet_rows) ? static_cast<const float *>(spot->data) : p.base[0];
+        p.base[2] = (fac && !quiet_rows) ? static_cast<const float *>(fac->data) : p.base[0];
+        p.contrast[1] = (spot && use_contrast) ? static_cast<const float *>(spot->contrast) : nullptr;
+        p.contrast[2] = (fac && use_contrast) ? static_cast<const float *>(fac->contrast) : nullptr;
         p.pitch = q->pitch;
         p.n_pix = q->n_pix;
         p.c0 = q->lambda0 / q->dlambda;
@@ -377,10 +384,10 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
     }
     SiaParams<T> p{};
     p.base[0] = static_cast<const T *>(q->data);
-    p.base[1] = spot ? static_cast<const T *>(spot->data) : p.base[0];
-    p.base[2] = fac ? static_cast<const T *>(fac->data) : p.base[0];
-    p.contrast[1] = spot ? static_cast<const T *>(spot->contrast) : nullptr;
-    p.contrast[2] = fac ? static_cast<const T *>(fac->contrast) : nullptr;
+    p.base[1] = (spot && !quiet_rows) ? static_cast<const T *>(spot->data) : p.base[0];
+    p.base[2] = (fac && !quiet_rows) ? static_cast<const T *>(fac->data) : p.base[0];
+    p.contrast[1] = (spot && use_contrast) ? static_cast<const T *>(spot->contrast) : nullptr;
+    p.contrast[2] = (fac && use_contrast) ? static_cast<const T *>(fac->contrast) : nullptr;
     p.pitch = q->pitch;
     p.n_pix = q->n_pix;
     p.c0 = q->lambda0 / q->dlambda;
@@ -626,9 +633,10 @@ int soap_integrate_quiet(soap_star *s, const soap_spectra *quiet, void *out, voi
     return quiet->dtype == SOAP_F32 ? quiet_impl<float>(s, quiet, out, st) : quiet_impl<double>(s, quiet, out, st);
 }
 
-int soap_active_timeseries(soap_star *s, const soap_spectra *quiet, const soap_spectra *spot, const soap_spectra *facula,
-                           const soap_region *regions, int32_t n_regions, const double *phases, int32_t n_phases,
-                           void *out_delta, int64_t out_pitch, int32_t *n_active, void *stream) {
+int soap_active_timeseries_effects(soap_star *s, const soap_spectra *quiet, const soap_spectra *spot,
+                                   const soap_spectra *facula, const soap_region *regions, int32_t n_regions,
+                                   const double *phases, int32_t n_phases, void *out_total, void *out_flux, void *out_cb,
+                                   int64_t out_pitch, int32_t *n_active, void *stream) {
     if (!s) return SOAP_ERR_INVALID_ARG;
     if (!s->ready) return s->fail(SOAP_ERR_NOT_READY, "soap_disk_geometry has not been called");
     int rc = check_spectra(s, quiet, "quiet");
@@ -637,14 +645,26 @@ int soap_active_timeseries(soap_star *s, const soap_spectra *quiet, const soap_s
     if (facula && ((rc = check_spectra(s, facula, "facula")) || (rc = check_same_grid(s, quiet, facula, "facula")))) return rc;
     if ((rc = check_regions(s, regions, n_regions, phases, n_phases, spot, facula))) return rc;
     if (n_phases == 0) return SOAP_OK;
-    if (!out_delta) return s->fail(SOAP_ERR_INVALID_ARG, "out_delta is NULL");
+    if (!out_total && !out_flux && !out_cb) return s->fail(SOAP_ERR_INVALID_ARG, "every output is NULL");
     if (out_pitch < quiet->n_pix) return s->fail(SOAP_ERR_INVALID_ARG, "out_pitch must be >= n_pix");
     SOAP_CUDA(s, cudaSetDevice(s->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if ((rc = upload_region_centres(s, regions, n_regions, phases, n_phases, st))) return rc;
-    rc = quiet->dtype == SOAP_F32 ? active_impl<float>(s, quiet, spot, facula, n_regions, n_phases, out_delta, out_pitch, st)
-                                  : active_impl<double>(s, quiet, spot, facula, n_regions, n_phases, out_delta, out_pitch, st);
-    if (rc) return rc;
+    // total and flux-only share the entry lists (weights w LB_t(mu)); CB-only needs the plain weights w, which
+    // are the same lists again when both limb-brightening laws are identically 1
+    const bool lb_is_one = (!spot || (spot->lb_c0 == 1.0 && spot->lb_c1 == 0.0 && spot->lb_c2 == 0.0)) &&
+                           (!facula || (facula->lb_c0 == 1.0 && facula->lb_c1 == 0.0 && facula->lb_c2 == 0.0));
+    struct Pass { int effect; void *out; } passes[3] = {{SOAP_EFFECT_TOTAL, out_total}, {SOAP_EFFECT_FLUX, out_flux}, {SOAP_EFFECT_CB, out_cb}};
+    bool have_lb_lists = false;
+    for (const Pass &ps : passes) {
+        if (!ps.out) continue;
+        const bool prepare = ps.effect == SOAP_EFFECT_CB ? !(have_lb_lists && lb_is_one) : !have_lb_lists;
+        rc = quiet->dtype == SOAP_F32
+                 ? active_impl<float>(s, quiet, spot, facula, n_regions, n_phases, ps.effect, prepare, ps.out, out_pitch, st)
+                 : active_impl<double>(s, quiet, spot, facula, n_regions, n_phases, ps.effect, prepare, ps.out, out_pitch, st);
+        if (rc) return rc;
+        if (ps.effect != SOAP_EFFECT_CB) have_lb_lists = true;
+    }
     if (n_active) {
         SOAP_CUDA(s, cudaMemcpyAsync(n_active, s->d_nactive.ptr, (size_t)n_phases * sizeof(int), cudaMemcpyDeviceToHost, st));
         SOAP_CUDA(s, cudaStreamSynchronize(st));
@@ -653,6 +673,14 @@ int soap_active_timeseries(soap_star *s, const soap_spectra *quiet, const soap_s
         s->last_active_cells = tot;
     }
     return SOAP_OK;
+}
+
+int soap_active_timeseries(soap_star *s, const soap_spectra *quiet, const soap_spectra *spot, const soap_spectra *facula,
+                           const soap_region *regions, int32_t n_regions, const double *phases, int32_t n_phases,
+                           void *out_delta, int64_t out_pitch, int32_t *n_active, void *stream) {
+    if (s && s->ready && n_phases > 0 && !out_delta) return s->fail(SOAP_ERR_INVALID_ARG, "out_delta is NULL");
+    return soap_active_timeseries_effects(s, quiet, spot, facula, regions, n_regions, phases, n_phases, out_delta, nullptr,
+                                          nullptr, out_pitch, n_active, stream);
 }
 
 int soap_get_stats(soap_star *s, soap_stats *stats, void *stream) {

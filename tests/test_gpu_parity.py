@@ -312,3 +312,72 @@ def test_argument_errors_leave_outputs_untouched(soap):
     torch.cuda.synchronize()
     assert torch.all(out == -7.0) and torch.all(D == -7.0)
     soap.soap_destroy(star)
+
+
+# ---- flux-only and CB-only outputs beside the total (Eq. 1-3) -------------------
+def _run_effects(soap, wl, which=(True, True, True)):
+    dev = torch.device("cuda:0")
+    star = soap.soap_create(0)
+    soap.soap_disk_geometry(star, wl)
+    q = soap.to_device_spectra(wl.quiet, wl.lambda0, wl.dlambda, dev)
+    s = None if wl.spot is None else soap.to_device_spectra(wl.spot, wl.lambda0, wl.dlambda, dev, wl.spot_contrast, wl.spot_lb)
+    f = None if wl.facula is None else soap.to_device_spectra(wl.facula, wl.lambda0, wl.dlambda, dev, wl.facula_contrast, wl.facula_lb)
+    tdt = torch.float32 if wl.dtype == np.float32 else torch.float64
+    outs = [torch.full((len(wl.phases), wl.n_pix), float("nan"), dtype=tdt, device=dev) if w else None for w in which]
+    na = soap.soap_active_timeseries_effects(star, q, s, f, wl.regions, wl.phases, outs[0], outs[1], outs[2], want_n_active=True)
+    torch.cuda.synchronize()
+    soap.soap_destroy(star)
+    return [o.cpu().numpy() if o is not None else None for o in outs], na
+
+
+def _check_effects(wl, outs, na, m_lo=0, m_hi=None):
+    scale = None
+    for effect, D in enumerate(outs):
+        if D is None:
+            continue
+        _, Do, nao = oracle.run_workload(wl, m_lo, m_hi, effect=effect)
+        assert np.array_equal(na, nao)
+        if scale is None:
+            scale = float(np.max(np.abs(oracle.run_workload(wl, m_lo, m_hi, effect=0)[1])))
+        # every effect is held to 1e-4 of its own max|delta|, and never looser than 1e-4 of the total's
+        tol = DELTA_TOL * min(float(np.max(np.abs(Do))), scale) if np.max(np.abs(Do)) > 0 else 0.0
+        err = float(np.max(np.abs(D[:, m_lo:m_hi].astype(np.float64) - Do)))
+        assert err <= tol, f"effect {effect}: {err:.3e} > {tol:.3e}"
+        for p in range(len(wl.phases)):
+            if nao[p] == 0:
+                assert np.all(D[p] == 0.0)
+
+
+def test_effects_match_oracle_fp32(soap):
+    wl = workloads.make_config3(n_pix=5000, n_phases=6, grid_n=120, nested=True)
+    wl.phases = np.array([0.35, 0.45, 0.5, 0.55, 0.65, 0.0])
+    outs, na = _run_effects(soap, wl)
+    assert na.max() > 0
+    _check_effects(wl, outs, na)
+
+
+def test_effects_match_oracle_fp64_config1(soap):
+    wl = workloads.make_config1()
+    outs, na = _run_effects(soap, wl)
+    _check_effects(wl, outs, na)
+
+
+def test_effects_subsets_and_total_is_unchanged(soap):
+    """Any subset of the outputs may be requested; the total equals soap_active_timeseries bit for bit."""
+    wl = workloads.make_config2(n_pix=4000, n_phases=5, grid_n=100)
+    wl.phases = np.linspace(0.4, 0.6, 5)
+    g = run_gpu(soap, wl)
+    (t, f, c), na = _run_effects(soap, wl)
+    assert np.array_equal(t, g["D"]) and np.array_equal(na, g["n_active"])
+    (t2, f2, c2), _ = _run_effects(soap, wl, which=(False, True, False))
+    assert t2 is None and c2 is None and np.array_equal(f2, f)
+    (t3, f3, c3), _ = _run_effects(soap, wl, which=(False, False, True))
+    assert np.array_equal(c3, c)
+    _check_effects(wl, (t, f, c), na)
+
+
+def test_effects_config3_full_size_sampled(soap):
+    wl = workloads.make_config3()
+    outs, na = _run_effects(soap, wl)
+    for lo, hi in _sample_ranges(wl.n_pix, n=2):
+        _check_effects(wl, outs, na, lo, hi)
