@@ -256,6 +256,42 @@ def run_graft(args):
     roofline["other_kernel"] = {"kernel": other, "kernel_ms": kern[other]["ms"],
                                 "achieved": kern[other]["units"] * FLOPS_PER_UNIT / (kern[other]["ms"] * 1e-3) / 1e12}
 
+    # ---- the run-collapsed form (SOAP_FORM_FIR): same sums, every run of entries with one integer
+    # shift collapsed into one record by the producer warps.  Reported beside the north_star form, never as it.
+    star_fir = soap.soap_create(local_rank)
+    soap.soap_set_option(star_fir, soap.binding.SOAP_OPT_FORM, 3)
+    Qf = torch.empty_like(Q)
+    Df = torch.empty_like(D)
+
+    def step_fir():
+        soap.soap_disk_geometry(star_fir, wl, want_info=False)
+        soap.soap_integrate_quiet(star_fir, q, Qf)
+        soap.soap_active_timeseries(star_fir, q, s, f, wl.regions, wl.phases, Df)
+
+    for _ in range(3):
+        step_fir()
+    fir_steps = max(5, min(args.steps, 30))
+    fir_ms = 0.0
+    soap.soap_set_option(star_fir, soap.binding.SOAP_OPT_KERNEL_TIMING, 1)
+    fq, fa = [], []
+    for _ in range(fir_steps):
+        flush_buf.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        step_fir()
+        b.record()
+        b.synchronize()
+        fir_ms += a.elapsed_time(b)
+        st = soap.soap_get_stats(star_fir)
+        fq.append(st["quiet_kernel_ms"])
+        fa.append(st["active_kernel_ms"])
+    fir_ms = sharding.max_over_ranks(fir_ms, dev) / fir_steps
+    fir = {"form": "fir (runs collapsed; SOAP_OPT_FORM=3)", "ms_per_step": fir_ms, "value": world * n_spec / (fir_ms * 1e-3),
+           "unit": "spectra/s", "quiet_kernel_ms": float(np.mean(fq)), "active_kernel_ms": float(np.mean(fa)),
+           "max_abs_diff_vs_binned_over_sum_w": float((Qf - Q).abs().max().item()) / info["sum_weights"],
+           "note": "event timing inside the library adds ~10 us per step to this figure"}
+    soap.soap_destroy(star_fir)
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ------------
     pitch = q.pitch
 
@@ -311,7 +347,7 @@ def run_graft(args):
         "executed_lerp_accumulates_per_s": world * exec_units / (ms_per_step * 1e-3),
         "definitional": {"n_visible": n_vis, "active_cells_all_phases": act_cells, "quiet_entries": stats["quiet_entries"],
                          "active_entries_all_phases": stats["active_entries"]},
-        "roofline": roofline, "clocks": clocks,
+        "roofline": roofline, "fir_form": fir, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "spectra/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms / e2e_steps, "api": "soap_synthesize_host (pinned host buffers)"},
         "gpu_launches": launches, "wall_s_timed_region": wall,

@@ -76,6 +76,7 @@ struct Params {
     int n_mu;
     int halo;                  // H: multiple of 4, >= max |delta| + 2
     int stage_bytes, raw_off, rec_off, run_off, desc_off;  // stage_layout(halo), filled by set_layout()
+    int collapse;              // SOAP_FORM_FIR: a run's entries are summed into one record {sum W, sum W a}
     const float2 *ent;         // raw entries (a_e, W_e)
     int n_tiles;
     // quiet launch
@@ -268,6 +269,65 @@ __device__ __forceinline__ void mbar_wait_backoff(uint64_t *bar, uint32_t parity
     while (!mbar_try_wait(bar, parity)) __nanosleep(40);
 }
 
+// One producer warp: turns the `count` raw entries (a, W) of a job into records and the run table of a tile
+// whose first / last pixel have lambda0/k + m = c_first / c_last.  Returns the number of runs; runs[n_runs] is
+// left to the caller.  Without `collapse`: rec[i] = {W, W a} per entry, runs[k] = (first entry, q or kFlip).
+// With it: rec[k] = {sum W, sum W a} over run k, runs[k] = (k, q), and a flip entry keeps (its raw index, kFlip).
+__device__ __forceinline__ int build_runs(const float2 *raw, int count, float c_first, float c_last, int H, int collapse,
+                                          float2 *rec, int2 *runs) {
+    const int lane = threadIdx.x & 31;
+                int n_runs = 0, carry = kFlip;  // kFlip never equals a q: the first entry opens a run
+                for (int i0 = 0; i0 < count; i0 += 32) {
+                    const int i = i0 + lane;
+                    const bool valid = i < count;
+                    int code = kFlip;
+                    float2 r2 = make_float2(0.f, 0.f);
+                    if (valid) {
+                        const float2 en = raw[i];
+                        const float qf = floorf(en.x * c_first), ql = floorf(en.x * c_last);
+                        int qi = (int)qf;
+                        qi = max(-H, min(H + 2, qi));
+                        r2 = make_float2(en.y, en.y * en.x);  // {W, W a}
+                        if (!collapse) rec[i] = r2;
+                        if (qf == ql) code = qi;
+                    }
+                    int prev = __shfl_up_sync(0xffffffffu, code, 1);
+                    if (lane == 0) prev = carry;
+                    const bool start = valid && (code == kFlip || code != prev);
+                    const unsigned mask = __ballot_sync(0xffffffffu, start);
+                    const int ridx = n_runs + __popc(mask & ((2u << lane) - 1u)) - 1;  // run this entry belongs to
+                    if (collapse) {
+                        // W lerp = W u + (W a) v is linear in {W, W a} for the fixed u, v of a run: the run's entries
+                        // collapse into one record {sum W, sum W a} (exact in exact arithmetic; fixed shuffle tree).
+                        // A flip entry keeps its raw index: the consumers read it from `raw`.
+                        const unsigned heads = mask | 1u;  // lane 0 heads a segment even when it continues a run
+                        const int seg0 = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));  // first lane of my segment
+                        const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+                        const bool tail = valid && (lane == 31 || !((vmask >> (lane + 1)) & 1u) || ((mask >> (lane + 1)) & 1u));
+    #pragma unroll
+                        for (int d = 1; d < 32; d <<= 1) {
+                            const float tx = __shfl_up_sync(0xffffffffu, r2.x, d), ty = __shfl_up_sync(0xffffffffu, r2.y, d);
+                            if (lane - d >= seg0) {
+                                r2.x += tx;
+                                r2.y += ty;
+                            }
+                        }
+                        if (tail && code != kFlip) {
+                            const bool fresh = (mask >> seg0) & 1u;  // the segment opened a run in this batch
+                            float2 acc2 = fresh ? make_float2(0.f, 0.f) : rec[ridx];
+                            rec[ridx] = make_float2(acc2.x + r2.x, acc2.y + r2.y);
+                        }
+                        if (start) runs[ridx] = make_int2(code == kFlip ? i : ridx, code);
+                        __syncwarp();
+                    } else if (start) {
+                        runs[ridx] = make_int2(i, code);
+                    }
+                    n_runs += __popc(mask);
+                    carry = __shfl_sync(0xffffffffu, code, 31);
+                }
+    return n_runs;
+}
+
 template <bool ACTIVE>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Params p) {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -338,29 +398,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             // -- records, run table, edge halo, descriptor ---------------------------------------------
             const float c_first = (float)(p.c0 + (double)m_t0);
             const float c_last = (float)(p.c0 + (double)(m_t0 + kTile - 1));
-            int n_runs = 0, carry = kFlip;  // kFlip never equals a q: the first entry opens a run
-            for (int i0 = 0; i0 < jb.count; i0 += 32) {
-                const int i = i0 + lane;
-                const bool valid = i < jb.count;
-                int code = kFlip;
-                if (valid) {
-                    const float2 en = raw[i];
-                    const float qf = floorf(en.x * c_first), ql = floorf(en.x * c_last);
-                    int qi = (int)qf;
-                    qi = max(-H, min(H + 2, qi));
-                    rec[i] = make_float2(en.y, en.y * en.x);  // {W, W a}
-                    if (qf == ql) code = qi;
-                }
-                int prev = __shfl_up_sync(0xffffffffu, code, 1);
-                if (lane == 0) prev = carry;
-                const bool start = valid && (code == kFlip || code != prev);
-                const unsigned mask = __ballot_sync(0xffffffffu, start);
-                if (start) runs[n_runs + __popc(mask & ((1u << lane) - 1u))] = make_int2(i, code);
-                n_runs += __popc(mask);
-                carry = __shfl_sync(0xffffffffu, code, 31);
-            }
+            const int n_runs = build_runs(raw, jb.count, c_first, c_last, H, p.collapse, rec, runs);
             if (lane == 0) {
-                runs[n_runs] = make_int2(jb.count, 0);  // sentinel: end of the last run
+                runs[n_runs] = make_int2(p.collapse ? n_runs : jb.count, 0);  // sentinel: end of the last run
                 desc->m_t0 = m_t0;
                 desc->flags = jb.flags;
                 desc->kind = jb.kind;
@@ -504,7 +544,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                     c = add2(c, bcast2((float)(2 * kConsumers)));  // rounding of c moves the shift by < 1e-6 px
                 }
             }
-            const int len = nxt - run.x;
+            const int len = p.collapse ? 1 : nxt - run.x;
             const float2 *re = rec + run.x;
             float2 rc = re[0];  // {W, W a}; the next record is fetched while this one is used
 #pragma unroll 2

@@ -219,6 +219,7 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     p.n_mu = s->prm.n_mu;
     p.halo = halo_for(s, q);
     f32::set_layout(p);
+    p.collapse = s->form_used == SOAP_FORM_FIR ? 1 : 0;
     p.ent = s->d_ent32.ptr;
     p.row_start = s->d_row_start.ptr;
     p.n_tiles = n_tiles;
@@ -361,6 +362,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         p.n_mu = n_mu;
         p.halo = halo_for(s, q);
         f32::set_layout(p);
+        p.collapse = s->form_used == SOAP_FORM_FIR ? 1 : 0;
         p.ent = reinterpret_cast<const float2 *>(s->d_aent.ptr);
         p.n_tiles = (int)((q->n_pix + f32::kTile - 1) / f32::kTile);
         p.jobs = s->d_jobs.ptr;
@@ -529,7 +531,6 @@ int soap_set_option(soap_star *s, int32_t option, int64_t value) {
     switch (option) {
         case SOAP_OPT_FORM:
             if (value < SOAP_FORM_AUTO || value > SOAP_FORM_FIR) return s->fail(SOAP_ERR_INVALID_ARG, "unknown form %lld", (long long)value);
-            if (value == SOAP_FORM_FIR) return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_FIR is not implemented in this build");
             if ((int)value != s->form) s->ready = false;  // entry list must be rebuilt
             s->form = (int)value;
             return SOAP_OK;
@@ -573,7 +574,7 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     s->cosi = cosi;
     const int N = prm->grid_n, n_mu = prm->n_mu;
     const size_t ncell = (size_t)N * N;
-    s->form_used = (s->form == SOAP_FORM_CELLS) ? SOAP_FORM_CELLS : SOAP_FORM_BINNED;
+    s->form_used = (s->form == SOAP_FORM_CELLS || s->form == SOAP_FORM_FIR) ? s->form : SOAP_FORM_BINNED;
     const double vmax = std::fabs(prm->vsini_kms * sini) * (double)(N - 1) / (double)N;
     s->amax = std::max(std::fabs(host_dshift(vmax, prm->doppler_mode)), std::fabs(host_dshift(-vmax, prm->doppler_mode)));
 

@@ -111,9 +111,9 @@ def test_config2_full(soap):
     assert_parity(wl, g)
 
 
-@pytest.mark.parametrize("form", [1, 2])
+@pytest.mark.parametrize("form", [1, 2, 3])
 def test_forms_agree_with_oracle(soap, form):
-    """Pre-binned (column, mu-bin) entries and the literal one-entry-per-cell form."""
+    """Pre-binned (column, mu-bin) entries, the literal one-entry-per-cell form, and the run-collapsed (FIR) form."""
     wl = workloads.make_config2(n_pix=3000, n_phases=8, grid_n=120)
     wl.phases = np.linspace(0.3, 0.7, 8)
     g = run_gpu(soap, wl, form=form)
@@ -381,3 +381,20 @@ def test_effects_config3_full_size_sampled(soap):
     outs, na = _run_effects(soap, wl)
     for lo, hi in _sample_ranges(wl.n_pix, n=2):
         _check_effects(wl, outs, na, lo, hi)
+
+
+def test_fir_form_config3_full_size_sampled(soap):
+    """SOAP_FORM_FIR (every run of entries with one integer shift collapsed into one record) at full size."""
+    wl = workloads.make_config3()
+    g = run_gpu(soap, wl, form=3)
+    assert g["stats"]["form"] == 3
+    for lo, hi in _sample_ranges(wl.n_pix, n=3):
+        assert_parity(wl, g, lo, hi)
+
+
+def test_fir_form_fast_rotator(soap):
+    wl = workloads.make_config5_star(3, n_pix=6000, n_phases=4, grid_n=90)
+    wl.vsini_kms = 20.0
+    wl.phases = np.array([0.4, 0.5, 0.6, 0.0])
+    g = run_gpu(soap, wl, form=3)
+    assert_parity(wl, g)
