@@ -46,6 +46,7 @@ struct ActiveCounters {  // device-resident
     unsigned long long active_entries;  // sum over phases of entries (pad entries not counted)
     unsigned int done;                  // CTAs finished (reset by the last one)
     unsigned int pad;
+    int item_next, item_ctas_done;      // hand-out of (phase, tile) items in the active launch (self-resetting)
 };
 
 struct PrepArgs {

@@ -37,8 +37,8 @@
 //   * quiet launch: the flattened (tile, entry) work list is cut into equal contiguous ranges, one per
 //     CTA, grid = resident CTA slots (one wave, no tail); a CTA writes one fp64 partial per tile it
 //     touches and the last CTA to deliver its share of a tile adds the shares in CTA order (deterministic).
-//   * active launch: persistent CTAs; the (phase, tile) items, heaviest phase first, are dealt to the
-//     CTAs in snake order (active_prepare_kernel builds the per-phase job lists and the order); the
+//   * active launch: persistent CTAs take the (phase, tile) items, heaviest phase first, from a global
+//     counter (active_prepare_kernel builds the per-phase job lists and the order); the
 //     post-shift contrast (I_ratio of Eq. 3) multiplies each kind's fp64 sum once per pixel (a6).
 #pragma once
 #include <climits>
@@ -88,6 +88,7 @@ struct Params {
     const ActiveJob *jobs;     // [n_phases][job_cap]
     const int *n_jobs;         // [n_phases]
     const int *phase_order;    // [n_phases] heaviest first
+    int *item_counters;        // [2] item hand-out (zero between launches)
     int job_cap, n_phases;
     float *out;                // [n_phases][out_pitch]
     long long out_pitch;
@@ -119,7 +120,7 @@ __host__ __device__ inline StageLayout stage_layout(int halo) {
     l.stage_bytes = (l.desc_off + sizeof(Desc) + 127) & ~(size_t)127;
     return l;
 }
-constexpr size_t kHeaderBytes = 128;                          // mbarriers (96 B) + tile hand-over words
+constexpr size_t kHeaderBytes = 512;                          // mbarriers (96 B), tile hand-over words, item queue (at 128)
 constexpr size_t kFinBytes = (size_t)kTile * (sizeof(double) + sizeof(float));  // active launch: per-pixel fp64
                                                                               // contrast-weighted sums + staged contrast
 __host__ inline size_t smem_bytes(int halo, bool active) {
@@ -202,44 +203,100 @@ struct QuietSource {
     }
 };
 
-// Active launch: items = (phase, tile), ordered heaviest phase first; round i deals items i G .. i G + G - 1 to
-// the G CTAs, forwards in even rounds and backwards in odd ones (snake order: static, hence deterministic,
-// and within one item's work of balanced).  An item's jobs are its phase's job list applied to its tile; a
-// phase without covered cells yields one empty job so that its zeros are written (reading S19).
+// Active launch: items = (phase, tile), ordered heaviest phase first, handed out through one global counter:
+// a CTA takes the next item whenever its producers run short of jobs (heaviest-first list scheduling: the
+// CTAs finish within one small item of each other).  Which CTA computes an item does not change its result,
+// so the output stays run-to-run identical.  Producer warp 0 is the CTA's scheduler: it fetches item numbers
+// and publishes (item, first job number) in a small shared-memory ring that the four producer warps read in
+// step; it stays kQueueAhead jobs ahead of its own position.  An item's jobs are its phase's job list applied
+// to its tile; a phase without covered cells yields one empty job so that its zeros are written (S19).
+constexpr int kQueueSlots = 32;  // items in flight per CTA: the producers are never more than ~16 jobs apart
+constexpr int kQueueAhead = 2 * kStages;
+struct ItemQueue {               // shared memory
+    int2 slot[kQueueSlots];      // (item index or -1 = no more items, number of the item's first job)
+    int tail;                    // items published
+};
+
 struct ActiveSource {
     const ActiveJob *jobs;
     const int *n_jobs, *phase_order;
-    long long n_items, G, c;
+    int *counters;  // [0] next item, [1] CTAs that finished fetching (both zero between launches)
+    ItemQueue *queue;
+    long long n_items;
     int n_tiles, job_cap;
-    long long i;
+    bool scheduler;
+    int pub, pub_end;  // scheduler: items published, job number after the last of them
+    bool pub_done;
+    int i;             // item this warp is working through
     int n0, nj, cnt, phase, tile;
     bool done;
-    __device__ void load_item() {
-        const long long idx = i * G + ((i & 1) ? (G - 1 - c) : c);
-        done = idx >= n_items;
-        if (done) return;
-        phase = __ldg(&phase_order[idx / n_tiles]);
-        tile = (int)(idx % n_tiles);
-        cnt = __ldg(&n_jobs[phase]);
-        nj = cnt > 0 ? cnt : 1;
+    __device__ int jobs_of(long long idx, int &ph, int &tl, int &c) const {
+        ph = __ldg(&phase_order[idx / n_tiles]);
+        tl = (int)(idx % n_tiles);
+        c = __ldg(&n_jobs[ph]);
+        return c > 0 ? c : 1;
     }
-    __device__ void init(const Params &p, long long cta, long long G_) {
+    // scheduler warp: publish items until they cover job number n_need (or the list is exhausted)
+    __device__ void publish_until(int n_need) {
+        const int lane = threadIdx.x & 31;
+        while (!pub_done && pub_end <= n_need) {
+            int idx = 0;
+            if (lane == 0) idx = atomicAdd(&counters[0], 1);
+            idx = __shfl_sync(0xffffffffu, idx, 0);
+            int add = 0;
+            if (idx >= n_items) {
+                pub_done = true;
+                idx = -1;
+                if (lane == 0 && atomicAdd(&counters[1], 1) == (int)gridDim.x - 1) {  // every CTA has stopped fetching
+                    counters[0] = 0;
+                    counters[1] = 0;
+                }
+            } else {
+                int ph, tl, c;
+                add = jobs_of(idx, ph, tl, c);
+            }
+            if (lane == 0) {
+                queue->slot[pub % kQueueSlots] = make_int2(idx, pub_end);
+                __threadfence_block();
+                *reinterpret_cast<volatile int *>(&queue->tail) = pub + 1;
+            }
+            ++pub;
+            pub_end += add;
+            __syncwarp();
+        }
+    }
+    __device__ void load_item() {
+        const volatile int *tail = reinterpret_cast<const volatile int *>(&queue->tail);
+        while (*tail <= i) __nanosleep(20);
+        __threadfence_block();
+        const volatile int *sl = reinterpret_cast<const volatile int *>(&queue->slot[i % kQueueSlots]);
+        const int idx = sl[0];
+        n0 = sl[1];
+        done = idx < 0;
+        if (done) return;
+        nj = jobs_of(idx, phase, tile, cnt);
+    }
+    __device__ void init(const Params &p, ItemQueue *q, bool is_scheduler) {
         jobs = p.jobs;
         n_jobs = p.n_jobs;
         phase_order = p.phase_order;
+        counters = p.item_counters;
+        queue = q;
         n_tiles = p.n_tiles;
         job_cap = p.job_cap;
         n_items = (long long)p.n_phases * p.n_tiles;
-        G = G_;
-        c = cta;
-        i = 0;
+        scheduler = is_scheduler;
+        pub = 0;
+        pub_end = 0;
+        pub_done = false;
+        i = -1;
         n0 = 0;
         nj = 0;
-        load_item();
+        done = false;
     }
     __device__ int get(int n, Job &j) {
+        if (scheduler) publish_until(n + kQueueAhead);
         while (!done && n >= n0 + nj) {
-            n0 += nj;
             ++i;
             load_item();
         }
@@ -328,6 +385,13 @@ __device__ __forceinline__ int build_runs(const float2 *raw, int count, float c_
     return n_runs;
 }
 
+__device__ __forceinline__ void init_source(QuietSource &src, const Params &p, ItemQueue *, bool) {
+    src.init(p, blockIdx.x, gridDim.x);
+}
+__device__ __forceinline__ void init_source(ActiveSource &src, const Params &p, ItemQueue *q, bool is_scheduler) {
+    src.init(p, q, is_scheduler);
+}
+
 template <bool ACTIVE>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Params p) {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -350,6 +414,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             mbar_init(&bar_empty[s], kConsumerWarps);
         }
         fence_mbar_init();
+        reinterpret_cast<ItemQueue *>(smem + 128)->tail = 0;
     }
     __syncthreads();
 
@@ -364,7 +429,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         int2 *runs = reinterpret_cast<int2 *>(sb + p.run_off);
         Desc *desc = reinterpret_cast<Desc *>(sb + p.desc_off);
         typename std::conditional<ACTIVE, ActiveSource, QuietSource>::type src;
-        src.init(p, blockIdx.x, gridDim.x);
+        init_source(src, p, reinterpret_cast<ItemQueue *>(smem + 128), st == 0);
         Job jb;
         for (int n = st, use = 0;; n += kStages, ++use) {
             const int status = src.get(n, jb);

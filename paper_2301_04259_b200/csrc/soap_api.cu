@@ -368,6 +368,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         p.jobs = s->d_jobs.ptr;
         p.n_jobs = d_njobs;
         p.phase_order = d_order;
+        p.item_counters = reinterpret_cast<int *>(&s->d_counters.ptr->item_next);
         p.job_cap = job_cap;
         p.n_phases = n_phases;
         p.out = static_cast<float *>(out);
