@@ -70,6 +70,9 @@ def _load():
             ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.POINTER(_Region), ctypes.c_int32,
             ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_void_p,
             ctypes.c_void_p]
+        lib.soap_oracle_lower_resolution.restype = ctypes.c_int
+        lib.soap_oracle_lower_resolution.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_double,
+                                                     ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -189,3 +192,19 @@ def run_workload(wl, m_lo: int = 0, m_hi: Optional[int] = None, effect: int = 0)
                              wl.phases, wl.spot_contrast, wl.facula_contrast, wl.spot_lb, wl.facula_lb,
                              m_lo, m_hi, effect)
     return Q, delta, n_active
+
+
+LSF_NSIG = 5.0  # truncation of the line-spread function in sigmas (reading R-LSF)
+
+
+def lower_resolution(rows, lambda0: float, k: float, R: float, nsig: float = LSF_NSIG) -> np.ndarray:
+    """Resolution lowering of PAPER.md:85 / Alg. 5 P:244 with a Gaussian LSF of FWHM lambda/R (reading R-LSF).
+    rows: [n_rows, P] (or [P]); returns the same shape in fp64."""
+    lib = _load()
+    a = _f64(np.atleast_2d(rows))
+    out = np.empty_like(a)
+    rc = lib.soap_oracle_lower_resolution(a.ctypes.data, a.shape[0], a.shape[1], float(lambda0), float(k), float(R),
+                                          float(nsig), out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"soap_oracle_lower_resolution failed: {rc}")
+    return out.reshape(np.shape(rows))

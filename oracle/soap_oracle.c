@@ -333,3 +333,43 @@ int soap_oracle_active_effect(const oracle_star *st, const double *S_quiet, cons
     free(w); free(mu); free(D); free(bin); free(type_map);
     return 0;
 }
+
+/* Resolution lowering (Alg. 2, Alg. 5: "lower the resolution of the final spectrum to
+ * match the resolution provided in the configuration file").  The paper names no kernel; reading R-LSF:
+ * a Gaussian line-spread function of FWHM lambda / R, sampled on the pixel grid at every output pixel,
+ *   sigma_m = lambda_m / (R * 2 sqrt(2 ln 2)),   g_m(j) = exp(-(j k)^2 / (2 sigma_m^2)),   |j| <= J_m = ceil(nsig sigma_m / k),
+ *   out[m] = sum_j g_m(j) in[clamp(m + j, 0, P-1)] / sum_j g_m(j)
+ * (discretely normalised, ends clamped like reading S8).  in / out: [n_rows][P], rows independent.  R <= 0 copies. */
+int soap_oracle_lower_resolution(const double *in, int64_t n_rows, int64_t P, double lambda0, double k,
+                                 double R, double nsig, double *out) {
+    if (!in || !out || P < 1 || n_rows < 0 || !(k > 0.0) || !(nsig > 0.0)) return -1;
+    const double fwhm_to_sigma = 1.0 / (2.0 * sqrt(2.0 * log(2.0)));
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < P; ++m) {
+        if (!(R > 0.0)) {
+            for (int64_t r = 0; r < n_rows; ++r) out[r * P + m] = in[r * P + m];
+            continue;
+        }
+        const double lam = lambda0 + k * (double)m;
+        const double sigma = lam / R * fwhm_to_sigma;
+        const int64_t J = (int64_t)ceil(nsig * sigma / k);
+        double norm = 0.0;
+        for (int64_t j = -J; j <= J; ++j) {
+            const double d = (double)j * k;
+            norm += exp(-(d * d) / (2.0 * sigma * sigma));
+        }
+        for (int64_t r = 0; r < n_rows; ++r) {
+            const double *row = in + r * P;
+            double acc = 0.0;
+            for (int64_t j = -J; j <= J; ++j) {
+                int64_t n = m + j;
+                if (n < 0) n = 0;
+                if (n > P - 1) n = P - 1;
+                const double d = (double)j * k;
+                acc += exp(-(d * d) / (2.0 * sigma * sigma)) * row[n];
+            }
+            out[r * P + m] = acc / norm;
+        }
+    }
+    return 0;
+}
