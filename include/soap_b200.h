@@ -184,6 +184,18 @@ int soap_active_timeseries_effects(soap_star *star, const soap_spectra *quiet, c
                                    const double *phases, int32_t n_phases, void *out_total, void *out_flux,
                                    void *out_cb, int64_t out_pitch, int32_t *n_active, void *stream);
 
+/* ---- resolution lowering (Alg. 2, Alg. 5) ------------------------------------
+ * "Lower the resolution of the final spectrum to match the resolution provided in the configuration file."  The
+ * paper names no kernel; this library's reading (DESIGN.md R-LSF) is a Gaussian line-spread function of FWHM
+ * lambda / resolution, sampled on the pixel grid and normalised at every output pixel, truncated at 5 sigma, ends
+ * clamped (S8):  out[r][m] = sum_j g_m(j) in[r][clamp(m+j)] / sum_j g_m(j),  g_m(j) = exp(-(j dlambda)^2 / 2 sigma_m^2),
+ * sigma_m = lambda_m / (resolution * 2 sqrt(2 ln 2)).  Rows are independent (e.g. Q + delta_p for every phase).
+ *   in:  DEVICE [n_rows][in_pitch] of `dtype`;  out: DEVICE [n_rows][out_pitch], must not alias `in`.
+ * Needs no geometry.  SOAP_ERR_UNSUPPORTED if the LSF is wider than 96 pixels on a side. */
+int soap_lower_resolution(soap_star *star, const void *in, int64_t n_rows, int64_t n_pix, int64_t in_pitch,
+                          int32_t dtype, double lambda0, double dlambda, double resolution, void *out,
+                          int64_t out_pitch, void *stream);
+
 /* ---- debug export of the geometry (HOST outputs, N*N each, any may be NULL; synchronous) --------
  * Hidden cells: mu = 0, vel = 0, w = 0, bin = -1. */
 int soap_export_geometry(soap_star *star, double *mu, double *vel, double *w, int32_t *bin);

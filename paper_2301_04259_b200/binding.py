@@ -28,7 +28,7 @@ SOAP_OPT_FORM, SOAP_OPT_QUIET_SPLITS, SOAP_OPT_KERNEL_TIMING = 1, 2, 3
 EXPORTED_SYMBOLS = (
     "soap_version", "soap_create", "soap_destroy", "soap_last_error", "soap_set_option", "soap_get_stats",
     "soap_disk_geometry", "soap_integrate_quiet", "soap_active_timeseries", "soap_active_timeseries_effects",
-    "soap_export_geometry",
+    "soap_export_geometry", "soap_lower_resolution",
     "soap_synthesize_host", "soap_batch_integrate_quiet", "soap_batch_active_timeseries",
 )
 
@@ -102,6 +102,8 @@ def load_library() -> ctypes.CDLL:
                                                    ctypes.POINTER(ctypes.c_double), i32, vp, vp, vp, i64,
                                                    ctypes.POINTER(i32), vp]
     lib.soap_export_geometry.argtypes = [vp, vp, vp, vp, vp]
+    lib.soap_lower_resolution.argtypes = [vp, vp, i64, i64, i64, i32, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                          vp, i64, vp]
     lib.soap_synthesize_host.argtypes = [vp, ctypes.POINTER(c_star_params), ctypes.POINTER(c_spectra),
                                          ctypes.POINTER(c_spectra), ctypes.POINTER(c_spectra),
                                          ctypes.POINTER(c_region), i32, ctypes.POINTER(ctypes.c_double), i32,
@@ -285,6 +287,18 @@ def soap_active_timeseries_effects(star: Star, quiet: Spectra, spot: Optional[Sp
         out_cb.data_ptr() if out_cb is not None else None, out_pitch,
         na.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)) if na is not None else None, _stream_handle(stream)))
     return na[:n_ph] if na is not None else None
+
+
+def soap_lower_resolution(star: Star, rows: torch.Tensor, n_pix: int, lambda0: float, dlambda: float, resolution: float,
+                          out: torch.Tensor, stream=None) -> None:
+    """rows, out: DEVICE tensors [n_rows, pitch] (or [pitch]) of one dtype; Gaussian LSF of FWHM lambda/resolution."""
+    r2 = rows if rows.dim() == 2 else rows.unsqueeze(0)
+    o2 = out if out.dim() == 2 else out.unsqueeze(0)
+    if r2.dtype != o2.dtype or r2.shape[0] != o2.shape[0]:
+        raise ValueError("rows and out must agree in dtype and row count")
+    star._check(star._lib.soap_lower_resolution(
+        star._h, r2.data_ptr(), int(r2.shape[0]), int(n_pix), int(r2.stride(0)), _dtype_code(r2), float(lambda0),
+        float(dlambda), float(resolution), o2.data_ptr(), int(o2.stride(0)), _stream_handle(stream)))
 
 
 def soap_export_geometry(star: Star, grid_n: int) -> dict:

@@ -1,0 +1,277 @@
+// Resolution lowering (Alg. 2, Alg. 5; reading R-LSF):
+// every spectrum row is convolved with a Gaussian line-spread function of FWHM lambda / R sampled on the pixel
+// grid, per output pixel m:
+//   sigma_m = lambda_m / (R 2 sqrt(2 ln 2)),  g_m(j) = exp(-(j k)^2 / (2 sigma_m^2)),  |j| <= J_m = ceil(nsig sigma_m / k),
+//   out[m] = sum_j g_m(j) in[clamp(m + j)] / sum_j g_m(j).
+//
+// The kernel is HBM-bound (one read and one write of every row; ~20 FMAs per pixel).  A thread owns one pixel
+// of a 256-pixel tile for ALL rows: its normalised weights (fp64 exp, rounded once to the I/O type) are computed
+// once (two exponentials and a product recurrence) and kept in shared memory ([tap][thread]: conflict-free),
+// then row after row the tile plus its halo is staged in shared memory with coalesced loads (double-buffered: the
+// next row is in flight while this one is computed) and every thread adds its symmetric taps from the outside in.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "ptx_helpers.cuh"
+
+namespace soap {
+
+constexpr int kLsfThreads = 256;
+constexpr int kLsfMaxJ = 96;      // taps on each side the kernel supports (host checks)
+constexpr double kLsfNsig = 5.0;  // truncation in sigmas (reading R-LSF); the oracle uses the same constant
+
+struct LsfArgs {
+    const void *in;
+    void *out;
+    long long n_rows, n_pix, in_pitch, out_pitch;
+    double lambda0, k, R, fwhm_to_sigma;
+    int J_max;  // J of the last pixel (sigma grows with lambda): halo of every tile
+};
+
+__host__ __device__ inline size_t lsf_smem_bytes(int J_max, size_t elem) {
+    return ((size_t)(J_max + 1) * kLsfThreads + 2 * (size_t)(kLsfThreads + 2 * J_max)) * elem;  // weights + 2 row tiles
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kLsfThreads) lower_resolution_kernel(const LsfArgs a) {
+    extern __shared__ __align__(16) unsigned char lsf_smem[];
+    T *w = reinterpret_cast<T *>(lsf_smem);            // [J_max + 1][kLsfThreads]
+    T *s = w + (size_t)(a.J_max + 1) * kLsfThreads;    // [kLsfThreads + 2 J_max]
+    const int tid = threadIdx.x, J = a.J_max;
+    const long long m0 = (long long)blockIdx.x * kLsfThreads;
+    const long long m = m0 + tid;
+    // ---- this pixel's weights -------------------------------------------------------------------------
+    int Jm = 0;
+    if (m < a.n_pix) {
+        const double lam = __dadd_rn(a.lambda0, __dmul_rn(a.k, (double)m));
+        const double sigma = __dmul_rn(__ddiv_rn(lam, a.R), a.fwhm_to_sigma);
+        Jm = (int)ceil(__ddiv_rn(__dmul_rn(kLsfNsig, sigma), a.k));
+        Jm = min(Jm, J);
+        // g(j) = exp(-j^2 h), h = k^2 / (2 sigma^2): g(j+1) = g(j) rho_j with rho_j = rho_{j-1} exp(-2h), rho_0 = exp(-h)
+        // (two exponentials per pixel instead of J; the products round to ~J ulp of fp64)
+        const double h = (a.k * a.k) / (2.0 * sigma * sigma);
+        const double q = exp(-2.0 * h);
+        double rho = exp(-h), g = 1.0, norm = 1.0;
+        for (int j = 1; j <= Jm; ++j) {
+            g *= rho;
+            rho *= q;
+            norm += 2.0 * g;
+        }
+        const double inv = 1.0 / norm;
+        rho = exp(-h);
+        g = 1.0;
+        for (int j = 0; j <= J; ++j) {
+            w[(size_t)j * kLsfThreads + tid] = j <= Jm ? (T)(g * inv) : (T)0;
+            g *= rho;
+            rho *= q;
+        }
+    }
+    // ---- rows --------------------------------------------------------------------------------------------
+    const T *in = static_cast<const T *>(a.in);
+    T *out = static_cast<T *>(a.out);
+    // double-buffered row tiles: the next row's samples are in flight (registers) while this row is computed
+    const int span = kLsfThreads + 2 * J;
+    constexpr int kPer = (kLsfThreads + 2 * kLsfMaxJ + kLsfThreads - 1) / kLsfThreads;  // samples a thread stages
+    auto fetch = [&](long long r, T (&v)[kPer]) {
+        const T *row = in + r * a.in_pitch;
+#pragma unroll
+        for (int u = 0; u < kPer; ++u) {
+            const int qq = tid + u * kLsfThreads;
+            long long n = m0 - J + qq;
+            n = n < 0 ? 0 : (n > a.n_pix - 1 ? a.n_pix - 1 : n);  // ends clamped (reading S8)
+            v[u] = qq < span ? row[n] : (T)0;
+        }
+    };
+    auto stage = [&](T *dst, const T (&v)[kPer]) {
+#pragma unroll
+        for (int u = 0; u < kPer; ++u) {
+            const int qq = tid + u * kLsfThreads;
+            if (qq < span) dst[qq] = v[u];
+        }
+    };
+    T v[kPer];
+    long long r = blockIdx.y;
+    if (r < a.n_rows) {
+        fetch(r, v);
+        stage(s, v);
+    }
+    int cur = 0;
+    __syncthreads();  // weights and the first tile are in place
+    for (; r < a.n_rows; r += gridDim.y) {
+        const long long rn = r + gridDim.y;
+        if (rn < a.n_rows) fetch(rn, v);
+        if (m < a.n_pix) {
+            const T *c = s + (size_t)cur * span + J + tid;
+            T acc0 = (T)0, acc1 = (T)0;  // two chains, both from the small outer taps inward
+            int j = Jm;
+            if (j & 1) {
+                acc1 = w[(size_t)j * kLsfThreads + tid] * (c[-j] + c[j]);
+                --j;
+            }
+#pragma unroll 2
+            for (; j >= 2; j -= 2) {
+                acc0 += w[(size_t)j * kLsfThreads + tid] * (c[-j] + c[j]);
+                acc1 += w[(size_t)(j - 1) * kLsfThreads + tid] * (c[-(j - 1)] + c[j - 1]);
+            }
+            out[r * a.out_pitch + m] = (acc0 + acc1) + w[tid] * c[0];
+        }
+        if (rn < a.n_rows) stage(s + (size_t)(cur ^ 1) * span, v);
+        cur ^= 1;
+        __syncthreads();
+    }
+}
+
+// ---- fp32 fast path -------------------------------------------------------------------------------------------
+// The generic kernel above issues ~200 instructions per output pixel (one shared-memory load per sample and per
+// weight).  Here a thread owns 4 consecutive pixels of a 1024-pixel tile: its sample window (4 + 2 J4 floats, J4 =
+// taps per side rounded up to a multiple of 4, a template parameter so that the window lives in registers) is read
+// with LDS.128, the 4 x (J4 + 1) weights stay in registers (from shared memory they would cost two thirds of the
+// shared-memory bandwidth and bind the kernel), and rows are written with 16-byte stores: ~30 instructions per output.  Persistent CTAs walk a contiguous range of (tile, row) items in tile-major order,
+// so the per-pixel weights (exact, as above) are recomputed only when the tile changes, and the next item's tile
+// is in flight while the current one is computed.  Requires 16-byte aligned rows (pitch % 4 == 0).
+constexpr int kLsfV = 4;
+constexpr int kLsfTileV = kLsfThreads * kLsfV;
+constexpr int kLsfStages = 8;  // row tiles in flight per CTA (cp.async ring): ~60 KB per SM in flight covers the HBM latency
+
+template <int J4>
+__host__ __device__ constexpr size_t lsf_v_smem_bytes() {
+    return kLsfStages * (size_t)(kLsfTileV + 2 * J4) * sizeof(float);
+}
+
+template <int J4>
+__global__ void __launch_bounds__(kLsfThreads, J4 <= 16 ? 2 : 1) lower_resolution_v_kernel(const LsfArgs a) {
+    extern __shared__ __align__(16) unsigned char lsf_smem[];
+    float *s = reinterpret_cast<float *>(lsf_smem);  // [kLsfStages][kLsfTileV + 2 J4]
+    float wr[J4 + 1][kLsfV];                         // this thread's weights: registers (shared memory would bind)
+    constexpr int span = kLsfTileV + 2 * J4, span4 = span / 4;
+    constexpr int kPer = (span4 + kLsfThreads - 1) / kLsfThreads;
+    const int tid = threadIdx.x;
+    const float *in = static_cast<const float *>(a.in);
+    float *out = static_cast<float *>(a.out);
+    const long long n_tiles = (a.n_pix + kLsfTileV - 1) / kLsfTileV;
+    const long long items = n_tiles * a.n_rows;
+    const long long it0 = items * blockIdx.x / gridDim.x, it1 = items * (blockIdx.x + 1) / gridDim.x;
+    if (it0 >= it1) return;
+
+    // asynchronous 16-byte copies straight into the ring (inner tiles); end tiles are clamped by hand (reading S8)
+    // (tile, row) cursors advance by increments: no 64-bit divisions in the loops
+    struct Cursor {
+        long long it;
+        int tile, r;
+    };
+    auto advance = [&](Cursor &c) {
+        ++c.it;
+        if (++c.r == (int)a.n_rows) {
+            c.r = 0;
+            ++c.tile;
+        }
+    };
+    auto issue = [&](const Cursor &ci, float *dst) {
+        if (ci.it < it1) {
+            const long long tile = ci.tile, r = ci.r;
+            const long long g0 = tile * kLsfTileV - J4;  // global pixel of tile-array position 0 (multiple of 4)
+            const float *row = in + r * a.in_pitch;
+            const bool inner = g0 >= 0 && g0 + span <= a.n_pix;
+#pragma unroll
+            for (int u = 0; u < kPer; ++u) {
+                const int q4 = tid + u * kLsfThreads;
+                if (q4 >= span4) continue;
+                if (inner) {
+                    cp_async_16(dst + 4 * q4, row + g0 + 4 * q4);
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        long long n = g0 + 4 * q4 + c;
+                        n = n < 0 ? 0 : (n > a.n_pix - 1 ? a.n_pix - 1 : n);
+                        dst[4 * q4 + c] = row[n];
+                    }
+                }
+            }
+        }
+        cp_async_commit();  // one group per item, empty or not: the wait below counts groups
+    };
+    auto weights = [&](long long tile) {  // exact per-pixel weights of this thread's 4 pixels (see the generic kernel)
+#pragma unroll
+        for (int p = 0; p < kLsfV; ++p) {
+            const long long m = tile * kLsfTileV + kLsfV * tid + p;
+            const double lam = __dadd_rn(a.lambda0, __dmul_rn(a.k, (double)m));
+            const double sigma = __dmul_rn(__ddiv_rn(lam, a.R), a.fwhm_to_sigma);
+            int Jm = (int)ceil(__ddiv_rn(__dmul_rn(kLsfNsig, sigma), a.k));
+            Jm = min(Jm, J4);
+            const double h = (a.k * a.k) / (2.0 * sigma * sigma);
+            const double q = exp(-2.0 * h), rho0 = exp(-h);
+            double rho = rho0, g = 1.0, norm = 1.0;
+            for (int j = 1; j <= Jm; ++j) {
+                g *= rho;
+                rho *= q;
+                norm += 2.0 * g;
+            }
+            const double inv = 1.0 / norm;
+            rho = rho0;
+            g = 1.0;
+#pragma unroll
+            for (int j = 0; j <= J4; ++j) {
+                wr[j][p] = j <= Jm ? (float)(g * inv) : 0.f;
+                g *= rho;
+                rho *= q;
+            }
+        }
+    };
+
+    Cursor cc, ci;  // compute and issue cursors
+    cc.it = it0;
+    cc.tile = (int)(it0 / a.n_rows);
+    cc.r = (int)(it0 - (long long)cc.tile * a.n_rows);
+    ci = cc;
+#pragma unroll 1
+    for (int d = 0; d < kLsfStages - 1; ++d) {
+        issue(ci, s + (size_t)d * span);
+        advance(ci);
+    }
+    long long cur_tile = cc.tile;
+    weights(cur_tile);
+    int cur = 0;
+    for (; cc.it < it1; advance(cc)) {
+        const long long tile = cc.tile, r = cc.r;
+        cp_async_wait_group<kLsfStages - 2>();  // this item's tile has landed (for this thread's copies) ...
+        __syncthreads();                        // ... and for everyone's; the previous item has been consumed
+        if (tile != cur_tile) {  // uniform: the whole CTA moves to the next tile
+            weights(tile);
+            cur_tile = tile;
+        }
+        issue(ci, s + (size_t)((cur + kLsfStages - 1) % kLsfStages) * span);
+        advance(ci);
+        // ---- this thread's window and its 4 outputs ---------------------------------------------------
+        float win[kLsfV + 2 * J4];
+        const float4 *c4 = reinterpret_cast<const float4 *>(s + (size_t)cur * span) + tid;  // window starts at float 4 tid
+#pragma unroll
+        for (int u = 0; u < (kLsfV + 2 * J4) / 4; ++u) {
+            const float4 t = c4[u];
+            win[4 * u] = t.x;
+            win[4 * u + 1] = t.y;
+            win[4 * u + 2] = t.z;
+            win[4 * u + 3] = t.w;
+        }
+        float acc[kLsfV] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int j = J4; j >= 1; --j) {  // small outer taps first
+#pragma unroll
+            for (int p = 0; p < kLsfV; ++p) acc[p] = fmaf(wr[j][p], win[J4 + p - j] + win[J4 + p + j], acc[p]);
+        }
+#pragma unroll
+        for (int p = 0; p < kLsfV; ++p) acc[p] = fmaf(wr[0][p], win[J4 + p], acc[p]);
+        const long long m = tile * kLsfTileV + kLsfV * tid;
+        float *o = out + r * a.out_pitch + m;
+        if (m + 3 < a.n_pix) {
+            *reinterpret_cast<float4 *>(o) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+        } else {
+#pragma unroll
+            for (int p = 0; p < kLsfV; ++p)
+                if (m + p < a.n_pix) o[p] = acc[p];
+        }
+        cur = (cur + 1) % kLsfStages;
+    }
+}
+
+}  // namespace soap

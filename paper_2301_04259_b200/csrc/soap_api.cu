@@ -16,6 +16,7 @@
 #include "../../include/soap_b200.h"
 #include "active.cuh"
 #include "geometry.cuh"
+#include "lsf.cuh"
 #include "sia.cuh"
 #include "sia_f32.cuh"
 
@@ -683,6 +684,77 @@ int soap_active_timeseries(soap_star *s, const soap_spectra *quiet, const soap_s
     if (s && s->ready && n_phases > 0 && !out_delta) return s->fail(SOAP_ERR_INVALID_ARG, "out_delta is NULL");
     return soap_active_timeseries_effects(s, quiet, spot, facula, regions, n_regions, phases, n_phases, out_delta, nullptr,
                                           nullptr, out_pitch, n_active, stream);
+}
+
+int soap_lower_resolution(soap_star *s, const void *in, int64_t n_rows, int64_t n_pix, int64_t in_pitch, int32_t dtype,
+                          double lambda0, double dlambda, double resolution, void *out, int64_t out_pitch, void *stream) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!in || !out) return s->fail(SOAP_ERR_INVALID_ARG, "in / out is NULL");
+    if (in == out) return s->fail(SOAP_ERR_INVALID_ARG, "in-place resolution lowering is not supported");
+    if (n_rows < 0 || n_pix < 1 || in_pitch < n_pix || out_pitch < n_pix) return s->fail(SOAP_ERR_INVALID_ARG, "bad n_rows / n_pix / pitch");
+    if (dtype != SOAP_F32 && dtype != SOAP_F64) return s->fail(SOAP_ERR_INVALID_ARG, "unknown dtype %d", dtype);
+    if (!(dlambda > 0.0) || !(lambda0 > 0.0) || !std::isfinite(dlambda) || !std::isfinite(lambda0))
+        return s->fail(SOAP_ERR_INVALID_ARG, "lambda0 and dlambda must be positive and finite");
+    if (!(resolution > 0.0) || !std::isfinite(resolution)) return s->fail(SOAP_ERR_INVALID_ARG, "resolution must be positive and finite");
+    if (n_rows == 0) return SOAP_OK;
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    LsfArgs a{};
+    a.in = in;
+    a.out = out;
+    a.n_rows = n_rows;
+    a.n_pix = n_pix;
+    a.in_pitch = in_pitch;
+    a.out_pitch = out_pitch;
+    a.lambda0 = lambda0;
+    a.k = dlambda;
+    a.R = resolution;
+    a.fwhm_to_sigma = 1.0 / (2.0 * std::sqrt(2.0 * std::log(2.0)));
+    const double lam_last = lambda0 + dlambda * (double)(n_pix - 1);
+    const double j_last = std::ceil(kLsfNsig * (lam_last / resolution * a.fwhm_to_sigma) / dlambda);
+    if (j_last > (double)kLsfMaxJ)
+        return s->fail(SOAP_ERR_UNSUPPORTED, "line-spread function of %.0f pixels half-width exceeds %d", j_last, kLsfMaxJ);
+    a.J_max = (int)j_last;
+    const size_t elem = dtype == SOAP_F64 ? 8 : 4;
+    const size_t smem = lsf_smem_bytes(a.J_max, elem);
+    const unsigned tiles = (unsigned)((n_pix + kLsfThreads - 1) / kLsfThreads);
+    // tiles x row groups, at least ~4 waves of CTAs so that the last wave is short; a CTA keeps its weights for all
+    // the rows of its group
+    unsigned gy = (unsigned)std::max<long long>(1, std::min<long long>(n_rows, ((long long)s->n_sm * 8 * 4 + tiles - 1) / tiles));
+    // fp32 with 16-byte aligned rows: the register-window kernel, persistent CTAs over (tile, row) items
+    const bool aligned = !(in_pitch & 3) && !(out_pitch & 3) && !(reinterpret_cast<uintptr_t>(in) & 15) &&
+                         !(reinterpret_cast<uintptr_t>(out) & 15);
+    if (dtype == SOAP_F32 && aligned && a.J_max <= 24) {
+        auto launch = [&](auto kern, size_t vsmem) -> int {
+            SOAP_CUDA(s, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vsmem));
+            int occ = 0;
+            SOAP_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kLsfThreads, vsmem));
+            if (occ < 1) return s->fail(SOAP_ERR_UNSUPPORTED, "resolution-lowering kernel does not fit on an SM");
+            const long long items = ((n_pix + kLsfTileV - 1) / kLsfTileV) * n_rows;
+            const unsigned g = (unsigned)std::max<long long>(1, std::min<long long>(items, (long long)s->n_sm * occ));
+            kern<<<g, kLsfThreads, vsmem, st>>>(a);
+            return SOAP_OK;
+        };
+        int rc;
+        if (a.J_max <= 4) rc = launch(lower_resolution_v_kernel<4>, lsf_v_smem_bytes<4>());
+        else if (a.J_max <= 8) rc = launch(lower_resolution_v_kernel<8>, lsf_v_smem_bytes<8>());
+        else if (a.J_max <= 12) rc = launch(lower_resolution_v_kernel<12>, lsf_v_smem_bytes<12>());
+        else if (a.J_max <= 16) rc = launch(lower_resolution_v_kernel<16>, lsf_v_smem_bytes<16>());
+        else if (a.J_max <= 20) rc = launch(lower_resolution_v_kernel<20>, lsf_v_smem_bytes<20>());
+        else rc = launch(lower_resolution_v_kernel<24>, lsf_v_smem_bytes<24>());
+        if (rc) return rc;
+        SOAP_LAUNCH_CHECK(s, "lower_resolution_v_kernel");
+        return SOAP_OK;
+    }
+    if (dtype == SOAP_F32) {
+        SOAP_CUDA(s, cudaFuncSetAttribute(lower_resolution_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        lower_resolution_kernel<float><<<dim3(tiles, gy), kLsfThreads, smem, st>>>(a);
+    } else {
+        SOAP_CUDA(s, cudaFuncSetAttribute(lower_resolution_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        lower_resolution_kernel<double><<<dim3(tiles, gy), kLsfThreads, smem, st>>>(a);
+    }
+    SOAP_LAUNCH_CHECK(s, "lower_resolution_kernel");
+    return SOAP_OK;
 }
 
 int soap_get_stats(soap_star *s, soap_stats *stats, void *stream) {
