@@ -381,6 +381,75 @@ def run_graft(args):
         dist.destroy_process_group()
 
 
+def run_configs(args):
+    """--workload C2|C4|C5|all: device-resident timing of the other BASELINE.json configs (parity-test cases, not the
+    headline): one JSON line per config with the step time and the two kernels' durations and ALU fractions."""
+    import torch
+
+    import paper_2301_04259_b200 as soap
+    import workloads
+
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    peaks = load_peaks()
+    peak_tflops = N_SM * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    flush_buf = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    which = ["C2", "C3", "C4", "C5"] if args.workload == "all" else [args.workload]
+    for name in which:
+        if name == "C5":
+            shared = workloads.make_config5_star(0)
+            wls = [shared] + [workloads.make_config5_star(k, shared=shared) for k in range(1, 64)]
+        else:
+            wls = [{"C2": workloads.make_config2, "C3": workloads.make_config3, "C4": workloads.make_config4}[name]()]
+        w0 = wls[0]
+        P, n_ph = w0.n_pix, len(w0.phases)
+        q = soap.to_device_spectra(w0.quiet, w0.lambda0, w0.dlambda, dev)
+        sp = soap.to_device_spectra(w0.spot, w0.lambda0, w0.dlambda, dev, w0.spot_contrast, w0.spot_lb)
+        fa = None if w0.facula is None else soap.to_device_spectra(w0.facula, w0.lambda0, w0.dlambda, dev, w0.facula_contrast, w0.facula_lb)
+        stars = [soap.soap_create(dev.index) for _ in wls]
+        Q = torch.empty((len(wls), P), dtype=torch.float32, device=dev)
+        D = torch.empty((len(wls), n_ph, P), dtype=torch.float32, device=dev)
+
+        def step():
+            for k, (st, wl) in enumerate(zip(stars, wls)):
+                soap.soap_disk_geometry(st, wl, want_info=False)
+                soap.soap_integrate_quiet(st, q, Q[k])
+                soap.soap_active_timeseries(st, q, sp, fa, wl.regions, wl.phases, D[k])
+
+        for _ in range(3):
+            step()
+        torch.cuda.synchronize()
+        steps = max(3, min(args.steps, 10))
+        ms = 0.0
+        for _ in range(steps):
+            flush_buf.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            step()
+            b.record()
+            b.synchronize()
+            ms += a.elapsed_time(b)
+        ms /= steps
+        # kernel durations of the first star
+        soap.soap_set_option(stars[0], soap.binding.SOAP_OPT_KERNEL_TIMING, 1)
+        soap.soap_disk_geometry(stars[0], wls[0], want_info=False)
+        soap.soap_integrate_quiet(stars[0], q, Q[0])
+        soap.soap_active_timeseries(stars[0], q, sp, fa, wls[0].regions, wls[0].phases, D[0])
+        st = soap.soap_get_stats(stars[0])
+        n_spec = len(wls) * (1 + n_ph)
+        line = {"workload": workloads.CONFIG_NAMES[int(name[1])], "stars": len(wls), "ms_per_step": ms,
+                "spectra_per_s": n_spec / (ms * 1e-3), "first_star": {
+                    "quiet_entries": st["quiet_entries"], "active_entries": st["active_entries"],
+                    "quiet_kernel_ms": st["quiet_kernel_ms"], "active_kernel_ms": st["active_kernel_ms"],
+                    "quiet_alu_frac": st["quiet_entries"] * P * FLOPS_PER_UNIT / (st["quiet_kernel_ms"] * 1e-3) / 1e12 / peak_tflops,
+                    "active_alu_frac": (st["active_entries"] * P * FLOPS_PER_UNIT / (st["active_kernel_ms"] * 1e-3) / 1e12 / peak_tflops)
+                    if st["active_kernel_ms"] > 0 else None}}
+        print(json.dumps(line))
+        for s_ in stars:
+            soap.soap_destroy(s_)
+        del Q, D, q, sp, fa
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -388,8 +457,12 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["graft", "reference"], default="graft")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", choices=["C3", "C2", "C4", "C5", "all"], default="C3",
+                    help="C3 (default) is the bench contract; the others print per-config timing lines only")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.impl != "reference" and args.workload != "C3":
+        run_configs(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_graft(args)

@@ -234,6 +234,7 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     long long G = s->opt_quiet_splits > 0 ? (long long)s->opt_quiet_splits : (long long)s->n_sm * occ;
     const long long max_entries = (long long)s->prm.grid_n * (s->form_used == SOAP_FORM_CELLS ? s->prm.grid_n : s->prm.n_mu);
     G = std::max(1LL, std::min(G, (long long)n_tiles * max_entries / 64));
+    if (s->opt_quiet_splits <= 0) G = std::min(G, (long long)n_tiles * 8);  // few tiles: at most 8 CTAs share one (cheap hand-over)
     p.max_seg = (int)(n_tiles / G) + 3;
     SOAP_CUDA(s, s->d_partial.reserve((size_t)G * p.max_seg * f32::kTile));
     p.partial = s->d_partial.ptr;
