@@ -25,7 +25,8 @@ _lib = None
 class _Star(ctypes.Structure):
     _fields_ = [("grid_n", ctypes.c_int32), ("vsini_kms", ctypes.c_double), ("incl_deg", ctypes.c_double),
                 ("ld_u1", ctypes.c_double), ("ld_u2", ctypes.c_double), ("n_mu", ctypes.c_int32),
-                ("mu_centres", ctypes.POINTER(ctypes.c_double)), ("doppler_mode", ctypes.c_int32)]
+                ("mu_centres", ctypes.POINTER(ctypes.c_double)), ("doppler_mode", ctypes.c_int32),
+                ("diff_rot", ctypes.c_double)]
 
 
 class _Region(ctypes.Structure):
@@ -89,7 +90,7 @@ def _star(s):
     mu = np.ascontiguousarray(np.asarray(s.mu_centres, dtype=np.float64))
     st = _Star(int(s.grid_n), float(s.vsini_kms), float(s.incl_deg), float(s.ld_u1), float(s.ld_u2),
                int(mu.shape[0]), mu.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
-               int(getattr(s, "doppler_mode", 0)))
+               int(getattr(s, "doppler_mode", 0)), float(getattr(s, "diff_rot", 0.0)))
     return st, mu  # keep mu alive
 
 

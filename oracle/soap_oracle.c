@@ -49,6 +49,7 @@ typedef struct {
     int32_t n_mu;
     const double *mu_centres; /* ascending */
     int32_t doppler_mode;     /* 0: relativistic (Eq. 6), 1: first order lambda (1 - v/c) */
+    double diff_rot;          /* omega_1 / omega_0 of omega = omega_0 + omega_1 sin^2(theta); 0 = solid body */
 } oracle_star;
 
 typedef struct {
@@ -104,6 +105,7 @@ int64_t soap_oracle_geometry(const oracle_star *st, double *x, double *y, double
                              double *w, double *dfac, int32_t *bin, uint8_t *visible, double *sum_w) {
     const int32_t N = st->grid_n;
     const double sini = sin(st->incl_deg * ORACLE_PI / 180.0);
+    const double cosi = cos(st->incl_deg * ORACLE_PI / 180.0);
     int64_t nvis = 0;
     double sw = 0.0;
     for (int32_t j = 0; j < N; ++j) {
@@ -119,6 +121,13 @@ int64_t soap_oracle_geometry(const oracle_star *st, double *x, double *y, double
                 double a = 1.0 - r2;
                 m = sqrt(a > 0.0 ? a : 0.0);
                 v = xc * st->vsini_kms * sini;
+                if (st->diff_rot != 0.0) {
+                    /* differential rotation (reading R-DR): the surface point (x, y, mu) of the
+                     * observer frame has sin(latitude) = y sin i + mu cos i (inverse of the tilt of reading S13) and
+                     * rotates at omega_0 (1 + diff_rot sin^2 latitude); its line-of-sight velocity is x omega R sin i */
+                    const double sinth = yc * sini + m * cosi;
+                    v = v * (1.0 + st->diff_rot * sinth * sinth);
+                }
                 ww = 1.0 - st->ld_u1 * (1.0 - m) - st->ld_u2 * (1.0 - m) * (1.0 - m);
                 b = nearest_bin(m, st->n_mu, st->mu_centres);
                 D = doppler_factor(v, st->doppler_mode);

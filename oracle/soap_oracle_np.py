@@ -22,11 +22,13 @@ def doppler_factor(v_kms: float, mode: int) -> float:
     return math.sqrt((1.0 - beta) / (1.0 + beta))  # Eq. 6, inverted (gather)
 
 
-def geometry(grid_n, vsini_kms, incl_deg, u1, u2, mu_centres, doppler_mode=0):
-    """List of visible cells as dicts, in (j, i) order (readings S1-S5, S9)."""
+def geometry(grid_n, vsini_kms, incl_deg, u1, u2, mu_centres, doppler_mode=0, diff_rot=0.0):
+    """List of visible cells as dicts, in (j, i) order (readings S1-S5, S9).  diff_rot = omega_1 / omega_0 of
+    omega = omega_0 + omega_1 sin^2(latitude) (reading R-DR)."""
     N = grid_n
     mu_centres = np.asarray(mu_centres, dtype=np.float64)
     sini = math.sin(math.radians(incl_deg))
+    cosi = math.cos(math.radians(incl_deg))
     cells = []
     for j in range(N):
         for i in range(N):
@@ -37,6 +39,8 @@ def geometry(grid_n, vsini_kms, incl_deg, u1, u2, mu_centres, doppler_mode=0):
                 continue
             mu = math.sqrt(max(0.0, 1.0 - r2))
             v = x * vsini_kms * sini
+            if diff_rot != 0.0:
+                v *= 1.0 + diff_rot * (y * sini + mu * cosi) ** 2  # sin(latitude) of the surface point (x, y, mu)
             w = 1.0 - u1 * (1.0 - mu) - u2 * (1.0 - mu) ** 2
             d = np.abs(mu - mu_centres)
             b = int(np.flatnonzero(d == d.min())[-1])  # tie -> larger mu

@@ -56,6 +56,8 @@ class Workload:
     spot_contrast: Optional[np.ndarray] = None
     facula_contrast: Optional[np.ndarray] = None
     # limb-brightening polynomial LB(mu) = c0 + c1 mu + c2 mu^2
+    # differential rotation omega_1 / omega_0 (-0.18 for the Sun); 0 = solid body
+    diff_rot: float = 0.0
     spot_lb: Tuple[float, float, float] = (1.0, 0.0, 0.0)
     facula_lb: Tuple[float, float, float] = (1.0, 0.0, 0.0)
     # active regions, list order matters: (lat_deg, lon_deg, radius, type)
