@@ -86,6 +86,9 @@ typedef struct {
     const double *mu_centres; /* HOST [n_mu], strictly ascending (S9: nearest centre, tie -> larger mu) */
     int32_t doppler_mode;     /* 0: relativistic, Eq. 6 (source wavelength lambda * sqrt((1-b)/(1+b)));
                                  1: first order, lambda * (1 - v/c)  (S6) */
+    double diff_rot;          /* differential rotation omega_1 / omega_0 of omega = omega_0 + omega_1 sin^2(latitude)
+                                 (-0.18 for the Sun); v_cell is multiplied by 1 + diff_rot sin^2(latitude).
+                                 0 = solid body.  Non-zero selects the per-cell form (R-DR); must be > -1. */
 } soap_star_params;
 
 #define SOAP_MAX_MU 64

@@ -43,7 +43,8 @@ class SoapError(RuntimeError):
 class c_star_params(ctypes.Structure):
     _fields_ = [("grid_n", ctypes.c_int32), ("vsini_kms", ctypes.c_double), ("incl_deg", ctypes.c_double),
                 ("ld_u1", ctypes.c_double), ("ld_u2", ctypes.c_double), ("n_mu", ctypes.c_int32),
-                ("mu_centres", ctypes.POINTER(ctypes.c_double)), ("doppler_mode", ctypes.c_int32)]
+                ("mu_centres", ctypes.POINTER(ctypes.c_double)), ("doppler_mode", ctypes.c_int32),
+                ("diff_rot", ctypes.c_double)]
 
 
 class c_spectra(ctypes.Structure):
@@ -216,7 +217,7 @@ def _params(p):
     mu = np.ascontiguousarray(np.asarray(p.mu_centres, dtype=np.float64))
     c = c_star_params(int(p.grid_n), float(p.vsini_kms), float(p.incl_deg), float(p.ld_u1), float(p.ld_u2),
                       int(mu.shape[0]), mu.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
-                      int(getattr(p, "doppler_mode", 0)))
+                      int(getattr(p, "doppler_mode", 0)), float(getattr(p, "diff_rot", 0.0)))
     return c, mu
 
 

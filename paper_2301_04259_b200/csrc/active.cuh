@@ -47,6 +47,7 @@ struct ActiveCounters {  // device-resident
     unsigned int done;                  // CTAs finished (reset by the last one)
     unsigned int pad;
     int item_next, item_ctas_done;      // hand-out of (phase, tile) items in the active launch (self-resetting)
+    int overflow;                       // per-cell form: a phase's entry pool was too small (cannot happen with the host's bound)
 };
 
 struct PrepArgs {
@@ -61,6 +62,10 @@ struct PrepArgs {
     ActiveJob *jobs;          // [n_phases][job_cap]
     int *n_jobs, *work, *phase_order;  // [n_phases] each
     ActiveCounters *counters;
+    // per-cell form (differential rotation / SOAP_FORM_CELLS): every covered cell is an entry with its own shift
+    const double *vel;        // [N*N] cell velocities
+    int mode;                 // doppler_mode
+    int pool_cap;             // entries a phase's pool can hold (even); ent = [n_phases][pool_cap]
 };
 
 __host__ __device__ inline size_t prep_smem_bytes(int n_mu, int chunk_cols) {
@@ -290,6 +295,282 @@ __global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThre
     __syncthreads();
     if (!s_misc[3]) return;
     // ---- last phase to finish: order the phases by work, heaviest first (ties by phase index: deterministic)
+    __threadfence();
+    const volatile int *work = a.work;
+    for (int ph = tid; ph < a.n_phases; ph += kPrepThreads) {
+        int rk = ph;
+        if (a.n_phases <= kScheduleSortMax) {
+            const int w = work[ph];
+            rk = 0;
+            for (int q = 0; q < a.n_phases; ++q) {
+                const int wq = work[q];
+                rk += (wq > w || (wq == w && q < ph)) ? 1 : 0;
+            }
+        }
+        a.phase_order[rk] = ph;
+    }
+    if (warp == 0) {
+        unsigned long long total = 0;
+        for (int ph = lane; ph < a.n_phases; ph += 32) total += (unsigned long long)work[ph];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) total += __shfl_xor_sync(0xffffffffu, total, d);
+        if (lane == 0) {
+            a.counters->active_entries = total;
+            a.counters->done = 0;  // ready for the next call on this handle
+        }
+    }
+}
+
+// Walks column j of one phase: calls f(c, b, t, mu, w) for every lane of every 32-row chunk the regions can reach
+// (warp-uniform number of calls; t = 0 for cells no region covers, b = -1 for hidden cells).
+template <typename F>
+__device__ __forceinline__ void walk_column(const PrepArgs &a, const RegionAtPhase *reg, int j, int lane, F &&f) {
+    const int N = a.N;
+    const double x = cell_coord(j, N);
+    double ylo = 2.0, yhi = -2.0;
+    for (int r = 0; r < a.n_regions; ++r) {
+        if (reg[r].type == 0) continue;
+        const double ch = reg[r].chord * (1.0 + 1e-9) + 1e-12;
+        if (fabs(x - reg[r].xr) > ch) continue;
+        ylo = fmin(ylo, reg[r].yr - ch);
+        yhi = fmax(yhi, reg[r].yr + ch);
+    }
+    if (ylo > yhi) return;
+    int i_lo = (int)floor((ylo + 1.0) * 0.5 * N - 0.5) - 1;
+    int i_hi = (int)ceil((yhi + 1.0) * 0.5 * N - 0.5) + 1;
+    i_lo = max(i_lo, 0);
+    i_hi = min(i_hi, N - 1);
+    for (int i0 = i_lo; i0 <= i_hi; i0 += 32) {
+        const int i = i0 + lane;
+        const bool in = i <= i_hi;
+        const size_t c = (size_t)j * N + (in ? i : i_hi);
+        const int b = in ? a.bin[c] : -1;
+        const double m = a.mu[c], wc = a.w[c];
+        int t = 0;
+        if (b >= 0) {
+            const double y = cell_coord(i, N);
+            for (int r = 0; r < a.n_regions; ++r) {  // list order: the last covering region wins
+                if (reg[r].type == 0) continue;
+                const double dot =
+                    __dadd_rn(__dadd_rn(__dmul_rn(x, reg[r].xr), __dmul_rn(y, reg[r].yr)), __dmul_rn(m, reg[r].zr));
+                if (dot >= reg[r].cos_alpha) t = reg[r].type;
+            }
+        }
+        f(c, b, t, m, wc);
+    }
+}
+
+// a4, per-cell form: the same cluster-per-phase structure as active_prepare_kernel, but every covered cell
+// becomes its own pair of entries (a_c, -w) in the quiet segment of its mu-bin and (a_c, +w LB_t(mu)) in its
+// kind's segment, because under differential rotation the cells of a column no longer share a
+// velocity.  Two passes over the columns (count, then write) with the per-(segment, column) counts in shared
+// memory; a phase's segments are packed back to back, in job order, in the phase's pool ent[p][pool_cap].
+// Within a segment the entries are in (column, row) order: neighbouring entries have nearly equal shifts.
+// dynamic shared memory = prep_cells_smem_bytes(n_mu, chunk_cols).
+__host__ __device__ inline size_t prep_cells_smem_bytes(int n_mu, int chunk_cols) {
+    return (size_t)3 * n_mu * chunk_cols * sizeof(int) + (size_t)4 * 3 * n_mu * sizeof(int) + 64;
+}
+
+template <typename EntT>
+__global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThreads)
+active_prepare_cells_kernel(const PrepArgs a) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    extern __shared__ __align__(16) unsigned char prep_smem[];
+    const int n_seg = 3 * a.n_mu, N = a.N, cc = a.chunk_cols;
+    int *cntc = reinterpret_cast<int *>(prep_smem);  // [n_seg][cc]: entries per (segment, column); then running offsets
+    int *cnt = cntc + (size_t)n_seg * cc;            // [n_seg] entries of this CTA (read by the others)
+    int *off = cnt + n_seg;                          // [n_seg] pool position of this CTA's block of the segment
+    int *tot = off + n_seg;                          // [n_seg] entries of the whole phase
+    int *base = tot + n_seg;                         // [n_seg] pool position of the segment
+    int *s_misc = base + n_seg;                      // j_lo, j_hi, covered cells of this CTA, last-phase flag
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = kPrepThreads / 32;
+    const int p = blockIdx.x / kPrepCluster;
+    const int rank = (int)cluster.block_rank();
+    const RegionAtPhase *reg = a.rp + (size_t)p * a.n_regions;
+    EntT *pool = static_cast<EntT *>(a.ent) + (size_t)p * a.pool_cap;
+
+    if (tid == 0) {
+        s_misc[0] = N;
+        s_misc[1] = -1;
+        s_misc[2] = 0;
+        s_misc[3] = 0;
+    }
+    __syncthreads();
+    for (int r = tid; r < a.n_regions; r += kPrepThreads) {
+        if (reg[r].type == 0) continue;
+        const double ch = reg[r].chord * (1.0 + 1e-9) + 1e-12;
+        int jl = (int)floor((reg[r].xr - ch + 1.0) * 0.5 * N - 0.5) - 1;
+        int jh = (int)ceil((reg[r].xr + ch + 1.0) * 0.5 * N - 0.5) + 1;
+        atomicMin(&s_misc[0], max(jl, 0));
+        atomicMax(&s_misc[1], min(jh, N - 1));
+    }
+    __syncthreads();
+    const int j_lo = s_misc[0], j_hi = s_misc[1];
+    const int per = (j_hi >= j_lo) ? (j_hi - j_lo + kPrepCluster) / kPrepCluster : 0;
+    const int c0 = j_lo + rank * per;
+    const int cols = max(0, min(per, j_hi + 1 - c0));
+    for (int s = warp; s < n_seg; s += n_warps)
+        for (int k = lane; k < cols; k += 32) cntc[(size_t)s * cc + k] = 0;
+    __syncthreads();
+    // ---- pass 1: count the covered cells per (segment, column) ------------------------------------------------
+    for (int j = c0 + warp; j < c0 + cols; j += n_warps) {
+        int *col = cntc + (j - c0);
+        int count = 0;
+        walk_column(a, reg, j, lane, [&](size_t, int b, int t, double, double) {
+            // the quiet segment of a mu-bin collects the covered cells of every type, the kind segments one type each
+            const unsigned same0 = __match_any_sync(0xffffffffu, t != 0 ? b : -1);
+            const unsigned same = __match_any_sync(0xffffffffu, t != 0 ? b * 4 + t : -1);
+            if (t != 0 && lane == __ffs(same0) - 1) col[(size_t)b * cc] += __popc(same0);  // one lane per distinct key
+            if (t != 0 && lane == __ffs(same) - 1) col[(size_t)(t * a.n_mu + b) * cc] += __popc(same);
+            __syncwarp();
+            count += __popc(__ballot_sync(0xffffffffu, t != 0));
+        });
+        if (lane == 0 && count) atomicAdd(&s_misc[2], count);
+    }
+    __syncthreads();
+    // ---- per segment: exclusive scan over this CTA's columns, CTA total ----------------------------------------
+    for (int s = warp; s < n_seg; s += n_warps) {
+        int *row = cntc + (size_t)s * cc;
+        int run = 0;
+        for (int k0 = 0; k0 < cols; k0 += 32) {
+            const int k = k0 + lane;
+            const int v = k < cols ? row[k] : 0;
+            int incl = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
+            }
+            if (k < cols) row[k] = run + incl - v;
+            run += __shfl_sync(0xffffffffu, incl, 31);
+        }
+        if (lane == 0) cnt[s] = run;
+    }
+    cluster.sync();
+    for (int s = tid; s < n_seg; s += kPrepThreads) {
+        int before = 0, all = 0;
+        for (int r = 0; r < kPrepCluster; ++r) {
+            const int c = cluster.map_shared_rank(cnt, r)[s];
+            before += r < rank ? c : 0;
+            all += c;
+        }
+        off[s] = before;
+        tot[s] = all;
+    }
+    int covered = 0;
+    if (rank == 0 && tid == 0)
+        for (int r = 0; r < kPrepCluster; ++r) covered += cluster.map_shared_rank(s_misc, r)[2];
+    cluster.sync();  // no CTA goes on to change cnt / s_misc while they are being read
+    // segment positions in the pool: job order (kinds 1, 2, then 0), each padded to an even length
+    if (warp == 0) {
+        const int per_lane = (n_seg + 31) / 32;
+        const int ss0 = min(n_seg, lane * per_lane), ss1 = min(n_seg, ss0 + per_lane);
+        int mine = 0;
+        for (int ss = ss0; ss < ss1; ++ss) mine += (tot[(ss + a.n_mu) % n_seg] + 1) & ~1;
+        int incl = mine;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        int pos = incl - mine;
+        for (int ss = ss0; ss < ss1; ++ss) {
+            const int s = (ss + a.n_mu) % n_seg;
+            base[s] = pos;
+            pos += (tot[s] + 1) & ~1;
+        }
+        if (lane == 31 && incl > a.pool_cap) a.counters->overflow = 1;
+    }
+    __syncthreads();
+    for (int s = tid; s < n_seg; s += kPrepThreads) off[s] += base[s];
+    __syncthreads();
+    // ---- pass 2: write the entries; cntc[s][column] is the running position inside this CTA's block ------------
+    for (int j = c0 + warp; j < c0 + cols; j += n_warps) {
+        int *col = cntc + (j - c0);
+        walk_column(a, reg, j, lane, [&](size_t c, int b, int t, double m, double wc) {
+            const unsigned same0 = __match_any_sync(0xffffffffu, t != 0 ? b : -1);
+            const unsigned same = __match_any_sync(0xffffffffu, t != 0 ? b * 4 + t : -1);
+            int p0 = 0, pt = 0;
+            if (t != 0) {  // rank among the chunk's cells of this mu-bin / of this (mu-bin, type), in row order
+                p0 = off[b] + col[(size_t)b * cc] + __popc(same0 & ((1u << lane) - 1u));
+                pt = off[t * a.n_mu + b] + col[(size_t)(t * a.n_mu + b) * cc] + __popc(same & ((1u << lane) - 1u));
+            }
+            __syncwarp();
+            if (t != 0 && lane == __ffs(same0) - 1) col[(size_t)b * cc] += __popc(same0);
+            if (t != 0 && lane == __ffs(same) - 1) col[(size_t)(t * a.n_mu + b) * cc] += __popc(same);
+            __syncwarp();
+            if (t != 0 && p0 < a.pool_cap && pt < a.pool_cap) {
+                const double ac = doppler_minus_one(a.vel[c], a.mode);
+                const double wl = wc * (a.lb.c[t][0] + a.lb.c[t][1] * m + a.lb.c[t][2] * m * m);
+                EntT e;
+                e.x = (decltype(e.x))ac;
+                e.y = (decltype(e.y))(-wc);
+                pool[p0] = e;
+                e.y = (decltype(e.y))wl;
+                pool[pt] = e;
+            }
+        });
+    }
+    if (rank != 0) return;
+    // ---- rank 0 finalises the phase: pad odd segments, job list (contrast-carrying kinds 1, 2 first) -------------
+    for (int s = tid; s < n_seg; s += kPrepThreads) {
+        const int c = tot[s];
+        if ((c & 1) && base[s] + c < a.pool_cap) {
+            EntT z;
+            z.x = 0;
+            z.y = 0;
+            pool[base[s] + c] = z;
+        }
+        if (a.seg_count) a.seg_count[p * n_seg + s] = c;
+    }
+    if (warp == 0) {
+        const int per_lane = (n_seg + 31) / 32;
+        const int ss0 = min(n_seg, lane * per_lane), ss1 = min(n_seg, ss0 + per_lane);
+        int nj = 0, wsum = 0;
+        for (int ss = ss0; ss < ss1; ++ss) {
+            const int c = tot[(ss + a.n_mu) % n_seg];
+            nj += (c + kActiveJobCap - 1) / kActiveJobCap;
+            wsum += c;
+        }
+        int incl = nj;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        int k = incl - nj;
+        for (int ss = ss0; ss < ss1; ++ss) {
+            const int s = (ss + a.n_mu) % n_seg;
+            const int c = tot[s];
+            for (int o = 0; o < c; o += kActiveJobCap) {
+                ActiveJob jb;
+                jb.begin = p * a.pool_cap + base[s] + o;  // fits: host checks n_phases * pool_cap < 2^31
+                jb.count = min(kActiveJobCap, c - o);
+                jb.kind = s / a.n_mu;
+                jb.row = s - jb.kind * a.n_mu;
+                if (k < a.job_cap) a.jobs[(size_t)p * a.job_cap + k] = jb;
+                ++k;
+            }
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) wsum += __shfl_xor_sync(0xffffffffu, wsum, d);
+        const int n_jobs_total = __shfl_sync(0xffffffffu, incl, 31);
+        if (lane == 0) {
+            a.n_jobs[p] = min(n_jobs_total, a.job_cap);
+            a.work[p] = wsum;
+            a.n_active[p] = covered;
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned ticket = atomicAdd(&a.counters->done, 1u);
+        s_misc[3] = (ticket == (unsigned)a.n_phases - 1u) ? 1 : 0;
+    }
+    __syncthreads();
+    if (!s_misc[3]) return;
+    // ---- last phase to finish: order the phases by work, heaviest first (ties by phase index: deterministic) ------
     __threadfence();
     const volatile int *work = a.work;
     for (int ph = tid; ph < a.n_phases; ph += kPrepThreads) {

@@ -24,7 +24,11 @@ __device__ __forceinline__ double cell_coord(int idx, int N) {
 }
 
 // One cell c = j*N + i: mu, limb-darkening weight, velocity and nearest mu bin (hidden: 0, 0, 0, -1).
-__device__ __forceinline__ void cell_geometry(int j, int i, int N, double vsini_sini, double u1, double u2, int n_mu,
+struct Rotation {  // v_cell = x vsini sin i (1 + diff_rot sin^2 latitude)  (S5, reading R-DR)
+    double vsini, sini, cosi, diff_rot;
+};
+
+__device__ __forceinline__ void cell_geometry(int j, int i, int N, const Rotation &rot, double u1, double u2, int n_mu,
                                               const double *__restrict__ mu_centres, double &mu, double &w, double &v,
                                               int &bin) {
     const double x = cell_coord(j, N), y = cell_coord(i, N);
@@ -36,7 +40,11 @@ __device__ __forceinline__ void cell_geometry(int j, int i, int N, double vsini_
     if (r2 <= 1.0) {  // cell counts iff its centre is on the disk (reading S2)
         const double a = __dadd_rn(1.0, -r2);
         mu = __dsqrt_rn(a > 0.0 ? a : 0.0);
-        v = __dmul_rn(x, vsini_sini);
+        v = __dmul_rn(__dmul_rn(x, rot.vsini), rot.sini);
+        if (rot.diff_rot != 0.0) {  // sin(latitude) of the surface point (x, y, mu): inverse of the tilt of reading S13
+            const double sinth = __dadd_rn(__dmul_rn(y, rot.sini), __dmul_rn(mu, rot.cosi));
+            v = __dmul_rn(v, __dadd_rn(1.0, __dmul_rn(__dmul_rn(rot.diff_rot, sinth), sinth)));
+        }
         const double om = __dadd_rn(1.0, -mu);
         // w = 1 - u1 (1-mu) - u2 (1-mu)^2, evaluated left to right
         w = __dadd_rn(__dadd_rn(1.0, -__dmul_rn(u1, om)), -__dmul_rn(__dmul_rn(u2, om), om));
@@ -89,7 +97,7 @@ struct MuCentres {  // passed by value as a kernel argument: no host -> device c
 // One warp, one column j, the 32-row chunks `chunk`, `chunk + stride`, ...: writes the cells' (mu, w, v, bin)
 // and adds the chunk's binned weights to s_W[64] (segmented warp scans, added in row order), returning
 // the warp's weight sum and visible-cell count.
-__device__ __forceinline__ void geometry_chunks(int j, int chunk, int stride, int N, double vsini_sini, double u1, double u2,
+__device__ __forceinline__ void geometry_chunks(int j, int chunk, int stride, int N, const Rotation &rot, double u1, double u2,
                                                 int n_mu, const double *s_mu, double *s_W, double *__restrict__ mu_out,
                                                 double *__restrict__ w_out, double *__restrict__ vel_out,
                                                 int *__restrict__ bin_out, double &sum, int &nvis) {
@@ -101,7 +109,7 @@ __device__ __forceinline__ void geometry_chunks(int j, int chunk, int stride, in
         double mu = 0.0, w = 0.0, v = 0.0;
         int bin = -1;
         if (i < N) {
-            cell_geometry(j, i, N, vsini_sini, u1, u2, n_mu, s_mu, mu, w, v, bin);
+            cell_geometry(j, i, N, rot, u1, u2, n_mu, s_mu, mu, w, v, bin);
             const size_t c = (size_t)j * N + i;
             mu_out[c] = mu;
             w_out[c] = w;
@@ -234,7 +242,7 @@ __host__ __device__ inline int geom_warps_per_col(int N) {
 __host__ __device__ inline int geom_cols_per_cta(int N) { return kGeomWarps / geom_warps_per_col(N); }
 
 __global__ void __launch_bounds__(32 * kGeomWarps)
-geometry_kernel(int N, double vsini_sini, double u1, double u2, int mode, int n_mu, const MuCentres mu_centres,
+geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n_mu, const MuCentres mu_centres,
                 double *__restrict__ mu_out, double *__restrict__ w_out, double *__restrict__ vel_out,
                 int *__restrict__ bin_out, double *__restrict__ col_a, double *__restrict__ Wbin /*[N][n_mu]*/,
                 double *__restrict__ col_sumw, int *__restrict__ col_nvis, float2 *__restrict__ ent32,
@@ -255,7 +263,7 @@ geometry_kernel(int N, double vsini_sini, double u1, double u2, int mode, int n_
     double sum = 0.0;
     int nvis = 0;
     if (cl < cpc && j < N)
-        geometry_chunks(j, chunk, wpc, N, vsini_sini, u1, u2, n_mu, s_mu, s_W[warp], mu_out, w_out, vel_out, bin_out, sum, nvis);
+        geometry_chunks(j, chunk, wpc, N, rot, u1, u2, n_mu, s_mu, s_W[warp], mu_out, w_out, vel_out, bin_out, sum, nvis);
     if (lane == 0) {
         s_sum[warp] = sum;
         s_nvis[warp] = nvis;
@@ -276,7 +284,8 @@ geometry_kernel(int N, double vsini_sini, double u1, double u2, int mode, int n_
                     sw += s_sum[warp * wpc + k];
                     nv += s_nvis[warp * wpc + k];
                 }
-                col_a[jj] = doppler_minus_one(__dmul_rn(cell_coord(jj, N), vsini_sini), mode);
+                // the column's shift factor (solid body; with differential rotation the per-cell form is used instead)
+                col_a[jj] = doppler_minus_one(__dmul_rn(__dmul_rn(cell_coord(jj, N), rot.vsini), rot.sini), mode);
                 col_sumw[jj] = sw;
                 col_nvis[jj] = nv;
             }
@@ -292,21 +301,30 @@ geometry_kernel(int N, double vsini_sini, double u1, double u2, int mode, int n_
     build_binned_entries(N, n_mu, col_a, Wbin, col_sumw, col_nvis, ent32, ent64, row_start, info);
 }
 
-// SOAP_FORM_CELLS: one entry per visible cell (the literal double loop of Alg. 1), same layout.
-// Two passes over the cells by one CTA; within a row the entries keep (j, i) order.
-__global__ void build_cell_entries_kernel(int N, int n_mu, const double *__restrict__ col_a,
+// Per-cell form (SOAP_FORM_CELLS, and always under differential rotation, where the cells of a column no longer
+// share a velocity): one entry per visible cell - the literal double loop of Alg. 1 - in the same layout, with the
+// cell's own shift factor D_c - 1 from its velocity.  Two passes over the cells by one CTA (loads in batches of
+// 8 x 32 cells); within a row the entries keep (j, i) order, so neighbouring entries have nearly equal shifts.
+__global__ void build_cell_entries_kernel(int N, int n_mu, int mode, const double *__restrict__ vel,
                                           const double *__restrict__ w, const int *__restrict__ bin,
                                           float2 *__restrict__ ent32, double2 *__restrict__ ent64,
                                           int *__restrict__ row_start) {
     __shared__ int s_cnt[64];
     __shared__ int s_start[65];
+    constexpr int kBatch = 8;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
     const int ncell = N * N;
     for (int b = warp; b < n_mu; b += n_warps) {
         int cnt = 0;
-        for (int c0 = 0; c0 < ncell; c0 += 32) {
-            const int c = c0 + lane;
-            cnt += __popc(__ballot_sync(0xffffffffu, (c < ncell) && bin[c] == b));
+        for (int c0 = 0; c0 < ncell; c0 += 32 * kBatch) {
+            int bb[kBatch];
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) {
+                const int c = c0 + 32 * k + lane;
+                bb[k] = c < ncell ? bin[c] : -1;
+            }
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) cnt += __popc(__ballot_sync(0xffffffffu, bb[k] == b));
         }
         if (lane == 0) s_cnt[b] = cnt;
     }
@@ -323,17 +341,26 @@ __global__ void build_cell_entries_kernel(int N, int n_mu, const double *__restr
     for (int b = threadIdx.x; b <= n_mu; b += blockDim.x) row_start[b] = s_start[b];
     for (int b = warp; b < n_mu; b += n_warps) {
         int pos = s_start[b];
-        for (int c0 = 0; c0 < ncell; c0 += 32) {
-            const int c = c0 + lane;
-            const bool in = (c < ncell) && bin[c] == b;
-            const unsigned m = __ballot_sync(0xffffffffu, in);
-            if (in) {
-                const int k = pos + __popc(m & ((1u << lane) - 1u));
-                const double a = col_a[c / N];
-                ent32[k] = make_float2((float)a, (float)w[c]);
-                ent64[k] = make_double2(a, w[c]);
+        for (int c0 = 0; c0 < ncell; c0 += 32 * kBatch) {
+            int bb[kBatch];
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) {
+                const int c = c0 + 32 * k + lane;
+                bb[k] = c < ncell ? bin[c] : -1;
             }
-            pos += __popc(m);
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) {
+                const int c = c0 + 32 * k + lane;
+                const bool in = bb[k] == b;
+                const unsigned m = __ballot_sync(0xffffffffu, in);
+                if (in) {
+                    const int e = pos + __popc(m & ((1u << lane) - 1u));
+                    const double a = doppler_minus_one(vel[c], mode);
+                    ent32[e] = make_float2((float)a, (float)w[c]);
+                    ent64[e] = make_double2(a, w[c]);
+                }
+                pos += __popc(m);
+            }
         }
         if (lane == 0 && (s_cnt[b] & 1)) {
             ent32[pos] = make_float2(0.f, 0.f);

@@ -60,6 +60,8 @@ struct soap_star {
     double sini = 1.0, cosi = 0.0;
     double amax = 0.0;  // host bound on max |D - 1|
     int form = SOAP_FORM_AUTO, form_used = SOAP_FORM_BINNED;
+    long long active_pool_cap = 0;  // per-cell active form: entries one phase's pool must hold (from the region radii)
+    bool cell_entries = false;  // one entry per cell (SOAP_FORM_CELLS, or differential rotation) instead of per (column, mu-bin)
     int opt_quiet_splits = 0;
     bool opt_timing = false;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};  // quiet start/stop, active start/stop
@@ -232,7 +234,7 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     SOAP_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f32::sia_f32_kernel<false>, f32::kThreads, smem));
     if (occ < 1) return s->fail(SOAP_ERR_UNSUPPORTED, "quiet kernel does not fit on an SM (halo %d)", p.halo);
     long long G = s->opt_quiet_splits > 0 ? (long long)s->opt_quiet_splits : (long long)s->n_sm * occ;
-    const long long max_entries = (long long)s->prm.grid_n * (s->form_used == SOAP_FORM_CELLS ? s->prm.grid_n : s->prm.n_mu);
+    const long long max_entries = (long long)s->prm.grid_n * (s->cell_entries ? s->prm.grid_n : s->prm.n_mu);
     G = std::max(1LL, std::min(G, (long long)n_tiles * max_entries / 64));
     if (s->opt_quiet_splits <= 0) G = std::min(G, (long long)n_tiles * 8);  // few tiles: at most 8 CTAs share one (cheap hand-over)
     p.max_seg = (int)(n_tiles / G) + 3;
@@ -261,7 +263,7 @@ int quiet_impl(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) 
     if (splits <= 0) {
         // ~8 CTAs of 128 threads per SM; the entry list is cut into `splits` chunks per wavelength tile
         splits = (int)std::lround((double)(s->n_sm * 8) / n_tiles);
-        const long long max_entries = (long long)s->prm.grid_n * (s->form_used == SOAP_FORM_CELLS ? s->prm.grid_n : s->prm.n_mu);
+        const long long max_entries = (long long)s->prm.grid_n * (s->cell_entries ? s->prm.grid_n : s->prm.n_mu);
         const int cap = (int)std::max(1LL, max_entries / 16);
         splits = std::max(1, std::min(std::min(splits, 256), cap));
     }
@@ -292,6 +294,11 @@ int quiet_impl(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) 
     return SOAP_OK;
 }
 
+inline int per_cell_cap(const soap_star *s, int n_mu, int ncap) {  // jobs one phase's list can hold
+    if (s->prm.diff_rot != 0.0) return 3 * n_mu + (int)(s->active_pool_cap / kActiveJobCap) + 2;
+    return 3 * n_mu * ((ncap + kActiveJobCap - 1) / kActiveJobCap);
+}
+
 template <typename T>
 int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, const soap_spectra *fac,
                 int n_regions, int n_phases, int effect, bool prepare, void *out, long long out_pitch, cudaStream_t st) {
@@ -313,11 +320,53 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         SOAP_CUDA(s, s->d_counters.reserve(1));
         SOAP_CUDA(s, cudaMemsetAsync(s->d_counters.ptr, 0, sizeof(ActiveCounters), st));  // once per handle
     }
-    const int job_cap = 3 * n_mu * ((ncap + kActiveJobCap - 1) / kActiveJobCap);
+    const int job_cap = per_cell_cap(s, n_mu, ncap);
     SOAP_CUDA(s, s->d_jobs.reserve((size_t)n_phases * job_cap));
     SOAP_CUDA(s, s->d_sched.reserve((size_t)3 * n_phases));
     int *d_njobs = s->d_sched.ptr, *d_order = d_njobs + n_phases, *d_work = d_order + n_phases;
-    if (prepare) {
+    const bool per_cell = s->prm.diff_rot != 0.0;  // the cells of a column no longer share a velocity (R-DR)
+    if (per_cell && sizeof(T) != 4)
+        return s->fail(SOAP_ERR_UNSUPPORTED, "differential rotation: the active time series is implemented for fp32 spectra only");
+    if (per_cell && prepare) {
+        const long long pool = s->active_pool_cap;
+        if ((long long)n_phases * pool >= (1LL << 31)) return s->fail(SOAP_ERR_UNSUPPORTED, "n_phases * entries per phase too large for one call");
+        SOAP_CUDA(s, s->d_aent.reserve((size_t)n_phases * pool * sizeof(Ent) + 64));
+        PrepArgs a{};
+        a.N = N;
+        a.n_regions = n_regions;
+        a.n_mu = n_mu;
+        a.seg_cap = 0;
+        a.n_phases = n_phases;
+        a.pool_cap = (int)pool;
+        a.job_cap = 3 * n_mu + (int)(pool / kActiveJobCap) + 2;
+        SOAP_CUDA(s, s->d_jobs.reserve((size_t)n_phases * a.job_cap));
+        a.chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);
+        if (prep_cells_smem_bytes(n_mu, a.chunk_cols) > 200 * 1024)
+            return s->fail(SOAP_ERR_UNSUPPORTED, "grid_n %d with %d mu bins exceeds the active-map kernel's shared memory", N, n_mu);
+        a.rp = s->d_rp.ptr;
+        a.mu = s->d_mu.ptr;
+        a.w = s->d_w.ptr;
+        a.col_a = s->d_col_a.ptr;
+        a.bin = s->d_bin.ptr;
+        a.vel = s->d_vel.ptr;
+        a.mode = s->prm.doppler_mode;
+        a.lb.c[1][0] = 1.0;
+        a.lb.c[2][0] = 1.0;
+        if (use_lb && spot) { a.lb.c[1][0] = spot->lb_c0; a.lb.c[1][1] = spot->lb_c1; a.lb.c[1][2] = spot->lb_c2; }
+        if (use_lb && fac) { a.lb.c[2][0] = fac->lb_c0; a.lb.c[2][1] = fac->lb_c1; a.lb.c[2][2] = fac->lb_c2; }
+        a.ent = s->d_aent.ptr;
+        a.seg_count = nullptr;
+        a.n_active = s->d_nactive.ptr;
+        a.jobs = s->d_jobs.ptr;
+        a.n_jobs = d_njobs;
+        a.work = d_work;
+        a.phase_order = d_order;
+        a.counters = s->d_counters.ptr;
+        const size_t smem = prep_cells_smem_bytes(n_mu, a.chunk_cols);
+        SOAP_CUDA(s, cudaFuncSetAttribute(active_prepare_cells_kernel<Ent>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        active_prepare_cells_kernel<Ent><<<n_phases * kPrepCluster, kPrepThreads, smem, st>>>(a);
+        SOAP_LAUNCH_CHECK(s, "active_prepare_cells_kernel");
+    } else if (prepare) {
         // a4 in one launch: one cluster of CTAs per phase bins, compacts and schedules (active.cuh)
         PrepArgs a{};
         a.N = N;
@@ -429,6 +478,18 @@ int check_regions(soap_star *s, const soap_region *regions, int n_regions, const
 // Localize (readings S11-S13): region centres in the observer frame for every phase.
 int upload_region_centres(soap_star *s, const soap_region *regions, int n_regions, const double *phases,
                           int n_phases, cudaStream_t st) {
+    {
+        // per-cell form: a region's covered cells lie in a disc of radius chord = 2 sin(alpha / 2) around its projected
+        // centre; with the cell-centre rule at most pi (chord N / 2 + 1.5)^2 of them, two entries each
+        const double pi_ = 3.14159265358979323846, half = 0.5 * (double)s->prm.grid_n;
+        double cells = 0.0;
+        for (int r = 0; r < n_regions; ++r) {
+            const double ch = 2.0 * std::sin(0.5 * std::asin(regions[r].radius)) * half + 1.5;
+            cells += pi_ * ch * ch;
+        }
+        cells = std::min(cells, (double)s->prm.grid_n * (double)s->prm.grid_n);
+        s->active_pool_cap = ((2LL * (long long)std::ceil(cells) + 2LL * 3 * s->prm.n_mu + 8) + 1) & ~1LL;
+    }
     const size_t n = (size_t)n_regions * n_phases;
     if (n == 0) return SOAP_OK;
     soap_star::PinnedSlot &slot = s->h_rp[s->h_rp_next];
@@ -565,7 +626,8 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     if (prm->doppler_mode != 0 && prm->doppler_mode != 1) return s->fail(SOAP_ERR_INVALID_ARG, "doppler_mode must be 0 or 1");
     const double pi = 3.14159265358979323846;
     const double sini = std::sin(prm->incl_deg * pi / 180.0), cosi = std::cos(prm->incl_deg * pi / 180.0);
-    if (std::fabs(prm->vsini_kms * sini) >= 0.1 * kSpeedOfLightKms) return s->fail(SOAP_ERR_INVALID_ARG, "|v| must be below 0.1 c");
+    if (std::fabs(prm->vsini_kms * sini) * std::max(1.0, 1.0 + prm->diff_rot) >= 0.1 * kSpeedOfLightKms)
+        return s->fail(SOAP_ERR_INVALID_ARG, "|v| must be below 0.1 c");
 
     SOAP_CUDA(s, cudaSetDevice(s->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -577,8 +639,13 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     s->cosi = cosi;
     const int N = prm->grid_n, n_mu = prm->n_mu;
     const size_t ncell = (size_t)N * N;
+    if (!std::isfinite(prm->diff_rot) || !(prm->diff_rot > -1.0)) return s->fail(SOAP_ERR_INVALID_ARG, "diff_rot must be finite and > -1");
+    if (prm->diff_rot != 0.0 && s->form == SOAP_FORM_BINNED)
+        return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_BINNED needs solid-body rotation: the cells of a column must share one velocity");
     s->form_used = (s->form == SOAP_FORM_CELLS || s->form == SOAP_FORM_FIR) ? s->form : SOAP_FORM_BINNED;
-    const double vmax = std::fabs(prm->vsini_kms * sini) * (double)(N - 1) / (double)N;
+    s->cell_entries = s->form == SOAP_FORM_CELLS || prm->diff_rot != 0.0;
+    if (s->cell_entries && s->form_used == SOAP_FORM_BINNED) s->form_used = SOAP_FORM_CELLS;
+    const double vmax = std::fabs(prm->vsini_kms * sini) * (double)(N - 1) / (double)N * std::max(1.0, 1.0 + prm->diff_rot);
     s->amax = std::max(std::fabs(host_dshift(vmax, prm->doppler_mode)), std::fabs(host_dshift(-vmax, prm->doppler_mode)));
 
     SOAP_CUDA(s, s->d_mu.reserve(ncell));
@@ -591,7 +658,7 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     SOAP_CUDA(s, s->d_col_nvis.reserve(N));
     SOAP_CUDA(s, s->d_row_start.reserve(n_mu + 1));
     SOAP_CUDA(s, s->d_info.reserve(1));
-    const size_t ent_cap = std::max(s->form_used == SOAP_FORM_CELLS ? ncell : (size_t)0, (size_t)N * n_mu) + 2 * (size_t)n_mu + 8;
+    const size_t ent_cap = std::max(s->cell_entries ? ncell : (size_t)0, (size_t)N * n_mu) + 2 * (size_t)n_mu + 8;
     SOAP_CUDA(s, s->d_ent32.reserve(ent_cap));
     SOAP_CUDA(s, s->d_ent64.reserve(ent_cap));
 
@@ -601,15 +668,15 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     }
     MuCentres mc{};
     for (int b = 0; b < n_mu; ++b) mc.v[b] = prm->mu_centres[b];
-    const double vs = prm->vsini_kms * sini;
+    Rotation rot{prm->vsini_kms, sini, cosi, prm->diff_rot};
     // a1 + a2 in one launch: the last CTA compacts the binned weights into the entry list
     geometry_kernel<<<(N + geom_cols_per_cta(N) - 1) / geom_cols_per_cta(N), 32 * kGeomWarps, 0, st>>>(
-        N, vs, prm->ld_u1, prm->ld_u2, prm->doppler_mode, n_mu, mc, s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr, s->d_bin.ptr,
+        N, rot, prm->ld_u1, prm->ld_u2, prm->doppler_mode, n_mu, mc, s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr, s->d_bin.ptr,
         s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr, s->d_ent32.ptr, s->d_ent64.ptr, s->d_row_start.ptr,
         s->d_info.ptr, s->d_geom_done.ptr);
     SOAP_LAUNCH_CHECK(s, "geometry_kernel");
-    if (s->form_used == SOAP_FORM_CELLS) {
-        build_cell_entries_kernel<<<1, 1024, 0, st>>>(N, n_mu, s->d_col_a.ptr, s->d_w.ptr, s->d_bin.ptr, s->d_ent32.ptr,
+    if (s->cell_entries) {
+        build_cell_entries_kernel<<<1, 1024, 0, st>>>(N, n_mu, prm->doppler_mode, s->d_vel.ptr, s->d_w.ptr, s->d_bin.ptr, s->d_ent32.ptr,
                                                       s->d_ent64.ptr, s->d_row_start.ptr);
         SOAP_LAUNCH_CHECK(s, "build_cell_entries_kernel");
     }
@@ -619,7 +686,7 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
         SOAP_CUDA(s, cudaMemcpyAsync(&di, s->d_info.ptr, sizeof(di), cudaMemcpyDeviceToHost, st));
         SOAP_CUDA(s, cudaStreamSynchronize(st));
         info->n_visible = di.n_visible;
-        info->n_entries = (s->form_used == SOAP_FORM_CELLS) ? di.n_visible : di.n_entries;
+        info->n_entries = s->cell_entries ? di.n_visible : di.n_entries;
         info->sum_weights = di.sum_weights;
         info->max_abs_dshift = di.max_abs_dshift;
     }
@@ -768,7 +835,7 @@ int soap_get_stats(soap_star *s, soap_stats *stats, void *stream) {
         DevInfo di;
         SOAP_CUDA(s, cudaMemcpyAsync(&di, s->d_info.ptr, sizeof(di), cudaMemcpyDeviceToHost, st));
         SOAP_CUDA(s, cudaStreamSynchronize(st));
-        stats->quiet_entries = (s->form_used == SOAP_FORM_CELLS) ? di.n_visible : di.n_entries;
+        stats->quiet_entries = s->cell_entries ? di.n_visible : di.n_entries;
     }
     if (s->d_counters.ptr) {
         ActiveCounters c;

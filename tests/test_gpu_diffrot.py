@@ -1,0 +1,91 @@
+"""Parity of the per-cell path under differential rotation against the oracle."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from test_gpu_parity import assert_parity, run_gpu, _sample_ranges
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def soap():
+    import paper_2301_04259_b200 as soap_mod
+    soap_mod.binding.load_library()
+    return soap_mod
+
+
+def test_diffrot_geometry_is_bit_exact(soap):
+    wl = workloads.make_config2(n_pix=2000, n_phases=2, grid_n=150)
+    wl.diff_rot, wl.incl_deg = -0.18, 60.0
+    g = run_gpu(soap, wl)
+    og = oracle.geometry(wl)
+    np.testing.assert_array_equal(g["geo"]["vel"], og["vel"])
+    np.testing.assert_array_equal(g["geo"]["bin"], og["bin"])
+    assert g["stats"]["form"] == 2 and g["info"]["n_entries"] == og["n_visible"]
+
+
+@pytest.mark.parametrize("dr,incl", [(-0.18, 90.0), (-0.18, 55.0), (0.25, 70.0)])
+def test_diffrot_quiet_and_active_parity(soap, dr, incl):
+    wl = workloads.make_config3(n_pix=6000, n_phases=6, grid_n=110, nested=True)
+    wl.diff_rot, wl.incl_deg, wl.vsini_kms = dr, incl, 6.0
+    wl.phases = np.array([0.35, 0.45, 0.5, 0.55, 0.65, 0.0])
+    g = run_gpu(soap, wl)
+    assert g["n_active"].max() > 0
+    assert_parity(wl, g)
+
+
+def test_diffrot_many_regions_and_limb(soap):
+    wl = workloads.make_config4(n_pix=5000, n_phases=8, grid_n=90)
+    wl.diff_rot = -0.2
+    g = run_gpu(soap, wl)
+    assert_parity(wl, g)
+
+
+def test_diffrot_fir_form_and_effects(soap):
+    wl = workloads.make_config3(n_pix=4000, n_phases=4, grid_n=80)
+    wl.diff_rot, wl.incl_deg = -0.18, 75.0
+    wl.phases = np.array([0.1, 0.2, 0.45, 0.55])
+    g = run_gpu(soap, wl, form=3)
+    assert_parity(wl, g)
+    from test_gpu_parity import _run_effects, _check_effects
+    outs, na = _run_effects(soap, wl)
+    _check_effects(wl, outs, na)
+
+
+def test_diffrot_full_size_config3_sampled(soap):
+    wl = workloads.make_config3()
+    wl.diff_rot = -0.18
+    g = run_gpu(soap, wl)
+    assert g["info"]["n_visible"] == 70688
+    for lo, hi in _sample_ranges(wl.n_pix, n=2):
+        assert_parity(wl, g, lo, hi)
+
+
+def test_diffrot_rejects_binned_form_and_fp64_active(soap):
+    wl = workloads.make_config1()
+    wl.diff_rot = -0.18
+    star = soap.soap_create(0)
+    soap.soap_set_option(star, soap.binding.SOAP_OPT_FORM, 1)
+    with pytest.raises(soap.SoapError) as e:
+        soap.soap_disk_geometry(star, wl)
+    assert e.value.code == soap.binding.SOAP_ERR_UNSUPPORTED
+    soap.soap_set_option(star, soap.binding.SOAP_OPT_FORM, 0)
+    soap.soap_disk_geometry(star, wl)
+    dev = torch.device("cuda:0")
+    q = soap.to_device_spectra(wl.quiet, wl.lambda0, wl.dlambda, dev)
+    s = soap.to_device_spectra(wl.spot, wl.lambda0, wl.dlambda, dev, wl.spot_contrast, wl.spot_lb)
+    Q = torch.empty(wl.n_pix, dtype=torch.float64, device=dev)
+    soap.soap_integrate_quiet(star, q, Q)                       # fp64 quiet works through the generic kernel
+    torch.cuda.synchronize()
+    Qo = oracle.quiet(wl, wl.quiet, wl.lambda0, wl.dlambda)
+    assert np.max(np.abs(Q.cpu().numpy() - Qo)) <= 1e-9 * oracle.geometry(wl)["sum_w"]
+    D = torch.empty((len(wl.phases), wl.n_pix), dtype=torch.float64, device=dev)
+    with pytest.raises(soap.SoapError) as e:
+        soap.soap_active_timeseries(star, q, s, None, wl.regions, wl.phases, D)
+    assert e.value.code == soap.binding.SOAP_ERR_UNSUPPORTED
+    soap.soap_destroy(star)
