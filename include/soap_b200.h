@@ -187,6 +187,15 @@ int soap_active_timeseries_effects(soap_star *star, const soap_spectra *quiet, c
                                    const double *phases, int32_t n_phases, void *out_total, void *out_flux,
                                    void *out_cb, int64_t out_pitch, int32_t *n_active, void *stream);
 
+/* ---- evolving regions: the same three outputs with a radius per (phase, region) -----------
+ * radii: HOST [n_phases][n_regions], the radius (same convention as soap_region.radius) of region r at phase p;
+ * a value <= 0 means the region is absent at that phase; every value must be < 1.  NULL = regions[r].radius.
+ * The evolution law itself (linear growth / decay, asymmetric Gaussian) is the caller's: it is input preparation. */
+int soap_active_timeseries_evolving(soap_star *star, const soap_spectra *quiet, const soap_spectra *spot,
+                                    const soap_spectra *facula, const soap_region *regions, int32_t n_regions,
+                                    const double *phases, int32_t n_phases, const double *radii, void *out_total,
+                                    void *out_flux, void *out_cb, int64_t out_pitch, int32_t *n_active, void *stream);
+
 /* ---- resolution lowering (Alg. 2, Alg. 5) ------------------------------------
  * "Lower the resolution of the final spectrum to match the resolution provided in the configuration file."  The
  * paper names no kernel; this library's reading (DESIGN.md R-LSF) is a Gaussian line-spread function of FWHM

@@ -209,3 +209,19 @@ def lower_resolution(rows, lambda0: float, k: float, R: float, nsig: float = LSF
     if rc != 0:
         raise RuntimeError(f"soap_oracle_lower_resolution failed: {rc}")
     return out.reshape(np.shape(rows))
+
+
+def active_evolving(star, S_quiet, S_spot, S_facula, lambda0: float, k: float, regions: Sequence, phases, radii,
+                    C_spot=None, C_facula=None, lb_spot=(1.0, 0.0, 0.0), lb_facula=(1.0, 0.0, 0.0),
+                    m_lo: int = 0, m_hi: Optional[int] = None, effect: int = 0):
+    """Evolving regions: phase p sees region r with radius radii[p][r] (<= 0: absent).  Plain loop
+    over the phases around `active` (Alg. 5 is per timestep: the region list is simply different at every step)."""
+    radii = np.asarray(radii, dtype=np.float64).reshape(len(phases), len(regions))
+    rows, counts = [], []
+    for p, ph in enumerate(phases):
+        regs = [(lat, lon, float(radii[p][r]), typ) for r, (lat, lon, _rad, typ) in enumerate(regions) if radii[p][r] > 0.0]
+        d, n = active(star, S_quiet, S_spot, S_facula, lambda0, k, regs, np.array([ph], dtype=np.float64), C_spot, C_facula,
+                      lb_spot, lb_facula, m_lo, m_hi, effect)
+        rows.append(d[0])
+        counts.append(int(n[0]))
+    return np.stack(rows), np.asarray(counts, dtype=np.int32)

@@ -28,7 +28,7 @@ SOAP_OPT_FORM, SOAP_OPT_QUIET_SPLITS, SOAP_OPT_KERNEL_TIMING = 1, 2, 3
 EXPORTED_SYMBOLS = (
     "soap_version", "soap_create", "soap_destroy", "soap_last_error", "soap_set_option", "soap_get_stats",
     "soap_disk_geometry", "soap_integrate_quiet", "soap_active_timeseries", "soap_active_timeseries_effects",
-    "soap_export_geometry", "soap_lower_resolution",
+    "soap_export_geometry", "soap_lower_resolution", "soap_active_timeseries_evolving",
     "soap_synthesize_host", "soap_batch_integrate_quiet", "soap_batch_active_timeseries",
 )
 
@@ -103,6 +103,10 @@ def load_library() -> ctypes.CDLL:
                                                    ctypes.POINTER(ctypes.c_double), i32, vp, vp, vp, i64,
                                                    ctypes.POINTER(i32), vp]
     lib.soap_export_geometry.argtypes = [vp, vp, vp, vp, vp]
+    lib.soap_active_timeseries_evolving.argtypes = [vp, ctypes.POINTER(c_spectra), ctypes.POINTER(c_spectra),
+                                                    ctypes.POINTER(c_spectra), ctypes.POINTER(c_region), i32,
+                                                    ctypes.POINTER(ctypes.c_double), i32, ctypes.POINTER(ctypes.c_double),
+                                                    vp, vp, vp, i64, ctypes.POINTER(i32), vp]
     lib.soap_lower_resolution.argtypes = [vp, vp, i64, i64, i64, i32, ctypes.c_double, ctypes.c_double, ctypes.c_double,
                                           vp, i64, vp]
     lib.soap_synthesize_host.argtypes = [vp, ctypes.POINTER(c_star_params), ctypes.POINTER(c_spectra),
@@ -284,6 +288,30 @@ def soap_active_timeseries_effects(star: Star, quiet: Spectra, spot: Optional[Sp
         star._h, ctypes.byref(cq), ctypes.byref(cs) if cs is not None else None,
         ctypes.byref(cf) if cf is not None else None, _regions(regions), len(regions),
         ph.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), n_ph,
+        out_total.data_ptr() if out_total is not None else None, out_flux.data_ptr() if out_flux is not None else None,
+        out_cb.data_ptr() if out_cb is not None else None, out_pitch,
+        na.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)) if na is not None else None, _stream_handle(stream)))
+    return na[:n_ph] if na is not None else None
+
+
+def soap_active_timeseries_evolving(star: Star, quiet: Spectra, spot: Optional[Spectra], facula: Optional[Spectra],
+                                    regions: Sequence, phases, radii, out_total: Optional[torch.Tensor] = None,
+                                    out_flux: Optional[torch.Tensor] = None, out_cb: Optional[torch.Tensor] = None,
+                                    want_n_active: bool = False, stream=None) -> Optional[np.ndarray]:
+    """As soap_active_timeseries_effects with radii[n_phases, n_regions] (HOST): evolving regions, <= 0 = absent."""
+    cq = quiet._c()
+    cs = spot._c() if spot is not None else None
+    cf = facula._c() if facula is not None else None
+    ph = np.ascontiguousarray(np.asarray(phases, dtype=np.float64))
+    n_ph = int(ph.shape[0])
+    rr = np.ascontiguousarray(np.asarray(radii, dtype=np.float64)).reshape(n_ph, len(regions))
+    na = np.zeros(max(1, n_ph), dtype=np.int32) if want_n_active else None
+    outs = [o for o in (out_total, out_flux, out_cb) if o is not None]
+    out_pitch = int(outs[0].shape[1]) if outs else int(quiet.n_pix)
+    star._check(star._lib.soap_active_timeseries_evolving(
+        star._h, ctypes.byref(cq), ctypes.byref(cs) if cs is not None else None,
+        ctypes.byref(cf) if cf is not None else None, _regions(regions), len(regions),
+        ph.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), n_ph, rr.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
         out_total.data_ptr() if out_total is not None else None, out_flux.data_ptr() if out_flux is not None else None,
         out_cb.data_ptr() if out_cb is not None else None, out_pitch,
         na.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)) if na is not None else None, _stream_handle(stream)))

@@ -476,15 +476,22 @@ int check_regions(soap_star *s, const soap_region *regions, int n_regions, const
 }
 
 // Localize (readings S11-S13): region centres in the observer frame for every phase.
+// `radii` (nullable): HOST [n_phases][n_regions] radius of every region at every phase (evolving regions);
+// <= 0 means the region is absent at that phase.  NULL: regions[r].radius at every phase.
 int upload_region_centres(soap_star *s, const soap_region *regions, int n_regions, const double *phases,
-                          int n_phases, cudaStream_t st) {
+                          int n_phases, const double *radii, cudaStream_t st) {
     {
         // per-cell form: a region's covered cells lie in a disc of radius chord = 2 sin(alpha / 2) around its projected
         // centre; with the cell-centre rule at most pi (chord N / 2 + 1.5)^2 of them, two entries each
         const double pi_ = 3.14159265358979323846, half = 0.5 * (double)s->prm.grid_n;
         double cells = 0.0;
         for (int r = 0; r < n_regions; ++r) {
-            const double ch = 2.0 * std::sin(0.5 * std::asin(regions[r].radius)) * half + 1.5;
+            double rad = regions[r].radius;
+            if (radii) {
+                rad = 0.0;
+                for (int p = 0; p < n_phases; ++p) rad = std::max(rad, radii[(size_t)p * n_regions + r]);
+            }
+            const double ch = 2.0 * std::sin(0.5 * std::asin(rad)) * half + 1.5;
             cells += pi_ * ch * ch;
         }
         cells = std::min(cells, (double)s->prm.grid_n * (double)s->prm.grid_n);
@@ -522,9 +529,11 @@ int upload_region_centres(soap_star *s, const soap_region *regions, int n_region
             o.xr = sx;
             o.yr = sy * s->sini - sz * s->cosi;
             o.zr = sy * s->cosi + sz * s->sini;
-            o.cos_alpha = std::sqrt(1.0 - g.radius * g.radius);
-            o.chord = 2.0 * std::sin(0.5 * std::asin(g.radius));
-            o.type = (o.zr < -g.radius - 1e-9) ? 0 : g.type;  // cap entirely on the far side
+            const double rad = radii ? radii[(size_t)p * n_regions + r] : g.radius;
+            const bool present = rad > 0.0;
+            o.cos_alpha = present ? std::sqrt(1.0 - rad * rad) : 2.0;
+            o.chord = present ? 2.0 * std::sin(0.5 * std::asin(rad)) : 0.0;
+            o.type = (!present || o.zr < -rad - 1e-9) ? 0 : g.type;  // absent at this phase, or entirely on the far side
             o.pad = 0;
         }
     }
@@ -704,10 +713,10 @@ int soap_integrate_quiet(soap_star *s, const soap_spectra *quiet, void *out, voi
     return quiet->dtype == SOAP_F32 ? quiet_impl<float>(s, quiet, out, st) : quiet_impl<double>(s, quiet, out, st);
 }
 
-int soap_active_timeseries_effects(soap_star *s, const soap_spectra *quiet, const soap_spectra *spot,
-                                   const soap_spectra *facula, const soap_region *regions, int32_t n_regions,
-                                   const double *phases, int32_t n_phases, void *out_total, void *out_flux, void *out_cb,
-                                   int64_t out_pitch, int32_t *n_active, void *stream) {
+int soap_active_timeseries_evolving(soap_star *s, const soap_spectra *quiet, const soap_spectra *spot,
+                                    const soap_spectra *facula, const soap_region *regions, int32_t n_regions,
+                                    const double *phases, int32_t n_phases, const double *radii, void *out_total,
+                                    void *out_flux, void *out_cb, int64_t out_pitch, int32_t *n_active, void *stream) {
     if (!s) return SOAP_ERR_INVALID_ARG;
     if (!s->ready) return s->fail(SOAP_ERR_NOT_READY, "soap_disk_geometry has not been called");
     int rc = check_spectra(s, quiet, "quiet");
@@ -715,12 +724,15 @@ int soap_active_timeseries_effects(soap_star *s, const soap_spectra *quiet, cons
     if (spot && ((rc = check_spectra(s, spot, "spot")) || (rc = check_same_grid(s, quiet, spot, "spot")))) return rc;
     if (facula && ((rc = check_spectra(s, facula, "facula")) || (rc = check_same_grid(s, quiet, facula, "facula")))) return rc;
     if ((rc = check_regions(s, regions, n_regions, phases, n_phases, spot, facula))) return rc;
+    if (radii)
+        for (size_t k = 0; k < (size_t)n_phases * (size_t)n_regions; ++k)
+            if (!(radii[k] < 1.0) || !std::isfinite(radii[k])) return s->fail(SOAP_ERR_INVALID_ARG, "radii[%zu] must be finite and < 1", k);
     if (n_phases == 0) return SOAP_OK;
     if (!out_total && !out_flux && !out_cb) return s->fail(SOAP_ERR_INVALID_ARG, "every output is NULL");
     if (out_pitch < quiet->n_pix) return s->fail(SOAP_ERR_INVALID_ARG, "out_pitch must be >= n_pix");
     SOAP_CUDA(s, cudaSetDevice(s->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if ((rc = upload_region_centres(s, regions, n_regions, phases, n_phases, st))) return rc;
+    if ((rc = upload_region_centres(s, regions, n_regions, phases, n_phases, radii, st))) return rc;
     // total and flux-only share the entry lists (weights w LB_t(mu)); CB-only needs the plain weights w, which
     // are the same lists again when both limb-brightening laws are identically 1
     const bool lb_is_one = (!spot || (spot->lb_c0 == 1.0 && spot->lb_c1 == 0.0 && spot->lb_c2 == 0.0)) &&
@@ -744,6 +756,14 @@ int soap_active_timeseries_effects(soap_star *s, const soap_spectra *quiet, cons
         s->last_active_cells = tot;
     }
     return SOAP_OK;
+}
+
+int soap_active_timeseries_effects(soap_star *s, const soap_spectra *quiet, const soap_spectra *spot,
+                                   const soap_spectra *facula, const soap_region *regions, int32_t n_regions,
+                                   const double *phases, int32_t n_phases, void *out_total, void *out_flux, void *out_cb,
+                                   int64_t out_pitch, int32_t *n_active, void *stream) {
+    return soap_active_timeseries_evolving(s, quiet, spot, facula, regions, n_regions, phases, n_phases, nullptr, out_total,
+                                           out_flux, out_cb, out_pitch, n_active, stream);
 }
 
 int soap_active_timeseries(soap_star *s, const soap_spectra *quiet, const soap_spectra *spot, const soap_spectra *facula,

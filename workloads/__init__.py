@@ -19,5 +19,6 @@ from .synth import (  # noqa: F401
     make_config4,
     make_config5_star,
     CONFIG_NAMES,
+    evolution_radii,
     SEED_BASE,
 )

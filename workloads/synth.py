@@ -339,3 +339,27 @@ def make_workload(config: int, **kw) -> Workload:
     if config == 5:
         return make_config5_star(kw.pop("star", 0), **kw)
     raise ValueError(f"unknown config {config}")
+
+
+# ---- active-region size evolution: input preparation for soap_active_timeseries_evolving ----
+MSH = 1e-6  # one millionth of the solar hemisphere; reading S11: filling factor f <-> radius sqrt(f)
+
+
+def evolution_radii(kind: str, t_days: np.ndarray, size0_msh: float = 10_000.0, rate_msh_per_day: float = 400.0,
+                    fwhm_days: float = 10.0, asymmetry: float = 0.09, t_peak_days: float = 0.0) -> np.ndarray:
+    """Radius (stellar radii) of one region at the times t_days under the three laws of P:280:
+    'growth' / 'decay': size(t) = size0 +/- rate t;  'gaussian': size0 exp(-(t - t_peak)^2 / 2 sigma^2) with
+    sigma = FWHM / 2.3548 * (1 -/+ asymmetry) before / after the peak (a stand-in for Murakozy et al. 2014, whose
+    exact form the paper does not give).  Sizes in MSH, clipped at 0; radius = sqrt(size * 1e-6)."""
+    t = np.asarray(t_days, dtype=np.float64)
+    if kind == "growth":
+        size = size0_msh + rate_msh_per_day * t
+    elif kind == "decay":
+        size = size0_msh - rate_msh_per_day * t
+    elif kind == "gaussian":
+        s0 = fwhm_days / (2.0 * np.sqrt(2.0 * np.log(2.0)))
+        sig = np.where(t < t_peak_days, s0 * (1.0 - asymmetry), s0 * (1.0 + asymmetry))
+        size = size0_msh * np.exp(-((t - t_peak_days) ** 2) / (2.0 * sig * sig))
+    else:
+        raise ValueError("kind must be 'growth', 'decay' or 'gaussian'")
+    return np.sqrt(np.clip(size, 0.0, None) * MSH)
