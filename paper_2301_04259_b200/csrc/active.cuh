@@ -73,6 +73,43 @@ __host__ __device__ inline size_t prep_smem_bytes(int n_mu, int chunk_cols) {
 }
 
 
+// The regions that can reach column x (|x - x_r| <= chord), in list order, gathered by one warp into cand[] so that
+// the per-cell membership loop visits only them (hundreds of regions: a column meets a few tens).  Returns their
+// number, or -1 when they do not fit (the caller then walks the whole list); [ylo, yhi] bounds the rows they reach.
+constexpr int kCandCap = 128;
+__device__ __forceinline__ int column_candidates(const RegionAtPhase *reg, int n_regions, double x, int lane, int *cand,
+                                                 double &ylo, double &yhi) {
+    int n = 0;
+    bool fits = true;
+    ylo = 2.0;
+    yhi = -2.0;
+    __syncwarp();
+    for (int r0 = 0; r0 < n_regions; r0 += 32) {
+        const int r = r0 + lane;
+        bool hit = false;
+        if (r < n_regions && reg[r].type != 0) {
+            const double ch = reg[r].chord * (1.0 + 1e-9) + 1e-12;
+            if (fabs(x - reg[r].xr) <= ch) {
+                hit = true;
+                ylo = fmin(ylo, reg[r].yr - ch);
+                yhi = fmax(yhi, reg[r].yr + ch);
+            }
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, hit);
+        const int k = n + __popc(m & ((1u << lane) - 1u));
+        if (hit && k < kCandCap) cand[k] = r;
+        n += __popc(m);
+        fits = fits && n <= kCandCap;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        ylo = fmin(ylo, __shfl_xor_sync(0xffffffffu, ylo, d));
+        yhi = fmax(yhi, __shfl_xor_sync(0xffffffffu, yhi, d));
+    }
+    __syncwarp();
+    return fits ? n : -1;
+}
+
 // grid = n_phases * kPrepCluster, block = kPrepThreads, cluster = kPrepCluster CTAs;
 // dynamic shared memory = prep_smem_bytes(n_mu, chunk_cols) with chunk_cols >= ceil(N / kPrepCluster).
 template <typename EntT>
@@ -81,6 +118,7 @@ __global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThre
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) unsigned char prep_smem[];
     const int n_seg = 3 * a.n_mu, N = a.N, cc = a.chunk_cols;
+    __shared__ int s_cand[kPrepThreads / 32][kCandCap];            // per warp: regions that can reach its column
     double *WDs = reinterpret_cast<double *>(prep_smem);           // [n_seg][cc]: this CTA's columns
     int *cnt = reinterpret_cast<int *>(WDs + (size_t)n_seg * cc);   // [n_seg] entries of this CTA (read by the others)
     int *off = cnt + n_seg;                                         // [n_seg] entries of the lower ranks
@@ -120,14 +158,9 @@ __global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThre
     // ---- bin: one warp per column, lanes over the rows (coalesced) --------------------------------------
     for (int j = c0 + warp; j < c0 + cols; j += n_warps) {
         const double x = cell_coord(j, N);
-        double ylo = 2.0, yhi = -2.0;
-        for (int r = 0; r < a.n_regions; ++r) {
-            if (reg[r].type == 0) continue;
-            const double ch = reg[r].chord * (1.0 + 1e-9) + 1e-12;
-            if (fabs(x - reg[r].xr) > ch) continue;
-            ylo = fmin(ylo, reg[r].yr - ch);
-            yhi = fmax(yhi, reg[r].yr + ch);
-        }
+        double ylo, yhi;
+        const int n_cand = column_candidates(reg, a.n_regions, x, lane, s_cand[warp], ylo, yhi);
+        const int n_loop = n_cand < 0 ? a.n_regions : n_cand;
         if (ylo > yhi) continue;
         int i_lo = (int)floor((ylo + 1.0) * 0.5 * N - 0.5) - 1;
         int i_hi = (int)ceil((yhi + 1.0) * 0.5 * N - 0.5) + 1;
@@ -158,7 +191,8 @@ __global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThre
                 double wc = 0.0, wl = 0.0;
                 if (b >= 0) {
                     const double y = cell_coord(i, N);
-                    for (int r = 0; r < a.n_regions; ++r) {  // list order: the last covering region wins
+                    for (int q = 0; q < n_loop; ++q) {  // list order: the last covering region wins
+                        const int r = n_cand < 0 ? q : s_cand[warp][q];
                         if (reg[r].type == 0) continue;
                         const double dot = __dadd_rn(__dadd_rn(__dmul_rn(x, reg[r].xr), __dmul_rn(y, reg[r].yr)),
                                                      __dmul_rn(m, reg[r].zr));
@@ -324,17 +358,12 @@ __global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThre
 // Walks column j of one phase: calls f(c, b, t, mu, w) for every lane of every 32-row chunk the regions can reach
 // (warp-uniform number of calls; t = 0 for cells no region covers, b = -1 for hidden cells).
 template <typename F>
-__device__ __forceinline__ void walk_column(const PrepArgs &a, const RegionAtPhase *reg, int j, int lane, F &&f) {
+__device__ __forceinline__ void walk_column(const PrepArgs &a, const RegionAtPhase *reg, int j, int lane, int *cand, F &&f) {
     const int N = a.N;
     const double x = cell_coord(j, N);
-    double ylo = 2.0, yhi = -2.0;
-    for (int r = 0; r < a.n_regions; ++r) {
-        if (reg[r].type == 0) continue;
-        const double ch = reg[r].chord * (1.0 + 1e-9) + 1e-12;
-        if (fabs(x - reg[r].xr) > ch) continue;
-        ylo = fmin(ylo, reg[r].yr - ch);
-        yhi = fmax(yhi, reg[r].yr + ch);
-    }
+    double ylo, yhi;
+    const int n_cand = column_candidates(reg, a.n_regions, x, lane, cand, ylo, yhi);
+    const int n_loop = n_cand < 0 ? a.n_regions : n_cand;
     if (ylo > yhi) return;
     int i_lo = (int)floor((ylo + 1.0) * 0.5 * N - 0.5) - 1;
     int i_hi = (int)ceil((yhi + 1.0) * 0.5 * N - 0.5) + 1;
@@ -349,7 +378,8 @@ __device__ __forceinline__ void walk_column(const PrepArgs &a, const RegionAtPha
         int t = 0;
         if (b >= 0) {
             const double y = cell_coord(i, N);
-            for (int r = 0; r < a.n_regions; ++r) {  // list order: the last covering region wins
+            for (int q = 0; q < n_loop; ++q) {  // list order: the last covering region wins
+                const int r = n_cand < 0 ? q : cand[q];
                 if (reg[r].type == 0) continue;
                 const double dot =
                     __dadd_rn(__dadd_rn(__dmul_rn(x, reg[r].xr), __dmul_rn(y, reg[r].yr)), __dmul_rn(m, reg[r].zr));
@@ -378,6 +408,7 @@ active_prepare_cells_kernel(const PrepArgs a) {
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) unsigned char prep_smem[];
     const int n_seg = 3 * a.n_mu, N = a.N, cc = a.chunk_cols;
+    __shared__ int s_cand[kPrepThreads / 32][kCandCap];  // per warp: regions that can reach its column
     int *cntc = reinterpret_cast<int *>(prep_smem);  // [n_seg][cc]: entries per (segment, column); then running offsets
     int *cnt = cntc + (size_t)n_seg * cc;            // [n_seg] entries of this CTA (read by the others)
     int *off = cnt + n_seg;                          // [n_seg] pool position of this CTA's block of the segment
@@ -417,7 +448,7 @@ active_prepare_cells_kernel(const PrepArgs a) {
     for (int j = c0 + warp; j < c0 + cols; j += n_warps) {
         int *col = cntc + (j - c0);
         int count = 0;
-        walk_column(a, reg, j, lane, [&](size_t, int b, int t, double, double) {
+        walk_column(a, reg, j, lane, s_cand[warp], [&](size_t, int b, int t, double, double) {
             // the quiet segment of a mu-bin collects the covered cells of every type, the kind segments one type each
             const unsigned same0 = __match_any_sync(0xffffffffu, t != 0 ? b : -1);
             const unsigned same = __match_any_sync(0xffffffffu, t != 0 ? b * 4 + t : -1);
@@ -488,7 +519,7 @@ active_prepare_cells_kernel(const PrepArgs a) {
     // ---- pass 2: write the entries; cntc[s][column] is the running position inside this CTA's block ------------
     for (int j = c0 + warp; j < c0 + cols; j += n_warps) {
         int *col = cntc + (j - c0);
-        walk_column(a, reg, j, lane, [&](size_t c, int b, int t, double m, double wc) {
+        walk_column(a, reg, j, lane, s_cand[warp], [&](size_t c, int b, int t, double m, double wc) {
             const unsigned same0 = __match_any_sync(0xffffffffu, t != 0 ? b : -1);
             const unsigned same = __match_any_sync(0xffffffffu, t != 0 ? b * 4 + t : -1);
             int p0 = 0, pt = 0;
