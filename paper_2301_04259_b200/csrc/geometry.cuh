@@ -95,10 +95,10 @@ struct MuCentres {  // passed by value as a kernel argument: no host -> device c
 
 
 // One warp, one column j, the 32-row chunks `chunk`, `chunk + stride`, ...: writes the cells' (mu, w, v, bin)
-// and adds the chunk's binned weights to s_W[64] (segmented warp scans, added in row order), returning
+// and adds the chunk's binned weights to s_W[64] and cell counts to s_C[64] (segmented warp scans, in row order), returning
 // the warp's weight sum and visible-cell count.
 __device__ __forceinline__ void geometry_chunks(int j, int chunk, int stride, int N, const Rotation &rot, double u1, double u2,
-                                                int n_mu, const double *s_mu, double *s_W, double *__restrict__ mu_out,
+                                                int n_mu, const double *s_mu, double *s_W, int *s_C, double *__restrict__ mu_out,
                                                 double *__restrict__ w_out, double *__restrict__ vel_out,
                                                 int *__restrict__ bin_out, double &sum, int &nvis) {
     const int lane = threadIdx.x & 31;
@@ -122,7 +122,10 @@ __device__ __forceinline__ void geometry_chunks(int j, int chunk, int stride, in
         unsigned tails = __ballot_sync(0xffffffffu, tail && bin >= 0);
         while (tails) {  // segments of one bin may repeat inside a chunk (apex of the column): add in lane order
             const int l = __ffs(tails) - 1;
-            if (lane == l) s_W[bin] += seg;
+            if (lane == l) {
+                s_W[bin] += seg;
+                s_C[bin] += lane - start + 1;  // cells of the segment
+            }
             __syncwarp();
             tails &= tails - 1;
         }
@@ -227,6 +230,65 @@ __device__ void build_binned_entries(int N, int n_mu, const double *col_a, const
     }
 }
 
+// Per-cell form (SOAP_FORM_CELLS, and always under differential rotation, where the cells of a column no longer
+// share a velocity): one entry per visible cell - the literal double loop of Alg. 1 - in the same layout, rows
+// sorted by (column, row) so that neighbouring entries have nearly equal shifts.  The last CTA of geometry_kernel
+// turns the per-(column, mu-bin) cell counts into row starts and per-column positions (one warp per mu-bin);
+// write_cell_entries_kernel then writes the entries, one warp per column.
+__device__ void build_cell_positions(int N, int n_mu, const int *colcnt, int *cellpos, int *row_start, float2 *ent32,
+                                     double2 *ent64) {
+    __shared__ int s_cnt[64];
+    __shared__ int s_start[65];
+    constexpr int kBatch = 8;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+    for (int b = warp; b < n_mu; b += n_warps) {
+        int cnt = 0;
+        for (int j0 = 0; j0 < N; j0 += 32 * kBatch) {
+            int v[kBatch];
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) {
+                const int j = j0 + 32 * k + lane;
+                v[k] = j < N ? colcnt[(size_t)j * n_mu + b] : 0;
+            }
+#pragma unroll
+            for (int k = 0; k < kBatch; ++k) cnt += v[k];
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, d);
+        if (lane == 0) s_cnt[b] = cnt;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int off = 0;
+        for (int b = 0; b < n_mu; ++b) {
+            s_start[b] = off;
+            off += (s_cnt[b] + 1) & ~1;
+        }
+        s_start[n_mu] = off;
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b <= n_mu; b += blockDim.x) row_start[b] = s_start[b];
+    for (int b = warp; b < n_mu; b += n_warps) {
+        int run = s_start[b];
+        for (int j0 = 0; j0 < N; j0 += 32) {
+            const int j = j0 + lane;
+            const int v = j < N ? colcnt[(size_t)j * n_mu + b] : 0;
+            int incl = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
+            }
+            if (j < N) cellpos[(size_t)b * N + j] = run + incl - v;
+            run += __shfl_sync(0xffffffffu, incl, 31);
+        }
+        if (lane == 0 && (s_cnt[b] & 1)) {  // zero-weight pad entry: rows stay 16-byte aligned
+            ent32[run] = make_float2(0.f, 0.f);
+            ent64[run] = make_double2(0.0, 0.0);
+        }
+    }
+}
+
 // a1 + a2.  The fp64 geometry of a cell costs a few hundred instructions, so the cells are spread over the
 // whole GPU: a CTA of 32 warps takes `cols_per_cta` columns, a warp takes one 32-row chunk of one column
 // (or several, strided, when a column has more chunks than the CTA has warps per column).  Per column:
@@ -247,15 +309,20 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
                 int *__restrict__ bin_out, double *__restrict__ col_a, double *__restrict__ Wbin /*[N][n_mu]*/,
                 double *__restrict__ col_sumw, int *__restrict__ col_nvis, float2 *__restrict__ ent32,
                 double2 *__restrict__ ent64, int *__restrict__ row_start, DevInfo *__restrict__ info,
-                unsigned int *__restrict__ done) {
+                unsigned int *__restrict__ done, int *__restrict__ colcnt /*[N][n_mu]*/,
+                int *__restrict__ cellpos /*[n_mu][N], per-cell form only*/, int cells) {
     __shared__ double s_W[kGeomWarps][64];
+    __shared__ int s_Cn[kGeomWarps][64];
     __shared__ double s_mu[64];
     __shared__ double s_sum[kGeomWarps];
     __shared__ int s_nvis[kGeomWarps];
     __shared__ int s_last;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int b = threadIdx.x; b < n_mu; b += blockDim.x) s_mu[b] = mu_centres.v[b];
-    for (int b = lane; b < 64; b += 32) s_W[warp][b] = 0.0;
+    for (int b = lane; b < 64; b += 32) {
+        s_W[warp][b] = 0.0;
+        s_Cn[warp][b] = 0;
+    }
     __syncthreads();
     const int wpc = geom_warps_per_col(N), cpc = kGeomWarps / wpc;
     const int cl = warp / wpc, chunk = warp - cl * wpc;  // local column, first chunk
@@ -263,7 +330,7 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
     double sum = 0.0;
     int nvis = 0;
     if (cl < cpc && j < N)
-        geometry_chunks(j, chunk, wpc, N, rot, u1, u2, n_mu, s_mu, s_W[warp], mu_out, w_out, vel_out, bin_out, sum, nvis);
+        geometry_chunks(j, chunk, wpc, N, rot, u1, u2, n_mu, s_mu, s_W[warp], s_Cn[warp], mu_out, w_out, vel_out, bin_out, sum, nvis);
     if (lane == 0) {
         s_sum[warp] = sum;
         s_nvis[warp] = nvis;
@@ -274,8 +341,13 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
         if (jj < N) {
             for (int b = lane; b < n_mu; b += 32) {
                 double W = 0.0;
-                for (int k = 0; k < wpc; ++k) W += s_W[warp * wpc + k][b];
+                int C = 0;
+                for (int k = 0; k < wpc; ++k) {
+                    W += s_W[warp * wpc + k][b];
+                    C += s_Cn[warp * wpc + k][b];
+                }
                 Wbin[(size_t)jj * n_mu + b] = W;
+                colcnt[(size_t)jj * n_mu + b] = C;
             }
             if (lane == 0) {
                 double sw = 0.0;
@@ -299,72 +371,40 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
     __threadfence();
     if (threadIdx.x == 0) *done = 0;
     build_binned_entries(N, n_mu, col_a, Wbin, col_sumw, col_nvis, ent32, ent64, row_start, info);
+    if (cells) {  // per-cell form: the entry list is rebuilt by write_cell_entries_kernel at these positions
+        __syncthreads();
+        build_cell_positions(N, n_mu, colcnt, cellpos, row_start, ent32, ent64);
+    }
 }
 
-// Per-cell form (SOAP_FORM_CELLS, and always under differential rotation, where the cells of a column no longer
-// share a velocity): one entry per visible cell - the literal double loop of Alg. 1 - in the same layout, with the
-// cell's own shift factor D_c - 1 from its velocity.  Two passes over the cells by one CTA (loads in batches of
-// 8 x 32 cells); within a row the entries keep (j, i) order, so neighbouring entries have nearly equal shifts.
-__global__ void build_cell_entries_kernel(int N, int n_mu, int mode, const double *__restrict__ vel,
-                                          const double *__restrict__ w, const int *__restrict__ bin,
-                                          float2 *__restrict__ ent32, double2 *__restrict__ ent64,
-                                          int *__restrict__ row_start) {
-    __shared__ int s_cnt[64];
-    __shared__ int s_start[65];
-    constexpr int kBatch = 8;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
-    const int ncell = N * N;
-    for (int b = warp; b < n_mu; b += n_warps) {
-        int cnt = 0;
-        for (int c0 = 0; c0 < ncell; c0 += 32 * kBatch) {
-            int bb[kBatch];
-#pragma unroll
-            for (int k = 0; k < kBatch; ++k) {
-                const int c = c0 + 32 * k + lane;
-                bb[k] = c < ncell ? bin[c] : -1;
-            }
-#pragma unroll
-            for (int k = 0; k < kBatch; ++k) cnt += __popc(__ballot_sync(0xffffffffu, bb[k] == b));
-        }
-        if (lane == 0) s_cnt[b] = cnt;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int off = 0;
-        for (int b = 0; b < n_mu; ++b) {
-            s_start[b] = off;
-            off += (s_cnt[b] + 1) & ~1;
-        }
-        s_start[n_mu] = off;
-    }
-    __syncthreads();
-    for (int b = threadIdx.x; b <= n_mu; b += blockDim.x) row_start[b] = s_start[b];
-    for (int b = warp; b < n_mu; b += n_warps) {
-        int pos = s_start[b];
-        for (int c0 = 0; c0 < ncell; c0 += 32 * kBatch) {
-            int bb[kBatch];
-#pragma unroll
-            for (int k = 0; k < kBatch; ++k) {
-                const int c = c0 + 32 * k + lane;
-                bb[k] = c < ncell ? bin[c] : -1;
-            }
-#pragma unroll
-            for (int k = 0; k < kBatch; ++k) {
-                const int c = c0 + 32 * k + lane;
-                const bool in = bb[k] == b;
-                const unsigned m = __ballot_sync(0xffffffffu, in);
-                if (in) {
-                    const int e = pos + __popc(m & ((1u << lane) - 1u));
-                    const double a = doppler_minus_one(vel[c], mode);
-                    ent32[e] = make_float2((float)a, (float)w[c]);
-                    ent64[e] = make_double2(a, w[c]);
-                }
-                pos += __popc(m);
-            }
-        }
-        if (lane == 0 && (s_cnt[b] & 1)) {
-            ent32[pos] = make_float2(0.f, 0.f);
-            ent64[pos] = make_double2(0.0, 0.0);
+// One warp per column: writes the column's cells as entries (a_c, w_c), a_c = D_c - 1 from the cell's own velocity,
+// at cellpos[bin][column] + rank among the column's earlier cells of that bin (row order).
+constexpr int kCellWarps = 8;
+__global__ void __launch_bounds__(32 * kCellWarps)
+write_cell_entries_kernel(int N, int n_mu, int mode, const double *__restrict__ vel, const double *__restrict__ w,
+                          const int *__restrict__ bin, const int *__restrict__ cellpos, float2 *__restrict__ ent32,
+                          double2 *__restrict__ ent64) {
+    __shared__ int s_pos[kCellWarps][64];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int j = blockIdx.x * kCellWarps + warp;
+    if (j >= N) return;
+    for (int b = lane; b < n_mu; b += 32) s_pos[warp][b] = cellpos[(size_t)b * N + j];
+    __syncwarp();
+    for (int i0 = 0; i0 < N; i0 += 32) {
+        const int i = i0 + lane;
+        const size_t c = (size_t)j * N + (i < N ? i : N - 1);
+        const int b = i < N ? bin[c] : -1;
+        const double v = vel[c], wc = w[c];
+        const unsigned same = __match_any_sync(0xffffffffu, b);
+        int e = 0;
+        if (b >= 0) e = s_pos[warp][b] + __popc(same & ((1u << lane) - 1u));
+        __syncwarp();
+        if (b >= 0 && lane == __ffs(same) - 1) s_pos[warp][b] += __popc(same);
+        __syncwarp();
+        if (b >= 0) {
+            const double a = doppler_minus_one(v, mode);
+            ent32[e] = make_float2((float)a, (float)wc);
+            ent64[e] = make_double2(a, wc);
         }
     }
 }

@@ -69,7 +69,7 @@ struct soap_star {
 
     // geometry (device)
     DevBuf<double> d_mu, d_w, d_vel, d_col_a, d_Wbin, d_col_sumw;
-    DevBuf<int> d_bin, d_col_nvis, d_row_start;
+    DevBuf<int> d_bin, d_col_nvis, d_row_start, d_colcnt, d_cellpos;
     DevBuf<float2> d_ent32;
     DevBuf<double2> d_ent64;
     DevBuf<DevInfo> d_info;
@@ -583,7 +583,7 @@ int soap_create(soap_star **out, int device) {
 int soap_destroy(soap_star *s) {
     if (!s) return SOAP_OK;
     cudaSetDevice(s->device);
-    s->d_geom_done.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
+    s->d_geom_done.release(); s->d_colcnt.release(); s->d_cellpos.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
     s->d_Wbin.release(); s->d_col_sumw.release(); s->d_bin.release(); s->d_col_nvis.release(); s->d_row_start.release();
     s->d_ent32.release(); s->d_ent64.release(); s->d_info.release(); s->d_partial.release(); s->d_tile_ticket.release(); s->d_rp.release();
     s->d_aent.release(); s->d_segcnt.release(); s->d_nactive.release(); s->d_counters.release(); s->d_sched.release(); s->d_jobs.release();
@@ -653,7 +653,9 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
         return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_BINNED needs solid-body rotation: the cells of a column must share one velocity");
     s->form_used = (s->form == SOAP_FORM_CELLS || s->form == SOAP_FORM_FIR) ? s->form : SOAP_FORM_BINNED;
     s->cell_entries = s->form == SOAP_FORM_CELLS || prm->diff_rot != 0.0;
-    if (s->cell_entries && s->form_used == SOAP_FORM_BINNED) s->form_used = SOAP_FORM_CELLS;
+    // AUTO under differential rotation: per-cell entries with every run collapsed (the binned form does not apply;
+    // the collapse is exact and ~5x cheaper than one lerp-accumulate per cell and pixel)
+    if (s->cell_entries && s->form_used == SOAP_FORM_BINNED) s->form_used = s->form == SOAP_FORM_AUTO ? SOAP_FORM_FIR : SOAP_FORM_CELLS;
     const double vmax = std::fabs(prm->vsini_kms * sini) * (double)(N - 1) / (double)N * std::max(1.0, 1.0 + prm->diff_rot);
     s->amax = std::max(std::fabs(host_dshift(vmax, prm->doppler_mode)), std::fabs(host_dshift(-vmax, prm->doppler_mode)));
 
@@ -665,6 +667,8 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     SOAP_CUDA(s, s->d_Wbin.reserve((size_t)N * n_mu));
     SOAP_CUDA(s, s->d_col_sumw.reserve(N));
     SOAP_CUDA(s, s->d_col_nvis.reserve(N));
+    SOAP_CUDA(s, s->d_colcnt.reserve((size_t)N * n_mu));
+    SOAP_CUDA(s, s->d_cellpos.reserve((size_t)N * n_mu));
     SOAP_CUDA(s, s->d_row_start.reserve(n_mu + 1));
     SOAP_CUDA(s, s->d_info.reserve(1));
     const size_t ent_cap = std::max(s->cell_entries ? ncell : (size_t)0, (size_t)N * n_mu) + 2 * (size_t)n_mu + 8;
@@ -682,12 +686,12 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     geometry_kernel<<<(N + geom_cols_per_cta(N) - 1) / geom_cols_per_cta(N), 32 * kGeomWarps, 0, st>>>(
         N, rot, prm->ld_u1, prm->ld_u2, prm->doppler_mode, n_mu, mc, s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr, s->d_bin.ptr,
         s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr, s->d_ent32.ptr, s->d_ent64.ptr, s->d_row_start.ptr,
-        s->d_info.ptr, s->d_geom_done.ptr);
+        s->d_info.ptr, s->d_geom_done.ptr, s->d_colcnt.ptr, s->d_cellpos.ptr, s->cell_entries ? 1 : 0);
     SOAP_LAUNCH_CHECK(s, "geometry_kernel");
     if (s->cell_entries) {
-        build_cell_entries_kernel<<<1, 1024, 0, st>>>(N, n_mu, prm->doppler_mode, s->d_vel.ptr, s->d_w.ptr, s->d_bin.ptr, s->d_ent32.ptr,
-                                                      s->d_ent64.ptr, s->d_row_start.ptr);
-        SOAP_LAUNCH_CHECK(s, "build_cell_entries_kernel");
+        write_cell_entries_kernel<<<(N + kCellWarps - 1) / kCellWarps, 32 * kCellWarps, 0, st>>>(
+            N, n_mu, prm->doppler_mode, s->d_vel.ptr, s->d_w.ptr, s->d_bin.ptr, s->d_cellpos.ptr, s->d_ent32.ptr, s->d_ent64.ptr);
+        SOAP_LAUNCH_CHECK(s, "write_cell_entries_kernel");
     }
     s->ready = true;
     if (info) {

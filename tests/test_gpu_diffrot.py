@@ -26,7 +26,7 @@ def test_diffrot_geometry_is_bit_exact(soap):
     og = oracle.geometry(wl)
     np.testing.assert_array_equal(g["geo"]["vel"], og["vel"])
     np.testing.assert_array_equal(g["geo"]["bin"], og["bin"])
-    assert g["stats"]["form"] == 2 and g["info"]["n_entries"] == og["n_visible"]
+    assert g["stats"]["form"] == 3 and g["info"]["n_entries"] == og["n_visible"]  # AUTO: per-cell entries, runs collapsed
 
 
 @pytest.mark.parametrize("dr,incl", [(-0.18, 90.0), (-0.18, 55.0), (0.25, 70.0)])
@@ -36,6 +36,16 @@ def test_diffrot_quiet_and_active_parity(soap, dr, incl):
     wl.phases = np.array([0.35, 0.45, 0.5, 0.55, 0.65, 0.0])
     g = run_gpu(soap, wl)
     assert g["n_active"].max() > 0
+    assert_parity(wl, g)
+
+
+def test_diffrot_direct_per_cell_form(soap):
+    """SOAP_FORM_CELLS under differential rotation: one lerp-accumulate per (cell, pixel), no run collapse."""
+    wl = workloads.make_config3(n_pix=5000, n_phases=4, grid_n=90)
+    wl.diff_rot, wl.incl_deg = -0.18, 65.0
+    wl.phases = np.array([0.1, 0.2, 0.45, 0.55])
+    g = run_gpu(soap, wl, form=2)
+    assert g["stats"]["form"] == 2
     assert_parity(wl, g)
 
 
