@@ -1,0 +1,81 @@
+"""Degenerate and extreme inputs of the hot path against the oracle (needs a B200: -m gpu)."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from test_gpu_parity import assert_parity, run_gpu
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def soap():
+    import paper_2301_04259_b200 as soap_mod
+    soap_mod.binding.load_library()
+    return soap_mod
+
+
+@pytest.mark.parametrize("grid_n", [1, 2, 3, 7, 33])
+def test_tiny_grids(soap, grid_n):
+    wl = workloads.make_config2(n_pix=2500, n_phases=3, grid_n=grid_n)
+    wl.regions = [(0.0, 180.0, 0.6, 1)]
+    wl.phases = np.array([0.5, 0.25, 0.0])
+    g = run_gpu(soap, wl)
+    assert g["info"]["n_visible"] == oracle.geometry(wl)["n_visible"]
+    assert_parity(wl, g, check_rv=False)
+
+
+def test_one_mu_bin_and_sixty_four_mu_bins(soap):
+    wl = workloads.make_config2(n_pix=3000, n_phases=2, grid_n=70)
+    wl.phases = np.array([0.5, 0.45])
+    one = workloads.make_config2(n_pix=3000, n_phases=2, grid_n=70)
+    one.phases = wl.phases
+    one.mu_centres = np.array([0.7])
+    one.quiet, one.spot = one.quiet[:1].copy(), one.spot[:1].copy()
+    assert_parity(one, run_gpu(soap, one))
+    many = workloads.make_config2(n_pix=3000, n_phases=2, grid_n=70)
+    many.phases = wl.phases
+    many.mu_centres = (np.arange(64) + 1.0) / 64.0
+    reps = [k * 20 // 64 for k in range(64)]
+    many.quiet, many.spot = many.quiet[reps].copy(), many.spot[reps].copy()
+    assert_parity(many, run_gpu(soap, many))
+
+
+def test_pole_on_star_and_polar_and_huge_regions(soap):
+    wl = workloads.make_config3(n_pix=3000, n_phases=4, grid_n=64)
+    wl.incl_deg = 0.0                                   # pole-on: no Doppler shift at all
+    wl.regions = [(90.0, 0.0, 0.3, 2), (10.0, 40.0, 0.95, 1), (-80.0, 200.0, 0.2, 2)]
+    wl.phases = np.array([0.0, 0.3, 0.5, 0.9])
+    g = run_gpu(soap, wl)
+    assert g["n_active"].max() > 500
+    assert_parity(wl, g, check_rv=False)
+    wl.incl_deg = 12.0
+    assert_parity(wl, run_gpu(soap, wl), check_rv=False)
+
+
+def test_thousands_of_phases_keep_their_order(soap):
+    """More phases than the heaviest-first ordering sorts (kScheduleSortMax = 4096): identity order, same results."""
+    wl = workloads.make_config2(n_pix=2048, n_phases=4, grid_n=40)
+    base = np.array([0.5, 0.47, 0.0, 0.53])
+    wl.phases = np.tile(base, 1100)                      # 4400 phases
+    g = run_gpu(soap, wl)
+    wl4 = workloads.make_config2(n_pix=2048, n_phases=4, grid_n=40)
+    wl4.phases = base
+    g4 = run_gpu(soap, wl4)
+    assert np.array_equal(g["D"].reshape(1100, 4, -1), np.broadcast_to(g4["D"], (1100, 4, 2048)))
+    assert_parity(wl4, g4)
+
+
+def test_fastest_supported_rotator_and_too_fast(soap):
+    wl = workloads.make_config2(n_pix=9000, n_phases=2, grid_n=60)
+    wl.vsini_kms = 150.0                                 # halo ~ 250 px at 5000 A
+    wl.phases = np.array([0.5, 0.4])
+    assert_parity(wl, run_gpu(soap, wl), check_rv=False)
+    wl.vsini_kms = 25000.0                               # |v| < 0.1 c, but the staged span would not fit in shared memory
+    with pytest.raises(soap.SoapError) as e:
+        run_gpu(soap, wl)
+    assert e.value.code == soap.binding.SOAP_ERR_UNSUPPORTED
