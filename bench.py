@@ -28,7 +28,7 @@ METRIC = "integrated spectra/s and cell*pixel interps/s (full visible, 300^2 gri
 N_SM, FP32_LANES_PER_SM = 148, 128
 FLOPS_PER_UNIT = 4  # one lerp-accumulate = 2 FP32 FMAs per (entry, pixel): acc += W u_r; acc += (W a) v_r
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this
-# workload (profiles/r01_v4_sia_full.md); algorithmic: active 74.4 MB in + 31 MB out, quiet 24.8 MB in.
+# workload (profiles/r01_v5_sia_full.md); algorithmic: active 74.4 MB in + 31 MB out, quiet 24.8 MB in.
 NCU_DRAM_TRAFFIC_BYTES = {"sia_f32_kernel<quiet>": 25.1e6, "sia_f32_kernel<active>": 109.5e6}
 
 
