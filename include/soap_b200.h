@@ -60,12 +60,14 @@ enum soap_effect { SOAP_EFFECT_TOTAL = 0, SOAP_EFFECT_FLUX = 1, SOAP_EFFECT_CB =
 /* How the shift-interpolate-accumulate sum is evaluated.  All forms compute the same sums (Alg. 1,
  * Eq. 3) and differ only in rounding order. */
 enum soap_form {
-    SOAP_FORM_AUTO = 0,   /* library picks (currently SOAP_FORM_BINNED for solid-body rotation) */
+    SOAP_FORM_AUTO = 0,   /* library picks: SOAP_FORM_BINNED for solid-body rotation; under differential rotation
+                             (diff_rot != 0) one entry per cell with the run collapse of SOAP_FORM_FIR */
     SOAP_FORM_BINNED = 1, /* cells pre-binned by (column, mu-bin): all cells of a column share one
                              velocity under solid-body rotation (BASELINE.json north_star) */
     SOAP_FORM_CELLS = 2,  /* one entry per visible cell - the literal double loop of Alg. 1 */
-    SOAP_FORM_FIR = 3     /* per-tile collapse of all entries with equal integer shift into FIR taps
-                             linear in the pixel index (exact in exact arithmetic) */
+    SOAP_FORM_FIR = 3     /* binned (or, under differential rotation, per-cell) entries; per wavelength tile every
+                             run of entries of one spectrum row with the same integer shift is collapsed into one
+                             record {sum W, sum W a}: taps linear in the pixel index (exact in exact arithmetic) */
 };
 
 enum soap_option {
