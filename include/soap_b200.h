@@ -23,7 +23,8 @@
  *     is enqueued on it; a call is asynchronous unless it has a non-NULL HOST output pointer
  *     (`info`, `n_active`, export, stats), in which case it synchronises that stream before returning.
  *     Scratch is (re)allocated with cudaMalloc when a call needs more than any earlier call did; once
- *     sizes have been seen, calls allocate nothing and can be captured in a CUDA graph.
+ *     sizes have been seen, calls allocate nothing.  soap_active_timeseries* stage the region centres
+ *     through a ring of pinned host buffers guarded by events, so they must not be stream-captured.
  *   - There is no CPU fallback and no other backend: without a CUDA device every compute entry point
  *     returns SOAP_ERR_CUDA.
  *   - Cell indexing: c = j * N + i with j the column (x) index and i the row (y) index;
