@@ -313,6 +313,26 @@ def run_graft(args):
            "algorithmic_bytes": lsf_bytes}
     lsf["frac"] = lsf["achieved"] / lsf["peak"]
 
+    # ---- first-moment RV of every generated line in every lowered spectrum (the reduction after the path)
+    centres = torch.from_numpy(wl.line_centres.astype(np.float64)).to(dev)
+    halfw = torch.from_numpy((3.0 * np.maximum(wl.line_sigmas, 0.03)).astype(np.float64)).to(dev)
+    norm = torch.full((n_spec,), float(info["sum_weights"]), dtype=torch.float64, device=dev)
+    rv_ms = []
+    for it in range(8):
+        flush_buf.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        rvs = soap.soap_line_rvs(star, Flow, P, wl.lambda0, wl.dlambda, centres, halfw, norm, 64)
+        b.record()
+        b.synchronize()
+        if it >= 3:
+            rv_ms.append(a.elapsed_time(b))
+    rv_bytes = n_spec * P * 4 + n_spec * len(wl.line_centres) * 8
+    line_rv = {"kernel": "line_rv_kernel<float>", "lines": int(len(wl.line_centres)), "rows": n_spec, "ms": float(np.mean(rv_ms)),
+               "bound": "hbm", "achieved": rv_bytes / (float(np.mean(rv_ms)) * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+               "algorithmic_bytes": rv_bytes, "finite": int(torch.isfinite(rvs).sum().item())}
+    line_rv["frac"] = line_rv["achieved"] / line_rv["peak"]
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ------------
     pitch = q.pitch
 
@@ -368,7 +388,7 @@ def run_graft(args):
         "executed_lerp_accumulates_per_s": world * exec_units / (ms_per_step * 1e-3),
         "definitional": {"n_visible": n_vis, "active_cells_all_phases": act_cells, "quiet_entries": stats["quiet_entries"],
                          "active_entries_all_phases": stats["active_entries"]},
-        "roofline": roofline, "fir_form": fir, "lower_resolution": lsf, "clocks": clocks,
+        "roofline": roofline, "fir_form": fir, "lower_resolution": lsf, "line_rvs": line_rv, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "spectra/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms / e2e_steps, "api": "soap_synthesize_host (pinned host buffers)"},
         "gpu_launches": launches, "wall_s_timed_region": wall,

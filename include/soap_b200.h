@@ -211,6 +211,18 @@ int soap_lower_resolution(soap_star *star, const void *in, int64_t n_rows, int64
                           int32_t dtype, double lambda0, double dlambda, double resolution, void *out,
                           int64_t out_pitch, void *stream);
 
+/* ---- first-moment radial velocity of spectral lines (the RV reduction that follows the path) -----
+ * The paper cross-correlates with a mask and fits a Gaussian; the mask is not available, and BASELINE.json's
+ * acceptance functional is a first-moment RV per line, which this entry point computes on the device:
+ *   window m_lo = ceil((lc - hw - lambda0)/dlambda) .. m_hi = floor((lc + hw - lambda0)/dlambda), depth = 1 - F[r][m]/norm[r],
+ *   out_rv[r][l] = c * sum (lambda_m - lc) depth / sum depth / lc   in cm/s;
+ *   NaN when the window is not inside [edge, n_pix - edge) or the depths sum to 0.
+ * rows: DEVICE [n_rows][pitch] of `dtype`;  centres, half_widths: DEVICE [n_lines] fp64 (Angstrom);
+ * norm: DEVICE [n_rows] fp64 (continuum level, e.g. sum_weights);  out_rv: DEVICE [n_rows][n_lines] fp64. */
+int soap_line_rvs(soap_star *star, const void *rows, int64_t n_rows, int64_t n_pix, int64_t pitch, int32_t dtype,
+                  double lambda0, double dlambda, const double *centres, const double *half_widths, int64_t n_lines,
+                  const double *norm, int64_t edge, double *out_rv, void *stream);
+
 /* ---- debug export of the geometry (HOST outputs, N*N each, any may be NULL; synchronous) --------
  * Hidden cells: mu = 0, vel = 0, w = 0, bin = -1. */
 int soap_export_geometry(soap_star *star, double *mu, double *vel, double *w, int32_t *bin);

@@ -74,6 +74,10 @@ def _load():
         lib.soap_oracle_lower_resolution.restype = ctypes.c_int
         lib.soap_oracle_lower_resolution.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_double,
                                                      ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_void_p]
+        lib.soap_oracle_line_rvs.restype = ctypes.c_int
+        lib.soap_oracle_line_rvs.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_double, ctypes.c_double,
+                                             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64,
+                                             ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -225,3 +229,18 @@ def active_evolving(star, S_quiet, S_spot, S_facula, lambda0: float, k: float, r
         rows.append(d[0])
         counts.append(int(n[0]))
     return np.stack(rows), np.asarray(counts, dtype=np.int32)
+
+
+def line_rvs(rows, lambda0: float, k: float, centres, half_widths, norm, edge: int = 0) -> np.ndarray:
+    """First-moment RV (cm/s) of every line in every row (north_star's acceptance functional).
+    rows [n_rows, P] (or [P]); norm: scalar or [n_rows] continuum level; returns [n_rows, n_lines] (NaN: window off-grid)."""
+    lib = _load()
+    a = _f64(np.atleast_2d(rows))
+    c, h = _f64(np.atleast_1d(centres)), _f64(np.atleast_1d(half_widths))
+    nrm = _f64(np.broadcast_to(np.asarray(norm, dtype=np.float64), (a.shape[0],)).copy())
+    out = np.empty((a.shape[0], c.shape[0]), dtype=np.float64)
+    rc = lib.soap_oracle_line_rvs(a.ctypes.data, a.shape[0], a.shape[1], float(lambda0), float(k), c.ctypes.data, h.ctypes.data,
+                                  c.shape[0], nrm.ctypes.data, int(edge), out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"soap_oracle_line_rvs failed: {rc}")
+    return out

@@ -382,3 +382,36 @@ int soap_oracle_lower_resolution(const double *in, int64_t n_rows, int64_t P, do
     }
     return 0;
 }
+
+/* First-moment radial velocity of spectral lines: the acceptance functional of BASELINE.json north_star ("a
+ * first-moment RV of each line"), made concrete in SURVEY section 8c; it stands in for the paper's CCF + Gaussian
+ * fit, whose mask is not available.  For row r and line l with centre lc and window half-width hw:
+ *   pixels m_lo = ceil((lc - hw - lambda0)/k) .. m_hi = floor((lc + hw - lambda0)/k)  (inclusive),
+ *   f = F[r][m] / norm[r],  depth = 1 - f,
+ *   rv[r][l] = c * sum_m (lambda_m - lc) depth / sum_m depth / lc          [cm/s, c = 299792.458e5]
+ * NaN when the window is not inside [edge, P - edge) or the depth sum is 0.  rows: [n_rows][P]; rv: [n_rows][n_lines]. */
+int soap_oracle_line_rvs(const double *rows, int64_t n_rows, int64_t P, double lambda0, double k,
+                         const double *centres, const double *half_widths, int64_t n_lines, const double *norm,
+                         int64_t edge, double *rv) {
+    if (!rows || !centres || !half_widths || !norm || !rv || P < 1 || !(k > 0.0)) return -1;
+    const double c_cms = SOAP_C_KMS * 1e5;
+#pragma omp parallel for schedule(static)
+    for (int64_t l = 0; l < n_lines; ++l) {
+        const double lc = centres[l], hw = half_widths[l];
+        const int64_t m_lo = (int64_t)ceil((lc - hw - lambda0) / k);
+        const int64_t m_hi = (int64_t)floor((lc + hw - lambda0) / k);
+        const int ok = (m_lo >= edge) && (m_hi < P - edge) && (m_hi >= m_lo);
+        for (int64_t r = 0; r < n_rows; ++r) {
+            double num = 0.0, den = 0.0;
+            if (ok) {
+                for (int64_t m = m_lo; m <= m_hi; ++m) {
+                    const double depth = 1.0 - rows[r * P + m] / norm[r];
+                    num += ((lambda0 + k * (double)m) - lc) * depth;
+                    den += depth;
+                }
+            }
+            rv[r * n_lines + l] = (ok && den != 0.0) ? c_cms * num / den / lc : NAN;
+        }
+    }
+    return 0;
+}

@@ -28,7 +28,7 @@ SOAP_OPT_FORM, SOAP_OPT_QUIET_SPLITS, SOAP_OPT_KERNEL_TIMING = 1, 2, 3
 EXPORTED_SYMBOLS = (
     "soap_version", "soap_create", "soap_destroy", "soap_last_error", "soap_set_option", "soap_get_stats",
     "soap_disk_geometry", "soap_integrate_quiet", "soap_active_timeseries", "soap_active_timeseries_effects",
-    "soap_export_geometry", "soap_lower_resolution", "soap_active_timeseries_evolving",
+    "soap_export_geometry", "soap_lower_resolution", "soap_active_timeseries_evolving", "soap_line_rvs",
     "soap_synthesize_host", "soap_batch_integrate_quiet", "soap_batch_active_timeseries",
 )
 
@@ -103,6 +103,7 @@ def load_library() -> ctypes.CDLL:
                                                    ctypes.POINTER(ctypes.c_double), i32, vp, vp, vp, i64,
                                                    ctypes.POINTER(i32), vp]
     lib.soap_export_geometry.argtypes = [vp, vp, vp, vp, vp]
+    lib.soap_line_rvs.argtypes = [vp, vp, i64, i64, i64, i32, ctypes.c_double, ctypes.c_double, vp, vp, i64, vp, i64, vp, vp]
     lib.soap_active_timeseries_evolving.argtypes = [vp, ctypes.POINTER(c_spectra), ctypes.POINTER(c_spectra),
                                                     ctypes.POINTER(c_spectra), ctypes.POINTER(c_region), i32,
                                                     ctypes.POINTER(ctypes.c_double), i32, ctypes.POINTER(ctypes.c_double),
@@ -316,6 +317,21 @@ def soap_active_timeseries_evolving(star: Star, quiet: Spectra, spot: Optional[S
         out_cb.data_ptr() if out_cb is not None else None, out_pitch,
         na.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)) if na is not None else None, _stream_handle(stream)))
     return na[:n_ph] if na is not None else None
+
+
+def soap_line_rvs(star: Star, rows: torch.Tensor, n_pix: int, lambda0: float, dlambda: float, centres: torch.Tensor,
+                  half_widths: torch.Tensor, norm: torch.Tensor, edge: int = 0, stream=None) -> torch.Tensor:
+    """First-moment RV (cm/s) of every line in every row; all tensors on the device, centres / half_widths / norm fp64."""
+    r2 = rows if rows.dim() == 2 else rows.unsqueeze(0)
+    for t in (centres, half_widths, norm):
+        if t.dtype != torch.float64 or not t.is_contiguous():
+            raise ValueError("centres, half_widths and norm must be contiguous fp64 device tensors")
+    out = torch.empty((r2.shape[0], centres.shape[0]), dtype=torch.float64, device=rows.device)
+    star._check(star._lib.soap_line_rvs(
+        star._h, r2.data_ptr(), int(r2.shape[0]), int(n_pix), int(r2.stride(0)), _dtype_code(r2), float(lambda0), float(dlambda),
+        centres.data_ptr(), half_widths.data_ptr(), int(centres.shape[0]), norm.data_ptr(), int(edge), out.data_ptr(),
+        _stream_handle(stream)))
+    return out
 
 
 def soap_lower_resolution(star: Star, rows: torch.Tensor, n_pix: int, lambda0: float, dlambda: float, resolution: float,

@@ -17,6 +17,7 @@
 #include "active.cuh"
 #include "geometry.cuh"
 #include "lsf.cuh"
+#include "rv.cuh"
 #include "sia.cuh"
 #include "sia_f32.cuh"
 
@@ -846,6 +847,38 @@ int soap_lower_resolution(soap_star *s, const void *in, int64_t n_rows, int64_t 
         lower_resolution_kernel<double><<<dim3(tiles, gy), kLsfThreads, smem, st>>>(a);
     }
     SOAP_LAUNCH_CHECK(s, "lower_resolution_kernel");
+    return SOAP_OK;
+}
+
+int soap_line_rvs(soap_star *s, const void *rows, int64_t n_rows, int64_t n_pix, int64_t pitch, int32_t dtype, double lambda0,
+                  double dlambda, const double *centres, const double *half_widths, int64_t n_lines, const double *norm,
+                  int64_t edge, double *out_rv, void *stream) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!rows || !centres || !half_widths || !norm || !out_rv) return s->fail(SOAP_ERR_INVALID_ARG, "NULL argument");
+    if (n_rows < 0 || n_lines < 0 || n_pix < 1 || pitch < n_pix || edge < 0) return s->fail(SOAP_ERR_INVALID_ARG, "bad sizes");
+    if (dtype != SOAP_F32 && dtype != SOAP_F64) return s->fail(SOAP_ERR_INVALID_ARG, "unknown dtype %d", dtype);
+    if (!(dlambda > 0.0) || !std::isfinite(dlambda) || !std::isfinite(lambda0)) return s->fail(SOAP_ERR_INVALID_ARG, "bad wavelength grid");
+    if (n_rows == 0 || n_lines == 0) return SOAP_OK;
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    RvArgs a{};
+    a.rows = rows;
+    a.n_rows = n_rows;
+    a.n_pix = n_pix;
+    a.pitch = pitch;
+    a.lambda0 = lambda0;
+    a.k = dlambda;
+    a.centres = centres;
+    a.half_widths = half_widths;
+    a.norm = norm;
+    a.n_lines = n_lines;
+    a.edge = edge;
+    a.rv = out_rv;
+    const unsigned gx = (unsigned)((n_lines + kRvWarps - 1) / kRvWarps);
+    const unsigned gy = (unsigned)std::min<long long>((n_rows + 31) / 32, 65535);  // one warp per (line, 32 rows)
+    if (dtype == SOAP_F32) line_rv_kernel<float><<<dim3(gx, gy), 32 * kRvWarps, 0, st>>>(a);
+    else line_rv_kernel<double><<<dim3(gx, gy), 32 * kRvWarps, 0, st>>>(a);
+    SOAP_LAUNCH_CHECK(s, "line_rv_kernel");
     return SOAP_OK;
 }
 
