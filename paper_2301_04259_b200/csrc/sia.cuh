@@ -6,6 +6,8 @@
 // a_e = D_e - 1 is the entry's Doppler shift factor, so m + delta_e(m) = (lambda_m D_e - lambda_0)/k is
 // the source coordinate of output pixel m; its integer part q and fraction t are closed-form, no search.
 // An entry is a (column, mu-bin) pair with its binned weight (pre-binned form) or a single cell.
+// This generic-precision kernel serves fp64 I/O (config C1); fp32 spectra take the warp-specialised kernel of
+// sia_f32.cuh, the one bench.py measures.
 //
 // Mapping to the SM (sm_100a):
 //   * one CTA = one wavelength tile of kThreads*R pixels x one chunk of the entry list (quiet) or one
