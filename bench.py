@@ -83,7 +83,7 @@ class ClockSampler:
                         self.reasons.add(name)
             except Exception:
                 pass
-            time.sleep(0.004)
+            time.sleep(0.001)
 
     def start(self):
         if self._h is not None:
