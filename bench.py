@@ -364,7 +364,9 @@ def run_graft(args):
     e2e_value = world * n_spec / (e2e_ms / e2e_steps * 1e-3)
     h2d = 3 * wl.n_mu * pitch * 4 + P * 4
     d2h = n_spec * P * 4
-    assert np.array_equal(hQ.numpy(), Q.cpu().numpy()) and np.array_equal(hD.numpy(), D.cpu().numpy())
+    # the host path computes wavelength chunks (different CTA ranges => different fp64 summation order): equal to rounding
+    assert float((hQ.to(dev) - Q).abs().max()) <= 1e-6 * info["sum_weights"]
+    assert float((hD.to(dev) - D).abs().max()) <= 1e-5 * float(D.abs().max())
 
     if rank != 0:
         if world > 1:

@@ -230,8 +230,12 @@ int soap_export_geometry(soap_star *star, double *mu, double *vel, double *w, in
 /* ---- end-to-end convenience with HOST buffers ---------------------------------------------------
  * Same computation as soap_disk_geometry + soap_integrate_quiet + soap_active_timeseries, but every
  * spectra / contrast pointer in quiet / spot / facula, `out_quiet` ([n_pix]) and `out_delta`
- * ([n_phases][n_pix], densely packed) are HOST pointers; the library stages them through device
- * buffers it owns (host->device and device->host copies are part of the call).  Synchronous. */
+ * ([n_phases][n_pix], densely packed) are HOST pointers; the library stages the tables through device
+ * buffers it owns (the copies are part of the call).  Synchronous.  Long fp32 spectra are processed in a
+ * few wavelength chunks so that the upload of one chunk overlaps the kernels of the previous one; when the
+ * outputs are pinned (device-visible) host memory the kernels store straight into them, otherwise they are
+ * staged and copied back chunk by chunk.  Results equal those of the device-resident calls up to the order
+ * of the fp64 partial sums (a few fp32 ulps). */
 int soap_synthesize_host(soap_star *star, const soap_star_params *params, const soap_spectra *quiet,
                          const soap_spectra *spot, const soap_spectra *facula, const soap_region *regions,
                          int32_t n_regions, const double *phases, int32_t n_phases, void *out_quiet,

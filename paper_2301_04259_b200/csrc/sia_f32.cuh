@@ -72,6 +72,10 @@ struct Params {
     const float *base[3];      // spectrum tables per kind (quiet launch: base[0] only)
     const float *contrast[3];  // per-pixel multiplier per kind or nullptr (== 1); kind 0 unused
     long long pitch, n_pix;
+    long long out_lo, out_hi;  // only pixels out_lo <= m < out_hi are stored (0, n_pix; narrower for a window whose margins
+                               // belong to its neighbours, see soap_synthesize_host)
+    long long row_len;         // elements of a row that may be read from its first pixel on (<= pitch; the pitch itself
+                               // unless the table is a window into a wider one, see soap_synthesize_host)
     double c0;                 // lambda0 / dlambda
     int n_mu;
     int halo;                  // H: multiple of 4, >= max |delta| + 2
@@ -447,7 +451,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             if (lane == 0) {
                 if (jb.count > 0) {
                     const long long g_lo = s_start < 0 ? 0 : s_start;
-                    const long long g_hi = (s_start + span) < p.pitch ? (s_start + span) : p.pitch;
+                    const long long g_hi = (s_start + span) < p.row_len ? (s_start + span) : p.row_len;
                     const uint32_t row_bytes = (uint32_t)((g_hi - g_lo) * (long long)sizeof(float));
                     const float *src_row = p.base[jb.kind] + (long long)jb.row * p.pitch + g_lo;
                     const uint32_t ent_bytes = (uint32_t)(((jb.count + 1) & ~1) * (int)sizeof(float2));
@@ -559,7 +563,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             }
             cnt = 0;
             if (ACTIVE) {
-                const long long rem = p.n_pix - (m_t0 + tid);
+                const long long rem = p.out_hi - (m_t0 + tid);
                 rmax = rem <= 0 ? 0 : (int)min((long long)kR, (rem + kConsumers - 1) / kConsumers);
                 fin_valid = false;  // only this thread ever touches its 16 slots of `fin` and `cst`
                 cur_kind = kind;
@@ -635,7 +639,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
 #pragma unroll
                 for (int r = 0; r < kR; ++r) {
                     const double f = fin_valid ? fin[r * kConsumers + tid] : 0.0;
-                    if (r < rmax) o[kConsumers * r] = (float)(tot[r] + f);
+                    if (r < rmax && m_t0 + tid + kConsumers * r >= p.out_lo) o[kConsumers * r] = (float)(tot[r] + f);
                 }
             } else {
                 double *o = p.partial + ((long long)blockIdx.x * p.max_seg + out_idx) * kTile;
@@ -684,7 +688,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                     float *qo = p.out + m_t0 + tid;
 #pragma unroll
                     for (int r = 0; r < kR; ++r)
-                        if (m_t0 + tid + kConsumers * r < p.n_pix) qo[kConsumers * r] = (float)sum[r];
+                        if (m_t0 + tid + kConsumers * r < p.out_hi && m_t0 + tid + kConsumers * r >= p.out_lo)
+                            qo[kConsumers * r] = (float)sum[r];
                 }
                 consumer_bar_sync();  // tile_ctl may be rewritten by the next tile
             }

@@ -61,6 +61,12 @@ struct soap_star {
     double sini = 1.0, cosi = 0.0;
     double amax = 0.0;  // host bound on max |D - 1|
     int form = SOAP_FORM_AUTO, form_used = SOAP_FORM_BINNED;
+    long long out_lo_override = -1, out_hi_override = -1;  // soap_synthesize_host: pixels of a window that are stored
+    long long clip_override = 0;    // soap_synthesize_host: readable row length of a window into a wider table (0 = pitch)
+    bool reuse_lists = false;       // soap_synthesize_host: the active map of the previous call is still valid
+    bool regions_uploaded = false;  // soap_synthesize_host: the region centres are already on the device
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    std::vector<cudaEvent_t> ev_pipe;
     long long active_pool_cap = 0;  // per-cell active form: entries one phase's pool must hold (from the region radii)
     bool cell_entries = false;  // one entry per cell (SOAP_FORM_CELLS, or differential rotation) instead of per (column, mu-bin)
     int opt_quiet_splits = 0;
@@ -218,6 +224,9 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     f32::Params p{};
     p.base[0] = static_cast<const float *>(q->data);
     p.pitch = q->pitch;
+    p.row_len = s->clip_override > 0 ? s->clip_override : q->pitch;
+    p.out_lo = s->out_lo_override >= 0 ? s->out_lo_override : 0;
+    p.out_hi = s->out_hi_override >= 0 ? s->out_hi_override : P;
     p.n_pix = P;
     p.c0 = q->lambda0 / q->dlambda;
     p.n_mu = s->prm.n_mu;
@@ -409,6 +418,9 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         p.contrast[1] = (spot && use_contrast) ? static_cast<const float *>(spot->contrast) : nullptr;
         p.contrast[2] = (fac && use_contrast) ? static_cast<const float *>(fac->contrast) : nullptr;
         p.pitch = q->pitch;
+        p.row_len = s->clip_override > 0 ? s->clip_override : q->pitch;
+        p.out_lo = s->out_lo_override >= 0 ? s->out_lo_override : 0;
+        p.out_hi = s->out_hi_override >= 0 ? s->out_hi_override : q->n_pix;
         p.n_pix = q->n_pix;
         p.c0 = q->lambda0 / q->dlambda;
         p.n_mu = n_mu;
@@ -544,6 +556,137 @@ int upload_region_centres(soap_star *s, const soap_region *regions, int n_region
     return SOAP_OK;
 }
 
+
+// soap_synthesize_host for long fp32 spectra: the wavelength axis is cut into chunks of whole tiles, and the upload of
+// chunk c+1, the kernels of chunk c and the download of chunk c-1 overlap on three streams (every output pixel depends
+// only on source pixels within the halo, so a chunk is the same computation on a window [m0 - Hc, m1 + Hc) of the
+// tables; only its interior [m0, m1) is kept).  The PCIe copies, not the kernels, bound this entry point.
+int synthesize_host_pipelined(soap_star *s, const soap_star_params *prm, const soap_spectra *quiet, const soap_spectra *spot,
+                              const soap_spectra *facula, const soap_region *regions, int32_t n_regions, const double *phases,
+                              int32_t n_phases, void *out_quiet, void *out_delta, int32_t *n_active, cudaStream_t st) {
+    const soap_spectra *in[3] = {quiet, spot, facula};
+    const long long P = quiet->n_pix, pitch = quiet->pitch;
+    for (int k = 1; k < 3; ++k) {
+        if (!in[k]) continue;
+        if (!in[k]->data || in[k]->n_pix != P || in[k]->pitch != pitch || in[k]->dtype != SOAP_F32)
+            return s->fail(SOAP_ERR_INVALID_ARG, "spectra %d: data / n_pix / pitch / dtype differ from quiet", k);
+    }
+    int rc = soap_disk_geometry(s, prm, st, nullptr);
+    if (rc) return rc;
+    // the (small) region upload goes first: copies of one direction are served in issue order, and behind the table
+    // uploads it would hold back the first chunk's kernels until every table has arrived
+    if ((rc = check_regions(s, regions, n_regions, phases, n_phases, spot, facula))) return rc;
+    if ((rc = upload_region_centres(s, regions, n_regions, phases, n_phases, nullptr, st))) return rc;
+    if (!s->s_h2d) SOAP_CUDA(s, cudaStreamCreateWithFlags(&s->s_h2d, cudaStreamNonBlocking));
+    if (!s->s_d2h) SOAP_CUDA(s, cudaStreamCreateWithFlags(&s->s_d2h, cudaStreamNonBlocking));
+    const long long tiles = (P + f32::kTile - 1) / f32::kTile;
+    const int K = (int)std::max(1LL, std::min(4LL, tiles / 32));  // measured: 3-4 chunks are best, more only add copies
+    const long long Lc = ((tiles + K - 1) / K) * f32::kTile;  // chunk length: whole tiles
+    const long long Hc = halo_for(s, quiet) + 4;              // halo of the whole spectrum (a multiple of 4)
+    while ((int)s->ev_pipe.size() < 1 + 3 * K) {
+        cudaEvent_t e;
+        SOAP_CUDA(s, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        s->ev_pipe.push_back(e);
+    }
+    cudaEvent_t ev_start = s->ev_pipe[0];
+    auto ev_up = [&](int c) { return s->ev_pipe[1 + c]; };
+    auto ev_done = [&](int c) { return s->ev_pipe[1 + K + c]; };
+    auto ev_out = [&](int c) { return s->ev_pipe[1 + 2 * K + c]; };
+    for (int k = 0; k < 3; ++k) {
+        if (!in[k]) continue;
+        SOAP_CUDA(s, s->d_stage[k].reserve((size_t)prm->n_mu * pitch * 4));
+        if (k > 0 && in[k]->contrast) SOAP_CUDA(s, s->d_stage_c[k].reserve((size_t)P * 4));
+    }
+    // Results go straight to the caller's arrays when those are pinned (device-visible) host memory: the kernels' stores
+    // cross PCIe while the next chunk's tables come in, and no device-to-host copy is queued at all.  Pageable outputs are
+    // staged in device memory and copied back chunk by chunk.
+    float *dq = nullptr, *dd = nullptr;
+    {
+        cudaPointerAttributes aq{}, ad{};
+        const bool okq = cudaPointerGetAttributes(&aq, out_quiet) == cudaSuccess && aq.type == cudaMemoryTypeHost && aq.devicePointer;
+        const bool okd = cudaPointerGetAttributes(&ad, out_delta) == cudaSuccess && ad.type == cudaMemoryTypeHost && ad.devicePointer;
+        cudaGetLastError();  // a pageable pointer is reported as an error by older runtimes: not ours to keep
+        if (okq && okd) {
+            dq = static_cast<float *>(aq.devicePointer);
+            dd = static_cast<float *>(ad.devicePointer);
+        }
+    }
+    const bool zero_copy = dq != nullptr;
+    if (!zero_copy) {
+        SOAP_CUDA(s, s->d_out_q.reserve((size_t)P * 4));
+        SOAP_CUDA(s, s->d_out_d.reserve((size_t)n_phases * P * 4));
+        dq = reinterpret_cast<float *>(s->d_out_q.ptr);
+        dd = reinterpret_cast<float *>(s->d_out_d.ptr);
+    }
+    // the copy streams start after whatever the caller's stream holds so far (buffers of an earlier call may be in use)
+    SOAP_CUDA(s, cudaEventRecord(ev_start, st));
+    SOAP_CUDA(s, cudaStreamWaitEvent(s->s_h2d, ev_start, 0));
+    SOAP_CUDA(s, cudaStreamWaitEvent(s->s_d2h, ev_start, 0));
+    // uploads: a partition of the columns, chunk c carrying [m0 + Hc, m1 + Hc) (the first from 0, the last up to P)
+    for (int c = 0; c < K; ++c) {
+        const long long m0 = c * Lc, m1 = std::min(P, m0 + Lc);
+        const long long u0 = c == 0 ? 0 : std::min(P, m0 + Hc), u1 = c == K - 1 ? P : std::min(P, m1 + Hc);
+        if (u1 > u0) {
+            for (int k = 0; k < 3; ++k) {
+                if (!in[k]) continue;
+                SOAP_CUDA(s, cudaMemcpy2DAsync(reinterpret_cast<float *>(s->d_stage[k].ptr) + u0, (size_t)pitch * 4,
+                                               static_cast<const float *>(in[k]->data) + u0, (size_t)pitch * 4, (size_t)(u1 - u0) * 4,
+                                               (size_t)prm->n_mu, cudaMemcpyHostToDevice, s->s_h2d));
+                if (k > 0 && in[k]->contrast)
+                    SOAP_CUDA(s, cudaMemcpyAsync(reinterpret_cast<float *>(s->d_stage_c[k].ptr) + u0,
+                                                 static_cast<const float *>(in[k]->contrast) + u0, (size_t)(u1 - u0) * 4,
+                                                 cudaMemcpyHostToDevice, s->s_h2d));
+            }
+        }
+        SOAP_CUDA(s, cudaEventRecord(ev_up(c), s->s_h2d));
+    }
+    for (int c = 0; c < K; ++c) {
+        const long long m0 = c * Lc, m1 = std::min(P, m0 + Lc);
+        if (m1 <= m0) {
+            SOAP_CUDA(s, cudaEventRecord(ev_out(c), s->s_d2h));
+            continue;
+        }
+        const long long v0 = std::max(0LL, m0 - Hc), v1 = std::min(P, m1 + Hc);  // the window this chunk computes on
+        soap_spectra dev[3];
+        for (int k = 0; k < 3; ++k) {
+            if (!in[k]) continue;
+            dev[k] = *in[k];
+            dev[k].data = reinterpret_cast<float *>(s->d_stage[k].ptr) + v0;
+            dev[k].n_pix = v1 - v0;
+            dev[k].lambda0 = in[k]->lambda0 + (double)v0 * in[k]->dlambda;
+            dev[k].contrast = (k > 0 && in[k]->contrast) ? reinterpret_cast<float *>(s->d_stage_c[k].ptr) + v0 : nullptr;
+        }
+        SOAP_CUDA(s, cudaStreamWaitEvent(st, ev_up(c), 0));
+        s->clip_override = pitch - v0;
+        s->out_lo_override = m0 - v0;  // the window's margins belong to the neighbouring chunks
+        s->out_hi_override = m1 - v0;
+        rc = soap_integrate_quiet(s, &dev[0], dq + v0, st);
+        if (!rc) {
+            s->reuse_lists = c > 0;  // the active map does not depend on the wavelength window
+            s->regions_uploaded = true;
+            rc = soap_active_timeseries(s, &dev[0], spot ? &dev[1] : nullptr, facula ? &dev[2] : nullptr, regions, n_regions, phases,
+                                        n_phases, dd + v0, P, nullptr, st);
+        }
+        s->clip_override = 0;
+        s->out_lo_override = s->out_hi_override = -1;
+        s->reuse_lists = false;
+        s->regions_uploaded = false;
+        if (rc) return rc;
+        SOAP_CUDA(s, cudaEventRecord(ev_done(c), st));
+        if (!zero_copy) {
+            SOAP_CUDA(s, cudaStreamWaitEvent(s->s_d2h, ev_done(c), 0));
+            SOAP_CUDA(s, cudaMemcpyAsync(static_cast<float *>(out_quiet) + m0, dq + m0, (size_t)(m1 - m0) * 4, cudaMemcpyDeviceToHost, s->s_d2h));
+            SOAP_CUDA(s, cudaMemcpy2DAsync(static_cast<float *>(out_delta) + m0, (size_t)P * 4, dd + m0, (size_t)P * 4,
+                                           (size_t)(m1 - m0) * 4, (size_t)n_phases, cudaMemcpyDeviceToHost, s->s_d2h));
+        }
+        SOAP_CUDA(s, cudaEventRecord(ev_out(c), s->s_d2h));
+    }
+    if (!zero_copy)
+        for (int c = 0; c < K; ++c) SOAP_CUDA(s, cudaStreamWaitEvent(st, ev_out(c), 0));
+    if (n_active) SOAP_CUDA(s, cudaMemcpyAsync(n_active, s->d_nactive.ptr, (size_t)n_phases * sizeof(int), cudaMemcpyDeviceToHost, st));
+    SOAP_CUDA(s, cudaStreamSynchronize(st));
+    return SOAP_OK;
+}
 }  // namespace
 
 extern "C" {
@@ -592,6 +735,9 @@ int soap_destroy(soap_star *s) {
     s->d_out_q.release(); s->d_out_d.release();
     for (auto &e : s->ev)
         if (e) cudaEventDestroy(e);
+    for (auto &e : s->ev_pipe) cudaEventDestroy(e);
+    if (s->s_h2d) cudaStreamDestroy(s->s_h2d);
+    if (s->s_d2h) cudaStreamDestroy(s->s_d2h);
     for (auto &slot : s->h_rp) {
         if (slot.ptr) cudaFreeHost(slot.ptr);
         if (slot.done) cudaEventDestroy(slot.done);
@@ -737,13 +883,14 @@ int soap_active_timeseries_evolving(soap_star *s, const soap_spectra *quiet, con
     if (out_pitch < quiet->n_pix) return s->fail(SOAP_ERR_INVALID_ARG, "out_pitch must be >= n_pix");
     SOAP_CUDA(s, cudaSetDevice(s->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if ((rc = upload_region_centres(s, regions, n_regions, phases, n_phases, radii, st))) return rc;
+    if (!s->reuse_lists && !s->regions_uploaded && (rc = upload_region_centres(s, regions, n_regions, phases, n_phases, radii, st)))
+        return rc;
     // total and flux-only share the entry lists (weights w LB_t(mu)); CB-only needs the plain weights w, which
     // are the same lists again when both limb-brightening laws are identically 1
     const bool lb_is_one = (!spot || (spot->lb_c0 == 1.0 && spot->lb_c1 == 0.0 && spot->lb_c2 == 0.0)) &&
                            (!facula || (facula->lb_c0 == 1.0 && facula->lb_c1 == 0.0 && facula->lb_c2 == 0.0));
     struct Pass { int effect; void *out; } passes[3] = {{SOAP_EFFECT_TOTAL, out_total}, {SOAP_EFFECT_FLUX, out_flux}, {SOAP_EFFECT_CB, out_cb}};
-    bool have_lb_lists = false;
+    bool have_lb_lists = s->reuse_lists;
     for (const Pass &ps : passes) {
         if (!ps.out) continue;
         const bool prepare = ps.effect == SOAP_EFFECT_CB ? !(have_lb_lists && lb_is_one) : !have_lb_lists;
@@ -935,6 +1082,10 @@ int soap_synthesize_host(soap_star *s, const soap_star_params *prm, const soap_s
     if (n_phases > 0 && !out_delta) return s->fail(SOAP_ERR_INVALID_ARG, "out_delta is NULL");
     SOAP_CUDA(s, cudaSetDevice(s->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (prm && quiet->dtype == SOAP_F32 && n_phases > 0 && quiet->n_pix >= 16LL * f32::kTile && prm->n_mu >= 1 &&
+        prm->n_mu <= SOAP_MAX_MU && quiet->pitch >= quiet->n_pix && !(quiet->pitch & 3))
+        return synthesize_host_pipelined(s, prm, quiet, spot, facula, regions, n_regions, phases, n_phases, out_quiet, out_delta,
+                                         n_active, st);
     const soap_spectra *in[3] = {quiet, spot, facula};
     soap_spectra dev[3];
     const size_t esz = quiet->dtype == SOAP_F64 ? 8 : 4;
