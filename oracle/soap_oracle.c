@@ -16,6 +16,12 @@
  *              so that S_final = S_quiet,integrated + delta (Eq. 4 P:83 with the sign flipped)
  *   mu bins    "closest mu" P:332
  *   contrast   per-pixel I_ratio applied after the shift, LB(mu) per cell
+ *   effects    flux-only / CB-only differences, Eq. 1-2 P:73-77 (soap_oracle_active_effect)
+ *   diff. rot. omega = omega_0 + omega_1 sin^2(latitude) P:250-252 (oracle_star.diff_rot = omega_1 / omega_0)
+ *   resolution "lower the resolution of the final spectrum" P:85, Alg. 5: Gaussian LSF of FWHM lambda / R
+ *              (reading R-LSF; soap_oracle_lower_resolution)
+ *   line RV    first-moment RV per line, BASELINE.json north_star's acceptance functional standing in for
+ *              the CCF fit of P:270 (soap_oracle_line_rvs)
  *
  * No blocking, fusion or reordering: per output pixel the cells are summed in (j, i) order exactly
  * as the double loop of Alg. 1 would.  OpenMP only splits the *wavelength* axis into chunks, which
@@ -26,7 +32,8 @@
  * load this library.
  *
  * Parity status: pinned against closed forms / invariants / brute force (tests/test_oracle_pins.py,
- * pins P1-P10 of DESIGN.md); "parity against values printed in the paper": unpinned - the paper
+ * pins P1-P10 of DESIGN.md; tests/test_oracle_effects.py, test_oracle_diffrot.py, test_oracle_lsf.py,
+ * test_oracle_rv.py for the additions); "parity against values printed in the paper": unpinned - the paper
  * prints no numeric output for this path.
  *
  * Cell indexing everywhere: c = j * N + i, j = column (x) index, i = row (y) index,
