@@ -423,6 +423,9 @@ def run_configs(args):
             wls = [shared] + [workloads.make_config5_star(k, shared=shared) for k in range(1, 64)]
         else:
             wls = [{"C2": workloads.make_config2, "C3": workloads.make_config3, "C4": workloads.make_config4}[name]()]
+        if args.vsini is not None:
+            for w in wls:
+                w.vsini_kms = args.vsini
         w0 = wls[0]
         P, n_ph = w0.n_pix, len(w0.phases)
         q = soap.to_device_spectra(w0.quiet, w0.lambda0, w0.dlambda, dev)
@@ -459,7 +462,7 @@ def run_configs(args):
         soap.soap_active_timeseries(stars[0], q, sp, fa, wls[0].regions, wls[0].phases, D[0])
         st = soap.soap_get_stats(stars[0])
         n_spec = len(wls) * (1 + n_ph)
-        line = {"workload": workloads.CONFIG_NAMES[int(name[1])], "stars": len(wls), "ms_per_step": ms,
+        line = {"workload": workloads.CONFIG_NAMES[int(name[1])], "vsini_kms": float(w0.vsini_kms), "stars": len(wls), "ms_per_step": ms,
                 "spectra_per_s": n_spec / (ms * 1e-3), "first_star": {
                     "quiet_entries": st["quiet_entries"], "active_entries": st["active_entries"],
                     "quiet_kernel_ms": st["quiet_kernel_ms"], "active_kernel_ms": st["active_kernel_ms"],
@@ -479,10 +482,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["graft", "reference"], default="graft")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--vsini", type=float, default=None, help="with --workload: override v sin i (km/s) of every star")
     ap.add_argument("--workload", choices=["C3", "C2", "C4", "C5", "all"], default="C3",
                     help="C3 (default) is the bench contract; the others print per-config timing lines only")
     args = ap.parse_args()
-    if args.impl != "reference" and args.workload != "C3":
+    if args.impl != "reference" and (args.workload != "C3" or args.vsini is not None):
         run_configs(args)
     elif args.impl == "reference":
         run_reference(args)
