@@ -436,10 +436,16 @@ def run_configs(args):
         D = torch.empty((len(wls), n_ph, P), dtype=torch.float32, device=dev)
 
         def step():
-            for k, (st, wl) in enumerate(zip(stars, wls)):
+            if len(wls) == 1:
+                soap.soap_disk_geometry(stars[0], wls[0], want_info=False)
+                soap.soap_integrate_quiet(stars[0], q, Q[0])
+                soap.soap_active_timeseries(stars[0], q, sp, fa, wls[0].regions, wls[0].phases, D[0])
+                return
+            for st, wl in zip(stars, wls):  # config 5: the batch entry points (three lanes, one stream to the caller)
                 soap.soap_disk_geometry(st, wl, want_info=False)
-                soap.soap_integrate_quiet(st, q, Q[k])
-                soap.soap_active_timeseries(st, q, sp, fa, wl.regions, wl.phases, D[k])
+            soap.soap_batch_integrate_quiet(stars, [q] * len(wls), [Q[k] for k in range(len(wls))])
+            soap.soap_batch_active_timeseries(stars, [q] * len(wls), [sp] * len(wls), [fa] * len(wls), [w.regions for w in wls],
+                                              [w.phases for w in wls], [D[k] for k in range(len(wls))])
 
         for _ in range(3):
             step()

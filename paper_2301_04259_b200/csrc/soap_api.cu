@@ -1128,15 +1128,48 @@ int soap_synthesize_host(soap_star *s, const soap_star_params *prm, const soap_s
     return SOAP_OK;
 }
 
+// Batch entry points (config 5): the stars are independent, so their work is dealt round-robin to three lanes - the
+// caller's stream and two side streams of the first handle, forked from and joined back into the caller's stream with
+// events.  Each star's big kernels fill the GPU on their own; what overlaps is the tail of one star's kernel with the
+// start of the next star's, and the small kernels (active map) of one star with the big kernels of another.
+static int batch_fork(soap_star *s0, cudaStream_t st, cudaStream_t lanes[3]) {
+    SOAP_CUDA(s0, cudaSetDevice(s0->device));
+    if (!s0->s_h2d) SOAP_CUDA(s0, cudaStreamCreateWithFlags(&s0->s_h2d, cudaStreamNonBlocking));
+    if (!s0->s_d2h) SOAP_CUDA(s0, cudaStreamCreateWithFlags(&s0->s_d2h, cudaStreamNonBlocking));
+    while (s0->ev_pipe.size() < 3) {
+        cudaEvent_t e;
+        SOAP_CUDA(s0, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        s0->ev_pipe.push_back(e);
+    }
+    lanes[0] = st;
+    lanes[1] = s0->s_h2d;
+    lanes[2] = s0->s_d2h;
+    SOAP_CUDA(s0, cudaEventRecord(s0->ev_pipe[0], st));
+    SOAP_CUDA(s0, cudaStreamWaitEvent(lanes[1], s0->ev_pipe[0], 0));
+    SOAP_CUDA(s0, cudaStreamWaitEvent(lanes[2], s0->ev_pipe[0], 0));
+    return SOAP_OK;
+}
+static int batch_join(soap_star *s0, cudaStream_t st, cudaStream_t lanes[3]) {
+    for (int l = 1; l < 3; ++l) {
+        SOAP_CUDA(s0, cudaEventRecord(s0->ev_pipe[l], lanes[l]));
+        SOAP_CUDA(s0, cudaStreamWaitEvent(st, s0->ev_pipe[l], 0));
+    }
+    return SOAP_OK;
+}
+
 int soap_batch_integrate_quiet(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet, void *const *out,
                                void *stream) {
     if (!stars || !quiet || !out || n_stars < 0) return SOAP_ERR_INVALID_ARG;
-    for (int k = 0; k < n_stars; ++k) {
+    for (int k = 0; k < n_stars; ++k)
         if (!stars[k]) return SOAP_ERR_INVALID_ARG;
-        int rc = soap_integrate_quiet(stars[k], quiet[k], out[k], stream);
-        if (rc) return rc;
-    }
-    return SOAP_OK;
+    if (n_stars == 0) return SOAP_OK;
+    cudaStream_t lanes[3];
+    int rc = batch_fork(stars[0], static_cast<cudaStream_t>(stream), lanes);
+    if (rc) return rc;
+    int first_error = SOAP_OK;
+    for (int k = 0; k < n_stars && !first_error; ++k) first_error = soap_integrate_quiet(stars[k], quiet[k], out[k], lanes[k % 3]);
+    rc = batch_join(stars[0], static_cast<cudaStream_t>(stream), lanes);  // joined even after an error: no dangling lane
+    return first_error ? first_error : rc;
 }
 
 int soap_batch_active_timeseries(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet,
@@ -1145,13 +1178,18 @@ int soap_batch_active_timeseries(soap_star *const *stars, int32_t n_stars, const
                                  const int32_t *n_phases, void *const *out_delta, const int64_t *out_pitch, void *stream) {
     if (!stars || !quiet || !regions || !n_regions || !phases || !n_phases || !out_delta || !out_pitch || n_stars < 0)
         return SOAP_ERR_INVALID_ARG;
-    for (int k = 0; k < n_stars; ++k) {
+    for (int k = 0; k < n_stars; ++k)
         if (!stars[k]) return SOAP_ERR_INVALID_ARG;
-        int rc = soap_active_timeseries(stars[k], quiet[k], spot ? spot[k] : nullptr, facula ? facula[k] : nullptr, regions[k],
-                                        n_regions[k], phases[k], n_phases[k], out_delta[k], out_pitch[k], nullptr, stream);
-        if (rc) return rc;
-    }
-    return SOAP_OK;
+    if (n_stars == 0) return SOAP_OK;
+    cudaStream_t lanes[3];
+    int rc = batch_fork(stars[0], static_cast<cudaStream_t>(stream), lanes);
+    if (rc) return rc;
+    int first_error = SOAP_OK;
+    for (int k = 0; k < n_stars && !first_error; ++k)
+        first_error = soap_active_timeseries(stars[k], quiet[k], spot ? spot[k] : nullptr, facula ? facula[k] : nullptr, regions[k],
+                                             n_regions[k], phases[k], n_phases[k], out_delta[k], out_pitch[k], nullptr, lanes[k % 3]);
+    rc = batch_join(stars[0], static_cast<cudaStream_t>(stream), lanes);
+    return first_error ? first_error : rc;
 }
 
 }  // extern "C"
