@@ -508,10 +508,13 @@ active_prepare_cells_kernel(const PrepArgs a) {
         int pos = incl - mine;
         for (int ss = ss0; ss < ss1; ++ss) {
             const int s = (ss + a.n_mu) % n_seg;
-            base[s] = pos;
+            // packed back to back (fp32 kernel: jobs carry their own positions), or - seg_cap > 0 - one fixed slot of
+            // seg_cap entries per segment, the layout the generic-precision kernel reads with seg_count
+            base[s] = a.seg_cap > 0 ? s * a.seg_cap : pos;
             pos += (tot[s] + 1) & ~1;
+            if (a.seg_cap > 0 && tot[s] + 1 > a.seg_cap) a.counters->overflow = 1;
         }
-        if (lane == 31 && incl > a.pool_cap) a.counters->overflow = 1;
+        if (lane == 31 && a.seg_cap == 0 && incl > a.pool_cap) a.counters->overflow = 1;
     }
     __syncthreads();
     for (int s = tid; s < n_seg; s += kPrepThreads) off[s] += base[s];

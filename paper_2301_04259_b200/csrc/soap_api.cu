@@ -335,17 +335,18 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
     SOAP_CUDA(s, s->d_sched.reserve((size_t)3 * n_phases));
     int *d_njobs = s->d_sched.ptr, *d_order = d_njobs + n_phases, *d_work = d_order + n_phases;
     const bool per_cell = s->prm.diff_rot != 0.0;  // the cells of a column no longer share a velocity (R-DR)
-    if (per_cell && sizeof(T) != 4)
-        return s->fail(SOAP_ERR_UNSUPPORTED, "differential rotation: the active time series is implemented for fp32 spectra only");
+    // fp64 I/O under differential rotation: the generic kernel reads fixed slots of seg_cap entries per segment, so every
+    // segment gets room for all the covered cells of a phase (fp64 is the small-configuration path)
+    const long long cell_seg_cap = (per_cell && sizeof(T) != 4) ? ((s->active_pool_cap / 2 + 2) & ~1LL) : 0;
     if (per_cell && prepare) {
-        const long long pool = s->active_pool_cap;
+        const long long pool = cell_seg_cap > 0 ? cell_seg_cap * 3 * n_mu : s->active_pool_cap;
         if ((long long)n_phases * pool >= (1LL << 31)) return s->fail(SOAP_ERR_UNSUPPORTED, "n_phases * entries per phase too large for one call");
         SOAP_CUDA(s, s->d_aent.reserve((size_t)n_phases * pool * sizeof(Ent) + 64));
         PrepArgs a{};
         a.N = N;
         a.n_regions = n_regions;
         a.n_mu = n_mu;
-        a.seg_cap = 0;
+        a.seg_cap = (int)cell_seg_cap;
         a.n_phases = n_phases;
         a.pool_cap = (int)pool;
         a.job_cap = 3 * n_mu + (int)(pool / kActiveJobCap) + 2;
@@ -365,7 +366,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         if (use_lb && spot) { a.lb.c[1][0] = spot->lb_c0; a.lb.c[1][1] = spot->lb_c1; a.lb.c[1][2] = spot->lb_c2; }
         if (use_lb && fac) { a.lb.c[2][0] = fac->lb_c0; a.lb.c[2][1] = fac->lb_c1; a.lb.c[2][2] = fac->lb_c2; }
         a.ent = s->d_aent.ptr;
-        a.seg_count = nullptr;
+        a.seg_count = cell_seg_cap > 0 ? s->d_segcnt.ptr : nullptr;
         a.n_active = s->d_nactive.ptr;
         a.jobs = s->d_jobs.ptr;
         a.n_jobs = d_njobs;
@@ -462,7 +463,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
     p.halo = halo_for(s, q);
     p.ent = reinterpret_cast<const Ent *>(s->d_aent.ptr);
     p.seg_count = s->d_segcnt.ptr;
-    p.seg_cap = ncap;
+    p.seg_cap = per_cell ? (int)cell_seg_cap : ncap;
     p.out = static_cast<T *>(out);
     p.out_pitch = out_pitch;
     const int n_tiles = (int)((q->n_pix + TP - 1) / TP);

@@ -76,7 +76,7 @@ def test_diffrot_full_size_config3_sampled(soap):
         assert_parity(wl, g, lo, hi)
 
 
-def test_diffrot_rejects_binned_form_and_fp64_active(soap):
+def test_diffrot_rejects_binned_form_and_runs_fp64(soap):
     wl = workloads.make_config1()
     wl.diff_rot = -0.18
     star = soap.soap_create(0)
@@ -84,18 +84,11 @@ def test_diffrot_rejects_binned_form_and_fp64_active(soap):
     with pytest.raises(soap.SoapError) as e:
         soap.soap_disk_geometry(star, wl)
     assert e.value.code == soap.binding.SOAP_ERR_UNSUPPORTED
-    soap.soap_set_option(star, soap.binding.SOAP_OPT_FORM, 0)
-    soap.soap_disk_geometry(star, wl)
-    dev = torch.device("cuda:0")
-    q = soap.to_device_spectra(wl.quiet, wl.lambda0, wl.dlambda, dev)
-    s = soap.to_device_spectra(wl.spot, wl.lambda0, wl.dlambda, dev, wl.spot_contrast, wl.spot_lb)
-    Q = torch.empty(wl.n_pix, dtype=torch.float64, device=dev)
-    soap.soap_integrate_quiet(star, q, Q)                       # fp64 quiet works through the generic kernel
-    torch.cuda.synchronize()
-    Qo = oracle.quiet(wl, wl.quiet, wl.lambda0, wl.dlambda)
-    assert np.max(np.abs(Q.cpu().numpy() - Qo)) <= 1e-9 * oracle.geometry(wl)["sum_w"]
-    D = torch.empty((len(wl.phases), wl.n_pix), dtype=torch.float64, device=dev)
-    with pytest.raises(soap.SoapError) as e:
-        soap.soap_active_timeseries(star, q, s, None, wl.regions, wl.phases, D)
-    assert e.value.code == soap.binding.SOAP_ERR_UNSUPPORTED
     soap.soap_destroy(star)
+    g = run_gpu(soap, wl)                                        # fp64 I/O: generic kernel, fixed-slot per-cell entries
+    Qo, Do, nao = oracle.run_workload(wl)
+    sw = oracle.geometry(wl)["sum_w"]
+    assert np.max(np.abs(g["Q"] - Qo)) <= 1e-9 * sw
+    assert np.array_equal(g["n_active"], nao) and nao.max() > 0
+    assert np.max(np.abs(g["D"] - Do)) <= 1e-9 * np.max(np.abs(Do))
+    assert_parity(wl, g)
