@@ -181,6 +181,8 @@ def run_graft(args):
     Q = torch.empty(P, dtype=torch.float32, device=dev)
     D = torch.empty((n_ph, P), dtype=torch.float32, device=dev)
     star = soap.soap_create(local_rank)
+    if args.form is not None:
+        soap.soap_set_option(star, soap.binding.SOAP_OPT_FORM, args.form)
     flush_buf = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
     def step():
@@ -383,7 +385,7 @@ def run_graft(args):
         "data": "synthetic",
         "config": {"workload": "C3 full visible range (BASELINE.json configs[2]): N=300, vsini=2 km/s, i=90, 310000 px 3800-6900 A, "
                                "20 mu bins x {quiet,spot,facula}, 25000 lines, 3% facula + 1% spot, 25 phases, fp32",
-                   "stars_per_gpu": 1, "spectra_per_step": n_spec, "form": {1: "binned", 2: "cells", 3: "fir"}[stats["form"]],
+                   "stars_per_gpu": 1, "spectra_per_step": n_spec, "form": {1: "binned", 2: "cells", 3: "fir", 4: "composite"}[stats["form"]],
                    "l2": "512 MB buffer written before every timed step (inputs+outputs 106 MB < 126 MB L2)",
                    "timing": "sum of per-step CUDA-event intervals, max over ranks", "sharding": "independent stars per rank, no collective"},
         "cell_pixel_interps_per_s": world * eff_interps / (ms_per_step * 1e-3),
@@ -432,6 +434,9 @@ def run_configs(args):
         sp = soap.to_device_spectra(w0.spot, w0.lambda0, w0.dlambda, dev, w0.spot_contrast, w0.spot_lb)
         fa = None if w0.facula is None else soap.to_device_spectra(w0.facula, w0.lambda0, w0.dlambda, dev, w0.facula_contrast, w0.facula_lb)
         stars = [soap.soap_create(dev.index) for _ in wls]
+        if args.form is not None:
+            for st_ in stars:
+                soap.soap_set_option(st_, soap.binding.SOAP_OPT_FORM, args.form)
         Q = torch.empty((len(wls), P), dtype=torch.float32, device=dev)
         D = torch.empty((len(wls), n_ph, P), dtype=torch.float32, device=dev)
 
@@ -488,6 +493,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["graft", "reference"], default="graft")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--form", type=int, default=None, help="SOAP_OPT_FORM of the timed star (default: the library's AUTO)")
     ap.add_argument("--vsini", type=float, default=None, help="with --workload: override v sin i (km/s) of every star")
     ap.add_argument("--workload", choices=["C3", "C2", "C4", "C5", "all"], default="C3",
                     help="C3 (default) is the bench contract; the others print per-config timing lines only")

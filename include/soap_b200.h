@@ -66,9 +66,14 @@ enum soap_form {
     SOAP_FORM_BINNED = 1, /* cells pre-binned by (column, mu-bin): all cells of a column share one
                              velocity under solid-body rotation (BASELINE.json north_star) */
     SOAP_FORM_CELLS = 2,  /* one entry per visible cell - the literal double loop of Alg. 1 */
-    SOAP_FORM_FIR = 3     /* binned (or, under differential rotation, per-cell) entries; per wavelength tile every
+    SOAP_FORM_FIR = 3,    /* binned (or, under differential rotation, per-cell) entries; per wavelength tile every
                              run of entries of one spectrum row with the same integer shift is collapsed into one
                              record {sum W, sum W a}: taps linear in the pixel index (exact in exact arithmetic) */
+    SOAP_FORM_COMPOSITE = 4 /* binned weights; quiet spectrum: per column j the composite T_j = sum_b W[j,b] S_b is formed
+                             from unshifted samples (1 FMA per (column, mu-bin, pixel)) and interpolated once per
+                             (column, pixel) - lerp is linear in the spectrum and the cells of a column share one
+                             velocity.  Cost independent of v sin i.  fp32 spectra, solid body, n_mu <= 24; otherwise
+                             (and for the active delta spectra) the binned entries are used */
 };
 
 enum soap_option {

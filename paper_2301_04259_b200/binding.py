@@ -22,7 +22,7 @@ SOAP_OK = 0
 SOAP_ERR_INVALID_ARG, SOAP_ERR_NOT_READY, SOAP_ERR_CUDA, SOAP_ERR_OOM, SOAP_ERR_UNSUPPORTED = -1, -2, -3, -4, -5
 SOAP_F32, SOAP_F64 = 0, 1
 SOAP_SPOT, SOAP_FACULA = 1, 2
-SOAP_FORM_AUTO, SOAP_FORM_BINNED, SOAP_FORM_CELLS, SOAP_FORM_FIR = 0, 1, 2, 3
+SOAP_FORM_AUTO, SOAP_FORM_BINNED, SOAP_FORM_CELLS, SOAP_FORM_FIR, SOAP_FORM_COMPOSITE = 0, 1, 2, 3, 4
 SOAP_OPT_FORM, SOAP_OPT_QUIET_SPLITS, SOAP_OPT_KERNEL_TIMING = 1, 2, 3
 
 EXPORTED_SYMBOLS = (

@@ -1,0 +1,435 @@
+// a3 of SURVEY section 8, composite-column form (SOAP_FORM_COMPOSITE) for fp32 spectra under solid-body rotation.
+//
+//   Q[m] = sum_j sum_b W[j,b] lerp(S_b; m + delta_j(m))  =  sum_j lerp(T_j; m + delta_j(m)),   T_j[n] = sum_b W[j,b] S_b[n]
+//
+// (Alg. 1 with Eq. 5-9 as a gather; cells pre-binned by (column, mu-bin) as BASELINE.json's
+// north_star allows.)  Linear interpolation is linear in the spectrum and all cells of a column share one velocity, so
+// the weighted rows of a column can be added BEFORE the shift: one FMA per (column, mu-bin, pixel) on unshifted
+// samples, then one interpolation per (column, pixel) - instead of two FMAs per (column, mu-bin, pixel) plus a
+// window set-up per run of entries.  Nothing depends on how the shifts are distributed, so fast rotators cost
+// the same as slow ones ("composite-column form").
+//
+//   * A CTA of 512 threads holds a span of 2048 source pixels of EVERY mu-bin row in registers (thread i: pixels
+//     n0 + 4 i .. + 3 of each row, one LDG.128 per row): 20 bins x 2048 px = 62 % of the SM's register file.  The
+//     span is an output tile of L = 2048 - 2 H pixels plus the halo H the shifts can reach on either side.
+//   * Columns are taken two at a time.  Compute phase: TU[r] = (T_j, T_j+1)[pixel r] accumulates
+//     (W[j,b], W[j+1,b]) * S_b[r] with packed FFMA2 (the weight pair is one LDS.128-broadcast operand, the sample a
+//     scalar-broadcast register): 4 FFMA2 per bin per thread.  The pair is written to shared memory interleaved as
+//     float2 (double-buffered: one CTA barrier per column pair).
+//   * Lerp phase: thread i owns output pixels m0 + i + 512 r (conflict-free LDS.64, two columns per load):
+//     t = a_j c_m - q_j, acc += x0 + t (x1 - x0): 4 packed instructions per (column pair, pixel).  The integer
+//     shift q_j is constant over the tile for ~99 % of the columns (checked per pair); the rest take a per-pixel
+//     floor.  Only the shift delta = a_j (lambda0/k + m) is formed in fp32, never the absolute source coordinate.
+//   * fp32 column sums are folded into fp64 every kFoldPairs pairs; fp64 totals are rounded once on store.
+//   * Work = the flattened (star, tile, column pair) list with a cost per pair (bins present + the lerp), cut into
+//     equal contiguous ranges, one per CTA (one wave, any number of tiles / stars per CTA, or many CTAs per tile
+//     when the spectrum is short).  A tile wholly inside one CTA's range is stored directly (STG.128 after a
+//     shared-memory transpose); a shared tile's fp64 partial sums are added in CTA order by the last CTA to
+//     deliver (atomic ticket, self-resetting): run-to-run identical.
+//   * Batch (config 5): the same launch walks an array of stars (soap_batch_integrate_quiet).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "ptx_helpers.cuh"
+
+namespace soap {
+namespace comp {
+
+constexpr int kThreads = 512;
+constexpr int kPx = 4;                 // source pixels per thread and mu-bin
+constexpr int kSpan = kThreads * kPx;  // source pixels per CTA span
+constexpr int kFoldPairs = 4;          // fp32 -> fp64 fold interval (column pairs = 8 columns)
+constexpr int kMaxBins = 24;           // mu bins the register-resident form can hold
+constexpr int kMaxStars = 256;         // stars per launch
+constexpr int kPairCostBase = 24;      // cost model: 8 FFMA2-slots per weight load + the lerp, barrier and loop
+
+struct PairHdr {  // one column pair (2p, 2p+1); entry [n_pairs] carries the total cost in cost0
+    float a0, a1;  // shift factors D - 1 of the two columns (0 for the missing column of an odd grid)
+    int nl;        // weight loads: bins 0 .. 2 nl - 1 hold every non-zero weight of the pair
+    int cost0;     // cost of the pairs before this one
+};
+
+struct Star {
+    const float *base;   // [n_mu][pitch]
+    float *out;          // [n_pix]
+    const float2 *Wp;    // [n_pairs][wp_stride]: (W[2p][b], W[2p+1][b])
+    const PairHdr *hdr;  // [n_pairs + 1]
+    int *ticket;         // [n_tiles] shares delivered per tile; zero between launches
+    long long pitch, n_pix, out_lo, out_hi;
+    double c0;           // lambda0 / dlambda
+    int n_mu, n_pairs, halo, L, n_tiles, wp_stride;
+};
+
+struct Params {
+    Star one;            // the star of a single-star launch (travels as a kernel argument: no copy)
+    const Star *many;    // batch: DEVICE [n_stars]; nullptr = `one`
+    int n_stars;
+    double *partial;     // [gridDim.x][2][kSpan]
+    int max_pairs;       // shared-memory table capacity
+};
+
+__host__ __device__ inline size_t smem_bytes(int nb, int max_pairs) {
+    return (size_t)2 * kSpan * sizeof(float2) + (size_t)max_pairs * nb * sizeof(float2) + (size_t)(max_pairs + 1) * sizeof(PairHdr) +
+           (size_t)(kMaxStars + 1) * sizeof(long long) + sizeof(Star) + 64;
+}
+
+// Built by the last CTA of geometry_kernel: the pair tables of the composite form.
+__device__ inline void build_composite_tables(int N, int n_mu, const double *col_a, const double *Wbin, float2 *Wp, int wp_stride,
+                                              PairHdr *hdr) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+    const int n_pairs = (N + 1) / 2;
+    for (int p = warp; p < n_pairs; p += n_warps) {
+        const int j0 = 2 * p, j1 = 2 * p + 1;
+        int hi = -1;
+        for (int b0 = 0; b0 < wp_stride; b0 += 32) {
+            const int b = b0 + lane;
+            double w0 = 0.0, w1 = 0.0;
+            if (b < n_mu) {
+                w0 = Wbin[(size_t)j0 * n_mu + b];
+                if (j1 < N) w1 = Wbin[(size_t)j1 * n_mu + b];
+            }
+            if (b < wp_stride) Wp[(size_t)p * wp_stride + b] = make_float2((float)w0, (float)w1);
+            const unsigned m = __ballot_sync(0xffffffffu, w0 != 0.0 || w1 != 0.0);
+            if (m) hi = b0 + 31 - __clz(m);
+        }
+        if (lane == 0) {
+            PairHdr h;
+            h.a0 = (float)col_a[j0];
+            h.a1 = j1 < N ? (float)col_a[j1] : 0.f;
+            h.nl = (hi + 2) / 2;
+            h.cost0 = 0;
+            hdr[p] = h;
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int run = 0;
+        for (int p = 0; p < n_pairs; ++p) {
+            const int c = 8 * hdr[p].nl + kPairCostBase;
+            hdr[p].cost0 = run;
+            run += c;
+        }
+        PairHdr t;
+        t.a0 = t.a1 = 0.f;
+        t.nl = 0;
+        t.cost0 = run;
+        hdr[n_pairs] = t;
+    }
+}
+
+// CTA that owns work unit u when U units are cut into G ranges [floor(g U / G), floor((g+1) U / G)).
+__device__ __forceinline__ long long owner_of(long long u, long long U, long long G) { return ((u + 1) * G - 1) / U; }
+
+template <int NB>
+__global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Params p) {
+    static_assert(NB % 4 == 0 && NB <= kMaxBins, "bins are loaded two per LDS.128 and unrolled four at a time");
+    extern __shared__ __align__(16) unsigned char smem[];
+    float2 *Tbuf = reinterpret_cast<float2 *>(smem);                                  // [2][kSpan]
+    float2 *Wsm = Tbuf + 2 * kSpan;                                                   // [max_pairs][NB]
+    PairHdr *hsm = reinterpret_cast<PairHdr *>(Wsm + (size_t)p.max_pairs * NB);        // [max_pairs + 1]
+    long long *unit0 = reinterpret_cast<long long *>(hsm + p.max_pairs + 1);          // [n_stars + 1]
+    Star *cur = reinterpret_cast<Star *>(unit0 + kMaxStars + 1);
+    int *ctl = reinterpret_cast<int *>(cur + 1);                                      // last-CTA flag
+
+    const int tid = threadIdx.x;
+    const long long G = gridDim.x, g = blockIdx.x;
+    const int n_stars = p.n_stars;
+
+    // ---- work units of every star: n_tiles x (cost of all its pairs) -------------------------------------------
+    for (int s = tid; s < n_stars; s += kThreads) {
+        const Star &st = p.many ? p.many[s] : p.one;
+        unit0[s + 1] = (long long)st.n_tiles * (long long)__ldg(&st.hdr[st.n_pairs].cost0);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        long long run = 0;
+        for (int s = 0; s < n_stars; ++s) {
+            const long long c = unit0[s + 1];
+            unit0[s] = run;
+            run += c;
+        }
+        unit0[n_stars] = run;
+    }
+    __syncthreads();
+    const long long U = unit0[n_stars];
+    if (U <= 0) return;
+    const long long B0 = (g * U) / G, B1 = ((g + 1) * U) / G;
+    if (B1 <= B0) return;
+
+    int s = 0;
+    while (unit0[s + 1] <= B0) ++s;  // the star that holds unit B0 (stars without work are skipped)
+    int cur_s = -1;
+    long long t = -1;
+    int k = 0;
+    bool first_seg = true;
+    unsigned it = 0;  // column pairs processed by this CTA: selects the T buffer
+
+    for (;;) {
+        if (s >= n_stars) break;
+        if (s != cur_s) {  // ---- this star's tables -> shared memory
+            __syncthreads();
+            const Star &st = p.many ? p.many[s] : p.one;
+            if (tid == 0) *cur = st;
+            const int np = st.n_pairs;
+            const float4 *src = reinterpret_cast<const float4 *>(st.Wp);
+            float4 *dst = reinterpret_cast<float4 *>(Wsm);
+            for (int i = tid; i < np * NB / 2; i += kThreads) dst[i] = __ldg(&src[i]);
+            const int4 *hs = reinterpret_cast<const int4 *>(st.hdr);
+            int4 *hd = reinterpret_cast<int4 *>(hsm);
+            for (int i = tid; i <= np; i += kThreads) hd[i] = __ldg(&hs[i]);
+            cur_s = s;
+            __syncthreads();
+        }
+        const int n_pairs = cur->n_pairs;
+        const long long C = hsm[n_pairs].cost0;
+        if (first_seg) {  // first pair whose start unit is >= B0
+            const long long rel = B0 - unit0[s];
+            t = rel / C;
+            const int r = (int)(rel - t * C);
+            int lo = 0, hi = n_pairs;  // first k with cost0[k] >= r
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (hsm[mid].cost0 >= r) hi = mid;
+                else lo = mid + 1;
+            }
+            k = lo;
+            if (k == n_pairs) {
+                k = 0;
+                ++t;
+            }
+            first_seg = false;
+            if (t >= cur->n_tiles) {
+                ++s;
+                t = 0;
+                first_seg = false;
+                continue;
+            }
+        }
+        const long long u_tile = unit0[s] + t * C;
+        if (u_tile + hsm[k].cost0 >= B1) break;
+        int k_end = n_pairs;
+        if (B1 - u_tile < C) {  // first pair whose start unit is >= B1
+            const int lim = (int)(B1 - u_tile);
+            int lo = k, hi = n_pairs;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (hsm[mid].cost0 >= lim) hi = mid;
+                else lo = mid + 1;
+            }
+            k_end = lo;
+        }
+
+        // ================= one segment: pairs [k, k_end) of tile t of star s =======================================
+        {
+            const int H = cur->halo, L = cur->L, n_mu = cur->n_mu;
+            const long long n_pix = cur->n_pix, pitch = cur->pitch;
+            const long long m0 = t * (long long)L, n0 = m0 - H;
+            // ---- the span of every mu-bin row -> registers (clamp-to-edge outside the grid, reading S8)
+            float S[NB][kPx];
+            {
+                const long long n = n0 + 4 * tid;
+                const bool inside = n >= 0 && n + 3 < n_pix;
+                const float *row = cur->base + n;
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    if (b < n_mu) {
+                        if (inside) {
+                            const float4 v = __ldg(reinterpret_cast<const float4 *>(row + (long long)b * pitch));
+                            S[b][0] = v.x;
+                            S[b][1] = v.y;
+                            S[b][2] = v.z;
+                            S[b][3] = v.w;
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < kPx; ++e) {
+                                long long nn = n + e;
+                                nn = nn < 0 ? 0 : (nn > n_pix - 1 ? n_pix - 1 : nn);
+                                S[b][e] = __ldg(cur->base + (long long)b * pitch + nn);
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < kPx; ++e) S[b][e] = 0.f;
+                    }
+                }
+            }
+            const float c_first = (float)(cur->c0 + (double)m0), c_last = (float)(cur->c0 + (double)(m0 + L - 1));
+            float cr[kPx];
+#pragma unroll
+            for (int r = 0; r < kPx; ++r) cr[r] = (float)(cur->c0 + (double)(m0 + tid + kThreads * r));
+            const int nvalid = L - tid <= 0 ? 0 : (L - tid + kThreads - 1) / kThreads;  // output pixels of this thread (<= 4)
+            float2 A[kPx];
+            double tot[kPx];
+#pragma unroll
+            for (int r = 0; r < kPx; ++r) {
+                A[r] = make_float2(0.f, 0.f);
+                tot[r] = 0.0;
+            }
+            int since_fold = 0;
+            for (int kk = k; kk < k_end; ++kk, ++it) {
+                // ---- compute phase: TU[r] = sum_b (W[j,b], W[j+1,b]) S_b[r]
+                const int4 hraw = *reinterpret_cast<const int4 *>(&hsm[kk]);
+                const float a0 = __int_as_float(hraw.x), a1 = __int_as_float(hraw.y);
+                const int nl = hraw.z;
+                float2 TU[kPx];
+#pragma unroll
+                for (int r = 0; r < kPx; ++r) TU[r] = make_float2(0.f, 0.f);
+                const float4 *wrow = reinterpret_cast<const float4 *>(Wsm + (size_t)kk * NB);
+#pragma unroll
+                for (int l = 0; l < NB / 2; ++l) {
+                    if (l < nl) {
+                        const float4 w = wrow[l];
+#pragma unroll
+                        for (int r = 0; r < kPx; ++r) TU[r] = fma2(make_float2(w.x, w.y), bcast2(S[2 * l][r]), TU[r]);
+#pragma unroll
+                        for (int r = 0; r < kPx; ++r) TU[r] = fma2(make_float2(w.z, w.w), bcast2(S[2 * l + 1][r]), TU[r]);
+                    }
+                }
+                float2 *buf = Tbuf + (it & 1u) * kSpan;
+                reinterpret_cast<float4 *>(buf)[2 * tid] = make_float4(TU[0].x, TU[0].y, TU[1].x, TU[1].y);
+                reinterpret_cast<float4 *>(buf)[2 * tid + 1] = make_float4(TU[2].x, TU[2].y, TU[3].x, TU[3].y);
+                __syncthreads();
+                // ---- lerp phase: acc += lerp(T_j; m + a_j c_m) for both columns
+                const float qf0 = floorf(a0 * c_first), qf1 = floorf(a1 * c_first);
+                const bool steady = qf0 == floorf(a0 * c_last) && qf1 == floorf(a1 * c_last);
+                if (steady) {
+                    int q0 = (int)qf0, q1 = (int)qf1;
+                    q0 = max(-(H - 1), min(H - 2, q0));
+                    q1 = max(-(H - 1), min(H - 2, q1));
+                    const float2 aa = make_float2(a0, a1), nq = make_float2(-(float)q0, -(float)q1);
+                    if (q0 == q1) {
+                        const float2 *w0 = buf + H + tid + q0;
+#pragma unroll
+                        for (int r = 0; r < kPx; ++r) {
+                            if (r < nvalid) {
+                                const float2 x0 = w0[kThreads * r], x1 = w0[kThreads * r + 1];
+                                const float2 tt = fma2(aa, bcast2(cr[r]), nq);
+                                const float2 d = fma2(bcast2(-1.f), x0, x1);
+                                A[r] = add2(fma2(tt, d, A[r]), x0);
+                            }
+                        }
+                    } else {
+                        const float *w0 = reinterpret_cast<const float *>(buf + H + tid + q0);
+                        const float *w1 = reinterpret_cast<const float *>(buf + H + tid + q1) + 1;
+#pragma unroll
+                        for (int r = 0; r < kPx; ++r) {
+                            if (r < nvalid) {
+                                const float2 x0 = make_float2(w0[2 * kThreads * r], w1[2 * kThreads * r]);
+                                const float2 x1 = make_float2(w0[2 * kThreads * r + 2], w1[2 * kThreads * r + 2]);
+                                const float2 tt = fma2(aa, bcast2(cr[r]), nq);
+                                const float2 d = fma2(bcast2(-1.f), x0, x1);
+                                A[r] = add2(fma2(tt, d, A[r]), x0);
+                            }
+                        }
+                    }
+                } else {  // an integer shift changes inside the tile: per-pixel floor
+                    const float *bf = reinterpret_cast<const float *>(buf + H + tid);
+#pragma unroll
+                    for (int r = 0; r < kPx; ++r) {
+                        if (r < nvalid) {
+                            const float q0f = floorf(a0 * cr[r]), q1f = floorf(a1 * cr[r]);
+                            const float t0 = fmaf(a0, cr[r], -q0f), t1 = fmaf(a1, cr[r], -q1f);
+                            int q0 = (int)q0f, q1 = (int)q1f;
+                            q0 = max(-(H - 1), min(H - 2, q0));
+                            q1 = max(-(H - 1), min(H - 2, q1));
+                            const float x00 = bf[2 * (kThreads * r + q0)], x01 = bf[2 * (kThreads * r + q0) + 2];
+                            const float x10 = bf[2 * (kThreads * r + q1) + 1], x11 = bf[2 * (kThreads * r + q1) + 3];
+                            A[r].x += fmaf(t0, x01 - x00, x00);
+                            A[r].y += fmaf(t1, x11 - x10, x10);
+                        }
+                    }
+                }
+                if (++since_fold == kFoldPairs) {
+#pragma unroll
+                    for (int r = 0; r < kPx; ++r) {
+                        tot[r] += (double)(A[r].x + A[r].y);
+                        A[r] = make_float2(0.f, 0.f);
+                    }
+                    since_fold = 0;
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < kPx; ++r) tot[r] += (double)(A[r].x + A[r].y);
+
+            // ---- a6: store.  A tile wholly inside this CTA's range goes straight out; otherwise the shares are added
+            // in CTA order by the last CTA to deliver.
+            const bool whole = k == 0 && k_end == n_pairs;
+            const long long lo = cur->out_lo, hi = cur->out_hi < n_pix ? cur->out_hi : n_pix;
+            float *out = cur->out;
+            const bool vec_ok = (reinterpret_cast<uintptr_t>(out) & 15) == 0;
+            __syncthreads();  // every lerp of this segment has read its T buffer
+            if (whole) {
+                float *stage = reinterpret_cast<float *>(Tbuf);
+#pragma unroll
+                for (int r = 0; r < kPx; ++r) stage[tid + kThreads * r] = (float)tot[r];
+                __syncthreads();
+                const int o = 4 * tid;
+                if (o < L) {
+                    const float4 v = reinterpret_cast<const float4 *>(stage)[tid];
+                    const long long m = m0 + o;
+                    if (vec_ok && m >= lo && m + 3 < hi) {
+                        *reinterpret_cast<float4 *>(out + m) = v;
+                    } else {
+                        const float e[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                        for (int q = 0; q < 4; ++q)
+                            if (m + q >= lo && m + q < hi) out[m + q] = e[q];
+                    }
+                }
+                __syncthreads();  // the stage is a T buffer again
+            } else {
+                const long long u_last = u_tile + hsm[n_pairs - 1].cost0;
+                const long long g_first = owner_of(u_tile, U, G), g_last = owner_of(u_last, U, G);
+                const int slot = g == g_first ? 1 : 0;  // a CTA's head share (k == 0) and tail share (k > 0) of two tiles
+                double *mine = p.partial + ((size_t)g * 2 + slot) * kSpan;
+#pragma unroll
+                for (int r = 0; r < kPx; ++r) mine[tid + kThreads * r] = tot[r];
+                __threadfence();
+                __syncthreads();
+                if (tid == 0) {
+                    const int ticket = atomicAdd(&cur->ticket[t], 1);
+                    const bool last = ticket == (int)(g_last - g_first);
+                    if (last) cur->ticket[t] = 0;  // ready for the next launch
+                    ctl[0] = last ? 1 : 0;
+                }
+                __syncthreads();
+                if (ctl[0]) {
+                    __threadfence();
+                    const int o = 4 * tid;
+                    if (o < L) {
+                        double sum[4] = {0.0, 0.0, 0.0, 0.0};
+                        for (long long c = g_first; c <= g_last; ++c) {
+                            const double *src = p.partial + ((size_t)c * 2 + (c == g_first ? 1 : 0)) * kSpan + o;
+                            const double2 v0 = __ldcg(reinterpret_cast<const double2 *>(src));
+                            const double2 v1 = __ldcg(reinterpret_cast<const double2 *>(src) + 1);
+                            sum[0] += v0.x;
+                            sum[1] += v0.y;
+                            sum[2] += v1.x;
+                            sum[3] += v1.y;
+                        }
+                        const long long m = m0 + o;
+                        if (vec_ok && m >= lo && m + 3 < hi) {
+                            *reinterpret_cast<float4 *>(out + m) = make_float4((float)sum[0], (float)sum[1], (float)sum[2], (float)sum[3]);
+                        } else {
+#pragma unroll
+                            for (int q = 0; q < 4; ++q)
+                                if (m + q >= lo && m + q < hi) out[m + q] = (float)sum[q];
+                        }
+                    }
+                }
+                __syncthreads();  // ctl may be rewritten by the next segment
+            }
+        }
+
+        if (k_end < n_pairs) break;  // the range ends inside this tile
+        k = 0;
+        if (++t >= cur->n_tiles) {
+            ++s;
+            t = 0;
+        }
+    }
+}
+
+}  // namespace comp
+}  // namespace soap

@@ -7,6 +7,8 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+#include "composite.cuh"
+
 namespace soap {
 
 constexpr double kSpeedOfLightKms = 299792.458;
@@ -310,7 +312,9 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
                 double *__restrict__ col_sumw, int *__restrict__ col_nvis, float2 *__restrict__ ent32,
                 double2 *__restrict__ ent64, int *__restrict__ row_start, DevInfo *__restrict__ info,
                 unsigned int *__restrict__ done, int *__restrict__ colcnt /*[N][n_mu]*/,
-                int *__restrict__ cellpos /*[n_mu][N], per-cell form only*/, int cells) {
+                int *__restrict__ cellpos /*[n_mu][N], per-cell form only*/, int cells,
+                float2 *__restrict__ comp_Wp /*composite form: [ceil(N/2)][comp_stride], or nullptr*/, int comp_stride,
+                comp::PairHdr *__restrict__ comp_hdr) {
     __shared__ double s_W[kGeomWarps][64];
     __shared__ int s_Cn[kGeomWarps][64];
     __shared__ double s_mu[64];
@@ -371,6 +375,10 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
     __threadfence();
     if (threadIdx.x == 0) *done = 0;
     build_binned_entries(N, n_mu, col_a, Wbin, col_sumw, col_nvis, ent32, ent64, row_start, info);
+    if (comp_Wp) {  // pair tables of the composite-column form (composite.cuh)
+        __syncthreads();
+        comp::build_composite_tables(N, n_mu, col_a, Wbin, comp_Wp, comp_stride, comp_hdr);
+    }
     if (cells) {  // per-cell form: the entry list is rebuilt by write_cell_entries_kernel at these positions
         __syncthreads();
         build_cell_positions(N, n_mu, colcnt, cellpos, row_start, ent32, ent64);

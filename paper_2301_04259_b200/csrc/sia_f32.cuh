@@ -525,12 +525,15 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         cp_async_commit();
     };
     auto fold_kind = [&](int kind) {
-        if (p.contrast[kind] == nullptr) return;  // weight 1: keeps accumulating with the next kind
+        // weight 1: keeps accumulating with the next kind - unless that kind's sum is about to be multiplied by
+        // its own contrast (job order is 1, 2, 0: only a spot sum without contrast ahead of a facula with one)
+        const bool has_c = p.contrast[kind] != nullptr;
+        if (!has_c && !(kind == 1 && p.contrast[2] != nullptr)) return;
         fold();
         cp_async_wait_all();
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
-            const double c = r < rmax ? (double)cst[r * kConsumers + tid] : 1.0;
+            const double c = (has_c && r < rmax) ? (double)cst[r * kConsumers + tid] : 1.0;
             const double f = fin_valid ? fin[r * kConsumers + tid] : 0.0;
             fin[r * kConsumers + tid] = f + c * tot[r];
             tot[r] = 0.0;

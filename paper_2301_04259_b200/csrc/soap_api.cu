@@ -15,6 +15,7 @@
 
 #include "../../include/soap_b200.h"
 #include "active.cuh"
+#include "composite.cuh"
 #include "geometry.cuh"
 #include "lsf.cuh"
 #include "rv.cuh"
@@ -82,6 +83,10 @@ struct soap_star {
     DevBuf<DevInfo> d_info;
     DevBuf<unsigned int> d_geom_done;
     size_t ent_cap = 0;
+    // composite-column form: pair tables built by the geometry kernel
+    DevBuf<float2> d_cWp;
+    DevBuf<comp::PairHdr> d_chdr;
+    int comp_stride = 0;  // bins per table row (multiple of 4); 0 = tables not built
 
     // quiet scratch
     DevBuf<double> d_partial;
@@ -144,6 +149,7 @@ inline double host_dshift(double v_kms, int mode) {
 }
 
 inline int round_up4(long long v) { return (int)((v + 3) & ~3LL); }
+inline bool n_mu_ok_for_composite(int n_mu) { return n_mu >= 1 && n_mu <= comp::kMaxBins; }
 
 int check_spectra(soap_star *s, const soap_spectra *sp, const char *name) {
     if (!sp) return s->fail(SOAP_ERR_INVALID_ARG, "%s spectra: NULL", name);
@@ -263,8 +269,109 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     return SOAP_OK;
 }
 
+// Composite-column form (composite.cuh): does the launch apply to this star and these spectra?
+bool composite_applies(const soap_star *s, const soap_spectra *q) {
+    if (s->form_used != SOAP_FORM_COMPOSITE || s->comp_stride == 0 || q->dtype != SOAP_F32) return false;
+    const int H = halo_for(s, q);
+    if (2 * H > comp::kSpan / 2) return false;
+    const int n_pairs = (s->prm.grid_n + 1) / 2;
+    return comp::smem_bytes(s->comp_stride, n_pairs) <= 200 * 1024;
+}
+
+void composite_fill(const soap_star *s, const soap_spectra *q, void *out, comp::Star &c) {
+    c.base = static_cast<const float *>(q->data);
+    c.out = static_cast<float *>(out);
+    c.Wp = s->d_cWp.ptr;
+    c.hdr = s->d_chdr.ptr;
+    c.ticket = s->d_tile_ticket.ptr;
+    c.pitch = q->pitch;
+    c.n_pix = q->n_pix;
+    c.out_lo = s->out_lo_override >= 0 ? s->out_lo_override : 0;
+    c.out_hi = s->out_hi_override >= 0 ? s->out_hi_override : q->n_pix;
+    c.c0 = q->lambda0 / q->dlambda;
+    c.n_mu = s->prm.n_mu;
+    c.n_pairs = (s->prm.grid_n + 1) / 2;
+    c.halo = halo_for(s, q);
+    c.L = comp::kSpan - 2 * c.halo;
+    c.n_tiles = (int)((q->n_pix + c.L - 1) / c.L);
+    c.wp_stride = s->comp_stride;
+}
+
+template <int NB>
+int launch_composite_nb(soap_star *s, const comp::Params &p, unsigned G, size_t smem, cudaStream_t st) {
+    static bool attr_set[64] = {};
+    if (!attr_set[s->device & 63]) {
+        SOAP_CUDA(s, cudaFuncSetAttribute(comp::composite_quiet_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_set[s->device & 63] = true;
+    }
+    comp::composite_quiet_kernel<NB><<<G, comp::kThreads, smem, st>>>(p);
+    return SOAP_OK;
+}
+
+// One launch for n_stars stars (n_stars == 1: the descriptor travels as a kernel argument).  `owner` provides the
+// scratch and the timing events.
+int launch_composite(soap_star *owner, const comp::Star *host_stars, const comp::Star *dev_stars, int n_stars, int nb,
+                     int max_pairs, int max_mu, cudaStream_t st) {
+    comp::Params p{};
+    p.one = host_stars[0];
+    p.many = n_stars > 1 ? dev_stars : nullptr;
+    p.n_stars = n_stars;
+    p.max_pairs = max_pairs;
+    // every CTA's range must hold at least one whole pair of every tile it shares (composite.cuh, ticket count)
+    const long long cmax = 8LL * ((max_mu + 1) / 2) + comp::kPairCostBase;
+    long long min_units = 0;
+    for (int k = 0; k < n_stars; ++k) min_units += (long long)host_stars[k].n_tiles * host_stars[k].n_pairs * comp::kPairCostBase;
+    const long long G = std::max(1LL, std::min((long long)owner->n_sm, min_units / (2 * cmax)));
+    SOAP_CUDA(owner, owner->d_partial.reserve((size_t)G * 2 * comp::kSpan));
+    p.partial = owner->d_partial.ptr;
+    const size_t smem = comp::smem_bytes(nb, max_pairs);
+    if (owner->opt_timing) {
+        for (int k = 0; k < 2; ++k)
+            if (!owner->ev[k]) SOAP_CUDA(owner, cudaEventCreate(&owner->ev[k]));
+        SOAP_CUDA(owner, cudaEventRecord(owner->ev[0], st));
+    }
+    int rc = SOAP_OK;
+    switch (nb) {
+        case 4: rc = launch_composite_nb<4>(owner, p, (unsigned)G, smem, st); break;
+        case 8: rc = launch_composite_nb<8>(owner, p, (unsigned)G, smem, st); break;
+        case 12: rc = launch_composite_nb<12>(owner, p, (unsigned)G, smem, st); break;
+        case 16: rc = launch_composite_nb<16>(owner, p, (unsigned)G, smem, st); break;
+        case 20: rc = launch_composite_nb<20>(owner, p, (unsigned)G, smem, st); break;
+        default: rc = launch_composite_nb<24>(owner, p, (unsigned)G, smem, st); break;
+    }
+    if (rc) return rc;
+    SOAP_LAUNCH_CHECK(owner, "composite_quiet_kernel");
+    if (owner->opt_timing) {
+        SOAP_CUDA(owner, cudaEventRecord(owner->ev[1], st));
+        owner->ev_valid[0] = true;
+    }
+    owner->last_quiet_splits = (int)G;
+    return SOAP_OK;
+}
+
+int reserve_tickets(soap_star *s, size_t n_tiles, cudaStream_t st) {
+    if (n_tiles > s->d_tile_ticket.cap) {
+        SOAP_CUDA(s, s->d_tile_ticket.reserve(n_tiles));
+        SOAP_CUDA(s, cudaMemsetAsync(s->d_tile_ticket.ptr, 0, s->d_tile_ticket.cap * sizeof(int), st));  // self-resetting after
+    }
+    return SOAP_OK;
+}
+
+int quiet_composite(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
+    comp::Star c{};
+    composite_fill(s, q, out, c);
+    int rc = reserve_tickets(s, (size_t)c.n_tiles + 1, st);
+    if (rc) return rc;
+    c.ticket = s->d_tile_ticket.ptr;
+    rc = launch_composite(s, &c, nullptr, 1, s->comp_stride, c.n_pairs, s->prm.n_mu, st);
+    if (rc) return rc;
+    s->last_tile_px = c.L;
+    return SOAP_OK;
+}
+
 template <typename T>
 int quiet_impl(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
+    if (sizeof(T) == 4 && composite_applies(s, q)) return quiet_composite(s, q, out, st);
     if (sizeof(T) == 4) return quiet_f32(s, q, out, st);
     constexpr int TP = sia_tile_px<T>();
     const long long P = q->n_pix;
@@ -728,6 +835,7 @@ int soap_create(soap_star **out, int device) {
 int soap_destroy(soap_star *s) {
     if (!s) return SOAP_OK;
     cudaSetDevice(s->device);
+    s->d_cWp.release(); s->d_chdr.release();
     s->d_geom_done.release(); s->d_colcnt.release(); s->d_cellpos.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
     s->d_Wbin.release(); s->d_col_sumw.release(); s->d_bin.release(); s->d_col_nvis.release(); s->d_row_start.release();
     s->d_ent32.release(); s->d_ent64.release(); s->d_info.release(); s->d_partial.release(); s->d_tile_ticket.release(); s->d_rp.release();
@@ -751,7 +859,7 @@ int soap_set_option(soap_star *s, int32_t option, int64_t value) {
     if (!s) return SOAP_ERR_INVALID_ARG;
     switch (option) {
         case SOAP_OPT_FORM:
-            if (value < SOAP_FORM_AUTO || value > SOAP_FORM_FIR) return s->fail(SOAP_ERR_INVALID_ARG, "unknown form %lld", (long long)value);
+            if (value < SOAP_FORM_AUTO || value > SOAP_FORM_COMPOSITE) return s->fail(SOAP_ERR_INVALID_ARG, "unknown form %lld", (long long)value);
             if ((int)value != s->form) s->ready = false;  // entry list must be rebuilt
             s->form = (int)value;
             return SOAP_OK;
@@ -799,7 +907,11 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     if (!std::isfinite(prm->diff_rot) || !(prm->diff_rot > -1.0)) return s->fail(SOAP_ERR_INVALID_ARG, "diff_rot must be finite and > -1");
     if (prm->diff_rot != 0.0 && s->form == SOAP_FORM_BINNED)
         return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_BINNED needs solid-body rotation: the cells of a column must share one velocity");
+    if (prm->diff_rot != 0.0 && s->form == SOAP_FORM_COMPOSITE)
+        return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_COMPOSITE needs solid-body rotation: the cells of a column must share one velocity");
     s->form_used = (s->form == SOAP_FORM_CELLS || s->form == SOAP_FORM_FIR) ? s->form : SOAP_FORM_BINNED;
+    // the composite-column form holds every mu-bin row of a span in registers: up to comp::kMaxBins bins
+    if (s->form == SOAP_FORM_COMPOSITE && n_mu_ok_for_composite(prm->n_mu)) s->form_used = SOAP_FORM_COMPOSITE;
     s->cell_entries = s->form == SOAP_FORM_CELLS || prm->diff_rot != 0.0;
     // AUTO under differential rotation: per-cell entries with every run collapsed (the binned form does not apply;
     // the collapse is exact and ~5x cheaper than one lerp-accumulate per cell and pixel)
@@ -822,6 +934,12 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     const size_t ent_cap = std::max(s->cell_entries ? ncell : (size_t)0, (size_t)N * n_mu) + 2 * (size_t)n_mu + 8;
     SOAP_CUDA(s, s->d_ent32.reserve(ent_cap));
     SOAP_CUDA(s, s->d_ent64.reserve(ent_cap));
+    s->comp_stride = 0;
+    if (s->form_used == SOAP_FORM_COMPOSITE) {
+        s->comp_stride = round_up4(n_mu);
+        SOAP_CUDA(s, s->d_cWp.reserve((size_t)((N + 1) / 2) * s->comp_stride));
+        SOAP_CUDA(s, s->d_chdr.reserve((size_t)(N + 1) / 2 + 1));
+    }
 
     if (!s->d_geom_done.ptr) {
         SOAP_CUDA(s, s->d_geom_done.reserve(1));
@@ -834,7 +952,8 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     geometry_kernel<<<(N + geom_cols_per_cta(N) - 1) / geom_cols_per_cta(N), 32 * kGeomWarps, 0, st>>>(
         N, rot, prm->ld_u1, prm->ld_u2, prm->doppler_mode, n_mu, mc, s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr, s->d_bin.ptr,
         s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr, s->d_ent32.ptr, s->d_ent64.ptr, s->d_row_start.ptr,
-        s->d_info.ptr, s->d_geom_done.ptr, s->d_colcnt.ptr, s->d_cellpos.ptr, s->cell_entries ? 1 : 0);
+        s->d_info.ptr, s->d_geom_done.ptr, s->d_colcnt.ptr, s->d_cellpos.ptr, s->cell_entries ? 1 : 0,
+        s->comp_stride ? s->d_cWp.ptr : nullptr, s->comp_stride, s->d_chdr.ptr);
     SOAP_LAUNCH_CHECK(s, "geometry_kernel");
     if (s->cell_entries) {
         write_cell_entries_kernel<<<(N + kCellWarps - 1) / kCellWarps, 32 * kCellWarps, 0, st>>>(

@@ -175,6 +175,21 @@ def test_splits_do_not_change_parity_and_runs_are_deterministic(soap):
     assert np.array_equal(b["Q"], c["Q"]) and np.array_equal(b["D"], c["D"])
 
 
+@pytest.mark.parametrize("which", ["facula_only", "spot_only", "neither", "both"])
+def test_contrast_array_on_either_kind_or_none(soap, which):
+    """A per-pixel contrast on the spot rows only, the facula rows only, both or neither (NULL == 1, soap_b200.h):
+    the kinds of one phase are summed in the order spot, facula, quiet and each sum takes only its own contrast."""
+    wl = workloads.make_config3(n_pix=5000, n_phases=4, grid_n=90)
+    wl.regions = [(-25.0, 170.0, 0.25, 2), (20.0, 185.0, 0.15, 1)]   # both kinds visible together, not nested
+    wl.phases = np.array([0.45, 0.5, 0.55, 0.0])
+    ramp = np.arange(wl.n_pix, dtype=np.float64) / wl.n_pix
+    wl.spot_contrast = (0.3 + 0.2 * ramp).astype(np.float32) if which in ("spot_only", "both") else None
+    wl.facula_contrast = (1.2 - 0.15 * ramp).astype(np.float32) if which in ("facula_only", "both") else None
+    g = run_gpu(soap, wl)
+    assert g["n_active"][:3].min() > 0
+    assert_parity(wl, g)
+
+
 def test_overlap_override_and_duplicates(soap):
     wl = workloads.make_config3(n_pix=2000, n_phases=3, grid_n=100, nested=True)
     wl.phases = np.array([0.45, 0.5, 0.55])
@@ -200,9 +215,9 @@ def test_no_regions_and_zero_rotation(soap):
 def _sample_ranges(n_pix, width=768, n=6):
     rng = np.random.default_rng(123)
     starts = [0, n_pix - width] + [int(v) for v in rng.integers(2048, n_pix - width - 2048, n)]
-    # make two of them straddle a tile boundary (tiles are 1024 px wide in fp32)
-    starts[2] = 1024 * (starts[2] // 1024) - width // 2
-    starts[3] = 1024 * (starts[3] // 1024) - 3
+    # make two of them straddle a tile boundary (f32::kTile = 2048 px; the library reports it as stats.tile_px)
+    starts[2] = 2048 * (starts[2] // 2048) - width // 2
+    starts[3] = 2048 * (starts[3] // 2048) - 3
     return [(s, s + width) for s in starts]
 
 
