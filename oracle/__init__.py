@@ -78,6 +78,9 @@ def _load():
         lib.soap_oracle_line_rvs.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_double, ctypes.c_double,
                                              ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64,
                                              ctypes.c_void_p]
+        lib.soap_oracle_contrast_planck.restype = ctypes.c_int
+        lib.soap_oracle_contrast_planck.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int64, ctypes.c_double,
+                                                    ctypes.c_double, ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -243,4 +246,14 @@ def line_rvs(rows, lambda0: float, k: float, centres, half_widths, norm, edge: i
                                   c.shape[0], nrm.ctypes.data, int(edge), out.ctypes.data)
     if rc != 0:
         raise RuntimeError(f"soap_oracle_line_rvs failed: {rc}")
+    return out
+
+
+def contrast_planck(lambda0: float, k: float, n_pix: int, t_quiet: float, t_active: float) -> np.ndarray:
+    """SOAPcontrast: B_lambda(t_active) / B_lambda(t_quiet) at lambda_m = lambda0 + m k (Angstrom), fp64."""
+    lib = _load()
+    out = np.empty(int(n_pix), dtype=np.float64)
+    rc = lib.soap_oracle_contrast_planck(float(lambda0), float(k), int(n_pix), float(t_quiet), float(t_active), out.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"soap_oracle_contrast_planck failed: {rc}")
     return out

@@ -22,6 +22,9 @@
  *              (reading R-LSF; soap_oracle_lower_resolution)
  *   line RV    first-moment RV per line, BASELINE.json north_star's acceptance functional standing in for
  *              the CCF fit of P:270 (soap_oracle_line_rvs)
+ *   SOAPcontrast  "derives the contrast by calculating the ratio of two Planck functions at two different effective
+ *              temperatures", one value per wavelength pixel, P:312 (and P:300 for SOAP 2.0's single-wavelength
+ *              version of it) (soap_oracle_contrast_planck)
  *
  * No blocking, fusion or reordering: per output pixel the cells are summed in (j, i) order exactly
  * as the double loop of Alg. 1 would.  OpenMP only splits the *wavelength* axis into chunks, which
@@ -33,7 +36,7 @@
  *
  * Parity status: pinned against closed forms / invariants / brute force (tests/test_oracle_pins.py,
  * pins P1-P10 of DESIGN.md; tests/test_oracle_effects.py, test_oracle_diffrot.py, test_oracle_lsf.py,
- * test_oracle_rv.py for the additions); "parity against values printed in the paper": unpinned - the paper
+ * test_oracle_rv.py, test_oracle_contrast.py for the additions); "parity against values printed in the paper": unpinned - the paper
  * prints no numeric output for this path.
  *
  * Cell indexing everywhere: c = j * N + i, j = column (x) index, i = row (y) index,
@@ -419,6 +422,29 @@ int soap_oracle_line_rvs(const double *rows, int64_t n_rows, int64_t P, double l
             }
             rv[r * n_lines + l] = (ok && den != 0.0) ? c_cms * num / den / lc : NAN;
         }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * SOAPcontrast: "each wavelength pixel is first accessed by the global index of the kernel.  Next on each
+ * thread, it derives the contrast by calculating the ratio of two Planck functions at two different effective
+ * temperatures."  With B_lambda(T) = (2 h c^2 / lambda^5) / (exp(h c / (lambda k_B T)) - 1) the prefactor cancels:
+ *     contrast[m] = B_lambda_m(T_active) / B_lambda_m(T_quiet) = (exp(x_q) - 1) / (exp(x_a) - 1),  x = h c / (lambda_m k_B T),
+ * lambda_m = lambda0 + m k in Angstrom (the unit of every wavelength in BASELINE.json's configs).  This is the
+ * I_ratio of Eq. 3 that multiplies the shifted active spectrum.  Constants: CODATA 2018 exact values.
+ * ------------------------------------------------------------------------------------------------ */
+#define ORACLE_PLANCK_H 6.62607015e-34 /* J s */
+#define ORACLE_BOLTZMANN 1.380649e-23  /* J / K */
+#define ORACLE_C_MS 299792458.0        /* m / s */
+
+int soap_oracle_contrast_planck(double lambda0, double k, int64_t n_pix, double T_quiet, double T_active, double *out) {
+    if (!(T_quiet > 0.0) || !(T_active > 0.0) || !(lambda0 > 0.0) || !(k > 0.0) || n_pix < 0) return -1;
+    const double hc_over_kb = ORACLE_PLANCK_H * ORACLE_C_MS / ORACLE_BOLTZMANN; /* m K */
+    for (int64_t m = 0; m < n_pix; ++m) {
+        const double lam_m = (lambda0 + k * (double)m) * 1e-10; /* Angstrom -> metre */
+        const double xq = hc_over_kb / (lam_m * T_quiet), xa = hc_over_kb / (lam_m * T_active);
+        out[m] = expm1(xq) / expm1(xa);
     }
     return 0;
 }
