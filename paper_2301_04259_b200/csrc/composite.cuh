@@ -42,6 +42,8 @@ constexpr int kSpan = kThreads * kPx;  // source pixels per CTA span
 constexpr int kFoldPairs = 4;          // fp32 -> fp64 fold interval (column pairs = 8 columns)
 constexpr int kMaxBins = 24;           // mu bins the register-resident form can hold
 constexpr int kMaxStars = 256;         // stars per launch
+constexpr int kFlipQ = -(1 << 30);      // shift-table marker: the integer shift changes inside the tile
+constexpr bool kAlternate = false;    // halves of the warps take the two phases in opposite order (measured: slower)
 constexpr int kPairCostBase = 24;      // cost model: 8 FFMA2-slots per weight load + the lerp, barrier and loop
 
 struct PairHdr {  // one column pair (2p, 2p+1); entry [n_pairs] carries the total cost in cost0
@@ -70,7 +72,8 @@ struct Params {
 };
 
 __host__ __device__ inline size_t smem_bytes(int nb, int max_pairs) {
-    return (size_t)2 * kSpan * sizeof(float2) + (size_t)max_pairs * nb * sizeof(float2) + (size_t)(max_pairs + 1) * sizeof(PairHdr) +
+    return (size_t)2 * 4 * kSpan * sizeof(float) + (size_t)kSpan * sizeof(double) + (size_t)(max_pairs + 1) * nb * sizeof(float2) +
+           (size_t)(max_pairs + 2) * sizeof(PairHdr) + (size_t)(max_pairs + 1) * sizeof(int4) +
            (size_t)(kMaxStars + 1) * sizeof(long long) + sizeof(Star) + 64;
 }
 
@@ -121,14 +124,36 @@ __device__ inline void build_composite_tables(int N, int n_mu, const double *col
 // CTA that owns work unit u when U units are cut into G ranges [floor(g U / G), floor((g+1) U / G)).
 __device__ __forceinline__ long long owner_of(long long u, long long U, long long G) { return ((u + 1) * G - 1) / U; }
 
+// Compute phase of one column quad (pairs kk, kk + 1), straight-line for NL weight loads per pair (2 mu bins each) so
+// that ptxas hoists the LDS.128 of the next bins above the FFMA2 of the current ones:
+// TU[0][r] = (T_j, T_j+1)[pixel r], TU[1][r] = (T_j+2, T_j+3)[pixel r].
+template <int NB, int NL>
+__device__ __forceinline__ void composite_columns(const float (&S)[NB][kPx], const float4 *__restrict__ w0,
+                                                  const float4 *__restrict__ w1, float2 (&TU)[2][kPx]) {
+#pragma unroll
+    for (int l = 0; l < NL; ++l) {
+        const float4 wa = w0[l], wb = w1[l];
+#pragma unroll
+        for (int r = 0; r < kPx; ++r) TU[0][r] = fma2(make_float2(wa.x, wa.y), bcast2(S[2 * l][r]), TU[0][r]);
+#pragma unroll
+        for (int r = 0; r < kPx; ++r) TU[1][r] = fma2(make_float2(wb.x, wb.y), bcast2(S[2 * l][r]), TU[1][r]);
+#pragma unroll
+        for (int r = 0; r < kPx; ++r) TU[0][r] = fma2(make_float2(wa.z, wa.w), bcast2(S[2 * l + 1][r]), TU[0][r]);
+#pragma unroll
+        for (int r = 0; r < kPx; ++r) TU[1][r] = fma2(make_float2(wb.z, wb.w), bcast2(S[2 * l + 1][r]), TU[1][r]);
+    }
+}
+
 template <int NB>
 __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Params p) {
     static_assert(NB % 4 == 0 && NB <= kMaxBins, "bins are loaded two per LDS.128 and unrolled four at a time");
     extern __shared__ __align__(16) unsigned char smem[];
-    float2 *Tbuf = reinterpret_cast<float2 *>(smem);                                  // [2][kSpan]
-    float2 *Wsm = Tbuf + 2 * kSpan;                                                   // [max_pairs][NB]
-    PairHdr *hsm = reinterpret_cast<PairHdr *>(Wsm + (size_t)p.max_pairs * NB);        // [max_pairs + 1]
-    long long *unit0 = reinterpret_cast<long long *>(hsm + p.max_pairs + 1);          // [n_stars + 1]
+    float *Tbuf = reinterpret_cast<float *>(smem);                                    // [2 buffers][4 columns][kSpan]
+    double *tot_s = reinterpret_cast<double *>(Tbuf + 2 * 4 * kSpan);                 // [kSpan] fp64 totals of the tile
+    float2 *Wsm = reinterpret_cast<float2 *>(tot_s + kSpan);                          // [max_pairs + 1][NB]
+    PairHdr *hsm = reinterpret_cast<PairHdr *>(Wsm + (size_t)(p.max_pairs + 1) * NB);  // [max_pairs + 2]
+    int4 *qtab = reinterpret_cast<int4 *>(hsm + p.max_pairs + 2);                     // [max_pairs + 1] shifts of the current tile
+    long long *unit0 = reinterpret_cast<long long *>(qtab + p.max_pairs + 1);         // [n_stars + 1]
     Star *cur = reinterpret_cast<Star *>(unit0 + kMaxStars + 1);
     int *ctl = reinterpret_cast<int *>(cur + 1);                                      // last-CTA flag
 
@@ -163,7 +188,7 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
     long long t = -1;
     int k = 0;
     bool first_seg = true;
-    unsigned it = 0;  // column pairs processed by this CTA: selects the T buffer
+    unsigned it = 0;  // column quads processed by this CTA: selects the T buffer
 
     for (;;) {
         if (s >= n_stars) break;
@@ -175,9 +200,11 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
             const float4 *src = reinterpret_cast<const float4 *>(st.Wp);
             float4 *dst = reinterpret_cast<float4 *>(Wsm);
             for (int i = tid; i < np * NB / 2; i += kThreads) dst[i] = __ldg(&src[i]);
+            for (int i = tid; i < NB / 2; i += kThreads) dst[np * NB / 2 + i] = make_float4(0.f, 0.f, 0.f, 0.f);  // the pad row
             const int4 *hs = reinterpret_cast<const int4 *>(st.hdr);
             int4 *hd = reinterpret_cast<int4 *>(hsm);
             for (int i = tid; i <= np; i += kThreads) hd[i] = __ldg(&hs[i]);
+            if (tid == 0) hd[np + 1] = make_int4(0, 0, 0, 0);
             cur_s = s;
             __syncthreads();
         }
@@ -202,7 +229,6 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
             if (t >= cur->n_tiles) {
                 ++s;
                 t = 0;
-                first_seg = false;
                 continue;
             }
         }
@@ -225,132 +251,132 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
             const int H = cur->halo, L = cur->L, n_mu = cur->n_mu;
             const long long n_pix = cur->n_pix, pitch = cur->pitch;
             const long long m0 = t * (long long)L, n0 = m0 - H;
-            // ---- the span of every mu-bin row -> registers (clamp-to-edge outside the grid, reading S8)
+            // ---- the span of every mu-bin row -> registers: thread i holds source pixels n0 + i + 512 r
+            // (clamp-to-edge outside the grid, reading S8)
             float S[NB][kPx];
-            {
-                const long long n = n0 + 4 * tid;
-                const bool inside = n >= 0 && n + 3 < n_pix;
-                const float *row = cur->base + n;
 #pragma unroll
-                for (int b = 0; b < NB; ++b) {
-                    if (b < n_mu) {
-                        if (inside) {
-                            const float4 v = __ldg(reinterpret_cast<const float4 *>(row + (long long)b * pitch));
-                            S[b][0] = v.x;
-                            S[b][1] = v.y;
-                            S[b][2] = v.z;
-                            S[b][3] = v.w;
-                        } else {
+            for (int b = 0; b < NB; ++b) {
 #pragma unroll
-                            for (int e = 0; e < kPx; ++e) {
-                                long long nn = n + e;
-                                nn = nn < 0 ? 0 : (nn > n_pix - 1 ? n_pix - 1 : nn);
-                                S[b][e] = __ldg(cur->base + (long long)b * pitch + nn);
-                            }
-                        }
-                    } else {
-#pragma unroll
-                        for (int e = 0; e < kPx; ++e) S[b][e] = 0.f;
-                    }
+                for (int r = 0; r < kPx; ++r) {
+                    long long nn = n0 + tid + kThreads * r;
+                    nn = nn < 0 ? 0 : (nn > n_pix - 1 ? n_pix - 1 : nn);
+                    S[b][r] = b < n_mu ? __ldg(cur->base + (long long)b * pitch + nn) : 0.f;
                 }
             }
             const float c_first = (float)(cur->c0 + (double)m0), c_last = (float)(cur->c0 + (double)(m0 + L - 1));
-            float cr[kPx];
-#pragma unroll
-            for (int r = 0; r < kPx; ++r) cr[r] = (float)(cur->c0 + (double)(m0 + tid + kThreads * r));
+            // integer shifts of this tile, once per (tile, column): {q0, -q0 as float, q1, -q1 as float} per pair, q = kFlipQ
+            // when the shift changes inside the tile (per-pixel path).  Read after the loop's first barrier.
+            for (int pp = k + tid; pp < k_end; pp += kThreads) {
+                const float a0 = hsm[pp].a0, a1 = hsm[pp].a1;
+                const float qf0 = floorf(a0 * c_first), qf1 = floorf(a1 * c_first);
+                const bool steady = qf0 == floorf(a0 * c_last) && qf1 == floorf(a1 * c_last);
+                int q0 = (int)qf0, q1 = (int)qf1;
+                q0 = max(-(H - 1), min(H - 2, q0));
+                q1 = max(-(H - 1), min(H - 2, q1));
+                qtab[pp] = make_int4(steady ? q0 : kFlipQ, __float_as_int(-(float)q0), q1, __float_as_int(-(float)q1));
+            }
+            const float c_mine = (float)(cur->c0 + (double)(m0 + tid));  // c of output pixel r: c_mine + 512 r (exact: integers < 2^24)
             const int nvalid = L - tid <= 0 ? 0 : (L - tid + kThreads - 1) / kThreads;  // output pixels of this thread (<= 4)
-            float2 A[kPx];
-            double tot[kPx];
+            float2 A[kPx];  // .x: even columns, .y: odd columns
 #pragma unroll
             for (int r = 0; r < kPx; ++r) {
                 A[r] = make_float2(0.f, 0.f);
-                tot[r] = 0.0;
+                tot_s[tid + kThreads * r] = 0.0;  // only this thread touches these four totals
             }
+            // Quad q (pairs kq, kq + 1) is computed into T buffer (it + q) & 1 and interpolated one barrier later.  Between two
+            // barriers a warp has two independent pieces of work - the lerp phase of quad q (shared-memory bound) and the
+            // compute phase of quad q + 1 (FP32-pipe bound) - and the two halves of every SM sub-partition's warps take
+            // them in opposite order, so that the two phases overlap instead of alternating CTA-wide.
+            const bool lerp_first = kAlternate && ((tid >> 7) & 1) != 0;  // warps 4-7 and 12-15: two of the four warps of each sub-partition
+            auto compute_quad = [&](int kk, float *buf) {
+                // (T_j .. T_j+3)[r] = sum_b W[j..j+3, b] S_b[r]
+                const int nl0 = hsm[kk].nl, nl1 = kk + 1 < k_end ? hsm[kk + 1].nl : 0;
+                const int nl = max(nl0, nl1);
+                float2 TU[2][kPx];
+#pragma unroll
+                for (int r = 0; r < kPx; ++r) TU[0][r] = TU[1][r] = make_float2(0.f, 0.f);
+                const float4 *w0 = reinterpret_cast<const float4 *>(Wsm + (size_t)kk * NB);
+                const float4 *w1 = reinterpret_cast<const float4 *>(Wsm + (size_t)(kk + 1) * NB);
+                const int step = (nl + 1) >> 1;  // variants of 2, 4, ... weight loads per pair
+                if (NB >= 4 && step <= 1) composite_columns<NB, (2 < NB / 2 ? 2 : NB / 2)>(S, w0, w1, TU);
+                else if (NB >= 8 && step == 2) composite_columns<NB, (4 < NB / 2 ? 4 : NB / 2)>(S, w0, w1, TU);
+                else if (NB >= 12 && step == 3) composite_columns<NB, (6 < NB / 2 ? 6 : NB / 2)>(S, w0, w1, TU);
+                else if (NB >= 16 && step == 4) composite_columns<NB, (8 < NB / 2 ? 8 : NB / 2)>(S, w0, w1, TU);
+                else if (NB >= 20 && step == 5) composite_columns<NB, (10 < NB / 2 ? 10 : NB / 2)>(S, w0, w1, TU);
+                else composite_columns<NB, NB / 2>(S, w0, w1, TU);
+#pragma unroll
+                for (int r = 0; r < kPx; ++r) {
+                    buf[0 * kSpan + tid + kThreads * r] = TU[0][r].x;
+                    buf[1 * kSpan + tid + kThreads * r] = TU[0][r].y;
+                    buf[2 * kSpan + tid + kThreads * r] = TU[1][r].x;
+                    buf[3 * kSpan + tid + kThreads * r] = TU[1][r].y;
+                }
+            };
+            auto lerp_quad = [&](int kk, const float *buf) {
+                // A[r] += lerp(T_j; m + a_j c_m) for the (up to) four columns
+#pragma unroll
+                for (int pr = 0; pr < 2; ++pr) {
+                    if (pr == 1 && kk + 1 >= k_end) break;  // the second pair belongs to the next CTA
+                    const float a0 = hsm[kk + pr].a0, a1 = hsm[kk + pr].a1;
+                    const float *b0 = buf + (2 * pr) * kSpan + H + tid, *b1 = b0 + kSpan;
+                    const int4 qq = qtab[kk + pr];
+                    if (qq.x != kFlipQ) {
+                        const float2 aa = make_float2(a0, a1), nq = make_float2(__int_as_float(qq.y), __int_as_float(qq.w));
+                        const float *w0p = b0 + qq.x, *w1p = b1 + qq.z;
+#pragma unroll
+                        for (int r = 0; r < kPx; ++r) {
+                            if (r < nvalid) {
+                                const float2 x0 = make_float2(w0p[kThreads * r], w1p[kThreads * r]);
+                                const float2 x1 = make_float2(w0p[kThreads * r + 1], w1p[kThreads * r + 1]);
+                                const float2 tt = fma2(aa, bcast2(c_mine + (float)(kThreads * r)), nq);
+                                const float2 d = fma2(bcast2(-1.f), x0, x1);
+                                A[r] = add2(fma2(tt, d, A[r]), x0);
+                            }
+                        }
+                    } else {  // an integer shift changes inside the tile: per-pixel floor
+#pragma unroll
+                        for (int r = 0; r < kPx; ++r) {
+                            if (r < nvalid) {
+                                const float cr = c_mine + (float)(kThreads * r);
+                                const float q0f = floorf(a0 * cr), q1f = floorf(a1 * cr);
+                                const float t0 = fmaf(a0, cr, -q0f), t1 = fmaf(a1, cr, -q1f);
+                                int q0 = (int)q0f, q1 = (int)q1f;
+                                q0 = max(-(H - 1), min(H - 2, q0));
+                                q1 = max(-(H - 1), min(H - 2, q1));
+                                const float x00 = b0[kThreads * r + q0], x01 = b0[kThreads * r + q0 + 1];
+                                const float x10 = b1[kThreads * r + q1], x11 = b1[kThreads * r + q1 + 1];
+                                A[r].x += fmaf(t0, x01 - x00, x00);
+                                A[r].y += fmaf(t1, x11 - x10, x10);
+                            }
+                        }
+                    }
+                }
+            };
             int since_fold = 0;
-            for (int kk = k; kk < k_end; ++kk, ++it) {
-                // ---- compute phase: TU[r] = sum_b (W[j,b], W[j+1,b]) S_b[r]
-                const int4 hraw = *reinterpret_cast<const int4 *>(&hsm[kk]);
-                const float a0 = __int_as_float(hraw.x), a1 = __int_as_float(hraw.y);
-                const int nl = hraw.z;
-                float2 TU[kPx];
-#pragma unroll
-                for (int r = 0; r < kPx; ++r) TU[r] = make_float2(0.f, 0.f);
-                const float4 *wrow = reinterpret_cast<const float4 *>(Wsm + (size_t)kk * NB);
-#pragma unroll
-                for (int l = 0; l < NB / 2; ++l) {
-                    if (l < nl) {
-                        const float4 w = wrow[l];
-#pragma unroll
-                        for (int r = 0; r < kPx; ++r) TU[r] = fma2(make_float2(w.x, w.y), bcast2(S[2 * l][r]), TU[r]);
-#pragma unroll
-                        for (int r = 0; r < kPx; ++r) TU[r] = fma2(make_float2(w.z, w.w), bcast2(S[2 * l + 1][r]), TU[r]);
-                    }
+            compute_quad(k, Tbuf + (it & 1u) * (4 * kSpan));
+            for (int kk = k; kk < k_end; kk += 2, ++it) {
+                __syncthreads();  // quad kk is in its buffer; the other buffer is free
+                float *buf = Tbuf + (it & 1u) * (4 * kSpan), *nxt = Tbuf + ((it + 1u) & 1u) * (4 * kSpan);
+                const bool more = kk + 2 < k_end;
+                if (lerp_first) {
+                    lerp_quad(kk, buf);
+                    if (more) compute_quad(kk + 2, nxt);
+                } else {
+                    if (more) compute_quad(kk + 2, nxt);
+                    lerp_quad(kk, buf);
                 }
-                float2 *buf = Tbuf + (it & 1u) * kSpan;
-                reinterpret_cast<float4 *>(buf)[2 * tid] = make_float4(TU[0].x, TU[0].y, TU[1].x, TU[1].y);
-                reinterpret_cast<float4 *>(buf)[2 * tid + 1] = make_float4(TU[2].x, TU[2].y, TU[3].x, TU[3].y);
-                __syncthreads();
-                // ---- lerp phase: acc += lerp(T_j; m + a_j c_m) for both columns
-                const float qf0 = floorf(a0 * c_first), qf1 = floorf(a1 * c_first);
-                const bool steady = qf0 == floorf(a0 * c_last) && qf1 == floorf(a1 * c_last);
-                if (steady) {
-                    int q0 = (int)qf0, q1 = (int)qf1;
-                    q0 = max(-(H - 1), min(H - 2, q0));
-                    q1 = max(-(H - 1), min(H - 2, q1));
-                    const float2 aa = make_float2(a0, a1), nq = make_float2(-(float)q0, -(float)q1);
-                    if (q0 == q1) {
-                        const float2 *w0 = buf + H + tid + q0;
-#pragma unroll
-                        for (int r = 0; r < kPx; ++r) {
-                            if (r < nvalid) {
-                                const float2 x0 = w0[kThreads * r], x1 = w0[kThreads * r + 1];
-                                const float2 tt = fma2(aa, bcast2(cr[r]), nq);
-                                const float2 d = fma2(bcast2(-1.f), x0, x1);
-                                A[r] = add2(fma2(tt, d, A[r]), x0);
-                            }
-                        }
-                    } else {
-                        const float *w0 = reinterpret_cast<const float *>(buf + H + tid + q0);
-                        const float *w1 = reinterpret_cast<const float *>(buf + H + tid + q1) + 1;
-#pragma unroll
-                        for (int r = 0; r < kPx; ++r) {
-                            if (r < nvalid) {
-                                const float2 x0 = make_float2(w0[2 * kThreads * r], w1[2 * kThreads * r]);
-                                const float2 x1 = make_float2(w0[2 * kThreads * r + 2], w1[2 * kThreads * r + 2]);
-                                const float2 tt = fma2(aa, bcast2(cr[r]), nq);
-                                const float2 d = fma2(bcast2(-1.f), x0, x1);
-                                A[r] = add2(fma2(tt, d, A[r]), x0);
-                            }
-                        }
-                    }
-                } else {  // an integer shift changes inside the tile: per-pixel floor
-                    const float *bf = reinterpret_cast<const float *>(buf + H + tid);
+                if (++since_fold == kFoldPairs / 2) {
 #pragma unroll
                     for (int r = 0; r < kPx; ++r) {
-                        if (r < nvalid) {
-                            const float q0f = floorf(a0 * cr[r]), q1f = floorf(a1 * cr[r]);
-                            const float t0 = fmaf(a0, cr[r], -q0f), t1 = fmaf(a1, cr[r], -q1f);
-                            int q0 = (int)q0f, q1 = (int)q1f;
-                            q0 = max(-(H - 1), min(H - 2, q0));
-                            q1 = max(-(H - 1), min(H - 2, q1));
-                            const float x00 = bf[2 * (kThreads * r + q0)], x01 = bf[2 * (kThreads * r + q0) + 2];
-                            const float x10 = bf[2 * (kThreads * r + q1) + 1], x11 = bf[2 * (kThreads * r + q1) + 3];
-                            A[r].x += fmaf(t0, x01 - x00, x00);
-                            A[r].y += fmaf(t1, x11 - x10, x10);
-                        }
-                    }
-                }
-                if (++since_fold == kFoldPairs) {
-#pragma unroll
-                    for (int r = 0; r < kPx; ++r) {
-                        tot[r] += (double)(A[r].x + A[r].y);
+                        tot_s[tid + kThreads * r] += (double)(A[r].x + A[r].y);
                         A[r] = make_float2(0.f, 0.f);
                     }
                     since_fold = 0;
                 }
             }
+            double tot[kPx];
 #pragma unroll
-            for (int r = 0; r < kPx; ++r) tot[r] += (double)(A[r].x + A[r].y);
+            for (int r = 0; r < kPx; ++r) tot[r] = tot_s[tid + kThreads * r] + (double)(A[r].x + A[r].y);
 
             // ---- a6: store.  A tile wholly inside this CTA's range goes straight out; otherwise the shares are added
             // in CTA order by the last CTA to deliver.
@@ -360,7 +386,7 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
             const bool vec_ok = (reinterpret_cast<uintptr_t>(out) & 15) == 0;
             __syncthreads();  // every lerp of this segment has read its T buffer
             if (whole) {
-                float *stage = reinterpret_cast<float *>(Tbuf);
+                float *stage = Tbuf;
 #pragma unroll
                 for (int r = 0; r < kPx; ++r) stage[tid + kThreads * r] = (float)tot[r];
                 __syncthreads();

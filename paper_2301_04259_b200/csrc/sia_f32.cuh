@@ -499,15 +499,20 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     const int base0 = H + tid;  // smem position of pixel r = 0 at zero shift
     long long m_t0 = 0;
     float cmf = 0.f;      // lambda0/k + m of this thread's first pixel
-    float2 acc[kR / 2];   // pair k = pixels r = 2k, 2k + 1: the operands of one packed FMA
+    // W lerp = W (s + t d), t = a c - q  ==>  W u + c (W a) d  with u = s - q d: the per-pixel factor c = lambda0/k + m is
+    // pulled out of the sum over entries.  acc1 collects W u, acc2 collects (W a) d; pair k = pixels r = 2k, 2k + 1 (the
+    // operands of one packed FMA).  A fold adds acc1 + c acc2 to the fp64 totals.
+    float2 acc1[kR / 2], acc2[kR / 2];
     double tot[kR];
     int cnt = 0, cur_kind = 0;
     auto fold = [&]() {
 #pragma unroll
         for (int k = 0; k < kR / 2; ++k) {
-            tot[2 * k] += (double)acc[k].x;
-            tot[2 * k + 1] += (double)acc[k].y;
-            acc[k] = make_float2(0.f, 0.f);
+            const float c0 = cmf + (float)(kConsumers * 2 * k), c1 = cmf + (float)(kConsumers * (2 * k + 1));
+            tot[2 * k] += (double)fmaf(c0, acc2[k].x, acc1[k].x);
+            tot[2 * k + 1] += (double)fmaf(c1, acc2[k].y, acc1[k].y);
+            acc1[k] = make_float2(0.f, 0.f);
+            acc2[k] = make_float2(0.f, 0.f);
         }
         cnt = 0;
     };
@@ -559,11 +564,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             m_t0 = desc->m_t0;
             cmf = (float)(p.c0 + (double)(m_t0 + tid));
 #pragma unroll
-            for (int r = 0; r < kR; ++r) {
-                if (r & 1) acc[r / 2].y = 0.f;
-                else acc[r / 2].x = 0.f;
-                tot[r] = 0.0;
-            }
+            for (int r = 0; r < kR; ++r) tot[r] = 0.0;
+#pragma unroll
+            for (int k = 0; k < kR / 2; ++k) acc1[k] = acc2[k] = make_float2(0.f, 0.f);
             cnt = 0;
             if (ACTIVE) {
                 const long long rem = p.out_hi - (m_t0 + tid);
@@ -594,26 +597,23 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                     int qi = (int)q;
                     qi = max(-H, min(H + 2, qi));
                     const float s0 = rs[base0 + kConsumers * r + qi], s1 = rs[base0 + kConsumers * r + qi + 1];
-                    float &ar = (r & 1) ? acc[r / 2].y : acc[r / 2].x;
+                    float &ar = (r & 1) ? acc1[r / 2].y : acc1[r / 2].x;
                     ar = fmaf(en.y, fmaf(t, s1 - s0, s0), ar);
                 }
                 if (++cnt >= kFold) fold();
                 continue;
             }
-            // W lerp = W u + (W a) v with u = s - q d and v = c d: u_r, v_r are per-pixel registers of the run
+            // u = s - q d and d = s[+1] - s are per-pixel registers of the run
             float2 u[kR / 2], v[kR / 2];
             {
                 const float *wv = rs + base0 + run.y;
                 const float2 nq = bcast2(-(float)run.y);
-                float2 c = make_float2(cmf, cmf + (float)kConsumers);
 #pragma unroll
                 for (int k = 0; k < kR / 2; ++k) {
                     const float2 s0 = make_float2(wv[kConsumers * 2 * k], wv[kConsumers * (2 * k + 1)]);
                     const float2 s1 = make_float2(wv[kConsumers * 2 * k + 1], wv[kConsumers * (2 * k + 1) + 1]);
-                    const float2 d = fma2(bcast2(-1.f), s0, s1);
-                    u[k] = fma2(nq, d, s0);
-                    v[k] = fma2(c, d, bcast2(0.f));
-                    c = add2(c, bcast2((float)(2 * kConsumers)));  // rounding of c moves the shift by < 1e-6 px
+                    v[k] = fma2(bcast2(-1.f), s0, s1);
+                    u[k] = fma2(nq, v[k], s0);
                 }
             }
             const int len = p.collapse ? 1 : nxt - run.x;
@@ -623,9 +623,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             for (int i = 0; i < len; ++i) {
                 const float2 nx = re[i + 1];  // one past the run's end is still inside the stage
 #pragma unroll
-                for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.x), u[k], acc[k]);  // (1) + W u_r
+                for (int k = 0; k < kR / 2; ++k) acc1[k] = fma2(bcast2(rc.x), u[k], acc1[k]);  // (1) + W u_r
 #pragma unroll
-                for (int k = 0; k < kR / 2; ++k) acc[k] = fma2(bcast2(rc.y), v[k], acc[k]);  // (2) + W a v_r
+                for (int k = 0; k < kR / 2; ++k) acc2[k] = fma2(bcast2(rc.y), v[k], acc2[k]);  // (2) + (W a) d_r
                 rc = nx;
             }
             cnt += len;
