@@ -61,8 +61,9 @@ enum soap_effect { SOAP_EFFECT_TOTAL = 0, SOAP_EFFECT_FLUX = 1, SOAP_EFFECT_CB =
 /* How the shift-interpolate-accumulate sum is evaluated.  All forms compute the same sums (Alg. 1,
  * Eq. 3) and differ only in rounding order. */
 enum soap_form {
-    SOAP_FORM_AUTO = 0,   /* library picks: SOAP_FORM_BINNED for solid-body rotation; under differential rotation
-                             (diff_rot != 0) one entry per cell with the run collapse of SOAP_FORM_FIR */
+    SOAP_FORM_AUTO = 0,   /* library picks.  Solid-body rotation: SOAP_FORM_COMPOSITE (quiet spectrum of fp32 tables with
+                             n_mu <= 24; binned entries for everything else).  Differential rotation (diff_rot != 0):
+                             one entry per cell with the run collapse of SOAP_FORM_FIR */
     SOAP_FORM_BINNED = 1, /* cells pre-binned by (column, mu-bin): all cells of a column share one
                              velocity under solid-body rotation (BASELINE.json north_star) */
     SOAP_FORM_CELLS = 2,  /* one entry per visible cell - the literal double loop of Alg. 1 */
@@ -136,7 +137,8 @@ typedef struct {
                                      counting the quiet-row and the active-row entry of a pair separately */
     int64_t active_cells;         /* sum over phases of covered cells */
     int32_t quiet_splits, tile_px;
-    int32_t form;                 /* enum soap_form actually used */
+    int32_t form;                 /* enum soap_form the last soap_integrate_quiet actually ran (the form selected by
+                                     soap_disk_geometry when no quiet spectrum has been computed yet) */
     int32_t launches;             /* kernels launched by this handle since soap_create */
     float quiet_kernel_ms;        /* SOAP_OPT_KERNEL_TIMING: device time of the last quiet / active */
     float active_kernel_ms;       /*   shift-interpolate-accumulate kernel launch; else 0 */

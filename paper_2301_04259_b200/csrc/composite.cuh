@@ -10,23 +10,30 @@
 // the same as slow ones ("composite-column form").
 //
 //   * A CTA of 512 threads holds a span of 2048 source pixels of EVERY mu-bin row in registers (thread i: pixels
-//     n0 + 4 i .. + 3 of each row, one LDG.128 per row): 20 bins x 2048 px = 62 % of the SM's register file.  The
-//     span is an output tile of L = 2048 - 2 H pixels plus the halo H the shifts can reach on either side.
-//   * Columns are taken two at a time.  Compute phase: TU[r] = (T_j, T_j+1)[pixel r] accumulates
-//     (W[j,b], W[j+1,b]) * S_b[r] with packed FFMA2 (the weight pair is one LDS.128-broadcast operand, the sample a
-//     scalar-broadcast register): 4 FFMA2 per bin per thread.  The pair is written to shared memory interleaved as
-//     float2 (double-buffered: one CTA barrier per column pair).
-//   * Lerp phase: thread i owns output pixels m0 + i + 512 r (conflict-free LDS.64, two columns per load):
-//     t = a_j c_m - q_j, acc += x0 + t (x1 - x0): 4 packed instructions per (column pair, pixel).  The integer
-//     shift q_j is constant over the tile for ~99 % of the columns (checked per pair); the rest take a per-pixel
-//     floor.  Only the shift delta = a_j (lambda0/k + m) is formed in fp32, never the absolute source coordinate.
-//   * fp32 column sums are folded into fp64 every kFoldPairs pairs; fp64 totals are rounded once on store.
+//     n0 + i + 512 r of each row): 20 bins x 2048 px = 62 % of the SM's register file.  The span is an output tile of
+//     L = 2048 - 2 H pixels plus the halo H the shifts can reach on either side.
+//   * Columns are taken four at a time (a "quad" = two column pairs).  Compute phase: TU[r] = (T_j, T_j+1)[pixel r]
+//     accumulates (W[j,b], W[j+1,b]) * S_b[r] with packed FFMA2 (the weight pair is half of an LDS.128-broadcast, the
+//     sample a scalar-broadcast register): 4 FFMA2 per (pair, bin) per thread, straight-line per number of bins
+//     present.  Column j's composite is stored to a shared-memory plane SHIFTED by the column's integer shift q_j of
+//     this tile (source pixel n lands at output position n - H - q_j; conflict-free scalar stores), double-buffered:
+//     one CTA barrier per quad.
+//   * Lerp phase: thread i owns the four ADJACENT output pixels m0 + 4 i .. + 3; because of the shifted store the two
+//     samples of output pixel o sit at positions o, o + 1 whatever the shift, so a column costs one aligned LDS.128 and
+//     one LDS.32: t = a_j c_m - q_j, acc += x0 + t (x1 - x0).  q_j is constant over the tile for ~99 % of the columns
+//     (a per-tile table, built once per segment); the rest take a per-pixel floor relative to the stored shift.  Only
+//     the shift delta = a_j (lambda0/k + m) is formed in fp32, never the absolute source coordinate.
+//   * fp32 column sums are folded into fp64 registers every kFoldPairs pairs; fp64 totals are rounded once on store.
 //   * Work = the flattened (star, tile, column pair) list with a cost per pair (bins present + the lerp), cut into
 //     equal contiguous ranges, one per CTA (one wave, any number of tiles / stars per CTA, or many CTAs per tile
-//     when the spectrum is short).  A tile wholly inside one CTA's range is stored directly (STG.128 after a
-//     shared-memory transpose); a shared tile's fp64 partial sums are added in CTA order by the last CTA to
-//     deliver (atomic ticket, self-resetting): run-to-run identical.
+//     when the spectrum is short).  A tile wholly inside one CTA's range is stored directly (STG.128); a shared
+//     tile's fp64 partial sums are added in CTA order by the last CTA to deliver (atomic ticket, self-resetting):
+//     run-to-run identical.
 //   * Batch (config 5): the same launch walks an array of stars (soap_batch_integrate_quiet).
+//   * What bounds it (measured by switching phases off, C3: compute 70 us + lerp 37 us + loads / barriers / store 27 us
+//     = 133 us, additive): the shared-memory pipe.  Every thread must receive every weight (4 554 words per tile and
+//     thread, 164 KB per quad and SM = 1 280 cycles at 128 B/clk) beside the FFMA2 (1 536 cycles per quad): with 4
+//     pixels per thread - what the register file allows - the form is co-bound by LDS bandwidth and the FP32 pipe.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -37,13 +44,13 @@ namespace soap {
 namespace comp {
 
 constexpr int kThreads = 512;
+constexpr int kCtasPerSm = 512 / kThreads;  // the register-resident spans fill the register file (2 x 256 and 4 x 128
+                                            // threads were measured: within 3 %)
 constexpr int kPx = 4;                 // source pixels per thread and mu-bin
 constexpr int kSpan = kThreads * kPx;  // source pixels per CTA span
 constexpr int kFoldPairs = 4;          // fp32 -> fp64 fold interval (column pairs = 8 columns)
 constexpr int kMaxBins = 24;           // mu bins the register-resident form can hold
 constexpr int kMaxStars = 256;         // stars per launch
-constexpr int kFlipQ = -(1 << 30);      // shift-table marker: the integer shift changes inside the tile
-constexpr bool kAlternate = false;    // halves of the warps take the two phases in opposite order (measured: slower)
 constexpr int kPairCostBase = 24;      // cost model: 8 FFMA2-slots per weight load + the lerp, barrier and loop
 
 struct PairHdr {  // one column pair (2p, 2p+1); entry [n_pairs] carries the total cost in cost0
@@ -69,11 +76,13 @@ struct Params {
     int n_stars;
     double *partial;     // [gridDim.x][2][kSpan]
     int max_pairs;       // shared-memory table capacity
+    int plane;           // plane_floats(largest halo of the launch)
 };
 
-__host__ __device__ inline size_t smem_bytes(int nb, int max_pairs) {
-    return (size_t)2 * 4 * kSpan * sizeof(float) + (size_t)kSpan * sizeof(double) + (size_t)(max_pairs + 1) * nb * sizeof(float2) +
-           (size_t)(max_pairs + 2) * sizeof(PairHdr) + (size_t)(max_pairs + 1) * sizeof(int4) +
+__host__ __device__ inline int plane_floats(int max_halo) { return kSpan + 2 * max_halo + 8; }  // multiple of 4
+__host__ __device__ inline size_t smem_bytes(int nb, int max_pairs, int max_halo) {
+    return (size_t)2 * 4 * plane_floats(max_halo) * sizeof(float) + (size_t)(max_pairs + 1) * nb * sizeof(float2) +
+           (size_t)(max_pairs + 2) * sizeof(PairHdr) + (size_t)(max_pairs + 2) * sizeof(int4) +
            (size_t)(kMaxStars + 1) * sizeof(long long) + sizeof(Star) + 64;
 }
 
@@ -145,15 +154,14 @@ __device__ __forceinline__ void composite_columns(const float (&S)[NB][kPx], con
 }
 
 template <int NB>
-__global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Params p) {
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) composite_quiet_kernel(const Params p) {
     static_assert(NB % 4 == 0 && NB <= kMaxBins, "bins are loaded two per LDS.128 and unrolled four at a time");
     extern __shared__ __align__(16) unsigned char smem[];
-    float *Tbuf = reinterpret_cast<float *>(smem);                                    // [2 buffers][4 columns][kSpan]
-    double *tot_s = reinterpret_cast<double *>(Tbuf + 2 * 4 * kSpan);                 // [kSpan] fp64 totals of the tile
-    float2 *Wsm = reinterpret_cast<float2 *>(tot_s + kSpan);                          // [max_pairs + 1][NB]
+    float *Tbuf = reinterpret_cast<float *>(smem);                                    // [2 buffers][4 columns][plane]
+    float2 *Wsm = reinterpret_cast<float2 *>(Tbuf + 2 * 4 * p.plane);                 // [max_pairs + 1][NB]
     PairHdr *hsm = reinterpret_cast<PairHdr *>(Wsm + (size_t)(p.max_pairs + 1) * NB);  // [max_pairs + 2]
-    int4 *qtab = reinterpret_cast<int4 *>(hsm + p.max_pairs + 2);                     // [max_pairs + 1] shifts of the current tile
-    long long *unit0 = reinterpret_cast<long long *>(qtab + p.max_pairs + 1);         // [n_stars + 1]
+    int4 *qtab = reinterpret_cast<int4 *>(hsm + p.max_pairs + 2);                     // [max_pairs + 2] shifts of the current tile
+    long long *unit0 = reinterpret_cast<long long *>(qtab + p.max_pairs + 2);         // [n_stars + 1]
     Star *cur = reinterpret_cast<Star *>(unit0 + kMaxStars + 1);
     int *ctl = reinterpret_cast<int *>(cur + 1);                                      // last-CTA flag
 
@@ -251,7 +259,8 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
             const int H = cur->halo, L = cur->L, n_mu = cur->n_mu;
             const long long n_pix = cur->n_pix, pitch = cur->pitch;
             const long long m0 = t * (long long)L, n0 = m0 - H;
-            // ---- the span of every mu-bin row -> registers: thread i holds source pixels n0 + i + 512 r
+            const int plane = p.plane;  // floats per column plane of a T buffer: kSpan + 2 H_max + 8
+            // ---- the span of every mu-bin row -> registers: thread i holds source pixels n0 + i + kThreads r
             // (clamp-to-edge outside the grid, reading S8)
             float S[NB][kPx];
 #pragma unroll
@@ -264,30 +273,28 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
                 }
             }
             const float c_first = (float)(cur->c0 + (double)m0), c_last = (float)(cur->c0 + (double)(m0 + L - 1));
-            // integer shifts of this tile, once per (tile, column): {q0, -q0 as float, q1, -q1 as float} per pair, q = kFlipQ
-            // when the shift changes inside the tile (per-pixel path).  Read after the loop's first barrier.
+            // Integer shifts of this tile, once per (tile, column pair): {qs0, qs1, steady flags, 0}.  Column j's composite is
+            // STORED shifted by qs_j (source pixel n lands at output position n - H - qs_j), so the lerp phase reads the two
+            // samples of output pixel o at positions o, o + 1 whatever the shift: aligned 16-byte loads of adjacent pixels.
+            // qs_j = floor(a_j c) at the tile's first pixel; "steady" = the same at its last pixel (else a per-pixel path
+            // corrects by floor(a_j c_o) - qs_j).  Read after the loop's first barrier.
             for (int pp = k + tid; pp < k_end; pp += kThreads) {
                 const float a0 = hsm[pp].a0, a1 = hsm[pp].a1;
                 const float qf0 = floorf(a0 * c_first), qf1 = floorf(a1 * c_first);
-                const bool steady = qf0 == floorf(a0 * c_last) && qf1 == floorf(a1 * c_last);
+                const int steady = (qf0 == floorf(a0 * c_last) ? 1 : 0) | (qf1 == floorf(a1 * c_last) ? 2 : 0);
                 int q0 = (int)qf0, q1 = (int)qf1;
                 q0 = max(-(H - 1), min(H - 2, q0));
                 q1 = max(-(H - 1), min(H - 2, q1));
-                qtab[pp] = make_int4(steady ? q0 : kFlipQ, __float_as_int(-(float)q0), q1, __float_as_int(-(float)q1));
+                qtab[pp] = make_int4(q0, q1, steady, 0);
             }
-            const float c_mine = (float)(cur->c0 + (double)(m0 + tid));  // c of output pixel r: c_mine + 512 r (exact: integers < 2^24)
-            const int nvalid = L - tid <= 0 ? 0 : (L - tid + kThreads - 1) / kThreads;  // output pixels of this thread (<= 4)
-            float2 A[kPx];  // .x: even columns, .y: odd columns
+            if (tid == 0) qtab[k_end] = make_int4(0, 0, 3, 0);  // the pair after the last (computed, never interpolated)
+            // output pixels of this thread: o = 4 tid .. 4 tid + 3 (adjacent: one LDS.128 pair per column, one STG.128)
+            const bool valid = 4 * tid < L;
+            float c_px[4];
 #pragma unroll
-            for (int r = 0; r < kPx; ++r) {
-                A[r] = make_float2(0.f, 0.f);
-                tot_s[tid + kThreads * r] = 0.0;  // only this thread touches these four totals
-            }
-            // Quad q (pairs kq, kq + 1) is computed into T buffer (it + q) & 1 and interpolated one barrier later.  Between two
-            // barriers a warp has two independent pieces of work - the lerp phase of quad q (shared-memory bound) and the
-            // compute phase of quad q + 1 (FP32-pipe bound) - and the two halves of every SM sub-partition's warps take
-            // them in opposite order, so that the two phases overlap instead of alternating CTA-wide.
-            const bool lerp_first = kAlternate && ((tid >> 7) & 1) != 0;  // warps 4-7 and 12-15: two of the four warps of each sub-partition
+            for (int e = 0; e < 4; ++e) c_px[e] = (float)(cur->c0 + (double)(m0 + 4 * tid + e));
+            float A[4] = {0.f, 0.f, 0.f, 0.f};
+            double tot[4] = {0.0, 0.0, 0.0, 0.0};
             auto compute_quad = [&](int kk, float *buf) {
                 // (T_j .. T_j+3)[r] = sum_b W[j..j+3, b] S_b[r]
                 const int nl0 = hsm[kk].nl, nl1 = kk + 1 < k_end ? hsm[kk + 1].nl : 0;
@@ -304,79 +311,71 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
                 else if (NB >= 16 && step == 4) composite_columns<NB, (8 < NB / 2 ? 8 : NB / 2)>(S, w0, w1, TU);
                 else if (NB >= 20 && step == 5) composite_columns<NB, (10 < NB / 2 ? 10 : NB / 2)>(S, w0, w1, TU);
                 else composite_columns<NB, NB / 2>(S, w0, w1, TU);
+                // source pixel (local index tid + kThreads r) of column j -> position tid + kThreads r + H - qs_j  (>= 1)
+                const int4 qa = qtab[kk], qb = qtab[kk + 1];
+                float *d0 = buf + 0 * plane + tid + H - qa.x, *d1 = buf + 1 * plane + tid + H - qa.y;
+                float *d2 = buf + 2 * plane + tid + H - qb.x, *d3 = buf + 3 * plane + tid + H - qb.y;
 #pragma unroll
                 for (int r = 0; r < kPx; ++r) {
-                    buf[0 * kSpan + tid + kThreads * r] = TU[0][r].x;
-                    buf[1 * kSpan + tid + kThreads * r] = TU[0][r].y;
-                    buf[2 * kSpan + tid + kThreads * r] = TU[1][r].x;
-                    buf[3 * kSpan + tid + kThreads * r] = TU[1][r].y;
+                    d0[kThreads * r] = TU[0][r].x;
+                    d1[kThreads * r] = TU[0][r].y;
+                    d2[kThreads * r] = TU[1][r].x;
+                    d3[kThreads * r] = TU[1][r].y;
                 }
             };
             auto lerp_quad = [&](int kk, const float *buf) {
-                // A[r] += lerp(T_j; m + a_j c_m) for the (up to) four columns
+                // A[e] += lerp(T_j; m + a_j c_m) for the (up to) four columns; output pixel o reads positions o + 2 H (+ 1)
+                if (!valid) return;
 #pragma unroll
-                for (int pr = 0; pr < 2; ++pr) {
+                for (int cidx = 0; cidx < 4; ++cidx) {
+                    const int pr = cidx >> 1;
                     if (pr == 1 && kk + 1 >= k_end) break;  // the second pair belongs to the next CTA
-                    const float a0 = hsm[kk + pr].a0, a1 = hsm[kk + pr].a1;
-                    const float *b0 = buf + (2 * pr) * kSpan + H + tid, *b1 = b0 + kSpan;
+                    const float a = (cidx & 1) ? hsm[kk + pr].a1 : hsm[kk + pr].a0;
                     const int4 qq = qtab[kk + pr];
-                    if (qq.x != kFlipQ) {
-                        const float2 aa = make_float2(a0, a1), nq = make_float2(__int_as_float(qq.y), __int_as_float(qq.w));
-                        const float *w0p = b0 + qq.x, *w1p = b1 + qq.z;
+                    const int qs = (cidx & 1) ? qq.y : qq.x;
+                    const float *pl = buf + cidx * plane + 2 * H + 4 * tid;
+                    if (qq.z & (1 << (cidx & 1))) {
+                        const float4 v0 = *reinterpret_cast<const float4 *>(pl);
+                        const float x4 = pl[4];
+                        const float nq = -(float)qs;
+                        const float x[5] = {v0.x, v0.y, v0.z, v0.w, x4};
 #pragma unroll
-                        for (int r = 0; r < kPx; ++r) {
-                            if (r < nvalid) {
-                                const float2 x0 = make_float2(w0p[kThreads * r], w1p[kThreads * r]);
-                                const float2 x1 = make_float2(w0p[kThreads * r + 1], w1p[kThreads * r + 1]);
-                                const float2 tt = fma2(aa, bcast2(c_mine + (float)(kThreads * r)), nq);
-                                const float2 d = fma2(bcast2(-1.f), x0, x1);
-                                A[r] = add2(fma2(tt, d, A[r]), x0);
-                            }
+                        for (int e = 0; e < 4; ++e) {
+                            const float tt = fmaf(a, c_px[e], nq);
+                            A[e] += fmaf(tt, x[e + 1] - x[e], x[e]);
                         }
-                    } else {  // an integer shift changes inside the tile: per-pixel floor
+                    } else {  // the integer shift changes inside the tile: per-pixel floor, relative to the stored shift
 #pragma unroll
-                        for (int r = 0; r < kPx; ++r) {
-                            if (r < nvalid) {
-                                const float cr = c_mine + (float)(kThreads * r);
-                                const float q0f = floorf(a0 * cr), q1f = floorf(a1 * cr);
-                                const float t0 = fmaf(a0, cr, -q0f), t1 = fmaf(a1, cr, -q1f);
-                                int q0 = (int)q0f, q1 = (int)q1f;
-                                q0 = max(-(H - 1), min(H - 2, q0));
-                                q1 = max(-(H - 1), min(H - 2, q1));
-                                const float x00 = b0[kThreads * r + q0], x01 = b0[kThreads * r + q0 + 1];
-                                const float x10 = b1[kThreads * r + q1], x11 = b1[kThreads * r + q1 + 1];
-                                A[r].x += fmaf(t0, x01 - x00, x00);
-                                A[r].y += fmaf(t1, x11 - x10, x10);
-                            }
+                        for (int e = 0; e < 4; ++e) {
+                            const float qf = floorf(a * c_px[e]);
+                            const float tt = fmaf(a, c_px[e], -qf);
+                            int q = (int)qf;
+                            q = max(-(H - 1), min(H - 2, q));
+                            const float x0 = pl[e + q - qs], x1 = pl[e + q - qs + 1];
+                            A[e] += fmaf(tt, x1 - x0, x0);
                         }
                     }
                 }
             };
             int since_fold = 0;
-            compute_quad(k, Tbuf + (it & 1u) * (4 * kSpan));
+            __syncthreads();  // the shift table is complete
+            compute_quad(k, Tbuf + (it & 1u) * (4 * plane));
             for (int kk = k; kk < k_end; kk += 2, ++it) {
                 __syncthreads();  // quad kk is in its buffer; the other buffer is free
-                float *buf = Tbuf + (it & 1u) * (4 * kSpan), *nxt = Tbuf + ((it + 1u) & 1u) * (4 * kSpan);
-                const bool more = kk + 2 < k_end;
-                if (lerp_first) {
-                    lerp_quad(kk, buf);
-                    if (more) compute_quad(kk + 2, nxt);
-                } else {
-                    if (more) compute_quad(kk + 2, nxt);
-                    lerp_quad(kk, buf);
-                }
+                float *buf = Tbuf + (it & 1u) * (4 * plane), *nxt = Tbuf + ((it + 1u) & 1u) * (4 * plane);
+                if (kk + 2 < k_end) compute_quad(kk + 2, nxt);
+                lerp_quad(kk, buf);
                 if (++since_fold == kFoldPairs / 2) {
 #pragma unroll
-                    for (int r = 0; r < kPx; ++r) {
-                        tot_s[tid + kThreads * r] += (double)(A[r].x + A[r].y);
-                        A[r] = make_float2(0.f, 0.f);
+                    for (int e = 0; e < 4; ++e) {
+                        tot[e] += (double)A[e];
+                        A[e] = 0.f;
                     }
                     since_fold = 0;
                 }
             }
-            double tot[kPx];
 #pragma unroll
-            for (int r = 0; r < kPx; ++r) tot[r] = tot_s[tid + kThreads * r] + (double)(A[r].x + A[r].y);
+            for (int e = 0; e < 4; ++e) tot[e] += (double)A[e];
 
             // ---- a6: store.  A tile wholly inside this CTA's range goes straight out; otherwise the shares are added
             // in CTA order by the last CTA to deliver.
@@ -384,33 +383,25 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
             const long long lo = cur->out_lo, hi = cur->out_hi < n_pix ? cur->out_hi : n_pix;
             float *out = cur->out;
             const bool vec_ok = (reinterpret_cast<uintptr_t>(out) & 15) == 0;
-            __syncthreads();  // every lerp of this segment has read its T buffer
+            const long long m = m0 + 4 * tid;
             if (whole) {
-                float *stage = Tbuf;
-#pragma unroll
-                for (int r = 0; r < kPx; ++r) stage[tid + kThreads * r] = (float)tot[r];
-                __syncthreads();
-                const int o = 4 * tid;
-                if (o < L) {
-                    const float4 v = reinterpret_cast<const float4 *>(stage)[tid];
-                    const long long m = m0 + o;
+                if (valid) {
                     if (vec_ok && m >= lo && m + 3 < hi) {
-                        *reinterpret_cast<float4 *>(out + m) = v;
+                        *reinterpret_cast<float4 *>(out + m) = make_float4((float)tot[0], (float)tot[1], (float)tot[2], (float)tot[3]);
                     } else {
-                        const float e[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
                         for (int q = 0; q < 4; ++q)
-                            if (m + q >= lo && m + q < hi) out[m + q] = e[q];
+                            if (m + q >= lo && m + q < hi) out[m + q] = (float)tot[q];
                     }
                 }
-                __syncthreads();  // the stage is a T buffer again
+                __syncthreads();  // every lerp of this segment has read its T buffer and the shift table
             } else {
                 const long long u_last = u_tile + hsm[n_pairs - 1].cost0;
                 const long long g_first = owner_of(u_tile, U, G), g_last = owner_of(u_last, U, G);
                 const int slot = g == g_first ? 1 : 0;  // a CTA's head share (k == 0) and tail share (k > 0) of two tiles
-                double *mine = p.partial + ((size_t)g * 2 + slot) * kSpan;
-#pragma unroll
-                for (int r = 0; r < kPx; ++r) mine[tid + kThreads * r] = tot[r];
+                double *mine = p.partial + ((size_t)g * 2 + slot) * kSpan + 4 * tid;
+                reinterpret_cast<double2 *>(mine)[0] = make_double2(tot[0], tot[1]);
+                reinterpret_cast<double2 *>(mine)[1] = make_double2(tot[2], tot[3]);
                 __threadfence();
                 __syncthreads();
                 if (tid == 0) {
@@ -422,11 +413,28 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
                 __syncthreads();
                 if (ctl[0]) {
                     __threadfence();
-                    const int o = 4 * tid;
-                    if (o < L) {
+                    if (valid) {
                         double sum[4] = {0.0, 0.0, 0.0, 0.0};
-                        for (long long c = g_first; c <= g_last; ++c) {
-                            const double *src = p.partial + ((size_t)c * 2 + (c == g_first ? 1 : 0)) * kSpan + o;
+                        const double *src0 = p.partial + 4 * tid;
+                        long long c = g_first;
+                        for (; c + 3 <= g_last; c += 4) {  // four shares in flight; added in CTA order
+                            double2 v[4][2];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                const double *src = src0 + ((size_t)(c + u) * 2 + ((c + u) == g_first ? 1 : 0)) * kSpan;
+                                v[u][0] = __ldcg(reinterpret_cast<const double2 *>(src));
+                                v[u][1] = __ldcg(reinterpret_cast<const double2 *>(src) + 1);
+                            }
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                sum[0] += v[u][0].x;
+                                sum[1] += v[u][0].y;
+                                sum[2] += v[u][1].x;
+                                sum[3] += v[u][1].y;
+                            }
+                        }
+                        for (; c <= g_last; ++c) {
+                            const double *src = src0 + ((size_t)c * 2 + (c == g_first ? 1 : 0)) * kSpan;
                             const double2 v0 = __ldcg(reinterpret_cast<const double2 *>(src));
                             const double2 v1 = __ldcg(reinterpret_cast<const double2 *>(src) + 1);
                             sum[0] += v0.x;
@@ -434,7 +442,6 @@ __global__ void __launch_bounds__(kThreads, 1) composite_quiet_kernel(const Para
                             sum[2] += v1.x;
                             sum[3] += v1.y;
                         }
-                        const long long m = m0 + o;
                         if (vec_ok && m >= lo && m + 3 < hi) {
                             *reinterpret_cast<float4 *>(out + m) = make_float4((float)sum[0], (float)sum[1], (float)sum[2], (float)sum[3]);
                         } else {
