@@ -112,11 +112,34 @@ __device__ __forceinline__ int column_candidates(const RegionAtPhase *reg, int n
 
 // grid = n_phases * kPrepCluster, block = kPrepThreads, cluster = kPrepCluster CTAs;
 // dynamic shared memory = prep_smem_bytes(n_mu, chunk_cols) with chunk_cols >= ceil(N / kPrepCluster).
+// Batch form (soap_batch_active_timeseries): `many` = DEVICE [n_stars] arguments, `phase0` = DEVICE [n_stars + 1] first
+// cluster (phase) of every star; cluster c serves phase c - phase0[s] of the star s that holds it.  many == nullptr: `one`.
 template <typename EntT>
-__global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThreads) active_prepare_kernel(const PrepArgs a) {
+__global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThreads)
+active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, const int *__restrict__ phase0, int n_stars) {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) unsigned char prep_smem[];
+    __shared__ PrepArgs s_args;
+    __shared__ int s_phase;
+    if (threadIdx.x == 0) {
+        const int c = blockIdx.x / kPrepCluster;
+        if (many) {
+            int lo = 0, hi = n_stars - 1;  // last star with phase0[s] <= c
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (__ldg(&phase0[mid]) <= c) lo = mid;
+                else hi = mid - 1;
+            }
+            s_args = many[lo];
+            s_phase = c - __ldg(&phase0[lo]);
+        } else {
+            s_args = one;
+            s_phase = c;
+        }
+    }
+    __syncthreads();
+    const PrepArgs &a = s_args;
     const int n_seg = 3 * a.n_mu, N = a.N, cc = a.chunk_cols;
     __shared__ int s_cand[kPrepThreads / 32][kCandCap];            // per warp: regions that can reach its column
     double *WDs = reinterpret_cast<double *>(prep_smem);           // [n_seg][cc]: this CTA's columns
@@ -125,7 +148,7 @@ __global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThre
     int *tot = off + n_seg;                                         // [n_seg] entries of the whole phase
     int *s_misc = tot + n_seg;  // j_lo, j_hi, covered cells of this CTA (read by rank 0), last-phase flag
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = kPrepThreads / 32;
-    const int p = blockIdx.x / kPrepCluster;
+    const int p = s_phase;
     const int rank = (int)cluster.block_rank();
     const RegionAtPhase *reg = a.rp + (size_t)p * a.n_regions;
     EntT *ent = static_cast<EntT *>(a.ent) + (size_t)p * n_seg * a.seg_cap;
@@ -151,7 +174,17 @@ __global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThre
     const int per = (j_hi >= j_lo) ? (j_hi - j_lo + kPrepCluster) / kPrepCluster : 0;  // columns per CTA, <= cc
     const int c0 = j_lo + rank * per;
     const int cols = max(0, min(per, j_hi + 1 - c0));
-
+    if (j_hi < j_lo && a.n_phases > 1) {
+        // No region of this phase faces the observer (every CTA of the cluster sees the same j_lo, j_hi): an empty phase.
+        // Rank 0 records it and takes part in the ordering of the phases; nothing is binned, exchanged or compacted.
+        if (rank != 0) return;
+        for (int s = tid; s < n_seg; s += kPrepThreads) a.seg_count[p * n_seg + s] = 0;
+        if (tid == 0) {
+            a.n_jobs[p] = 0;
+            a.work[p] = 0;
+            a.n_active[p] = 0;
+        }
+    } else {
     for (int s = warp; s < n_seg; s += n_warps)
         for (int k = lane; k < cols; k += 32) WDs[(size_t)s * cc + k] = 0.0;
     __syncthreads();
@@ -320,6 +353,7 @@ __global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThre
             a.n_active[p] = covered;
         }
     }
+    }  // (a phase with visible regions)
     __threadfence();
     __syncthreads();
     if (tid == 0) {

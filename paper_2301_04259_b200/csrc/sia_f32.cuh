@@ -68,7 +68,9 @@ static_assert(kConsumerWarps == 4 && kProducerWarps == 4, "setmaxnreg acts on al
 
 enum : int { kJobFirst = 1, kJobLast = 2, kJobExit = 4 };
 
-struct Params {
+// What a launch needs to know about one star.  The quiet launch carries one as a kernel argument; the active launch
+// reads a DEVICE array of them, one per star of the batch (soap_batch_active_timeseries: ONE launch for all stars).
+struct StarBlock {
     const float *base[3];      // spectrum tables per kind (quiet launch: base[0] only)
     const float *contrast[3];  // per-pixel multiplier per kind or nullptr (== 1); kind 0 unused
     long long pitch, n_pix;
@@ -76,27 +78,51 @@ struct Params {
                                // belong to its neighbours, see soap_synthesize_host)
     long long row_len;         // elements of a row that may be read from its first pixel on (<= pitch; the pitch itself
                                // unless the table is a window into a wider one, see soap_synthesize_host)
+    long long out_pitch;
     double c0;                 // lambda0 / dlambda
-    int n_mu;
+    const float2 *ent;         // raw entries (a_e, W_e)
+    float *out;                // quiet: [n_pix]; active: [n_phases][out_pitch]
+    // active launch
+    const ActiveJob *jobs;     // [n_phases][job_cap]
+    const int *n_jobs;         // [n_phases]
+    const int *phase_order;    // [n_phases] heaviest first
+    long long item0;           // first (phase, tile) item of this star in the launch's item list
     int halo;                  // H: multiple of 4, >= max |delta| + 2
+    int n_mu, n_tiles, job_cap, n_phases, pad;
+};
+static_assert(sizeof(StarBlock) % 16 == 0 && sizeof(StarBlock) <= 192, "producer warps cache a block with 16-byte copies");
+
+constexpr int kMaxBatchStars = 96;   // stars per active launch (their item offsets live in shared memory)
+
+struct Params {
+    StarBlock one;             // quiet launch: the star
+    const StarBlock *many;     // active launch: DEVICE [n_stars]
+    int n_stars;
+    long long n_items;         // active launch: (phase, tile) items of all stars
+    int halo;                  // largest halo of the launch: sizes the stages
     int stage_bytes, raw_off, rec_off, run_off, desc_off;  // stage_layout(halo), filled by set_layout()
     int collapse;              // SOAP_FORM_FIR: a run's entries are summed into one record {sum W, sum W a}
-    const float2 *ent;         // raw entries (a_e, W_e)
-    int n_tiles;
     // quiet launch
     const int *row_start;      // [n_mu + 1] entry offsets (even)
     double *partial;           // [gridDim.x][max_seg][kTile]
     int max_seg;
     int *tile_ticket;          // [n_tiles] shares delivered per tile; zero between launches
     // active launch
-    const ActiveJob *jobs;     // [n_phases][job_cap]
-    const int *n_jobs;         // [n_phases]
-    const int *phase_order;    // [n_phases] heaviest first
     int *item_counters;        // [2] item hand-out (zero between launches)
-    int job_cap, n_phases;
-    float *out;                // [n_phases][out_pitch]
-    long long out_pitch;
+    int item_chunk;            // items a CTA takes per hand-out (1 unless the list is very long: a batch of stars)
 };
+
+// __ldg of a pointer-valued field
+template <typename P>
+__device__ __forceinline__ P *ldg_ptr(P *const *addr) {
+    return reinterpret_cast<P *>(__ldg(reinterpret_cast<const unsigned long long *>(addr)));
+}
+
+template <bool ACTIVE>
+__device__ __forceinline__ const StarBlock &star_block(const Params &p, int star) {
+    if (ACTIVE) return p.many[star];
+    return p.one;
+}
 
 // First unit of CTA c when U units (U even) are cut into G contiguous ranges with even boundaries.
 __host__ __device__ inline long long range_begin(long long c, long long U, long long G) {
@@ -108,7 +134,12 @@ __host__ __device__ constexpr int span_px(int halo) { return kTile + 2 * halo + 
 struct Desc {  // written by the producer with the rest of the stage
     long long m_t0;  // first pixel of the tile
     int flags, kind, out_idx, n_runs;
-    int pad[2];
+    // active launch: what the consumers need to know about the item's star (a batch mixes stars)
+    int star, halo;
+    double c0;
+    long long out_lo, out_hi, out_pitch;
+    float *out;
+    const float *contrast[2];  // of kinds 1, 2
 };
 
 struct StageLayout {
@@ -124,7 +155,10 @@ __host__ __device__ inline StageLayout stage_layout(int halo) {
     l.stage_bytes = (l.desc_off + sizeof(Desc) + 127) & ~(size_t)127;
     return l;
 }
-constexpr size_t kHeaderBytes = 512;                          // mbarriers (96 B), tile hand-over words, item queue (at 128)
+constexpr size_t kPrefixOff = 1280;                           // active launch: first item of every star, [kMaxBatchStars + 1]
+constexpr size_t kBlockCacheOff = 2176;                       // active launch: the star block each producer warp works on
+constexpr size_t kBlockCacheStride = 192;                     // >= sizeof(StarBlock), multiple of 16
+constexpr size_t kHeaderBytes = 3072;                         // mbarriers (96 B), tile hand-over words, item queue (at 128), prefix, blocks
 constexpr size_t kFinBytes = (size_t)kTile * (sizeof(double) + sizeof(float));  // active launch: per-pixel fp64
                                                                               // contrast-weighted sums + staged contrast
 __host__ inline size_t smem_bytes(int halo, bool active) {
@@ -142,6 +176,7 @@ inline void set_layout(Params &p) {  // host: the stage layout travels as kernel
 
 struct Job {
     long long tile;
+    int star;
     int kind, row;
     int begin;  // first entry (global index, even)
     int count;  // entries, <= kJobCap (0: an item without entries)
@@ -160,8 +195,8 @@ struct QuietSource {
     bool done;
     __device__ void init(const Params &p, long long cta, long long G) {
         row_start = p.row_start;
-        E = __ldg(&row_start[p.n_mu]);
-        const long long U = E * p.n_tiles;
+        E = __ldg(&row_start[p.one.n_mu]);
+        const long long U = E * p.one.n_tiles;
         u0 = range_begin(cta, U, G);
         u1 = range_begin(cta + 1, U, G);
         done = u1 <= u0;
@@ -189,6 +224,7 @@ struct QuietSource {
         while (__ldg(&row_start[s + 1]) <= e) ++s;  // rows without entries are skipped
         const int end = min(min(e + kJobCap, __ldg(&row_start[s + 1])), e_hi);
         j.tile = t;
+        j.star = 0;
         j.kind = 0;
         j.row = s;
         j.begin = e;
@@ -214,58 +250,79 @@ struct QuietSource {
 // and publishes (item, first job number) in a small shared-memory ring that the four producer warps read in
 // step; it stays kQueueAhead jobs ahead of its own position.  An item's jobs are its phase's job list applied
 // to its tile; a phase without covered cells yields one empty job so that its zeros are written (S19).
-constexpr int kQueueSlots = 32;  // items in flight per CTA: the producers are never more than ~16 jobs apart
+constexpr int kQueueSlots = 64;  // items in flight per CTA: the producers are never more than ~16 jobs apart, a hand-out <= 16 items
 constexpr int kQueueAhead = 2 * kStages;
+constexpr int kMaxItemChunk = 16;
 struct ItemQueue {               // shared memory
-    int2 slot[kQueueSlots];      // (item index or -1 = no more items, number of the item's first job)
+    int4 slot[kQueueSlots];      // {number of the item's first job, phase (-1 = no more items), tile, jobs of the phase << 8 | star}
     int tail;                    // items published
 };
+static_assert(kMaxBatchStars <= 256, "the star index travels in 8 bits of a queue slot");
 
 struct ActiveSource {
-    const ActiveJob *jobs;
-    const int *n_jobs, *phase_order;
+    const StarBlock *many;
+    const long long *prefix;  // shared memory: first item of every star, prefix[n_stars] = n_items
     int *counters;  // [0] next item, [1] CTAs that finished fetching (both zero between launches)
     ItemQueue *queue;
+    StarBlock *cache;  // shared memory: this warp's copy of the block of the star it is working on
     long long n_items;
-    int n_tiles, job_cap;
+    int n_stars, chunk;
     bool scheduler;
     int pub, pub_end;  // scheduler: items published, job number after the last of them
     bool pub_done;
+    int cs_pub;        // scheduler: star of the last hand-out's first item (item numbers only grow)
+    int cached_star;
     int i;             // item this warp is working through
-    int n0, nj, cnt, phase, tile;
+    int n0, nj, cnt, phase, tile, star;
     bool done;
-    __device__ int jobs_of(long long idx, int &ph, int &tl, int &c) const {
-        ph = __ldg(&phase_order[idx / n_tiles]);
-        tl = (int)(idx % n_tiles);
-        c = __ldg(&n_jobs[ph]);
-        return c > 0 ? c : 1;
-    }
-    // scheduler warp: publish items until they cover job number n_need (or the list is exhausted)
+    // scheduler warp: publish items until they cover job number n_need (or the list is exhausted).  A hand-out takes
+    // `chunk` consecutive items; lane l looks up item l of it (star, phase, tile, jobs of the phase).
     __device__ void publish_until(int n_need) {
         const int lane = threadIdx.x & 31;
         while (!pub_done && pub_end <= n_need) {
-            int idx = 0;
-            if (lane == 0) idx = atomicAdd(&counters[0], 1);
-            idx = __shfl_sync(0xffffffffu, idx, 0);
-            int add = 0;
-            if (idx >= n_items) {
+            int first = 0;
+            if (lane == 0) first = atomicAdd(&counters[0], chunk);
+            first = __shfl_sync(0xffffffffu, first, 0);
+            const long long idx = (long long)first + lane;
+            const bool valid = lane < chunk && idx < n_items;
+            int ph = -1, tl = 0, c = 0, stx = cs_pub;
+            if (valid) {
+                while (idx >= prefix[stx + 1]) ++stx;
+                const StarBlock &b = many[stx];
+                const int nt = __ldg(&b.n_tiles);
+                const int *po = ldg_ptr(&b.phase_order), *njp = ldg_ptr(&b.n_jobs);
+                const long long local = idx - prefix[stx];
+                ph = __ldg(&po[local / nt]);
+                tl = (int)(local % nt);
+                c = __ldg(&njp[ph]);
+            }
+            const int jobs = valid ? (c > 0 ? c : 1) : 0;
+            int incl = jobs;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
+            }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            const int n_valid = __popc(__ballot_sync(0xffffffffu, valid));
+            const bool ended = n_valid < chunk;  // the list is exhausted: an end marker follows the last item
+            if (valid) queue->slot[(pub + lane) % kQueueSlots] = make_int4(pub_end + incl - jobs, ph, tl, (c << 8) | stx);
+            if (ended && lane == n_valid) queue->slot[(pub + lane) % kQueueSlots] = make_int4(pub_end + total, -1, 0, 0);
+            if (ended) {
                 pub_done = true;
-                idx = -1;
                 if (lane == 0 && atomicAdd(&counters[1], 1) == (int)gridDim.x - 1) {  // every CTA has stopped fetching
                     counters[0] = 0;
                     counters[1] = 0;
                 }
-            } else {
-                int ph, tl, c;
-                add = jobs_of(idx, ph, tl, c);
             }
+            __syncwarp();
             if (lane == 0) {
-                queue->slot[pub % kQueueSlots] = make_int2(idx, pub_end);
                 __threadfence_block();
-                *reinterpret_cast<volatile int *>(&queue->tail) = pub + 1;
+                *reinterpret_cast<volatile int *>(&queue->tail) = pub + n_valid + (ended ? 1 : 0);
             }
-            ++pub;
-            pub_end += add;
+            pub += n_valid + (ended ? 1 : 0);
+            pub_end += total;
+            cs_pub = __shfl_sync(0xffffffffu, stx, 0);
             __syncwarp();
         }
     }
@@ -274,28 +331,43 @@ struct ActiveSource {
         while (*tail <= i) __nanosleep(20);
         __threadfence_block();
         const volatile int *sl = reinterpret_cast<const volatile int *>(&queue->slot[i % kQueueSlots]);
-        const int idx = sl[0];
-        n0 = sl[1];
-        done = idx < 0;
+        n0 = sl[0];
+        phase = sl[1];
+        tile = sl[2];
+        const int w = sl[3];
+        done = phase < 0;
         if (done) return;
-        nj = jobs_of(idx, phase, tile, cnt);
+        cnt = w >> 8;
+        star = w & 255;
+        nj = cnt > 0 ? cnt : 1;
+        if (star != cached_star) {  // this warp moves on to another star: copy its block
+            const int lane = threadIdx.x & 31;
+            __syncwarp();
+            if (lane < (int)(sizeof(StarBlock) / 16))
+                reinterpret_cast<uint4 *>(cache)[lane] = __ldg(reinterpret_cast<const uint4 *>(many + star) + lane);
+            __syncwarp();
+            cached_star = star;
+        }
     }
-    __device__ void init(const Params &p, ItemQueue *q, bool is_scheduler) {
-        jobs = p.jobs;
-        n_jobs = p.n_jobs;
-        phase_order = p.phase_order;
+    __device__ void init(const Params &p, ItemQueue *q, const long long *pref, StarBlock *my_cache, bool is_scheduler) {
+        many = p.many;
+        prefix = pref;
         counters = p.item_counters;
         queue = q;
-        n_tiles = p.n_tiles;
-        job_cap = p.job_cap;
-        n_items = (long long)p.n_phases * p.n_tiles;
+        cache = my_cache;
+        n_items = p.n_items;
+        n_stars = p.n_stars;
+        chunk = p.item_chunk;
         scheduler = is_scheduler;
         pub = 0;
         pub_end = 0;
         pub_done = false;
+        cs_pub = 0;
+        cached_star = -1;
         i = -1;
         n0 = 0;
         nj = 0;
+        star = 0;
         done = false;
     }
     __device__ int get(int n, Job &j) {
@@ -307,12 +379,13 @@ struct ActiveSource {
         if (done) return n == n0 ? kSrcExit : kSrcBeyond;
         const int k = n - n0;
         j.tile = tile;
+        j.star = star;
         j.out_idx = phase;
         if (cnt == 0) {
             j.kind = j.row = j.begin = j.count = 0;
             j.flags = kJobFirst | kJobLast;
         } else {
-            const int4 a = __ldg(reinterpret_cast<const int4 *>(jobs + (size_t)phase * job_cap + k));
+            const int4 a = __ldg(reinterpret_cast<const int4 *>(cache->jobs + (size_t)phase * cache->job_cap + k));
             j.begin = a.x;
             j.count = a.y;
             j.kind = a.z;
@@ -389,12 +462,15 @@ __device__ __forceinline__ int build_runs(const float2 *raw, int count, float c_
     return n_runs;
 }
 
-__device__ __forceinline__ void init_source(QuietSource &src, const Params &p, ItemQueue *, bool) {
+__device__ __forceinline__ void init_source(QuietSource &src, const Params &p, ItemQueue *, const long long *, StarBlock *, bool) {
     src.init(p, blockIdx.x, gridDim.x);
 }
-__device__ __forceinline__ void init_source(ActiveSource &src, const Params &p, ItemQueue *q, bool is_scheduler) {
-    src.init(p, q, is_scheduler);
+__device__ __forceinline__ void init_source(ActiveSource &src, const Params &p, ItemQueue *q, const long long *prefix,
+                                            StarBlock *cache, bool is_scheduler) {
+    src.init(p, q, prefix, cache, is_scheduler);
 }
+__device__ __forceinline__ const StarBlock &source_block(const QuietSource &, const Params &p) { return p.one; }
+__device__ __forceinline__ const StarBlock &source_block(const ActiveSource &src, const Params &) { return *src.cache; }
 
 template <bool ACTIVE>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Params p) {
@@ -403,8 +479,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     uint64_t *bar_ready = bar_tma + kStages;                 // [kStages] stage post-processed (count 1)
     uint64_t *bar_empty = bar_ready + kStages;               // [kStages] consumers done       (count kConsumerWarps)
     int *tile_ctl = reinterpret_cast<int *>(smem + 96);      // quiet launch: last-CTA flag, first / last sharing CTA
-    const int H = p.halo;
-    const int span = span_px(H);
+    long long *prefix = reinterpret_cast<long long *>(smem + kPrefixOff);  // active launch: first item of every star
     double *fin = reinterpret_cast<double *>(smem + kHeaderBytes);  // active launch only: [kR][kConsumers]
     float *cst = reinterpret_cast<float *>(fin + kTile);            // active launch only: contrast of the current kind
     unsigned char *stage0 = smem + kHeaderBytes + (ACTIVE ? kFinBytes : 0);
@@ -420,6 +495,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         fence_mbar_init();
         reinterpret_cast<ItemQueue *>(smem + 128)->tail = 0;
     }
+    if (ACTIVE) {
+        for (int k = tid; k <= p.n_stars; k += kThreads) prefix[k] = k < p.n_stars ? __ldg(&p.many[k].item0) : p.n_items;
+    }
     __syncthreads();
 
     if (warp >= kConsumerWarps) {
@@ -433,7 +511,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         int2 *runs = reinterpret_cast<int2 *>(sb + p.run_off);
         Desc *desc = reinterpret_cast<Desc *>(sb + p.desc_off);
         typename std::conditional<ACTIVE, ActiveSource, QuietSource>::type src;
-        init_source(src, p, reinterpret_cast<ItemQueue *>(smem + 128), st == 0);
+        init_source(src, p, reinterpret_cast<ItemQueue *>(smem + 128), prefix,
+                    reinterpret_cast<StarBlock *>(smem + kBlockCacheOff + (size_t)st * kBlockCacheStride), st == 0);
         Job jb;
         for (int n = st, use = 0;; n += kStages, ++use) {
             const int status = src.get(n, jb);
@@ -446,27 +525,32 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                 }
                 break;
             }
+            const StarBlock &blk = source_block(src, p);  // quiet: the kernel argument; active: this warp's cached copy
+            const int H = blk.halo;
+            const int span = span_px(H);
+            const long long row_len = blk.row_len, n_pix = blk.n_pix;
+            const double c0 = blk.c0;
             const long long m_t0 = jb.tile * kTile;
             const long long s_start = m_t0 - H;  // global pixel of smem position 0 (multiple of 4)
             if (lane == 0) {
                 if (jb.count > 0) {
                     const long long g_lo = s_start < 0 ? 0 : s_start;
-                    const long long g_hi = (s_start + span) < p.row_len ? (s_start + span) : p.row_len;
+                    const long long g_hi = (s_start + span) < row_len ? (s_start + span) : row_len;
                     const uint32_t row_bytes = (uint32_t)((g_hi - g_lo) * (long long)sizeof(float));
-                    const float *src_row = p.base[jb.kind] + (long long)jb.row * p.pitch + g_lo;
+                    const float *src_row = blk.base[jb.kind] + (long long)jb.row * blk.pitch + g_lo;
                     const uint32_t ent_bytes = (uint32_t)(((jb.count + 1) & ~1) * (int)sizeof(float2));
                     fence_proxy_async_smem();
                     mbar_arrive_expect_tx(&bar_tma[st], row_bytes + ent_bytes);
                     tma_load_1d(sb + (size_t)(g_lo - s_start) * sizeof(float), src_row, row_bytes, &bar_tma[st]);
-                    tma_load_1d(sb + p.raw_off, p.ent + jb.begin, ent_bytes, &bar_tma[st]);
+                    tma_load_1d(sb + p.raw_off, blk.ent + jb.begin, ent_bytes, &bar_tma[st]);
                 } else {
                     mbar_arrive(&bar_tma[st]);  // nothing to load: keeps the barrier's phase in step
                 }
             }
             mbar_wait(&bar_tma[st], (uint32_t)(use & 1));
             // -- records, run table, edge halo, descriptor ---------------------------------------------
-            const float c_first = (float)(p.c0 + (double)m_t0);
-            const float c_last = (float)(p.c0 + (double)(m_t0 + kTile - 1));
+            const float c_first = (float)(c0 + (double)m_t0);
+            const float c_last = (float)(c0 + (double)(m_t0 + kTile - 1));
             const int n_runs = build_runs(raw, jb.count, c_first, c_last, H, p.collapse, rec, runs);
             if (lane == 0) {
                 runs[n_runs] = make_int2(p.collapse ? n_runs : jb.count, 0);  // sentinel: end of the last run
@@ -475,6 +559,15 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                 desc->kind = jb.kind;
                 desc->out_idx = jb.out_idx;
                 desc->n_runs = n_runs;
+                desc->star = jb.star;
+                desc->halo = H;
+                desc->c0 = c0;
+                desc->out_lo = blk.out_lo;
+                desc->out_hi = blk.out_hi;
+                desc->out_pitch = blk.out_pitch;
+                desc->out = blk.out;
+                desc->contrast[0] = blk.contrast[1];
+                desc->contrast[1] = blk.contrast[2];
             }
             if (jb.count > 0) {
                 if (s_start < 0) {  // clamp-to-edge below the grid (reading S8)
@@ -482,8 +575,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                     const float v = rs[nb];
                     for (int q = lane; q < nb; q += 32) rs[q] = v;
                 }
-                if (s_start + span > p.n_pix) {  // ... and above it
-                    const int first = (int)(p.n_pix - s_start);
+                if (s_start + span > n_pix) {  // ... and above it
+                    const int first = (int)(n_pix - s_start);
                     const float v = rs[first - 1];
                     for (int q = first + lane; q < span; q += 32) rs[q] = v;
                 }
@@ -496,7 +589,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
 
     // =================================== consumer warps ===============================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsConsumer));
-    const int base0 = H + tid;  // smem position of pixel r = 0 at zero shift
+    int H = p.halo, base0 = H + tid;  // halo of the current item's star; smem position of pixel r = 0 at zero shift
+    int cmask = 0;                     // bit k: kind k of the current item's star carries a contrast array
+    long long out_lo = 0, out_hi = 0;  // of the current item's star
     long long m_t0 = 0;
     float cmf = 0.f;      // lambda0/k + m of this thread's first pixel
     // W lerp = W (s + t d), t = a c - q  ==>  W u + c (W a) d  with u = s - q d: the per-pixel factor c = lambda0/k + m is
@@ -521,9 +616,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     // The contrast values of the current kind are fetched with cp.async while its jobs run.
     int rmax = 0;            // pixels r < rmax of this thread lie inside the spectrum
     bool fin_valid = false;  // `fin` holds a weighted sum of this item
+    const Desc *desc = nullptr;  // descriptor of the current job
     auto prefetch_contrast = [&](int kind) {
-        const float *ck = p.contrast[kind];
-        if (ck == nullptr) return;
+        if (!((cmask >> kind) & 1)) return;
+        const float *ck = desc->contrast[kind - 1];
 #pragma unroll
         for (int r = 0; r < kR; ++r)
             if (r < rmax) cp_async_4(&cst[r * kConsumers + tid], ck + m_t0 + tid + kConsumers * r);
@@ -532,8 +628,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     auto fold_kind = [&](int kind) {
         // weight 1: keeps accumulating with the next kind - unless that kind's sum is about to be multiplied by
         // its own contrast (job order is 1, 2, 0: only a spot sum without contrast ahead of a facula with one)
-        const bool has_c = p.contrast[kind] != nullptr;
-        if (!has_c && !(kind == 1 && p.contrast[2] != nullptr)) return;
+        const bool has_c = (cmask >> kind) & 1;
+        if (!has_c && !(kind == 1 && ((cmask >> 2) & 1))) return;
         fold();
         cp_async_wait_all();
 #pragma unroll
@@ -554,7 +650,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         const float2 *raw = reinterpret_cast<const float2 *>(sb + p.raw_off);
         const float2 *rec = reinterpret_cast<const float2 *>(sb + p.rec_off);
         const int2 *runs = reinterpret_cast<const int2 *>(sb + p.run_off);
-        const Desc *desc = reinterpret_cast<const Desc *>(sb + p.desc_off);
+        desc = reinterpret_cast<const Desc *>(sb + p.desc_off);
         const int flags = desc->flags;
         if (flags & kJobExit) break;
         const int n_runs = desc->n_runs;
@@ -562,14 +658,19 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         const int out_idx = desc->out_idx;
         if (flags & kJobFirst) {
             m_t0 = desc->m_t0;
-            cmf = (float)(p.c0 + (double)(m_t0 + tid));
+            H = desc->halo;
+            base0 = H + tid;
+            out_lo = desc->out_lo;
+            out_hi = desc->out_hi;
+            cmask = (desc->contrast[0] ? 2 : 0) | (desc->contrast[1] ? 4 : 0);
+            cmf = (float)(desc->c0 + (double)(m_t0 + tid));
 #pragma unroll
             for (int r = 0; r < kR; ++r) tot[r] = 0.0;
 #pragma unroll
             for (int k = 0; k < kR / 2; ++k) acc1[k] = acc2[k] = make_float2(0.f, 0.f);
             cnt = 0;
             if (ACTIVE) {
-                const long long rem = p.out_hi - (m_t0 + tid);
+                const long long rem = out_hi - (m_t0 + tid);
                 rmax = rem <= 0 ? 0 : (int)min((long long)kR, (rem + kConsumers - 1) / kConsumers);
                 fin_valid = false;  // only this thread ever touches its 16 slots of `fin` and `cst`
                 cur_kind = kind;
@@ -631,6 +732,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             cnt += len;
             if (cnt >= kFold) fold();  // at most kFold + one run's entries are ever summed in fp32
         }
+        float *o_row = nullptr;  // active launch: this thread's first output pixel (read before the stage is released)
+        if (ACTIVE && (flags & kJobLast)) o_row = desc->out + (long long)out_idx * desc->out_pitch + m_t0 + tid;
         __syncwarp();
         if (lane == 0) mbar_arrive(&bar_empty[st]);  // the stage may be refilled while the tile is stored
 
@@ -638,11 +741,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             fold();
             if (ACTIVE) {
                 fold_kind(cur_kind);
-                float *o = p.out + (long long)out_idx * p.out_pitch + m_t0 + tid;
+                float *o = o_row;
 #pragma unroll
                 for (int r = 0; r < kR; ++r) {
                     const double f = fin_valid ? fin[r * kConsumers + tid] : 0.0;
-                    if (r < rmax && m_t0 + tid + kConsumers * r >= p.out_lo) o[kConsumers * r] = (float)(tot[r] + f);
+                    if (r < rmax && m_t0 + tid + kConsumers * r >= out_lo) o[kConsumers * r] = (float)(tot[r] + f);
                 }
             } else {
                 double *o = p.partial + ((long long)blockIdx.x * p.max_seg + out_idx) * kTile;
@@ -651,7 +754,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                 // a6: the last CTA to deliver its share of this tile adds all shares in CTA order (the same
                 // order whoever comes last: deterministic) and rounds once to fp32.
                 const long long tile = m_t0 / kTile;
-                const long long E = __ldg(&p.row_start[p.n_mu]), U = E * p.n_tiles, G = gridDim.x;
+                const long long E = __ldg(&p.row_start[p.one.n_mu]), U = E * p.one.n_tiles, G = gridDim.x;
                 const long long ub = tile * E, ue = ub + E;
                 __threadfence();
                 consumer_bar_sync();
@@ -688,10 +791,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
 #pragma unroll
                         for (int r = 0; r < kR; ++r) sum[r] += __ldcg(&src[kConsumers * r]);
                     }
-                    float *qo = p.out + m_t0 + tid;
+                    float *qo = p.one.out + m_t0 + tid;
 #pragma unroll
                     for (int r = 0; r < kR; ++r)
-                        if (m_t0 + tid + kConsumers * r < p.out_hi && m_t0 + tid + kConsumers * r >= p.out_lo)
+                        if (m_t0 + tid + kConsumers * r < out_hi && m_t0 + tid + kConsumers * r >= out_lo)
                             qo[kConsumers * r] = (float)sum[r];
                 }
                 consumer_bar_sync();  // tile_ctl may be rewritten by the next tile

@@ -87,6 +87,7 @@ struct soap_star {
     DevBuf<float2> d_cWp;
     DevBuf<comp::PairHdr> d_chdr;
     int comp_stride = 0;  // bins per table row (multiple of 4); 0 = tables not built
+    DevBuf<comp::Star> d_cstars;  // batch launches: the stars' descriptors (owned by the first star of the batch)
 
     // quiet scratch
     DevBuf<double> d_partial;
@@ -105,6 +106,20 @@ struct soap_star {
     DevBuf<int> d_segcnt, d_nactive, d_sched;
     DevBuf<ActiveJob> d_jobs;
     DevBuf<ActiveCounters> d_counters;
+    // f32 active launch: region centres + map arguments + star blocks of a call (a batch: of all its stars), staged in one
+    // pinned buffer and copied with one cudaMemcpyAsync (owned by the first star of the batch)
+    DevBuf<unsigned char> d_call;
+    struct PinnedBytes {
+        unsigned char *ptr = nullptr;
+        size_t cap = 0;
+        cudaEvent_t done = nullptr;
+        bool in_flight = false;
+    } h_call[4];
+    int h_call_next = 0;
+    size_t call_rp_off = 0, call_prep_off = 0, call_blk_off = 0, call_ph_off = 0;  // sections of d_call of the last prepared call
+    bool attr_active_set = false, attr_prep_set = false;
+    int occ_active = 0;
+    size_t occ_active_smem = 0;
 
     // host-buffer staging (soap_synthesize_host)
     DevBuf<unsigned char> d_stage[3], d_stage_c[3], d_out_q, d_out_d;
@@ -228,20 +243,22 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     const long long P = q->n_pix;
     const int n_tiles = (int)((P + f32::kTile - 1) / f32::kTile);
     f32::Params p{};
-    p.base[0] = static_cast<const float *>(q->data);
-    p.pitch = q->pitch;
-    p.row_len = s->clip_override > 0 ? s->clip_override : q->pitch;
-    p.out_lo = s->out_lo_override >= 0 ? s->out_lo_override : 0;
-    p.out_hi = s->out_hi_override >= 0 ? s->out_hi_override : P;
-    p.n_pix = P;
-    p.c0 = q->lambda0 / q->dlambda;
-    p.n_mu = s->prm.n_mu;
-    p.halo = halo_for(s, q);
+    p.one.base[0] = static_cast<const float *>(q->data);
+    p.one.pitch = q->pitch;
+    p.one.row_len = s->clip_override > 0 ? s->clip_override : q->pitch;
+    p.one.out_lo = s->out_lo_override >= 0 ? s->out_lo_override : 0;
+    p.one.out_hi = s->out_hi_override >= 0 ? s->out_hi_override : P;
+    p.one.n_pix = P;
+    p.one.c0 = q->lambda0 / q->dlambda;
+    p.one.n_mu = s->prm.n_mu;
+    p.one.halo = halo_for(s, q);
+    p.one.ent = s->d_ent32.ptr;
+    p.one.n_tiles = n_tiles;
+    p.n_stars = 1;
+    p.halo = p.one.halo;
     f32::set_layout(p);
     p.collapse = s->form_used == SOAP_FORM_FIR ? 1 : 0;
-    p.ent = s->d_ent32.ptr;
     p.row_start = s->d_row_start.ptr;
-    p.n_tiles = n_tiles;
     // one CTA per resident slot (a single wave); fewer when there is too little work to share out
     const size_t smem = f32::smem_bytes(p.halo, false);
     if (smem > 227 * 1024) return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", p.halo, smem);
@@ -261,7 +278,7 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
         SOAP_CUDA(s, cudaMemsetAsync(s->d_tile_ticket.ptr, 0, s->d_tile_ticket.cap * sizeof(int), st));  // self-resetting after
     }
     p.tile_ticket = s->d_tile_ticket.ptr;
-    p.out = static_cast<float *>(out);
+    p.one.out = static_cast<float *>(out);
     int rc = launch_sia_f32<false>(s, p, dim3((unsigned)G), st);
     if (rc) return rc;
     s->last_quiet_splits = (int)G;
@@ -422,9 +439,269 @@ inline int per_cell_cap(const soap_star *s, int n_mu, int ncap) {  // jobs one p
     return 3 * n_mu * ((ncap + kActiveJobCap - 1) / kActiveJobCap);
 }
 
+// Localize (readings S11-S13): region centres in the observer frame for every phase, written to
+// out[n_phases][n_regions] (HOST).
+void localize_regions(const soap_star *s, const soap_region *regions, int n_regions, const double *phases, int n_phases,
+                      const double *radii, RegionAtPhase *out) {
+    const double pi = 3.14159265358979323846;
+    for (int p = 0; p < n_phases; ++p) {
+        for (int r = 0; r < n_regions; ++r) {
+            const soap_region &g = regions[r];
+            const double lat = g.lat_deg * pi / 180.0;
+            const double L = g.lon_deg * pi / 180.0 + 2.0 * pi * phases[p];
+            const double sx = std::cos(lat) * std::sin(L), sy = std::sin(lat), sz = std::cos(lat) * std::cos(L);
+            RegionAtPhase &o = out[(size_t)p * n_regions + r];
+            o.xr = sx;
+            o.yr = sy * s->sini - sz * s->cosi;
+            o.zr = sy * s->cosi + sz * s->sini;
+            const double rad = radii ? radii[(size_t)p * n_regions + r] : g.radius;
+            const bool present = rad > 0.0;
+            o.cos_alpha = present ? std::sqrt(1.0 - rad * rad) : 2.0;
+            o.chord = present ? 2.0 * std::sin(0.5 * std::asin(rad)) : 0.0;
+            o.type = (!present || o.zr < -rad - 1e-9) ? 0 : g.type;  // absent at this phase, or entirely on the far side
+            o.pad = 0;
+        }
+    }
+}
+
+// ---- f32 spectra, solid-body rotation: the active path of one call - of ALL the stars of a batch call - in ONE active-map
+// launch and ONE shift-interpolate-accumulate launch.  Region centres (Localize), the map kernel's arguments and the
+// stars' blocks are staged in one pinned buffer of the first star and cross in one copy.
+struct ActiveCall {  // one star's arguments
+    soap_star *s;
+    const soap_spectra *q, *spot, *fac;
+    const soap_region *regions;
+    int n_regions;
+    const double *phases;
+    int n_phases;
+    const double *radii;  // nullable
+    void *out;
+    long long out_pitch;
+};
+
+inline size_t align16(size_t v) { return (v + 15) & ~(size_t)15; }
+
+// `external_map`: the entry lists were built by the caller (per-cell form under differential rotation): only the blocks
+// are staged.
+int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, bool external_map, cudaStream_t st) {
+    soap_star *own = calls[0].s;
+    const bool use_lb = effect != SOAP_EFFECT_CB, use_contrast = effect != SOAP_EFFECT_CB;
+    const bool quiet_rows = effect == SOAP_EFFECT_FLUX;
+    // ---- per-star scratch, totals --------------------------------------------------------------------------------------
+    size_t n_rp = 0;
+    long long total_phases = 0, n_items = 0;
+    int max_halo = 0;
+    size_t prep_smem = 0;
+    for (int k = 0; k < n; ++k) {
+        const ActiveCall &c = calls[k];
+        soap_star *s = c.s;
+        const int N = s->prm.grid_n, n_mu = s->prm.n_mu;
+        const int ncap = ((N + 1) & ~1) + 2;
+        const long long n_seg = (long long)c.n_phases * 3 * n_mu;
+        if (n_seg * ncap >= (1LL << 31)) return s->fail(SOAP_ERR_UNSUPPORTED, "n_phases * 3 * n_mu * N too large for one call");
+        SOAP_CUDA(s, s->d_aent.reserve((size_t)n_seg * ncap * sizeof(float2) + 64));
+        SOAP_CUDA(s, s->d_segcnt.reserve((size_t)n_seg));
+        SOAP_CUDA(s, s->d_nactive.reserve((size_t)c.n_phases));
+        if (!s->d_counters.ptr) {
+            SOAP_CUDA(s, s->d_counters.reserve(1));
+            SOAP_CUDA(s, cudaMemsetAsync(s->d_counters.ptr, 0, sizeof(ActiveCounters), st));  // once per handle
+        }
+        SOAP_CUDA(s, s->d_jobs.reserve((size_t)c.n_phases * per_cell_cap(s, n_mu, ncap)));
+        SOAP_CUDA(s, s->d_sched.reserve((size_t)3 * c.n_phases));
+        const int chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);
+        if (prep_smem_bytes(n_mu, chunk_cols) > 200 * 1024)
+            return s->fail(SOAP_ERR_UNSUPPORTED, "grid_n %d with %d mu bins exceeds the active-map kernel's shared memory", N, n_mu);
+        prep_smem = std::max(prep_smem, prep_smem_bytes(n_mu, chunk_cols));
+        n_rp += (size_t)c.n_regions * c.n_phases;
+        total_phases += c.n_phases;
+        max_halo = std::max(max_halo, halo_for(s, c.q));
+        n_items += (long long)c.n_phases * ((c.q->n_pix + f32::kTile - 1) / f32::kTile);
+    }
+    if (total_phases * kPrepCluster >= (1LL << 31) || n_items >= (1LL << 31) - (1LL << 20))
+        return own->fail(SOAP_ERR_UNSUPPORTED, "too many phases / (phase, tile) items for one launch");
+    const size_t smem = f32::smem_bytes(max_halo, true);
+    if (smem > 227 * 1024) return own->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", max_halo, smem);
+
+    // ---- staging: [region centres][map arguments][star blocks][first phase of every star] -------------------------------
+    size_t rp_off = 0, prep_off = 0, blk_off = 0, ph_off = 0, total = 0;
+    if (external_map) {
+        prepare = false;
+        blk_off = 0;
+        ph_off = align16((size_t)n * sizeof(f32::StarBlock));
+        total = ph_off;
+        own->call_blk_off = blk_off;
+        own->call_ph_off = ph_off;
+    } else if (prepare) {
+        prep_off = align16(n_rp * sizeof(RegionAtPhase));
+        blk_off = align16(prep_off + (size_t)n * sizeof(PrepArgs));
+        ph_off = align16(blk_off + (size_t)n * sizeof(f32::StarBlock));
+        total = ph_off + (size_t)(n + 1) * sizeof(int);
+        own->call_rp_off = rp_off;
+        own->call_prep_off = prep_off;
+        own->call_blk_off = blk_off;
+        own->call_ph_off = ph_off;
+    } else {  // the lists of the previous (prepared) call of these stars are reused: only the blocks change
+        blk_off = own->call_blk_off;
+        ph_off = own->call_ph_off;
+        total = ph_off;
+        if (!own->d_call.ptr || blk_off + (size_t)n * sizeof(f32::StarBlock) > ph_off)
+            return own->fail(SOAP_ERR_NOT_READY, "no prepared active map to reuse");
+    }
+    soap_star::PinnedBytes &slot = own->h_call[own->h_call_next];
+    own->h_call_next = (own->h_call_next + 1) & 3;
+    if (slot.in_flight) {
+        SOAP_CUDA(own, cudaEventSynchronize(slot.done));
+        slot.in_flight = false;
+    }
+    if (!slot.done) SOAP_CUDA(own, cudaEventCreateWithFlags(&slot.done, cudaEventDisableTiming));
+    if (total > slot.cap) {
+        if (slot.ptr) cudaFreeHost(slot.ptr);
+        slot.ptr = nullptr;
+        slot.cap = 0;
+        SOAP_CUDA(own, cudaMallocHost(reinterpret_cast<void **>(&slot.ptr), total + 4096));
+        slot.cap = total + 4096;
+    }
+    if (total > own->d_call.cap) {
+        SOAP_CUDA(own, cudaDeviceSynchronize());  // growing frees the old buffer, which an earlier launch may still read
+        SOAP_CUDA(own, own->d_call.reserve(total + 4096));
+    }
+    unsigned char *h = slot.ptr, *d = own->d_call.ptr;
+    f32::StarBlock *hb = reinterpret_cast<f32::StarBlock *>(h + blk_off);
+    PrepArgs *hp = reinterpret_cast<PrepArgs *>(h + prep_off);
+    int *hph = reinterpret_cast<int *>(h + ph_off);
+    size_t rp_pos = 0;
+    long long item0 = 0;
+    int phase0 = 0;
+    for (int k = 0; k < n; ++k) {
+        const ActiveCall &c = calls[k];
+        soap_star *s = c.s;
+        const int N = s->prm.grid_n, n_mu = s->prm.n_mu;
+        const int ncap = ((N + 1) & ~1) + 2;
+        const int job_cap = per_cell_cap(s, n_mu, ncap);
+        int *d_njobs = s->d_sched.ptr, *d_order = d_njobs + c.n_phases, *d_work = d_order + c.n_phases;
+        if (prepare) {
+            RegionAtPhase *rp = reinterpret_cast<RegionAtPhase *>(h + rp_off) + rp_pos;
+            localize_regions(s, c.regions, c.n_regions, c.phases, c.n_phases, c.radii, rp);
+            PrepArgs a{};
+            a.N = N;
+            a.n_regions = c.n_regions;
+            a.n_mu = n_mu;
+            a.seg_cap = ncap;
+            a.job_cap = job_cap;
+            a.n_phases = c.n_phases;
+            a.chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);  // columns a CTA of the cluster may own
+            a.rp = reinterpret_cast<const RegionAtPhase *>(d + rp_off) + rp_pos;
+            a.mu = s->d_mu.ptr;
+            a.w = s->d_w.ptr;
+            a.col_a = s->d_col_a.ptr;
+            a.bin = s->d_bin.ptr;
+            a.lb.c[1][0] = 1.0;
+            a.lb.c[2][0] = 1.0;
+            if (use_lb && c.spot) { a.lb.c[1][0] = c.spot->lb_c0; a.lb.c[1][1] = c.spot->lb_c1; a.lb.c[1][2] = c.spot->lb_c2; }
+            if (use_lb && c.fac) { a.lb.c[2][0] = c.fac->lb_c0; a.lb.c[2][1] = c.fac->lb_c1; a.lb.c[2][2] = c.fac->lb_c2; }
+            a.ent = s->d_aent.ptr;
+            a.seg_count = s->d_segcnt.ptr;
+            a.n_active = s->d_nactive.ptr;
+            a.jobs = s->d_jobs.ptr;
+            a.n_jobs = d_njobs;
+            a.work = d_work;
+            a.phase_order = d_order;
+            a.counters = s->d_counters.ptr;
+            hp[k] = a;
+            hph[k] = phase0;
+            rp_pos += (size_t)c.n_regions * c.n_phases;
+            phase0 += c.n_phases;
+        }
+        f32::StarBlock b{};
+        b.base[0] = static_cast<const float *>(c.q->data);
+        b.base[1] = (c.spot && !quiet_rows) ? static_cast<const float *>(c.spot->data) : b.base[0];
+        b.base[2] = (c.fac && !quiet_rows) ? static_cast<const float *>(c.fac->data) : b.base[0];
+        b.contrast[1] = (c.spot && use_contrast) ? static_cast<const float *>(c.spot->contrast) : nullptr;
+        b.contrast[2] = (c.fac && use_contrast) ? static_cast<const float *>(c.fac->contrast) : nullptr;
+        b.pitch = c.q->pitch;
+        b.row_len = s->clip_override > 0 ? s->clip_override : c.q->pitch;
+        b.out_lo = s->out_lo_override >= 0 ? s->out_lo_override : 0;
+        b.out_hi = s->out_hi_override >= 0 ? s->out_hi_override : c.q->n_pix;
+        b.n_pix = c.q->n_pix;
+        b.c0 = c.q->lambda0 / c.q->dlambda;
+        b.n_mu = n_mu;
+        b.halo = halo_for(s, c.q);
+        b.ent = reinterpret_cast<const float2 *>(s->d_aent.ptr);
+        b.n_tiles = (int)((c.q->n_pix + f32::kTile - 1) / f32::kTile);
+        b.jobs = s->d_jobs.ptr;
+        b.n_jobs = d_njobs;
+        b.phase_order = d_order;
+        b.job_cap = job_cap;
+        b.n_phases = c.n_phases;
+        b.out = static_cast<float *>(c.out);
+        b.out_pitch = c.out_pitch;
+        b.item0 = item0;
+        hb[k] = b;
+        item0 += (long long)c.n_phases * b.n_tiles;
+        s->last_tile_px = f32::kTile;
+    }
+    if (prepare) {
+        hph[n] = phase0;
+        SOAP_CUDA(own, cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, st));
+    } else {
+        SOAP_CUDA(own, cudaMemcpyAsync(d + blk_off, h + blk_off, (size_t)n * sizeof(f32::StarBlock), cudaMemcpyHostToDevice, st));
+    }
+    SOAP_CUDA(own, cudaEventRecord(slot.done, st));
+    slot.in_flight = true;
+
+    if (prepare && total_phases > 0) {
+        // a4: one cluster of CTAs per (star, phase) bins, compacts and schedules (active.cuh)
+        if (!own->attr_prep_set) {
+            SOAP_CUDA(own, cudaFuncSetAttribute(active_prepare_kernel<float2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            own->attr_prep_set = true;
+        }
+        PrepArgs none{};
+        active_prepare_kernel<float2><<<(unsigned)(total_phases * kPrepCluster), kPrepThreads, prep_smem, st>>>(
+            none, reinterpret_cast<const PrepArgs *>(d + prep_off), reinterpret_cast<const int *>(d + ph_off), n);
+        SOAP_LAUNCH_CHECK(own, "active_prepare_kernel");
+    }
+    if (n_items == 0) return SOAP_OK;
+    // a5 + a6: persistent CTAs over the (star, phase, tile) items
+    f32::Params p{};
+    p.many = reinterpret_cast<const f32::StarBlock *>(d + blk_off);
+    p.n_stars = n;
+    p.n_items = n_items;
+    p.halo = max_halo;
+    f32::set_layout(p);
+    p.collapse = own->form_used == SOAP_FORM_FIR ? 1 : 0;
+    p.item_counters = reinterpret_cast<int *>(&own->d_counters.ptr->item_next);
+    if (!own->attr_active_set) {
+        SOAP_CUDA(own, cudaFuncSetAttribute(f32::sia_f32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        own->attr_active_set = true;
+    }
+    if (own->occ_active_smem != smem) {  // the occupancy query is cached per shared-memory size
+        int occ = 0;
+        SOAP_CUDA(own, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f32::sia_f32_kernel<true>, f32::kThreads, smem));
+        if (occ < 1) return own->fail(SOAP_ERR_UNSUPPORTED, "active kernel does not fit on an SM (halo %d)", max_halo);
+        own->occ_active = occ;
+        own->occ_active_smem = smem;
+    }
+    const long long G = std::max(1LL, std::min((long long)own->n_sm * own->occ_active, n_items));
+    // very long item lists (a batch of stars) are handed out several items at a time
+    p.item_chunk = (int)std::max(1LL, std::min((long long)f32::kMaxItemChunk, n_items / (G * 64)));
+    if (own->opt_timing) {
+        for (int k = 2; k < 4; ++k)
+            if (!own->ev[k]) SOAP_CUDA(own, cudaEventCreate(&own->ev[k]));
+        SOAP_CUDA(own, cudaEventRecord(own->ev[2], st));
+    }
+    f32::sia_f32_kernel<true><<<(unsigned)G, f32::kThreads, smem, st>>>(p);
+    SOAP_LAUNCH_CHECK(own, "sia_f32_kernel<active>");
+    if (own->opt_timing) {
+        SOAP_CUDA(own, cudaEventRecord(own->ev[3], st));
+        own->ev_valid[1] = true;
+    }
+    return SOAP_OK;
+}
+
 template <typename T>
 int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, const soap_spectra *fac,
                 int n_regions, int n_phases, int effect, bool prepare, void *out, long long out_pitch, cudaStream_t st) {
+    // (fp64 I/O, and fp32 under differential rotation; fp32 with solid-body rotation goes through active_f32_launch)
     // The three effects of Eq. 1-3 differ only in which table, weight and contrast an active entry uses:
     //   total: S_t, w LB_t(mu), C_t;   flux only: S_quiet, w LB_t(mu), C_t;   CB only: S_t, w, 1.
     // `prepare` = false reuses the entry lists of the previous pass (same weights).
@@ -521,47 +798,12 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         a.counters = s->d_counters.ptr;
         const size_t smem = prep_smem_bytes(n_mu, a.chunk_cols);
         SOAP_CUDA(s, cudaFuncSetAttribute(active_prepare_kernel<Ent>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        active_prepare_kernel<Ent><<<n_phases * kPrepCluster, kPrepThreads, smem, st>>>(a);
+        active_prepare_kernel<Ent><<<n_phases * kPrepCluster, kPrepThreads, smem, st>>>(a, nullptr, nullptr, 1);
         SOAP_LAUNCH_CHECK(s, "active_prepare_kernel");
     }
     if (sizeof(T) == 4) {
-        f32::Params p{};
-        p.base[0] = static_cast<const float *>(q->data);
-        p.base[1] = (spot && !quiet_rows) ? static_cast<const float *>(spot->data) : p.base[0];
-        p.base[2] = (fac && !quiet_rows) ? static_cast<const float *>(fac->data) : p.base[0];
-        p.contrast[1] = (spot && use_contrast) ? static_cast<const float *>(spot->contrast) : nullptr;
-        p.contrast[2] = (fac && use_contrast) ? static_cast<const float *>(fac->contrast) : nullptr;
-        p.pitch = q->pitch;
-        p.row_len = s->clip_override > 0 ? s->clip_override : q->pitch;
-        p.out_lo = s->out_lo_override >= 0 ? s->out_lo_override : 0;
-        p.out_hi = s->out_hi_override >= 0 ? s->out_hi_override : q->n_pix;
-        p.n_pix = q->n_pix;
-        p.c0 = q->lambda0 / q->dlambda;
-        p.n_mu = n_mu;
-        p.halo = halo_for(s, q);
-        f32::set_layout(p);
-        p.collapse = s->form_used == SOAP_FORM_FIR ? 1 : 0;
-        p.ent = reinterpret_cast<const float2 *>(s->d_aent.ptr);
-        p.n_tiles = (int)((q->n_pix + f32::kTile - 1) / f32::kTile);
-        p.jobs = s->d_jobs.ptr;
-        p.n_jobs = d_njobs;
-        p.phase_order = d_order;
-        p.item_counters = reinterpret_cast<int *>(&s->d_counters.ptr->item_next);
-        p.job_cap = job_cap;
-        p.n_phases = n_phases;
-        p.out = static_cast<float *>(out);
-        p.out_pitch = out_pitch;
-        s->last_tile_px = f32::kTile;
-        // persistent CTAs: one per resident slot, fewer when there are fewer (phase, tile) items
-        const size_t smem = f32::smem_bytes(p.halo, true);
-        if (smem > 227 * 1024) return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", p.halo, smem);
-        SOAP_CUDA(s, cudaFuncSetAttribute(f32::sia_f32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int occ = 0;
-        SOAP_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f32::sia_f32_kernel<true>, f32::kThreads, smem));
-        if (occ < 1) return s->fail(SOAP_ERR_UNSUPPORTED, "active kernel does not fit on an SM (halo %d)", p.halo);
-        const long long items = (long long)n_phases * p.n_tiles;
-        const long long G = std::max(1LL, std::min((long long)s->n_sm * occ, items));
-        return launch_sia_f32<true>(s, p, dim3((unsigned)G), st);
+        ActiveCall c{s, q, spot, fac, nullptr, n_regions, nullptr, n_phases, nullptr, out, out_pitch};
+        return active_f32_launch(&c, 1, effect, false, true, st);
     }
     SiaParams<T> p{};
     p.base[0] = static_cast<const T *>(q->data);
@@ -602,7 +844,7 @@ int check_regions(soap_star *s, const soap_region *regions, int n_regions, const
     return SOAP_OK;
 }
 
-// Localize (readings S11-S13): region centres in the observer frame for every phase.
+// upload_region_centres: the same for the calls that are not batched (fp64 I/O, differential rotation).
 // `radii` (nullable): HOST [n_phases][n_regions] radius of every region at every phase (evolving regions);
 // <= 0 means the region is absent at that phase.  NULL: regions[r].radius at every phase.
 int upload_region_centres(soap_star *s, const soap_region *regions, int n_regions, const double *phases,
@@ -645,25 +887,7 @@ int upload_region_centres(soap_star *s, const soap_region *regions, int n_region
         SOAP_CUDA(s, cudaDeviceSynchronize());
         SOAP_CUDA(s, s->d_rp.reserve(n));
     }
-    const double pi = 3.14159265358979323846;
-    for (int p = 0; p < n_phases; ++p) {
-        for (int r = 0; r < n_regions; ++r) {
-            const soap_region &g = regions[r];
-            const double lat = g.lat_deg * pi / 180.0;
-            const double L = g.lon_deg * pi / 180.0 + 2.0 * pi * phases[p];
-            const double sx = std::cos(lat) * std::sin(L), sy = std::sin(lat), sz = std::cos(lat) * std::cos(L);
-            RegionAtPhase &o = slot.ptr[(size_t)p * n_regions + r];
-            o.xr = sx;
-            o.yr = sy * s->sini - sz * s->cosi;
-            o.zr = sy * s->cosi + sz * s->sini;
-            const double rad = radii ? radii[(size_t)p * n_regions + r] : g.radius;
-            const bool present = rad > 0.0;
-            o.cos_alpha = present ? std::sqrt(1.0 - rad * rad) : 2.0;
-            o.chord = present ? 2.0 * std::sin(0.5 * std::asin(rad)) : 0.0;
-            o.type = (!present || o.zr < -rad - 1e-9) ? 0 : g.type;  // absent at this phase, or entirely on the far side
-            o.pad = 0;
-        }
-    }
+    localize_regions(s, regions, n_regions, phases, n_phases, radii, slot.ptr);
     SOAP_CUDA(s, cudaMemcpyAsync(s->d_rp.ptr, slot.ptr, n * sizeof(RegionAtPhase), cudaMemcpyHostToDevice, st));
     SOAP_CUDA(s, cudaEventRecord(slot.done, st));
     slot.in_flight = true;
@@ -841,7 +1065,7 @@ int soap_create(soap_star **out, int device) {
 int soap_destroy(soap_star *s) {
     if (!s) return SOAP_OK;
     cudaSetDevice(s->device);
-    s->d_cWp.release(); s->d_chdr.release();
+    s->d_cWp.release(); s->d_chdr.release(); s->d_cstars.release();
     s->d_geom_done.release(); s->d_colcnt.release(); s->d_cellpos.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
     s->d_Wbin.release(); s->d_col_sumw.release(); s->d_bin.release(); s->d_col_nvis.release(); s->d_row_start.release();
     s->d_ent32.release(); s->d_ent64.release(); s->d_info.release(); s->d_partial.release(); s->d_tile_ticket.release(); s->d_rp.release();
@@ -857,6 +1081,11 @@ int soap_destroy(soap_star *s) {
         if (slot.ptr) cudaFreeHost(slot.ptr);
         if (slot.done) cudaEventDestroy(slot.done);
     }
+    for (auto &slot : s->h_call) {
+        if (slot.ptr) cudaFreeHost(slot.ptr);
+        if (slot.done) cudaEventDestroy(slot.done);
+    }
+    s->d_call.release();
     delete s;
     return SOAP_OK;
 }
@@ -1013,7 +1242,9 @@ int soap_active_timeseries_evolving(soap_star *s, const soap_spectra *quiet, con
     if (out_pitch < quiet->n_pix) return s->fail(SOAP_ERR_INVALID_ARG, "out_pitch must be >= n_pix");
     SOAP_CUDA(s, cudaSetDevice(s->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (!s->reuse_lists && !s->regions_uploaded && (rc = upload_region_centres(s, regions, n_regions, phases, n_phases, radii, st)))
+    const bool one_launch_path = quiet->dtype == SOAP_F32 && s->prm.diff_rot == 0.0;
+    if (!one_launch_path && !s->reuse_lists && !s->regions_uploaded &&
+        (rc = upload_region_centres(s, regions, n_regions, phases, n_phases, radii, st)))
         return rc;
     // total and flux-only share the entry lists (weights w LB_t(mu)); CB-only needs the plain weights w, which
     // are the same lists again when both limb-brightening laws are identically 1
@@ -1024,6 +1255,13 @@ int soap_active_timeseries_evolving(soap_star *s, const soap_spectra *quiet, con
     for (const Pass &ps : passes) {
         if (!ps.out) continue;
         const bool prepare = ps.effect == SOAP_EFFECT_CB ? !(have_lb_lists && lb_is_one) : !have_lb_lists;
+        if (one_launch_path) {
+            ActiveCall c{s, quiet, spot, facula, regions, n_regions, phases, n_phases, radii, ps.out, out_pitch};
+            rc = active_f32_launch(&c, 1, ps.effect, prepare, false, st);
+            if (rc) return rc;
+            if (ps.effect != SOAP_EFFECT_CB) have_lb_lists = true;
+            continue;
+        }
         rc = quiet->dtype == SOAP_F32
                  ? active_impl<float>(s, quiet, spot, facula, n_regions, n_phases, ps.effect, prepare, ps.out, out_pitch, st)
                  : active_impl<double>(s, quiet, spot, facula, n_regions, n_phases, ps.effect, prepare, ps.out, out_pitch, st);
@@ -1293,12 +1531,60 @@ int soap_batch_integrate_quiet(soap_star *const *stars, int32_t n_stars, const s
     for (int k = 0; k < n_stars; ++k)
         if (!stars[k]) return SOAP_ERR_INVALID_ARG;
     if (n_stars == 0) return SOAP_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    soap_star *s0 = stars[0];
+    // ---- every argument is checked before anything is enqueued ---------------------------------------------------------
+    bool one_launch = true;
+    for (int k = 0; k < n_stars; ++k) {
+        soap_star *s = stars[k];
+        if (!s->ready) return s->fail(SOAP_ERR_NOT_READY, "soap_disk_geometry has not been called (star %d of the batch)", k);
+        int rc = check_spectra(s, quiet[k], "quiet");
+        if (rc) return rc;
+        if (!out[k]) return s->fail(SOAP_ERR_INVALID_ARG, "out is NULL (star %d of the batch)", k);
+        for (int j = 0; j < k; ++j)
+            if (stars[j] == s) return s->fail(SOAP_ERR_INVALID_ARG, "star %d appears twice in the batch", k);
+        one_launch = one_launch && s->device == s0->device && composite_applies(s, quiet[k]) && s->comp_stride == s0->comp_stride;
+    }
+    SOAP_CUDA(s0, cudaSetDevice(s0->device));
+    if (one_launch) {
+        // the composite-column kernel walks the flattened (star, tile, column pair) list: ONE launch for the batch
+        // (groups of comp::kMaxStars stars when the batch is larger)
+        for (int k0 = 0; k0 < n_stars; k0 += comp::kMaxStars) {
+            const int n = std::min(comp::kMaxStars, n_stars - k0);
+            std::vector<comp::Star> hs((size_t)n);
+            int max_pairs = 0, max_mu = 0;
+            for (int k = 0; k < n; ++k) {
+                soap_star *s = stars[k0 + k];
+                composite_fill(s, quiet[k0 + k], out[k0 + k], hs[k]);
+                int rc = reserve_tickets(s, (size_t)hs[k].n_tiles + 1, st);
+                if (rc) return rc;
+                hs[k].ticket = s->d_tile_ticket.ptr;
+                max_pairs = std::max(max_pairs, hs[k].n_pairs);
+                max_mu = std::max(max_mu, s->prm.n_mu);
+                s->last_tile_px = hs[k].L;
+                s->last_form = SOAP_FORM_COMPOSITE;
+            }
+            if (n > 1) {
+                if ((size_t)n > s0->d_cstars.cap) {
+                    SOAP_CUDA(s0, cudaStreamSynchronize(st));  // an earlier launch may still read the old buffer
+                    SOAP_CUDA(s0, s0->d_cstars.reserve((size_t)std::max(n, 64)));
+                }
+                // pageable source: the runtime stages it before returning, so `hs` may go out of scope
+                SOAP_CUDA(s0, cudaMemcpyAsync(s0->d_cstars.ptr, hs.data(), (size_t)n * sizeof(comp::Star), cudaMemcpyHostToDevice, st));
+            }
+            int rc = launch_composite(s0, hs.data(), s0->d_cstars.ptr, n, s0->comp_stride, max_pairs, max_mu, st);
+            if (rc) return rc;
+        }
+        return SOAP_OK;
+    }
+    // mixed batch (fp64 tables, differential rotation, more than comp::kMaxBins mu bins, several devices): per-star launches
+    // dealt to three lanes
     cudaStream_t lanes[3];
-    int rc = batch_fork(stars[0], static_cast<cudaStream_t>(stream), lanes);
+    int rc = batch_fork(s0, st, lanes);
     if (rc) return rc;
     int first_error = SOAP_OK;
     for (int k = 0; k < n_stars && !first_error; ++k) first_error = soap_integrate_quiet(stars[k], quiet[k], out[k], lanes[k % 3]);
-    rc = batch_join(stars[0], static_cast<cudaStream_t>(stream), lanes);  // joined even after an error: no dangling lane
+    rc = batch_join(s0, st, lanes);  // joined even after an error: no dangling lane
     return first_error ? first_error : rc;
 }
 
@@ -1311,14 +1597,50 @@ int soap_batch_active_timeseries(soap_star *const *stars, int32_t n_stars, const
     for (int k = 0; k < n_stars; ++k)
         if (!stars[k]) return SOAP_ERR_INVALID_ARG;
     if (n_stars == 0) return SOAP_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    soap_star *s0 = stars[0];
+    // ---- every argument of every star is checked before anything is enqueued ----------------------------------------
+    bool one_launch = true;
+    std::vector<ActiveCall> calls;
+    calls.reserve((size_t)n_stars);
+    for (int k = 0; k < n_stars; ++k) {
+        soap_star *s = stars[k];
+        const soap_spectra *sp = spot ? spot[k] : nullptr, *fa = facula ? facula[k] : nullptr;
+        if (!s->ready) return s->fail(SOAP_ERR_NOT_READY, "soap_disk_geometry has not been called (star %d of the batch)", k);
+        int rc = check_spectra(s, quiet[k], "quiet");
+        if (rc) return rc;
+        if (sp && ((rc = check_spectra(s, sp, "spot")) || (rc = check_same_grid(s, quiet[k], sp, "spot")))) return rc;
+        if (fa && ((rc = check_spectra(s, fa, "facula")) || (rc = check_same_grid(s, quiet[k], fa, "facula")))) return rc;
+        if ((rc = check_regions(s, regions[k], n_regions[k], phases[k], n_phases[k], sp, fa))) return rc;
+        if (n_phases[k] > 0 && !out_delta[k]) return s->fail(SOAP_ERR_INVALID_ARG, "out_delta is NULL (star %d of the batch)", k);
+        if (out_pitch[k] < quiet[k]->n_pix) return s->fail(SOAP_ERR_INVALID_ARG, "out_pitch must be >= n_pix (star %d of the batch)", k);
+        for (int j = 0; j < k; ++j)
+            if (stars[j] == s) return s->fail(SOAP_ERR_INVALID_ARG, "star %d appears twice in the batch", k);
+        one_launch = one_launch && s->device == s0->device && quiet[k]->dtype == SOAP_F32 && s->prm.diff_rot == 0.0 &&
+                     (s->form_used == SOAP_FORM_FIR) == (s0->form_used == SOAP_FORM_FIR);
+        if (n_phases[k] > 0)
+            calls.push_back(ActiveCall{s, quiet[k], sp, fa, regions[k], n_regions[k], phases[k], n_phases[k], nullptr, out_delta[k], out_pitch[k]});
+    }
+    if (calls.empty()) return SOAP_OK;
+    SOAP_CUDA(s0, cudaSetDevice(s0->device));
+    if (one_launch) {
+        // ONE active-map launch and ONE shift-interpolate-accumulate launch for the batch (groups of f32::kMaxBatchStars)
+        for (size_t k0 = 0; k0 < calls.size(); k0 += f32::kMaxBatchStars) {
+            const int n = (int)std::min<size_t>(f32::kMaxBatchStars, calls.size() - k0);
+            int rc = active_f32_launch(calls.data() + k0, n, SOAP_EFFECT_TOTAL, true, false, st);
+            if (rc) return rc;
+        }
+        return SOAP_OK;
+    }
+    // mixed batch (fp64 tables, differential rotation, several devices): per-star launches dealt to three lanes
     cudaStream_t lanes[3];
-    int rc = batch_fork(stars[0], static_cast<cudaStream_t>(stream), lanes);
+    int rc = batch_fork(s0, st, lanes);
     if (rc) return rc;
     int first_error = SOAP_OK;
     for (int k = 0; k < n_stars && !first_error; ++k)
         first_error = soap_active_timeseries(stars[k], quiet[k], spot ? spot[k] : nullptr, facula ? facula[k] : nullptr, regions[k],
                                              n_regions[k], phases[k], n_phases[k], out_delta[k], out_pitch[k], nullptr, lanes[k % 3]);
-    rc = batch_join(stars[0], static_cast<cudaStream_t>(stream), lanes);
+    rc = batch_join(s0, st, lanes);
     return first_error ? first_error : rc;
 }
 

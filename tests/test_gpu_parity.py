@@ -282,6 +282,51 @@ def test_config5_batch_sampled(soap):
         soap.soap_destroy(st)
 
 
+def test_batch_entry_points_equal_per_star_calls(soap):
+    """soap_batch_* enqueue O(1) launches for the whole batch; every star's result equals the one its own calls give:
+    to the last bit for the delta spectra (an item's result does not depend on which CTA computes it), and to an fp32
+    rounding for the quiet spectra (the fp64 partial sums of a tile are grouped by CTA range, which depends on the batch)."""
+    dev = torch.device("cuda:0")
+    n_stars, n_pix, n_ph = 7, 30_000, 6
+    shared = workloads.make_config5_star(0, n_pix=n_pix, n_phases=n_ph, grid_n=90)
+    wls = [shared] + [workloads.make_config5_star(k, n_pix=n_pix, n_phases=n_ph, grid_n=90, shared=shared) for k in range(1, n_stars)]
+    wls[2].regions = []                       # a star without regions: exact zeros
+    wls[3].grid_n = 61                        # another grid: other column pairs, other tables
+    q = soap.to_device_spectra(shared.quiet, shared.lambda0, shared.dlambda, dev)
+    s = soap.to_device_spectra(shared.spot, shared.lambda0, shared.dlambda, dev, shared.spot_contrast, shared.spot_lb)
+    f = soap.to_device_spectra(shared.facula, shared.lambda0, shared.dlambda, dev, shared.facula_contrast, shared.facula_lb)
+    stars = [soap.soap_create(0) for _ in range(n_stars)]
+    for st, wl in zip(stars, wls):
+        soap.soap_disk_geometry(st, wl, want_info=False)
+    Qb = torch.full((n_stars, n_pix), float("nan"), dtype=torch.float32, device=dev)
+    Db = torch.full((n_stars, n_ph, n_pix), float("nan"), dtype=torch.float32, device=dev)
+    launches0 = sum(soap.soap_get_stats(st)["launches"] for st in stars)
+    soap.soap_batch_integrate_quiet(stars, [q] * n_stars, [Qb[k] for k in range(n_stars)])
+    soap.soap_batch_active_timeseries(stars, [q] * n_stars, [s] * n_stars, [f] * n_stars, [w.regions for w in wls],
+                                      [w.phases for w in wls], [Db[k] for k in range(n_stars)])
+    torch.cuda.synchronize()
+    launches = sum(soap.soap_get_stats(st)["launches"] for st in stars) - launches0
+    assert launches <= 4, f"{launches} launches for {n_stars} stars: the batch entry points must not launch per star"
+    assert not torch.isnan(Qb).any() and not torch.isnan(Db).any()
+    for k, (st, wl) in enumerate(zip(stars, wls)):
+        Q1 = torch.empty(n_pix, dtype=torch.float32, device=dev)
+        D1 = torch.empty((n_ph, n_pix), dtype=torch.float32, device=dev)
+        soap.soap_integrate_quiet(st, q, Q1)
+        soap.soap_active_timeseries(st, q, s, f, wl.regions, wl.phases, D1)
+        torch.cuda.synchronize()
+        sw = oracle.geometry(wl)["sum_w"]
+        assert float((Q1 - Qb[k]).abs().max()) <= 2.5e-7 * sw, f"star {k}"   # an fp32 ulp at the continuum level is 6e-8
+        assert torch.equal(D1, Db[k]), f"star {k}"
+        if not wl.regions:
+            assert torch.all(Db[k] == 0.0)
+    # and against the oracle for two of them
+    for k in (1, 3):
+        g = dict(Q=Qb[k].cpu().numpy(), D=Db[k].cpu().numpy(), n_active=oracle.run_workload(wls[k], 0, 16)[2])
+        assert_parity(wls[k], g)
+    for st in stars:
+        soap.soap_destroy(st)
+
+
 def test_host_buffer_entry_point(soap):
     wl = workloads.make_config2(n_pix=4000, n_phases=5, grid_n=80)
     wl.phases = np.linspace(0.35, 0.65, 5)
