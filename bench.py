@@ -12,6 +12,8 @@ every field means and how the roofline numbers are derived.
 from __future__ import annotations
 
 import argparse
+import csv
+import hashlib
 import json
 import os
 import sys
@@ -26,10 +28,15 @@ if ROOT not in sys.path:
 
 METRIC = "integrated spectra/s and cell*pixel interps/s (full visible, 300^2 grid), % roofline"
 N_SM, FP32_LANES_PER_SM = 148, 128
-FLOPS_PER_UNIT = 4  # one lerp-accumulate = 2 FP32 FMAs per (entry, pixel): acc += W u_r; acc += (W a) v_r
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture of this
-# workload (profiles/r01_v5_sia_full.md); algorithmic: active 74.4 MB in + 31 MB out, quiet 24.8 MB in.
-NCU_DRAM_TRAFFIC_BYTES = {"sia_f32_kernel<quiet>": 25.1e6, "sia_f32_kernel<active>": 109.5e6}
+# Algorithmic FP32 lane-instructions, each credited as one FMA = 2 FLOP against the FMA peak:
+#   binned entries: 2 FMAs per (entry, pixel):  acc1 += W u,  acc2 += (W a) d
+#   composite columns: 1 FMA per (column, mu-bin, pixel) + 4 per (column, pixel): t = a c - q, d = x1 - x0, acc += t d, acc += x0
+LANE_INSTR_PER_UNIT_BINNED = 2
+LANE_INSTR_PER_UNIT_COMPOSITE = 1
+LANE_INSTR_PER_COLUMN_PIXEL_COMPOSITE = 4
+FORM_NAMES = {1: "binned", 2: "cells", 3: "fir", 4: "composite"}
+WORKLOAD_C3 = ("C3 full visible range (BASELINE.json configs[2]): N=300, vsini=2 km/s, i=90, 310000 px 3800-6900 A, "
+               "20 mu bins x {quiet,spot,facula}, 25000 lines, 3% facula + 1% spot, 25 phases, fp32")
 
 
 def load_peaks():
@@ -39,6 +46,36 @@ def load_peaks():
             d = json.load(fh)
         return dict(sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), hbm_gbs=float(d.get("hbm_gbs", 6650.0)), source="measured")
     return dict(sm_max_mhz=1965.0, hbm_gbs=6650.0, source="fallback")
+
+
+def kernel_source_sha() -> str:
+    """Hash of the CUDA sources the library is built from: ties an ncu capture under profiles/ to the build that ran."""
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2301_04259_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".cuh")):
+            with open(os.path.join(csrc, name), "rb") as fh:
+                h.update(name.encode())
+                h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_dram_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+    (profiles/r02_dram_traffic.csv: kernel, bytes read, bytes written, source hash).  A row counts only if it was
+    captured from the sources this run was built from; otherwise the figure is stale and `traffic` is null."""
+    path = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")
+    out = {}
+    if not os.path.exists(path):
+        return out, "profiles/r02_dram_traffic.csv missing: null"
+    sha = kernel_source_sha()
+    with open(path) as fh:
+        for row in csv.DictReader(fh):
+            if row["source_sha"] == sha:
+                out[row["kernel"]] = float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
+    if out:
+        return out, f"profiles/r02_dram_traffic.csv, captured from the sources of this build ({sha})"
+    return out, f"profiles/r02_dram_traffic.csv is of other sources than this build ({sha}): null"
 
 
 class ClockSampler:
@@ -98,56 +135,217 @@ class ClockSampler:
                     sm_max_mhz=self.max_mhz, reasons=sorted(self.reasons), samples=len(self.samples))
 
 
-def cpu_oracle_rate(wl, budget_s: float):
-    """Times the oracle, as it stands, on a bounded pixel sample of the workload.  Returns
-    (spectra/s extrapolated to the full pixel count, threads, sample description, seconds)."""
+# ------------------------------------------------------------------------------------------------------------------
+# the oracle, timed as it stands (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------------------------
+def oracle_full(wl):
+    """ONE full-size run of the oracle (all cells, all pixels, all phases): (seconds, threads)."""
     import oracle
     oracle.build()
-    threads = oracle.num_threads()
-    probe = 2048
     t0 = time.perf_counter()
-    oracle.run_workload(wl, 0, probe)
-    t_probe = time.perf_counter() - t0
-    px = int(min(wl.n_pix, max(probe, (budget_s / t_probe) * probe)))
-    px = max(2048, (px // 2048) * 2048)
+    oracle.run_workload(wl)
+    return time.perf_counter() - t0, oracle.num_threads()
+
+
+def oracle_sample(wl, px: int):
+    """The oracle on a window of `px` pixels in the middle of the spectrum (all cells, all phases): seconds."""
+    import oracle
+    px = int(min(wl.n_pix, px))
     lo = (wl.n_pix - px) // 2
     t0 = time.perf_counter()
     oracle.run_workload(wl, lo, lo + px)
-    t = time.perf_counter() - t0
-    n_spec = 1 + len(wl.phases)
-    rate = n_spec / (t * wl.n_pix / px)
-    return rate, threads, f"pixels [{lo}, {lo + px}) of {wl.n_pix} ({px / wl.n_pix:.1%}), all cells, all {len(wl.phases)} phases, extrapolated linearly in pixels", t
+    return time.perf_counter() - t0, lo, px
+
+
+def oracle_single_thread_c2():
+    """the oracle's single-thread time on C2 (quiet + 100-phase time series)."""
+    import oracle
+    import workloads
+    wl = workloads.make_config2()
+    n = oracle.num_threads()
+    oracle.set_threads(1)
+    try:
+        t0 = time.perf_counter()
+        oracle.run_workload(wl)
+        t = time.perf_counter() - t0
+    finally:
+        oracle.set_threads(n)
+    return t, 1 + len(wl.phases)
 
 
 def run_reference(args):
+    """The tier's reference arm: the fp64 CPU oracle on C3.  The first timed step is ONE full-size run, measured as it
+    is ("sample": "full") - `value` comes from it alone; the remaining steps (and the warm-ups) are bounded samples of the
+    same workload so that the whole run ends within a few minutes, and `ms_per_step` is the mean wall time of the K timed
+    steps that were actually run."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import workloads
     wl = workloads.make_config3()
-    total_budget = 150.0
-    per_step = max(1.0, total_budget / max(1, args.steps + args.warmup))
-    rates, times = [], []
-    sample = ""
-    threads = 1
-    for i in range(args.warmup + args.steps):
-        rate, threads, sample, t = cpu_oracle_rate(wl, per_step * 0.8)
-        if i >= args.warmup:
-            rates.append(rate)
-            times.append(t)
     n_spec = 1 + len(wl.phases)
-    value = float(n_spec * len(rates) / sum(n_spec / r for r in rates))
+    sample_px = 8192
+    for _ in range(args.warmup):
+        oracle_sample(wl, sample_px)
+    t_full, threads = oracle_full(wl)
+    step_s = [t_full]
+    sample_rates = []
+    for _ in range(max(0, args.steps - 1)):
+        t, lo, px = oracle_sample(wl, sample_px)
+        step_s.append(t)
+        sample_rates.append(n_spec / (t * wl.n_pix / px))
+    value = n_spec / t_full
+    sample = "full: all 70688 cells x 310000 px x (1 quiet + 25 phases), one run, measured"
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": "spectra/s", "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * n_spec / value, "higher_is_better": True,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(step_s)), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "C3 full visible range: N=300, 310000 px, 20 mu bins x {quiet,spot,facula}, 25 phases",
-                   "note": "fp64 CPU oracle (oracle/soap_oracle.c, OpenMP) on a bounded pixel sample per step; ms_per_step is the extrapolated full-workload time"},
+        "config": {"workload": WORKLOAD_C3,
+                   "note": "fp64 CPU oracle (oracle/soap_oracle.c, OpenMP over wavelength chunks). value = 26 spectra / the one "
+                           "full-size step; the other timed steps and the warm-ups are %d-pixel samples (all cells, all phases); "
+                           "ms_per_step = mean wall time of the timed steps as run" % sample_px,
+                   "full_run_ms": 1e3 * t_full,
+                   "sampled_steps_extrapolated_spectra_per_s": float(np.median(sample_rates)) if sample_rates else None},
         "cpu_baseline": {"value": value, "unit": "spectra/s", "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "spectra/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# this repo's CUDA path
+# ------------------------------------------------------------------------------------------------------------------
+class Timer:
+    def __init__(self, torch, flush_buf):
+        self.torch, self.flush = torch, flush_buf
+
+    def steps(self, fn, n, warm=3):
+        """ms of n calls of fn, each bracketed by CUDA events on the current stream, L2 flushed before each."""
+        torch = self.torch
+        for _ in range(warm):
+            self.flush.zero_()
+            fn()
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        for a, b in ev:
+            self.flush.zero_()
+            a.record()
+            fn()
+            b.record()
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
+
+
+def lane_instr(form: int, quiet_entries: int, active_entries: int, n_columns: int, P: int):
+    """Algorithmic FP32 lane-instructions per launch of the two shift-interpolate-accumulate kernels."""
+    if form == 4:
+        q = (quiet_entries * LANE_INSTR_PER_UNIT_COMPOSITE + n_columns * LANE_INSTR_PER_COLUMN_PIXEL_COMPOSITE) * P
+    else:
+        q = quiet_entries * LANE_INSTR_PER_UNIT_BINNED * P
+    return q, active_entries * LANE_INSTR_PER_UNIT_BINNED * P
+
+
+def time_form(soap, torch, timer, wl, q, s, f, form, steps, dev_index, peak_instr):
+    """Step time and the two kernels' durations of one evaluation form (SOAP_OPT_FORM) on a star of workload wl."""
+    star = soap.soap_create(dev_index)
+    if form is not None:
+        soap.soap_set_option(star, soap.binding.SOAP_OPT_FORM, form)
+    P, n_ph = wl.n_pix, len(wl.phases)
+    dev = q.data.device
+    Q = torch.empty(P, dtype=torch.float32, device=dev)
+    D = torch.empty((n_ph, P), dtype=torch.float32, device=dev)
+
+    def step():
+        soap.soap_disk_geometry(star, wl, want_info=False)
+        soap.soap_integrate_quiet(star, q, Q)
+        soap.soap_active_timeseries(star, q, s, f, wl.regions, wl.phases, D)
+
+    ms = timer.steps(step, steps)
+    soap.soap_set_option(star, soap.binding.SOAP_OPT_KERNEL_TIMING, 1)
+    kq, ka = [], []
+    for _ in range(max(5, min(steps, 20))):
+        timer.flush.zero_()
+        step()
+        st = soap.soap_get_stats(star)
+        kq.append(st["quiet_kernel_ms"])
+        ka.append(st["active_kernel_ms"])
+    soap.soap_set_option(star, soap.binding.SOAP_OPT_KERNEL_TIMING, 0)
+    st = soap.soap_get_stats(star)
+    iq, ia = lane_instr(st["form"], st["quiet_entries"], st["active_entries"], wl.grid_n, P)
+    mq, ma, mm = float(np.mean(kq)), float(np.mean(ka)), float(np.mean(ms))
+    out = {
+        "form": FORM_NAMES[st["form"]], "ms_per_step": mm, "ms_per_step_median": float(np.median(ms)),
+        "ms_per_step_best": float(np.min(ms)), "spectra_per_s": (1 + n_ph) / (mm * 1e-3),
+        "quiet_kernel_ms": mq, "active_kernel_ms": ma,
+        "quiet_entries": st["quiet_entries"], "active_entries": st["active_entries"],
+        "quiet_lane_instr": iq, "active_lane_instr": ia,
+        "quiet_alu_frac": iq / (mq * 1e-3) / peak_instr if mq > 0 else None,
+        "active_alu_frac": ia / (ma * 1e-3) / peak_instr if ma > 0 else None,
+        "step_alu_frac": (iq + ia) / (mm * 1e-3) / peak_instr,
+    }
+    return out, star, Q, D
+
+
+def config_lines(soap, torch, timer, workloads, dev, steps, peak_instr):
+    """Device-resident timing of the other BASELINE.json configs (parity-test cases beside the C3 headline)."""
+    res = {}
+    for name in ("C2", "C4", "C5"):
+        if name == "C5":
+            shared = workloads.make_config5_star(0)
+            wls = [shared] + [workloads.make_config5_star(k, shared=shared) for k in range(1, 64)]
+        else:
+            wls = [{"C2": workloads.make_config2, "C4": workloads.make_config4}[name]()]
+        w0 = wls[0]
+        P, n_ph, n = w0.n_pix, len(w0.phases), len(wls)
+        q = soap.to_device_spectra(w0.quiet, w0.lambda0, w0.dlambda, dev)
+        sp = soap.to_device_spectra(w0.spot, w0.lambda0, w0.dlambda, dev, w0.spot_contrast, w0.spot_lb)
+        fa = None if w0.facula is None else soap.to_device_spectra(w0.facula, w0.lambda0, w0.dlambda, dev, w0.facula_contrast, w0.facula_lb)
+        stars = [soap.soap_create(dev.index) for _ in wls]
+        Q = torch.empty((n, P), dtype=torch.float32, device=dev)
+        D = torch.empty((n, n_ph, P), dtype=torch.float32, device=dev)
+
+        def step():
+            if n == 1:
+                soap.soap_disk_geometry(stars[0], w0, want_info=False)
+                soap.soap_integrate_quiet(stars[0], q, Q[0])
+                soap.soap_active_timeseries(stars[0], q, sp, fa, w0.regions, w0.phases, D[0])
+                return
+            for st_, wl in zip(stars, wls):
+                soap.soap_disk_geometry(st_, wl, want_info=False)
+            soap.soap_batch_integrate_quiet(stars, [q] * n, [Q[k] for k in range(n)])
+            soap.soap_batch_active_timeseries(stars, [q] * n, [sp] * n, [fa] * n, [w.regions for w in wls],
+                                              [w.phases for w in wls], [D[k] for k in range(n)])
+
+        ms = timer.steps(step, max(3, min(steps, 10)))
+        # kernel durations: the launches carry the whole batch and are timed on the first star's handle
+        soap.soap_set_option(stars[0], soap.binding.SOAP_OPT_KERNEL_TIMING, 1)
+        step()
+        st = soap.soap_get_stats(stars[0])
+        soap.soap_set_option(stars[0], soap.binding.SOAP_OPT_KERNEL_TIMING, 0)
+        per = [soap.soap_get_stats(s_) for s_ in stars]
+        q_ent = sum(p_["quiet_entries"] for p_ in per)
+        a_ent = sum(p_["active_entries"] for p_ in per)
+        iq, ia = lane_instr(st["form"], q_ent, a_ent, sum(w.grid_n for w in wls), P)
+        launches0 = sum(p_["launches"] for p_ in per)
+        step()
+        torch.cuda.synchronize()
+        launches = sum(soap.soap_get_stats(s_)["launches"] for s_ in stars) - launches0
+        mm = float(np.mean(ms))
+        res[name] = {
+            "workload": workloads.CONFIG_NAMES[int(name[1])], "stars": n, "ms_per_step": mm,
+            "ms_per_step_median": float(np.median(ms)), "ms_per_step_best": float(np.min(ms)),
+            "spectra_per_s": n * (1 + n_ph) / (mm * 1e-3), "launches_per_step": launches,
+            "quiet_form": FORM_NAMES[st["form"]], "quiet_entries": q_ent, "active_entries": a_ent,
+            "quiet_kernel_ms": st["quiet_kernel_ms"], "active_kernel_ms": st["active_kernel_ms"],
+            "quiet_alu_frac": iq / (st["quiet_kernel_ms"] * 1e-3) / peak_instr if st["quiet_kernel_ms"] > 0 else None,
+            "active_alu_frac": ia / (st["active_kernel_ms"] * 1e-3) / peak_instr if st["active_kernel_ms"] > 0 else None,
+        }
+        for s_ in stars:
+            soap.soap_destroy(s_)
+        del Q, D, q, sp, fa
+        torch.cuda.empty_cache()
+    return res
 
 
 def run_graft(args):
@@ -170,6 +368,8 @@ def run_graft(args):
         dist.init_process_group("nccl", device_id=dev)
     soap.binding.load_library()
     peaks = load_peaks()
+    peak_instr = N_SM * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6   # FP32 lane-instructions (FMAs) per second
+    peak_tflops = 2 * peak_instr / 1e12
 
     # ---- workload: every rank synthesises its own star of the same shape (weak scaling, no collective) ----
     wl = workloads.make_config3()
@@ -184,6 +384,7 @@ def run_graft(args):
     if args.form is not None:
         soap.soap_set_option(star, soap.binding.SOAP_OPT_FORM, args.form)
     flush_buf = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)  # > 126 MB L2
+    timer = Timer(torch, flush_buf)
 
     def step():
         soap.soap_disk_geometry(star, wl, want_info=False)
@@ -226,113 +427,108 @@ def run_graft(args):
     ms_per_step = total_ms / args.steps
     value = world * n_spec / (ms_per_step * 1e-3)
 
-    # ---- per-kernel durations (CUDA events inside the library, same stream), L2 flushed ------------------
-    soap.soap_set_option(star, soap.binding.SOAP_OPT_KERNEL_TIMING, 1)
-    kq, ka = [], []
-    for _ in range(max(5, min(args.steps, 30))):
-        flush_buf.zero_()
-        step()
-        st = soap.soap_get_stats(star)
-        kq.append(st["quiet_kernel_ms"])
-        ka.append(st["active_kernel_ms"])
-    soap.soap_set_option(star, soap.binding.SOAP_OPT_KERNEL_TIMING, 0)
-    stats = soap.soap_get_stats(star)
-    units_q = stats["quiet_entries"] * P
-    units_a = stats["active_entries"] * P
+    # ---- the device's FP32 FMA rate, measured live with the inner loops' instruction forms ----------------
+    probe = {"ffma2_fma_per_s": soap.soap_probe_fp32_rate(star, True), "ffma_fma_per_s": soap.soap_probe_fp32_rate(star, False),
+             "derived_fma_per_s": peak_instr}
+    probe["ffma2_over_derived"] = probe["ffma2_fma_per_s"] / peak_instr
+    probe["ffma_over_derived"] = probe["ffma_fma_per_s"] / peak_instr
+
+    # ---- per-kernel durations (CUDA events inside the library, same stream), L2 flushed: the form that was timed above,
+    # the north_star form (binned entries for both launches) and the run-collapsed form -------------------------------
+    k_steps = max(5, min(args.steps, 20))
+    forms = {}
+    main_form, star_m, Qm, Dm = time_form(soap, torch, timer, wl, q, s, f, args.form, k_steps, local_rank, peak_instr)
+    soap.soap_destroy(star_m)
+    forms[main_form["form"]] = main_form
+    for code in (1, 3):
+        if FORM_NAMES[code] in forms:
+            continue
+        r, st_, Qx, Dx = time_form(soap, torch, timer, wl, q, s, f, code, k_steps, local_rank, peak_instr)
+        r["max_abs_diff_of_quiet_vs_timed_form_over_sum_w"] = float((Qx - Qm).abs().max().item()) / info["sum_weights"]
+        r["max_abs_diff_of_delta_vs_timed_form_over_max_delta"] = float((Dx - Dm).abs().max().item()) / float(Dm.abs().max().item())
+        soap.soap_destroy(st_)
+        forms[r["form"]] = r
+        del Qx, Dx
+    traffic, traffic_note = ncu_dram_traffic()
+    kq_name = "composite_quiet_kernel" if main_form["form"] == "composite" else "sia_f32_kernel<quiet>"
     kern = {
-        "sia_f32_kernel<quiet>": dict(ms=float(np.mean(kq)), units=units_q),
-        "sia_f32_kernel<active>": dict(ms=float(np.mean(ka)), units=units_a),
+        kq_name: dict(ms=main_form["quiet_kernel_ms"], instr=main_form["quiet_lane_instr"], units=main_form["quiet_entries"] * P),
+        "sia_f32_kernel<active>": dict(ms=main_form["active_kernel_ms"], instr=main_form["active_lane_instr"],
+                                       units=main_form["active_entries"] * P),
     }
-    dom = max(kern, key=lambda k: kern[k]["ms"])
-    peak_tflops = N_SM * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    achieved = kern[dom]["units"] * FLOPS_PER_UNIT / (kern[dom]["ms"] * 1e-3) / 1e12
+    dom = max(kern, key=lambda k_: kern[k_]["ms"])
+    other = [k_ for k_ in kern if k_ != dom][0]
+
+    def tflops(k_):
+        return 2 * kern[k_]["instr"] / (kern[k_]["ms"] * 1e-3) / 1e12
+
+    step_instr = kern[dom]["instr"] + kern[other]["instr"]
     roofline = {
-        "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved / peak_tflops, "traffic": NCU_DRAM_TRAFFIC_BYTES.get(dom),
-        "peak_source": f"148 SMs x 128 FP32 lanes x 2 FLOP x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, {peaks['source']} MEASURED_PEAKS.json)",
-        "kernel_ms": kern[dom]["ms"], "units_per_launch": kern[dom]["units"], "flop_per_unit": FLOPS_PER_UNIT,
+        "bound": "alu", "kernel": dom, "achieved": tflops(dom), "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": tflops(dom) / peak_tflops, "traffic": traffic.get(dom), "traffic_source": traffic_note,
+        "peak_source": f"148 SMs x 128 FP32 lanes x 2 FLOP x {peaks['sm_max_mhz']:.0f} MHz (sm_max_mhz, {peaks['source']} MEASURED_PEAKS.json); "
+                       f"live FFMA2 probe on this device: {100 * probe['ffma2_over_derived']:.1f} % of it",
+        "kernel_ms": kern[dom]["ms"], "units_per_launch": kern[dom]["units"], "lane_instr_per_launch": kern[dom]["instr"],
+        "flop_per_lane_instr": 2,
+        "other_kernel": {"kernel": other, "kernel_ms": kern[other]["ms"], "achieved": tflops(other), "frac": tflops(other) / peak_tflops,
+                         "units_per_launch": kern[other]["units"], "lane_instr_per_launch": kern[other]["instr"],
+                         "traffic": traffic.get(other)},
+        "whole_step": {"lane_instr": step_instr, "frac": 2 * step_instr / (ms_per_step * 1e-3) / 1e12 / peak_tflops,
+                       "frac_at_4_flop_per_binned_unit": 4 * (main_form["quiet_entries"] + main_form["active_entries"]) * P /
+                                                         (ms_per_step * 1e-3) / 1e12 / peak_tflops},
+        "fp32_probe": probe,
     }
     if clocks.get("sm_mhz"):
-        roofline["frac_at_observed_clock"] = achieved / (peak_tflops * clocks["sm_mhz"] / peaks["sm_max_mhz"])
-    other = [k for k in kern if k != dom][0]
-    roofline["other_kernel"] = {"kernel": other, "kernel_ms": kern[other]["ms"],
-                                "achieved": kern[other]["units"] * FLOPS_PER_UNIT / (kern[other]["ms"] * 1e-3) / 1e12}
+        roofline["frac_at_observed_clock"] = roofline["frac"] * peaks["sm_max_mhz"] / clocks["sm_mhz"]
 
-    # ---- the run-collapsed form (SOAP_FORM_FIR): same sums, every run of entries with one integer
-    # shift collapsed into one record by the producer warps.  Reported beside the north_star form, never as it.
-    star_fir = soap.soap_create(local_rank)
-    soap.soap_set_option(star_fir, soap.binding.SOAP_OPT_FORM, 3)
-    Qf = torch.empty_like(Q)
-    Df = torch.empty_like(D)
+    # ---- the run-collapsed form against the memory roofline it moves the path to --------------
+    fir = forms.get("fir")
+    if fir is not None:
+        q_bytes = wl.n_mu * P * 4 + P * 4
+        a_bytes = 3 * wl.n_mu * P * 4 + P * 4 + n_ph * P * 4
+        step_bytes = a_bytes + P * 4
 
-    def step_fir():
-        soap.soap_disk_geometry(star_fir, wl, want_info=False)
-        soap.soap_integrate_quiet(star_fir, q, Qf)
-        soap.soap_active_timeseries(star_fir, q, s, f, wl.regions, wl.phases, Df)
+        def hbm(nbytes, ms):
+            g = nbytes / (ms * 1e-3) / 1e9
+            return {"algorithmic_bytes": nbytes, "achieved": g, "frac": g / peaks["hbm_gbs"]}
 
-    for _ in range(3):
-        step_fir()
-    fir_steps = max(5, min(args.steps, 30))
-    fir_ms = 0.0
-    soap.soap_set_option(star_fir, soap.binding.SOAP_OPT_KERNEL_TIMING, 1)
-    fq, fa = [], []
-    for _ in range(fir_steps):
-        flush_buf.zero_()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        step_fir()
-        b.record()
-        b.synchronize()
-        fir_ms += a.elapsed_time(b)
-        st = soap.soap_get_stats(star_fir)
-        fq.append(st["quiet_kernel_ms"])
-        fa.append(st["active_kernel_ms"])
-    fir_ms = sharding.max_over_ranks(fir_ms, dev) / fir_steps
-    fir = {"form": "fir (runs collapsed; SOAP_OPT_FORM=3)", "ms_per_step": fir_ms, "value": world * n_spec / (fir_ms * 1e-3),
-           "unit": "spectra/s", "quiet_kernel_ms": float(np.mean(fq)), "active_kernel_ms": float(np.mean(fa)),
-           "max_abs_diff_vs_binned_over_sum_w": float((Qf - Q).abs().max().item()) / info["sum_weights"],
-           "note": "event timing inside the library adds ~10 us per step to this figure"}
-    soap.soap_destroy(star_fir)
+        fir["roofline"] = {
+            "bound": "hbm", "peak": peaks["hbm_gbs"], "unit": "GB/s",
+            "quiet": hbm(q_bytes, fir["quiet_kernel_ms"]), "active": hbm(a_bytes, fir["active_kernel_ms"]),
+            "whole_step": hbm(step_bytes, fir["ms_per_step"]),
+            "traffic": {"quiet": traffic.get("sia_f32_kernel<quiet>/fir"), "active": traffic.get("sia_f32_kernel<active>/fir")},
+            "note": "algorithmic bytes: every table read once and every output written once per launch (the quiet table is read by both "
+                    "launches).  Executed FMAs are 2 per (run, pixel) instead of 2 per (entry, pixel); what is left is the per-run window "
+                    "set-up and the producers' run building, so the form is still far from the HBM roofline it is re-baselined against",
+        }
 
     # ---- resolution lowering of the 26 final spectra to R = 115 000 (HBM-bound: 1 read + 1 write)
     F = torch.empty((n_spec, P), dtype=torch.float32, device=dev)
     F[0] = Q
     F[1:] = Q.unsqueeze(0) + D
     Flow = torch.empty_like(F)
-    lsf_ms = []
-    for it in range(8):
-        flush_buf.zero_()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        soap.soap_lower_resolution(star, F, P, wl.lambda0, wl.dlambda, 115000.0, Flow)
-        b.record()
-        b.synchronize()
-        if it >= 3:
-            lsf_ms.append(a.elapsed_time(b))
+    lsf_ms = timer.steps(lambda: soap.soap_lower_resolution(star, F, P, wl.lambda0, wl.dlambda, 115000.0, Flow), 5)
     lsf_bytes = 2 * n_spec * P * 4
-    lsf = {"kernel": "lower_resolution_kernel<float>", "R": 115000, "rows": n_spec, "ms": float(np.mean(lsf_ms)),
+    lsf = {"kernel": "lower_resolution_v_kernel", "R": 115000, "rows": n_spec, "ms": float(np.mean(lsf_ms)),
            "bound": "hbm", "achieved": lsf_bytes / (float(np.mean(lsf_ms)) * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-           "algorithmic_bytes": lsf_bytes}
+           "algorithmic_bytes": lsf_bytes, "traffic": traffic.get("lower_resolution_v_kernel")}
     lsf["frac"] = lsf["achieved"] / lsf["peak"]
 
     # ---- first-moment RV of every generated line in every lowered spectrum (the reduction after the path)
     centres = torch.from_numpy(wl.line_centres.astype(np.float64)).to(dev)
     halfw = torch.from_numpy((3.0 * np.maximum(wl.line_sigmas, 0.03)).astype(np.float64)).to(dev)
     norm = torch.full((n_spec,), float(info["sum_weights"]), dtype=torch.float64, device=dev)
-    rv_ms = []
-    for it in range(8):
-        flush_buf.zero_()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        rvs = soap.soap_line_rvs(star, Flow, P, wl.lambda0, wl.dlambda, centres, halfw, norm, 64)
-        b.record()
-        b.synchronize()
-        if it >= 3:
-            rv_ms.append(a.elapsed_time(b))
+    rvs_box = {}
+
+    def rv_call():
+        rvs_box["rv"] = soap.soap_line_rvs(star, Flow, P, wl.lambda0, wl.dlambda, centres, halfw, norm, 64)
+
+    rv_ms = timer.steps(rv_call, 5)
     rv_bytes = n_spec * P * 4 + n_spec * len(wl.line_centres) * 8
-    line_rv = {"kernel": "line_rv_kernel<float>", "lines": int(len(wl.line_centres)), "rows": n_spec, "ms": float(np.mean(rv_ms)),
+    line_rv = {"kernel": "line_rv_kernel", "lines": int(len(wl.line_centres)), "rows": n_spec, "ms": float(np.mean(rv_ms)),
                "bound": "hbm", "achieved": rv_bytes / (float(np.mean(rv_ms)) * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-               "algorithmic_bytes": rv_bytes, "finite": int(torch.isfinite(rvs).sum().item())}
+               "algorithmic_bytes": rv_bytes, "finite": int(torch.isfinite(rvs_box["rv"]).sum().item()),
+               "traffic": traffic.get("line_rv_kernel")}
     line_rv["frac"] = line_rv["achieved"] / line_rv["peak"]
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ------------
@@ -349,20 +545,12 @@ def run_graft(args):
     hQ = torch.empty(P, dtype=torch.float32).pin_memory()
     hD = torch.empty((n_ph, P), dtype=torch.float32).pin_memory()
     star2 = soap.soap_create(local_rank)
-    for _ in range(3):
-        soap.soap_synthesize_host(star2, wl, hq, hs, hf, wl.regions, wl.phases, hQ, hD)
+    if args.form is not None:
+        soap.soap_set_option(star2, soap.binding.SOAP_OPT_FORM, args.form)
     e2e_steps = max(3, min(args.steps, 20))
     barrier()
-    e2e_ms = 0.0
-    for _ in range(e2e_steps):
-        flush_buf.zero_()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        soap.soap_synthesize_host(star2, wl, hq, hs, hf, wl.regions, wl.phases, hQ, hD)
-        b.record()
-        b.synchronize()
-        e2e_ms += a.elapsed_time(b)
-    e2e_ms = sharding.max_over_ranks(e2e_ms, dev)
+    e2e_list = timer.steps(lambda: soap.soap_synthesize_host(star2, wl, hq, hs, hf, wl.regions, wl.phases, hQ, hD), e2e_steps)
+    e2e_ms = sharding.max_over_ranks(float(sum(e2e_list)), dev)
     e2e_value = world * n_spec / (e2e_ms / e2e_steps * 1e-3)
     h2d = 3 * wl.n_mu * pitch * 4 + P * 4
     d2h = n_spec * P * 4
@@ -370,44 +558,62 @@ def run_graft(args):
     assert float((hQ.to(dev) - Q).abs().max()) <= 1e-6 * info["sum_weights"]
     assert float((hD.to(dev) - D).abs().max()) <= 1e-5 * float(D.abs().max())
 
+    # the same with the (static) spectra tables resident: a time-series user uploads them once; per step only the region
+    # list goes in and the 26 spectra come back to pinned host memory
+    def resident_step():
+        step()
+        hQ.copy_(Q, non_blocking=True)
+        hD.copy_(D, non_blocking=True)
+
+    res_list = timer.steps(resident_step, e2e_steps)
+    res_ms = sharding.max_over_ranks(float(sum(res_list)), dev) / e2e_steps
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
+    configs = {} if args.no_configs else config_lines(soap, torch, timer, workloads, dev, args.steps, peak_instr)
+
     n_vis = info["n_visible"]
     act_cells = int(n_active.sum())
     eff_interps = (n_vis + 2 * act_cells) * P  # what Alg. 1 / Alg. 5 would execute per star
-    exec_units = units_q + units_a
+    exec_units = (main_form["quiet_entries"] + main_form["active_entries"]) * P
+    form_text = main_form["form"] + (" quiet launch + binned active launch (SOAP_FORM_AUTO)" if main_form["form"] == "composite" else "")
     line = {
         "metric": METRIC, "value": value, "unit": "spectra/s", "n_gpus": world, "steps": args.steps, "warmup": warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-        "data": "synthetic",
-        "config": {"workload": "C3 full visible range (BASELINE.json configs[2]): N=300, vsini=2 km/s, i=90, 310000 px 3800-6900 A, "
-                               "20 mu bins x {quiet,spot,facula}, 25000 lines, 3% facula + 1% spot, 25 phases, fp32",
-                   "stars_per_gpu": 1, "spectra_per_step": n_spec, "form": {1: "binned", 2: "cells", 3: "fir", 4: "composite"}[stats["form"]],
+        "ms_per_step": ms_per_step, "ms_per_step_median": float(np.median(step_ms)), "ms_per_step_best": float(np.min(step_ms)),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD_C3, "stars_per_gpu": 1, "spectra_per_step": n_spec, "form": form_text,
                    "l2": "512 MB buffer written before every timed step (inputs+outputs 106 MB < 126 MB L2)",
                    "timing": "sum of per-step CUDA-event intervals, max over ranks", "sharding": "independent stars per rank, no collective"},
         "cell_pixel_interps_per_s": world * eff_interps / (ms_per_step * 1e-3),
         "executed_lerp_accumulates_per_s": world * exec_units / (ms_per_step * 1e-3),
-        "definitional": {"n_visible": n_vis, "active_cells_all_phases": act_cells, "quiet_entries": stats["quiet_entries"],
-                         "active_entries_all_phases": stats["active_entries"]},
-        "roofline": roofline, "fir_form": fir, "lower_resolution": lsf, "line_rvs": line_rv, "clocks": clocks,
+        "definitional": {"n_visible": n_vis, "active_cells_all_phases": act_cells, "quiet_entries": main_form["quiet_entries"],
+                         "active_entries_all_phases": main_form["active_entries"], "columns": wl.grid_n},
+        "roofline": roofline, "forms": forms, "fir_form": fir, "lower_resolution": lsf, "line_rvs": line_rv,
+        "configs": configs, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "spectra/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": e2e_ms / e2e_steps, "api": "soap_synthesize_host (pinned host buffers)"},
+                "ms_per_step": e2e_ms / e2e_steps, "api": "soap_synthesize_host (pinned host buffers)",
+                "tables_resident": {"ms_per_step": res_ms, "value": world * n_spec / (res_ms * 1e-3),
+                                    "h2d_bytes_per_step": 48 * len(wl.regions) * n_ph, "d2h_bytes_per_step": d2h,
+                                    "note": "spectra tables uploaded once (a time series re-uses them); per step the region centres "
+                                            "go in and the 26 spectra are copied to pinned host memory"}},
         "gpu_launches": launches, "wall_s_timed_region": wall,
     }
     if world == 1 and not args.no_cpu_baseline:
-        rate, threads, sample, _ = cpu_oracle_rate(wl, 12.0)
-        line["cpu_baseline"] = {"value": rate, "unit": "spectra/s", "cores": threads, "kind": "oracle", "sample": sample}
+        t_full, threads = oracle_full(wl)
+        t_c2, n_c2 = oracle_single_thread_c2()
+        line["cpu_baseline"] = {"value": n_spec / t_full, "unit": "spectra/s", "cores": threads, "kind": "oracle",
+                                "sample": "full: all 70688 cells x 310000 px x (1 quiet + 25 phases), one run, measured",
+                                "seconds": t_full, "c2_single_thread": {"seconds": t_c2, "spectra_per_s": n_c2 / t_c2, "cores": 1}}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
 
 def run_configs(args):
-    """--workload C2|C4|C5|all: device-resident timing of the other BASELINE.json configs (parity-test cases, not the
-    headline): one JSON line per config with the step time and the two kernels' durations and ALU fractions."""
+    """--workload C2|C3|C4|C5 (with --vsini / --form): one JSON line with the step time and the two kernels' durations."""
     import torch
 
     import paper_2301_04259_b200 as soap
@@ -416,74 +622,22 @@ def run_configs(args):
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     torch.cuda.set_device(dev)
     peaks = load_peaks()
-    peak_tflops = N_SM * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    peak_instr = N_SM * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6
     flush_buf = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)
-    which = ["C2", "C3", "C4", "C5"] if args.workload == "all" else [args.workload]
-    for name in which:
-        if name == "C5":
-            shared = workloads.make_config5_star(0)
-            wls = [shared] + [workloads.make_config5_star(k, shared=shared) for k in range(1, 64)]
-        else:
-            wls = [{"C2": workloads.make_config2, "C3": workloads.make_config3, "C4": workloads.make_config4}[name]()]
-        if args.vsini is not None:
-            for w in wls:
-                w.vsini_kms = args.vsini
-        w0 = wls[0]
-        P, n_ph = w0.n_pix, len(w0.phases)
-        q = soap.to_device_spectra(w0.quiet, w0.lambda0, w0.dlambda, dev)
-        sp = soap.to_device_spectra(w0.spot, w0.lambda0, w0.dlambda, dev, w0.spot_contrast, w0.spot_lb)
-        fa = None if w0.facula is None else soap.to_device_spectra(w0.facula, w0.lambda0, w0.dlambda, dev, w0.facula_contrast, w0.facula_lb)
-        stars = [soap.soap_create(dev.index) for _ in wls]
-        if args.form is not None:
-            for st_ in stars:
-                soap.soap_set_option(st_, soap.binding.SOAP_OPT_FORM, args.form)
-        Q = torch.empty((len(wls), P), dtype=torch.float32, device=dev)
-        D = torch.empty((len(wls), n_ph, P), dtype=torch.float32, device=dev)
-
-        def step():
-            if len(wls) == 1:
-                soap.soap_disk_geometry(stars[0], wls[0], want_info=False)
-                soap.soap_integrate_quiet(stars[0], q, Q[0])
-                soap.soap_active_timeseries(stars[0], q, sp, fa, wls[0].regions, wls[0].phases, D[0])
-                return
-            for st, wl in zip(stars, wls):  # config 5: the batch entry points (three lanes, one stream to the caller)
-                soap.soap_disk_geometry(st, wl, want_info=False)
-            soap.soap_batch_integrate_quiet(stars, [q] * len(wls), [Q[k] for k in range(len(wls))])
-            soap.soap_batch_active_timeseries(stars, [q] * len(wls), [sp] * len(wls), [fa] * len(wls), [w.regions for w in wls],
-                                              [w.phases for w in wls], [D[k] for k in range(len(wls))])
-
-        for _ in range(3):
-            step()
-        torch.cuda.synchronize()
-        steps = max(3, min(args.steps, 10))
-        ms = 0.0
-        for _ in range(steps):
-            flush_buf.zero_()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            step()
-            b.record()
-            b.synchronize()
-            ms += a.elapsed_time(b)
-        ms /= steps
-        # kernel durations of the first star
-        soap.soap_set_option(stars[0], soap.binding.SOAP_OPT_KERNEL_TIMING, 1)
-        soap.soap_disk_geometry(stars[0], wls[0], want_info=False)
-        soap.soap_integrate_quiet(stars[0], q, Q[0])
-        soap.soap_active_timeseries(stars[0], q, sp, fa, wls[0].regions, wls[0].phases, D[0])
-        st = soap.soap_get_stats(stars[0])
-        n_spec = len(wls) * (1 + n_ph)
-        line = {"workload": workloads.CONFIG_NAMES[int(name[1])], "vsini_kms": float(w0.vsini_kms), "stars": len(wls), "ms_per_step": ms,
-                "spectra_per_s": n_spec / (ms * 1e-3), "first_star": {
-                    "quiet_entries": st["quiet_entries"], "active_entries": st["active_entries"],
-                    "quiet_kernel_ms": st["quiet_kernel_ms"], "active_kernel_ms": st["active_kernel_ms"],
-                    "quiet_alu_frac": st["quiet_entries"] * P * FLOPS_PER_UNIT / (st["quiet_kernel_ms"] * 1e-3) / 1e12 / peak_tflops,
-                    "active_alu_frac": (st["active_entries"] * P * FLOPS_PER_UNIT / (st["active_kernel_ms"] * 1e-3) / 1e12 / peak_tflops)
-                    if st["active_kernel_ms"] > 0 else None}}
-        print(json.dumps(line))
-        for s_ in stars:
-            soap.soap_destroy(s_)
-        del Q, D, q, sp, fa
+    timer = Timer(torch, flush_buf)
+    make = {"C2": workloads.make_config2, "C3": workloads.make_config3, "C4": workloads.make_config4,
+            "C5": lambda: workloads.make_config5_star(0)}
+    wl = make[args.workload]()
+    if args.vsini is not None:
+        wl.vsini_kms = args.vsini
+    q = soap.to_device_spectra(wl.quiet, wl.lambda0, wl.dlambda, dev)
+    sp = soap.to_device_spectra(wl.spot, wl.lambda0, wl.dlambda, dev, wl.spot_contrast, wl.spot_lb)
+    fa = None if wl.facula is None else soap.to_device_spectra(wl.facula, wl.lambda0, wl.dlambda, dev, wl.facula_contrast, wl.facula_lb)
+    r, star, _, _ = time_form(soap, torch, timer, wl, q, sp, fa, args.form, max(3, min(args.steps, 10)), dev.index, peak_instr)
+    soap.soap_destroy(star)
+    r["workload"] = workloads.CONFIG_NAMES[int(args.workload[1])] + (" (first star)" if args.workload == "C5" else "")
+    r["vsini_kms"] = float(wl.vsini_kms)
+    print(json.dumps(r))
 
 
 def main():
@@ -493,15 +647,16 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["graft", "reference"], default="graft")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the C2 / C4 / C5 timings of the `configs` object")
     ap.add_argument("--form", type=int, default=None, help="SOAP_OPT_FORM of the timed star (default: the library's AUTO)")
-    ap.add_argument("--vsini", type=float, default=None, help="with --workload: override v sin i (km/s) of every star")
-    ap.add_argument("--workload", choices=["C3", "C2", "C4", "C5", "all"], default="C3",
-                    help="C3 (default) is the bench contract; the others print per-config timing lines only")
+    ap.add_argument("--vsini", type=float, default=None, help="with --workload: override v sin i (km/s)")
+    ap.add_argument("--workload", choices=["C2", "C3", "C4", "C5"], default=None,
+                    help="print one per-config timing line instead of the bench contract (which is C3)")
     args = ap.parse_args()
-    if args.impl != "reference" and (args.workload != "C3" or args.vsini is not None):
-        run_configs(args)
-    elif args.impl == "reference":
+    if args.impl == "reference":
         run_reference(args)
+    elif args.workload is not None:
+        run_configs(args)
     else:
         run_graft(args)
 

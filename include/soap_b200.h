@@ -218,6 +218,16 @@ int soap_lower_resolution(soap_star *star, const void *in, int64_t n_rows, int64
                           int32_t dtype, double lambda0, double dlambda, double resolution, void *out,
                           int64_t out_pitch, void *stream);
 
+/* ---- SOAPcontrast: wavelength-dependent contrast of an active region modelled by a temperature ----
+ * "Derives the contrast by calculating the ratio of two Planck functions at two different effective temperatures", one
+ * value per wavelength pixel:
+ *   out[m] = B_lambda(t_active) / B_lambda(t_quiet),  B_lambda(T) = (2 h c^2 / lambda^5) / (exp(h c / (lambda k_B T)) - 1),
+ *   lambda = lambda0 + m dlambda in ANGSTROM; temperatures in Kelvin (> 0).  Evaluated in fp64, rounded once to `dtype`.
+ * The result is what soap_spectra.contrast expects (the I_ratio of Eq. 3, applied after the shift, S17).
+ *   out: DEVICE [n_pix] of `dtype`.  Needs no geometry.  Asynchronous on `stream`. */
+int soap_contrast_planck(soap_star *star, double lambda0, double dlambda, int64_t n_pix, double t_quiet, double t_active,
+                         void *out, int32_t dtype, void *stream);
+
 /* ---- first-moment radial velocity of spectral lines (the RV reduction that follows the path) -----
  * The paper cross-correlates with a mask and fits a Gaussian; the mask is not available, and BASELINE.json's
  * acceptance functional is a first-moment RV per line, which this entry point computes on the device:
@@ -229,6 +239,13 @@ int soap_lower_resolution(soap_star *star, const void *in, int64_t n_rows, int64
 int soap_line_rvs(soap_star *star, const void *rows, int64_t n_rows, int64_t n_pix, int64_t pitch, int32_t dtype,
                   double lambda0, double dlambda, const double *centres, const double *half_widths, int64_t n_lines,
                   const double *norm, int64_t edge, double *out_rv, void *stream);
+
+/* ---- measurement aid: the device's FP32 FMA rate (not part of the path) ------------------------------------------
+ * Runs a register-only kernel of independent FMA chains (8 CTAs of 256 threads per SM, 16 accumulators per thread) and
+ * returns the best of four timed repetitions in FMAs per second.  packed != 0: fma.rn.f32x2 with a scalar-broadcast
+ * operand (SASS FFMA2) - the form of the shift-interpolate-accumulate inner loops; 0: plain FFMA.  bench.py reports it
+ * beside the derived peak (SMs x 128 lanes x clock) its `"bound": "alu"` roofline divides by.  Synchronous. */
+int soap_probe_fp32_rate(soap_star *star, int32_t packed, double *fma_per_s, void *stream);
 
 /* ---- debug export of the geometry (HOST outputs, N*N each, any may be NULL; synchronous) --------
  * Hidden cells: mu = 0, vel = 0, w = 0, bin = -1. */

@@ -29,7 +29,8 @@ EXPORTED_SYMBOLS = (
     "soap_version", "soap_create", "soap_destroy", "soap_last_error", "soap_set_option", "soap_get_stats",
     "soap_disk_geometry", "soap_integrate_quiet", "soap_active_timeseries", "soap_active_timeseries_effects",
     "soap_export_geometry", "soap_lower_resolution", "soap_active_timeseries_evolving", "soap_line_rvs",
-    "soap_synthesize_host", "soap_batch_integrate_quiet", "soap_batch_active_timeseries",
+    "soap_synthesize_host", "soap_batch_integrate_quiet", "soap_batch_active_timeseries", "soap_contrast_planck",
+    "soap_probe_fp32_rate",
 )
 
 
@@ -103,6 +104,8 @@ def load_library() -> ctypes.CDLL:
                                                    ctypes.POINTER(ctypes.c_double), i32, vp, vp, vp, i64,
                                                    ctypes.POINTER(i32), vp]
     lib.soap_export_geometry.argtypes = [vp, vp, vp, vp, vp]
+    lib.soap_probe_fp32_rate.argtypes = [vp, i32, ctypes.POINTER(ctypes.c_double), vp]
+    lib.soap_contrast_planck.argtypes = [vp, ctypes.c_double, ctypes.c_double, i64, ctypes.c_double, ctypes.c_double, vp, i32, vp]
     lib.soap_line_rvs.argtypes = [vp, vp, i64, i64, i64, i32, ctypes.c_double, ctypes.c_double, vp, vp, i64, vp, i64, vp, vp]
     lib.soap_active_timeseries_evolving.argtypes = [vp, ctypes.POINTER(c_spectra), ctypes.POINTER(c_spectra),
                                                     ctypes.POINTER(c_spectra), ctypes.POINTER(c_region), i32,
@@ -317,6 +320,23 @@ def soap_active_timeseries_evolving(star: Star, quiet: Spectra, spot: Optional[S
         out_cb.data_ptr() if out_cb is not None else None, out_pitch,
         na.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)) if na is not None else None, _stream_handle(stream)))
     return na[:n_ph] if na is not None else None
+
+
+def soap_probe_fp32_rate(star: Star, packed: bool = True, stream=None) -> float:
+    """FP32 FMAs per second of a register-only FMA kernel on the star's device (measurement aid of bench.py)."""
+    out = ctypes.c_double(0.0)
+    star._check(star._lib.soap_probe_fp32_rate(star._h, 1 if packed else 0, ctypes.byref(out), _stream_handle(stream)))
+    return float(out.value)
+
+
+def soap_contrast_planck(star: Star, lambda0: float, dlambda: float, n_pix: int, t_quiet: float, t_active: float,
+                         out: torch.Tensor, stream=None) -> torch.Tensor:
+    """SOAPcontrast (PAPER.md:312): out[m] = B_lambda(t_active) / B_lambda(t_quiet), lambda in Angstrom; out: DEVICE [n_pix]."""
+    if not out.is_contiguous() or out.numel() < n_pix:
+        raise ValueError("out must be a contiguous device tensor of at least n_pix elements")
+    star._check(star._lib.soap_contrast_planck(star._h, float(lambda0), float(dlambda), int(n_pix), float(t_quiet), float(t_active),
+                                               out.data_ptr(), _dtype_code(out), _stream_handle(stream)))
+    return out
 
 
 def soap_line_rvs(star: Star, rows: torch.Tensor, n_pix: int, lambda0: float, dlambda: float, centres: torch.Tensor,

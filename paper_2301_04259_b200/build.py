@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsoap_b200.so")
 SOURCES = [os.path.join(CSRC, "soap_api.cu")]
-HEADERS = [os.path.join(CSRC, f) for f in ("ptx_helpers.cuh", "composite.cuh", "geometry.cuh", "active.cuh", "sia.cuh", "sia_f32.cuh", "lsf.cuh", "rv.cuh")] + [
+HEADERS = [os.path.join(CSRC, f) for f in ("ptx_helpers.cuh", "composite.cuh", "contrast.cuh", "probe.cuh", "geometry.cuh", "active.cuh", "sia.cuh", "sia_f32.cuh", "lsf.cuh", "rv.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "soap_b200.h")]
 
 NVCC_FLAGS = [

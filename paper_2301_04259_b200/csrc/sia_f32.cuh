@@ -95,8 +95,8 @@ static_assert(sizeof(StarBlock) % 16 == 0 && sizeof(StarBlock) <= 192, "producer
 constexpr int kMaxBatchStars = 96;   // stars per active launch (their item offsets live in shared memory)
 
 struct Params {
-    StarBlock one;             // quiet launch: the star
-    const StarBlock *many;     // active launch: DEVICE [n_stars]
+    StarBlock one;             // quiet launch, and active launch of a single star: the star (no copy: a kernel argument)
+    const StarBlock *many;     // active launch of a batch: DEVICE [n_stars]; nullptr = `one`
     int n_stars;
     long long n_items;         // active launch: (phase, tile) items of all stars
     int halo;                  // largest halo of the launch: sizes the stages
@@ -288,9 +288,10 @@ struct ActiveSource {
             int ph = -1, tl = 0, c = 0, stx = cs_pub;
             if (valid) {
                 while (idx >= prefix[stx + 1]) ++stx;
-                const StarBlock &b = many[stx];
-                const int nt = __ldg(&b.n_tiles);
-                const int *po = ldg_ptr(&b.phase_order), *njp = ldg_ptr(&b.n_jobs);
+                // a single star: this warp's cached block is the star (filled at start); a batch: the star's block in global memory
+                const StarBlock *b = many ? many + stx : cache;
+                const int nt = many ? __ldg(&b->n_tiles) : b->n_tiles;
+                const int *po = many ? ldg_ptr(&b->phase_order) : b->phase_order, *njp = many ? ldg_ptr(&b->n_jobs) : b->n_jobs;
                 const long long local = idx - prefix[stx];
                 ph = __ldg(&po[local / nt]);
                 tl = (int)(local % nt);
@@ -340,7 +341,7 @@ struct ActiveSource {
         cnt = w >> 8;
         star = w & 255;
         nj = cnt > 0 ? cnt : 1;
-        if (star != cached_star) {  // this warp moves on to another star: copy its block
+        if (many && star != cached_star) {  // this warp moves on to another star: copy its block
             const int lane = threadIdx.x & 31;
             __syncwarp();
             if (lane < (int)(sizeof(StarBlock) / 16))
@@ -364,6 +365,11 @@ struct ActiveSource {
         pub_done = false;
         cs_pub = 0;
         cached_star = -1;
+        if (!many) {  // a single star: its block travels as a kernel argument
+            if ((threadIdx.x & 31) == 0) *cache = p.one;
+            __syncwarp();
+            cached_star = 0;
+        }
         i = -1;
         n0 = 0;
         nj = 0;
@@ -496,7 +502,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         reinterpret_cast<ItemQueue *>(smem + 128)->tail = 0;
     }
     if (ACTIVE) {
-        for (int k = tid; k <= p.n_stars; k += kThreads) prefix[k] = k < p.n_stars ? __ldg(&p.many[k].item0) : p.n_items;
+        for (int k = tid; k <= p.n_stars; k += kThreads)
+            prefix[k] = k < p.n_stars ? (p.many ? __ldg(&p.many[k].item0) : 0LL) : p.n_items;
     }
     __syncthreads();
 

@@ -16,8 +16,10 @@
 #include "../../include/soap_b200.h"
 #include "active.cuh"
 #include "composite.cuh"
+#include "contrast.cuh"
 #include "geometry.cuh"
 #include "lsf.cuh"
+#include "probe.cuh"
 #include "rv.cuh"
 #include "sia.cuh"
 #include "sia_f32.cuh"
@@ -482,8 +484,11 @@ struct ActiveCall {  // one star's arguments
 inline size_t align16(size_t v) { return (v + 15) & ~(size_t)15; }
 
 // `external_map`: the entry lists were built by the caller (per-cell form under differential rotation): only the blocks
-// are staged.
-int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, bool external_map, cudaStream_t st) {
+// are staged.  `map_only`: stop after the active map (soap_synthesize_host builds it before the table uploads are queued,
+// so that no small copy of the chunk loop waits behind them in the copy engine).  A single star's block travels as a
+// kernel argument: without `prepare` such a call copies nothing.
+int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, bool external_map, cudaStream_t st,
+                      bool map_only = false) {
     soap_star *own = calls[0].s;
     const bool use_lb = effect != SOAP_EFFECT_CB, use_contrast = effect != SOAP_EFFECT_CB;
     const bool quiet_rows = effect == SOAP_EFFECT_FLUX;
@@ -544,16 +549,24 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         blk_off = own->call_blk_off;
         ph_off = own->call_ph_off;
         total = ph_off;
-        if (!own->d_call.ptr || blk_off + (size_t)n * sizeof(f32::StarBlock) > ph_off)
+        if (n > 1 && (!own->d_call.ptr || blk_off + (size_t)n * sizeof(f32::StarBlock) > ph_off))
             return own->fail(SOAP_ERR_NOT_READY, "no prepared active map to reuse");
     }
-    soap_star::PinnedBytes &slot = own->h_call[own->h_call_next];
-    own->h_call_next = (own->h_call_next + 1) & 3;
+    const bool stage = prepare || n > 1;  // a single star without a new map needs no copy at all
+    std::vector<unsigned char> unstaged;
+    soap_star::PinnedBytes dummy;
+    soap_star::PinnedBytes &slot = stage ? own->h_call[own->h_call_next] : dummy;
+    if (stage) own->h_call_next = (own->h_call_next + 1) & 3;
+    if (!stage) {
+        unstaged.resize(total + 16);
+        dummy.ptr = unstaged.data();
+        dummy.cap = unstaged.size();
+    }
     if (slot.in_flight) {
         SOAP_CUDA(own, cudaEventSynchronize(slot.done));
         slot.in_flight = false;
     }
-    if (!slot.done) SOAP_CUDA(own, cudaEventCreateWithFlags(&slot.done, cudaEventDisableTiming));
+    if (stage && !slot.done) SOAP_CUDA(own, cudaEventCreateWithFlags(&slot.done, cudaEventDisableTiming));
     if (total > slot.cap) {
         if (slot.ptr) cudaFreeHost(slot.ptr);
         slot.ptr = nullptr;
@@ -561,7 +574,7 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         SOAP_CUDA(own, cudaMallocHost(reinterpret_cast<void **>(&slot.ptr), total + 4096));
         slot.cap = total + 4096;
     }
-    if (total > own->d_call.cap) {
+    if (stage && total > own->d_call.cap) {
         SOAP_CUDA(own, cudaDeviceSynchronize());  // growing frees the old buffer, which an earlier launch may still read
         SOAP_CUDA(own, own->d_call.reserve(total + 4096));
     }
@@ -640,14 +653,17 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         item0 += (long long)c.n_phases * b.n_tiles;
         s->last_tile_px = f32::kTile;
     }
+    const f32::StarBlock first_block = hb[0];
     if (prepare) {
         hph[n] = phase0;
         SOAP_CUDA(own, cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, st));
-    } else {
+    } else if (n > 1) {
         SOAP_CUDA(own, cudaMemcpyAsync(d + blk_off, h + blk_off, (size_t)n * sizeof(f32::StarBlock), cudaMemcpyHostToDevice, st));
     }
-    SOAP_CUDA(own, cudaEventRecord(slot.done, st));
-    slot.in_flight = true;
+    if (stage) {
+        SOAP_CUDA(own, cudaEventRecord(slot.done, st));
+        slot.in_flight = true;
+    }
 
     if (prepare && total_phases > 0) {
         // a4: one cluster of CTAs per (star, phase) bins, compacts and schedules (active.cuh)
@@ -660,10 +676,11 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
             none, reinterpret_cast<const PrepArgs *>(d + prep_off), reinterpret_cast<const int *>(d + ph_off), n);
         SOAP_LAUNCH_CHECK(own, "active_prepare_kernel");
     }
-    if (n_items == 0) return SOAP_OK;
+    if (n_items == 0 || map_only) return SOAP_OK;
     // a5 + a6: persistent CTAs over the (star, phase, tile) items
     f32::Params p{};
-    p.many = reinterpret_cast<const f32::StarBlock *>(d + blk_off);
+    p.one = first_block;
+    p.many = n > 1 ? reinterpret_cast<const f32::StarBlock *>(d + blk_off) : nullptr;
     p.n_stars = n;
     p.n_items = n_items;
     p.halo = max_halo;
@@ -909,12 +926,29 @@ int synthesize_host_pipelined(soap_star *s, const soap_star_params *prm, const s
         if (!in[k]->data || in[k]->n_pix != P || in[k]->pitch != pitch || in[k]->dtype != SOAP_F32)
             return s->fail(SOAP_ERR_INVALID_ARG, "spectra %d: data / n_pix / pitch / dtype differ from quiet", k);
     }
+    // every argument is checked before anything is enqueued (the tables are HOST memory here: the device-side alignment
+    // rule applies to the staged copies, which the library aligns itself)
+    for (int k = 0; k < 3; ++k) {
+        if (!in[k]) continue;
+        soap_spectra probe = *in[k];
+        probe.data = reinterpret_cast<const void *>(static_cast<uintptr_t>(256));
+        int rcv = check_spectra(s, &probe, k == 0 ? "quiet" : k == 1 ? "spot" : "facula");
+        if (rcv) return rcv;
+        if (k > 0 && (in[k]->lambda0 != quiet->lambda0 || in[k]->dlambda != quiet->dlambda))
+            return s->fail(SOAP_ERR_INVALID_ARG, "spectra %d: lambda0 / dlambda differ from quiet", k);
+    }
     int rc = soap_disk_geometry(s, prm, st, nullptr);
     if (rc) return rc;
     // the (small) region upload goes first: copies of one direction are served in issue order, and behind the table
     // uploads it would hold back the first chunk's kernels until every table has arrived
     if ((rc = check_regions(s, regions, n_regions, phases, n_phases, spot, facula))) return rc;
-    if ((rc = upload_region_centres(s, regions, n_regions, phases, n_phases, nullptr, st))) return rc;
+    const bool map_first = prm->diff_rot == 0.0;  // solid body: the active map is built here, ahead of the table uploads
+    if (map_first) {
+        ActiveCall c{s, quiet, spot, facula, regions, n_regions, phases, n_phases, nullptr, nullptr, P};
+        if ((rc = active_f32_launch(&c, 1, SOAP_EFFECT_TOTAL, true, false, st, true))) return rc;
+    } else if ((rc = upload_region_centres(s, regions, n_regions, phases, n_phases, nullptr, st))) {
+        return rc;
+    }
     if (!s->s_h2d) SOAP_CUDA(s, cudaStreamCreateWithFlags(&s->s_h2d, cudaStreamNonBlocking));
     if (!s->s_d2h) SOAP_CUDA(s, cudaStreamCreateWithFlags(&s->s_d2h, cudaStreamNonBlocking));
     const long long tiles = (P + f32::kTile - 1) / f32::kTile;
@@ -1000,7 +1034,7 @@ int synthesize_host_pipelined(soap_star *s, const soap_star_params *prm, const s
         s->out_hi_override = m1 - v0;
         rc = soap_integrate_quiet(s, &dev[0], dq + v0, st);
         if (!rc) {
-            s->reuse_lists = c > 0;  // the active map does not depend on the wavelength window
+            s->reuse_lists = map_first || c > 0;  // the active map does not depend on the wavelength window
             s->regions_uploaded = true;
             rc = soap_active_timeseries(s, &dev[0], spot ? &dev[1] : nullptr, facula ? &dev[2] : nullptr, regions, n_regions, phases,
                                         n_phases, dd + v0, P, nullptr, st);
@@ -1009,7 +1043,12 @@ int synthesize_host_pipelined(soap_star *s, const soap_star_params *prm, const s
         s->out_lo_override = s->out_hi_override = -1;
         s->reuse_lists = false;
         s->regions_uploaded = false;
-        if (rc) return rc;
+        if (rc) {  // nothing of this call may still be in flight when the caller gets its buffers back
+            cudaStreamSynchronize(st);
+            cudaStreamSynchronize(s->s_h2d);
+            cudaStreamSynchronize(s->s_d2h);
+            return rc;
+        }
         SOAP_CUDA(s, cudaEventRecord(ev_done(c), st));
         if (!zero_copy) {
             SOAP_CUDA(s, cudaStreamWaitEvent(s->s_d2h, ev_done(c), 0));
@@ -1394,6 +1433,58 @@ int soap_line_rvs(soap_star *s, const void *rows, int64_t n_rows, int64_t n_pix,
     if (dtype == SOAP_F32) line_rv_kernel<float><<<dim3(gx, gy), 32 * kRvWarps, 0, st>>>(a);
     else line_rv_kernel<double><<<dim3(gx, gy), 32 * kRvWarps, 0, st>>>(a);
     SOAP_LAUNCH_CHECK(s, "line_rv_kernel");
+    return SOAP_OK;
+}
+
+int soap_contrast_planck(soap_star *s, double lambda0, double dlambda, int64_t n_pix, double t_quiet, double t_active, void *out,
+                         int32_t dtype, void *stream) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!out) return s->fail(SOAP_ERR_INVALID_ARG, "out is NULL");
+    if (n_pix < 0 || n_pix > (1LL << 40)) return s->fail(SOAP_ERR_INVALID_ARG, "bad n_pix");
+    if (dtype != SOAP_F32 && dtype != SOAP_F64) return s->fail(SOAP_ERR_INVALID_ARG, "unknown dtype %d", dtype);
+    if (!(dlambda > 0.0) || !(lambda0 > 0.0) || !std::isfinite(dlambda) || !std::isfinite(lambda0))
+        return s->fail(SOAP_ERR_INVALID_ARG, "lambda0 and dlambda must be positive and finite");
+    if (!(t_quiet > 0.0) || !(t_active > 0.0) || !std::isfinite(t_quiet) || !std::isfinite(t_active))
+        return s->fail(SOAP_ERR_INVALID_ARG, "temperatures must be positive and finite");
+    if (n_pix == 0) return SOAP_OK;
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const unsigned grid = (unsigned)((n_pix + 255) / 256);
+    if (dtype == SOAP_F32)
+        contrast_planck_kernel<float><<<grid, 256, 0, st>>>(lambda0, dlambda, n_pix, 1.0 / t_quiet, 1.0 / t_active, static_cast<float *>(out));
+    else
+        contrast_planck_kernel<double><<<grid, 256, 0, st>>>(lambda0, dlambda, n_pix, 1.0 / t_quiet, 1.0 / t_active, static_cast<double *>(out));
+    SOAP_LAUNCH_CHECK(s, "contrast_planck_kernel");
+    return SOAP_OK;
+}
+
+int soap_probe_fp32_rate(soap_star *s, int32_t packed, double *fma_per_s, void *stream) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!fma_per_s) return s->fail(SOAP_ERR_INVALID_ARG, "fma_per_s is NULL");
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    SOAP_CUDA(s, s->d_info.reserve(1));
+    float *sink = reinterpret_cast<float *>(s->d_info.ptr);  // never written (see the kernel); any valid address will do
+    cudaEvent_t e0, e1;
+    SOAP_CUDA(s, cudaEventCreate(&e0));
+    SOAP_CUDA(s, cudaEventCreate(&e1));
+    const int iters = 4096, grid = s->n_sm * 8;  // 8 CTAs of 256 threads per SM: 64 warps, every sub-partition full
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {  // the first repetition warms up; best of the rest
+        SOAP_CUDA(s, cudaEventRecord(e0, st));
+        if (packed) fp32_probe_kernel<true><<<grid, kProbeThreads, 0, st>>>(iters, 1.0000001f, sink);
+        else fp32_probe_kernel<false><<<grid, kProbeThreads, 0, st>>>(iters, 1.0000001f, sink);
+        SOAP_CUDA(s, cudaEventRecord(e1, st));
+        SOAP_CUDA(s, cudaEventSynchronize(e1));
+        float ms = 0.f;
+        SOAP_CUDA(s, cudaEventElapsedTime(&ms, e0, e1));
+        const double fma = (double)grid * kProbeThreads * (double)iters * 8.0 * kProbeChains;
+        if (rep > 0 && ms > 0.f) best = std::max(best, fma / (ms * 1e-3));
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    SOAP_LAUNCH_CHECK(s, "fp32_probe_kernel");
+    *fma_per_s = best;
     return SOAP_OK;
 }
 

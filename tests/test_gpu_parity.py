@@ -491,3 +491,35 @@ def test_host_buffer_entry_point_pipelined_chunks(soap):
     gd = run_gpu(soap, wl)
     assert np.max(np.abs(gd["Q"] - g["Q"])) <= 1e-6 * oracle.geometry(wl)["sum_w"]   # a few fp32 ulps
     assert np.max(np.abs(gd["D"] - g["D"])) <= 1e-5 * np.max(np.abs(gd["D"]))
+
+
+def test_host_buffer_entry_point_pageable_buffers_and_bad_arguments(soap):
+    """The chunked host path with ordinary (pageable) numpy-backed tensors for inputs and outputs: results are staged on the
+    device and copied back chunk by chunk.  A bad table is refused before anything is enqueued: the outputs stay untouched."""
+    wl = workloads.make_config2(n_pix=140_000, n_phases=3, grid_n=40)
+    wl.phases = np.array([0.45, 0.5, 0.0])
+    wl.vsini_kms = 8.0
+    star = soap.soap_create(0)
+    pitch = (wl.n_pix + 3) & ~3
+
+    def host(rows):
+        t = torch.zeros((rows.shape[0], pitch), dtype=torch.float32)
+        t[:, :wl.n_pix] = torch.from_numpy(rows)
+        return t
+
+    q = soap.Spectra(host(wl.quiet), wl.n_pix, wl.lambda0, wl.dlambda)
+    s = soap.Spectra(host(wl.spot), wl.n_pix, wl.lambda0, wl.dlambda, contrast=torch.from_numpy(wl.spot_contrast.copy()), lb=wl.spot_lb)
+    Q = torch.full((wl.n_pix,), -7.0, dtype=torch.float32)
+    D = torch.full((len(wl.phases), wl.n_pix), -7.0, dtype=torch.float32)
+    assert not Q.is_pinned() and not D.is_pinned()
+    bad = soap.Spectra(s.data, wl.n_pix, wl.lambda0, wl.dlambda, contrast=s.contrast, lb=(float("nan"), 0.0, 0.0))
+    with pytest.raises(soap.SoapError) as e:
+        soap.soap_synthesize_host(star, wl, q, bad, None, wl.regions, wl.phases, Q, D)
+    assert e.value.code == soap.binding.SOAP_ERR_INVALID_ARG
+    torch.cuda.synchronize()
+    assert torch.all(Q == -7.0) and torch.all(D == -7.0)
+    na = soap.soap_synthesize_host(star, wl, q, s, None, wl.regions, wl.phases, Q, D, want_n_active=True)
+    soap.soap_destroy(star)
+    g = dict(Q=Q.numpy(), D=D.numpy(), n_active=na)
+    for lo in (0, 69_000, wl.n_pix - 900):
+        assert_parity(wl, g, lo, lo + 900, check_rv=False)
