@@ -40,14 +40,11 @@ constexpr int kActiveJobCap = 128;      // == f32::kJobCap
 constexpr int kPrepCluster = 8;         // CTAs per phase (portable cluster size)
 constexpr int kPrepThreads = 512;       // 16 warps per CTA
 constexpr int kPrepChunks = 4;          // 32-row chunks of a column whose cell data is loaded together
-constexpr int kScheduleSortMax = 4096;  // beyond this many phases the order is left as given
 
 struct ActiveCounters {  // device-resident
-    unsigned long long active_entries;  // sum over phases of entries (pad entries not counted)
-    unsigned int done;                  // CTAs finished (reset by the last one)
-    unsigned int pad;
     int item_next, item_ctas_done;      // hand-out of (phase, tile) items in the active launch (self-resetting)
     int overflow;                       // per-cell form: a phase's entry pool was too small (cannot happen with the host's bound)
+    int pad;
 };
 
 struct PrepArgs {
@@ -60,7 +57,7 @@ struct PrepArgs {
     int *seg_count;           // [n_phases * 3 n_mu]
     int *n_active;            // [n_phases] covered cells
     ActiveJob *jobs;          // [n_phases][job_cap]
-    int *n_jobs, *work, *phase_order;  // [n_phases] each
+    int *n_jobs, *work;       // [n_phases] each: jobs and entries of the phase (the active launch takes the heaviest first)
     ActiveCounters *counters;
     // per-cell form (differential rotation / SOAP_FORM_CELLS): every covered cell is an entry with its own shift
     const double *vel;        // [N*N] cell velocities
@@ -68,8 +65,20 @@ struct PrepArgs {
     int pool_cap;             // entries a phase's pool can hold (even); ent = [n_phases][pool_cap]
 };
 
-__host__ __device__ inline size_t prep_smem_bytes(int n_mu, int chunk_cols) {
-    return (size_t)3 * n_mu * chunk_cols * sizeof(double) + (size_t)3 * 3 * n_mu * sizeof(int) + 64;
+constexpr int kPrepRegSmem = 256;       // regions of a phase held in shared memory (more: read from global memory)
+struct PrepLayout {  // dynamic shared memory of active_prepare_kernel (byte offsets, each a multiple of 16)
+    size_t cnt_off, cols_off, reg_off, bytes;
+};
+__host__ __device__ inline PrepLayout prep_layout(int n_mu, int chunk_cols, int N, int n_regions) {
+    PrepLayout l;
+    l.cnt_off = ((size_t)3 * n_mu * chunk_cols * sizeof(double) + 15) & ~(size_t)15;
+    l.cols_off = l.cnt_off + (((size_t)kPrepCluster * 3 * n_mu * sizeof(int) + 15) & ~(size_t)15);
+    l.reg_off = l.cols_off + (((size_t)N * sizeof(int) + 15) & ~(size_t)15);
+    l.bytes = l.reg_off + (size_t)(n_regions <= kPrepRegSmem ? n_regions : 0) * sizeof(RegionAtPhase) + 16;
+    return l;
+}
+__host__ __device__ inline size_t prep_smem_bytes(int n_mu, int chunk_cols, int N, int n_regions) {
+    return prep_layout(n_mu, chunk_cols, N, n_regions).bytes;
 }
 
 
@@ -111,18 +120,42 @@ __device__ __forceinline__ int column_candidates(const RegionAtPhase *reg, int n
 }
 
 // grid = n_phases * kPrepCluster, block = kPrepThreads, cluster = kPrepCluster CTAs;
-// dynamic shared memory = prep_smem_bytes(n_mu, chunk_cols) with chunk_cols >= ceil(N / kPrepCluster).
+// dynamic shared memory = prep_smem_bytes(n_mu, chunk_cols, n_regions) with chunk_cols >= ceil(N / kPrepCluster).
 // Batch form (soap_batch_active_timeseries): `many` = DEVICE [n_stars] arguments, `phase0` = DEVICE [n_stars + 1] first
 // cluster (phase) of every star; cluster c serves phase c - phase0[s] of the star s that holds it.  many == nullptr: `one`.
-template <typename EntT>
+//
+// The kernel is latency-sized (a few thousand cells per phase), so its structure follows its dependent steps, not its
+// arithmetic: (1) arguments, the phase's regions -> shared memory, accumulators zeroed; (2) the columns any region can
+// reach, compacted into a list that the CTAs of the cluster share out evenly (two far-apart regions do not leave half
+// of the CTAs idle); (3) bin; (4) per-segment counts PUSHED into every CTA of the cluster through distributed shared
+// memory, one cluster barrier; (5) compaction behind the lower ranks' entries; rank 0 writes the job list (parallel
+// scan over the segments).  No CTA waits for another phase: the order in which the shift-interpolate-accumulate launch
+// takes the phases (heaviest first) is derived there from work[] (sia_f32.cuh).
+// `inl` (K > 0): the region centres of a single star's call travel as a kernel argument - [n_phases][n_regions], at most K -
+// so that the call needs no host -> device copy at all; K == 0: they are read from a.rp.
+template <int K>
+struct InlineRegions {
+    RegionAtPhase r[K > 0 ? K : 1];
+};
+constexpr int kInlineRegions = 192;  // 9 KB of kernel arguments
+
+template <typename EntT, int K>
 __global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThreads)
-active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, const int *__restrict__ phase0, int n_stars) {
+active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, const int *__restrict__ phase0, int n_stars,
+                      const __grid_constant__ InlineRegions<K> inl) {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) unsigned char prep_smem[];
     __shared__ PrepArgs s_args;
     __shared__ int s_phase;
-    if (threadIdx.x == 0) {
+    __shared__ int s_cand[kPrepThreads / 32][kCandCap];  // per warp: regions that can reach its column
+    __shared__ int s_misc[4];                            // reachable columns, covered cells of this CTA
+    __shared__ int s_cov[kPrepCluster];                  // rank 0: covered cells of every CTA (pushed)
+    __shared__ int s_wsum[kPrepThreads / 32 + 1], s_wjobs[kPrepThreads / 32 + 1];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = kPrepThreads / 32;
+    // every CTA of the cluster must be running before its shared memory is written remotely: arrive now, wait in (4)
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+    if (tid == 0) {
         const int c = blockIdx.x / kPrepCluster;
         if (many) {
             int lo = 0, hi = n_stars - 1;  // last star with phase0[s] <= c
@@ -137,46 +170,62 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
             s_args = one;
             s_phase = c;
         }
+        s_misc[0] = 0;
+        s_misc[2] = 0;
     }
     __syncthreads();
     const PrepArgs &a = s_args;
     const int n_seg = 3 * a.n_mu, N = a.N, cc = a.chunk_cols;
-    __shared__ int s_cand[kPrepThreads / 32][kCandCap];            // per warp: regions that can reach its column
-    double *WDs = reinterpret_cast<double *>(prep_smem);           // [n_seg][cc]: this CTA's columns
-    int *cnt = reinterpret_cast<int *>(WDs + (size_t)n_seg * cc);   // [n_seg] entries of this CTA (read by the others)
-    int *off = cnt + n_seg;                                         // [n_seg] entries of the lower ranks
-    int *tot = off + n_seg;                                         // [n_seg] entries of the whole phase
-    int *s_misc = tot + n_seg;  // j_lo, j_hi, covered cells of this CTA (read by rank 0), last-phase flag
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = kPrepThreads / 32;
+    const PrepLayout lay = prep_layout(a.n_mu, cc, N, a.n_regions);
+    double *WDs = reinterpret_cast<double *>(prep_smem);                  // [n_seg][cc]: this CTA's columns
+    int *cnt_all = reinterpret_cast<int *>(prep_smem + lay.cnt_off);      // [kPrepCluster][n_seg] entries of every CTA (pushed)
+    int *s_cols = reinterpret_cast<int *>(prep_smem + lay.cols_off);      // [N] reachable columns, ascending
+    const int n_reg_sm = a.n_regions <= kPrepRegSmem ? a.n_regions : 0;
+    RegionAtPhase *s_reg = reinterpret_cast<RegionAtPhase *>(prep_smem + lay.reg_off);  // [n_reg_sm]
     const int p = s_phase;
     const int rank = (int)cluster.block_rank();
-    const RegionAtPhase *reg = a.rp + (size_t)p * a.n_regions;
+    const RegionAtPhase *greg = (K > 0 ? inl.r : a.rp) + (size_t)p * a.n_regions;
     EntT *ent = static_cast<EntT *>(a.ent) + (size_t)p * n_seg * a.seg_cap;
 
-    if (tid == 0) {
-        s_misc[0] = N;
-        s_misc[1] = -1;
-        s_misc[2] = 0;
-        s_misc[3] = 0;
+    // ---- (1) regions -> shared memory (16-byte copies), accumulators zeroed ----------------------------------------------
+    {
+        const uint4 *src = reinterpret_cast<const uint4 *>(greg);
+        uint4 *dst = reinterpret_cast<uint4 *>(s_reg);
+        for (int k = tid; k < n_reg_sm * (int)(sizeof(RegionAtPhase) / 16); k += kPrepThreads) dst[k] = K > 0 ? src[k] : __ldg(&src[k]);
+        for (int k = tid; k < n_seg * cc; k += kPrepThreads) WDs[k] = 0.0;
     }
     __syncthreads();
-    // columns any region of this phase can reach (conservative: chord bound, slightly inflated)
-    for (int r = tid; r < a.n_regions; r += kPrepThreads) {
-        if (reg[r].type == 0) continue;
-        const double ch = reg[r].chord * (1.0 + 1e-9) + 1e-12;
-        int jl = (int)floor((reg[r].xr - ch + 1.0) * 0.5 * N - 0.5) - 1;
-        int jh = (int)ceil((reg[r].xr + ch + 1.0) * 0.5 * N - 0.5) + 1;
-        atomicMin(&s_misc[0], max(jl, 0));
-        atomicMax(&s_misc[1], min(jh, N - 1));
+    const RegionAtPhase *reg = n_reg_sm ? s_reg : greg;
+    // ---- (2) the columns some region of this phase can reach (conservative: chord bound, slightly inflated) -------------
+    for (int j0 = 0; j0 < N; j0 += kPrepThreads) {
+        const int j = j0 + tid;
+        bool hit = false;
+        if (j < N) {
+            const double x = cell_coord(j, N);
+            for (int r = 0; r < a.n_regions && !hit; ++r)
+                hit = reg[r].type != 0 && fabs(x - reg[r].xr) <= reg[r].chord * (1.0 + 1e-9) + 1e-12;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, hit);
+        if (lane == 0) s_wsum[warp] = __popc(m);
+        __syncthreads();
+        int before = s_misc[0];
+        for (int w = 0; w < warp; ++w) before += s_wsum[w];
+        if (hit) s_cols[before + __popc(m & ((1u << lane) - 1u))] = j;
+        __syncthreads();
+        if (tid == 0) {
+            int t = 0;
+            for (int w = 0; w < n_warps; ++w) t += s_wsum[w];
+            s_misc[0] += t;
+        }
+        __syncthreads();
     }
-    __syncthreads();
-    const int j_lo = s_misc[0], j_hi = s_misc[1];
-    const int per = (j_hi >= j_lo) ? (j_hi - j_lo + kPrepCluster) / kPrepCluster : 0;  // columns per CTA, <= cc
-    const int c0 = j_lo + rank * per;
-    const int cols = max(0, min(per, j_hi + 1 - c0));
-    if (j_hi < j_lo && a.n_phases > 1) {
-        // No region of this phase faces the observer (every CTA of the cluster sees the same j_lo, j_hi): an empty phase.
-        // Rank 0 records it and takes part in the ordering of the phases; nothing is binned, exchanged or compacted.
+    const int n_reach = s_misc[0];
+    const int per = (n_reach + kPrepCluster - 1) / kPrepCluster;  // columns per CTA, <= cc
+    const int k0c = rank * per;
+    const int cols = max(0, min(per, n_reach - k0c));
+    if (n_reach == 0 && a.n_phases > 1) {
+        // No region of this phase faces the observer (every CTA of the cluster sees the same list): an empty phase.
+        // Rank 0 records it; nothing is binned, exchanged or compacted.
         if (rank != 0) return;
         for (int s = tid; s < n_seg; s += kPrepThreads) a.seg_count[p * n_seg + s] = 0;
         if (tid == 0) {
@@ -184,12 +233,11 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
             a.work[p] = 0;
             a.n_active[p] = 0;
         }
-    } else {
-    for (int s = warp; s < n_seg; s += n_warps)
-        for (int k = lane; k < cols; k += 32) WDs[(size_t)s * cc + k] = 0.0;
-    __syncthreads();
-    // ---- bin: one warp per column, lanes over the rows (coalesced) --------------------------------------
-    for (int j = c0 + warp; j < c0 + cols; j += n_warps) {
+        return;
+    }
+    // ---- (3) bin: one warp per column, lanes over the rows (coalesced) -------------------------------------------------
+    for (int kc = warp; kc < cols; kc += n_warps) {
+        const int j = s_cols[k0c + kc];
         const double x = cell_coord(j, N);
         double ylo, yhi;
         const int n_cand = column_candidates(reg, a.n_regions, x, lane, s_cand[warp], ylo, yhi);
@@ -199,7 +247,7 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
         int i_hi = (int)ceil((yhi + 1.0) * 0.5 * N - 0.5) + 1;
         i_lo = max(i_lo, 0);
         i_hi = min(i_hi, N - 1);
-        double *col = WDs + (j - c0);
+        double *col = WDs + kc;
         int count = 0;
         for (int i00 = i_lo; i00 <= i_hi; i00 += 32 * kPrepChunks) {
             // all loads of up to kPrepChunks chunks are issued before any is used: one memory round trip
@@ -258,7 +306,8 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
         if (lane == 0 && count) atomicAdd(&s_misc[2], count);  // integer: order-independent
     }
     __syncthreads();
-    // ---- count this CTA's entries per segment, exchange through distributed shared memory ------------------
+    // ---- (4) this CTA's entries per segment, pushed to every CTA of the cluster -------------------------------------------
+    asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
     for (int s = warp; s < n_seg; s += n_warps) {
         const double *src = WDs + (size_t)s * cc;
         int c = 0;
@@ -266,28 +315,16 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
             const int k = k0 + lane;
             c += __popc(__ballot_sync(0xffffffffu, k < cols && src[k] != 0.0));
         }
-        if (lane == 0) cnt[s] = c;
+        if (lane < kPrepCluster) cluster.map_shared_rank(cnt_all, lane)[rank * n_seg + s] = c;
     }
-    cluster.sync();
-    for (int s = tid; s < n_seg; s += kPrepThreads) {
-        int before = 0, all = 0;
-        for (int r = 0; r < kPrepCluster; ++r) {
-            const int c = cluster.map_shared_rank(cnt, r)[s];
-            before += r < rank ? c : 0;
-            all += c;
-        }
-        off[s] = before;
-        tot[s] = all;
-    }
-    int covered = 0;
-    if (rank == 0 && tid == 0)
-        for (int r = 0; r < kPrepCluster; ++r) covered += cluster.map_shared_rank(s_misc, r)[2];
-    cluster.sync();  // no CTA leaves (or goes on to change cnt) while its shared memory is being read
-    // ---- compact: one warp per segment, this CTA's columns in order, behind the lower ranks' entries -------
+    if (tid == 0) cluster.map_shared_rank(s_cov, 0)[rank] = s_misc[2];
+    cluster.sync();  // every count has arrived; nobody touches another CTA's shared memory after this
+    // ---- (5) compact: one warp per segment, this CTA's columns in order, behind the lower ranks' entries -------------
     for (int s = warp; s < n_seg; s += n_warps) {
         const double sign = (s < a.n_mu) ? -1.0 : 1.0;
         const double *src = WDs + (size_t)s * cc;
-        int ps = off[s];
+        int ps = 0;
+        for (int r = 0; r < rank; ++r) ps += cnt_all[r * n_seg + s];
         EntT *dst = ent + (size_t)s * a.seg_cap;
         for (int k0 = 0; k0 < cols; k0 += 32) {
             const int k = k0 + lane;
@@ -295,7 +332,7 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
             const unsigned m = __ballot_sync(0xffffffffu, W != 0.0);
             if (W != 0.0) {
                 EntT e;
-                e.x = (decltype(e.x))a.col_a[c0 + k];
+                e.x = (decltype(e.x))a.col_a[s_cols[k0c + k]];
                 e.y = (decltype(e.y))(sign * W);
                 dst[ps + __popc(m & ((1u << lane) - 1u))] = e;
             }
@@ -303,88 +340,56 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
         }
     }
     if (rank != 0) return;
-    // ---- rank 0 finalises the phase: pad odd segments, counts, job list (contrast-carrying kinds 1, 2 first)
-    for (int s = tid; s < n_seg; s += kPrepThreads) {
-        const int c = tot[s];
-        if (c & 1) {  // zero-weight pad entry: every job's entry block stays a multiple of 16 bytes
-            EntT z;
-            z.x = 0;
-            z.y = 0;
-            ent[(size_t)s * a.seg_cap + c] = z;
+    // ---- rank 0 finalises the phase: pad odd segments, counts, job list (kinds 1, 2, then 0).  Thread t takes the t-th
+    // segment of the job order; jobs are numbered by a block-wide exclusive scan of the segments' job counts.
+    for (int t0 = 0, jobs_before = 0, work_sum = 0; t0 < n_seg || t0 == 0; t0 += kPrepThreads) {
+        const int t = t0 + tid;
+        int s = 0, c = 0;
+        if (t < n_seg) {
+            s = t + a.n_mu;
+            if (s >= n_seg) s -= n_seg;
+            for (int r = 0; r < kPrepCluster; ++r) c += cnt_all[r * n_seg + s];
+            if (c & 1) {  // zero-weight pad entry: every job's entry block stays a multiple of 16 bytes
+                EntT z;
+                z.x = 0;
+                z.y = 0;
+                ent[(size_t)s * a.seg_cap + c] = z;
+            }
+            a.seg_count[p * n_seg + s] = c;
         }
-        a.seg_count[p * n_seg + s] = c;
-    }
-    if (warp == 0) {
-        // lane l takes the segments ss in [l per_lane, (l+1) per_lane) of the job order; jobs are numbered by an
-        // exclusive warp scan of the lanes' job counts
-        const int per_lane = (n_seg + 31) / 32;
-        const int ss0 = lane * per_lane, ss1 = min(n_seg, ss0 + per_lane);
-        int nj = 0, wsum = 0;
-        for (int ss = ss0; ss < ss1; ++ss) {
-            const int c = tot[(ss + a.n_mu) % n_seg];
-            nj += (c + kActiveJobCap - 1) / kActiveJobCap;
-            wsum += c;
-        }
-        int incl = nj;
+        const int nj = (c + kActiveJobCap - 1) / kActiveJobCap;
+        int incl = nj, wsum = c;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += t;
-        }
-        int k = incl - nj;
-        for (int ss = ss0; ss < ss1; ++ss) {
-            const int s = (ss + a.n_mu) % n_seg;
-            const int c = tot[s];
-            for (int o = 0; o < c; o += kActiveJobCap) {
-                ActiveJob jb;
-                jb.begin = (p * n_seg + s) * a.seg_cap + o;  // fits: host checks n_phases * 3 n_mu * seg_cap < 2^31
-                jb.count = min(kActiveJobCap, c - o);
-                jb.kind = s / a.n_mu;
-                jb.row = s - jb.kind * a.n_mu;
-                a.jobs[(size_t)p * a.job_cap + k++] = jb;
-            }
+            const int u = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += u;
         }
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) wsum += __shfl_xor_sync(0xffffffffu, wsum, d);
-        const int n_jobs_total = __shfl_sync(0xffffffffu, incl, 31);
-        if (lane == 0) {
-            a.n_jobs[p] = n_jobs_total;
-            a.work[p] = wsum;
+        if (lane == 31) s_wjobs[warp] = incl;
+        if (lane == 0) s_wsum[warp] = wsum;
+        __syncthreads();
+        int k = jobs_before + incl - nj;
+        for (int w = 0; w < warp; ++w) k += s_wjobs[w];
+        for (int o = 0; o < c; o += kActiveJobCap) {
+            ActiveJob jb;
+            jb.begin = (p * n_seg + s) * a.seg_cap + o;  // fits: host checks n_phases * 3 n_mu * seg_cap < 2^31
+            jb.count = min(kActiveJobCap, c - o);
+            jb.kind = s / a.n_mu;
+            jb.row = s - jb.kind * a.n_mu;
+            a.jobs[(size_t)p * a.job_cap + k++] = jb;
+        }
+        for (int w = 0; w < n_warps; ++w) {
+            jobs_before += s_wjobs[w];
+            work_sum += s_wsum[w];
+        }
+        __syncthreads();
+        if (t0 + kPrepThreads >= n_seg && tid == 0) {
+            int covered = 0;
+            for (int r = 0; r < kPrepCluster; ++r) covered += s_cov[r];
+            a.n_jobs[p] = jobs_before;
+            a.work[p] = work_sum;
             a.n_active[p] = covered;
-        }
-    }
-    }  // (a phase with visible regions)
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-        const unsigned ticket = atomicAdd(&a.counters->done, 1u);
-        s_misc[3] = (ticket == (unsigned)a.n_phases - 1u) ? 1 : 0;
-    }
-    __syncthreads();
-    if (!s_misc[3]) return;
-    // ---- last phase to finish: order the phases by work, heaviest first (ties by phase index: deterministic)
-    __threadfence();
-    const volatile int *work = a.work;
-    for (int ph = tid; ph < a.n_phases; ph += kPrepThreads) {
-        int rk = ph;
-        if (a.n_phases <= kScheduleSortMax) {
-            const int w = work[ph];
-            rk = 0;
-            for (int q = 0; q < a.n_phases; ++q) {
-                const int wq = work[q];
-                rk += (wq > w || (wq == w && q < ph)) ? 1 : 0;
-            }
-        }
-        a.phase_order[rk] = ph;
-    }
-    if (warp == 0) {
-        unsigned long long total = 0;
-        for (int ph = lane; ph < a.n_phases; ph += 32) total += (unsigned long long)work[ph];
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) total += __shfl_xor_sync(0xffffffffu, total, d);
-        if (lane == 0) {
-            a.counters->active_entries = total;
-            a.counters->done = 0;  // ready for the next call on this handle
         }
     }
 }
@@ -448,7 +453,7 @@ active_prepare_cells_kernel(const PrepArgs a) {
     int *off = cnt + n_seg;                          // [n_seg] pool position of this CTA's block of the segment
     int *tot = off + n_seg;                          // [n_seg] entries of the whole phase
     int *base = tot + n_seg;                         // [n_seg] pool position of the segment
-    int *s_misc = base + n_seg;                      // j_lo, j_hi, covered cells of this CTA, last-phase flag
+    int *s_misc = base + n_seg;                      // j_lo, j_hi, covered cells of this CTA
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = kPrepThreads / 32;
     const int p = blockIdx.x / kPrepCluster;
     const int rank = (int)cluster.block_rank();
@@ -628,39 +633,6 @@ active_prepare_cells_kernel(const PrepArgs a) {
             a.n_jobs[p] = min(n_jobs_total, a.job_cap);
             a.work[p] = wsum;
             a.n_active[p] = covered;
-        }
-    }
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-        const unsigned ticket = atomicAdd(&a.counters->done, 1u);
-        s_misc[3] = (ticket == (unsigned)a.n_phases - 1u) ? 1 : 0;
-    }
-    __syncthreads();
-    if (!s_misc[3]) return;
-    // ---- last phase to finish: order the phases by work, heaviest first (ties by phase index: deterministic) ------
-    __threadfence();
-    const volatile int *work = a.work;
-    for (int ph = tid; ph < a.n_phases; ph += kPrepThreads) {
-        int rk = ph;
-        if (a.n_phases <= kScheduleSortMax) {
-            const int w = work[ph];
-            rk = 0;
-            for (int q = 0; q < a.n_phases; ++q) {
-                const int wq = work[q];
-                rk += (wq > w || (wq == w && q < ph)) ? 1 : 0;
-            }
-        }
-        a.phase_order[rk] = ph;
-    }
-    if (warp == 0) {
-        unsigned long long total = 0;
-        for (int ph = lane; ph < a.n_phases; ph += 32) total += (unsigned long long)work[ph];
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) total += __shfl_xor_sync(0xffffffffu, total, d);
-        if (lane == 0) {
-            a.counters->active_entries = total;
-            a.counters->done = 0;  // ready for the next call on this handle
         }
     }
 }

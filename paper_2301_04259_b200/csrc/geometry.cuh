@@ -232,6 +232,221 @@ __device__ void build_binned_entries(int N, int n_mu, const double *col_a, const
     }
 }
 
+// The same compaction - and the pair tables of the composite-column form (composite.cuh) - for grids whose binned
+// weights fit in shared memory (fin_smem_bytes(N, n_mu) <= kFinSmemMax: every configuration of BASELINE.json).  The last
+// CTA is alone on the critical path of the launch, and what it costs is dependent round trips to L2, not arithmetic:
+// here W[j][b], a_j and the per-column sums are fetched ONCE, all loads in flight together, into a transposed
+// shared-memory copy sW[b][j] (row pitch = 1 mod 16 doubles: conflict-free for the bin-major stores and the
+// column-major reads); counts, prefix sums, entries and pair tables are then built from shared memory.
+constexpr size_t kFinSmemMax = 160 * 1024;
+__host__ __device__ inline int fin_pitch(int N) { return ((N + 14) / 16) * 16 + 1; }  // >= N, = 1 (mod 16)
+__host__ __device__ inline size_t fin_smem_bytes(int N, int n_mu) {
+    return ((size_t)n_mu * fin_pitch(N) + (size_t)N) * sizeof(double) + ((size_t)(N + 1) / 2 + 2) * sizeof(int);
+}
+
+__device__ void finalize_columns_smem(int N, int n_mu, const double *col_a, const double *Wbin, const double *col_sumw,
+                                      const int *col_nvis, float2 *ent32, double2 *ent64, int *row_start, DevInfo *info,
+                                      float2 *comp_Wp, int comp_stride, comp::PairHdr *comp_hdr, unsigned char *dyn) {
+    __shared__ int s_cnt[64];
+    __shared__ int s_start[65];
+    __shared__ long long s_nv[32];
+    __shared__ double s_sw[32], s_am[32];
+    __shared__ int s_carry[33];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = blockDim.x >> 5, nt = blockDim.x;
+    const int Np = fin_pitch(N);
+    double *sW = reinterpret_cast<double *>(dyn);  // [n_mu][Np]
+    double *sA = sW + (size_t)n_mu * Np;           // [N]
+    int *s_cost = reinterpret_cast<int *>(sA + N);  // [n_pairs + 1] exclusive cost prefix of the column pairs
+    // ---- one round trip: every load is independent of every other (written by other SMs: read through L2) ----------
+    constexpr int kInFlight = 8;  // loads a thread issues before it uses the first
+    long long nv = 0;
+    double sw = 0.0, am = 0.0;
+    {
+        const int j = tid;  // first round of the per-column sums: in flight with the first weights
+        const int c = j < N ? __ldcg(&col_nvis[j]) : 0;
+        const double a = j < N ? __ldcg(&col_a[j]) : 0.0, cs = j < N ? __ldcg(&col_sumw[j]) : 0.0;
+        for (int k0 = 0; k0 < N * n_mu; k0 += nt * kInFlight) {
+            double v[kInFlight];
+#pragma unroll
+            for (int u = 0; u < kInFlight; ++u) {
+                const int k = k0 + u * nt + tid;
+                v[u] = k < N * n_mu ? __ldcg(&Wbin[k]) : 0.0;
+            }
+#pragma unroll
+            for (int u = 0; u < kInFlight; ++u) {
+                const int k = k0 + u * nt + tid;
+                if (k < N * n_mu) {
+                    const int jj = k / n_mu, b = k - jj * n_mu;
+                    sW[(size_t)b * Np + jj] = v[u];
+                }
+            }
+        }
+        if (j < N) {
+            sA[j] = a;
+            nv = c;
+            sw = cs;
+            if (c > 0) am = fabs(a);
+        }
+    }
+    for (int j = tid + nt; j < N; j += nt) {
+        const int c = __ldcg(&col_nvis[j]);
+        const double a = __ldcg(&col_a[j]);
+        sA[j] = a;
+        nv += c;
+        sw += __ldcg(&col_sumw[j]);
+        if (c > 0) am = fmax(am, fabs(a));
+    }
+    // summary: fixed xor tree inside the warps, then over the warps (deterministic)
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        nv += __shfl_xor_sync(0xffffffffu, nv, d);
+        sw += __shfl_xor_sync(0xffffffffu, sw, d);
+        am = fmax(am, __shfl_xor_sync(0xffffffffu, am, d));
+    }
+    if (lane == 0) {
+        s_nv[warp] = nv;
+        s_sw[warp] = sw;
+        s_am[warp] = am;
+    }
+    __syncthreads();  // sW, sA complete
+    // ---- entries per mu bin ------------------------------------------------------------------------------------------
+    for (int b = warp; b < n_mu; b += n_warps) {
+        const double *row = sW + (size_t)b * Np;
+        int cnt = 0;
+        for (int j0 = 0; j0 < N; j0 += 32) {
+            const int j = j0 + lane;
+            cnt += __popc(__ballot_sync(0xffffffffu, j < N && row[j] != 0.0));
+        }
+        if (lane == 0) s_cnt[b] = cnt;
+    }
+    __syncthreads();
+    if (warp == 0) {
+        // row starts (rows padded to an even length) by a warp scan over <= 64 bins; the summary's last step
+        int v0 = lane < n_mu ? ((s_cnt[lane] + 1) & ~1) : 0, v1 = lane + 32 < n_mu ? ((s_cnt[lane + 32] + 1) & ~1) : 0;
+        int t0 = lane < n_mu ? s_cnt[lane] : 0, t1 = lane + 32 < n_mu ? s_cnt[lane + 32] : 0;
+        int i0 = v0, i1 = v1;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int u0 = __shfl_up_sync(0xffffffffu, i0, d), u1 = __shfl_up_sync(0xffffffffu, i1, d);
+            if (lane >= d) {
+                i0 += u0;
+                i1 += u1;
+            }
+        }
+        const int first = __shfl_sync(0xffffffffu, i0, 31);
+        s_start[lane] = i0 - v0;
+        s_start[lane + 32] = first + i1 - v1;
+        if (lane == 31) s_start[64] = first + i1;
+        int total = t0 + t1;
+        long long nvt = lane < n_warps ? s_nv[lane] : 0;
+        double swt = 0.0, amt = lane < n_warps ? s_am[lane] : 0.0;
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            total += __shfl_xor_sync(0xffffffffu, total, d);
+            nvt += __shfl_xor_sync(0xffffffffu, nvt, d);
+            amt = fmax(amt, __shfl_xor_sync(0xffffffffu, amt, d));
+        }
+        if (lane == 0) {
+            for (int w = 0; w < n_warps; ++w) swt += s_sw[w];  // warp order
+            info->n_visible = nvt;
+            info->n_entries = total;
+            info->sum_weights = swt;
+            info->max_abs_dshift = amt;
+        }
+    }
+    __syncthreads();
+    for (int b = tid; b <= n_mu; b += nt) row_start[b] = s_start[b];  // s_start[n_mu] = the padded total
+    for (int b = warp; b < n_mu; b += n_warps) {
+        const double *row = sW + (size_t)b * Np;
+        int pos = s_start[b];
+        for (int j0 = 0; j0 < N; j0 += 32) {
+            const int j = j0 + lane;
+            const double W = j < N ? row[j] : 0.0;
+            const unsigned m = __ballot_sync(0xffffffffu, W != 0.0);
+            if (W != 0.0) {
+                const int e = pos + __popc(m & ((1u << lane) - 1u));
+                const double A = sA[j];
+                ent32[e] = make_float2((float)A, (float)W);
+                ent64[e] = make_double2(A, W);
+            }
+            pos += __popc(m);
+        }
+        if (lane == 0 && (s_cnt[b] & 1)) {
+            ent32[pos] = make_float2(0.f, 0.f);
+            ent64[pos] = make_double2(0.0, 0.0);
+        }
+    }
+    if (!comp_Wp) return;
+    // ---- pair tables of the composite-column form: (W[2p][b], W[2p+1][b]) as float2, the pair's shift factors, the
+    // number of weight loads that cover its non-zero bins, and the exclusive prefix of the pairs' costs ---------------
+    const int n_pairs = (N + 1) / 2;
+    for (int k = tid; k < n_pairs * comp_stride; k += nt) {
+        const int p = k / comp_stride, b = k - p * comp_stride;
+        float2 w = make_float2(0.f, 0.f);
+        if (b < n_mu) {
+            w.x = (float)sW[(size_t)b * Np + 2 * p];
+            if (2 * p + 1 < N) w.y = (float)sW[(size_t)b * Np + 2 * p + 1];
+        }
+        comp_Wp[k] = w;
+    }
+    for (int p = warp; p < n_pairs; p += n_warps) {
+        const int j0 = 2 * p, j1 = 2 * p + 1;
+        int hi = -1;
+        for (int b0 = 0; b0 < n_mu; b0 += 32) {
+            const int b = b0 + lane;
+            const bool nz = b < n_mu && (sW[(size_t)b * Np + j0] != 0.0 || (j1 < N && sW[(size_t)b * Np + j1] != 0.0));
+            const unsigned m = __ballot_sync(0xffffffffu, nz);
+            if (m) hi = b0 + 31 - __clz(m);
+        }
+        if (lane == 0) s_cost[p] = (hi + 2) / 2;  // nl for now
+    }
+    __syncthreads();
+    // exclusive scan of the costs, 32 * n_warps pairs per round (one round up to N = 2048)
+    int carry = 0;
+    for (int p0 = 0; p0 < n_pairs; p0 += nt) {
+        const int p = p0 + tid;
+        const int nl = p < n_pairs ? s_cost[p] : 0;
+        const int c = p < n_pairs ? 8 * nl + comp::kPairCostBase : 0;
+        int incl = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int u = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += u;
+        }
+        if (lane == 31) s_carry[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            const int v = lane < n_warps ? s_carry[lane] : 0;
+            int iw = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int u = __shfl_up_sync(0xffffffffu, iw, d);
+                if (lane >= d) iw += u;
+            }
+            s_carry[lane] = iw - v;
+            if (lane == 31) s_carry[32] = iw;
+        }
+        __syncthreads();
+        if (p < n_pairs) {
+            comp::PairHdr h;
+            h.a0 = (float)sA[2 * p];
+            h.a1 = 2 * p + 1 < N ? (float)sA[2 * p + 1] : 0.f;
+            h.nl = nl;
+            h.cost0 = carry + s_carry[warp] + incl - c;
+            comp_hdr[p] = h;
+        }
+        carry += s_carry[32];
+        __syncthreads();
+    }
+    if (tid == 0) {
+        comp::PairHdr t;
+        t.a0 = t.a1 = 0.f;
+        t.nl = 0;
+        t.cost0 = carry;
+        comp_hdr[n_pairs] = t;
+    }
+}
+
 // Per-cell form (SOAP_FORM_CELLS, and always under differential rotation, where the cells of a column no longer
 // share a velocity): one entry per visible cell - the literal double loop of Alg. 1 - in the same layout, rows
 // sorted by (column, row) so that neighbouring entries have nearly equal shifts.  The last CTA of geometry_kernel
@@ -314,7 +529,8 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
                 unsigned int *__restrict__ done, int *__restrict__ colcnt /*[N][n_mu]*/,
                 int *__restrict__ cellpos /*[n_mu][N], per-cell form only*/, int cells,
                 float2 *__restrict__ comp_Wp /*composite form: [ceil(N/2)][comp_stride], or nullptr*/, int comp_stride,
-                comp::PairHdr *__restrict__ comp_hdr) {
+                comp::PairHdr *__restrict__ comp_hdr, int fin_smem /*dynamic shared memory holds fin_smem_bytes(N, n_mu)*/) {
+    extern __shared__ __align__(16) unsigned char geom_dyn[];
     __shared__ double s_W[kGeomWarps][64];
     __shared__ int s_Cn[kGeomWarps][64];
     __shared__ double s_mu[64];
@@ -333,8 +549,13 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
     const int j = blockIdx.x * cpc + cl;
     double sum = 0.0;
     int nvis = 0;
-    if (cl < cpc && j < N)
+    if (cl < cpc && j < N) {
         geometry_chunks(j, chunk, wpc, N, rot, u1, u2, n_mu, s_mu, s_W[warp], s_Cn[warp], mu_out, w_out, vel_out, bin_out, sum, nvis);
+        // the column's shift factor (solid body; with differential rotation the per-cell form is used instead): by the
+        // warp of the column's first chunk, whose cells are mostly off the disk - it has time to spare
+        if (chunk == 0 && lane == 0)
+            col_a[j] = doppler_minus_one(__dmul_rn(__dmul_rn(cell_coord(j, N), rot.vsini), rot.sini), mode);
+    }
     if (lane == 0) {
         s_sum[warp] = sum;
         s_nvis[warp] = nvis;
@@ -360,8 +581,6 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
                     sw += s_sum[warp * wpc + k];
                     nv += s_nvis[warp * wpc + k];
                 }
-                // the column's shift factor (solid body; with differential rotation the per-cell form is used instead)
-                col_a[jj] = doppler_minus_one(__dmul_rn(__dmul_rn(cell_coord(jj, N), rot.vsini), rot.sini), mode);
                 col_sumw[jj] = sw;
                 col_nvis[jj] = nv;
             }
@@ -374,10 +593,15 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
     if (!s_last) return;
     __threadfence();
     if (threadIdx.x == 0) *done = 0;
-    build_binned_entries(N, n_mu, col_a, Wbin, col_sumw, col_nvis, ent32, ent64, row_start, info);
-    if (comp_Wp) {  // pair tables of the composite-column form (composite.cuh)
-        __syncthreads();
-        comp::build_composite_tables(N, n_mu, col_a, Wbin, comp_Wp, comp_stride, comp_hdr);
+    if (fin_smem) {
+        finalize_columns_smem(N, n_mu, col_a, Wbin, col_sumw, col_nvis, ent32, ent64, row_start, info, comp_Wp, comp_stride, comp_hdr,
+                              geom_dyn);
+    } else {
+        build_binned_entries(N, n_mu, col_a, Wbin, col_sumw, col_nvis, ent32, ent64, row_start, info);
+        if (comp_Wp) {  // pair tables of the composite-column form (composite.cuh)
+            __syncthreads();
+            comp::build_composite_tables(N, n_mu, col_a, Wbin, comp_Wp, comp_stride, comp_hdr);
+        }
     }
     if (cells) {  // per-cell form: the entry list is rebuilt by write_cell_entries_kernel at these positions
         __syncthreads();

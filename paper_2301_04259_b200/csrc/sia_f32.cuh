@@ -85,7 +85,7 @@ struct StarBlock {
     // active launch
     const ActiveJob *jobs;     // [n_phases][job_cap]
     const int *n_jobs;         // [n_phases]
-    const int *phase_order;    // [n_phases] heaviest first
+    const int *work;           // [n_phases] entries of every phase: the launch takes the heaviest phases first
     long long item0;           // first (phase, tile) item of this star in the launch's item list
     int halo;                  // H: multiple of 4, >= max |delta| + 2
     int n_mu, n_tiles, job_cap, n_phases, pad;
@@ -158,7 +158,10 @@ __host__ __device__ inline StageLayout stage_layout(int halo) {
 constexpr size_t kPrefixOff = 1280;                           // active launch: first item of every star, [kMaxBatchStars + 1]
 constexpr size_t kBlockCacheOff = 2176;                       // active launch: the star block each producer warp works on
 constexpr size_t kBlockCacheStride = 192;                     // >= sizeof(StarBlock), multiple of 16
-constexpr size_t kHeaderBytes = 3072;                         // mbarriers (96 B), tile hand-over words, item queue (at 128), prefix, blocks
+constexpr int kOrderCap = 256;                                // phases of one star the scheduler orders by work (more: as given)
+constexpr size_t kOrderOff = 3072;                            // active launch, scheduler warp: order and jobs of the phases of one
+                                                              // star, [kOrderCap] unsigned short each
+constexpr size_t kHeaderBytes = 3072 + kOrderCap * 4;         // mbarriers (96 B), tile hand-over words, item queue (at 128), prefix, blocks, order
 constexpr size_t kFinBytes = (size_t)kTile * (sizeof(double) + sizeof(float));  // active launch: per-pixel fp64
                                                                               // contrast-weighted sums + staged contrast
 __host__ inline size_t smem_bytes(int halo, bool active) {
@@ -265,6 +268,10 @@ struct ActiveSource {
     int *counters;  // [0] next item, [1] CTAs that finished fetching (both zero between launches)
     ItemQueue *queue;
     StarBlock *cache;  // shared memory: this warp's copy of the block of the star it is working on
+    unsigned short *s_order;    // scheduler: the phases of star `ord_star`, heaviest first (ties by phase index)
+    unsigned short *s_njobs;    // scheduler: jobs of its phases
+    int ord_star;
+    bool ord_identity;          // more than kOrderCap phases: taken as given
     long long n_items;
     int n_stars, chunk;
     bool scheduler;
@@ -275,6 +282,42 @@ struct ActiveSource {
     int i;             // item this warp is working through
     int n0, nj, cnt, phase, tile, star;
     bool done;
+    // scheduler warp: the phases of star `st` ordered by work, heaviest first (list scheduling: the CTAs then finish within
+    // one small item of each other).  Which CTA computes an item, and when, does not change its result.
+    __device__ void load_order(int st) {
+        const int lane = threadIdx.x & 31;
+        const StarBlock *b = many ? many + st : cache;
+        const int n = many ? __ldg(&b->n_phases) : b->n_phases;
+        const int *wk = many ? ldg_ptr(&b->work) : b->work, *njp = many ? ldg_ptr(&b->n_jobs) : b->n_jobs;
+        ord_star = st;
+        ord_identity = n > kOrderCap;
+#ifdef EXP_NOORDER
+        ord_identity = true;
+#endif
+        if (ord_identity) return;
+        __syncwarp();
+        bool wide = false;
+        for (int k = lane; k < n; k += 32) {
+            const int nj = __ldg(&njp[k]);
+            s_njobs[k] = (unsigned short)nj;
+            wide = wide || nj > 0xffff;
+        }
+        if (__any_sync(0xffffffffu, wide)) {  // job counts beyond 16 bits: taken as given, counts read from global memory
+            ord_identity = true;
+            return;
+        }
+        for (int ph = lane; ph < n; ph += 32) {  // rank of phase ph = phases that go before it (the list is L1-resident)
+            const int w = __ldg(&wk[ph]);
+            int rk = 0;
+#pragma unroll 4
+            for (int q = 0; q < n; ++q) {
+                const int wq = __ldg(&wk[q]);
+                rk += (wq > w || (wq == w && q < ph)) ? 1 : 0;
+            }
+            s_order[rk] = (unsigned short)ph;
+        }
+        __syncwarp();
+    }
     // scheduler warp: publish items until they cover job number n_need (or the list is exhausted).  A hand-out takes
     // `chunk` consecutive items; lane l looks up item l of it (star, phase, tile, jobs of the phase).
     __device__ void publish_until(int n_need) {
@@ -286,16 +329,28 @@ struct ActiveSource {
             const long long idx = (long long)first + lane;
             const bool valid = lane < chunk && idx < n_items;
             int ph = -1, tl = 0, c = 0, stx = cs_pub;
-            if (valid) {
+            if (valid)
                 while (idx >= prefix[stx + 1]) ++stx;
-                // a single star: this warp's cached block is the star (filled at start); a batch: the star's block in global memory
-                const StarBlock *b = many ? many + stx : cache;
-                const int nt = many ? __ldg(&b->n_tiles) : b->n_tiles;
-                const int *po = many ? ldg_ptr(&b->phase_order) : b->phase_order, *njp = many ? ldg_ptr(&b->n_jobs) : b->n_jobs;
-                const long long local = idx - prefix[stx];
-                ph = __ldg(&po[local / nt]);
-                tl = (int)(local % nt);
-                c = __ldg(&njp[ph]);
+            unsigned todo = __ballot_sync(0xffffffffu, valid);
+            while (todo) {  // star by star (a hand-out rarely spans more than one)
+                const int st = __shfl_sync(0xffffffffu, stx, __ffs(todo) - 1);
+                if (st != ord_star) load_order(st);
+                const bool mine = valid && stx == st;
+                if (mine) {
+                    const StarBlock *b = many ? many + st : cache;
+                    const int nt = many ? __ldg(&b->n_tiles) : b->n_tiles;
+                    const long long local = idx - prefix[st];
+                    const int k = (int)(local / nt);
+                    tl = (int)(local - (long long)k * nt);
+                    if (ord_identity) {
+                        ph = k;
+                        c = __ldg((many ? ldg_ptr(&b->n_jobs) : b->n_jobs) + ph);
+                    } else {
+                        ph = s_order[k];
+                        c = s_njobs[ph];
+                    }
+                }
+                todo &= ~__ballot_sync(0xffffffffu, mine);
             }
             const int jobs = valid ? (c > 0 ? c : 1) : 0;
             int incl = jobs;
@@ -350,7 +405,12 @@ struct ActiveSource {
             cached_star = star;
         }
     }
-    __device__ void init(const Params &p, ItemQueue *q, const long long *pref, StarBlock *my_cache, bool is_scheduler) {
+    __device__ void init(const Params &p, ItemQueue *q, const long long *pref, StarBlock *my_cache, bool is_scheduler,
+                         unsigned char *order_mem) {
+        s_order = reinterpret_cast<unsigned short *>(order_mem);
+        s_njobs = s_order + kOrderCap;
+        ord_star = -1;
+        ord_identity = false;
         many = p.many;
         prefix = pref;
         counters = p.item_counters;
@@ -406,7 +466,12 @@ struct ActiveSource {
 __device__ __forceinline__ void consumer_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory"); }
 
 __device__ __forceinline__ void mbar_wait_backoff(uint64_t *bar, uint32_t parity) {
+#ifdef EXP_WAITHINT
+    while (!mbar_try_wait_hint(bar, parity, EXP_WAITHINT)) {
+    }
+#else
     while (!mbar_try_wait(bar, parity)) __nanosleep(40);
+#endif
 }
 
 // One producer warp: turns the `count` raw entries (a, W) of a job into records and the run table of a tile
@@ -468,12 +533,13 @@ __device__ __forceinline__ int build_runs(const float2 *raw, int count, float c_
     return n_runs;
 }
 
-__device__ __forceinline__ void init_source(QuietSource &src, const Params &p, ItemQueue *, const long long *, StarBlock *, bool) {
+__device__ __forceinline__ void init_source(QuietSource &src, const Params &p, ItemQueue *, const long long *, StarBlock *, bool,
+                                            unsigned char *) {
     src.init(p, blockIdx.x, gridDim.x);
 }
 __device__ __forceinline__ void init_source(ActiveSource &src, const Params &p, ItemQueue *q, const long long *prefix,
-                                            StarBlock *cache, bool is_scheduler) {
-    src.init(p, q, prefix, cache, is_scheduler);
+                                            StarBlock *cache, bool is_scheduler, unsigned char *order_mem) {
+    src.init(p, q, prefix, cache, is_scheduler, order_mem);
 }
 __device__ __forceinline__ const StarBlock &source_block(const QuietSource &, const Params &p) { return p.one; }
 __device__ __forceinline__ const StarBlock &source_block(const ActiveSource &src, const Params &) { return *src.cache; }
@@ -519,7 +585,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         Desc *desc = reinterpret_cast<Desc *>(sb + p.desc_off);
         typename std::conditional<ACTIVE, ActiveSource, QuietSource>::type src;
         init_source(src, p, reinterpret_cast<ItemQueue *>(smem + 128), prefix,
-                    reinterpret_cast<StarBlock *>(smem + kBlockCacheOff + (size_t)st * kBlockCacheStride), st == 0);
+                    reinterpret_cast<StarBlock *>(smem + kBlockCacheOff + (size_t)st * kBlockCacheStride), st == 0, smem + kOrderOff);
         Job jb;
         for (int n = st, use = 0;; n += kStages, ++use) {
             const int status = src.get(n, jb);

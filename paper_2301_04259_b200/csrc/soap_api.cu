@@ -119,7 +119,7 @@ struct soap_star {
     } h_call[4];
     int h_call_next = 0;
     size_t call_rp_off = 0, call_prep_off = 0, call_blk_off = 0, call_ph_off = 0;  // sections of d_call of the last prepared call
-    bool attr_active_set = false, attr_prep_set = false;
+    bool attr_active_set = false, attr_prep_set = false, attr_prep_inl_set = false, attr_geom_set = false;
     int occ_active = 0;
     size_t occ_active_smem = 0;
 
@@ -129,6 +129,7 @@ struct soap_star {
     // stats
     int last_quiet_splits = 0, last_tile_px = 0, launches = 0, last_form = 0;
     long long last_active_cells = 0;
+    int last_n_phases = 0;  // phases of the last active call: d_sched = [n_jobs | entries] of each
 
     int fail(int code, const char *fmt, ...) {
         char buf[512];
@@ -512,11 +513,12 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
             SOAP_CUDA(s, cudaMemsetAsync(s->d_counters.ptr, 0, sizeof(ActiveCounters), st));  // once per handle
         }
         SOAP_CUDA(s, s->d_jobs.reserve((size_t)c.n_phases * per_cell_cap(s, n_mu, ncap)));
-        SOAP_CUDA(s, s->d_sched.reserve((size_t)3 * c.n_phases));
+        SOAP_CUDA(s, s->d_sched.reserve((size_t)2 * c.n_phases));
         const int chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);
-        if (prep_smem_bytes(n_mu, chunk_cols) > 200 * 1024)
+        if (prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions) > 200 * 1024)
             return s->fail(SOAP_ERR_UNSUPPORTED, "grid_n %d with %d mu bins exceeds the active-map kernel's shared memory", N, n_mu);
-        prep_smem = std::max(prep_smem, prep_smem_bytes(n_mu, chunk_cols));
+        prep_smem = std::max(prep_smem, prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions));
+        s->last_n_phases = c.n_phases;
         n_rp += (size_t)c.n_regions * c.n_phases;
         total_phases += c.n_phases;
         max_halo = std::max(max_halo, halo_for(s, c.q));
@@ -552,7 +554,9 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         if (n > 1 && (!own->d_call.ptr || blk_off + (size_t)n * sizeof(f32::StarBlock) > ph_off))
             return own->fail(SOAP_ERR_NOT_READY, "no prepared active map to reuse");
     }
-    const bool stage = prepare || n > 1;  // a single star without a new map needs no copy at all
+    // a single star's region centres travel as a kernel argument when they fit: such a call copies nothing
+    const bool inline_rp = prepare && n == 1 && n_rp <= (size_t)kInlineRegions;
+    const bool stage = (prepare && !inline_rp) || n > 1;  // a single star without a new map needs no copy either
     std::vector<unsigned char> unstaged;
     soap_star::PinnedBytes dummy;
     soap_star::PinnedBytes &slot = stage ? own->h_call[own->h_call_next] : dummy;
@@ -591,7 +595,7 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         const int N = s->prm.grid_n, n_mu = s->prm.n_mu;
         const int ncap = ((N + 1) & ~1) + 2;
         const int job_cap = per_cell_cap(s, n_mu, ncap);
-        int *d_njobs = s->d_sched.ptr, *d_order = d_njobs + c.n_phases, *d_work = d_order + c.n_phases;
+        int *d_njobs = s->d_sched.ptr, *d_work = d_njobs + c.n_phases;
         if (prepare) {
             RegionAtPhase *rp = reinterpret_cast<RegionAtPhase *>(h + rp_off) + rp_pos;
             localize_regions(s, c.regions, c.n_regions, c.phases, c.n_phases, c.radii, rp);
@@ -618,7 +622,6 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
             a.jobs = s->d_jobs.ptr;
             a.n_jobs = d_njobs;
             a.work = d_work;
-            a.phase_order = d_order;
             a.counters = s->d_counters.ptr;
             hp[k] = a;
             hph[k] = phase0;
@@ -643,7 +646,7 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         b.n_tiles = (int)((c.q->n_pix + f32::kTile - 1) / f32::kTile);
         b.jobs = s->d_jobs.ptr;
         b.n_jobs = d_njobs;
-        b.phase_order = d_order;
+        b.work = d_work;
         b.job_cap = job_cap;
         b.n_phases = c.n_phases;
         b.out = static_cast<float *>(c.out);
@@ -654,7 +657,7 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         s->last_tile_px = f32::kTile;
     }
     const f32::StarBlock first_block = hb[0];
-    if (prepare) {
+    if (prepare && !inline_rp) {
         hph[n] = phase0;
         SOAP_CUDA(own, cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, st));
     } else if (n > 1) {
@@ -668,12 +671,25 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
     if (prepare && total_phases > 0) {
         // a4: one cluster of CTAs per (star, phase) bins, compacts and schedules (active.cuh)
         if (!own->attr_prep_set) {
-            SOAP_CUDA(own, cudaFuncSetAttribute(active_prepare_kernel<float2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            SOAP_CUDA(own, (cudaFuncSetAttribute(active_prepare_kernel<float2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)));
             own->attr_prep_set = true;
         }
-        PrepArgs none{};
-        active_prepare_kernel<float2><<<(unsigned)(total_phases * kPrepCluster), kPrepThreads, prep_smem, st>>>(
-            none, reinterpret_cast<const PrepArgs *>(d + prep_off), reinterpret_cast<const int *>(d + ph_off), n);
+        if (inline_rp) {
+            if (!own->attr_prep_inl_set) {
+                SOAP_CUDA(own, (cudaFuncSetAttribute(active_prepare_kernel<float2, kInlineRegions>,
+                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)));
+                own->attr_prep_inl_set = true;
+            }
+            InlineRegions<kInlineRegions> inl;
+            std::memcpy(inl.r, h + rp_off, n_rp * sizeof(RegionAtPhase));
+            active_prepare_kernel<float2, kInlineRegions><<<(unsigned)(total_phases * kPrepCluster), kPrepThreads, prep_smem, st>>>(
+                hp[0], nullptr, nullptr, 1, inl);
+        } else {
+            PrepArgs none{};
+            InlineRegions<0> no_inl{};
+            active_prepare_kernel<float2, 0><<<(unsigned)(total_phases * kPrepCluster), kPrepThreads, prep_smem, st>>>(
+                none, reinterpret_cast<const PrepArgs *>(d + prep_off), reinterpret_cast<const int *>(d + ph_off), n, no_inl);
+        }
         SOAP_LAUNCH_CHECK(own, "active_prepare_kernel");
     }
     if (n_items == 0 || map_only) return SOAP_OK;
@@ -739,8 +755,9 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
     }
     const int job_cap = per_cell_cap(s, n_mu, ncap);
     SOAP_CUDA(s, s->d_jobs.reserve((size_t)n_phases * job_cap));
-    SOAP_CUDA(s, s->d_sched.reserve((size_t)3 * n_phases));
-    int *d_njobs = s->d_sched.ptr, *d_order = d_njobs + n_phases, *d_work = d_order + n_phases;
+    SOAP_CUDA(s, s->d_sched.reserve((size_t)2 * n_phases));
+    int *d_njobs = s->d_sched.ptr, *d_work = d_njobs + n_phases;
+    s->last_n_phases = n_phases;
     const bool per_cell = s->prm.diff_rot != 0.0;  // the cells of a column no longer share a velocity (R-DR)
     // fp64 I/O under differential rotation: the generic kernel reads fixed slots of seg_cap entries per segment, so every
     // segment gets room for all the covered cells of a phase (fp64 is the small-configuration path)
@@ -778,7 +795,6 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         a.jobs = s->d_jobs.ptr;
         a.n_jobs = d_njobs;
         a.work = d_work;
-        a.phase_order = d_order;
         a.counters = s->d_counters.ptr;
         const size_t smem = prep_cells_smem_bytes(n_mu, a.chunk_cols);
         SOAP_CUDA(s, cudaFuncSetAttribute(active_prepare_cells_kernel<Ent>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -794,7 +810,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         a.job_cap = job_cap;
         a.n_phases = n_phases;
         a.chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);  // columns a CTA of the cluster may own
-        if (prep_smem_bytes(n_mu, a.chunk_cols) > 200 * 1024)
+        if (prep_smem_bytes(n_mu, a.chunk_cols, N, n_regions) > 200 * 1024)
             return s->fail(SOAP_ERR_UNSUPPORTED, "grid_n %d with %d mu bins exceeds the active-map kernel's shared memory", N, n_mu);
         a.rp = s->d_rp.ptr;
         a.mu = s->d_mu.ptr;
@@ -811,11 +827,11 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         a.jobs = s->d_jobs.ptr;
         a.n_jobs = d_njobs;
         a.work = d_work;
-        a.phase_order = d_order;
         a.counters = s->d_counters.ptr;
-        const size_t smem = prep_smem_bytes(n_mu, a.chunk_cols);
-        SOAP_CUDA(s, cudaFuncSetAttribute(active_prepare_kernel<Ent>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        active_prepare_kernel<Ent><<<n_phases * kPrepCluster, kPrepThreads, smem, st>>>(a, nullptr, nullptr, 1);
+        const size_t smem = prep_smem_bytes(n_mu, a.chunk_cols, N, n_regions);
+        SOAP_CUDA(s, (cudaFuncSetAttribute(active_prepare_kernel<Ent, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)));
+        InlineRegions<0> no_inl{};
+        active_prepare_kernel<Ent, 0><<<n_phases * kPrepCluster, kPrepThreads, smem, st>>>(a, nullptr, nullptr, 1, no_inl);
         SOAP_LAUNCH_CHECK(s, "active_prepare_kernel");
     }
     if (sizeof(T) == 4) {
@@ -1226,12 +1242,19 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     MuCentres mc{};
     for (int b = 0; b < n_mu; ++b) mc.v[b] = prm->mu_centres[b];
     Rotation rot{prm->vsini_kms, sini, cosi, prm->diff_rot};
-    // a1 + a2 in one launch: the last CTA compacts the binned weights into the entry list
-    geometry_kernel<<<(N + geom_cols_per_cta(N) - 1) / geom_cols_per_cta(N), 32 * kGeomWarps, 0, st>>>(
+    // a1 + a2 in one launch: the last CTA compacts the binned weights into the entry list - from a shared-memory copy of
+    // the binned weights when they fit (geometry.cuh, finalize_columns_smem)
+    const size_t fin_bytes = fin_smem_bytes(N, n_mu);
+    const bool fin_smem = fin_bytes <= kFinSmemMax;
+    if (fin_smem && !s->attr_geom_set) {
+        SOAP_CUDA(s, cudaFuncSetAttribute(geometry_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmemMax));
+        s->attr_geom_set = true;
+    }
+    geometry_kernel<<<(N + geom_cols_per_cta(N) - 1) / geom_cols_per_cta(N), 32 * kGeomWarps, fin_smem ? fin_bytes : 0, st>>>(
         N, rot, prm->ld_u1, prm->ld_u2, prm->doppler_mode, n_mu, mc, s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr, s->d_bin.ptr,
         s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr, s->d_ent32.ptr, s->d_ent64.ptr, s->d_row_start.ptr,
         s->d_info.ptr, s->d_geom_done.ptr, s->d_colcnt.ptr, s->d_cellpos.ptr, s->cell_entries ? 1 : 0,
-        s->comp_stride ? s->d_cWp.ptr : nullptr, s->comp_stride, s->d_chdr.ptr);
+        s->comp_stride ? s->d_cWp.ptr : nullptr, s->comp_stride, s->d_chdr.ptr, fin_smem ? 1 : 0);
     SOAP_LAUNCH_CHECK(s, "geometry_kernel");
     if (s->cell_entries) {
         write_cell_entries_kernel<<<(N + kCellWarps - 1) / kCellWarps, 32 * kCellWarps, 0, st>>>(
@@ -1500,11 +1523,16 @@ int soap_get_stats(soap_star *s, soap_stats *stats, void *stream) {
         SOAP_CUDA(s, cudaStreamSynchronize(st));
         stats->quiet_entries = s->cell_entries ? di.n_visible : di.n_entries;
     }
-    if (s->d_counters.ptr) {
+    if (s->d_counters.ptr && s->d_sched.ptr && s->last_n_phases > 0) {
         ActiveCounters c;
+        std::vector<int> work((size_t)s->last_n_phases);
         SOAP_CUDA(s, cudaMemcpyAsync(&c, s->d_counters.ptr, sizeof(c), cudaMemcpyDeviceToHost, st));
+        SOAP_CUDA(s, cudaMemcpyAsync(work.data(), s->d_sched.ptr + s->last_n_phases, work.size() * sizeof(int), cudaMemcpyDeviceToHost, st));
         SOAP_CUDA(s, cudaStreamSynchronize(st));
-        stats->active_entries = (long long)c.active_entries;
+        if (c.overflow) return s->fail(SOAP_ERR_CUDA, "active map: a phase's entry pool overflowed (the result of the last call is incomplete)");
+        long long total = 0;
+        for (int w : work) total += w;
+        stats->active_entries = total;  // pad entries not counted
     }
     stats->active_cells = s->last_active_cells;
     stats->quiet_splits = s->last_quiet_splits;
