@@ -16,6 +16,7 @@
 #include <cuda_runtime.h>
 
 #include "geometry.cuh"
+#include "ptx_helpers.cuh"
 
 namespace soap {
 
@@ -155,6 +156,9 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = kPrepThreads / 32;
     // every CTA of the cluster must be running before its shared memory is written remotely: arrive now, wait in (4)
     asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+    // (launched with programmatic stream serialization: the geometry this kernel reads is complete after the wait)
+    trigger_dependents();
+    grid_dependency_wait();
     if (tid == 0) {
         const int c = blockIdx.x / kPrepCluster;
         if (many) {

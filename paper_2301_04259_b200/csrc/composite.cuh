@@ -169,6 +169,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) composite_quiet_kernel(c
     const long long G = gridDim.x, g = blockIdx.x;
     const int n_stars = p.n_stars;
 
+    // (launched with programmatic stream serialization: the pair tables are the geometry launch's, which may still be
+    // finishing)
+    trigger_dependents();
+    grid_dependency_wait();
     // ---- work units of every star: n_tiles x (cost of all its pairs) -------------------------------------------
     for (int s = tid; s < n_stars; s += kThreads) {
         const Star &st = p.many ? p.many[s] : p.one;

@@ -8,6 +8,7 @@
 #include <cuda_runtime.h>
 
 #include "composite.cuh"
+#include "ptx_helpers.cuh"
 
 namespace soap {
 
@@ -538,6 +539,7 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
     __shared__ int s_nvis[kGeomWarps];
     __shared__ int s_last;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    trigger_dependents();  // the quiet launch that follows may stage its spectra while this kernel runs (ptx_helpers.cuh)
     for (int b = threadIdx.x; b < n_mu; b += blockDim.x) s_mu[b] = mu_centres.v[b];
     for (int b = lane; b < 64; b += 32) {
         s_W[warp][b] = 0.0;

@@ -162,8 +162,7 @@ constexpr int kOrderCap = 256;                                // phases of one s
 constexpr size_t kOrderOff = 3072;                            // active launch, scheduler warp: order and jobs of the phases of one
                                                               // star, [kOrderCap] unsigned short each
 constexpr size_t kHeaderBytes = 3072 + kOrderCap * 4;         // mbarriers (96 B), tile hand-over words, item queue (at 128), prefix, blocks, order
-constexpr size_t kFinBytes = (size_t)kTile * (sizeof(double) + sizeof(float));  // active launch: per-pixel fp64
-                                                                              // contrast-weighted sums + staged contrast
+constexpr size_t kFinBytes = (size_t)kTile * sizeof(float);  // active launch: staged contrast of the current kind
 __host__ inline size_t smem_bytes(int halo, bool active) {
     return kHeaderBytes + (active ? kFinBytes : 0) + kStages * stage_layout(halo).stage_bytes;
 }
@@ -291,9 +290,6 @@ struct ActiveSource {
         const int *wk = many ? ldg_ptr(&b->work) : b->work, *njp = many ? ldg_ptr(&b->n_jobs) : b->n_jobs;
         ord_star = st;
         ord_identity = n > kOrderCap;
-#ifdef EXP_NOORDER
-        ord_identity = true;
-#endif
         if (ord_identity) return;
         __syncwarp();
         bool wide = false;
@@ -466,12 +462,7 @@ struct ActiveSource {
 __device__ __forceinline__ void consumer_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumers) : "memory"); }
 
 __device__ __forceinline__ void mbar_wait_backoff(uint64_t *bar, uint32_t parity) {
-#ifdef EXP_WAITHINT
-    while (!mbar_try_wait_hint(bar, parity, EXP_WAITHINT)) {
-    }
-#else
     while (!mbar_try_wait(bar, parity)) __nanosleep(40);
-#endif
 }
 
 // One producer warp: turns the `count` raw entries (a, W) of a job into records and the run table of a tile
@@ -552,8 +543,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     uint64_t *bar_empty = bar_ready + kStages;               // [kStages] consumers done       (count kConsumerWarps)
     int *tile_ctl = reinterpret_cast<int *>(smem + 96);      // quiet launch: last-CTA flag, first / last sharing CTA
     long long *prefix = reinterpret_cast<long long *>(smem + kPrefixOff);  // active launch: first item of every star
-    double *fin = reinterpret_cast<double *>(smem + kHeaderBytes);  // active launch only: [kR][kConsumers]
-    float *cst = reinterpret_cast<float *>(fin + kTile);            // active launch only: contrast of the current kind
+    float *cst = reinterpret_cast<float *>(smem + kHeaderBytes);    // active launch only: contrast of the current kind, [kR][kConsumers]
     unsigned char *stage0 = smem + kHeaderBytes + (ACTIVE ? kFinBytes : 0);
 
     const int tid = threadIdx.x;
@@ -567,6 +557,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         fence_mbar_init();
         reinterpret_cast<ItemQueue *>(smem + 128)->tail = 0;
     }
+    // (launched with programmatic stream serialization: everything above overlaps the predecessor's tail)
+    trigger_dependents();
+    grid_dependency_wait();
     if (ACTIVE) {
         for (int k = tid; k <= p.n_stars; k += kThreads)
             prefix[k] = k < p.n_stars ? (p.many ? __ldg(&p.many[k].item0) : 0LL) : p.n_items;
@@ -673,46 +666,46 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     float2 acc1[kR / 2], acc2[kR / 2];
     double tot[kR];
     int cnt = 0, cur_kind = 0;
+    // a6: post-shift contrast (I_ratio of Eq. 3) per output pixel: a fold multiplies the fp32 partial sums of the current
+    // kind by the kind's contrast C[m] in fp64 (the product is exact) on their way into the fp64 totals - no per-kind
+    // totals are kept.  The contrast values of the current kind are fetched with cp.async while its first jobs run.
+    int rmax = 0;            // pixels r < rmax of this thread lie inside the spectrum
+    bool kind_c = false;     // the current kind carries a contrast array
+    const Desc *desc = nullptr;  // descriptor of the current job
     auto fold = [&]() {
+        if (ACTIVE && kind_c) {
+            cp_async_wait_all();
 #pragma unroll
-        for (int k = 0; k < kR / 2; ++k) {
-            const float c0 = cmf + (float)(kConsumers * 2 * k), c1 = cmf + (float)(kConsumers * (2 * k + 1));
-            tot[2 * k] += (double)fmaf(c0, acc2[k].x, acc1[k].x);
-            tot[2 * k + 1] += (double)fmaf(c1, acc2[k].y, acc1[k].y);
-            acc1[k] = make_float2(0.f, 0.f);
-            acc2[k] = make_float2(0.f, 0.f);
+            for (int k = 0; k < kR / 2; ++k) {
+                const float c0 = cmf + (float)(kConsumers * 2 * k), c1 = cmf + (float)(kConsumers * (2 * k + 1));
+                const double w0 = 2 * k < rmax ? (double)cst[(2 * k) * kConsumers + tid] : 1.0;
+                const double w1 = 2 * k + 1 < rmax ? (double)cst[(2 * k + 1) * kConsumers + tid] : 1.0;
+                tot[2 * k] = fma((double)fmaf(c0, acc2[k].x, acc1[k].x), w0, tot[2 * k]);
+                tot[2 * k + 1] = fma((double)fmaf(c1, acc2[k].y, acc1[k].y), w1, tot[2 * k + 1]);
+                acc1[k] = make_float2(0.f, 0.f);
+                acc2[k] = make_float2(0.f, 0.f);
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < kR / 2; ++k) {
+                const float c0 = cmf + (float)(kConsumers * 2 * k), c1 = cmf + (float)(kConsumers * (2 * k + 1));
+                tot[2 * k] += (double)fmaf(c0, acc2[k].x, acc1[k].x);
+                tot[2 * k + 1] += (double)fmaf(c1, acc2[k].y, acc1[k].y);
+                acc1[k] = make_float2(0.f, 0.f);
+                acc2[k] = make_float2(0.f, 0.f);
+            }
         }
         cnt = 0;
     };
-    // a6: post-shift contrast (I_ratio of Eq. 3) per output pixel.  Kinds with a contrast array come first in
-    // a phase's job list (active_prepare_kernel); their fp64 sums are weighted into `fin` when the kind ends.
-    // The contrast values of the current kind are fetched with cp.async while its jobs run.
-    int rmax = 0;            // pixels r < rmax of this thread lie inside the spectrum
-    bool fin_valid = false;  // `fin` holds a weighted sum of this item
-    const Desc *desc = nullptr;  // descriptor of the current job
-    auto prefetch_contrast = [&](int kind) {
-        if (!((cmask >> kind) & 1)) return;
+    auto begin_kind = [&](int kind) {  // after a fold: only this thread ever touches its 16 slots of `cst`
+        cur_kind = kind;
+        kind_c = (cmask >> kind) & 1;
+        if (!kind_c) return;
         const float *ck = desc->contrast[kind - 1];
 #pragma unroll
         for (int r = 0; r < kR; ++r)
             if (r < rmax) cp_async_4(&cst[r * kConsumers + tid], ck + m_t0 + tid + kConsumers * r);
         cp_async_commit();
-    };
-    auto fold_kind = [&](int kind) {
-        // weight 1: keeps accumulating with the next kind - unless that kind's sum is about to be multiplied by
-        // its own contrast (job order is 1, 2, 0: only a spot sum without contrast ahead of a facula with one)
-        const bool has_c = (cmask >> kind) & 1;
-        if (!has_c && !(kind == 1 && ((cmask >> 2) & 1))) return;
-        fold();
-        cp_async_wait_all();
-#pragma unroll
-        for (int r = 0; r < kR; ++r) {
-            const double c = (has_c && r < rmax) ? (double)cst[r * kConsumers + tid] : 1.0;
-            const double f = fin_valid ? fin[r * kConsumers + tid] : 0.0;
-            fin[r * kConsumers + tid] = f + c * tot[r];
-            tot[r] = 0.0;
-        }
-        fin_valid = true;
     };
 
     for (int n = 0;; ++n) {
@@ -745,15 +738,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             if (ACTIVE) {
                 const long long rem = out_hi - (m_t0 + tid);
                 rmax = rem <= 0 ? 0 : (int)min((long long)kR, (rem + kConsumers - 1) / kConsumers);
-                fin_valid = false;  // only this thread ever touches its 16 slots of `fin` and `cst`
-                cur_kind = kind;
-                prefetch_contrast(kind);
+                begin_kind(kind);
             }
         }
         if (ACTIVE && kind != cur_kind) {
-            fold_kind(cur_kind);
-            cur_kind = kind;
-            prefetch_contrast(kind);
+            if (kind_c || ((cmask >> kind) & 1)) fold();  // the multiplier changes: what was summed so far goes to the totals
+            begin_kind(kind);
         }
         int2 run_next = runs[0];
         for (int ri = 0; ri < n_runs; ++ri) {
@@ -813,13 +803,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
         if (flags & kJobLast) {
             fold();
             if (ACTIVE) {
-                fold_kind(cur_kind);
                 float *o = o_row;
 #pragma unroll
-                for (int r = 0; r < kR; ++r) {
-                    const double f = fin_valid ? fin[r * kConsumers + tid] : 0.0;
-                    if (r < rmax && m_t0 + tid + kConsumers * r >= out_lo) o[kConsumers * r] = (float)(tot[r] + f);
-                }
+                for (int r = 0; r < kR; ++r)
+                    if (r < rmax && m_t0 + tid + kConsumers * r >= out_lo) o[kConsumers * r] = (float)tot[r];
             } else {
                 double *o = p.partial + ((long long)blockIdx.x * p.max_seg + out_idx) * kTile;
 #pragma unroll

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <type_traits>
+#include <utility>
 #include <new>
 #include <string>
 #include <vector>
@@ -160,6 +161,24 @@ namespace {
         (star)->launches++;                                                                              \
     } while (0)
 
+// Launch with programmatic stream serialization: the kernel may be scheduled while its predecessor in the stream drains;
+// it calls grid_dependency_wait() (ptx_helpers.cuh) before it reads what the predecessor wrote.  The four launches of a
+// step (geometry, quiet, active map, active delta) are chained this way: launch latency and prologues overlap the tails.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 inline double host_dshift(double v_kms, int mode) {
     const double b = v_kms / kSpeedOfLightKms;
     if (mode == 1) return -b;
@@ -233,7 +252,7 @@ int launch_sia_f32(soap_star *s, const f32::Params &p, dim3 grid, cudaStream_t s
             if (!s->ev[k]) SOAP_CUDA(s, cudaEventCreate(&s->ev[k]));
         SOAP_CUDA(s, cudaEventRecord(s->ev[e0], st));
     }
-    f32::sia_f32_kernel<ACTIVE><<<grid, f32::kThreads, smem, st>>>(p);
+    SOAP_CUDA(s, launch_pdl(f32::sia_f32_kernel<ACTIVE>, grid, dim3(f32::kThreads), smem, st, p));
     SOAP_LAUNCH_CHECK(s, ACTIVE ? "sia_f32_kernel<active>" : "sia_f32_kernel<quiet>");
     if (s->opt_timing) {
         SOAP_CUDA(s, cudaEventRecord(s->ev[e0 + 1], st));
@@ -324,7 +343,7 @@ int launch_composite_nb(soap_star *s, const comp::Params &p, unsigned G, size_t 
         SOAP_CUDA(s, cudaFuncSetAttribute(comp::composite_quiet_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set[s->device & 63] = true;
     }
-    comp::composite_quiet_kernel<NB><<<G, comp::kThreads, smem, st>>>(p);
+    SOAP_CUDA(s, launch_pdl(comp::composite_quiet_kernel<NB>, dim3(G), dim3(comp::kThreads), smem, st, p));
     return SOAP_OK;
 }
 
@@ -682,13 +701,14 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
             }
             InlineRegions<kInlineRegions> inl;
             std::memcpy(inl.r, h + rp_off, n_rp * sizeof(RegionAtPhase));
-            active_prepare_kernel<float2, kInlineRegions><<<(unsigned)(total_phases * kPrepCluster), kPrepThreads, prep_smem, st>>>(
-                hp[0], nullptr, nullptr, 1, inl);
+            SOAP_CUDA(own, launch_pdl(active_prepare_kernel<float2, kInlineRegions>, dim3((unsigned)(total_phases * kPrepCluster)),
+                                      dim3(kPrepThreads), prep_smem, st, hp[0], (const PrepArgs *)nullptr, (const int *)nullptr, 1, inl));
         } else {
             PrepArgs none{};
             InlineRegions<0> no_inl{};
-            active_prepare_kernel<float2, 0><<<(unsigned)(total_phases * kPrepCluster), kPrepThreads, prep_smem, st>>>(
-                none, reinterpret_cast<const PrepArgs *>(d + prep_off), reinterpret_cast<const int *>(d + ph_off), n, no_inl);
+            SOAP_CUDA(own, launch_pdl(active_prepare_kernel<float2, 0>, dim3((unsigned)(total_phases * kPrepCluster)), dim3(kPrepThreads),
+                                      prep_smem, st, none, reinterpret_cast<const PrepArgs *>(d + prep_off),
+                                      reinterpret_cast<const int *>(d + ph_off), n, no_inl));
         }
         SOAP_LAUNCH_CHECK(own, "active_prepare_kernel");
     }
@@ -722,7 +742,7 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
             if (!own->ev[k]) SOAP_CUDA(own, cudaEventCreate(&own->ev[k]));
         SOAP_CUDA(own, cudaEventRecord(own->ev[2], st));
     }
-    f32::sia_f32_kernel<true><<<(unsigned)G, f32::kThreads, smem, st>>>(p);
+    SOAP_CUDA(own, launch_pdl(f32::sia_f32_kernel<true>, dim3((unsigned)G), dim3(f32::kThreads), smem, st, p));
     SOAP_LAUNCH_CHECK(own, "sia_f32_kernel<active>");
     if (own->opt_timing) {
         SOAP_CUDA(own, cudaEventRecord(own->ev[3], st));
