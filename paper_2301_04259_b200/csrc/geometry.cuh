@@ -259,37 +259,22 @@ __device__ void finalize_columns_smem(int N, int n_mu, const double *col_a, cons
     double *sA = sW + (size_t)n_mu * Np;           // [N]
     int *s_cost = reinterpret_cast<int *>(sA + N);  // [n_pairs + 1] exclusive cost prefix of the column pairs
     // ---- one round trip: every load is independent of every other (written by other SMs: read through L2) ----------
-    constexpr int kInFlight = 8;  // loads a thread issues before it uses the first
+    // a warp takes a column at a time, lanes over the mu bins (no index arithmetic per element); four columns in flight
     long long nv = 0;
     double sw = 0.0, am = 0.0;
-    {
-        const int j = tid;  // first round of the per-column sums: in flight with the first weights
-        const int c = j < N ? __ldcg(&col_nvis[j]) : 0;
-        const double a = j < N ? __ldcg(&col_a[j]) : 0.0, cs = j < N ? __ldcg(&col_sumw[j]) : 0.0;
-        for (int k0 = 0; k0 < N * n_mu; k0 += nt * kInFlight) {
+    constexpr int kInFlight = 4;
+    for (int j0 = warp * kInFlight; j0 < N; j0 += n_warps * kInFlight) {
+        for (int b0 = 0; b0 < n_mu; b0 += 32) {
+            const int b = b0 + lane;
             double v[kInFlight];
 #pragma unroll
-            for (int u = 0; u < kInFlight; ++u) {
-                const int k = k0 + u * nt + tid;
-                v[u] = k < N * n_mu ? __ldcg(&Wbin[k]) : 0.0;
-            }
+            for (int u = 0; u < kInFlight; ++u) v[u] = (b < n_mu && j0 + u < N) ? __ldcg(&Wbin[(size_t)(j0 + u) * n_mu + b]) : 0.0;
 #pragma unroll
-            for (int u = 0; u < kInFlight; ++u) {
-                const int k = k0 + u * nt + tid;
-                if (k < N * n_mu) {
-                    const int jj = k / n_mu, b = k - jj * n_mu;
-                    sW[(size_t)b * Np + jj] = v[u];
-                }
-            }
-        }
-        if (j < N) {
-            sA[j] = a;
-            nv = c;
-            sw = cs;
-            if (c > 0) am = fabs(a);
+            for (int u = 0; u < kInFlight; ++u)
+                if (b < n_mu && j0 + u < N) sW[(size_t)b * Np + j0 + u] = v[u];
         }
     }
-    for (int j = tid + nt; j < N; j += nt) {
+    for (int j = tid; j < N; j += nt) {
         const int c = __ldcg(&col_nvis[j]);
         const double a = __ldcg(&col_a[j]);
         sA[j] = a;
