@@ -120,7 +120,7 @@ struct soap_star {
     } h_call[4];
     int h_call_next = 0;
     size_t call_rp_off = 0, call_prep_off = 0, call_blk_off = 0, call_ph_off = 0;  // sections of d_call of the last prepared call
-    bool attr_active_set = false, attr_prep_set = false, attr_prep_inl_set = false, attr_geom_set = false;
+    bool attr_active_set = false, attr_prep_set = false, attr_prep_inl_set = false, attr_geom_set = false, attr_rv_set = false;
     int occ_active = 0;
     size_t occ_active_smem = 0;
 
@@ -1471,10 +1471,16 @@ int soap_line_rvs(soap_star *s, const void *rows, int64_t n_rows, int64_t n_pix,
     a.n_lines = n_lines;
     a.edge = edge;
     a.rv = out_rv;
+    a.rows_pass = (int)std::min<long long>(kRvRows, n_rows);
     const unsigned gx = (unsigned)((n_lines + kRvWarps - 1) / kRvWarps);
-    const unsigned gy = (unsigned)std::min<long long>((n_rows + 31) / 32, 65535);  // one warp per (line, 32 rows)
-    if (dtype == SOAP_F32) line_rv_kernel<float><<<dim3(gx, gy), 32 * kRvWarps, 0, st>>>(a);
-    else line_rv_kernel<double><<<dim3(gx, gy), 32 * kRvWarps, 0, st>>>(a);
+    const unsigned gy = (unsigned)std::min<long long>((n_rows + a.rows_pass - 1) / a.rows_pass, 65535);  // one warp per (line, rows_pass rows)
+    if (!s->attr_rv_set) {
+        SOAP_CUDA(s, cudaFuncSetAttribute(line_rv_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rv_smem_bytes<float>(kRvRows)));
+        SOAP_CUDA(s, cudaFuncSetAttribute(line_rv_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rv_smem_bytes<double>(kRvRows)));
+        s->attr_rv_set = true;
+    }
+    if (dtype == SOAP_F32) line_rv_kernel<float><<<dim3(gx, gy), 32 * kRvWarps, rv_smem_bytes<float>(a.rows_pass), st>>>(a);
+    else line_rv_kernel<double><<<dim3(gx, gy), 32 * kRvWarps, rv_smem_bytes<double>(a.rows_pass), st>>>(a);
     SOAP_LAUNCH_CHECK(s, "line_rv_kernel");
     return SOAP_OK;
 }
