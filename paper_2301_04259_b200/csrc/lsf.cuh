@@ -177,9 +177,9 @@ __global__ void __launch_bounds__(kLsfThreads, J4 <= 16 ? 2 : 1) lower_resolutio
             for (int u = 0; u < kPer; ++u) {
                 const int q4 = tid + u * kLsfThreads;
                 if (q4 >= span4) continue;
-                if (inner) {
+                if (inner || (g0 + 4 * q4 >= 0 && g0 + 4 * q4 + 3 < a.n_pix)) {  // the four pixels lie inside the row
                     cp_async_16(dst + 4 * q4, row + g0 + 4 * q4);
-                } else {
+                } else {  // an end tile's out-of-range pixels: clamped by hand
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
                         long long n = g0 + 4 * q4 + c;
@@ -200,22 +200,23 @@ __global__ void __launch_bounds__(kLsfThreads, J4 <= 16 ? 2 : 1) lower_resolutio
             int Jm = (int)ceil(__ddiv_rn(__dmul_rn(kLsfNsig, sigma), a.k));
             Jm = min(Jm, J4);
             const double h = (a.k * a.k) / (2.0 * sigma * sigma);
-            const double q = exp(-2.0 * h), rho0 = exp(-h);
+            const double rho0 = exp(-h), q = rho0 * rho0;  // exp(-2h) to 1 ulp of fp64
+            // one pass: the unnormalised taps go to the registers as they are formed (fp64 recurrence, rounded once),
+            // the norm is summed in fp64, and the taps are scaled by the rounded reciprocal afterwards (one more fp32
+            // rounding per tap: 6e-8 relative, far inside the fp32 path's tolerance)
             double rho = rho0, g = 1.0, norm = 1.0;
-            for (int j = 1; j <= Jm; ++j) {
-                g *= rho;
-                rho *= q;
-                norm += 2.0 * g;
-            }
-            const double inv = 1.0 / norm;
-            rho = rho0;
-            g = 1.0;
+            wr[0][p] = 1.f;
 #pragma unroll
-            for (int j = 0; j <= J4; ++j) {
-                wr[j][p] = j <= Jm ? (float)(g * inv) : 0.f;
+            for (int j = 1; j <= J4; ++j) {
                 g *= rho;
                 rho *= q;
+                const bool in = j <= Jm;
+                wr[j][p] = in ? (float)g : 0.f;
+                norm += in ? 2.0 * g : 0.0;
             }
+            const float inv = (float)(1.0 / norm);
+#pragma unroll
+            for (int j = 0; j <= J4; ++j) wr[j][p] *= inv;
         }
     };
 
