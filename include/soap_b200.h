@@ -23,8 +23,16 @@
  *     is enqueued on it; a call is asynchronous unless it has a non-NULL HOST output pointer
  *     (`info`, `n_active`, export, stats), in which case it synchronises that stream before returning.
  *     Scratch is (re)allocated with cudaMalloc when a call needs more than any earlier call did; once
- *     sizes have been seen, calls allocate nothing.  soap_active_timeseries* stage the region centres
- *     through a ring of pinned host buffers guarded by events, so they must not be stream-captured.
+ *     sizes have been seen, calls allocate nothing.  A single star's soap_active_timeseries* call passes its
+ *     region centres as kernel arguments (up to 192 (phase, region) pairs) and copies nothing; larger calls
+ *     and the batch calls stage them through a ring of pinned host buffers guarded by events, so the
+ *     time-series calls must not be stream-captured.
+ *   - The launches of a handle's consecutive calls on one stream (geometry, quiet, active map, active delta)
+ *     are chained with programmatic dependent launch: a launch may start while its predecessor drains and
+ *     waits on the device before it reads what the predecessor wrote.  Nothing changes for the caller.
+ *   - A handle is not re-entrant: calls on one soap_star must not run concurrently (from several host
+ *     threads or on several streams at once) - its scratch, its self-resetting device counters and its
+ *     staging ring belong to one call at a time.  Different handles are independent.
  *   - There is no CPU fallback and no other backend: without a CUDA device every compute entry point
  *     returns SOAP_ERR_CUDA.
  *   - Cell indexing: c = j * N + i with j the column (x) index and i the row (y) index;
@@ -266,8 +274,15 @@ int soap_synthesize_host(soap_star *star, const soap_star_params *params, const 
                          void *out_delta, int32_t *n_active, void *stream);
 
 /* ---- config 5: many independent stars in one call ----------------------------------------------
- * Arrays of length n_stars of the arguments above; star k uses stars[k], quiet[k], ...  All device
- * work of all stars is enqueued on `stream`. */
+ * Arrays of length n_stars of the arguments above; star k uses stars[k], quiet[k], ...  Every argument of
+ * every star is checked before anything is enqueued.  fp32 tables under solid-body rotation (the composite-
+ * column form for the quiet spectra) take ONE launch per call for all stars - soap_batch_active_timeseries:
+ * one active-map launch (a cluster per (star, phase)) and one shift-interpolate-accumulate launch over the
+ * (star, phase, tile) items - enqueued on `stream`; the stars' descriptors are staged in scratch of
+ * stars[0], which must therefore outlive the call's device work.  Mixed batches (fp64 tables, differential
+ * rotation, several devices) fall back to per-star launches dealt to `stream` and two side streams of
+ * stars[0], forked from and joined back into `stream` with events.  A star must not appear twice in a batch;
+ * no stream capture. */
 int soap_batch_integrate_quiet(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet,
                                void *const *out, void *stream);
 int soap_batch_active_timeseries(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet,
