@@ -58,7 +58,7 @@ def test_pole_on_star_and_polar_and_huge_regions(soap):
 
 
 def test_thousands_of_phases_keep_their_order(soap):
-    """More phases than the heaviest-first ordering sorts (kScheduleSortMax = 4096): identity order, same results."""
+    """More phases than the active launch's scheduler ranks by work (f32::kOrderCap = 256): taken as given, same results."""
     wl = workloads.make_config2(n_pix=2048, n_phases=4, grid_n=40)
     base = np.array([0.5, 0.47, 0.0, 0.53])
     wl.phases = np.tile(base, 1100)                      # 4400 phases
@@ -79,3 +79,31 @@ def test_fastest_supported_rotator_and_too_fast(soap):
     with pytest.raises(soap.SoapError) as e:
         run_gpu(soap, wl)
     assert e.value.code == soap.binding.SOAP_ERR_UNSUPPORTED
+
+
+def test_phase_counts_around_the_ordering_cap(soap):
+    """255 / 256 / 257 phases of unequal work: ranked heaviest first up to f32::kOrderCap, taken as given beyond it -
+    the order in which items are computed must not show in the result."""
+    base = workloads.make_config2(n_pix=2300, n_phases=8, grid_n=48)
+    base.regions = [(20.0, 180.0, 0.25, 1), (-30.0, 40.0, 0.1, 1)]
+    base.phases = np.array([0.5, 0.31, 0.77, 0.02, 0.44, 0.9, 0.62, 0.13])
+    g8 = run_gpu(soap, base)
+    assert_parity(base, g8, check_rv=False)
+    for n in (255, 256, 257):
+        wl = workloads.make_config2(n_pix=2300, n_phases=8, grid_n=48)
+        wl.regions = base.regions
+        wl.phases = np.resize(base.phases, n)
+        g = run_gpu(soap, wl)
+        assert np.array_equal(g["D"], g8["D"][np.arange(n) % 8])
+        assert np.array_equal(g["n_active"], g8["n_active"][np.arange(n) % 8])
+
+
+def test_grid_too_large_for_the_shared_memory_finalisation(soap):
+    """N x n_mu binned weights beyond geometry.cuh's kFinSmemMax (160 KB): the last CTA finalises from global memory."""
+    wl = workloads.make_config2(n_pix=2100, n_phases=2, grid_n=1100)
+    wl.phases = np.array([0.5, 0.46])
+    g = run_gpu(soap, wl)
+    og = oracle.geometry(wl)
+    assert g["info"]["n_visible"] == og["n_visible"]
+    assert abs(g["info"]["sum_weights"] - og["sum_w"]) <= 1e-9 * og["sum_w"]
+    assert_parity(wl, g, check_rv=False)
