@@ -275,4 +275,159 @@ __global__ void __launch_bounds__(kLsfThreads, J4 <= 16 ? 2 : 1) lower_resolutio
     }
 }
 
+
+// ---- fp32 fast path, rows in pairs -------------------------------------------------------------------------------
+// The weights depend on the pixel only, so two rows can share every multiply: a thread owns 2 consecutive pixels of a
+// 512-pixel tile for a PAIR of rows, the pair's samples are interleaved in shared memory ((row a, row b) per pixel), its
+// window is read with LDS.128 (2 pixels x 2 rows each) and every tap is one packed add and one packed FMA (FADD2 / FFMA2,
+// weight in the scalar-broadcast operand) over the two rows: half the floating-point instructions of the kernel above,
+// no special case for the end tiles (every staged sample is one clamped 4-byte cp.async) and no index arithmetic in the
+// inner part.  Persistent CTAs walk a contiguous range of (tile, row pair) items in tile-major order as above.
+// Used when the LSF is at most 16 taps per side (the window and the weights must fit in registers).
+constexpr int kLsfTileP = kLsfThreads * 2;
+constexpr int kLsfStagesP = 8;
+
+template <int J4>
+__host__ __device__ constexpr size_t lsf_p_smem_bytes() {
+    return kLsfStagesP * (size_t)(kLsfTileP + 2 * J4) * 2 * sizeof(float);
+}
+
+template <int J4>
+__global__ void __launch_bounds__(kLsfThreads, 2) lower_resolution_p_kernel(const LsfArgs a) {
+    static_assert(J4 % 2 == 0, "the window starts on an even pixel");
+    extern __shared__ __align__(16) unsigned char lsf_smem[];
+    float2 *s = reinterpret_cast<float2 *>(lsf_smem);  // [kLsfStagesP][span] of (row a, row b)
+    constexpr int span = kLsfTileP + 2 * J4;
+    constexpr int kPer = (span + kLsfThreads - 1) / kLsfThreads;
+    float wr[J4 + 1][2];  // this thread's weights: registers
+    const int tid = threadIdx.x;
+    const float *in = static_cast<const float *>(a.in);
+    float *out = static_cast<float *>(a.out);
+    const int n_pairs = (int)((a.n_rows + 1) / 2);
+    const long long n_tiles = (a.n_pix + kLsfTileP - 1) / kLsfTileP;
+    const long long items = n_tiles * n_pairs;
+    const long long it0 = items * blockIdx.x / gridDim.x, it1 = items * (blockIdx.x + 1) / gridDim.x;
+    if (it0 >= it1) return;
+
+    struct Cursor {
+        long long it;
+        int tile, rp;
+    };
+    auto advance = [&](Cursor &c) {
+        ++c.it;
+        if (++c.rp == n_pairs) {
+            c.rp = 0;
+            ++c.tile;
+        }
+    };
+    auto issue = [&](const Cursor &ci, float2 *dst) {
+        if (ci.it < it1) {
+            const long long g0 = (long long)ci.tile * kLsfTileP - J4;  // global pixel of tile-array position 0
+            const long long ra = 2LL * ci.rp, rb = ra + 1 < a.n_rows ? ra + 1 : ra;  // an odd last row is paired with itself
+            // position q of the tile array holds pixel g0 + q; only the two end tiles need the clamp (reading S8)
+            const float *pa = in + ra * a.in_pitch + g0 + tid, *pb = in + rb * a.in_pitch + g0 + tid;
+            float2 *d = dst + tid;
+            if (g0 >= 0 && g0 + span <= a.n_pix) {
+#pragma unroll
+                for (int u = 0; u < kPer; ++u) {
+                    if (tid + u * kLsfThreads < span) {
+                        cp_async_4(&d[u * kLsfThreads].x, pa + u * kLsfThreads);
+                        cp_async_4(&d[u * kLsfThreads].y, pb + u * kLsfThreads);
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int u = 0; u < kPer; ++u) {
+                    const int q = tid + u * kLsfThreads;
+                    if (q >= span) continue;
+                    long long n = g0 + q;
+                    n = n < 0 ? 0 : (n > a.n_pix - 1 ? a.n_pix - 1 : n);
+                    const int off = (int)(n - g0) - tid;
+                    cp_async_4(&d[u * kLsfThreads].x, pa + off);
+                    cp_async_4(&d[u * kLsfThreads].y, pb + off);
+                }
+            }
+        }
+        cp_async_commit();  // one group per item, empty or not: the wait below counts groups
+    };
+    auto weights = [&](long long tile) {  // exact per-pixel weights of this thread's 2 pixels (see the kernels above)
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            const long long m = tile * kLsfTileP + 2 * tid + p;
+            const double lam = __dadd_rn(a.lambda0, __dmul_rn(a.k, (double)m));
+            const double sigma = __dmul_rn(__ddiv_rn(lam, a.R), a.fwhm_to_sigma);
+            int Jm = (int)ceil(__ddiv_rn(__dmul_rn(kLsfNsig, sigma), a.k));
+            Jm = min(Jm, J4);
+            const double h = (a.k * a.k) / (2.0 * sigma * sigma);
+            const double rho0 = exp(-h), q = rho0 * rho0;
+            double rho = rho0, g = 1.0, norm = 1.0;
+            wr[0][p] = 1.f;
+#pragma unroll
+            for (int j = 1; j <= J4; ++j) {
+                g *= rho;
+                rho *= q;
+                const bool inw = j <= Jm;
+                wr[j][p] = inw ? (float)g : 0.f;
+                norm += inw ? 2.0 * g : 0.0;
+            }
+            const float inv = (float)(1.0 / norm);
+#pragma unroll
+            for (int j = 0; j <= J4; ++j) wr[j][p] *= inv;
+        }
+    };
+
+    Cursor cc, ci;
+    cc.it = it0;
+    cc.tile = (int)(it0 / n_pairs);
+    cc.rp = (int)(it0 - (long long)cc.tile * n_pairs);
+    ci = cc;
+#pragma unroll 1
+    for (int d = 0; d < kLsfStagesP - 1; ++d) {
+        issue(ci, s + (size_t)d * span);
+        advance(ci);
+    }
+    long long cur_tile = cc.tile;
+    weights(cur_tile);
+    int cur = 0;
+    for (; cc.it < it1; advance(cc)) {
+        const long long tile = cc.tile;
+        cp_async_wait_group<kLsfStagesP - 2>();  // this item's samples have landed (for this thread's copies) ...
+        __syncthreads();                         // ... and for everyone's; the previous item has been consumed
+        if (tile != cur_tile) {
+            weights(tile);
+            cur_tile = tile;
+        }
+        issue(ci, s + (size_t)((cur + kLsfStagesP - 1) % kLsfStagesP) * span);
+        advance(ci);
+        // ---- this thread's window (2 + 2 J4 pixels of both rows) and its 2 x 2 outputs -------------------------------
+        float2 win[2 + 2 * J4];
+        const float4 *c4 = reinterpret_cast<const float4 *>(s + (size_t)cur * span) + tid;  // window starts at pixel 2 tid
+#pragma unroll
+        for (int u = 0; u < (2 + 2 * J4) / 2; ++u) {
+            const float4 t = c4[u];
+            win[2 * u] = make_float2(t.x, t.y);
+            win[2 * u + 1] = make_float2(t.z, t.w);
+        }
+        float2 acc[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+#pragma unroll
+        for (int j = J4; j >= 1; --j) {  // small outer taps first
+#pragma unroll
+            for (int p = 0; p < 2; ++p) acc[p] = fma2(bcast2(wr[j][p]), add2(win[J4 + p - j], win[J4 + p + j]), acc[p]);
+        }
+#pragma unroll
+        for (int p = 0; p < 2; ++p) acc[p] = fma2(bcast2(wr[0][p]), win[J4 + p], acc[p]);
+        const long long m = tile * kLsfTileP + 2 * tid;
+        const long long ra = 2LL * cc.rp;
+        float *oa = out + ra * a.out_pitch + m;
+        if (m + 1 < a.n_pix) {
+            *reinterpret_cast<float2 *>(oa) = make_float2(acc[0].x, acc[1].x);
+            if (ra + 1 < a.n_rows) *reinterpret_cast<float2 *>(oa + a.out_pitch) = make_float2(acc[0].y, acc[1].y);
+        } else if (m < a.n_pix) {
+            oa[0] = acc[0].x;
+            if (ra + 1 < a.n_rows) oa[a.out_pitch] = acc[0].y;
+        }
+        cur = (cur + 1) % kLsfStagesP;
+    }
+}
+
 }  // namespace soap

@@ -1425,7 +1425,27 @@ int soap_lower_resolution(soap_star *s, const void *in, int64_t n_rows, int64_t 
             kern<<<g, kLsfThreads, vsmem, st>>>(a);
             return SOAP_OK;
         };
+        auto launch_p = [&](auto kern, size_t psmem) -> int {  // rows in pairs (lsf.cuh, lower_resolution_p_kernel)
+            SOAP_CUDA(s, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psmem));
+            int occ = 0;
+            SOAP_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kLsfThreads, psmem));
+            if (occ < 1) return s->fail(SOAP_ERR_UNSUPPORTED, "resolution-lowering kernel does not fit on an SM");
+            const long long items = ((n_pix + kLsfTileP - 1) / kLsfTileP) * ((n_rows + 1) / 2);
+            const unsigned g = (unsigned)std::max<long long>(1, std::min<long long>(items, (long long)s->n_sm * occ));
+            kern<<<g, kLsfThreads, psmem, st>>>(a);
+            return SOAP_OK;
+        };
         int rc;
+        if (a.J_max <= 16) {
+            if (a.J_max <= 4) rc = launch_p(lower_resolution_p_kernel<4>, lsf_p_smem_bytes<4>());
+            else if (a.J_max <= 8) rc = launch_p(lower_resolution_p_kernel<8>, lsf_p_smem_bytes<8>());
+            else if (a.J_max <= 12) rc = launch_p(lower_resolution_p_kernel<12>, lsf_p_smem_bytes<12>());
+            else if (a.J_max <= 14) rc = launch_p(lower_resolution_p_kernel<14>, lsf_p_smem_bytes<14>());
+            else rc = launch_p(lower_resolution_p_kernel<16>, lsf_p_smem_bytes<16>());
+            if (rc) return rc;
+            SOAP_LAUNCH_CHECK(s, "lower_resolution_p_kernel");
+            return SOAP_OK;
+        }
         if (a.J_max <= 4) rc = launch(lower_resolution_v_kernel<4>, lsf_v_smem_bytes<4>());
         else if (a.J_max <= 8) rc = launch(lower_resolution_v_kernel<8>, lsf_v_smem_bytes<8>());
         else if (a.J_max <= 12) rc = launch(lower_resolution_v_kernel<12>, lsf_v_smem_bytes<12>());
