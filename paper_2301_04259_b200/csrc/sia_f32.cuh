@@ -110,6 +110,7 @@ struct Params {
     // active launch
     int *item_counters;        // [2] item hand-out (zero between launches)
     int item_chunk;            // items a CTA takes per hand-out (1 unless the list is very long: a batch of stars)
+    int order_phases;          // active launch: take a star's phases heaviest first (0: as given)
 };
 
 // __ldg of a pointer-valued field
@@ -273,7 +274,7 @@ struct ActiveSource {
     bool ord_identity;          // more than kOrderCap phases: taken as given
     long long n_items;
     int n_stars, chunk;
-    bool scheduler;
+    bool scheduler, order;
     int pub, pub_end;  // scheduler: items published, job number after the last of them
     bool pub_done;
     int cs_pub;        // scheduler: star of the last hand-out's first item (item numbers only grow)
@@ -289,7 +290,7 @@ struct ActiveSource {
         const int n = many ? __ldg(&b->n_phases) : b->n_phases;
         const int *wk = many ? ldg_ptr(&b->work) : b->work, *njp = many ? ldg_ptr(&b->n_jobs) : b->n_jobs;
         ord_star = st;
-        ord_identity = n > kOrderCap;
+        ord_identity = n > kOrderCap || !order;
         if (ord_identity) return;
         __syncwarp();
         bool wide = false;
@@ -415,6 +416,7 @@ struct ActiveSource {
         n_items = p.n_items;
         n_stars = p.n_stars;
         chunk = p.item_chunk;
+        order = p.order_phases != 0;
         scheduler = is_scheduler;
         pub = 0;
         pub_end = 0;

@@ -363,7 +363,10 @@ int launch_composite(soap_star *owner, const comp::Star *host_stars, const comp:
     const long long cmax = 8LL * ((max_mu + 1) / 2) + comp::kPairCostBase;
     long long min_units = 0;
     for (int k = 0; k < n_stars; ++k) min_units += (long long)host_stars[k].n_tiles * host_stars[k].n_pairs * comp::kPairCostBase;
-    const long long G = std::max(1LL, std::min((long long)owner->n_sm * comp::kCtasPerSm, min_units / (2 * cmax)));
+    // (short spectra: a CTA's range should hold a few pairs of every tile it shares - the span loads and the hand-over of the
+    // shares are what a small launch costs; C2: 60 - 80 CTAs 26.6 us, 40 or 86 CTAs 30.7 us)
+    long long G = std::max(1LL, std::min((long long)owner->n_sm * comp::kCtasPerSm, min_units * 2 / (5 * cmax)));
+    if (owner->opt_quiet_splits > 0) G = std::max(1LL, std::min(G, (long long)owner->opt_quiet_splits));  // SOAP_OPT_QUIET_SPLITS caps the grid
     SOAP_CUDA(owner, owner->d_partial.reserve((size_t)G * 2 * comp::kSpan));
     p.partial = owner->d_partial.ptr;
     const size_t smem = comp::smem_bytes(nb, max_pairs, max_halo);
@@ -737,6 +740,7 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
     const long long G = std::max(1LL, std::min((long long)own->n_sm * own->occ_active, n_items));
     // very long item lists (a batch of stars) are handed out several items at a time
     p.item_chunk = (int)std::max(1LL, std::min((long long)f32::kMaxItemChunk, n_items / (G * 64)));
+    p.order_phases = n_items > 2 * G ? 1 : 0;  // with an item or two per CTA the order of the hand-out buys nothing
     if (own->opt_timing) {
         for (int k = 2; k < 4; ++k)
             if (!own->ev[k]) SOAP_CUDA(own, cudaEventCreate(&own->ev[k]));
