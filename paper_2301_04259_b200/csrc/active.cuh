@@ -1,13 +1,14 @@
 // a4 of SURVEY section 8: per-phase active map and compaction (InfoMap of Alg. 5).
 //
 // The paper rewrites an N x N type map on the device at every timestamp.  Here the map is never
-// materialised.  One thread-block cluster of 8 CTAs per phase; CTA `rank` owns a contiguous eighth of the
+// materialised.  One thread-block cluster of 8 CTAs per (star, phase); CTA `rank` owns an eighth of the list of
 // columns the phase's regions can reach.  A warp walks a column, decides each cell's type by spherical
 // angular distance with list-order override, and bins the covered cells by (kind, mu-bin) - all cells of a
-// column share one velocity - into shared memory.  The CTAs exchange their per-segment entry counts through
-// distributed shared memory, so that each can compact its non-zero bins of every (kind, mu-bin) segment
-// behind those of the lower ranks: the entry list the shift-interpolate-accumulate kernel consumes is in
-// column order.  Rank 0 writes the phase's job list; the last phase to finish orders the phases by work.
+// column share one velocity - into shared memory.  The CTAs push their per-segment entry counts into each
+// other's shared memory (distributed shared memory), so that each can compact its non-zero bins of every
+// (kind, mu-bin) segment behind those of the lower ranks: the entry list the shift-interpolate-accumulate
+// kernel consumes is in column order.  Rank 0 writes the phase's job list and its job / entry counts; the
+// active launch takes the phases heaviest first by the latter (sia_f32.cuh).
 // One launch, no scratch to zero, no floating-point atomics (every sum has a fixed order).
 // Kinds: 0 = quiet row of a covered cell (weight -w), 1 = spot row, 2 = facula row (weight +w LB_t(mu)).
 #pragma once

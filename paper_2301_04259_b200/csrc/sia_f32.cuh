@@ -37,9 +37,10 @@
 //   * quiet launch: the flattened (tile, entry) work list is cut into equal contiguous ranges, one per
 //     CTA, grid = resident CTA slots (one wave, no tail); a CTA writes one fp64 partial per tile it
 //     touches and the last CTA to deliver its share of a tile adds the shares in CTA order (deterministic).
-//   * active launch: persistent CTAs take the (phase, tile) items, heaviest phase first, from a global
-//     counter (active_prepare_kernel builds the per-phase job lists and the order); the
-//     post-shift contrast (I_ratio of Eq. 3) multiplies each kind's fp64 sum once per pixel (a6).
+//   * active launch: persistent CTAs take the (star, phase, tile) items, heaviest phase first, from a global
+//     counter (active_prepare_kernel builds the per-phase job lists; a CTA's scheduler warp ranks a star's
+//     phases by their entry counts); the post-shift contrast (I_ratio of Eq. 3) of a kind multiplies the
+//     fp32 partial sums of that kind in fp64 when they are folded into the fp64 totals (a6).
 #pragma once
 #include <climits>
 #include <cstdint>
