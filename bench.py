@@ -332,10 +332,26 @@ def config_lines(soap, torch, timer, workloads, dev, steps, peak_instr):
         torch.cuda.synchronize()
         launches = sum(soap.soap_get_stats(s_)["launches"] for s_ in stars) - launches0
         mm = float(np.mean(ms))
+        graph_ms = None
+        if n == 1 and len(w0.regions) * n_ph <= 192:  # a single star's step whose region centres travel as kernel arguments
+            # enqueues kernels only and can be captured in a CUDA graph (include/soap_b200.h)
+            try:
+                side = torch.cuda.Stream()
+                with torch.cuda.stream(side):
+                    step()
+                    side.synchronize()
+                    graph = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(graph, stream=side):
+                        step()
+                torch.cuda.synchronize()
+                graph_ms = float(np.mean(timer.steps(graph.replay, max(3, min(steps, 10)))))
+            except Exception:
+                graph_ms = None
         res[name] = {
             "workload": workloads.CONFIG_NAMES[int(name[1])], "stars": n, "ms_per_step": mm,
             "ms_per_step_median": float(np.median(ms)), "ms_per_step_best": float(np.min(ms)),
             "spectra_per_s": n * (1 + n_ph) / (mm * 1e-3), "launches_per_step": launches,
+            "ms_per_step_cuda_graph": graph_ms,
             "quiet_form": FORM_NAMES[st["form"]], "quiet_entries": q_ent, "active_entries": a_ent,
             "quiet_kernel_ms": st["quiet_kernel_ms"], "active_kernel_ms": st["active_kernel_ms"],
             "quiet_alu_frac": iq / (st["quiet_kernel_ms"] * 1e-3) / peak_instr if st["quiet_kernel_ms"] > 0 else None,
@@ -426,6 +442,23 @@ def run_graft(args):
     total_ms = sharding.max_over_ranks(total_ms, dev)
     ms_per_step = total_ms / args.steps
     value = world * n_spec / (ms_per_step * 1e-3)
+
+    # ---- the same step captured once in a CUDA graph and replayed (a single star's step enqueues four kernels and nothing
+    # else, so it can be captured; the host-side cost of the three calls drops out) ------------------------------------------
+    graph_ms = None
+    try:
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            step()
+            side.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                step()
+        torch.cuda.synchronize()
+        graph_ms = float(np.mean(timer.steps(graph.replay, max(5, min(args.steps, 20)))))
+    except Exception as exc:  # reported, never fatal: the graph leg is informational
+        graph_ms = None
+        sys.stderr.write(f"cuda graph leg skipped: {exc}\n")
 
     # ---- the device's FP32 FMA rate, measured live with the inner loops' instruction forms ----------------
     probe = {"ffma2_fma_per_s": soap.soap_probe_fp32_rate(star, True), "ffma_fma_per_s": soap.soap_probe_fp32_rate(star, False),
@@ -600,6 +633,7 @@ def run_graft(args):
                                     "note": "spectra tables uploaded once (a time series re-uses them); per step the region centres "
                                             "go in and the 26 spectra are copied to pinned host memory"}},
         "gpu_launches": launches, "wall_s_timed_region": wall,
+        "cuda_graph": {"ms_per_step": graph_ms, "note": "the timed step captured once and replayed (4 kernel nodes with programmatic edges)"},
     }
     if world == 1 and not args.no_cpu_baseline:
         t_full, threads = oracle_full(wl)

@@ -25,8 +25,11 @@
  *     Scratch is (re)allocated with cudaMalloc when a call needs more than any earlier call did; once
  *     sizes have been seen, calls allocate nothing.  A single star's soap_active_timeseries* call passes its
  *     region centres as kernel arguments (up to 192 (phase, region) pairs) and copies nothing; larger calls
- *     and the batch calls stage them through a ring of pinned host buffers guarded by events, so the
- *     time-series calls must not be stream-captured.
+ *     and the batch calls stage them through a ring of pinned host buffers guarded by events and must not be
+ *     stream-captured.  A single star's geometry / quiet / time-series calls with HOST outputs NULL, after one
+ *     un-captured call of the same sizes (scratch allocated), enqueue kernels only and CAN be captured in a
+ *     CUDA graph (tests/test_gpu_edges.py); the captured step is fixed: its regions and phases are kernel
+ *     arguments of the graph's nodes.
  *   - The launches of a handle's consecutive calls on one stream (geometry, quiet, active map, active delta)
  *     are chained with programmatic dependent launch: a launch may start while its predecessor drains and
  *     waits on the device before it reads what the predecessor wrote.  Nothing changes for the caller.
