@@ -311,8 +311,7 @@ def config_lines(soap, torch, timer, workloads, dev, steps, peak_instr):
                 soap.soap_integrate_quiet(stars[0], q, Q[0])
                 soap.soap_active_timeseries(stars[0], q, sp, fa, w0.regions, w0.phases, D[0])
                 return
-            for st_, wl in zip(stars, wls):
-                soap.soap_disk_geometry(st_, wl, want_info=False)
+            soap.soap_batch_disk_geometry(stars, wls)
             soap.soap_batch_integrate_quiet(stars, [q] * n, [Q[k] for k in range(n)])
             soap.soap_batch_active_timeseries(stars, [q] * n, [sp] * n, [fa] * n, [w.regions for w in wls],
                                               [w.phases for w in wls], [D[k] for k in range(n)])

@@ -286,6 +286,11 @@ int soap_synthesize_host(soap_star *star, const soap_star_params *params, const 
  * rotation, several devices) fall back to per-star launches dealt to `stream` and two side streams of
  * stars[0], forked from and joined back into `stream` with events.  A star must not appear twice in a batch;
  * no stream capture. */
+/* soap_disk_geometry for n_stars stars in ONE launch (every star's CTAs side by side, each star with its own
+ * finalisation).  params: HOST array of n_stars pointers.  infos: HOST [n_stars] or NULL; non-NULL synchronises `stream`.
+ * Stars on several devices (or n_stars == 1) are served by per-star calls. */
+int soap_batch_disk_geometry(soap_star *const *stars, int32_t n_stars, const soap_star_params *const *params, void *stream,
+                             soap_geom_info *infos);
 int soap_batch_integrate_quiet(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet,
                                void *const *out, void *stream);
 int soap_batch_active_timeseries(soap_star *const *stars, int32_t n_stars, const soap_spectra *const *quiet,

@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = (
     "soap_disk_geometry", "soap_integrate_quiet", "soap_active_timeseries", "soap_active_timeseries_effects",
     "soap_export_geometry", "soap_lower_resolution", "soap_active_timeseries_evolving", "soap_line_rvs",
     "soap_synthesize_host", "soap_batch_integrate_quiet", "soap_batch_active_timeseries", "soap_contrast_planck",
-    "soap_probe_fp32_rate",
+    "soap_probe_fp32_rate", "soap_batch_disk_geometry",
 )
 
 
@@ -117,6 +117,8 @@ def load_library() -> ctypes.CDLL:
                                          ctypes.POINTER(c_spectra), ctypes.POINTER(c_spectra),
                                          ctypes.POINTER(c_region), i32, ctypes.POINTER(ctypes.c_double), i32,
                                          vp, vp, ctypes.POINTER(i32), vp]
+    lib.soap_batch_disk_geometry.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(ctypes.POINTER(c_star_params)), vp,
+                                             ctypes.POINTER(c_geom_info)]
     lib.soap_batch_integrate_quiet.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(ctypes.POINTER(c_spectra)),
                                                ctypes.POINTER(vp), vp]
     lib.soap_batch_active_timeseries.argtypes = [
@@ -398,6 +400,24 @@ def soap_synthesize_host(star: Star, params, quiet: Spectra, spot: Optional[Spec
         _ptr(out_delta) if out_delta is not None else None,
         na.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)) if na is not None else None, _stream_handle(stream)))
     return na[:n_ph] if na is not None else None
+
+
+def soap_batch_disk_geometry(stars: Sequence[Star], params: Sequence, stream=None, want_info: bool = False):
+    """The geometry of many stars in one launch; params[k] as for soap_disk_geometry.  Returns a list of info dicts or None."""
+    n = len(stars)
+    lib = stars[0]._lib
+    hs = (ctypes.c_void_p * n)(*[s._h for s in stars])
+    cps = [_params(p) for p in params]  # (struct, mu array kept alive)
+    pp = (ctypes.POINTER(c_star_params) * n)(*[ctypes.pointer(c) for c, _ in cps])
+    infos = (c_geom_info * n)() if want_info else None
+    rc = lib.soap_batch_disk_geometry(hs, n, pp, _stream_handle(stream), infos)
+    if rc != SOAP_OK:
+        msgs = [lib.soap_last_error(s._h).decode() for s in stars]
+        raise SoapError(rc, "; ".join(m for m in msgs if m))
+    if not want_info:
+        return None
+    return [dict(n_visible=int(i.n_visible), n_entries=int(i.n_entries), sum_weights=float(i.sum_weights),
+                 max_abs_dshift=float(i.max_abs_dshift)) for i in infos]
 
 
 def soap_batch_integrate_quiet(stars: Sequence[Star], quiet: Sequence[Spectra], out: Sequence[torch.Tensor],

@@ -148,8 +148,8 @@ __device__ void build_binned_entries(int N, int n_mu, const double *col_a, const
                                      const int *col_nvis, float2 *ent32, double2 *ent64, int *row_start, DevInfo *info) {
     __shared__ int s_cnt[64];
     __shared__ int s_start[65];
-    __shared__ int s_nv[1024];  // blockDim.x == 1024 (a power of two); N <= 8192 so N^2 fits an int
-    __shared__ double s_sw[1024], s_am[1024];
+    __shared__ long long s_nv[32];  // per-warp partial sums of the summary
+    __shared__ double s_sw[32], s_am[32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
     constexpr int kBatch = 8;  // loads of 8 x 32 columns are issued together: one memory round trip per batch
     for (int b = warp; b < n_mu; b += n_warps) {
@@ -167,7 +167,7 @@ __device__ void build_binned_entries(int N, int n_mu, const double *col_a, const
         if (lane == 0) s_cnt[b] = cnt;
     }
     __syncthreads();
-    // summary: per-thread strided partials, then a fixed shared-memory tree (deterministic)
+    // summary: per-thread strided partials, a fixed xor tree inside the warps, then the warps in order (deterministic)
     {
         long long nv = 0;
         double sw = 0.0, am = 0.0;
@@ -177,19 +177,27 @@ __device__ void build_binned_entries(int N, int n_mu, const double *col_a, const
             sw += col_sumw[j];
             if (c > 0) am = fmax(am, fabs(col_a[j]));
         }
-        s_nv[threadIdx.x] = (int)nv;
-        s_sw[threadIdx.x] = sw;
-        s_am[threadIdx.x] = am;
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            nv += __shfl_xor_sync(0xffffffffu, nv, d);
+            sw += __shfl_xor_sync(0xffffffffu, sw, d);
+            am = fmax(am, __shfl_xor_sync(0xffffffffu, am, d));
+        }
+        if (lane == 0) {
+            s_nv[warp] = nv;
+            s_sw[warp] = sw;
+            s_am[warp] = am;
+        }
     }
     __syncthreads();
-    for (int d = blockDim.x >> 1; d > 0; d >>= 1) {
-        if (threadIdx.x < d) {
-            s_nv[threadIdx.x] += s_nv[threadIdx.x + d];
-            s_sw[threadIdx.x] += s_sw[threadIdx.x + d];
-            s_am[threadIdx.x] = fmax(s_am[threadIdx.x], s_am[threadIdx.x + d]);
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < n_warps; ++w) {
+            s_nv[0] += s_nv[w];
+            s_sw[0] += s_sw[w];
+            s_am[0] = fmax(s_am[0], s_am[w]);
         }
-        __syncthreads();
     }
+    __syncthreads();
     if (threadIdx.x == 0) {
         int off = 0, total = 0;
         for (int b = 0; b < n_mu; ++b) {
@@ -506,23 +514,67 @@ __host__ __device__ inline int geom_warps_per_col(int N) {
 }
 __host__ __device__ inline int geom_cols_per_cta(int N) { return kGeomWarps / geom_warps_per_col(N); }
 
+struct GeomArgs {  // one star's geometry launch
+    int N, mode, n_mu, cells, comp_stride, fin_smem, n_ctas, pad;
+    Rotation rot;
+    double u1, u2;
+    MuCentres mu_centres;
+    double *mu_out, *w_out, *vel_out;
+    int *bin_out;
+    double *col_a, *Wbin /*[N][n_mu]*/, *col_sumw;
+    int *col_nvis;
+    float2 *ent32;
+    double2 *ent64;
+    int *row_start;
+    DevInfo *info;
+    unsigned int *done;
+    int *colcnt /*[N][n_mu]*/, *cellpos /*[n_mu][N], per-cell form only*/;
+    float2 *comp_Wp /*composite form: [ceil(N/2)][comp_stride], or nullptr*/;
+    comp::PairHdr *comp_hdr;
+};
+static_assert(sizeof(GeomArgs) % 8 == 0, "copied to shared memory in 8-byte words");
+
+// `one`: a single star (many == nullptr).  Batch (soap_batch_disk_geometry): `many` = DEVICE [n_stars] arguments, `cta0` =
+// DEVICE [n_stars + 1] first CTA of every star; every star keeps its own last-CTA ticket.
+// dynamic shared memory = the largest fin_smem_bytes(N, n_mu) of the stars with fin_smem set.
 __global__ void __launch_bounds__(32 * kGeomWarps)
-geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n_mu, const MuCentres mu_centres,
-                double *__restrict__ mu_out, double *__restrict__ w_out, double *__restrict__ vel_out,
-                int *__restrict__ bin_out, double *__restrict__ col_a, double *__restrict__ Wbin /*[N][n_mu]*/,
-                double *__restrict__ col_sumw, int *__restrict__ col_nvis, float2 *__restrict__ ent32,
-                double2 *__restrict__ ent64, int *__restrict__ row_start, DevInfo *__restrict__ info,
-                unsigned int *__restrict__ done, int *__restrict__ colcnt /*[N][n_mu]*/,
-                int *__restrict__ cellpos /*[n_mu][N], per-cell form only*/, int cells,
-                float2 *__restrict__ comp_Wp /*composite form: [ceil(N/2)][comp_stride], or nullptr*/, int comp_stride,
-                comp::PairHdr *__restrict__ comp_hdr, int fin_smem /*dynamic shared memory holds fin_smem_bytes(N, n_mu)*/) {
+geometry_kernel(const GeomArgs one, const GeomArgs *__restrict__ many, const int *__restrict__ cta0, int n_stars) {
     extern __shared__ __align__(16) unsigned char geom_dyn[];
     __shared__ double s_W[kGeomWarps][64];
     __shared__ int s_Cn[kGeomWarps][64];
     __shared__ double s_mu[64];
     __shared__ double s_sum[kGeomWarps];
     __shared__ int s_nvis[kGeomWarps];
-    __shared__ int s_last;
+    __shared__ int s_last, s_first;
+    __shared__ GeomArgs s_a;
+    {
+        int star = 0, first = 0;
+        if (many) {
+            int lo = 0, hi = n_stars - 1;  // last star with cta0[s] <= blockIdx.x
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (__ldg(&cta0[mid]) <= (int)blockIdx.x) lo = mid;
+                else hi = mid - 1;
+            }
+            star = lo;
+            first = __ldg(&cta0[lo]);
+        }
+        const unsigned long long *src = reinterpret_cast<const unsigned long long *>(many ? many + star : &one);
+        unsigned long long *dst = reinterpret_cast<unsigned long long *>(&s_a);
+        for (int k = threadIdx.x; k < (int)(sizeof(GeomArgs) / 8); k += blockDim.x) dst[k] = src[k];
+        if (threadIdx.x == 0) s_first = first;
+    }
+    __syncthreads();
+    const int N = s_a.N, mode = s_a.mode, n_mu = s_a.n_mu;
+    const Rotation rot = s_a.rot;
+    const double u1 = s_a.u1, u2 = s_a.u2;
+    const MuCentres &mu_centres = s_a.mu_centres;
+    double *__restrict__ mu_out = s_a.mu_out, *__restrict__ w_out = s_a.w_out, *__restrict__ vel_out = s_a.vel_out;
+    int *__restrict__ bin_out = s_a.bin_out;
+    double *__restrict__ col_a = s_a.col_a, *__restrict__ Wbin = s_a.Wbin, *__restrict__ col_sumw = s_a.col_sumw;
+    int *__restrict__ col_nvis = s_a.col_nvis, *__restrict__ colcnt = s_a.colcnt;
+    unsigned int *__restrict__ done = s_a.done;
+    const int bid = (int)blockIdx.x - s_first;  // this star's CTA number
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     trigger_dependents();  // the quiet launch that follows may stage its spectra while this kernel runs (ptx_helpers.cuh)
     for (int b = threadIdx.x; b < n_mu; b += blockDim.x) s_mu[b] = mu_centres.v[b];
@@ -533,7 +585,7 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
     __syncthreads();
     const int wpc = geom_warps_per_col(N), cpc = kGeomWarps / wpc;
     const int cl = warp / wpc, chunk = warp - cl * wpc;  // local column, first chunk
-    const int j = blockIdx.x * cpc + cl;
+    const int j = bid * cpc + cl;
     double sum = 0.0;
     int nvis = 0;
     if (cl < cpc && j < N) {
@@ -549,7 +601,7 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
     }
     __syncthreads();
     if (warp < cpc) {  // warp `warp` finishes local column `warp`
-        const int jj = blockIdx.x * cpc + warp;
+        const int jj = bid * cpc + warp;
         if (jj < N) {
             for (int b = lane; b < n_mu; b += 32) {
                 double W = 0.0;
@@ -575,24 +627,24 @@ geometry_kernel(int N, const Rotation rot, double u1, double u2, int mode, int n
     }
     __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(done, 1u) == gridDim.x - 1) ? 1 : 0;
+    if (threadIdx.x == 0) s_last = (atomicAdd(done, 1u) == (unsigned)s_a.n_ctas - 1u) ? 1 : 0;
     __syncthreads();
     if (!s_last) return;
     __threadfence();
     if (threadIdx.x == 0) *done = 0;
-    if (fin_smem) {
-        finalize_columns_smem(N, n_mu, col_a, Wbin, col_sumw, col_nvis, ent32, ent64, row_start, info, comp_Wp, comp_stride, comp_hdr,
-                              geom_dyn);
+    if (s_a.fin_smem) {
+        finalize_columns_smem(N, n_mu, col_a, Wbin, col_sumw, col_nvis, s_a.ent32, s_a.ent64, s_a.row_start, s_a.info, s_a.comp_Wp,
+                              s_a.comp_stride, s_a.comp_hdr, geom_dyn);
     } else {
-        build_binned_entries(N, n_mu, col_a, Wbin, col_sumw, col_nvis, ent32, ent64, row_start, info);
-        if (comp_Wp) {  // pair tables of the composite-column form (composite.cuh)
+        build_binned_entries(N, n_mu, col_a, Wbin, col_sumw, col_nvis, s_a.ent32, s_a.ent64, s_a.row_start, s_a.info);
+        if (s_a.comp_Wp) {  // pair tables of the composite-column form (composite.cuh)
             __syncthreads();
-            comp::build_composite_tables(N, n_mu, col_a, Wbin, comp_Wp, comp_stride, comp_hdr);
+            comp::build_composite_tables(N, n_mu, col_a, Wbin, s_a.comp_Wp, s_a.comp_stride, s_a.comp_hdr);
         }
     }
-    if (cells) {  // per-cell form: the entry list is rebuilt by write_cell_entries_kernel at these positions
+    if (s_a.cells) {  // per-cell form: the entry list is rebuilt by write_cell_entries_kernel at these positions
         __syncthreads();
-        build_cell_positions(N, n_mu, colcnt, cellpos, row_start, ent32, ent64);
+        build_cell_positions(N, n_mu, colcnt, s_a.cellpos, s_a.row_start, s_a.ent32, s_a.ent64);
     }
 }
 

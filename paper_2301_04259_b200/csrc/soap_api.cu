@@ -90,7 +90,8 @@ struct soap_star {
     DevBuf<float2> d_cWp;
     DevBuf<comp::PairHdr> d_chdr;
     int comp_stride = 0;  // bins per table row (multiple of 4); 0 = tables not built
-    DevBuf<comp::Star> d_cstars;  // batch launches: the stars' descriptors (owned by the first star of the batch)
+    DevBuf<comp::Star> d_cstars;
+    DevBuf<unsigned char> d_gargs;  // batch geometry: the stars' kernel arguments (owned by the first star of the batch)  // batch launches: the stars' descriptors (owned by the first star of the batch)
 
     // quiet scratch
     DevBuf<double> d_partial;
@@ -1144,7 +1145,7 @@ int soap_create(soap_star **out, int device) {
 int soap_destroy(soap_star *s) {
     if (!s) return SOAP_OK;
     cudaSetDevice(s->device);
-    s->d_cWp.release(); s->d_chdr.release(); s->d_cstars.release();
+    s->d_cWp.release(); s->d_chdr.release(); s->d_cstars.release(); s->d_gargs.release();
     s->d_geom_done.release(); s->d_colcnt.release(); s->d_cellpos.release(); s->d_mu.release(); s->d_w.release(); s->d_vel.release(); s->d_col_a.release();
     s->d_Wbin.release(); s->d_col_sumw.release(); s->d_bin.release(); s->d_col_nvis.release(); s->d_row_start.release();
     s->d_ent32.release(); s->d_ent64.release(); s->d_info.release(); s->d_partial.release(); s->d_tile_ticket.release(); s->d_rp.release();
@@ -1190,8 +1191,9 @@ int soap_set_option(soap_star *s, int32_t option, int64_t value) {
     }
 }
 
-int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, soap_geom_info *info) {
-    if (!s) return SOAP_ERR_INVALID_ARG;
+// soap_disk_geometry in three parts, so that the batch entry point can check every star before anything is enqueued and
+// launch once for all of them: argument checks; state, scratch and the kernel's arguments; what follows the launch.
+static int geometry_check(soap_star *s, const soap_star_params *prm) {
     if (!prm) return s->fail(SOAP_ERR_INVALID_ARG, "params is NULL");
     if (prm->grid_n < 1 || prm->grid_n > 8192) return s->fail(SOAP_ERR_INVALID_ARG, "grid_n must be in 1..8192");
     if (prm->n_mu < 1 || prm->n_mu > SOAP_MAX_MU) return s->fail(SOAP_ERR_INVALID_ARG, "n_mu must be in 1..%d", SOAP_MAX_MU);
@@ -1208,8 +1210,18 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     if (std::fabs(prm->vsini_kms * sini) * std::max(1.0, 1.0 + prm->diff_rot) >= 0.1 * kSpeedOfLightKms)
         return s->fail(SOAP_ERR_INVALID_ARG, "|v| must be below 0.1 c");
 
+    if (!std::isfinite(prm->diff_rot) || !(prm->diff_rot > -1.0)) return s->fail(SOAP_ERR_INVALID_ARG, "diff_rot must be finite and > -1");
+    if (prm->diff_rot != 0.0 && s->form == SOAP_FORM_BINNED)
+        return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_BINNED needs solid-body rotation: the cells of a column must share one velocity");
+    if (prm->diff_rot != 0.0 && s->form == SOAP_FORM_COMPOSITE)
+        return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_COMPOSITE needs solid-body rotation: the cells of a column must share one velocity");
+    return SOAP_OK;
+}
+
+static int geometry_prepare(soap_star *s, const soap_star_params *prm, cudaStream_t st, GeomArgs &ga, size_t &fin_bytes_out) {
+    const double pi = 3.14159265358979323846;
+    const double sini = std::sin(prm->incl_deg * pi / 180.0), cosi = std::cos(prm->incl_deg * pi / 180.0);
     SOAP_CUDA(s, cudaSetDevice(s->device));
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
     s->ready = false;
     s->last_form = 0;
     s->prm = *prm;
@@ -1219,11 +1231,6 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
     s->cosi = cosi;
     const int N = prm->grid_n, n_mu = prm->n_mu;
     const size_t ncell = (size_t)N * N;
-    if (!std::isfinite(prm->diff_rot) || !(prm->diff_rot > -1.0)) return s->fail(SOAP_ERR_INVALID_ARG, "diff_rot must be finite and > -1");
-    if (prm->diff_rot != 0.0 && s->form == SOAP_FORM_BINNED)
-        return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_BINNED needs solid-body rotation: the cells of a column must share one velocity");
-    if (prm->diff_rot != 0.0 && s->form == SOAP_FORM_COMPOSITE)
-        return s->fail(SOAP_ERR_UNSUPPORTED, "SOAP_FORM_COMPOSITE needs solid-body rotation: the cells of a column must share one velocity");
     s->form_used = (s->form == SOAP_FORM_CELLS || s->form == SOAP_FORM_FIR) ? s->form : SOAP_FORM_BINNED;
     // the composite-column form holds every mu-bin row of a span in registers: up to comp::kMaxBins bins
     // AUTO takes it for the quiet spectrum whenever it applies: its cost does not depend on v sin i, and it is at least as
@@ -1274,12 +1281,42 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
         SOAP_CUDA(s, cudaFuncSetAttribute(geometry_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFinSmemMax));
         s->attr_geom_set = true;
     }
-    geometry_kernel<<<(N + geom_cols_per_cta(N) - 1) / geom_cols_per_cta(N), 32 * kGeomWarps, fin_smem ? fin_bytes : 0, st>>>(
-        N, rot, prm->ld_u1, prm->ld_u2, prm->doppler_mode, n_mu, mc, s->d_mu.ptr, s->d_w.ptr, s->d_vel.ptr, s->d_bin.ptr,
-        s->d_col_a.ptr, s->d_Wbin.ptr, s->d_col_sumw.ptr, s->d_col_nvis.ptr, s->d_ent32.ptr, s->d_ent64.ptr, s->d_row_start.ptr,
-        s->d_info.ptr, s->d_geom_done.ptr, s->d_colcnt.ptr, s->d_cellpos.ptr, s->cell_entries ? 1 : 0,
-        s->comp_stride ? s->d_cWp.ptr : nullptr, s->comp_stride, s->d_chdr.ptr, fin_smem ? 1 : 0);
-    SOAP_LAUNCH_CHECK(s, "geometry_kernel");
+    ga = GeomArgs{};
+    ga.N = N;
+    ga.mode = prm->doppler_mode;
+    ga.n_mu = n_mu;
+    ga.cells = s->cell_entries ? 1 : 0;
+    ga.comp_stride = s->comp_stride;
+    ga.fin_smem = fin_smem ? 1 : 0;
+    ga.n_ctas = (N + geom_cols_per_cta(N) - 1) / geom_cols_per_cta(N);
+    ga.rot = rot;
+    ga.u1 = prm->ld_u1;
+    ga.u2 = prm->ld_u2;
+    ga.mu_centres = mc;
+    ga.mu_out = s->d_mu.ptr;
+    ga.w_out = s->d_w.ptr;
+    ga.vel_out = s->d_vel.ptr;
+    ga.bin_out = s->d_bin.ptr;
+    ga.col_a = s->d_col_a.ptr;
+    ga.Wbin = s->d_Wbin.ptr;
+    ga.col_sumw = s->d_col_sumw.ptr;
+    ga.col_nvis = s->d_col_nvis.ptr;
+    ga.ent32 = s->d_ent32.ptr;
+    ga.ent64 = s->d_ent64.ptr;
+    ga.row_start = s->d_row_start.ptr;
+    ga.info = s->d_info.ptr;
+    ga.done = s->d_geom_done.ptr;
+    ga.colcnt = s->d_colcnt.ptr;
+    ga.cellpos = s->d_cellpos.ptr;
+    ga.comp_Wp = s->comp_stride ? s->d_cWp.ptr : nullptr;
+    ga.comp_hdr = s->d_chdr.ptr;
+    fin_bytes_out = fin_smem ? fin_bytes : 0;
+    return SOAP_OK;
+}
+
+static int geometry_finish(soap_star *s, cudaStream_t st, soap_geom_info *info) {
+    const soap_star_params *prm = &s->prm;
+    const int N = prm->grid_n, n_mu = prm->n_mu;
     if (s->cell_entries) {
         write_cell_entries_kernel<<<(N + kCellWarps - 1) / kCellWarps, 32 * kCellWarps, 0, st>>>(
             N, n_mu, prm->doppler_mode, s->d_vel.ptr, s->d_w.ptr, s->d_bin.ptr, s->d_cellpos.ptr, s->d_ent32.ptr, s->d_ent64.ptr);
@@ -1294,6 +1331,77 @@ int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, 
         info->n_entries = s->cell_entries ? di.n_visible : di.n_entries;
         info->sum_weights = di.sum_weights;
         info->max_abs_dshift = di.max_abs_dshift;
+    }
+    return SOAP_OK;
+}
+
+int soap_disk_geometry(soap_star *s, const soap_star_params *prm, void *stream, soap_geom_info *info) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    int rc = geometry_check(s, prm);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    GeomArgs ga;
+    size_t fin_bytes = 0;
+    if ((rc = geometry_prepare(s, prm, st, ga, fin_bytes))) return rc;
+    // a1 + a2 in one launch: the last CTA compacts the binned weights into the entry list
+    geometry_kernel<<<ga.n_ctas, 32 * kGeomWarps, fin_bytes, st>>>(ga, nullptr, nullptr, 1);
+    SOAP_LAUNCH_CHECK(s, "geometry_kernel");
+    return geometry_finish(s, st, info);
+}
+
+// config 5: the geometry of many stars in ONE launch (every star's CTAs side by side, each star with its own last-CTA
+// finalisation); per-cell entry lists (differential rotation) are written by one more launch per such star.
+int soap_batch_disk_geometry(soap_star *const *stars, int32_t n_stars, const soap_star_params *const *params, void *stream,
+                             soap_geom_info *infos) {
+    if (!stars || !params || n_stars < 0) return SOAP_ERR_INVALID_ARG;
+    for (int k = 0; k < n_stars; ++k)
+        if (!stars[k]) return SOAP_ERR_INVALID_ARG;
+    if (n_stars == 0) return SOAP_OK;
+    soap_star *s0 = stars[0];
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    bool one_launch = n_stars > 1;
+    for (int k = 0; k < n_stars; ++k) {  // every argument of every star is checked before anything is enqueued
+        int rc = geometry_check(stars[k], params[k]);
+        if (rc) return rc;
+        for (int j = 0; j < k; ++j)
+            if (stars[j] == stars[k]) return stars[k]->fail(SOAP_ERR_INVALID_ARG, "star %d appears twice in the batch", k);
+        one_launch = one_launch && stars[k]->device == s0->device;
+    }
+    if (!one_launch) {  // a single star, or several devices: per-star calls
+        for (int k = 0; k < n_stars; ++k) {
+            int rc = soap_disk_geometry(stars[k], params[k], stream, infos ? infos + k : nullptr);
+            if (rc) return rc;
+        }
+        return SOAP_OK;
+    }
+    std::vector<GeomArgs> args((size_t)n_stars);
+    std::vector<int> cta0((size_t)n_stars + 1);
+    size_t fin_bytes = 0;
+    int total = 0;
+    for (int k = 0; k < n_stars; ++k) {
+        size_t fb = 0;
+        int rc = geometry_prepare(stars[k], params[k], st, args[k], fb);
+        if (rc) return rc;
+        fin_bytes = std::max(fin_bytes, fb);
+        cta0[k] = total;
+        total += args[k].n_ctas;
+    }
+    cta0[n_stars] = total;
+    const size_t a_bytes = (size_t)n_stars * sizeof(GeomArgs), c_off = (a_bytes + 15) & ~(size_t)15;
+    const size_t bytes = c_off + (size_t)(n_stars + 1) * sizeof(int);
+    if (bytes > s0->d_gargs.cap) {
+        SOAP_CUDA(s0, cudaStreamSynchronize(st));  // an earlier launch may still read the old buffer
+        SOAP_CUDA(s0, s0->d_gargs.reserve(bytes + 4096));
+    }
+    // pageable sources: the runtime stages them before returning, so the vectors may go out of scope
+    SOAP_CUDA(s0, cudaMemcpyAsync(s0->d_gargs.ptr, args.data(), a_bytes, cudaMemcpyHostToDevice, st));
+    SOAP_CUDA(s0, cudaMemcpyAsync(s0->d_gargs.ptr + c_off, cta0.data(), (size_t)(n_stars + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
+    geometry_kernel<<<total, 32 * kGeomWarps, fin_bytes, st>>>(args[0], reinterpret_cast<const GeomArgs *>(s0->d_gargs.ptr),
+                                                            reinterpret_cast<const int *>(s0->d_gargs.ptr + c_off), n_stars);
+    SOAP_LAUNCH_CHECK(s0, "geometry_kernel");
+    for (int k = 0; k < n_stars; ++k) {
+        int rc = geometry_finish(stars[k], st, infos ? infos + k : nullptr);
+        if (rc) return rc;
     }
     return SOAP_OK;
 }

@@ -296,17 +296,24 @@ def test_batch_entry_points_equal_per_star_calls(soap):
     s = soap.to_device_spectra(shared.spot, shared.lambda0, shared.dlambda, dev, shared.spot_contrast, shared.spot_lb)
     f = soap.to_device_spectra(shared.facula, shared.lambda0, shared.dlambda, dev, shared.facula_contrast, shared.facula_lb)
     stars = [soap.soap_create(0) for _ in range(n_stars)]
-    for st, wl in zip(stars, wls):
-        soap.soap_disk_geometry(st, wl, want_info=False)
+    launches0 = sum(soap.soap_get_stats(st)["launches"] for st in stars)
+    infos = soap.soap_batch_disk_geometry(stars, wls, want_info=True)
+    for k, wl in enumerate(wls):              # one geometry launch for the batch: every star's cells as its own call gives them
+        og = oracle.geometry(wl)
+        assert infos[k]["n_visible"] == og["n_visible"] and abs(infos[k]["sum_weights"] - og["sum_w"]) <= 1e-9 * og["sum_w"]
+    ref = soap.soap_create(0)
+    soap.soap_disk_geometry(ref, wls[3], want_info=False)
+    ga, gb = soap.soap_export_geometry(stars[3], wls[3].grid_n), soap.soap_export_geometry(ref, wls[3].grid_n)
+    assert all(np.array_equal(ga[key], gb[key]) for key in ("mu", "w", "vel", "bin"))
+    soap.soap_destroy(ref)
     Qb = torch.full((n_stars, n_pix), float("nan"), dtype=torch.float32, device=dev)
     Db = torch.full((n_stars, n_ph, n_pix), float("nan"), dtype=torch.float32, device=dev)
-    launches0 = sum(soap.soap_get_stats(st)["launches"] for st in stars)
     soap.soap_batch_integrate_quiet(stars, [q] * n_stars, [Qb[k] for k in range(n_stars)])
     soap.soap_batch_active_timeseries(stars, [q] * n_stars, [s] * n_stars, [f] * n_stars, [w.regions for w in wls],
                                       [w.phases for w in wls], [Db[k] for k in range(n_stars)])
     torch.cuda.synchronize()
     launches = sum(soap.soap_get_stats(st)["launches"] for st in stars) - launches0
-    assert launches <= 4, f"{launches} launches for {n_stars} stars: the batch entry points must not launch per star"
+    assert launches <= 5, f"{launches} launches for {n_stars} stars: the batch entry points must not launch per star"
     assert not torch.isnan(Qb).any() and not torch.isnan(Db).any()
     for k, (st, wl) in enumerate(zip(stars, wls)):
         Q1 = torch.empty(n_pix, dtype=torch.float32, device=dev)
