@@ -92,3 +92,40 @@ def test_diffrot_rejects_binned_form_and_runs_fp64(soap):
     assert np.array_equal(g["n_active"], nao) and nao.max() > 0
     assert np.max(np.abs(g["D"] - Do)) <= 1e-9 * np.max(np.abs(Do))
     assert_parity(wl, g)
+
+
+def test_mixed_batch_with_a_differentially_rotating_star(soap):
+    """soap_batch_* with one differentially rotating star among solid-body ones: one geometry launch for all (plus the star's
+    per-cell entry launch), the quiet / active calls fall back to per-star launches; every star's result equals its own calls'."""
+    dev = torch.device("cuda:0")
+    n_pix, n_ph = 12_000, 4
+    shared = workloads.make_config5_star(0, n_pix=n_pix, n_phases=n_ph, grid_n=70)
+    wls = [shared] + [workloads.make_config5_star(k, n_pix=n_pix, n_phases=n_ph, grid_n=70, shared=shared) for k in (1, 2)]
+    wls[1].diff_rot = -0.18
+    q = soap.to_device_spectra(shared.quiet, shared.lambda0, shared.dlambda, dev)
+    s = soap.to_device_spectra(shared.spot, shared.lambda0, shared.dlambda, dev, shared.spot_contrast, shared.spot_lb)
+    f = soap.to_device_spectra(shared.facula, shared.lambda0, shared.dlambda, dev, shared.facula_contrast, shared.facula_lb)
+    stars = [soap.soap_create(0) for _ in wls]
+    soap.soap_batch_disk_geometry(stars, wls)
+    Qb = torch.full((3, n_pix), float("nan"), dtype=torch.float32, device=dev)
+    Db = torch.full((3, n_ph, n_pix), float("nan"), dtype=torch.float32, device=dev)
+    soap.soap_batch_integrate_quiet(stars, [q] * 3, [Qb[k] for k in range(3)])
+    soap.soap_batch_active_timeseries(stars, [q] * 3, [s] * 3, [f] * 3, [w.regions for w in wls], [w.phases for w in wls],
+                                      [Db[k] for k in range(3)])
+    torch.cuda.synchronize()
+    for k, wl in enumerate(wls):
+        ref = soap.soap_create(0)
+        soap.soap_disk_geometry(ref, wl, want_info=False)
+        Q1 = torch.empty(n_pix, dtype=torch.float32, device=dev)
+        D1 = torch.empty((n_ph, n_pix), dtype=torch.float32, device=dev)
+        soap.soap_integrate_quiet(ref, q, Q1)
+        soap.soap_active_timeseries(ref, q, s, f, wl.regions, wl.phases, D1)
+        torch.cuda.synchronize()
+        assert torch.equal(Q1, Qb[k]) and torch.equal(D1, Db[k]), f"star {k}"
+        soap.soap_destroy(ref)
+    Qo, Do, _ = oracle.run_workload(wls[1])
+    sw = oracle.geometry(wls[1])["sum_w"]
+    assert float(np.max(np.abs(Qb[1].cpu().numpy() - Qo))) <= 1e-5 * sw
+    assert float(np.max(np.abs(Db[1].cpu().numpy() - Do))) <= 1e-4 * float(np.max(np.abs(Do)))
+    for st in stars:
+        soap.soap_destroy(st)
