@@ -92,8 +92,10 @@ enum soap_option {
     SOAP_OPT_FORM = 1,         /* value: enum soap_form; default SOAP_FORM_AUTO */
     SOAP_OPT_QUIET_SPLITS = 2, /* value: >0 forces the number of entry-chunks the quiet sum is split
                                   into across CTAs; 0 (default) = sized from the SM count */
-    SOAP_OPT_KERNEL_TIMING = 3 /* value: 1 brackets the shift-interpolate-accumulate kernel of each call with
+    SOAP_OPT_KERNEL_TIMING = 3, /* value: 1 brackets the shift-interpolate-accumulate kernel of each call with
                                   CUDA events on the caller's stream; soap_get_stats reports the durations */
+    SOAP_OPT_EFFECT_PASSES = 4 /* value: 1 makes soap_active_timeseries_effects / _evolving run one pass per
+                                  requested effect; 0 (default): two or three effects come from one pass */
 };
 
 /* Star / disk description.  HOST, read only during the call. */
@@ -201,8 +203,14 @@ int soap_active_timeseries(soap_star *star, const soap_spectra *quiet, const soa
  *   out_flux [p][m] = sum w_c ( I_ratio lerp(S_quiet[bin_c]) - lerp(S_quiet[bin_c]) ) (negative of Eq. 1)
  *   out_cb   [p][m] = sum w_c (         lerp(S_t[bin_c]) - lerp(S_quiet[bin_c]) )     (negative of Eq. 2)
  * Each output: DEVICE [n_phases][out_pitch] or NULL (that effect is skipped); at least one non-NULL.
- * One shift-interpolate-accumulate launch per requested effect; the active map is built once for total and
- * flux, and once more for CB only when a limb-brightening law differs from 1. */
+ * fp32 spectra, solid-body rotation, two or three outputs requested: ONE active map and ONE
+ * shift-interpolate-accumulate launch (2 launches per call) - the outputs are three weightings of the same
+ * interpolated sums, kept apart per region type: the cost of the total alone when both limb-brightening laws
+ * are 1, and the entries of a type with a law other than 1 are walked twice (weights w and w LB_t).  Results
+ * agree with the pass-per-effect form to rounding (not bit for bit; each form is run-to-run identical).
+ * Otherwise (one output, fp64 spectra, differential rotation, SOAP_OPT_EFFECT_PASSES = 1): one launch per
+ * requested effect; the active map is built once for total and flux, and once more for CB only when a
+ * limb-brightening law differs from 1. */
 int soap_active_timeseries_effects(soap_star *star, const soap_spectra *quiet, const soap_spectra *spot,
                                    const soap_spectra *facula, const soap_region *regions, int32_t n_regions,
                                    const double *phases, int32_t n_phases, void *out_total, void *out_flux,

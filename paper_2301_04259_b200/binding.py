@@ -23,7 +23,7 @@ SOAP_ERR_INVALID_ARG, SOAP_ERR_NOT_READY, SOAP_ERR_CUDA, SOAP_ERR_OOM, SOAP_ERR_
 SOAP_F32, SOAP_F64 = 0, 1
 SOAP_SPOT, SOAP_FACULA = 1, 2
 SOAP_FORM_AUTO, SOAP_FORM_BINNED, SOAP_FORM_CELLS, SOAP_FORM_FIR, SOAP_FORM_COMPOSITE = 0, 1, 2, 3, 4
-SOAP_OPT_FORM, SOAP_OPT_QUIET_SPLITS, SOAP_OPT_KERNEL_TIMING = 1, 2, 3
+SOAP_OPT_FORM, SOAP_OPT_QUIET_SPLITS, SOAP_OPT_KERNEL_TIMING, SOAP_OPT_EFFECT_PASSES = 1, 2, 3, 4
 
 EXPORTED_SYMBOLS = (
     "soap_version", "soap_create", "soap_destroy", "soap_last_error", "soap_set_option", "soap_get_stats",

@@ -11,6 +11,10 @@
 // active launch takes the phases heaviest first by the latter (sia_f32.cuh).
 // One launch, no scratch to zero, no floating-point atomics (every sum has a fixed order).
 // Kinds: 0 = quiet row of a covered cell (weight -w), 1 = spot row, 2 = facula row (weight +w LB_t(mu)).
+// Effects form (the three outputs of Eq. 1-3 from one pass, sia_f32.cuh): the quiet rows are kept per region type -
+// kind 0 = quiet row under a spot, 3 = under a facula - and, for a region type whose limb-brightening law differs from 1
+// (PrepArgs::lb_types), kinds 4, 5 = quiet row with weight +w LB_t(mu) and 6, 7 = spot / facula row with weight +w
+// (flux-only and CB-only use them).
 #pragma once
 #include <cstdint>
 #include <cooperative_groups.h>
@@ -51,12 +55,14 @@ struct ActiveCounters {  // device-resident
 
 struct PrepArgs {
     int N, n_regions, n_mu, seg_cap, chunk_cols, job_cap, n_phases;
+    int n_kinds;              // 3; effects form: 4 (both limb-brightening laws are 1) or 8
+    int lb_types;             // effects form with 8 kinds: bit t = region type t has a limb-brightening law other than 1
     const RegionAtPhase *rp;  // [n_phases][n_regions]
     const double *mu, *w, *col_a;
     const int *bin;
     LbCoef lb;
-    void *ent;                // [n_phases * 3 n_mu][seg_cap] of EntT
-    int *seg_count;           // [n_phases * 3 n_mu]
+    void *ent;                // [n_phases * n_kinds n_mu][seg_cap] of EntT
+    int *seg_count;           // [n_phases * n_kinds n_mu]
     int *n_active;            // [n_phases] covered cells
     ActiveJob *jobs;          // [n_phases][job_cap]
     int *n_jobs, *work;       // [n_phases] each: jobs and entries of the phase (the active launch takes the heaviest first)
@@ -71,16 +77,16 @@ constexpr int kPrepRegSmem = 256;       // regions of a phase held in shared mem
 struct PrepLayout {  // dynamic shared memory of active_prepare_kernel (byte offsets, each a multiple of 16)
     size_t cnt_off, cols_off, reg_off, bytes;
 };
-__host__ __device__ inline PrepLayout prep_layout(int n_mu, int chunk_cols, int N, int n_regions) {
+__host__ __device__ inline PrepLayout prep_layout(int n_mu, int chunk_cols, int N, int n_regions, int n_kinds = 3) {
     PrepLayout l;
-    l.cnt_off = ((size_t)3 * n_mu * chunk_cols * sizeof(double) + 15) & ~(size_t)15;
-    l.cols_off = l.cnt_off + (((size_t)kPrepCluster * 3 * n_mu * sizeof(int) + 15) & ~(size_t)15);
+    l.cnt_off = ((size_t)n_kinds * n_mu * chunk_cols * sizeof(double) + 15) & ~(size_t)15;
+    l.cols_off = l.cnt_off + (((size_t)kPrepCluster * n_kinds * n_mu * sizeof(int) + 15) & ~(size_t)15);
     l.reg_off = l.cols_off + (((size_t)N * sizeof(int) + 15) & ~(size_t)15);
     l.bytes = l.reg_off + (size_t)(n_regions <= kPrepRegSmem ? n_regions : 0) * sizeof(RegionAtPhase) + 16;
     return l;
 }
-__host__ __device__ inline size_t prep_smem_bytes(int n_mu, int chunk_cols, int N, int n_regions) {
-    return prep_layout(n_mu, chunk_cols, N, n_regions).bytes;
+__host__ __device__ inline size_t prep_smem_bytes(int n_mu, int chunk_cols, int N, int n_regions, int n_kinds = 3) {
+    return prep_layout(n_mu, chunk_cols, N, n_regions, n_kinds).bytes;
 }
 
 
@@ -180,8 +186,8 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
     }
     __syncthreads();
     const PrepArgs &a = s_args;
-    const int n_seg = 3 * a.n_mu, N = a.N, cc = a.chunk_cols;
-    const PrepLayout lay = prep_layout(a.n_mu, cc, N, a.n_regions);
+    const int n_seg = a.n_kinds * a.n_mu, N = a.N, cc = a.chunk_cols;
+    const PrepLayout lay = prep_layout(a.n_mu, cc, N, a.n_regions, a.n_kinds);
     double *WDs = reinterpret_cast<double *>(prep_smem);                  // [n_seg][cc]: this CTA's columns
     int *cnt_all = reinterpret_cast<int *>(prep_smem + lay.cnt_off);      // [kPrepCluster][n_seg] entries of every CTA (pushed)
     int *s_cols = reinterpret_cast<int *>(prep_smem + lay.cols_off);      // [N] reachable columns, ascending
@@ -299,8 +305,13 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
                 while (tails) {
                     const int l = __ffs(tails) - 1;
                     if (lane == l) {
-                        col[(size_t)(0 * a.n_mu + b) * cc] += seg_w;
+                        const int kq = (a.n_kinds > 3 && t == 2) ? 3 : 0;  // effects form: quiet rows per region type
+                        col[(size_t)(kq * a.n_mu + b) * cc] += seg_w;
                         col[(size_t)(t * a.n_mu + b) * cc] += seg_wl;
+                        if (a.n_kinds == 8 && ((a.lb_types >> t) & 1)) {
+                            col[(size_t)((3 + t) * a.n_mu + b) * cc] += seg_wl;
+                            col[(size_t)((5 + t) * a.n_mu + b) * cc] += seg_w;
+                        }
                     }
                     __syncwarp();
                     tails &= tails - 1;
@@ -326,7 +337,8 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
     cluster.sync();  // every count has arrived; nobody touches another CTA's shared memory after this
     // ---- (5) compact: one warp per segment, this CTA's columns in order, behind the lower ranks' entries -------------
     for (int s = warp; s < n_seg; s += n_warps) {
-        const double sign = (s < a.n_mu) ? -1.0 : 1.0;
+        const int sk = s / a.n_mu;
+        const double sign = (sk == 0 || (sk == 3 && a.n_kinds > 3)) ? -1.0 : 1.0;
         const double *src = WDs + (size_t)s * cc;
         int ps = 0;
         for (int r = 0; r < rank; ++r) ps += cnt_all[r * n_seg + s];
@@ -378,7 +390,7 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
         for (int w = 0; w < warp; ++w) k += s_wjobs[w];
         for (int o = 0; o < c; o += kActiveJobCap) {
             ActiveJob jb;
-            jb.begin = (p * n_seg + s) * a.seg_cap + o;  // fits: host checks n_phases * 3 n_mu * seg_cap < 2^31
+            jb.begin = (p * n_seg + s) * a.seg_cap + o;  // fits: host checks n_phases * n_kinds n_mu * seg_cap < 2^31
             jb.count = min(kActiveJobCap, c - o);
             jb.kind = s / a.n_mu;
             jb.row = s - jb.kind * a.n_mu;

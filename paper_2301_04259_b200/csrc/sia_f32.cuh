@@ -41,6 +41,10 @@
 //     counter (active_prepare_kernel builds the per-phase job lists; a CTA's scheduler warp ranks a star's
 //     phases by their entry counts); the post-shift contrast (I_ratio of Eq. 3) of a kind multiplies the
 //     fp32 partial sums of that kind in fp64 when they are folded into the fp64 totals (a6).
+//   * effects launch (EFFECTS): the three outputs of Eq. 1-3 - total, flux only, CB only - from ONE pass over the entries.
+//     They are three weightings of the same interpolated sums: with P the fp32 partial sum of a kind (active.cuh lists the
+//     kinds) and C the contrast of its region type, every output adds (a + b C) P for a pair (a, b) in {0, 1, -1} that
+//     depends on (kind, output) only - Params::eff.  The consumers keep three sets of fp64 totals (208 registers; 2 CTAs per SM).
 #pragma once
 #include <climits>
 #include <cstdint>
@@ -65,6 +69,9 @@ constexpr int kFold = 64;                                   // fp32 -> fp64 fold
 constexpr int kFlip = INT_MIN;                              // run marker: per-pixel path
 constexpr int kCtasPerSm = 3;
 constexpr int kRegsConsumer = 120, kRegsProducer = 40;      // (120 + 40) * 128 = 80 * 256: the launch allocation
+constexpr int kCtasPerSmEffects = 2;                        // effects launch: three sets of fp64 totals per consumer thread
+constexpr int kRegsConsumerEffects = 208;                   // (208 + 40) * 128 <= 128 * 256
+constexpr int kEffKinds = 8;                                // kinds of the effects form (active.cuh)
 static_assert(kConsumerWarps == 4 && kProducerWarps == 4, "setmaxnreg acts on aligned groups of 4 warps");
 
 enum : int { kJobFirst = 1, kJobLast = 2, kJobExit = 4 };
@@ -82,7 +89,8 @@ struct StarBlock {
     long long out_pitch;
     double c0;                 // lambda0 / dlambda
     const float2 *ent;         // raw entries (a_e, W_e)
-    float *out;                // quiet: [n_pix]; active: [n_phases][out_pitch]
+    float *out;                // quiet: [n_pix]; active: [n_phases][out_pitch]; effects launch: the total (nullable)
+    float *out_fc[2];          // effects launch: flux-only and CB-only outputs (nullable)
     // active launch
     const ActiveJob *jobs;     // [n_phases][job_cap]
     const int *n_jobs;         // [n_phases]
@@ -112,7 +120,15 @@ struct Params {
     int *item_counters;        // [2] item hand-out (zero between launches)
     int item_chunk;            // items a CTA takes per hand-out (1 unless the list is very long: a batch of stars)
     int order_phases;          // active launch: take a star's phases heaviest first (0: as given)
+    // effects launch, per kind: bits 0-1 spectrum table (0 quiet, 1 spot, 2 facula), bits 2-3 region type whose contrast C
+    // applies (0: none), then for output o = 0 total, 1 flux only, 2 CB only two bits at 4 + 2 o: the multiplier of the
+    // kind's partial sum - 0: 0, 1: 1, 2: C, 3: 1 - C
+    int eff[kEffKinds];
 };
+enum : int { kMulZero = 0, kMulOne = 1, kMulC = 2, kMulOneMinusC = 3 };
+__host__ __device__ constexpr int eff_code(int table, int ctype, int m_total, int m_flux, int m_cb) {
+    return table | (ctype << 2) | (m_total << 4) | (m_flux << 6) | (m_cb << 8);
+}
 
 // __ldg of a pointer-valued field
 template <typename P>
@@ -141,7 +157,8 @@ struct Desc {  // written by the producer with the rest of the stage
     double c0;
     long long out_lo, out_hi, out_pitch;
     float *out;
-    const float *contrast[2];  // of kinds 1, 2
+    float *out_fc[2];          // effects launch
+    const float *contrast[2];  // of region types 1, 2
 };
 
 struct StageLayout {
@@ -538,8 +555,10 @@ __device__ __forceinline__ void init_source(ActiveSource &src, const Params &p, 
 __device__ __forceinline__ const StarBlock &source_block(const QuietSource &, const Params &p) { return p.one; }
 __device__ __forceinline__ const StarBlock &source_block(const ActiveSource &src, const Params &) { return *src.cache; }
 
-template <bool ACTIVE>
-__global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Params p) {
+template <bool ACTIVE, bool EFFECTS = false>
+__global__ void __launch_bounds__(kThreads, EFFECTS ? kCtasPerSmEffects : kCtasPerSm) sia_f32_kernel(const Params p) {
+    static_assert(ACTIVE || !EFFECTS, "the effects form is an active launch");
+    constexpr int NOUT = EFFECTS ? 3 : 1;
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *bar_tma = reinterpret_cast<uint64_t *>(smem);  // [kStages] TMA landed          (count 1 + tx)
     uint64_t *bar_ready = bar_tma + kStages;                 // [kStages] stage post-processed (count 1)
@@ -606,7 +625,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                     const long long g_lo = s_start < 0 ? 0 : s_start;
                     const long long g_hi = (s_start + span) < row_len ? (s_start + span) : row_len;
                     const uint32_t row_bytes = (uint32_t)((g_hi - g_lo) * (long long)sizeof(float));
-                    const float *src_row = blk.base[jb.kind] + (long long)jb.row * blk.pitch + g_lo;
+                    const float *src_row = blk.base[EFFECTS ? (p.eff[jb.kind] & 3) : jb.kind] + (long long)jb.row * blk.pitch + g_lo;
                     const uint32_t ent_bytes = (uint32_t)(((jb.count + 1) & ~1) * (int)sizeof(float2));
                     fence_proxy_async_smem();
                     mbar_arrive_expect_tx(&bar_tma[st], row_bytes + ent_bytes);
@@ -635,6 +654,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
                 desc->out_hi = blk.out_hi;
                 desc->out_pitch = blk.out_pitch;
                 desc->out = blk.out;
+                if (EFFECTS) {
+                    desc->out_fc[0] = blk.out_fc[0];
+                    desc->out_fc[1] = blk.out_fc[1];
+                }
                 desc->contrast[0] = blk.contrast[1];
                 desc->contrast[1] = blk.contrast[2];
             }
@@ -657,7 +680,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     }
 
     // =================================== consumer warps ===============================================
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsConsumer));
+    if (EFFECTS) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsConsumerEffects));
+    else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsConsumer));
     int H = p.halo, base0 = H + tid;  // halo of the current item's star; smem position of pixel r = 0 at zero shift
     int cmask = 0;                     // bit k: kind k of the current item's star carries a contrast array
     long long out_lo = 0, out_hi = 0;  // of the current item's star
@@ -667,8 +691,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     // pulled out of the sum over entries.  acc1 collects W u, acc2 collects (W a) d; pair k = pixels r = 2k, 2k + 1 (the
     // operands of one packed FMA).  A fold adds acc1 + c acc2 to the fp64 totals.
     float2 acc1[kR / 2], acc2[kR / 2];
-    double tot[kR];
+    double tot[NOUT][kR];
     int cnt = 0, cur_kind = 0;
+    int kcode = 0;  // effects launch: Params::eff of the current kind
     // a6: post-shift contrast (I_ratio of Eq. 3) per output pixel: a fold multiplies the fp32 partial sums of the current
     // kind by the kind's contrast C[m] in fp64 (the product is exact) on their way into the fp64 totals - no per-kind
     // totals are kept.  The contrast values of the current kind are fetched with cp.async while its first jobs run.
@@ -676,15 +701,39 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     bool kind_c = false;     // the current kind carries a contrast array
     const Desc *desc = nullptr;  // descriptor of the current job
     auto fold = [&]() {
-        if (ACTIVE && kind_c) {
+        if (EFFECTS) {
+            // (a + b C) P per output: a, b from the kind's code; C = 1 where the kind carries no contrast array
+            if (kind_c) cp_async_wait_all();
+            double ma[NOUT], mb[NOUT];
+#pragma unroll
+            for (int o = 0; o < NOUT; ++o) {
+                const int c = (kcode >> (4 + 2 * o)) & 3;
+                ma[o] = (c == kMulOne || c == kMulOneMinusC) ? 1.0 : 0.0;
+                mb[o] = c == kMulC ? 1.0 : c == kMulOneMinusC ? -1.0 : 0.0;
+            }
+#pragma unroll
+            for (int k = 0; k < kR / 2; ++k) {
+                const float c0 = cmf + (float)(kConsumers * 2 * k), c1 = cmf + (float)(kConsumers * (2 * k + 1));
+                const double w0 = (kind_c && 2 * k < rmax) ? (double)cst[(2 * k) * kConsumers + tid] : 1.0;
+                const double w1 = (kind_c && 2 * k + 1 < rmax) ? (double)cst[(2 * k + 1) * kConsumers + tid] : 1.0;
+                const double p0 = (double)fmaf(c0, acc2[k].x, acc1[k].x), p1 = (double)fmaf(c1, acc2[k].y, acc1[k].y);
+#pragma unroll
+                for (int o = 0; o < NOUT; ++o) {
+                    tot[o][2 * k] = fma(p0, fma(mb[o], w0, ma[o]), tot[o][2 * k]);
+                    tot[o][2 * k + 1] = fma(p1, fma(mb[o], w1, ma[o]), tot[o][2 * k + 1]);
+                }
+                acc1[k] = make_float2(0.f, 0.f);
+                acc2[k] = make_float2(0.f, 0.f);
+            }
+        } else if (ACTIVE && kind_c) {
             cp_async_wait_all();
 #pragma unroll
             for (int k = 0; k < kR / 2; ++k) {
                 const float c0 = cmf + (float)(kConsumers * 2 * k), c1 = cmf + (float)(kConsumers * (2 * k + 1));
                 const double w0 = 2 * k < rmax ? (double)cst[(2 * k) * kConsumers + tid] : 1.0;
                 const double w1 = 2 * k + 1 < rmax ? (double)cst[(2 * k + 1) * kConsumers + tid] : 1.0;
-                tot[2 * k] = fma((double)fmaf(c0, acc2[k].x, acc1[k].x), w0, tot[2 * k]);
-                tot[2 * k + 1] = fma((double)fmaf(c1, acc2[k].y, acc1[k].y), w1, tot[2 * k + 1]);
+                tot[0][2 * k] = fma((double)fmaf(c0, acc2[k].x, acc1[k].x), w0, tot[0][2 * k]);
+                tot[0][2 * k + 1] = fma((double)fmaf(c1, acc2[k].y, acc1[k].y), w1, tot[0][2 * k + 1]);
                 acc1[k] = make_float2(0.f, 0.f);
                 acc2[k] = make_float2(0.f, 0.f);
             }
@@ -692,8 +741,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
 #pragma unroll
             for (int k = 0; k < kR / 2; ++k) {
                 const float c0 = cmf + (float)(kConsumers * 2 * k), c1 = cmf + (float)(kConsumers * (2 * k + 1));
-                tot[2 * k] += (double)fmaf(c0, acc2[k].x, acc1[k].x);
-                tot[2 * k + 1] += (double)fmaf(c1, acc2[k].y, acc1[k].y);
+                tot[0][2 * k] += (double)fmaf(c0, acc2[k].x, acc1[k].x);
+                tot[0][2 * k + 1] += (double)fmaf(c1, acc2[k].y, acc1[k].y);
                 acc1[k] = make_float2(0.f, 0.f);
                 acc2[k] = make_float2(0.f, 0.f);
             }
@@ -702,9 +751,14 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
     };
     auto begin_kind = [&](int kind) {  // after a fold: only this thread ever touches its 16 slots of `cst`
         cur_kind = kind;
-        kind_c = (cmask >> kind) & 1;
+        int ctype = kind;  // region type whose contrast array the kind's partial sums meet
+        if (EFFECTS) {
+            kcode = p.eff[kind];
+            ctype = (kcode >> 2) & 3;
+        }
+        kind_c = (cmask >> ctype) & 1;
         if (!kind_c) return;
-        const float *ck = desc->contrast[kind - 1];
+        const float *ck = desc->contrast[ctype - 1];
 #pragma unroll
         for (int r = 0; r < kR; ++r)
             if (r < rmax) cp_async_4(&cst[r * kConsumers + tid], ck + m_t0 + tid + kConsumers * r);
@@ -734,7 +788,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             cmask = (desc->contrast[0] ? 2 : 0) | (desc->contrast[1] ? 4 : 0);
             cmf = (float)(desc->c0 + (double)(m_t0 + tid));
 #pragma unroll
-            for (int r = 0; r < kR; ++r) tot[r] = 0.0;
+            for (int r = 0; r < kR; ++r)
+#pragma unroll
+                for (int o = 0; o < NOUT; ++o) tot[o][r] = 0.0;
 #pragma unroll
             for (int k = 0; k < kR / 2; ++k) acc1[k] = acc2[k] = make_float2(0.f, 0.f);
             cnt = 0;
@@ -745,7 +801,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             }
         }
         if (ACTIVE && kind != cur_kind) {
-            if (kind_c || ((cmask >> kind) & 1)) fold();  // the multiplier changes: what was summed so far goes to the totals
+            // the multiplier changes: what was summed so far goes to the totals
+            if (EFFECTS || kind_c || ((cmask >> kind) & 1)) fold();
             begin_kind(kind);
         }
         int2 run_next = runs[0];
@@ -799,21 +856,33 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) sia_f32_kernel(const Par
             if (cnt >= kFold) fold();  // at most kFold + one run's entries are ever summed in fp32
         }
         float *o_row = nullptr;  // active launch: this thread's first output pixel (read before the stage is released)
-        if (ACTIVE && (flags & kJobLast)) o_row = desc->out + (long long)out_idx * desc->out_pitch + m_t0 + tid;
+        float *o_fc[2] = {nullptr, nullptr};
+        if (ACTIVE && (flags & kJobLast)) {
+            const long long off = (long long)out_idx * desc->out_pitch + m_t0 + tid;
+            o_row = (EFFECTS && !desc->out) ? nullptr : desc->out + off;
+            if (EFFECTS) {
+                o_fc[0] = desc->out_fc[0] ? desc->out_fc[0] + off : nullptr;
+                o_fc[1] = desc->out_fc[1] ? desc->out_fc[1] + off : nullptr;
+            }
+        }
         __syncwarp();
         if (lane == 0) mbar_arrive(&bar_empty[st]);  // the stage may be refilled while the tile is stored
 
         if (flags & kJobLast) {
             fold();
             if (ACTIVE) {
-                float *o = o_row;
 #pragma unroll
-                for (int r = 0; r < kR; ++r)
-                    if (r < rmax && m_t0 + tid + kConsumers * r >= out_lo) o[kConsumers * r] = (float)tot[r];
+                for (int oi = 0; oi < NOUT; ++oi) {
+                    float *o = oi == 0 ? o_row : o_fc[oi - 1];
+                    if (EFFECTS && !o) continue;
+#pragma unroll
+                    for (int r = 0; r < kR; ++r)
+                        if (r < rmax && m_t0 + tid + kConsumers * r >= out_lo) o[kConsumers * r] = (float)tot[oi][r];
+                }
             } else {
                 double *o = p.partial + ((long long)blockIdx.x * p.max_seg + out_idx) * kTile;
 #pragma unroll
-                for (int r = 0; r < kR; ++r) o[tid + kConsumers * r] = tot[r];
+                for (int r = 0; r < kR; ++r) o[tid + kConsumers * r] = tot[0][r];
                 // a6: the last CTA to deliver its share of this tile adds all shares in CTA order (the same
                 // order whoever comes last: deterministic) and rounds once to fp32.
                 const long long tile = m_t0 / kTile;

@@ -67,6 +67,7 @@ struct soap_star {
     int form = SOAP_FORM_AUTO, form_used = SOAP_FORM_BINNED;
     long long out_lo_override = -1, out_hi_override = -1;  // soap_synthesize_host: pixels of a window that are stored
     long long clip_override = 0;    // soap_synthesize_host: readable row length of a window into a wider table (0 = pitch)
+    int lists_kinds = 3;            // kinds of the entry lists the last active map wrote (effect_kinds)
     bool reuse_lists = false;       // soap_synthesize_host: the active map of the previous call is still valid
     bool regions_uploaded = false;  // soap_synthesize_host: the region centres are already on the device
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
@@ -75,6 +76,7 @@ struct soap_star {
     bool cell_entries = false;  // one entry per cell (SOAP_FORM_CELLS, or differential rotation) instead of per (column, mu-bin)
     int opt_quiet_splits = 0;
     bool opt_timing = false;
+    bool opt_effect_passes = false;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};  // quiet start/stop, active start/stop
     bool ev_valid[2] = {false, false};
 
@@ -122,8 +124,9 @@ struct soap_star {
     int h_call_next = 0;
     size_t call_rp_off = 0, call_prep_off = 0, call_blk_off = 0, call_ph_off = 0;  // sections of d_call of the last prepared call
     bool attr_active_set = false, attr_prep_set = false, attr_prep_inl_set = false, attr_geom_set = false, attr_rv_set = false;
-    int occ_active = 0;
-    size_t occ_active_smem = 0;
+    int occ_active = 0, occ_effects = 0;
+    size_t occ_active_smem = 0, occ_effects_smem = 0;
+    bool attr_effects_set = false;
 
     // host-buffer staging (soap_synthesize_host)
     DevBuf<unsigned char> d_stage[3], d_stage_c[3], d_out_q, d_out_d;
@@ -460,9 +463,9 @@ int quiet_impl(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) 
     return SOAP_OK;
 }
 
-inline int per_cell_cap(const soap_star *s, int n_mu, int ncap) {  // jobs one phase's list can hold
+inline int per_cell_cap(const soap_star *s, int n_mu, int ncap, int n_kinds = 3) {  // jobs one phase's list can hold
     if (s->prm.diff_rot != 0.0) return 3 * n_mu + (int)(s->active_pool_cap / kActiveJobCap) + 2;
-    return 3 * n_mu * ((ncap + kActiveJobCap - 1) / kActiveJobCap);
+    return n_kinds * n_mu * ((ncap + kActiveJobCap - 1) / kActiveJobCap);
 }
 
 // Localize (readings S11-S13): region centres in the observer frame for every phase, written to
@@ -503,7 +506,15 @@ struct ActiveCall {  // one star's arguments
     const double *radii;  // nullable
     void *out;
     long long out_pitch;
+    void *out_flux, *out_cb;  // kEffectAll only (each nullable, like out)
 };
+constexpr int kEffectAll = 3;  // internal: total, flux only and CB only from one pass (sia_f32.cuh, effects launch)
+
+inline bool lb_is_one(const soap_spectra *t) { return !t || (t->lb_c0 == 1.0 && t->lb_c1 == 0.0 && t->lb_c2 == 0.0); }
+// kinds of the entry lists (active.cuh): 3; effects form 4, or 8 when a limb-brightening law differs from 1
+inline int effect_kinds(int effect, const soap_spectra *spot, const soap_spectra *fac) {
+    return effect != kEffectAll ? 3 : (lb_is_one(spot) && lb_is_one(fac)) ? 4 : 8;
+}
 
 inline size_t align16(size_t v) { return (v + 15) & ~(size_t)15; }
 
@@ -516,6 +527,9 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
     soap_star *own = calls[0].s;
     const bool use_lb = effect != SOAP_EFFECT_CB, use_contrast = effect != SOAP_EFFECT_CB;
     const bool quiet_rows = effect == SOAP_EFFECT_FLUX;
+    const bool all_effects = effect == kEffectAll;
+    if (all_effects && n != 1) return own->fail(SOAP_ERR_UNSUPPORTED, "the one-pass effects form takes one star per launch");
+    const int n_kinds = effect_kinds(effect, calls[0].spot, calls[0].fac);
     // ---- per-star scratch, totals --------------------------------------------------------------------------------------
     size_t n_rp = 0;
     long long total_phases = 0, n_items = 0;
@@ -526,8 +540,8 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         soap_star *s = c.s;
         const int N = s->prm.grid_n, n_mu = s->prm.n_mu;
         const int ncap = ((N + 1) & ~1) + 2;
-        const long long n_seg = (long long)c.n_phases * 3 * n_mu;
-        if (n_seg * ncap >= (1LL << 31)) return s->fail(SOAP_ERR_UNSUPPORTED, "n_phases * 3 * n_mu * N too large for one call");
+        const long long n_seg = (long long)c.n_phases * n_kinds * n_mu;
+        if (n_seg * ncap >= (1LL << 31)) return s->fail(SOAP_ERR_UNSUPPORTED, "n_phases * %d * n_mu * N too large for one call", n_kinds);
         SOAP_CUDA(s, s->d_aent.reserve((size_t)n_seg * ncap * sizeof(float2) + 64));
         SOAP_CUDA(s, s->d_segcnt.reserve((size_t)n_seg));
         SOAP_CUDA(s, s->d_nactive.reserve((size_t)c.n_phases));
@@ -535,12 +549,12 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
             SOAP_CUDA(s, s->d_counters.reserve(1));
             SOAP_CUDA(s, cudaMemsetAsync(s->d_counters.ptr, 0, sizeof(ActiveCounters), st));  // once per handle
         }
-        SOAP_CUDA(s, s->d_jobs.reserve((size_t)c.n_phases * per_cell_cap(s, n_mu, ncap)));
+        SOAP_CUDA(s, s->d_jobs.reserve((size_t)c.n_phases * per_cell_cap(s, n_mu, ncap, n_kinds)));
         SOAP_CUDA(s, s->d_sched.reserve((size_t)2 * c.n_phases));
         const int chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);
-        if (prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions) > 200 * 1024)
+        if (prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions, n_kinds) > 200 * 1024)
             return s->fail(SOAP_ERR_UNSUPPORTED, "grid_n %d with %d mu bins exceeds the active-map kernel's shared memory", N, n_mu);
-        prep_smem = std::max(prep_smem, prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions));
+        prep_smem = std::max(prep_smem, prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions, n_kinds));
         s->last_n_phases = c.n_phases;
         n_rp += (size_t)c.n_regions * c.n_phases;
         total_phases += c.n_phases;
@@ -551,6 +565,7 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         return own->fail(SOAP_ERR_UNSUPPORTED, "too many phases / (phase, tile) items for one launch");
     const size_t smem = f32::smem_bytes(max_halo, true);
     if (smem > 227 * 1024) return own->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", max_halo, smem);
+    own->lists_kinds = n_kinds;
 
     // ---- staging: [region centres][map arguments][star blocks][first phase of every star] -------------------------------
     size_t rp_off = 0, prep_off = 0, blk_off = 0, ph_off = 0, total = 0;
@@ -617,7 +632,7 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         soap_star *s = c.s;
         const int N = s->prm.grid_n, n_mu = s->prm.n_mu;
         const int ncap = ((N + 1) & ~1) + 2;
-        const int job_cap = per_cell_cap(s, n_mu, ncap);
+        const int job_cap = per_cell_cap(s, n_mu, ncap, n_kinds);
         int *d_njobs = s->d_sched.ptr, *d_work = d_njobs + c.n_phases;
         if (prepare) {
             RegionAtPhase *rp = reinterpret_cast<RegionAtPhase *>(h + rp_off) + rp_pos;
@@ -629,6 +644,8 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
             a.seg_cap = ncap;
             a.job_cap = job_cap;
             a.n_phases = c.n_phases;
+            a.n_kinds = n_kinds;
+            a.lb_types = (lb_is_one(c.spot) ? 0 : 2) | (lb_is_one(c.fac) ? 0 : 4);
             a.chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);  // columns a CTA of the cluster may own
             a.rp = reinterpret_cast<const RegionAtPhase *>(d + rp_off) + rp_pos;
             a.mu = s->d_mu.ptr;
@@ -673,6 +690,10 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         b.job_cap = job_cap;
         b.n_phases = c.n_phases;
         b.out = static_cast<float *>(c.out);
+        if (all_effects) {
+            b.out_fc[0] = static_cast<float *>(c.out_flux);
+            b.out_fc[1] = static_cast<float *>(c.out_cb);
+        }
         b.out_pitch = c.out_pitch;
         b.item0 = item0;
         hb[k] = b;
@@ -727,6 +748,60 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
     f32::set_layout(p);
     p.collapse = own->form_used == SOAP_FORM_FIR ? 1 : 0;
     p.item_counters = reinterpret_cast<int *>(&own->d_counters.ptr->item_next);
+    if (all_effects) {
+        using f32::eff_code;
+        using f32::sia_f32_kernel;
+        using f32::kMulZero; using f32::kMulOne; using f32::kMulC; using f32::kMulOneMinusC;
+        // the multipliers of every kind's partial sum P (sia_f32.cuh, Params::eff); quiet-row kinds carry the weight -w
+        if (n_kinds == 4) {  // LB = 1: total = sum C A_t - Q, flux = sum (C - 1) Q_t, CB = sum A_t - Q
+            p.eff[0] = eff_code(0, 1, kMulOne, kMulOneMinusC, kMulOne);
+            p.eff[1] = eff_code(1, 1, kMulC, kMulZero, kMulOne);
+            p.eff[2] = eff_code(2, 2, kMulC, kMulZero, kMulOne);
+            p.eff[3] = eff_code(0, 2, kMulOne, kMulOneMinusC, kMulOne);
+        } else {
+            // a type with a limb-brightening law: its quiet rows weighted w LB (kinds 4, 5) serve flux only, its own rows
+            // weighted w (kinds 6, 7) CB only; a type without one keeps the two-kind form above (its kinds 4-7 stay empty)
+            const soap_spectra *tab[3] = {nullptr, calls[0].spot, calls[0].fac};
+            for (int t = 1; t <= 2; ++t) {
+                const int kq = t == 1 ? 0 : 3;
+                if (lb_is_one(tab[t])) {
+                    p.eff[kq] = eff_code(0, t, kMulOne, kMulOneMinusC, kMulOne);
+                    p.eff[t] = eff_code(t, t, kMulC, kMulZero, kMulOne);
+                } else {
+                    p.eff[kq] = eff_code(0, 0, kMulOne, kMulOne, kMulOne);
+                    p.eff[t] = eff_code(t, t, kMulC, kMulZero, kMulZero);
+                }
+                p.eff[3 + t] = eff_code(0, t, kMulZero, kMulC, kMulZero);
+                p.eff[5 + t] = eff_code(t, 0, kMulZero, kMulZero, kMulOne);
+            }
+        }
+        if (!own->attr_effects_set) {
+            SOAP_CUDA(own, (cudaFuncSetAttribute(sia_f32_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)));
+            own->attr_effects_set = true;
+        }
+        if (own->occ_effects_smem != smem) {
+            int occ = 0;
+            SOAP_CUDA(own, (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sia_f32_kernel<true, true>, f32::kThreads, smem)));
+            if (occ < 1) return own->fail(SOAP_ERR_UNSUPPORTED, "active kernel does not fit on an SM (halo %d)", max_halo);
+            own->occ_effects = occ;
+            own->occ_effects_smem = smem;
+        }
+        const long long G = std::max(1LL, std::min((long long)own->n_sm * own->occ_effects, n_items));
+        p.item_chunk = 1;
+        p.order_phases = n_items > 2 * G ? 1 : 0;
+        if (own->opt_timing) {
+            for (int k = 2; k < 4; ++k)
+                if (!own->ev[k]) SOAP_CUDA(own, cudaEventCreate(&own->ev[k]));
+            SOAP_CUDA(own, cudaEventRecord(own->ev[2], st));
+        }
+        SOAP_CUDA(own, launch_pdl(sia_f32_kernel<true, true>, dim3((unsigned)G), dim3(f32::kThreads), smem, st, p));
+        SOAP_LAUNCH_CHECK(own, "sia_f32_kernel<effects>");
+        if (own->opt_timing) {
+            SOAP_CUDA(own, cudaEventRecord(own->ev[3], st));
+            own->ev_valid[1] = true;
+        }
+        return SOAP_OK;
+    }
     if (!own->attr_active_set) {
         SOAP_CUDA(own, cudaFuncSetAttribute(f32::sia_f32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         own->attr_active_set = true;
@@ -795,6 +870,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         a.N = N;
         a.n_regions = n_regions;
         a.n_mu = n_mu;
+        a.n_kinds = 3;
         a.seg_cap = (int)cell_seg_cap;
         a.n_phases = n_phases;
         a.pool_cap = (int)pool;
@@ -831,6 +907,7 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         a.N = N;
         a.n_regions = n_regions;
         a.n_mu = n_mu;
+        a.n_kinds = 3;
         a.seg_cap = ncap;
         a.job_cap = job_cap;
         a.n_phases = n_phases;
@@ -1186,6 +1263,9 @@ int soap_set_option(soap_star *s, int32_t option, int64_t value) {
             s->opt_timing = value != 0;
             s->ev_valid[0] = s->ev_valid[1] = false;
             return SOAP_OK;
+        case SOAP_OPT_EFFECT_PASSES:
+            s->opt_effect_passes = value != 0;
+            return SOAP_OK;
         default:
             return s->fail(SOAP_ERR_INVALID_ARG, "unknown option %d", option);
     }
@@ -1440,15 +1520,32 @@ int soap_active_timeseries_evolving(soap_star *s, const soap_spectra *quiet, con
     if (!one_launch_path && !s->reuse_lists && !s->regions_uploaded &&
         (rc = upload_region_centres(s, regions, n_regions, phases, n_phases, radii, st)))
         return rc;
+    // Two or three outputs of a solid-body fp32 star: ONE map and ONE shift-interpolate-accumulate pass (effects launch,
+    // sia_f32.cuh) unless SOAP_OPT_EFFECT_PASSES asks for a pass per effect or the wider map does not fit in shared memory.
+    const int n_out = (out_total ? 1 : 0) + (out_flux ? 1 : 0) + (out_cb ? 1 : 0);
+    if (one_launch_path && n_out >= 2 && !s->reuse_lists && !s->opt_effect_passes) {
+        const int N = s->prm.grid_n, kinds = effect_kinds(kEffectAll, spot, facula);
+        if (prep_smem_bytes(s->prm.n_mu, std::max(32, (N + kPrepCluster - 1) / kPrepCluster), N, n_regions, kinds) <= 200 * 1024) {
+            ActiveCall c{s, quiet, spot, facula, regions, n_regions, phases, n_phases, radii, out_total, out_pitch, out_flux, out_cb};
+            if ((rc = active_f32_launch(&c, 1, kEffectAll, true, false, st))) return rc;
+            if (n_active) {
+                SOAP_CUDA(s, cudaMemcpyAsync(n_active, s->d_nactive.ptr, (size_t)n_phases * sizeof(int), cudaMemcpyDeviceToHost, st));
+                SOAP_CUDA(s, cudaStreamSynchronize(st));
+                long long tot = 0;
+                for (int p = 0; p < n_phases; ++p) tot += n_active[p];
+                s->last_active_cells = tot;
+            }
+            return SOAP_OK;
+        }
+    }
     // total and flux-only share the entry lists (weights w LB_t(mu)); CB-only needs the plain weights w, which
     // are the same lists again when both limb-brightening laws are identically 1
-    const bool lb_is_one = (!spot || (spot->lb_c0 == 1.0 && spot->lb_c1 == 0.0 && spot->lb_c2 == 0.0)) &&
-                           (!facula || (facula->lb_c0 == 1.0 && facula->lb_c1 == 0.0 && facula->lb_c2 == 0.0));
+    const bool lb_one = lb_is_one(spot) && lb_is_one(facula);
     struct Pass { int effect; void *out; } passes[3] = {{SOAP_EFFECT_TOTAL, out_total}, {SOAP_EFFECT_FLUX, out_flux}, {SOAP_EFFECT_CB, out_cb}};
     bool have_lb_lists = s->reuse_lists;
     for (const Pass &ps : passes) {
         if (!ps.out) continue;
-        const bool prepare = ps.effect == SOAP_EFFECT_CB ? !(have_lb_lists && lb_is_one) : !have_lb_lists;
+        const bool prepare = ps.effect == SOAP_EFFECT_CB ? !(have_lb_lists && lb_one) : !have_lb_lists;
         if (one_launch_path) {
             ActiveCall c{s, quiet, spot, facula, regions, n_regions, phases, n_phases, radii, ps.out, out_pitch};
             rc = active_f32_launch(&c, 1, ps.effect, prepare, false, st);

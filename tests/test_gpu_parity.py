@@ -382,9 +382,12 @@ def test_argument_errors_leave_outputs_untouched(soap):
 
 
 # ---- flux-only and CB-only outputs beside the total (Eq. 1-3) -------------------
-def _run_effects(soap, wl, which=(True, True, True)):
+def _run_effects(soap, wl, which=(True, True, True), passes=False):
+    """`passes`: one shift-interpolate-accumulate pass per requested effect instead of one pass for all of them."""
     dev = torch.device("cuda:0")
     star = soap.soap_create(0)
+    if passes:
+        soap.soap_set_option(star, soap.binding.SOAP_OPT_EFFECT_PASSES, 1)
     soap.soap_disk_geometry(star, wl)
     q = soap.to_device_spectra(wl.quiet, wl.lambda0, wl.dlambda, dev)
     s = None if wl.spot is None else soap.to_device_spectra(wl.spot, wl.lambda0, wl.dlambda, dev, wl.spot_contrast, wl.spot_lb)
@@ -430,17 +433,49 @@ def test_effects_match_oracle_fp64_config1(soap):
 
 
 def test_effects_subsets_and_total_is_unchanged(soap):
-    """Any subset of the outputs may be requested; the total equals soap_active_timeseries bit for bit."""
+    """Any subset of the outputs may be requested; with one pass per effect the total equals soap_active_timeseries bit
+    for bit, and a single requested effect is that same pass."""
     wl = workloads.make_config2(n_pix=4000, n_phases=5, grid_n=100)
     wl.phases = np.linspace(0.4, 0.6, 5)
     g = run_gpu(soap, wl)
-    (t, f, c), na = _run_effects(soap, wl)
+    (t, f, c), na = _run_effects(soap, wl, passes=True)
     assert np.array_equal(t, g["D"]) and np.array_equal(na, g["n_active"])
     (t2, f2, c2), _ = _run_effects(soap, wl, which=(False, True, False))
     assert t2 is None and c2 is None and np.array_equal(f2, f)
     (t3, f3, c3), _ = _run_effects(soap, wl, which=(False, False, True))
     assert np.array_equal(c3, c)
     _check_effects(wl, (t, f, c), na)
+
+
+def _two_type_workload(lb):
+    """A spot and a facula that overlap (columns and mu bins that hold cells of both types), second facula apart."""
+    wl = workloads.make_config3(n_pix=5000, n_phases=5, grid_n=120, nested=True)
+    wl.phases = np.array([0.42, 0.5, 0.58, 0.75, 0.0])
+    wl.regions = list(wl.regions) + [(-20.0, 200.0, 0.12, 1)]
+    wl.facula_contrast = (1.0 + 0.05 * np.sin(np.arange(wl.n_pix) / 50.0)).astype(np.float32)
+    wl.spot_lb = (0.9, 0.1, 0.0) if lb == "both" else (1.0, 0.0, 0.0)
+    wl.facula_lb = (1.1, -0.1, 0.0) if lb != "one" else (1.0, 0.0, 0.0)
+    return wl
+
+
+@pytest.mark.parametrize("lb", ["one", "facula", "both"])
+def test_effects_one_pass_against_oracle_and_against_a_pass_per_effect(soap, lb):
+    """Two or three requested effects come from ONE pass (entry lists of 4 kinds when both limb-brightening laws are 1;
+    a type with a law gets two more): each against the oracle, and against the pass-per-effect form to a tenth of the
+    parity tolerance."""
+    wl = _two_type_workload(lb)
+    assert {r[3] for r in wl.regions} == {1, 2}, "the workload must hold both region types"
+    one, na = _run_effects(soap, wl)
+    per, na2 = _run_effects(soap, wl, passes=True)
+    assert np.array_equal(na, na2) and na.max() > 0
+    _check_effects(wl, one, na)
+    for a, b in zip(one, per):
+        assert np.max(np.abs(a.astype(np.float64) - b)) <= 0.1 * DELTA_TOL * np.max(np.abs(b))
+    # two of the three: the same pass with one output left out
+    (t, f, c), _ = _run_effects(soap, wl, which=(True, False, True))
+    assert f is None and np.array_equal(t, one[0]) and np.array_equal(c, one[2])
+    (t, f, c), _ = _run_effects(soap, wl, which=(False, True, True))
+    assert t is None and np.array_equal(f, one[1]) and np.array_equal(c, one[2])
 
 
 def test_effects_config3_full_size_sampled(soap):
