@@ -563,6 +563,28 @@ def run_graft(args):
                "traffic": traffic.get("line_rv_kernel")}
     line_rv["frac"] = line_rv["achieved"] / line_rv["peak"]
 
+    # ---- total, flux-only and CB-only delta spectra (Eq. 1-3): one pass for the three against the total alone and against
+    # a pass per effect (SOAP_OPT_EFFECT_PASSES); the workload's facula has a limb-brightening law, so its entries are walked twice
+    def effects_leg():
+        outs = [torch.empty((n_ph, P), dtype=torch.float32, device=dev) for _ in range(3)]
+
+        def alone():
+            soap.soap_active_timeseries(star, q, s, f, wl.regions, wl.phases, outs[0])
+
+        def three():
+            soap.soap_active_timeseries_effects(star, q, s, f, wl.regions, wl.phases, outs[0], outs[1], outs[2])
+
+        t_alone = float(np.mean(timer.steps(alone, 5)))
+        t_one = float(np.mean(timer.steps(three, 5)))
+        soap.soap_set_option(star, soap.binding.SOAP_OPT_EFFECT_PASSES, 1)
+        t_per = float(np.mean(timer.steps(three, 5)))
+        soap.soap_set_option(star, soap.binding.SOAP_OPT_EFFECT_PASSES, 0)
+        return {"total_alone_ms": t_alone, "three_effects_one_pass_ms": t_one, "three_effects_pass_per_effect_ms": t_per,
+                "one_pass_over_total_alone": t_one / t_alone, "limb_brightening_laws": {"spot": list(wl.spot_lb), "facula": list(wl.facula_lb)},
+                "note": "active map + shift-interpolate-accumulate launch(es) of soap_active_timeseries[_effects], L2 flushed between calls"}
+
+    effects = effects_leg()
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ------------
     pitch = q.pitch
 
@@ -623,7 +645,7 @@ def run_graft(args):
         "executed_lerp_accumulates_per_s": world * exec_units / (ms_per_step * 1e-3),
         "definitional": {"n_visible": n_vis, "active_cells_all_phases": act_cells, "quiet_entries": main_form["quiet_entries"],
                          "active_entries_all_phases": main_form["active_entries"], "columns": wl.grid_n},
-        "roofline": roofline, "forms": forms, "fir_form": fir, "lower_resolution": lsf, "line_rvs": line_rv,
+        "roofline": roofline, "forms": forms, "fir_form": fir, "lower_resolution": lsf, "line_rvs": line_rv, "effects": effects,
         "configs": configs, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "spectra/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms / e2e_steps, "api": "soap_synthesize_host (pinned host buffers)",
