@@ -293,7 +293,7 @@ __host__ __device__ constexpr size_t lsf_p_smem_bytes() {
 }
 
 template <int J4>
-__global__ void __launch_bounds__(kLsfThreads, 2) lower_resolution_p_kernel(const LsfArgs a) {
+__global__ void __launch_bounds__(kLsfThreads, 3) lower_resolution_p_kernel(const LsfArgs a) {
     static_assert(J4 % 2 == 0, "the window starts on an even pixel");
     extern __shared__ __align__(16) unsigned char lsf_smem[];
     float2 *s = reinterpret_cast<float2 *>(lsf_smem);  // [kLsfStagesP][span] of (row a, row b)
@@ -408,14 +408,19 @@ __global__ void __launch_bounds__(kLsfThreads, 2) lower_resolution_p_kernel(cons
             win[2 * u] = make_float2(t.x, t.y);
             win[2 * u + 1] = make_float2(t.z, t.w);
         }
-        float2 acc[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        // two partial sums per pixel (odd and even taps): four independent FFMA2 chains per thread.  From the centre outwards,
+        // so that the window's registers are released as the taps are used (77 registers: 3 CTAs per SM).
+        float2 acc[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)}, acb[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll
-        for (int j = J4; j >= 1; --j) {  // small outer taps first
+        for (int j = 1; j <= J4; ++j) {
 #pragma unroll
-            for (int p = 0; p < 2; ++p) acc[p] = fma2(bcast2(wr[j][p]), add2(win[J4 + p - j], win[J4 + p + j]), acc[p]);
+            for (int p = 0; p < 2; ++p) {
+                float2 &t = (j & 1) ? acb[p] : acc[p];
+                t = fma2(bcast2(wr[j][p]), add2(win[J4 + p - j], win[J4 + p + j]), t);
+            }
         }
 #pragma unroll
-        for (int p = 0; p < 2; ++p) acc[p] = fma2(bcast2(wr[0][p]), win[J4 + p], acc[p]);
+        for (int p = 0; p < 2; ++p) acc[p] = add2(fma2(bcast2(wr[0][p]), win[J4 + p], acc[p]), acb[p]);
         const long long m = tile * kLsfTileP + 2 * tid;
         const long long ra = 2LL * cc.rp;
         float *oa = out + ra * a.out_pitch + m;
