@@ -19,6 +19,7 @@ namespace soap {
 
 constexpr int kLsfThreads = 256;
 constexpr int kLsfMaxJ = 96;      // taps on each side the kernel supports (host checks)
+constexpr int kLsfBreaks = 16;
 constexpr double kLsfNsig = 5.0;  // truncation in sigmas (reading R-LSF); the oracle uses the same constant
 
 struct LsfArgs {
@@ -27,6 +28,12 @@ struct LsfArgs {
     long long n_rows, n_pix, in_pitch, out_pitch;
     double lambda0, k, R, fwhm_to_sigma;
     int J_max;  // J of the last pixel (sigma grows with lambda): halo of every tile
+    // lower_resolution_p_kernel: the half-width J(m) = ceil(5 sigma_m / k) is a non-decreasing step function of the pixel;
+    // the host evaluates the defining expression (the same IEEE operations) at the steps only:
+    // J(m) = jm0 + #{b : jm_break[b] <= m}; at most kLsfBreaks steps, as the kernel serves J <= 16.
+    int jm0, n_breaks;
+    long long jm_break[kLsfBreaks];
+    double h_scale;  // (k R / fwhm_to_sigma)^2 / 2: k^2 / (2 sigma_m^2) = h_scale / lambda_m^2
 };
 
 __host__ __device__ inline size_t lsf_smem_bytes(int J_max, size_t elem) {
@@ -350,16 +357,28 @@ __global__ void __launch_bounds__(kLsfThreads, 3) lower_resolution_p_kernel(cons
         }
         cp_async_commit();  // one group per item, empty or not: the wait below counts groups
     };
-    auto weights = [&](long long tile) {  // exact per-pixel weights of this thread's 2 pixels (see the kernels above)
+    // Per-pixel weights of this thread's 2 pixels, once per tile (13 row pairs share them), in fp64: g_j = exp(-h j^2) by the
+    // recurrence of the kernels above.  What differs: J(m) comes from the host's step table; h = h_scale / lambda^2 with one
+    // reciprocal; the second pixel's exp(-h) is the first's times exp(h - h') by its Taylor series (h - h' ~ 4e-6 h: the
+    // cubic term is below 1e-17); 1 / norm by one Newton step from the fp32 reciprocal.  All within a few ulp of fp64:
+    // the taps are rounded to fp32 afterwards.
+    auto weights = [&](long long tile) {
+        const long long m0 = tile * kLsfTileP + 2 * tid;
+        int jb = a.jm0, b0 = 0;
+        for (; b0 < a.n_breaks && a.jm_break[b0] <= tile * kLsfTileP; ++b0) ++jb;
+        const double lam0 = __dadd_rn(a.lambda0, __dmul_rn(a.k, (double)m0));
+        const double inv_lam = 1.0 / lam0;
+        const double h0 = a.h_scale * inv_lam * inv_lam;
+        const double eps = a.k * inv_lam;
+        const double dh = h0 * eps * (2.0 - 3.0 * eps);  // h(m0) - h(m0 + 1)
+        const double e0 = exp(-h0);
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
-            const long long m = tile * kLsfTileP + 2 * tid + p;
-            const double lam = __dadd_rn(a.lambda0, __dmul_rn(a.k, (double)m));
-            const double sigma = __dmul_rn(__ddiv_rn(lam, a.R), a.fwhm_to_sigma);
-            int Jm = (int)ceil(__ddiv_rn(__dmul_rn(kLsfNsig, sigma), a.k));
+            const long long m = m0 + p;
+            int Jm = jb;
+            for (int b = b0; b < a.n_breaks && a.jm_break[b] <= m; ++b) ++Jm;
             Jm = min(Jm, J4);
-            const double h = (a.k * a.k) / (2.0 * sigma * sigma);
-            const double rho0 = exp(-h), q = rho0 * rho0;
+            const double rho0 = p == 0 ? e0 : e0 * (1.0 + dh * (1.0 + 0.5 * dh)), q = rho0 * rho0;
             double rho = rho0, g = 1.0, norm = 1.0;
             wr[0][p] = 1.f;
 #pragma unroll
@@ -370,7 +389,9 @@ __global__ void __launch_bounds__(kLsfThreads, 3) lower_resolution_p_kernel(cons
                 wr[j][p] = inw ? (float)g : 0.f;
                 norm += inw ? 2.0 * g : 0.0;
             }
-            const float inv = (float)(1.0 / norm);
+            double r = (double)(1.f / (float)norm);
+            r = r * (2.0 - norm * r);  // relative error (2^-23)^2
+            const float inv = (float)r;
 #pragma unroll
             for (int j = 0; j <= J4; ++j) wr[j][p] *= inv;
         }

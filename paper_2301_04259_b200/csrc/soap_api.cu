@@ -1614,6 +1614,33 @@ int soap_lower_resolution(soap_star *s, const void *in, int64_t n_rows, int64_t 
     if (j_last > (double)kLsfMaxJ)
         return s->fail(SOAP_ERR_UNSUPPORTED, "line-spread function of %.0f pixels half-width exceeds %d", j_last, kLsfMaxJ);
     a.J_max = (int)j_last;
+    {
+        // the steps of J(m) = ceil(5 sigma_m / k) (non-decreasing: every operation is monotone), by bisection on the defining
+        // expression - the operations, and so the results, of the kernels' per-pixel evaluation
+        auto jm = [&](long long m) {
+            volatile double t = dlambda * (double)m;  // (no contraction into an FMA)
+            const double lam = lambda0 + t;
+            volatile double sg = lam / resolution;
+            volatile double sigma = sg * a.fwhm_to_sigma;
+            volatile double five = kLsfNsig * sigma;
+            return (int)std::ceil(five / dlambda);
+        };
+        a.jm0 = jm(0);
+        a.n_breaks = 0;
+        const int j_end = jm(n_pix - 1);
+        // (the table serves the row-pair kernel, J <= 16: at most 16 steps; wider functions never read it)
+        for (int J = a.jm0 + 1; J <= j_end && a.n_breaks < kLsfBreaks; ++J) {
+            long long lo = 0, hi = n_pix - 1;  // jm(lo) < J <= jm(hi)
+            while (hi - lo > 1) {
+                const long long mid = lo + (hi - lo) / 2;
+                if (jm(mid) >= J) hi = mid;
+                else lo = mid;
+            }
+            a.jm_break[a.n_breaks++] = hi;
+        }
+        const double kr = dlambda * resolution / a.fwhm_to_sigma;
+        a.h_scale = 0.5 * kr * kr;
+    }
     const size_t elem = dtype == SOAP_F64 ? 8 : 4;
     const size_t smem = lsf_smem_bytes(a.J_max, elem);
     const unsigned tiles = (unsigned)((n_pix + kLsfThreads - 1) / kLsfThreads);
