@@ -143,3 +143,21 @@ def test_step_captured_in_a_cuda_graph_replays_bit_identically(soap):
     soap.soap_destroy(star)
     g = dict(Q=Q0.cpu().numpy(), D=D0.cpu().numpy(), n_active=oracle.run_workload(wl)[2])
     assert_parity(wl, g, check_rv=False)
+
+
+def test_effects_in_one_pass_without_regions_and_with_hidden_regions(soap):
+    """The three-output launch with an empty region list, and with phases at which every region is on the far side:
+    exact zeros in all three outputs (S19), counts of zero."""
+    from test_gpu_parity import _run_effects
+    wl = workloads.make_config3(n_pix=4500, n_phases=3, grid_n=60)
+    wl.phases = np.array([0.0, 0.5, 0.98])
+    wl.regions = []
+    outs, na = _run_effects(soap, wl)
+    assert list(na) == [0, 0, 0]
+    for o in outs:
+        assert o.shape == (3, 4500) and np.all(o == 0.0)
+    wl.regions = [(10.0, 180.0, 0.15, 1), (-5.0, 170.0, 0.2, 2)]
+    outs, na = _run_effects(soap, wl)
+    assert na[0] == 0 and na[1] > 0
+    for o in outs:
+        assert np.all(o[0] == 0.0) and np.any(o[1] != 0.0)

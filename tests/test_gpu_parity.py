@@ -382,12 +382,14 @@ def test_argument_errors_leave_outputs_untouched(soap):
 
 
 # ---- flux-only and CB-only outputs beside the total (Eq. 1-3) -------------------
-def _run_effects(soap, wl, which=(True, True, True), passes=False):
+def _run_effects(soap, wl, which=(True, True, True), passes=False, form=None):
     """`passes`: one shift-interpolate-accumulate pass per requested effect instead of one pass for all of them."""
     dev = torch.device("cuda:0")
     star = soap.soap_create(0)
     if passes:
         soap.soap_set_option(star, soap.binding.SOAP_OPT_EFFECT_PASSES, 1)
+    if form is not None:
+        soap.soap_set_option(star, soap.binding.SOAP_OPT_FORM, form)
     soap.soap_disk_geometry(star, wl)
     q = soap.to_device_spectra(wl.quiet, wl.lambda0, wl.dlambda, dev)
     s = None if wl.spot is None else soap.to_device_spectra(wl.spot, wl.lambda0, wl.dlambda, dev, wl.spot_contrast, wl.spot_lb)
@@ -483,6 +485,15 @@ def test_effects_config3_full_size_sampled(soap):
     outs, na = _run_effects(soap, wl)
     for lo, hi in _sample_ranges(wl.n_pix, n=2):
         _check_effects(wl, outs, na, lo, hi)
+
+
+@pytest.mark.parametrize("form", [1, 3], ids=["binned", "fir"])
+def test_effects_one_pass_in_the_binned_and_the_run_collapsed_form(soap, form):
+    """The one-pass effects launch under SOAP_FORM_BINNED / SOAP_FORM_FIR (the active launch collapses runs of entries)."""
+    wl = _two_type_workload("facula")
+    wl.vsini_kms = 9.0
+    outs, na = _run_effects(soap, wl, form=form)
+    _check_effects(wl, outs, na)
 
 
 def test_fir_form_config3_full_size_sampled(soap):
