@@ -473,6 +473,8 @@ def test_effects_one_pass_against_oracle_and_against_a_pass_per_effect(soap, lb)
     _check_effects(wl, one, na)
     for a, b in zip(one, per):
         assert np.max(np.abs(a.astype(np.float64) - b)) <= 0.1 * DELTA_TOL * np.max(np.abs(b))
+    again, _ = _run_effects(soap, wl)
+    assert all(np.array_equal(a, b) for a, b in zip(one, again)), "the one-pass launch is run-to-run identical"
     # two of the three: the same pass with one output left out
     (t, f, c), _ = _run_effects(soap, wl, which=(True, False, True))
     assert f is None and np.array_equal(t, one[0]) and np.array_equal(c, one[2])
