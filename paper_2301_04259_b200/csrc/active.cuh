@@ -44,7 +44,7 @@ struct ActiveJob {  // one job of a phase's list: <= kActiveJobCap consecutive e
 };
 constexpr int kActiveJobCap = 128;      // == f32::kJobCap
 constexpr int kPrepCluster = 8;         // CTAs per phase (portable cluster size)
-constexpr int kPrepThreads = 512;       // 16 warps per CTA
+constexpr int kPrepThreads = 512;       // 16 warps per CTA (active_prepare_kernel: THREADS, see below)
 constexpr int kPrepChunks = 4;          // 32-row chunks of a column whose cell data is loaded together
 
 struct ActiveCounters {  // device-resident
@@ -127,7 +127,7 @@ __device__ __forceinline__ int column_candidates(const RegionAtPhase *reg, int n
     return fits ? n : -1;
 }
 
-// grid = n_phases * kPrepCluster, block = kPrepThreads, cluster = kPrepCluster CTAs;
+// grid = n_phases * kPrepCluster, block = THREADS, cluster = kPrepCluster CTAs;
 // dynamic shared memory = prep_smem_bytes(n_mu, chunk_cols, n_regions) with chunk_cols >= ceil(N / kPrepCluster).
 // Batch form (soap_batch_active_timeseries): `many` = DEVICE [n_stars] arguments, `phase0` = DEVICE [n_stars + 1] first
 // cluster (phase) of every star; cluster c serves phase c - phase0[s] of the star s that holds it.  many == nullptr: `one`.
@@ -139,6 +139,9 @@ __device__ __forceinline__ int column_candidates(const RegionAtPhase *reg, int n
 // memory, one cluster barrier; (5) compaction behind the lower ranks' entries; rank 0 writes the job list (parallel
 // scan over the segments).  No CTA waits for another phase: the order in which the shift-interpolate-accumulate launch
 // takes the phases (heaviest first) is derived there from work[] (sia_f32.cuh).
+// THREADS: 512 when all the clusters of the launch are resident at once (the launch is then as long as its slowest cluster:
+// the more warps share a phase's columns the better); 256 beyond that - half of the warps of a cluster wait at its barriers
+// at any time (load imbalance between columns), and twice the clusters per SM fill the idle issue slots (C4: 99 -> 67 us).
 // `inl` (K > 0): the region centres of a single star's call travel as a kernel argument - [n_phases][n_regions], at most K -
 // so that the call needs no host -> device copy at all; K == 0: they are read from a.rp.
 template <int K>
@@ -147,8 +150,8 @@ struct InlineRegions {
 };
 constexpr int kInlineRegions = 192;  // 9 KB of kernel arguments
 
-template <typename EntT, int K>
-__global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(kPrepThreads)
+template <typename EntT, int K, int THREADS>
+__global__ void __cluster_dims__(kPrepCluster, 1, 1) __launch_bounds__(THREADS)
 active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, const int *__restrict__ phase0, int n_stars,
                       const __grid_constant__ InlineRegions<K> inl) {
     namespace cg = cooperative_groups;
@@ -156,11 +159,11 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
     extern __shared__ __align__(16) unsigned char prep_smem[];
     __shared__ PrepArgs s_args;
     __shared__ int s_phase;
-    __shared__ int s_cand[kPrepThreads / 32][kCandCap];  // per warp: regions that can reach its column
+    __shared__ int s_cand[THREADS / 32][kCandCap];  // per warp: regions that can reach its column
     __shared__ int s_misc[4];                            // reachable columns, covered cells of this CTA
     __shared__ int s_cov[kPrepCluster];                  // rank 0: covered cells of every CTA (pushed)
-    __shared__ int s_wsum[kPrepThreads / 32 + 1], s_wjobs[kPrepThreads / 32 + 1];
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = kPrepThreads / 32;
+    __shared__ int s_wsum[THREADS / 32 + 1], s_wjobs[THREADS / 32 + 1];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, n_warps = THREADS / 32;
     // every CTA of the cluster must be running before its shared memory is written remotely: arrive now, wait in (4)
     asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
     // (launched with programmatic stream serialization: the geometry this kernel reads is complete after the wait)
@@ -202,13 +205,13 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
     {
         const uint4 *src = reinterpret_cast<const uint4 *>(greg);
         uint4 *dst = reinterpret_cast<uint4 *>(s_reg);
-        for (int k = tid; k < n_reg_sm * (int)(sizeof(RegionAtPhase) / 16); k += kPrepThreads) dst[k] = K > 0 ? src[k] : __ldg(&src[k]);
-        for (int k = tid; k < n_seg * cc; k += kPrepThreads) WDs[k] = 0.0;
+        for (int k = tid; k < n_reg_sm * (int)(sizeof(RegionAtPhase) / 16); k += THREADS) dst[k] = K > 0 ? src[k] : __ldg(&src[k]);
+        for (int k = tid; k < n_seg * cc; k += THREADS) WDs[k] = 0.0;
     }
     __syncthreads();
     const RegionAtPhase *reg = n_reg_sm ? s_reg : greg;
     // ---- (2) the columns some region of this phase can reach (conservative: chord bound, slightly inflated) -------------
-    for (int j0 = 0; j0 < N; j0 += kPrepThreads) {
+    for (int j0 = 0; j0 < N; j0 += THREADS) {
         const int j = j0 + tid;
         bool hit = false;
         if (j < N) {
@@ -238,7 +241,7 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
         // No region of this phase faces the observer (every CTA of the cluster sees the same list): an empty phase.
         // Rank 0 records it; nothing is binned, exchanged or compacted.
         if (rank != 0) return;
-        for (int s = tid; s < n_seg; s += kPrepThreads) a.seg_count[p * n_seg + s] = 0;
+        for (int s = tid; s < n_seg; s += THREADS) a.seg_count[p * n_seg + s] = 0;
         if (tid == 0) {
             a.n_jobs[p] = 0;
             a.work[p] = 0;
@@ -359,7 +362,7 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
     if (rank != 0) return;
     // ---- rank 0 finalises the phase: pad odd segments, counts, job list (kinds 1, 2, then 0).  Thread t takes the t-th
     // segment of the job order; jobs are numbered by a block-wide exclusive scan of the segments' job counts.
-    for (int t0 = 0, jobs_before = 0, work_sum = 0; t0 < n_seg || t0 == 0; t0 += kPrepThreads) {
+    for (int t0 = 0, jobs_before = 0, work_sum = 0; t0 < n_seg || t0 == 0; t0 += THREADS) {
         const int t = t0 + tid;
         int s = 0, c = 0;
         if (t < n_seg) {
@@ -401,7 +404,7 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
             work_sum += s_wsum[w];
         }
         __syncthreads();
-        if (t0 + kPrepThreads >= n_seg && tid == 0) {
+        if (t0 + THREADS >= n_seg && tid == 0) {
             int covered = 0;
             for (int r = 0; r < kPrepCluster; ++r) covered += s_cov[r];
             a.n_jobs[p] = jobs_before;

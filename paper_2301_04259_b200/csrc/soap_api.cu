@@ -123,7 +123,8 @@ struct soap_star {
     } h_call[4];
     int h_call_next = 0;
     size_t call_rp_off = 0, call_prep_off = 0, call_blk_off = 0, call_ph_off = 0;  // sections of d_call of the last prepared call
-    bool attr_active_set = false, attr_prep_set = false, attr_prep_inl_set = false, attr_geom_set = false, attr_rv_set = false;
+    bool attr_active_set = false, attr_geom_set = false, attr_rv_set = false;
+    bool attr_prep_set[4] = {false, false, false, false};  // active_prepare_kernel per (threads, inline regions)
     int occ_active = 0, occ_effects = 0;
     size_t occ_active_smem = 0, occ_effects_smem = 0;
     bool attr_effects_set = false;
@@ -713,28 +714,41 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
     }
 
     if (prepare && total_phases > 0) {
-        // a4: one cluster of CTAs per (star, phase) bins, compacts and schedules (active.cuh)
-        if (!own->attr_prep_set) {
-            SOAP_CUDA(own, (cudaFuncSetAttribute(active_prepare_kernel<float2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)));
-            own->attr_prep_set = true;
-        }
-        if (inline_rp) {
-            if (!own->attr_prep_inl_set) {
-                SOAP_CUDA(own, (cudaFuncSetAttribute(active_prepare_kernel<float2, kInlineRegions>,
-                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)));
-                own->attr_prep_inl_set = true;
+        // a4: one cluster of CTAs per (star, phase) bins, compacts and schedules (active.cuh).  CTAs of 512 threads while
+        // every cluster of the launch is resident at once, smaller ones beyond that (see the kernel's header).
+        const int threads = total_phases * kPrepCluster <= 2LL * own->n_sm ? 512 : 256;
+        const dim3 grid((unsigned)(total_phases * kPrepCluster));
+        auto launch_map = [&](auto tag) -> int {
+            constexpr int T = decltype(tag)::value;
+            const int slot = (T == 512 ? 0 : 1) * 2 + (inline_rp ? 1 : 0);
+            if (inline_rp) {
+                if (!own->attr_prep_set[slot]) {
+                    SOAP_CUDA(own, (cudaFuncSetAttribute(active_prepare_kernel<float2, kInlineRegions, T>,
+                                                         cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)));
+                    own->attr_prep_set[slot] = true;
+                }
+                InlineRegions<kInlineRegions> inl;
+                std::memcpy(inl.r, h + rp_off, n_rp * sizeof(RegionAtPhase));
+                SOAP_CUDA(own, launch_pdl(active_prepare_kernel<float2, kInlineRegions, T>, grid, dim3(T), prep_smem, st, hp[0],
+                                          (const PrepArgs *)nullptr, (const int *)nullptr, 1, inl));
+            } else {
+                if (!own->attr_prep_set[slot]) {
+                    SOAP_CUDA(own, (cudaFuncSetAttribute(active_prepare_kernel<float2, 0, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                         200 * 1024)));
+                    own->attr_prep_set[slot] = true;
+                }
+                PrepArgs none{};
+                InlineRegions<0> no_inl{};
+                SOAP_CUDA(own, launch_pdl(active_prepare_kernel<float2, 0, T>, grid, dim3(T), prep_smem, st, none,
+                                          reinterpret_cast<const PrepArgs *>(d + prep_off), reinterpret_cast<const int *>(d + ph_off), n,
+                                          no_inl));
             }
-            InlineRegions<kInlineRegions> inl;
-            std::memcpy(inl.r, h + rp_off, n_rp * sizeof(RegionAtPhase));
-            SOAP_CUDA(own, launch_pdl(active_prepare_kernel<float2, kInlineRegions>, dim3((unsigned)(total_phases * kPrepCluster)),
-                                      dim3(kPrepThreads), prep_smem, st, hp[0], (const PrepArgs *)nullptr, (const int *)nullptr, 1, inl));
-        } else {
-            PrepArgs none{};
-            InlineRegions<0> no_inl{};
-            SOAP_CUDA(own, launch_pdl(active_prepare_kernel<float2, 0>, dim3((unsigned)(total_phases * kPrepCluster)), dim3(kPrepThreads),
-                                      prep_smem, st, none, reinterpret_cast<const PrepArgs *>(d + prep_off),
-                                      reinterpret_cast<const int *>(d + ph_off), n, no_inl));
-        }
+            return SOAP_OK;
+        };
+        int rcm;
+        if (threads == 512) rcm = launch_map(std::integral_constant<int, 512>{});
+        else rcm = launch_map(std::integral_constant<int, 256>{});
+        if (rcm) return rcm;
         SOAP_LAUNCH_CHECK(own, "active_prepare_kernel");
     }
     if (n_items == 0 || map_only) return SOAP_OK;
@@ -931,9 +945,9 @@ int active_impl(soap_star *s, const soap_spectra *q, const soap_spectra *spot, c
         a.work = d_work;
         a.counters = s->d_counters.ptr;
         const size_t smem = prep_smem_bytes(n_mu, a.chunk_cols, N, n_regions);
-        SOAP_CUDA(s, (cudaFuncSetAttribute(active_prepare_kernel<Ent, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)));
+        SOAP_CUDA(s, (cudaFuncSetAttribute(active_prepare_kernel<Ent, 0, kPrepThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)));
         InlineRegions<0> no_inl{};
-        active_prepare_kernel<Ent, 0><<<n_phases * kPrepCluster, kPrepThreads, smem, st>>>(a, nullptr, nullptr, 1, no_inl);
+        active_prepare_kernel<Ent, 0, kPrepThreads><<<n_phases * kPrepCluster, kPrepThreads, smem, st>>>(a, nullptr, nullptr, 1, no_inl);
         SOAP_LAUNCH_CHECK(s, "active_prepare_kernel");
     }
     if (sizeof(T) == 4) {
