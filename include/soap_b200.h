@@ -181,6 +181,29 @@ int soap_disk_geometry(soap_star *star, const soap_star_params *params, void *st
  * clamped to the end values outside the grid (S8).  `out`: DEVICE [n_pix] of quiet->dtype. */
 int soap_integrate_quiet(soap_star *star, const soap_spectra *quiet, void *out, void *stream);
 
+/* ---- a3 for callers that must not allocate device memory (Alg. 1) ------------------------
+ * The same sum as soap_integrate_quiet, same arguments, fp32 or fp64 tables, any rotation law - but this call never
+ * allocates or frees device memory, on any call, whatever the sizes.  It is meant for programs in which the library may
+ * not go to the CUDA allocator once they are running: an application that has given the whole device to its own memory
+ * pool, so that a cudaMalloc here would fail; or a service loop that cannot take the device-wide synchronisation a
+ * cudaMalloc / cudaFree brings.  Create the handle and call soap_disk_geometry during set-up (those do allocate); from
+ * then on this entry point only enqueues two kernels on `stream`.
+ *   Scratch: the fp64 partial sums of the entry chunks live in a 4 MiB array that is part of the library image
+ *     (every device that loads the library holds it until the process exits).  The limit that follows:
+ *     round_up4(n_pix) <= 524 288, else SOAP_ERR_UNSUPPORTED with a message naming the limit and nothing is written.
+ *     Within the limit the entry list is cut into fewer chunks when the array cannot hold as many as
+ *     soap_integrate_quiet would take, so long spectra run with less parallelism over entries.
+ *   First call on a device: looks up the array's device address (once per device, with that device current).  Make
+ *     that first call during set-up, before any stream capture is under way in the process.
+ *   Sharing: every call on a device, from every handle, uses the one array.  Each call overwrites what it later reads,
+ *     so nothing left by an earlier call matters; but two calls whose kernels overlap on the GPU (different streams,
+ *     no dependency between them) race on it and give wrong spectra.  Order them on one stream or with events.
+ *   Result: the direct (binned or per-cell) form with fp64 chunk sums added in chunk order; equal to
+ *     soap_integrate_quiet to rounding (bit-identical for fp64 tables when both take the same number of chunks).
+ *   SOAP_OPT_QUIET_SPLITS is honoured up to what the array holds; SOAP_OPT_KERNEL_TIMING and soap_get_stats' quiet
+ *     fields are not updated by this call. */
+int soap_integrate_quiet_static(soap_star *star, const soap_spectra *quiet, void *out, void *stream);
+
 /* ---- a4 + a5 + a6: active-region delta spectra for every phase (Alg. 5, Eq. 3; S11-S19) ----------
  * For phase p: type[c] = type of the LAST region in list order covering visible cell c, and
  *   out_delta[p][m] = sum over covered cells of

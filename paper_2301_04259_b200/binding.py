@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = (
     "soap_disk_geometry", "soap_integrate_quiet", "soap_active_timeseries", "soap_active_timeseries_effects",
     "soap_export_geometry", "soap_lower_resolution", "soap_active_timeseries_evolving", "soap_line_rvs",
     "soap_synthesize_host", "soap_batch_integrate_quiet", "soap_batch_active_timeseries", "soap_contrast_planck",
-    "soap_probe_fp32_rate", "soap_batch_disk_geometry",
+    "soap_probe_fp32_rate", "soap_batch_disk_geometry", "soap_integrate_quiet_static",
 )
 
 
@@ -95,6 +95,7 @@ def load_library() -> ctypes.CDLL:
     lib.soap_get_stats.argtypes = [vp, ctypes.POINTER(c_stats), vp]
     lib.soap_disk_geometry.argtypes = [vp, ctypes.POINTER(c_star_params), vp, ctypes.POINTER(c_geom_info)]
     lib.soap_integrate_quiet.argtypes = [vp, ctypes.POINTER(c_spectra), vp, vp]
+    lib.soap_integrate_quiet_static.argtypes = [vp, ctypes.POINTER(c_spectra), vp, vp]
     lib.soap_active_timeseries.argtypes = [vp, ctypes.POINTER(c_spectra), ctypes.POINTER(c_spectra),
                                            ctypes.POINTER(c_spectra), ctypes.POINTER(c_region), i32,
                                            ctypes.POINTER(ctypes.c_double), i32, vp, i64,
@@ -246,6 +247,13 @@ def soap_disk_geometry(star: Star, params, stream=None, want_info: bool = True) 
 def soap_integrate_quiet(star: Star, quiet: Spectra, out: torch.Tensor, stream=None) -> None:
     cq = quiet._c()
     star._check(star._lib.soap_integrate_quiet(star._h, ctypes.byref(cq), out.data_ptr(), _stream_handle(stream)))
+
+
+def soap_integrate_quiet_static(star: Star, quiet: Spectra, out: torch.Tensor, stream=None) -> None:
+    """soap_integrate_quiet for callers that must not allocate device memory: the partial sums go to a fixed 4 MiB
+    array inside the library (n_pix <= 524 288; calls that overlap on the GPU race on it) - include/soap_b200.h."""
+    cq = quiet._c()
+    star._check(star._lib.soap_integrate_quiet_static(star._h, ctypes.byref(cq), out.data_ptr(), _stream_handle(stream)))
 
 
 def _regions(regions: Sequence):

@@ -6,6 +6,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <type_traits>
 #include <utility>
 #include <new>
@@ -1198,6 +1199,95 @@ int synthesize_host_pipelined(soap_star *s, const soap_star_params *prm, const s
 }
 }  // namespace
 
+// ---- soap_integrate_quiet_static: the quiet spectrum without any device allocation ---------------------------------
+// soap_integrate_quiet keeps its per-chunk fp64 partial sums in a buffer it (re)allocates with cudaMalloc when a call
+// needs more than any call before it.  Some callers cannot afford that: a host application that has handed all of the
+// device's memory to its own pool (cudaMalloc then simply fails), or a loop that must never stall (cudaMalloc and
+// cudaFree synchronise the whole device).  For them the same two kernels (sia.cuh: sia_kernel<T, false>, reduce_partials_kernel<T>) run with their
+// partial sums in the array below instead: fixed size, part of the library image, so every device that loads the library
+// gives up these 4 MiB until the process exits, whether the entry point is ever called or not.
+//
+// Only device code may name the array directly.  In host code `g_static_partial` is a host-side shadow symbol, not a device
+// address: the kernels are given what cudaGetSymbolAddress returns for the device that is current, looked up once per
+// device (static_partial_address).
+constexpr long long kStaticPartialDoubles = 512LL * 1024;  // 4 MiB of fp64 partial sums: n_splits * round_up4(n_pix) <= this
+static __device__ __align__(256) double g_static_partial[kStaticPartialDoubles];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+double *g_static_partial_dev[kStaticMaxDevices] = {};  // device address of g_static_partial on device d (nullptr: not looked up)
+
+// Device address of the static scratch on s->device.  The device must be current.  The first call on a device performs
+// the look-up (which loads the library's module on that device if nothing has yet); later calls read the cached pointer.
+int static_partial_address(soap_star *s, double **out) {
+    if (s->device < 0 || s->device >= kStaticMaxDevices)
+        return s->fail(SOAP_ERR_UNSUPPORTED, "static scratch: device %d is outside 0..%d", s->device, kStaticMaxDevices - 1);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    double *&slot = g_static_partial_dev[s->device];
+    if (!slot) {
+        double *p = nullptr;
+        SOAP_CUDA(s, cudaGetSymbolAddress(reinterpret_cast<void **>(&p), g_static_partial));
+        if (!p) return s->fail(SOAP_ERR_CUDA, "cudaGetSymbolAddress returned a null address for the static scratch");
+        slot = p;
+    }
+    *out = slot;
+    return SOAP_OK;
+}
+
+template <typename T>
+int quiet_static_impl(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
+    constexpr int TP = sia_tile_px<T>();
+    const long long P = q->n_pix;
+    const long long part_pitch = (P + 3) & ~3LL;
+    if (part_pitch > kStaticPartialDoubles)
+        return s->fail(SOAP_ERR_UNSUPPORTED, "soap_integrate_quiet_static: n_pix = %lld exceeds the static scratch (at most %lld pixels); "
+                       "use soap_integrate_quiet", P, kStaticPartialDoubles);
+    const size_t smem = sia_smem_bytes<T>(halo_for(s, q));
+    if (smem > 227 * 1024)
+        return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", halo_for(s, q), smem);
+    double *partial = nullptr;
+    int rc = static_partial_address(s, &partial);
+    if (rc) return rc;
+    const int n_tiles = (int)((P + TP - 1) / TP);
+    // the entry list is cut into as many chunks as soap_integrate_quiet's generic path would take, capped by what the
+    // static array holds
+    int splits = s->opt_quiet_splits;
+    if (splits <= 0) {
+        splits = (int)std::lround((double)(s->n_sm * 8) / n_tiles);
+        const long long max_entries = (long long)s->prm.grid_n * (s->cell_entries ? s->prm.grid_n : s->prm.n_mu);
+        const int cap = (int)std::max(1LL, max_entries / 16);
+        splits = std::max(1, std::min(std::min(splits, 256), cap));
+    }
+    splits = (int)std::max(1LL, std::min<long long>(splits, kStaticPartialDoubles / part_pitch));
+    SiaParams<T> p{};
+    p.base[0] = static_cast<const T *>(q->data);
+    p.pitch = q->pitch;
+    p.n_pix = P;
+    p.c0 = q->lambda0 / q->dlambda;
+    p.n_mu = s->prm.n_mu;
+    p.halo = halo_for(s, q);
+    if (sizeof(T) == 4) p.ent = reinterpret_cast<const typename SiaTraits<T>::Ent *>(s->d_ent32.ptr);
+    else p.ent = reinterpret_cast<const typename SiaTraits<T>::Ent *>(s->d_ent64.ptr);
+    p.row_start = s->d_row_start.ptr;
+    p.n_splits = splits;
+    p.partial = partial;
+    p.part_pitch = part_pitch;
+    if (smem > 48 * 1024)
+        SOAP_CUDA(s, cudaFuncSetAttribute(sia_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // every partial[split][m], m < n_pix, is stored by the first launch before the second reads it: nothing in the array
+    // has to start at zero, and what an earlier call left there is never read
+    sia_kernel<T, false><<<dim3(n_tiles, splits), kThreads, smem, st>>>(p);
+    SOAP_LAUNCH_CHECK(s, "sia_kernel<quiet> (static scratch)");
+    const int threads = 256;
+    const long long quads = (P + 3) / 4;
+    reduce_partials_kernel<T><<<(unsigned)((quads + threads - 1) / threads), threads, 0, st>>>(partial, part_pitch, splits, P,
+                                                                                             static_cast<T *>(out));
+    SOAP_LAUNCH_CHECK(s, "reduce_partials_kernel (static scratch)");
+    return SOAP_OK;
+}
+}  // namespace
+
 extern "C" {
 
 int soap_version(void) { return SOAP_B200_VERSION; }
@@ -1509,6 +1599,17 @@ int soap_integrate_quiet(soap_star *s, const soap_spectra *quiet, void *out, voi
     SOAP_CUDA(s, cudaSetDevice(s->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     return quiet->dtype == SOAP_F32 ? quiet_impl<float>(s, quiet, out, st) : quiet_impl<double>(s, quiet, out, st);
+}
+
+int soap_integrate_quiet_static(soap_star *s, const soap_spectra *quiet, void *out, void *stream) {
+    if (!s) return SOAP_ERR_INVALID_ARG;
+    if (!s->ready) return s->fail(SOAP_ERR_NOT_READY, "soap_disk_geometry has not been called");
+    int rc = check_spectra(s, quiet, "quiet");
+    if (rc) return rc;
+    if (!out) return s->fail(SOAP_ERR_INVALID_ARG, "out is NULL");
+    SOAP_CUDA(s, cudaSetDevice(s->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    return quiet->dtype == SOAP_F32 ? quiet_static_impl<float>(s, quiet, out, st) : quiet_static_impl<double>(s, quiet, out, st);
 }
 
 int soap_active_timeseries_evolving(soap_star *s, const soap_spectra *quiet, const soap_spectra *spot,
