@@ -553,10 +553,12 @@ int active_f32_launch(const ActiveCall *calls, int n, int effect, bool prepare, 
         }
         SOAP_CUDA(s, s->d_jobs.reserve((size_t)c.n_phases * per_cell_cap(s, n_mu, ncap, n_kinds)));
         SOAP_CUDA(s, s->d_sched.reserve((size_t)2 * c.n_phases));
-        const int chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);
-        if (prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions, n_kinds) > 200 * 1024)
-            return s->fail(SOAP_ERR_UNSUPPORTED, "grid_n %d with %d mu bins exceeds the active-map kernel's shared memory", N, n_mu);
-        prep_smem = std::max(prep_smem, prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions, n_kinds));
+        if (!external_map) {  // (an external map was built by active_prepare_cells_kernel, with its own limit: active_impl)
+            const int chunk_cols = std::max(32, (N + kPrepCluster - 1) / kPrepCluster);
+            if (prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions, n_kinds) > 200 * 1024)
+                return s->fail(SOAP_ERR_UNSUPPORTED, "grid_n %d with %d mu bins exceeds the active-map kernel's shared memory", N, n_mu);
+            prep_smem = std::max(prep_smem, prep_smem_bytes(n_mu, chunk_cols, N, c.n_regions, n_kinds));
+        }
         s->last_n_phases = c.n_phases;
         n_rp += (size_t)c.n_regions * c.n_phases;
         total_phases += c.n_phases;
@@ -2062,6 +2064,16 @@ int soap_batch_integrate_quiet(soap_star *const *stars, int32_t n_stars, const s
         one_launch = one_launch && s->device == s0->device && composite_applies(s, quiet[k]) && s->comp_stride == s0->comp_stride;
     }
     SOAP_CUDA(s0, cudaSetDevice(s0->device));
+    // a launch sizes its shared memory for the largest pair table AND the largest halo among its stars: a group that mixes
+    // a fine grid with a fast rotator may not fit although each star does on its own - such a batch takes the per-star lanes
+    for (int k0 = 0; one_launch && k0 < n_stars; k0 += comp::kMaxStars) {
+        int max_pairs = 0, max_halo = 0;
+        for (int k = k0; k < std::min(n_stars, k0 + comp::kMaxStars); ++k) {
+            max_pairs = std::max(max_pairs, (stars[k]->prm.grid_n + 1) / 2);
+            max_halo = std::max(max_halo, halo_for(stars[k], quiet[k]));
+        }
+        one_launch = comp::smem_bytes(s0->comp_stride, max_pairs, max_halo) <= (size_t)200 * 1024 / comp::kCtasPerSm;
+    }
     if (one_launch) {
         // the composite-column kernel walks the flattened (star, tile, column pair) list: ONE launch for the batch
         // (groups of comp::kMaxStars stars when the batch is larger)
