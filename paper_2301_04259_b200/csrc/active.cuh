@@ -175,11 +175,11 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
             int lo = 0, hi = n_stars - 1;  // last star with phase0[s] <= c
             while (lo < hi) {
                 const int mid = (lo + hi + 1) >> 1;
-                if (__ldg(&phase0[mid]) <= c) lo = mid;
+                if (__ldcg(&phase0[mid]) <= c) lo = mid;
                 else hi = mid - 1;
             }
             s_args = many[lo];
-            s_phase = c - __ldg(&phase0[lo]);
+            s_phase = c - __ldcg(&phase0[lo]);
         } else {
             s_args = one;
             s_phase = c;
@@ -205,7 +205,7 @@ active_prepare_kernel(const PrepArgs one, const PrepArgs *__restrict__ many, con
     {
         const uint4 *src = reinterpret_cast<const uint4 *>(greg);
         uint4 *dst = reinterpret_cast<uint4 *>(s_reg);
-        for (int k = tid; k < n_reg_sm * (int)(sizeof(RegionAtPhase) / 16); k += THREADS) dst[k] = K > 0 ? src[k] : __ldg(&src[k]);
+        for (int k = tid; k < n_reg_sm * (int)(sizeof(RegionAtPhase) / 16); k += THREADS) dst[k] = K > 0 ? src[k] : __ldcg(&src[k]);
         for (int k = tid; k < n_seg * cc; k += THREADS) WDs[k] = 0.0;
     }
     __syncthreads();

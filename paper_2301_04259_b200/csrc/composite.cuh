@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) composite_quiet_kernel(c
     // ---- work units of every star: n_tiles x (cost of all its pairs) -------------------------------------------
     for (int s = tid; s < n_stars; s += kThreads) {
         const Star &st = p.many ? p.many[s] : p.one;
-        unit0[s + 1] = (long long)st.n_tiles * (long long)__ldg(&st.hdr[st.n_pairs].cost0);
+        unit0[s + 1] = (long long)st.n_tiles * (long long)__ldcg(&st.hdr[st.n_pairs].cost0);
     }
     __syncthreads();
     if (tid == 0) {
@@ -211,11 +211,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) composite_quiet_kernel(c
             const int np = st.n_pairs;
             const float4 *src = reinterpret_cast<const float4 *>(st.Wp);
             float4 *dst = reinterpret_cast<float4 *>(Wsm);
-            for (int i = tid; i < np * NB / 2; i += kThreads) dst[i] = __ldg(&src[i]);
+            for (int i = tid; i < np * NB / 2; i += kThreads) dst[i] = __ldcg(&src[i]);
             for (int i = tid; i < NB / 2; i += kThreads) dst[np * NB / 2 + i] = make_float4(0.f, 0.f, 0.f, 0.f);  // the pad row
             const int4 *hs = reinterpret_cast<const int4 *>(st.hdr);
             int4 *hd = reinterpret_cast<int4 *>(hsm);
-            for (int i = tid; i <= np; i += kThreads) hd[i] = __ldg(&hs[i]);
+            for (int i = tid; i <= np; i += kThreads) hd[i] = __ldcg(&hs[i]);
             if (tid == 0) hd[np + 1] = make_int4(0, 0, 0, 0);
             cur_s = s;
             __syncthreads();

@@ -553,11 +553,11 @@ geometry_kernel(const GeomArgs one, const GeomArgs *__restrict__ many, const int
             int lo = 0, hi = n_stars - 1;  // last star with cta0[s] <= blockIdx.x
             while (lo < hi) {
                 const int mid = (lo + hi + 1) >> 1;
-                if (__ldg(&cta0[mid]) <= (int)blockIdx.x) lo = mid;
+                if (__ldcg(&cta0[mid]) <= (int)blockIdx.x) lo = mid;
                 else hi = mid - 1;
             }
             star = lo;
-            first = __ldg(&cta0[lo]);
+            first = __ldcg(&cta0[lo]);
         }
         const unsigned long long *src = reinterpret_cast<const unsigned long long *>(many ? many + star : &one);
         unsigned long long *dst = reinterpret_cast<unsigned long long *>(&s_a);

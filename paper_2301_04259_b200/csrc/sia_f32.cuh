@@ -130,10 +130,10 @@ __host__ __device__ constexpr int eff_code(int table, int ctype, int m_total, in
     return table | (ctype << 2) | (m_total << 4) | (m_flux << 6) | (m_cb << 8);
 }
 
-// __ldg of a pointer-valued field
+// __ldcg of a pointer-valued field
 template <typename P>
 __device__ __forceinline__ P *ldg_ptr(P *const *addr) {
-    return reinterpret_cast<P *>(__ldg(reinterpret_cast<const unsigned long long *>(addr)));
+    return reinterpret_cast<P *>(__ldcg(reinterpret_cast<const unsigned long long *>(addr)));
 }
 
 template <bool ACTIVE>
@@ -216,7 +216,7 @@ struct QuietSource {
     bool done;
     __device__ void init(const Params &p, long long cta, long long G) {
         row_start = p.row_start;
-        E = __ldg(&row_start[p.one.n_mu]);
+        E = __ldcg(&row_start[p.one.n_mu]);
         const long long U = E * p.one.n_tiles;
         u0 = range_begin(cta, U, G);
         u1 = range_begin(cta + 1, U, G);
@@ -242,8 +242,8 @@ struct QuietSource {
             }
             open_tile();
         }
-        while (__ldg(&row_start[s + 1]) <= e) ++s;  // rows without entries are skipped
-        const int end = min(min(e + kJobCap, __ldg(&row_start[s + 1])), e_hi);
+        while (__ldcg(&row_start[s + 1]) <= e) ++s;  // rows without entries are skipped
+        const int end = min(min(e + kJobCap, __ldcg(&row_start[s + 1])), e_hi);
         j.tile = t;
         j.star = 0;
         j.kind = 0;
@@ -305,7 +305,7 @@ struct ActiveSource {
     __device__ void load_order(int st) {
         const int lane = threadIdx.x & 31;
         const StarBlock *b = many ? many + st : cache;
-        const int n = many ? __ldg(&b->n_phases) : b->n_phases;
+        const int n = many ? __ldcg(&b->n_phases) : b->n_phases;
         const int *wk = many ? ldg_ptr(&b->work) : b->work, *njp = many ? ldg_ptr(&b->n_jobs) : b->n_jobs;
         ord_star = st;
         ord_identity = n > kOrderCap || !order;
@@ -313,7 +313,7 @@ struct ActiveSource {
         __syncwarp();
         bool wide = false;
         for (int k = lane; k < n; k += 32) {
-            const int nj = __ldg(&njp[k]);
+            const int nj = __ldcg(&njp[k]);
             s_njobs[k] = (unsigned short)nj;
             wide = wide || nj > 0xffff;
         }
@@ -321,12 +321,14 @@ struct ActiveSource {
             ord_identity = true;
             return;
         }
-        for (int ph = lane; ph < n; ph += 32) {  // rank of phase ph = phases that go before it (the list is L1-resident)
-            const int w = __ldg(&wk[ph]);
+        // rank of phase ph = phases that go before it.  The list stays L1-resident: ld.global.ca, which - unlike the read-only
+        // path - is coherent with what the active-map launch wrote once the dependency wait has returned
+        for (int ph = lane; ph < n; ph += 32) {
+            const int w = __ldca(&wk[ph]);
             int rk = 0;
 #pragma unroll 4
             for (int q = 0; q < n; ++q) {
-                const int wq = __ldg(&wk[q]);
+                const int wq = __ldca(&wk[q]);
                 rk += (wq > w || (wq == w && q < ph)) ? 1 : 0;
             }
             s_order[rk] = (unsigned short)ph;
@@ -353,13 +355,13 @@ struct ActiveSource {
                 const bool mine = valid && stx == st;
                 if (mine) {
                     const StarBlock *b = many ? many + st : cache;
-                    const int nt = many ? __ldg(&b->n_tiles) : b->n_tiles;
+                    const int nt = many ? __ldcg(&b->n_tiles) : b->n_tiles;
                     const long long local = idx - prefix[st];
                     const int k = (int)(local / nt);
                     tl = (int)(local - (long long)k * nt);
                     if (ord_identity) {
                         ph = k;
-                        c = __ldg((many ? ldg_ptr(&b->n_jobs) : b->n_jobs) + ph);
+                        c = __ldcg((many ? ldg_ptr(&b->n_jobs) : b->n_jobs) + ph);
                     } else {
                         ph = s_order[k];
                         c = s_njobs[ph];
@@ -415,7 +417,7 @@ struct ActiveSource {
             const int lane = threadIdx.x & 31;
             __syncwarp();
             if (lane < (int)(sizeof(StarBlock) / 16))
-                reinterpret_cast<uint4 *>(cache)[lane] = __ldg(reinterpret_cast<const uint4 *>(many + star) + lane);
+                reinterpret_cast<uint4 *>(cache)[lane] = __ldcg(reinterpret_cast<const uint4 *>(many + star) + lane);
             __syncwarp();
             cached_star = star;
         }
@@ -467,7 +469,7 @@ struct ActiveSource {
             j.kind = j.row = j.begin = j.count = 0;
             j.flags = kJobFirst | kJobLast;
         } else {
-            const int4 a = __ldg(reinterpret_cast<const int4 *>(cache->jobs + (size_t)phase * cache->job_cap + k));
+            const int4 a = __ldca(reinterpret_cast<const int4 *>(cache->jobs + (size_t)phase * cache->job_cap + k));
             j.begin = a.x;
             j.count = a.y;
             j.kind = a.z;
@@ -584,7 +586,7 @@ __global__ void __launch_bounds__(kThreads, EFFECTS ? kCtasPerSmEffects : kCtasP
     grid_dependency_wait();
     if (ACTIVE) {
         for (int k = tid; k <= p.n_stars; k += kThreads)
-            prefix[k] = k < p.n_stars ? (p.many ? __ldg(&p.many[k].item0) : 0LL) : p.n_items;
+            prefix[k] = k < p.n_stars ? (p.many ? __ldcg(&p.many[k].item0) : 0LL) : p.n_items;
     }
     __syncthreads();
 
@@ -886,7 +888,7 @@ __global__ void __launch_bounds__(kThreads, EFFECTS ? kCtasPerSmEffects : kCtasP
                 // a6: the last CTA to deliver its share of this tile adds all shares in CTA order (the same
                 // order whoever comes last: deterministic) and rounds once to fp32.
                 const long long tile = m_t0 / kTile;
-                const long long E = __ldg(&p.row_start[p.one.n_mu]), U = E * p.one.n_tiles, G = gridDim.x;
+                const long long E = __ldcg(&p.row_start[p.one.n_mu]), U = E * p.one.n_tiles, G = gridDim.x;
                 const long long ub = tile * E, ue = ub + E;
                 __threadfence();
                 consumer_bar_sync();
