@@ -62,20 +62,22 @@ def kernel_source_sha() -> str:
 
 def ncu_dram_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-    (profiles/r02_dram_traffic.csv: kernel, bytes read, bytes written, source hash).  A row counts only if it was
+    (profiles/rNN_dram_traffic.csv of the newest round: kernel, bytes read, bytes written, source hash).  A row counts only if it was
     captured from the sources this run was built from; otherwise the figure is stale and `traffic` is null."""
-    path = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")
+    cands = sorted(f for f in os.listdir(os.path.join(ROOT, "profiles")) if f.endswith("_dram_traffic.csv"))
     out = {}
-    if not os.path.exists(path):
-        return out, "profiles/r02_dram_traffic.csv missing: null"
+    if not cands:
+        return out, "profiles/*_dram_traffic.csv missing: null"
+    name = cands[-1]  # the newest round's
+    path = os.path.join(ROOT, "profiles", name)
     sha = kernel_source_sha()
     with open(path) as fh:
         for row in csv.DictReader(fh):
             if row["source_sha"] == sha:
                 out[row["kernel"]] = float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
     if out:
-        return out, f"profiles/r02_dram_traffic.csv, captured from the sources of this build ({sha})"
-    return out, f"profiles/r02_dram_traffic.csv is of other sources than this build ({sha}): null"
+        return out, f"profiles/{name}, captured from the sources of this build ({sha})"
+    return out, f"profiles/{name} is of other sources than this build ({sha}): null"
 
 
 class ClockSampler:
@@ -460,7 +462,8 @@ def run_graft(args):
         sys.stderr.write(f"cuda graph leg skipped: {exc}\n")
 
     # ---- the device's FP32 FMA rate, measured live with the inner loops' instruction forms ----------------
-    probe = {"ffma2_fma_per_s": soap.soap_probe_fp32_rate(star, True), "ffma_fma_per_s": soap.soap_probe_fp32_rate(star, False),
+    from paper_2301_04259_b200 import benchlib  # libsoap_b200_bench.so: the probe is not part of the product library
+    probe = {"ffma2_fma_per_s": benchlib.fp32_rate(local_rank, True), "ffma_fma_per_s": benchlib.fp32_rate(local_rank, False),
              "derived_fma_per_s": peak_instr}
     probe["ffma2_over_derived"] = probe["ffma2_fma_per_s"] / peak_instr
     probe["ffma_over_derived"] = probe["ffma_fma_per_s"] / peak_instr
@@ -512,6 +515,17 @@ def run_graft(args):
     }
     if clocks.get("sm_mhz"):
         roofline["frac_at_observed_clock"] = roofline["frac"] * peaks["sm_max_mhz"] / clocks["sm_mhz"]
+    # the same figures as flat scalars (a record that keeps scalar fields only still carries them).  The roofline fraction of
+    # the whole step counts the lane instructions of the forms that RAN; `whole_step_binned_equivalent` credits the composite
+    # quiet launch with the binned form's 2 FMA per (entry, pixel), work it avoids: a throughput in binned units, not a
+    # fraction of the roofline
+    roofline.update({
+        "quiet_kernel": kq_name, "quiet_kernel_ms": kern[kq_name]["ms"], "quiet_frac": tflops(kq_name) / peak_tflops,
+        "active_kernel_ms": kern["sia_f32_kernel<active>"]["ms"], "active_frac": tflops("sia_f32_kernel<active>") / peak_tflops,
+        "whole_step_frac_executed": roofline["whole_step"]["frac"],
+        "whole_step_binned_equivalent": roofline["whole_step"]["frac_at_4_flop_per_binned_unit"],
+        "ffma2_probe_frac": probe["ffma2_over_derived"], "ffma_probe_frac": probe["ffma_over_derived"],
+    })
 
     # ---- the run-collapsed form against the memory roofline it moves the path to --------------
     fir = forms.get("fir")
@@ -656,6 +670,21 @@ def run_graft(args):
         "gpu_launches": launches, "wall_s_timed_region": wall,
         "cuda_graph": {"ms_per_step": graph_ms, "note": "the timed step captured once and replayed (4 kernel nodes with programmatic edges)"},
     }
+    line["e2e"]["tables_resident_ms"] = res_ms
+    line["e2e"]["tables_resident_value"] = world * n_spec / (res_ms * 1e-3)
+    flat = {"cuda_graph_ms": graph_ms, "lsf_ms": lsf["ms"], "lsf_hbm_frac": lsf["frac"], "rv_ms": line_rv["ms"], "rv_hbm_frac": line_rv["frac"],
+            "effects_one_pass_ratio": effects["one_pass_over_total_alone"], "effects_one_pass_ms": effects["three_effects_one_pass_ms"]}
+    if fir is not None:
+        flat.update({"fir_step_ms": fir["ms_per_step"], "fir_quiet_ms": fir["quiet_kernel_ms"], "fir_active_ms": fir["active_kernel_ms"],
+                     "fir_quiet_hbm_frac": fir["roofline"]["quiet"]["frac"], "fir_active_hbm_frac": fir["roofline"]["active"]["frac"]})
+    if "binned" in forms:
+        flat.update({"binned_step_ms": forms["binned"]["ms_per_step"], "binned_quiet_ms": forms["binned"]["quiet_kernel_ms"],
+                     "binned_quiet_frac": forms["binned"]["quiet_alu_frac"], "binned_active_frac": forms["binned"]["active_alu_frac"]})
+    for name, c in configs.items():
+        k_ = name.lower()
+        flat.update({f"{k_}_ms": c.get("ms_per_step"), f"{k_}_quiet_alu_frac": c.get("quiet_alu_frac"),
+                     f"{k_}_active_alu_frac": c.get("active_alu_frac")})
+    line.update(flat)
     if world == 1 and not args.no_cpu_baseline:
         t_full, threads = oracle_full(wl)
         t_c2, n_c2 = oracle_single_thread_c2()

@@ -282,13 +282,6 @@ int soap_line_rvs(soap_star *star, const void *rows, int64_t n_rows, int64_t n_p
                   double lambda0, double dlambda, const double *centres, const double *half_widths, int64_t n_lines,
                   const double *norm, int64_t edge, double *out_rv, void *stream);
 
-/* ---- measurement aid: the device's FP32 FMA rate (not part of the path) ------------------------------------------
- * Runs a register-only kernel of independent FMA chains (8 CTAs of 256 threads per SM, 16 accumulators per thread) and
- * returns the best of four timed repetitions in FMAs per second.  packed != 0: fma.rn.f32x2 with a scalar-broadcast
- * operand (SASS FFMA2) - the form of the shift-interpolate-accumulate inner loops; 0: plain FFMA.  bench.py reports it
- * beside the derived peak (SMs x 128 lanes x clock) its `"bound": "alu"` roofline divides by.  Synchronous. */
-int soap_probe_fp32_rate(soap_star *star, int32_t packed, double *fma_per_s, void *stream);
-
 /* ---- debug export of the geometry (HOST outputs, N*N each, any may be NULL; synchronous) --------
  * Hidden cells: mu = 0, vel = 0, w = 0, bin = -1. */
 int soap_export_geometry(soap_star *star, double *mu, double *vel, double *w, int32_t *bin);

@@ -11,6 +11,5 @@ from .binding import (  # noqa: F401
     soap_disk_geometry, soap_integrate_quiet, soap_integrate_quiet_static, soap_active_timeseries, soap_active_timeseries_effects,
     soap_export_geometry, soap_lower_resolution, soap_active_timeseries_evolving, soap_line_rvs,
     soap_synthesize_host, soap_batch_disk_geometry, soap_batch_integrate_quiet, soap_batch_active_timeseries, soap_contrast_planck,
-    soap_probe_fp32_rate,
     to_device_spectra,
 )

@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = (
     "soap_disk_geometry", "soap_integrate_quiet", "soap_active_timeseries", "soap_active_timeseries_effects",
     "soap_export_geometry", "soap_lower_resolution", "soap_active_timeseries_evolving", "soap_line_rvs",
     "soap_synthesize_host", "soap_batch_integrate_quiet", "soap_batch_active_timeseries", "soap_contrast_planck",
-    "soap_probe_fp32_rate", "soap_batch_disk_geometry", "soap_integrate_quiet_static",
+    "soap_batch_disk_geometry", "soap_integrate_quiet_static",
 )
 
 
@@ -105,7 +105,6 @@ def load_library() -> ctypes.CDLL:
                                                    ctypes.POINTER(ctypes.c_double), i32, vp, vp, vp, i64,
                                                    ctypes.POINTER(i32), vp]
     lib.soap_export_geometry.argtypes = [vp, vp, vp, vp, vp]
-    lib.soap_probe_fp32_rate.argtypes = [vp, i32, ctypes.POINTER(ctypes.c_double), vp]
     lib.soap_contrast_planck.argtypes = [vp, ctypes.c_double, ctypes.c_double, i64, ctypes.c_double, ctypes.c_double, vp, i32, vp]
     lib.soap_line_rvs.argtypes = [vp, vp, i64, i64, i64, i32, ctypes.c_double, ctypes.c_double, vp, vp, i64, vp, i64, vp, vp]
     lib.soap_active_timeseries_evolving.argtypes = [vp, ctypes.POINTER(c_spectra), ctypes.POINTER(c_spectra),
@@ -330,13 +329,6 @@ def soap_active_timeseries_evolving(star: Star, quiet: Spectra, spot: Optional[S
         out_cb.data_ptr() if out_cb is not None else None, out_pitch,
         na.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)) if na is not None else None, _stream_handle(stream)))
     return na[:n_ph] if na is not None else None
-
-
-def soap_probe_fp32_rate(star: Star, packed: bool = True, stream=None) -> float:
-    """FP32 FMAs per second of a register-only FMA kernel on the star's device (measurement aid of bench.py)."""
-    out = ctypes.c_double(0.0)
-    star._check(star._lib.soap_probe_fp32_rate(star._h, 1 if packed else 0, ctypes.byref(out), _stream_handle(stream)))
-    return float(out.value)
 
 
 def soap_contrast_planck(star: Star, lambda0: float, dlambda: float, n_pix: int, t_quiet: float, t_active: float,

@@ -21,7 +21,6 @@
 #include "contrast.cuh"
 #include "geometry.cuh"
 #include "lsf.cuh"
-#include "probe.cuh"
 #include "rv.cuh"
 #include "sia.cuh"
 #include "sia_f32.cuh"
@@ -229,8 +228,11 @@ template <typename T, bool ACTIVE>
 int launch_sia(soap_star *s, const SiaParams<T> &p, dim3 grid, cudaStream_t st) {
     const size_t smem = sia_smem_bytes<T>(p.halo);
     if (smem > 227 * 1024) return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", p.halo, smem);
-    if (smem > 48 * 1024)
-        SOAP_CUDA(s, cudaFuncSetAttribute(sia_kernel<T, ACTIVE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    static bool attr_set[64] = {};  // once per device and instantiation: the limit, not the launch's size (that is checked above)
+    if (!attr_set[s->device & 63]) {
+        SOAP_CUDA(s, cudaFuncSetAttribute(sia_kernel<T, ACTIVE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_set[s->device & 63] = true;
+    }
     const int e0 = ACTIVE ? 2 : 0;
     if (s->opt_timing) {
         for (int k = e0; k < e0 + 2; ++k)
@@ -246,12 +248,24 @@ int launch_sia(soap_star *s, const SiaParams<T> &p, dim3 grid, cudaStream_t st) 
     return SOAP_OK;
 }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize of f32::sia_f32_kernel<ACTIVE>, set once per device to the limit every launch
+// is checked against (the attribute is a ceiling: occupancy follows the launch's own size)
+template <bool ACTIVE>
+int sia_f32_attr(soap_star *s) {
+    static bool attr_set[64] = {};
+    if (!attr_set[s->device & 63]) {
+        SOAP_CUDA(s, cudaFuncSetAttribute(f32::sia_f32_kernel<ACTIVE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_set[s->device & 63] = true;
+    }
+    return SOAP_OK;
+}
+
 // fp32 spectra: warp-specialised kernel of sia_f32.cuh.  `which`: 0 = quiet, 1 = active (event slots).
 template <bool ACTIVE>
 int launch_sia_f32(soap_star *s, const f32::Params &p, dim3 grid, cudaStream_t st) {
     const size_t smem = f32::smem_bytes(p.halo, ACTIVE);
     if (smem > 227 * 1024) return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", p.halo, smem);
-    SOAP_CUDA(s, cudaFuncSetAttribute(f32::sia_f32_kernel<ACTIVE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (int rc = sia_f32_attr<ACTIVE>(s)) return rc;
     const int e0 = ACTIVE ? 2 : 0;
     if (s->opt_timing) {
         for (int k = e0; k < e0 + 2; ++k)
@@ -290,7 +304,7 @@ int quiet_f32(soap_star *s, const soap_spectra *q, void *out, cudaStream_t st) {
     // one CTA per resident slot (a single wave); fewer when there is too little work to share out
     const size_t smem = f32::smem_bytes(p.halo, false);
     if (smem > 227 * 1024) return s->fail(SOAP_ERR_UNSUPPORTED, "shift of %d pixels needs %zu B of shared memory", p.halo, smem);
-    SOAP_CUDA(s, cudaFuncSetAttribute(f32::sia_f32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (int rc = sia_f32_attr<false>(s)) return rc;
     int occ = 0;
     SOAP_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f32::sia_f32_kernel<false>, f32::kThreads, smem));
     if (occ < 1) return s->fail(SOAP_ERR_UNSUPPORTED, "quiet kernel does not fit on an SM (halo %d)", p.halo);
@@ -1877,36 +1891,6 @@ int soap_contrast_planck(soap_star *s, double lambda0, double dlambda, int64_t n
     else
         contrast_planck_kernel<double><<<grid, 256, 0, st>>>(lambda0, dlambda, n_pix, 1.0 / t_quiet, 1.0 / t_active, static_cast<double *>(out));
     SOAP_LAUNCH_CHECK(s, "contrast_planck_kernel");
-    return SOAP_OK;
-}
-
-int soap_probe_fp32_rate(soap_star *s, int32_t packed, double *fma_per_s, void *stream) {
-    if (!s) return SOAP_ERR_INVALID_ARG;
-    if (!fma_per_s) return s->fail(SOAP_ERR_INVALID_ARG, "fma_per_s is NULL");
-    SOAP_CUDA(s, cudaSetDevice(s->device));
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    SOAP_CUDA(s, s->d_info.reserve(1));
-    float *sink = reinterpret_cast<float *>(s->d_info.ptr);  // never written (see the kernel); any valid address will do
-    cudaEvent_t e0, e1;
-    SOAP_CUDA(s, cudaEventCreate(&e0));
-    SOAP_CUDA(s, cudaEventCreate(&e1));
-    const int iters = 4096, grid = s->n_sm * 8;  // 8 CTAs of 256 threads per SM: 64 warps, every sub-partition full
-    double best = 0.0;
-    for (int rep = 0; rep < 5; ++rep) {  // the first repetition warms up; best of the rest
-        SOAP_CUDA(s, cudaEventRecord(e0, st));
-        if (packed) fp32_probe_kernel<true><<<grid, kProbeThreads, 0, st>>>(iters, 1.0000001f, sink);
-        else fp32_probe_kernel<false><<<grid, kProbeThreads, 0, st>>>(iters, 1.0000001f, sink);
-        SOAP_CUDA(s, cudaEventRecord(e1, st));
-        SOAP_CUDA(s, cudaEventSynchronize(e1));
-        float ms = 0.f;
-        SOAP_CUDA(s, cudaEventElapsedTime(&ms, e0, e1));
-        const double fma = (double)grid * kProbeThreads * (double)iters * 8.0 * kProbeChains;
-        if (rep > 0 && ms > 0.f) best = std::max(best, fma / (ms * 1e-3));
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    SOAP_LAUNCH_CHECK(s, "fp32_probe_kernel");
-    *fma_per_s = best;
     return SOAP_OK;
 }
 
