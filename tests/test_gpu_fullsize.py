@@ -127,10 +127,45 @@ def test_config4_every_pixel_every_line(soap):
     _assert_every_pixel_and_line(wl, ref, Q, D, na)
 
 
-def test_config5_batch_eight_stars_16k_pixel_windows(soap):
+def test_config3_nested_spot_in_facula_every_pixel_every_line(soap):
+    """The spot-inside-a-facula variant of C3 (list order decides, the spot listed after the facula overrides it)."""
+    wl = workloads.make_config3(nested=True)
+    ref = _oracle_all(wl)
+    Q, D, na, _ = _run(soap, wl, None)
+    assert int(na.sum()) == 14694 and na.max() == 1825
+    _assert_every_pixel_and_line(wl, ref, Q, D, na)
+
+
+def test_config3_three_effects_in_one_pass_every_pixel(soap, c3):
+    """Total, flux-only and CB-only delta spectra (Eq. 1-3) from the one-pass launch on C3 as configured (the facula has a
+    limb-brightening law, so its entries are walked with both weights): every pixel of every phase of the three outputs against
+    the oracle's three effects, each held to 1e-4 of its own max|delta| and never looser than 1e-4 of the total's."""
+    from test_gpu_parity import _run_effects
+    wl, ref = c3
+    outs, na = _run_effects(soap, wl)
+    assert np.array_equal(na, ref["n_active"])
+    scale = float(np.max(np.abs(ref["D"])))
+    for effect, D in enumerate(outs):
+        assert not np.isnan(D).any()
+        if effect == 0:
+            Do = ref["D"]
+        else:
+            Do, nao = oracle.active(wl, wl.quiet, wl.spot, wl.facula, wl.lambda0, wl.dlambda, wl.regions, wl.phases,
+                                    wl.spot_contrast, wl.facula_contrast, wl.spot_lb, wl.facula_lb, 0, None, effect)
+            assert np.array_equal(nao, ref["n_active"])
+        own = float(np.max(np.abs(Do)))
+        assert own > 0
+        err = float(np.max(np.abs(D.astype(np.float64) - Do)))
+        assert err <= DELTA_TOL * min(own, scale), f"effect {effect}: {err / min(own, scale):.3e} of max|delta|"
+        for p_ in np.nonzero(ref["n_active"] == 0)[0]:
+            assert np.all(D[p_] == 0.0)
+
+
+def test_config5_batch_all_stars_16k_pixel_windows(soap):
     """64 stars through the batch entry points; the slowest and fastest rotator, the most pole-on and most equator-on star,
     the stars with the most and the fewest regions and the first and last star are compared with the oracle on three
-    16 384-pixel windows each: both ends of the spectrum (clamped halo) and a stretch across tile boundaries."""
+    16 384-pixel windows each: both ends of the spectrum (clamped halo) and a stretch across tile boundaries; every other
+    star on one window whose position moves along the spectrum with the star's index."""
     dev = torch.device("cuda:0")
     n_stars, n_pix, n_ph = 64, 200_000, 50
     shared = workloads.make_config5_star(0, n_pix=n_pix, n_phases=n_ph)
@@ -156,11 +191,12 @@ def test_config5_batch_eight_stars_16k_pixel_windows(soap):
     if len(picks) < 8:
         picks = sorted(set(picks) | set(range(1, 64, 9)))[:max(8, len(picks))]
     W = 16384
-    for k in picks:
+    for k in range(n_stars):
         wl = wls[k]
         Qk, Dk = Q[k].cpu().numpy(), D[k].cpu().numpy()
         sw = oracle.geometry(wl)["sum_w"]
-        for lo in (0, 96_000, n_pix - W):
+        windows = (0, 96_000, n_pix - W) if k in picks else ((k * 2897) % ((n_pix - W) // 64) * 64,)
+        for lo in windows:
             hi = lo + W
             Qo, Do, _ = oracle.run_workload(wl, lo, hi)
             assert check_quiet(Qk[lo:hi], Qo, sw) <= QUIET_TOL, f"star {k} window {lo}"
