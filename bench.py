@@ -724,6 +724,89 @@ def run_configs(args):
     print(json.dumps(r))
 
 
+def run_sweep(args):
+    """--workload C5 --sweep [--gpus N]: the 64-star parameter sweep as ONE job dealt to the ranks (stars first).
+
+    Rank r owns the contiguous block sharding.shard_range(64, r, N) and runs the three batch calls on it; nothing crosses
+    NVLink while it computes.  Total work is fixed, so `scaling` is "strong"; value = 64 x 51 spectra / max-over-ranks
+    device time.  Afterwards every star's checksum row (sum of Q, sum of |delta|) is gathered in star order
+    (sharding.gather_unit_summaries).  The delta checksums do not depend on how the job was dealt (an item's result does not
+    depend on which CTA, launch or rank computes it): `delta_checksums_sha16` must be the same for every N.  The quiet
+    spectra agree to an fp32 rounding only (the batch launch groups its fp64 shares by CTA range), so their checksum is
+    printed as a number, `quiet_checksum_sum`."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_2301_04259_b200 as soap
+    import workloads
+    from paper_2301_04259_b200 import sharding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    n_stars = 64
+    b, e = sharding.shard_range(n_stars, rank, world)
+    shared = workloads.make_config5_star(0)  # the spectra set is shared by all stars: every rank holds it
+    wls = [shared if k == 0 else workloads.make_config5_star(k, shared=shared) for k in range(b, e)]
+    n, P, n_ph = len(wls), shared.n_pix, len(shared.phases)
+    q = soap.to_device_spectra(shared.quiet, shared.lambda0, shared.dlambda, dev)
+    sp = soap.to_device_spectra(shared.spot, shared.lambda0, shared.dlambda, dev, shared.spot_contrast, shared.spot_lb)
+    fa = soap.to_device_spectra(shared.facula, shared.lambda0, shared.dlambda, dev, shared.facula_contrast, shared.facula_lb)
+    stars = [soap.soap_create(local_rank) for _ in wls]
+    Q = torch.zeros((max(n, 1), P), dtype=torch.float32, device=dev)
+    D = torch.zeros((max(n, 1), n_ph, P), dtype=torch.float32, device=dev)
+    flush_buf = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    timer = Timer(torch, flush_buf)
+
+    def step():
+        if n == 0:
+            return
+        if n == 1:
+            soap.soap_disk_geometry(stars[0], wls[0], want_info=False)
+            soap.soap_integrate_quiet(stars[0], q, Q[0])
+            soap.soap_active_timeseries(stars[0], q, sp, fa, wls[0].regions, wls[0].phases, D[0])
+            return
+        soap.soap_batch_disk_geometry(stars, wls)
+        soap.soap_batch_integrate_quiet(stars, [q] * n, [Q[k] for k in range(n)])
+        soap.soap_batch_active_timeseries(stars, [q] * n, [sp] * n, [fa] * n, [w.regions for w in wls],
+                                          [w.phases for w in wls], [D[k] for k in range(n)])
+
+    steps = max(3, min(args.steps, 10))
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ms = timer.steps(step, steps, warm=max(3, args.warmup))
+    if world > 1:
+        dist.barrier()
+    total_ms = sharding.max_over_ranks(float(sum(ms)), dev)
+    local = torch.stack([Q[:n].double().sum(dim=1), D[:n].double().abs().sum(dim=(1, 2))], dim=1) if n else torch.zeros((0, 2), dtype=torch.float64, device=dev)
+    rows = sharding.gather_unit_summaries(local, n_stars)
+    if rank == 0:
+        ms_per_step = total_ms / steps
+        rows_h = rows.cpu().numpy()
+        digest = hashlib.sha256(np.ascontiguousarray(rows_h[:, 1]).tobytes()).hexdigest()[:16]
+        print(json.dumps({
+            "metric": METRIC, "value": n_stars * (1 + n_ph) / (ms_per_step * 1e-3), "unit": "spectra/s", "n_gpus": world,
+            "steps": steps, "warmup": max(3, args.warmup), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workloads.CONFIG_NAMES[5], "stars": n_stars, "stars_on_rank0": n,
+                       "sharding": "contiguous blocks of stars per rank (sharding.shard_range), no data-path collective",
+                       "l2": "512 MB buffer written before every timed step"},
+            "delta_checksums_sha16": digest, "quiet_checksum_sum": float(rows_h[:, 0].sum()), "stars_gathered": int(rows.shape[0]),
+            "checksum_star0": [float(rows_h[0, 0]), float(rows_h[0, 1])]}))
+    for s_ in stars:
+        soap.soap_destroy(s_)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -736,9 +819,13 @@ def main():
     ap.add_argument("--vsini", type=float, default=None, help="with --workload: override v sin i (km/s)")
     ap.add_argument("--workload", choices=["C2", "C3", "C4", "C5"], default=None,
                     help="print one per-config timing line instead of the bench contract (which is C3)")
+    ap.add_argument("--sweep", action="store_true",
+                    help="with --workload C5: the 64 stars as one job dealt to the --gpus ranks (strong scaling), one JSON line")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "C5" and args.sweep:
+        run_sweep(args)
     elif args.workload is not None:
         run_configs(args)
     else:
